@@ -1,0 +1,849 @@
+/*
+ * hq_oracle.c — the ORACLE for HyperQuant's inference hot path (arxiv/paper_2606_23406).
+ *
+ * TEST INFRASTRUCTURE ONLY.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * --impl reference legs may build, load or call this file.  The product (paper_2606_23406_b200/)
+ * never does and shares no code, header, table or generator with it.
+ *
+ * Plain, slow, obviously-correct C: scalar loops in the paper's order and notation, following
+ * docs/FORMAT.md for everything the paper leaves open (readings G1..G18 in DESIGN.md).  Citations
+ * are PAPER.md line numbers.  Encode-side floating point is IEEE binary32 without FMA contraction
+ * (build: gcc -O2 -ffp-contract=off, no -ffast-math) because it decides integers; reconstruction /
+ * attention / dense-RHT checks are in double.
+ *
+ * Parity pins (tests/test_oracle_*.py): Philox known-answer vectors; H·Hᵀ = n·I and the dense
+ * double RHT; brute-force nearest point; Voronoi second moments vs Table 2 (L139-142); strip
+ * bijection and Table 3 savings (L284); Rice round trip; printed rates at 21 dB (L289); Table 14
+ * α (L887-890); Table 11 A2 SNRs (L550-552); dither moments and unbiasedness (L786-808).
+ * Parity unpinned: none.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#define HQO_Z 1
+#define HQO_A2 2
+#define HQO_D4 4
+#define HQO_E8 8
+
+/* ------------------------------------------------------------------------------------------ */
+/* Counter RNG: Philox4x32-10 (docs/FORMAT.md §1).                                              */
+/* ------------------------------------------------------------------------------------------ */
+void hqo_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
+    uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3], k0 = key[0], k1 = key[1];
+    for (int round = 0; round < 10; ++round) {
+        uint64_t p0 = (uint64_t)0xD2511F53u * c0;
+        uint64_t p1 = (uint64_t)0xCD9E8D57u * c2;
+        uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0;
+        uint32_t n1 = (uint32_t)p1;
+        uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+        uint32_t n3 = (uint32_t)p0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+/* sign d_i in {+1,-1}: stream 1 = RHT D (eq.(1)), stream 2 = KV rotation S (L216). */
+void hqo_signs(uint64_t seed, uint32_t stream, int64_t n, int8_t* out) {
+    uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
+    for (int64_t i = 0; i < n; ++i) {
+        uint32_t ctr[4] = {(uint32_t)(i >> 7), 0u, 0u, stream}, o[4];
+        hqo_philox4x32_10(ctr, key, o);
+        out[i] = ((o[(i >> 5) & 3] >> (i & 31)) & 1u) ? -1 : 1;
+    }
+}
+
+/* dither uniform e of (token, head, role): odd 24-bit integer w = 2r+1 (FORMAT §1). */
+static uint32_t dither_w(uint64_t seed, uint32_t e, uint32_t token, uint32_t head, uint32_t role) {
+    uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
+    uint32_t ctr[4] = {e >> 2, token, head | (role << 16), 3u}, o[4];
+    hqo_philox4x32_10(ctr, key, o);
+    return 2u * (o[e & 3] >> 9) + 1u;
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* fp16 (storage of the norm, L500), bf16 helpers.                                             */
+/* ------------------------------------------------------------------------------------------ */
+static uint16_t f32_to_f16_bits(float f) { /* RNE, saturating at 65504 (FORMAT R3) */
+    if (!(f == f)) return 0x7e00;
+    float a = fabsf(f);
+    uint16_t sign = signbit(f) ? 0x8000 : 0;
+    if (a >= 65520.0f) return sign | 0x7bff; /* would round to inf: saturate */
+    if (a < 5.9604644775390625e-8f * 0.5f) return sign;
+    int e;
+    float m = frexpf(a, &e); /* a = m * 2^e, m in [0.5,1) */
+    int E = e - 1;            /* a = (2m) * 2^E, 2m in [1,2) */
+    if (E < -14) {            /* subnormal: units of 2^-24 */
+        float q = rintf(ldexpf(a, 24));
+        return sign | (uint16_t)q; /* q may be 1024 = smallest normal: bit pattern still right */
+    }
+    float q = rintf(ldexpf(m, 11)); /* mantissa in [1024, 2048] */
+    if (q == 2048.0f) { q = 1024.0f; E += 1; }
+    return sign | (uint16_t)(((E + 15) << 10) + ((int)q - 1024));
+}
+static float f16_bits_to_f32(uint16_t h) {
+    int s = h >> 15, e = (h >> 10) & 31, m = h & 1023;
+    float v;
+    if (e == 0) v = ldexpf((float)m, -24);
+    else if (e == 31) v = m ? NAN : INFINITY;
+    else v = ldexpf((float)(m + 1024), e - 25);
+    return s ? -v : v;
+}
+uint16_t hqo_f32_to_f16_bits(float f) { return f32_to_f16_bits(f); }
+float hqo_f16_bits_to_f32(uint16_t h) { return f16_bits_to_f32(h); }
+
+/* ------------------------------------------------------------------------------------------ */
+/* RHT (§3.1 eq.(1), §4.1; FORMAT R1).                                               */
+/* ------------------------------------------------------------------------------------------ */
+void hqo_fwht_f32(float* v, int n) { /* unnormalized Sylvester butterfly, ascending stride */
+    for (int h = 1; h < n; h <<= 1)
+        for (int i = 0; i < n; ++i)
+            if ((i & h) == 0) {
+                float a = v[i], b = v[i + h];
+                v[i] = a + b;
+                v[i + h] = a - b;
+            }
+}
+void hqo_rht_f32(const float* x, const int8_t* d, int n, float* u) {
+    float cn = (float)(1.0 / sqrt((double)n));
+    for (int i = 0; i < n; ++i) u[i] = (d[i] < 0) ? -x[i] : x[i];
+    hqo_fwht_f32(u, n);
+    for (int i = 0; i < n; ++i) u[i] = u[i] * cn;
+}
+/* the definition, dense and in double: u = (1/sqrt n) H D x, H[i][j] = (-1)^popcount(i&j). */
+void hqo_rht_dense_f64(const double* x, const int8_t* d, int n, double* u) {
+    for (int i = 0; i < n; ++i) {
+        double s = 0.0;
+        for (int j = 0; j < n; ++j) {
+            int par = __builtin_popcount((unsigned)(i & j)) & 1;
+            double t = (double)d[j] * x[j];
+            s += par ? -t : t;
+        }
+        u[i] = s / sqrt((double)n);
+    }
+}
+/* inverse of the orthonormal RHT in double: x = D H u / sqrt n. */
+static void rht_inverse_f64(const double* u, const int8_t* d, int n, double* x) {
+    for (int j = 0; j < n; ++j) {
+        double s = 0.0;
+        for (int i = 0; i < n; ++i) {
+            int par = __builtin_popcount((unsigned)(i & j)) & 1;
+            s += par ? -u[i] : u[i];
+        }
+        x[j] = (double)d[j] * s / sqrt((double)n);
+    }
+}
+
+static float treesum_f32(float* a, int m) { /* FORMAT R2, destroys a */
+    for (int h = 1; h < m; h <<= 1)
+        for (int i = 0; i + h < m; i += 2 * h) a[i] = a[i] + a[i + h];
+    return a[0];
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* Scale α (eq.(9)) and lattice constants (Table 2, covolumes from L241).          */
+/* ------------------------------------------------------------------------------------------ */
+int hqo_dim(int lattice) { return lattice; }
+double hqo_second_moment(int lattice) { /* M = G(Λ) · V^{2/N} of the integer realization */
+    switch (lattice) {
+        case HQO_Z: return 1.0 / 12.0;
+        case HQO_A2: return 0.0802 * 2.0 * sqrt(3.0); /* V = 2·sqrt3, N = 2 */
+        case HQO_D4: return 0.0766 * sqrt(2.0);       /* V = 2, N = 4 */
+        case HQO_E8: return 0.0717 * 4.0;             /* V = 2^8, N = 8 */
+    }
+    return 0.0;
+}
+double hqo_alpha(int lattice, double snr_db) {
+    return sqrt(pow(10.0, snr_db / 10.0) * hqo_second_moment(lattice));
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* Nearest lattice point (§3.2, §4.5; FORMAT R5, R6).                                 */
+/* ------------------------------------------------------------------------------------------ */
+static const float S3 = 1.7320508075688772f; /* (float)sqrt(3.0) */
+
+static void nearest_Dm(const float* z, int m, int32_t* f) { /* Conway–Sloane D_m */
+    float delta[8];
+    int sum = 0;
+    for (int i = 0; i < m; ++i) {
+        float r = rintf(z[i]);
+        f[i] = (int32_t)r;
+        delta[i] = z[i] - r;
+        sum += f[i];
+    }
+    if (sum & 1) {
+        int j = 0;
+        for (int i = 1; i < m; ++i)
+            if (fabsf(delta[i]) > fabsf(delta[j])) j = i;
+        f[j] += (delta[j] < 0.0f) ? -1 : 1;
+    }
+}
+
+/* Q_Λ(y) without the INT8 pre-clamp. For A2 the block is (y, x) and c = (n_y, n_x). */
+static void nearest_noclamp(int lattice, const float* y, int32_t* c) {
+    if (lattice == HQO_Z) {
+        c[0] = (int32_t)rintf(y[0]);
+    } else if (lattice == HQO_D4) {
+        nearest_Dm(y, 4, c);
+    } else if (lattice == HQO_E8) {
+        float za[8], zb[8], da[8], db[8];
+        int32_t a[8], b[8];
+        for (int i = 0; i < 8; ++i) { za[i] = y[i] * 0.5f; zb[i] = (y[i] - 1.0f) * 0.5f; }
+        nearest_Dm(za, 8, a);
+        nearest_Dm(zb, 8, b);
+        for (int i = 0; i < 8; ++i) {
+            a[i] = 2 * a[i];
+            b[i] = 2 * b[i] + 1;
+            float ea = y[i] - (float)a[i], eb = y[i] - (float)b[i];
+            da[i] = ea * ea;
+            db[i] = eb * eb;
+        }
+        float dist_a = treesum_f32(da, 8), dist_b = treesum_f32(db, 8);
+        memcpy(c, (dist_a <= dist_b) ? a : b, 8 * sizeof(int32_t));
+    } else { /* A2 */
+        float two_s3 = 2.0f * S3;
+        int32_t ay = 2 * (int32_t)rintf(y[0] / two_s3), ax = 2 * (int32_t)rintf(y[1] * 0.5f);
+        int32_t by = 2 * (int32_t)rintf((y[0] - S3) / two_s3) + 1;
+        int32_t bx = 2 * (int32_t)rintf((y[1] - 1.0f) * 0.5f) + 1;
+        float eay = y[0] - S3 * (float)ay, eax = y[1] - (float)ax;
+        float eby = y[0] - S3 * (float)by, ebx = y[1] - (float)bx;
+        float dist_a = eay * eay + eax * eax, dist_b = eby * eby + ebx * ebx;
+        if (dist_a <= dist_b) { c[0] = ay; c[1] = ax; } else { c[0] = by; c[1] = bx; }
+    }
+}
+
+/* with the INT8 pre-clamp of the quantizer input (G8 / FORMAT R5); returns #coordinates clamped */
+static int clamp_block(int lattice, const float* y, float* z) {
+    int n = lattice, cnt = 0;
+    for (int i = 0; i < n; ++i) {
+        float lim = (lattice == HQO_E8) ? 125.0f : (lattice == HQO_Z) ? 127.0f : 126.0f;
+        if (lattice == HQO_A2 && i == 0) lim = 126.0f * S3;
+        float v = y[i];
+        if (v > lim) { v = lim; cnt++; }
+        if (v < -lim) { v = -lim; cnt++; }
+        z[i] = v;
+    }
+    return cnt;
+}
+int hqo_nearest(int lattice, const float* y, int32_t* c) {
+    float z[8];
+    int cnt = clamp_block(lattice, y, z);
+    nearest_noclamp(lattice, z, c);
+    return cnt;
+}
+void hqo_nearest_noclamp(int lattice, const float* y, int32_t* c) { nearest_noclamp(lattice, y, c); }
+
+/* dither U = π_Λ(box-uniform) for block `blk` of a vector (A.6 L843-847; FORMAT R4). */
+static void dither_block(int lattice, uint64_t seed, uint32_t blk, uint32_t token, uint32_t head,
+                         uint32_t role, float* U) {
+    int dim = lattice;
+    float y[8];
+    int32_t c[8];
+    for (int j = 0; j < dim; ++j) {
+        float w = (float)dither_w(seed, (uint32_t)dim * blk + (uint32_t)j, token, head, role);
+        if (lattice == HQO_E8) y[j] = w * 0x1p-22f - 2.0f;
+        else if (lattice == HQO_D4) y[j] = w * 0x1p-23f - 1.0f;
+        else if (lattice == HQO_Z) y[j] = w * 0x1p-24f - 0.5f;
+        else y[j] = (j == 0) ? (w * 0x1p-23f - 1.0f) * S3 : (w * 0x1p-23f - 1.0f);
+    }
+    nearest_noclamp(lattice, y, c);
+    for (int j = 0; j < dim; ++j) {
+        float p = (float)c[j];
+        if (lattice == HQO_A2 && j == 0) p = S3 * p;
+        U[j] = y[j] - p;
+    }
+}
+void hqo_dither_block(int lattice, uint64_t seed, uint32_t blk, uint32_t token, uint32_t head,
+                      uint32_t role, float* U) {
+    dither_block(lattice, seed, blk, token, head, role, U);
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* Strip / un-strip with zig-zag (§4.6; FORMAT §3).                                    */
+/* ------------------------------------------------------------------------------------------ */
+static int32_t zigzag(int32_t v) { return v >= 0 ? 2 * v : -2 * v - 1; }
+static int32_t unzigzag(int32_t z) { return (z & 1) ? -((z + 1) >> 1) : (z >> 1); }
+static int32_t half_exact(int32_t v) { return v >> 1; } /* callers guarantee v even */
+
+void hqo_strip(int lattice, const int32_t* c, int32_t* z) {
+    if (lattice == HQO_E8) {
+        int32_t coset = c[0] & 1, s[8], sum = 0;
+        for (int i = 0; i < 8; ++i) s[i] = half_exact(c[i] - coset);
+        for (int i = 0; i < 7; ++i) sum += s[i];
+        int32_t p = sum & 1, t = half_exact(s[7] - p);
+        for (int i = 0; i < 7; ++i) z[i] = zigzag(s[i]);
+        z[7] = 2 * zigzag(t) + coset; /* comb, L274 */
+    } else if (lattice == HQO_D4) {
+        int32_t p = (c[0] + c[1] + c[2]) & 1, t = half_exact(c[3] - p);
+        z[0] = zigzag(c[0]); z[1] = zigzag(c[1]); z[2] = zigzag(c[2]); z[3] = zigzag(t);
+    } else if (lattice == HQO_A2) {
+        int32_t p = c[1] & 1, ty = half_exact(c[0] - p);
+        z[0] = zigzag(ty); z[1] = zigzag(c[1]);
+    } else {
+        z[0] = zigzag(c[0]);
+    }
+}
+void hqo_unstrip(int lattice, const int32_t* z, int32_t* c) {
+    if (lattice == HQO_E8) {
+        int32_t s[8], sum = 0, coset = z[7] & 1, t = unzigzag(z[7] >> 1);
+        for (int i = 0; i < 7; ++i) { s[i] = unzigzag(z[i]); sum += s[i]; }
+        s[7] = 2 * t + (sum & 1);
+        for (int i = 0; i < 8; ++i) c[i] = 2 * s[i] + coset;
+    } else if (lattice == HQO_D4) {
+        c[0] = unzigzag(z[0]); c[1] = unzigzag(z[1]); c[2] = unzigzag(z[2]);
+        c[3] = 2 * unzigzag(z[3]) + ((c[0] + c[1] + c[2]) & 1);
+    } else if (lattice == HQO_A2) {
+        c[1] = unzigzag(z[1]);
+        c[0] = 2 * unzigzag(z[0]) + (c[1] & 1);
+    } else {
+        c[0] = unzigzag(z[0]);
+    }
+}
+static int sym_class(int lattice, int j) {
+    if (lattice == HQO_D4) return (j & 3) == 3;
+    if (lattice == HQO_A2) return j & 1;
+    return 0;
+}
+/* symbols of a whole tile of n codes (block-major) */
+static void tile_symbols(int lattice, const int8_t* codes, int n, int32_t* z) {
+    int dim = lattice;
+    for (int b = 0; b < n / dim; ++b) {
+        int32_t c[8];
+        for (int i = 0; i < dim; ++i) c[i] = codes[b * dim + i];
+        hqo_strip(lattice, c, z + b * dim);
+    }
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* Rice coding of a tile into the split-plane tile stream (§3.3, §4.7; FORMAT §3-4).   */
+/* ------------------------------------------------------------------------------------------ */
+static void put_bit(uint32_t* words, uint64_t p, uint32_t bit) { /* MSB-first */
+    if (bit) words[p >> 5] |= 1u << (31 - (p & 31));
+}
+static uint32_t get_bit(const uint32_t* words, uint64_t p) {
+    return (words[p >> 5] >> (31 - (p & 31))) & 1u;
+}
+static void put_word(uint32_t* words, uint64_t p, uint32_t v, int nbits) { /* v's bit nbits-1 first */
+    for (int i = 0; i < nbits; ++i) put_bit(words, p + i, (v >> (nbits - 1 - i)) & 1u);
+}
+
+/* bit length of a tile: Σ (k_j + 1 + q_j) */
+int64_t hqo_tile_bits(int lattice, const int8_t* codes, int n, const int* k) {
+    int32_t z[1024];
+    tile_symbols(lattice, codes, n, z);
+    int64_t L = 0;
+    for (int j = 0; j < n; ++j) {
+        int kk = k[sym_class(lattice, j)];
+        L += kk + 1 + (z[j] >> kk);
+    }
+    return L;
+}
+
+/* write one tile stream at bit position pos; returns its length */
+static int64_t write_tile(int lattice, const int8_t* codes, int n, const int* k, uint32_t* words,
+                          uint64_t pos) {
+    int32_t z[1024];
+    uint64_t p = pos;
+    tile_symbols(lattice, codes, n, z);
+    int nclass = (lattice == HQO_D4 || lattice == HQO_A2) ? 2 : 1;
+    for (int a = 0; a < nclass; ++a) { /* R-section */
+        int32_t r[1024];
+        int na = 0, ka = k[a];
+        for (int j = 0; j < n; ++j)
+            if (sym_class(lattice, j) == a) r[na++] = z[j] & ((1 << ka) - 1);
+        for (int ch = 0; ch * 32 < na; ++ch) {
+            int w = na - ch * 32 < 32 ? na - ch * 32 : 32;
+            for (int b = 0; b < ka; ++b) {
+                if (w == 32) {
+                    uint32_t V = 0;
+                    for (int u = 0; u < 32; ++u)
+                        V |= (uint32_t)((r[ch * 32 + u] >> b) & 1) << (8 * (u & 3) + (u >> 2));
+                    put_word(words, p, V, 32);
+                } else {
+                    for (int u = 0; u < w; ++u) put_bit(words, p + u, (r[ch * 32 + u] >> b) & 1);
+                }
+                p += w;
+            }
+        }
+    }
+    for (int j = 0; j < n; ++j) { /* U-section: q zeros then a one */
+        int q = z[j] >> k[sym_class(lattice, j)];
+        p += q;
+        put_bit(words, p, 1u);
+        p += 1;
+    }
+    return (int64_t)(p - pos);
+}
+
+/* read one tile stream of n symbols at bit position pos -> codes; returns bits consumed */
+static int64_t read_tile(int lattice, int n, const int* k, const uint32_t* words, uint64_t pos,
+                         int8_t* codes) {
+    int32_t z[1024], rem[1024];
+    uint64_t p = pos;
+    int nclass = (lattice == HQO_D4 || lattice == HQO_A2) ? 2 : 1;
+    for (int a = 0; a < nclass; ++a) {
+        int idx[1024], na = 0, ka = k[a];
+        for (int j = 0; j < n; ++j)
+            if (sym_class(lattice, j) == a) { idx[na++] = j; rem[j] = 0; }
+        for (int ch = 0; ch * 32 < na; ++ch) {
+            int w = na - ch * 32 < 32 ? na - ch * 32 : 32;
+            for (int b = 0; b < ka; ++b) {
+                for (int u = 0; u < w; ++u) {
+                    int bitpos = (w == 32) ? 31 - (8 * (u & 3) + (u >> 2)) : u;
+                    rem[idx[ch * 32 + u]] |= (int32_t)get_bit(words, p + bitpos) << b;
+                }
+                p += w;
+            }
+        }
+    }
+    for (int j = 0; j < n; ++j) {
+        int q = 0;
+        while (!get_bit(words, p)) { ++q; ++p; }
+        ++p;
+        z[j] = (q << k[sym_class(lattice, j)]) | rem[j];
+    }
+    int dim = lattice;
+    for (int b = 0; b < n / dim; ++b) {
+        int32_t c[8];
+        hqo_unstrip(lattice, z + b * dim, c);
+        for (int i = 0; i < dim; ++i) codes[b * dim + i] = (int8_t)c[i];
+    }
+    return (int64_t)(p - pos);
+}
+
+/* single-tile entry points for the round-trip pins */
+int64_t hqo_write_tile(int lattice, const int8_t* codes, int n, const int* k, uint32_t* words,
+                       uint64_t pos) {
+    return write_tile(lattice, codes, n, k, words, pos);
+}
+int64_t hqo_read_tile(int lattice, int n, const int* k, const uint32_t* words, uint64_t pos,
+                      int8_t* codes) {
+    return read_tile(lattice, n, k, words, pos, codes);
+}
+
+/* The textbook Rice code of the same symbols (q zeros, a one, k bits MSB-first), interleaved per
+ * symbol: used only to pin that the split-plane stream has exactly the Rice code's length. */
+int64_t hqo_rice_reference_bits(int lattice, const int8_t* codes, int n, const int* k,
+                                uint32_t* words) {
+    int32_t z[1024];
+    uint64_t p = 0;
+    tile_symbols(lattice, codes, n, z);
+    for (int j = 0; j < n; ++j) {
+        int kk = k[sym_class(lattice, j)], q = z[j] >> kk;
+        p += q;
+        put_bit(words, p++, 1u);
+        put_word(words, p, (uint32_t)(z[j] & ((1 << kk) - 1)), kk);
+        p += kk;
+    }
+    return (int64_t)p;
+}
+
+/* marginal symbol histograms of a code array (for the B.4 scalar_entropy pin, L908) */
+void hqo_symbol_histogram(int lattice, const int8_t* codes, int64_t ntiles, int n, int64_t* hist
+                          /* [dim][512] */) {
+    int dim = lattice;
+    int32_t z[1024];
+    for (int64_t t = 0; t < ntiles; ++t) {
+        tile_symbols(lattice, codes + t * n, n, z);
+        for (int j = 0; j < n; ++j) hist[(j % dim) * 512 + z[j]]++;
+    }
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* O1 steps 1-5: quantize rows of a matrix tile by tile (weights: no rotation, no dither).       */
+/* W [m, n_in] fp32 (bf16 inputs are passed already widened, exactly).                           */
+/* ------------------------------------------------------------------------------------------ */
+static int64_t quantize_tile(int lattice, int n, float A, const float* u, int with_dither,
+                             uint64_t seed, uint32_t token, uint32_t head, uint32_t role,
+                             int8_t* codes, uint16_t* norm_bits) {
+    float sq[1024];
+    int64_t clamps = 0;
+    for (int i = 0; i < n; ++i) sq[i] = u[i] * u[i];
+    float rho32 = sqrtf(treesum_f32(sq, n));
+    uint16_t hb = f32_to_f16_bits(rho32);
+    float rho = f16_bits_to_f32(hb);
+    *norm_bits = hb;
+    if (rho == 0.0f) { /* G18 */
+        memset(codes, 0, (size_t)n);
+        return 0;
+    }
+    float g = A / rho;
+    int dim = lattice;
+    for (int b = 0; b < n / dim; ++b) {
+        float y[8], U[8];
+        int32_t c[8];
+        for (int i = 0; i < dim; ++i) y[i] = u[b * dim + i] * g;
+        if (with_dither) {
+            dither_block(lattice, seed, (uint32_t)b, token, head, role, U);
+            for (int i = 0; i < dim; ++i) y[i] = y[i] + U[i];
+        }
+        clamps += hqo_nearest(lattice, y, c);
+        for (int i = 0; i < dim; ++i) codes[b * dim + i] = (int8_t)c[i];
+    }
+    return clamps;
+}
+
+int64_t hqo_quantize_weights(const float* W, int64_t m, int64_t n_in, int64_t ld, int lattice,
+                             int n, double snr_db, uint64_t seed, int8_t* codes /*[m,n_in]*/,
+                             uint16_t* norms /*[m,n_in/n]*/) {
+    int64_t n_kt = n_in / n, clamps = 0;
+    float A = (float)(hqo_alpha(lattice, snr_db) * sqrt((double)n));
+    int8_t* d = (int8_t*)malloc((size_t)n_in);
+    hqo_signs(seed, 1u, n_in, d);
+#pragma omp parallel for reduction(+ : clamps) schedule(static)
+    for (int64_t r = 0; r < m; ++r) {
+        float u[1024];
+        for (int64_t kt = 0; kt < n_kt; ++kt) {
+            hqo_rht_f32(W + r * ld + kt * n, d + kt * n, n, u);
+            clamps += quantize_tile(lattice, n, A, u, 0, 0, 0, 0, 0, codes + r * n_in + kt * n,
+                                    norms + r * n_kt + kt);
+        }
+    }
+    free(d);
+    return clamps;
+}
+
+/* total bits of a code array for given k (also used by auto-k, FORMAT §3) */
+int64_t hqo_total_bits(const int8_t* codes, int64_t ntiles, int lattice, int n, const int* k) {
+    int64_t total = 0;
+#pragma omp parallel for reduction(+ : total) schedule(static)
+    for (int64_t t = 0; t < ntiles; ++t) total += hqo_tile_bits(lattice, codes + t * n, n, k);
+    return total;
+}
+void hqo_choose_k(const int8_t* codes, int64_t ntiles, int lattice, int n, int* k_out) {
+    /* per-class totals for k = 0..7 */
+    int64_t tot[2][8];
+    memset(tot, 0, sizeof tot);
+    for (int64_t t = 0; t < ntiles; ++t) {
+        int32_t z[1024];
+        tile_symbols(lattice, codes + t * n, n, z);
+        for (int j = 0; j < n; ++j)
+            for (int kk = 0; kk < 8; ++kk) tot[sym_class(lattice, j)][kk] += kk + 1 + (z[j] >> kk);
+    }
+    if (lattice == HQO_D4) { /* k_t = max(k_s - 1, 0), minimize the sum (L272, L295) */
+        int best = 0;
+        int64_t bv = -1;
+        for (int ks = 0; ks < 8; ++ks) {
+            int kt = ks > 0 ? ks - 1 : 0;
+            int64_t v = tot[0][ks] + tot[1][kt];
+            if (bv < 0 || v < bv) { bv = v; best = ks; }
+        }
+        k_out[0] = best;
+        k_out[1] = best > 0 ? best - 1 : 0;
+        return;
+    }
+    for (int a = 0; a < 2; ++a) {
+        int best = 0;
+        for (int kk = 1; kk < 8; ++kk)
+            if (tot[a][kk] < tot[a][best]) best = kk;
+        k_out[a] = best;
+    }
+    if (lattice != HQO_A2) k_out[1] = k_out[0];
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* Weight container (FORMAT §5): pack / unpack.                                                */
+/* ------------------------------------------------------------------------------------------ */
+/* returns blob size in bytes; if blob == NULL only sizes (group_off) are computed. */
+int64_t hqo_pack_weights(const int8_t* codes, const uint16_t* norms, int64_t m, int64_t n_in,
+                         int lattice, int n, const int* k, uint8_t* blob,
+                         uint32_t* group_off /*[G+1]*/) {
+    int64_t n_kt = n_in / n, n_rb = (m + 127) / 128, off16 = 0;
+    for (int64_t rb = 0; rb < n_rb; ++rb)
+        for (int64_t kt = 0; kt < n_kt; ++kt) {
+            int64_t g = rb * n_kt + kt, bits = 0;
+            group_off[g] = (uint32_t)off16;
+            uint16_t* len = blob ? (uint16_t*)(blob + 16 * off16) : NULL;
+            uint16_t* nrm = len ? len + 128 : NULL;
+            uint32_t* payload = blob ? (uint32_t*)(blob + 16 * off16 + 512) : NULL;
+            for (int i = 0; i < 128; ++i) {
+                int64_t r = rb * 128 + i;
+                int64_t L = (r < m) ? hqo_tile_bits(lattice, codes + r * n_in + kt * n, n, k) : 0;
+                if (blob) {
+                    len[i] = (uint16_t)L;
+                    nrm[i] = (r < m) ? norms[r * n_kt + kt] : 0;
+                }
+                bits += L;
+            }
+            int64_t pay16 = (bits + 127) / 128;
+            if (blob) {
+                memset(payload, 0, (size_t)pay16 * 16);
+                uint64_t p = 0;
+                for (int i = 0; i < 128; ++i) {
+                    int64_t r = rb * 128 + i;
+                    if (r < m) p += (uint64_t)write_tile(lattice, codes + r * n_in + kt * n, n, k, payload, p);
+                }
+            }
+            off16 += 32 + pay16;
+        }
+    group_off[n_rb * n_kt] = (uint32_t)off16;
+    return off16 * 16;
+}
+
+/* O2: decode the container back to codes and norms */
+void hqo_unpack_weights(const uint8_t* blob, const uint32_t* group_off, int64_t m, int64_t n_in,
+                        int lattice, int n, const int* k, int8_t* codes, uint16_t* norms) {
+    int64_t n_kt = n_in / n, n_rb = (m + 127) / 128;
+#pragma omp parallel for schedule(static)
+    for (int64_t g = 0; g < n_rb * n_kt; ++g) {
+        int64_t rb = g / n_kt, kt = g % n_kt;
+        const uint16_t* len = (const uint16_t*)(blob + 16 * (int64_t)group_off[g]);
+        const uint16_t* nrm = len + 128;
+        const uint32_t* payload = (const uint32_t*)(blob + 16 * (int64_t)group_off[g] + 512);
+        uint64_t p = 0;
+        for (int i = 0; i < 128; ++i) {
+            int64_t r = rb * 128 + i;
+            if (r >= m) break;
+            norms[r * n_kt + kt] = nrm[i];
+            read_tile(lattice, n, k, payload, p, codes + r * n_in + kt * n);
+            p += len[i];
+        }
+    }
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* O3: activations (FORMAT R7) and the INT8 contraction (§4.8).                            */
+/* ------------------------------------------------------------------------------------------ */
+void hqo_act_quant(const float* x, int64_t B, int64_t n_in, int64_t ldx, int lattice, int n,
+                   uint64_t seed, int8_t* q /*[B,n_in]*/, float* s_x /*[B,n_kt]*/,
+                   float* u_out /*[B,n_in] or NULL: the fp32 RHT output*/) {
+    int64_t n_kt = n_in / n;
+    int8_t* d = (int8_t*)malloc((size_t)n_in);
+    hqo_signs(seed, 1u, n_in, d);
+    for (int64_t b = 0; b < B; ++b)
+        for (int64_t kt = 0; kt < n_kt; ++kt) {
+            float u[1024], amax = 0.0f;
+            hqo_rht_f32(x + b * ldx + kt * n, d + kt * n, n, u);
+            if (u_out) memcpy(u_out + b * n_in + kt * n, u, (size_t)n * sizeof(float));
+            if (lattice == HQO_A2)
+                for (int i = 0; i < n; i += 2) u[i] = u[i] * S3;
+            for (int i = 0; i < n; ++i)
+                if (fabsf(u[i]) > amax) amax = fabsf(u[i]);
+            int8_t* qq = q + b * n_in + kt * n;
+            if (amax == 0.0f) {
+                memset(qq, 0, (size_t)n);
+                s_x[b * n_kt + kt] = 0.0f;
+                continue;
+            }
+            float inv = 127.0f / amax;
+            for (int i = 0; i < n; ++i) {
+                float v = rintf(u[i] * inv);
+                if (v > 127.0f) v = 127.0f;
+                if (v < -127.0f) v = -127.0f;
+                qq[i] = (int8_t)v;
+            }
+            s_x[b * n_kt + kt] = amax / 127.0f;
+        }
+    free(d);
+}
+
+/* acc[kt,b,r] = Σ_{i in tile} c[r,i]·q[b,i];  y[b,r] = Σ_kt (ρ[r,kt]/(α√n))·s_x[b,kt]·acc  (double) */
+void hqo_linear(const int8_t* codes, const uint16_t* norms, int64_t m, int64_t n_in, int lattice,
+                int n, double snr_db, const int8_t* q, const float* s_x, int64_t B,
+                int32_t* acc /*[n_kt,B,m] or NULL*/, double* y /*[B,m]*/) {
+    int64_t n_kt = n_in / n;
+    double inv_A = 1.0 / (hqo_alpha(lattice, snr_db) * sqrt((double)n));
+#pragma omp parallel for schedule(static)
+    for (int64_t r = 0; r < m; ++r)
+        for (int64_t b = 0; b < B; ++b) {
+            double yy = 0.0;
+            for (int64_t kt = 0; kt < n_kt; ++kt) {
+                int32_t a = 0;
+                for (int i = 0; i < n; ++i)
+                    a += (int32_t)codes[r * n_in + kt * n + i] * (int32_t)q[b * n_in + kt * n + i];
+                if (acc) acc[(kt * B + b) * m + r] = a;
+                yy += (double)f16_bits_to_f32(norms[r * n_kt + kt]) * inv_A *
+                      (double)s_x[b * n_kt + kt] * (double)a;
+            }
+            y[b * m + r] = yy;
+        }
+}
+
+/* sampled version for sizes where the full contraction is too slow on a CPU: outputs (b_s, r_s) */
+void hqo_linear_sampled(const int8_t* codes, const uint16_t* norms, int64_t m, int64_t n_in,
+                        int lattice, int n, double snr_db, const int8_t* q, const float* s_x,
+                        int64_t B, int64_t ns, const int64_t* bs, const int64_t* rs,
+                        int32_t* acc /*[ns,n_kt]*/, double* y /*[ns]*/) {
+    int64_t n_kt = n_in / n;
+    double inv_A = 1.0 / (hqo_alpha(lattice, snr_db) * sqrt((double)n));
+    (void)B; (void)m;
+    for (int64_t s = 0; s < ns; ++s) {
+        int64_t b = bs[s], r = rs[s];
+        double yy = 0.0;
+        for (int64_t kt = 0; kt < n_kt; ++kt) {
+            int32_t a = 0;
+            for (int i = 0; i < n; ++i)
+                a += (int32_t)codes[r * n_in + kt * n + i] * (int32_t)q[b * n_in + kt * n + i];
+            acc[s * n_kt + kt] = a;
+            yy += (double)f16_bits_to_f32(norms[r * n_kt + kt]) * inv_A *
+                  (double)s_x[b * n_kt + kt] * (double)a;
+        }
+        y[s] = yy;
+    }
+}
+
+/* Ŵ in the original (un-rotated) domain, double: Ŵ[r,tile] = RHT^{-1}( (ρ/(α√n))·c ).  Used for
+ * the MSE / realized-SNR pins (L874) and y_exact = Ŵx. */
+void hqo_dequant_weights(const int8_t* codes, const uint16_t* norms, int64_t m, int64_t n_in,
+                         int lattice, int n, double snr_db, uint64_t seed, double* What) {
+    int64_t n_kt = n_in / n;
+    double inv_A = 1.0 / (hqo_alpha(lattice, snr_db) * sqrt((double)n));
+    int8_t* d = (int8_t*)malloc((size_t)n_in);
+    hqo_signs(seed, 1u, n_in, d);
+#pragma omp parallel for schedule(static)
+    for (int64_t r = 0; r < m; ++r)
+        for (int64_t kt = 0; kt < n_kt; ++kt) {
+            double u[1024], x[1024];
+            double sc = (double)f16_bits_to_f32(norms[r * n_kt + kt]) * inv_A;
+            for (int i = 0; i < n; ++i) {
+                double p = (double)codes[r * n_in + kt * n + i];
+                if (lattice == HQO_A2 && (i & 1) == 0) p *= sqrt(3.0);
+                u[i] = sc * p;
+            }
+            rht_inverse_f64(u, d + kt * n, n, x);
+            for (int i = 0; i < n; ++i) What[r * n_in + kt * n + i] = x[i];
+        }
+    free(d);
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* KV path (§5.2): encode vectors [n_tok, heads, d] of one role.                        */
+/* rotation: 0 none, 1 signs.  token0 = index of the first token of this call.                   */
+/* ------------------------------------------------------------------------------------------ */
+int64_t hqo_kv_quantize(const float* kv, int64_t n_tok, int heads, int d, int64_t token0, int role,
+                        int lattice, double snr_db, int rotation, int dither, uint64_t seed,
+                        int8_t* codes /*[n_tok,heads,d]*/, uint16_t* norms /*[n_tok,heads]*/) {
+    float A = (float)(hqo_alpha(lattice, snr_db) * sqrt((double)d));
+    int8_t *D = (int8_t*)malloc((size_t)d), *S = (int8_t*)malloc((size_t)d);
+    int64_t clamps = 0;
+    hqo_signs(seed, 1u, d, D);
+    hqo_signs(seed, 2u, d, S);
+#pragma omp parallel for reduction(+ : clamps) schedule(static)
+    for (int64_t t = 0; t < n_tok; ++t)
+        for (int h = 0; h < heads; ++h) {
+            float u[1024];
+            hqo_rht_f32(kv + (t * heads + h) * d, D, d, u);
+            if (rotation == 1)
+                for (int i = 0; i < d; ++i) u[i] = (S[i] < 0) ? -u[i] : u[i];
+            clamps += quantize_tile(lattice, d, A, u, dither, seed, (uint32_t)(token0 + t),
+                                    (uint32_t)h, (uint32_t)role, codes + (t * heads + h) * d,
+                                    norms + t * heads + h);
+        }
+    free(D); free(S);
+    return clamps;
+}
+
+/* pack one (role, head) stream: vectors of tokens [0, n_tok) appended after bit position pos0.
+ * len[t] written; returns new bit position.  words must be zero-initialized beyond pos0. */
+int64_t hqo_kv_pack_head(const int8_t* codes /*[n_tok,heads,d]*/, int64_t n_tok, int heads, int d,
+                         int head, int lattice, const int* k, uint32_t* words, int64_t pos0,
+                         uint16_t* len /*[n_tok]*/) {
+    uint64_t p = (uint64_t)pos0;
+    for (int64_t t = 0; t < n_tok; ++t) {
+        int64_t L = write_tile(lattice, codes + (t * heads + head) * d, d, k, words, p);
+        len[t] = (uint16_t)L;
+        p += (uint64_t)L;
+    }
+    return (int64_t)p;
+}
+
+/* reconstruct one cached vector the long way (O4): decode -> c - U -> un-normalize -> Sᵀ -> RHT⁻¹ */
+static void kv_reconstruct(const int8_t* codes, uint16_t norm_bits, int d, int lattice, double inv_A,
+                           int rotation, int dither, uint64_t seed, uint32_t token, uint32_t head,
+                           uint32_t role, const int8_t* D, const int8_t* S, double* out) {
+    double u[1024];
+    double sc = (double)f16_bits_to_f32(norm_bits) * inv_A;
+    int dim = lattice;
+    for (int b = 0; b < d / dim; ++b) {
+        float U[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+        if (dither) dither_block(lattice, seed, (uint32_t)b, token, head, role, U);
+        for (int i = 0; i < dim; ++i) {
+            double p = (double)codes[b * dim + i];
+            if (lattice == HQO_A2 && i == 0) p *= sqrt(3.0);
+            u[b * dim + i] = sc * (p - (double)U[i]);
+        }
+    }
+    if (norm_bits == 0) for (int i = 0; i < d; ++i) u[i] = 0.0;
+    if (rotation == 1)
+        for (int i = 0; i < d; ++i) u[i] = (S[i] < 0) ? -u[i] : u[i];
+    rht_inverse_f64(u, D, d, out);
+}
+void hqo_kv_reconstruct(const int8_t* codes /*[n_tok,heads,d]*/, const uint16_t* norms, int64_t n_tok,
+                        int heads, int d, int64_t token0, int role, int lattice, double snr_db,
+                        int rotation, int dither, uint64_t seed, double* out /*[n_tok,heads,d]*/) {
+    double inv_A = 1.0 / (hqo_alpha(lattice, snr_db) * sqrt((double)d));
+    int8_t *D = (int8_t*)malloc((size_t)d), *S = (int8_t*)malloc((size_t)d);
+    hqo_signs(seed, 1u, d, D);
+    hqo_signs(seed, 2u, d, S);
+#pragma omp parallel for schedule(static)
+    for (int64_t t = 0; t < n_tok; ++t)
+        for (int h = 0; h < heads; ++h)
+            kv_reconstruct(codes + (t * heads + h) * d, norms[t * heads + h], d, lattice, inv_A,
+                           rotation, dither, seed, (uint32_t)(token0 + t), (uint32_t)h,
+                           (uint32_t)role, D, S, out + (t * heads + h) * d);
+    free(D); free(S);
+}
+
+/* O4: textbook attention (L178) in double over reconstructed K̂,V̂ [T,heads,d]; the last `window`
+ * tokens are taken from exact (bf16-valued) K,V instead (L562).  q [q_heads, d]. */
+void hqo_attend(const double* Khat, const double* Vhat, const float* Kexact, const float* Vexact,
+                int64_t T, int heads, int d, int window, const float* q, int q_heads,
+                double* out /*[q_heads,d]*/) {
+    int gsz = q_heads / heads;
+    int64_t w0 = T - window < 0 ? 0 : T - window;
+#pragma omp parallel for schedule(static)
+    for (int qh = 0; qh < q_heads; ++qh) {
+        int h = qh / gsz;
+        double* s = (double*)malloc((size_t)T * sizeof(double));
+        double mx = -INFINITY, den = 0.0;
+        for (int64_t t = 0; t < T; ++t) {
+            double dot = 0.0;
+            for (int i = 0; i < d; ++i) {
+                double kk = (t >= w0) ? (double)Kexact[(t * heads + h) * d + i]
+                                      : Khat[(t * heads + h) * d + i];
+                dot += (double)q[qh * d + i] * kk;
+            }
+            s[t] = dot / sqrt((double)d);
+            if (s[t] > mx) mx = s[t];
+        }
+        for (int64_t t = 0; t < T; ++t) { s[t] = exp(s[t] - mx); den += s[t]; }
+        for (int i = 0; i < d; ++i) {
+            double a = 0.0;
+            for (int64_t t = 0; t < T; ++t) {
+                double vv = (t >= w0) ? (double)Vexact[(t * heads + h) * d + i]
+                                      : Vhat[(t * heads + h) * d + i];
+                a += s[t] * vv;
+            }
+            out[qh * d + i] = a / den;
+        }
+        free(s);
+    }
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* Calibration helper (B.1 L857): quantize iid-Gaussian tiles at one SNR; report realized SNR.   */
+/* tiles [nt, n] fp32 ~ N(0,1) are the "post-RHT" vectors themselves (no RHT applied).          */
+/* ------------------------------------------------------------------------------------------ */
+void hqo_calib_quantize(const float* tiles, int64_t nt, int n, int lattice, double snr_db,
+                        int8_t* codes, double* sig_pow, double* err_pow) {
+    float A = (float)(hqo_alpha(lattice, snr_db) * sqrt((double)n));
+    double inv_A = 1.0 / (hqo_alpha(lattice, snr_db) * sqrt((double)n));
+    double sp = 0.0, ep = 0.0;
+#pragma omp parallel for reduction(+ : sp, ep) schedule(static)
+    for (int64_t t = 0; t < nt; ++t) {
+        uint16_t nb;
+        quantize_tile(lattice, n, A, tiles + t * n, 0, 0, 0, 0, 0, codes + t * n, &nb);
+        double sc = (double)f16_bits_to_f32(nb) * inv_A;
+        for (int i = 0; i < n; ++i) {
+            double p = (double)codes[t * n + i];
+            if (lattice == HQO_A2 && (i & 1) == 0) p *= sqrt(3.0);
+            double x = (double)tiles[t * n + i], e = x - sc * p;
+            sp += x * x;
+            ep += e * e;
+        }
+    }
+    *sig_pow = sp;
+    *err_pow = ep;
+}
