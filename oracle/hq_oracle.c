@@ -341,34 +341,71 @@ int64_t hqo_tile_bits(int lattice, const int8_t* codes, int n, const int* k) {
     return L;
 }
 
-/* write one tile stream at bit position pos; returns its length */
-static int64_t write_tile(int lattice, const int8_t* codes, int n, const int* k, uint32_t* words,
-                          uint64_t pos) {
+/* Field planes of a k-bit remainder (FORMAT §4): one plane of width w = 1, 2, 4 for each set bit
+ * of k = b0 + 2·b1 + 4·b2, in that order, each covering the next w remainder bits from bit 0 up
+ * (k = 3: a 1-bit plane holding bit 0, then a 2-bit plane holding bits 1-2). */
+static int field_planes(int k, int* w, int* lo) {
+    int np = 0, at = 0;
+    for (int b = 0; b < 3; ++b)
+        if (k & (1 << b)) { w[np] = 1 << b; lo[np] = at; at += 1 << b; ++np; }
+    return np;
+}
+static int rbits_of(int lattice, int n, const int* k) {
+    int r = 0;
+    for (int j = 0; j < n; ++j) r += k[sym_class(lattice, j)];
+    return r;
+}
+int hqo_rbits(int lattice, int n, const int* k) { return rbits_of(lattice, n, k); }
+
+/* R-section of one tile at bit position pos of `words` (FORMAT §4); returns its length n_0 k_0 + n_1 k_1 */
+static int64_t write_tile_R(int lattice, const int8_t* codes, int n, const int* k, uint32_t* words,
+                            uint64_t pos) {
     int32_t z[1024];
     uint64_t p = pos;
     tile_symbols(lattice, codes, n, z);
     int nclass = (lattice == HQO_D4 || lattice == HQO_A2) ? 2 : 1;
-    for (int a = 0; a < nclass; ++a) { /* R-section */
+    for (int a = 0; a < nclass; ++a) {
         int32_t r[1024];
-        int na = 0, ka = k[a];
+        int na = 0, ka = k[a], w[3], lo[3];
+        int np = field_planes(ka, w, lo);
         for (int j = 0; j < n; ++j)
             if (sym_class(lattice, j) == a) r[na++] = z[j] & ((1 << ka) - 1);
         for (int ch = 0; ch * 32 < na; ++ch) {
-            int w = na - ch * 32 < 32 ? na - ch * 32 : 32;
-            for (int b = 0; b < ka; ++b) {
-                if (w == 32) {
-                    uint32_t V = 0;
-                    for (int u = 0; u < 32; ++u)
-                        V |= (uint32_t)((r[ch * 32 + u] >> b) & 1) << (8 * (u & 3) + (u >> 2));
-                    put_word(words, p, V, 32);
-                } else {
-                    for (int u = 0; u < w; ++u) put_bit(words, p + u, (r[ch * 32 + u] >> b) & 1);
+            int cnt = na - ch * 32 < 32 ? na - ch * 32 : 32;
+            for (int pl = 0; pl < np; ++pl) {
+                int wd = w[pl], per = 8 / wd; /* groups of 4 symbols per word */
+                if (cnt == 32) {
+                    for (int i = 0; i < wd; ++i) {
+                        uint32_t V = 0;
+                        for (int u = 0; u < 32; ++u) {
+                            int g = u >> 2;
+                            if (g / per != i) continue;
+                            uint32_t f = (uint32_t)(r[ch * 32 + u] >> lo[pl]) & ((1u << wd) - 1u);
+                            V |= f << (8 * (u & 3) + wd * (g % per));
+                        }
+                        put_word(words, p, V, 32);
+                        p += 32;
+                    }
+                } else { /* partial chunk: fields in symbol order, each MSB-first */
+                    for (int u = 0; u < cnt; ++u) {
+                        uint32_t f = (uint32_t)(r[ch * 32 + u] >> lo[pl]) & ((1u << wd) - 1u);
+                        put_word(words, p, f, wd);
+                        p += wd;
+                    }
                 }
-                p += w;
             }
         }
     }
-    for (int j = 0; j < n; ++j) { /* U-section: q zeros then a one */
+    return (int64_t)(p - pos);
+}
+
+/* U-section: for j = 0..n-1, q_j zeros then a one (§3.3); returns its length n + Σ q_j */
+static int64_t write_tile_U(int lattice, const int8_t* codes, int n, const int* k, uint32_t* words,
+                            uint64_t pos) {
+    int32_t z[1024];
+    uint64_t p = pos;
+    tile_symbols(lattice, codes, n, z);
+    for (int j = 0; j < n; ++j) {
         int q = z[j] >> k[sym_class(lattice, j)];
         p += q;
         put_bit(words, p, 1u);
@@ -377,30 +414,46 @@ static int64_t write_tile(int lattice, const int8_t* codes, int n, const int* k,
     return (int64_t)(p - pos);
 }
 
-/* read one tile stream of n symbols at bit position pos -> codes; returns bits consumed */
-static int64_t read_tile(int lattice, int n, const int* k, const uint32_t* words, uint64_t pos,
-                         int8_t* codes) {
+/* decode one tile from its R-section (rwords, rpos) and U-section (uwords, upos); returns U bits used */
+static int64_t read_tile_RU(int lattice, int n, const int* k, const uint32_t* rwords, uint64_t rpos,
+                            const uint32_t* uwords, uint64_t upos, int8_t* codes) {
     int32_t z[1024], rem[1024];
-    uint64_t p = pos;
+    uint64_t p = rpos;
     int nclass = (lattice == HQO_D4 || lattice == HQO_A2) ? 2 : 1;
     for (int a = 0; a < nclass; ++a) {
-        int idx[1024], na = 0, ka = k[a];
+        int idx[1024], na = 0, ka = k[a], w[3], lo[3];
+        int np = field_planes(ka, w, lo);
         for (int j = 0; j < n; ++j)
             if (sym_class(lattice, j) == a) { idx[na++] = j; rem[j] = 0; }
         for (int ch = 0; ch * 32 < na; ++ch) {
-            int w = na - ch * 32 < 32 ? na - ch * 32 : 32;
-            for (int b = 0; b < ka; ++b) {
-                for (int u = 0; u < w; ++u) {
-                    int bitpos = (w == 32) ? 31 - (8 * (u & 3) + (u >> 2)) : u;
-                    rem[idx[ch * 32 + u]] |= (int32_t)get_bit(words, p + bitpos) << b;
+            int cnt = na - ch * 32 < 32 ? na - ch * 32 : 32;
+            for (int pl = 0; pl < np; ++pl) {
+                int wd = w[pl], per = 8 / wd;
+                if (cnt == 32) {
+                    for (int i = 0; i < wd; ++i) {
+                        for (int u = 0; u < 32; ++u) {
+                            int g = u >> 2;
+                            if (g / per != i) continue;
+                            int sh = 8 * (u & 3) + wd * (g % per); /* field's bit 0 in V */
+                            for (int b = 0; b < wd; ++b)
+                                rem[idx[ch * 32 + u]] |= (int32_t)get_bit(rwords, p + (31 - (sh + b))) << (lo[pl] + b);
+                        }
+                        p += 32;
+                    }
+                } else {
+                    for (int u = 0; u < cnt; ++u) {
+                        for (int b = 0; b < wd; ++b)
+                            rem[idx[ch * 32 + u]] |= (int32_t)get_bit(rwords, p + b) << (lo[pl] + wd - 1 - b);
+                        p += wd;
+                    }
                 }
-                p += w;
             }
         }
     }
+    p = upos;
     for (int j = 0; j < n; ++j) {
         int q = 0;
-        while (!get_bit(words, p)) { ++q; ++p; }
+        while (!get_bit(uwords, p)) { ++q; ++p; }
         ++p;
         z[j] = (q << k[sym_class(lattice, j)]) | rem[j];
     }
@@ -410,7 +463,19 @@ static int64_t read_tile(int lattice, int n, const int* k, const uint32_t* words
         hqo_unstrip(lattice, z + b * dim, c);
         for (int i = 0; i < dim; ++i) codes[b * dim + i] = (int8_t)c[i];
     }
-    return (int64_t)(p - pos);
+    return (int64_t)(p - upos);
+}
+
+/* the logical tile stream = R-section ‖ U-section at one bit position; returns its length L */
+static int64_t write_tile(int lattice, const int8_t* codes, int n, const int* k, uint32_t* words,
+                          uint64_t pos) {
+    int64_t R = write_tile_R(lattice, codes, n, k, words, pos);
+    return R + write_tile_U(lattice, codes, n, k, words, pos + (uint64_t)R);
+}
+static int64_t read_tile(int lattice, int n, const int* k, const uint32_t* words, uint64_t pos,
+                         int8_t* codes) {
+    int R = rbits_of(lattice, n, k);
+    return R + read_tile_RU(lattice, n, k, words, pos, words, pos + (uint64_t)R, codes);
 }
 
 /* single-tile entry points for the round-trip pins */
@@ -551,32 +616,36 @@ int64_t hqo_pack_weights(const int8_t* codes, const uint16_t* norms, int64_t m, 
                          int lattice, int n, const int* k, uint8_t* blob,
                          uint32_t* group_off /*[G+1]*/) {
     int64_t n_kt = n_in / n, n_rb = (m + 127) / 128, off16 = 0;
+    int64_t Rbits = rbits_of(lattice, n, k), r16 = (128 * Rbits + 127) / 128;
     for (int64_t rb = 0; rb < n_rb; ++rb)
         for (int64_t kt = 0; kt < n_kt; ++kt) {
-            int64_t g = rb * n_kt + kt, bits = 0;
+            int64_t g = rb * n_kt + kt, ubits = 0;
             group_off[g] = (uint32_t)off16;
-            uint16_t* len = blob ? (uint16_t*)(blob + 16 * off16) : NULL;
-            uint16_t* nrm = len ? len + 128 : NULL;
-            uint32_t* payload = blob ? (uint32_t*)(blob + 16 * off16 + 512) : NULL;
+            uint16_t* ulen = blob ? (uint16_t*)(blob + 16 * off16) : NULL;
+            uint16_t* nrm = ulen ? ulen + 128 : NULL;
+            uint32_t* rarea = blob ? (uint32_t*)(blob + 16 * (off16 + 32)) : NULL;
+            uint32_t* uarea = blob ? (uint32_t*)(blob + 16 * (off16 + 32 + r16)) : NULL;
             for (int i = 0; i < 128; ++i) {
                 int64_t r = rb * 128 + i;
-                int64_t L = (r < m) ? hqo_tile_bits(lattice, codes + r * n_in + kt * n, n, k) : 0;
+                int64_t U = (r < m) ? hqo_tile_bits(lattice, codes + r * n_in + kt * n, n, k) - Rbits : 0;
                 if (blob) {
-                    len[i] = (uint16_t)L;
+                    ulen[i] = (uint16_t)U;
                     nrm[i] = (r < m) ? norms[r * n_kt + kt] : 0;
                 }
-                bits += L;
+                ubits += U;
             }
-            int64_t pay16 = (bits + 127) / 128;
+            int64_t u16 = (ubits + 127) / 128;
             if (blob) {
-                memset(payload, 0, (size_t)pay16 * 16);
+                memset(rarea, 0, (size_t)(r16 + u16) * 16);
                 uint64_t p = 0;
                 for (int i = 0; i < 128; ++i) {
                     int64_t r = rb * 128 + i;
-                    if (r < m) p += (uint64_t)write_tile(lattice, codes + r * n_in + kt * n, n, k, payload, p);
+                    if (r >= m) break;
+                    write_tile_R(lattice, codes + r * n_in + kt * n, n, k, rarea, (uint64_t)(i * Rbits));
+                    p += (uint64_t)write_tile_U(lattice, codes + r * n_in + kt * n, n, k, uarea, p);
                 }
             }
-            off16 += 32 + pay16;
+            off16 += 32 + r16 + u16;
         }
     group_off[n_rb * n_kt] = (uint32_t)off16;
     return off16 * 16;
@@ -586,19 +655,22 @@ int64_t hqo_pack_weights(const int8_t* codes, const uint16_t* norms, int64_t m, 
 void hqo_unpack_weights(const uint8_t* blob, const uint32_t* group_off, int64_t m, int64_t n_in,
                         int lattice, int n, const int* k, int8_t* codes, uint16_t* norms) {
     int64_t n_kt = n_in / n, n_rb = (m + 127) / 128;
+    int64_t Rbits = rbits_of(lattice, n, k), r16 = (128 * Rbits + 127) / 128;
 #pragma omp parallel for schedule(static)
     for (int64_t g = 0; g < n_rb * n_kt; ++g) {
         int64_t rb = g / n_kt, kt = g % n_kt;
-        const uint16_t* len = (const uint16_t*)(blob + 16 * (int64_t)group_off[g]);
-        const uint16_t* nrm = len + 128;
-        const uint32_t* payload = (const uint32_t*)(blob + 16 * (int64_t)group_off[g] + 512);
+        const uint8_t* base = blob + 16 * (int64_t)group_off[g];
+        const uint16_t* ulen = (const uint16_t*)base;
+        const uint16_t* nrm = ulen + 128;
+        const uint32_t* rarea = (const uint32_t*)(base + 512);
+        const uint32_t* uarea = (const uint32_t*)(base + 512 + 16 * r16);
         uint64_t p = 0;
         for (int i = 0; i < 128; ++i) {
             int64_t r = rb * 128 + i;
             if (r >= m) break;
             norms[r * n_kt + kt] = nrm[i];
-            read_tile(lattice, n, k, payload, p, codes + r * n_in + kt * n);
-            p += len[i];
+            read_tile_RU(lattice, n, k, rarea, (uint64_t)(i * Rbits), uarea, p, codes + r * n_in + kt * n);
+            p += ulen[i];
         }
     }
 }
@@ -735,18 +807,28 @@ int64_t hqo_kv_quantize(const float* kv, int64_t n_tok, int heads, int d, int64_
     return clamps;
 }
 
-/* pack one (role, head) stream: vectors of tokens [0, n_tok) appended after bit position pos0.
- * len[t] written; returns new bit position.  words must be zero-initialized beyond pos0. */
+/* pack one (role, head) of the KV container (FORMAT §6): token t's R-section goes to bit
+ * (t0 + t)·Rbits of `rem`, its U-section is appended to `una` after bit position upos0.
+ * ulen[t] written; returns the new U position.  Both word arrays zero-initialized by the caller. */
 int64_t hqo_kv_pack_head(const int8_t* codes /*[n_tok,heads,d]*/, int64_t n_tok, int heads, int d,
-                         int head, int lattice, const int* k, uint32_t* words, int64_t pos0,
-                         uint16_t* len /*[n_tok]*/) {
-    uint64_t p = (uint64_t)pos0;
+                         int head, int lattice, const int* k, int64_t t0, uint32_t* rem,
+                         uint32_t* una, int64_t upos0, uint16_t* ulen /*[n_tok]*/) {
+    uint64_t p = (uint64_t)upos0;
+    int64_t Rbits = rbits_of(lattice, d, k);
     for (int64_t t = 0; t < n_tok; ++t) {
-        int64_t L = write_tile(lattice, codes + (t * heads + head) * d, d, k, words, p);
-        len[t] = (uint16_t)L;
-        p += (uint64_t)L;
+        const int8_t* c = codes + (t * heads + head) * d;
+        write_tile_R(lattice, c, d, k, rem, (uint64_t)((t0 + t) * Rbits));
+        int64_t U = write_tile_U(lattice, c, d, k, una, p);
+        ulen[t] = (uint16_t)U;
+        p += (uint64_t)U;
     }
     return (int64_t)p;
+}
+/* decode token t of a packed (role, head): R-section at t·Rbits of rem, U-section at upos of una */
+int64_t hqo_kv_unpack_token(int lattice, int d, const int* k, const uint32_t* rem, int64_t t,
+                            const uint32_t* una, int64_t upos, int8_t* codes) {
+    int64_t Rbits = rbits_of(lattice, d, k);
+    return read_tile_RU(lattice, d, k, rem, (uint64_t)(t * Rbits), una, (uint64_t)upos, codes);
 }
 
 /* reconstruct one cached vector the long way (O4): decode -> c - U -> un-normalize -> Sᵀ -> RHT⁻¹ */

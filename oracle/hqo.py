@@ -30,7 +30,7 @@ def lib():
         _lib.hqo_f32_to_f16_bits.argtypes = [C.c_float]
         for name in ("hqo_tile_bits", "hqo_write_tile", "hqo_read_tile", "hqo_rice_reference_bits",
                      "hqo_quantize_weights", "hqo_total_bits", "hqo_pack_weights",
-                     "hqo_kv_quantize", "hqo_kv_pack_head"):
+                     "hqo_kv_quantize", "hqo_kv_pack_head", "hqo_kv_unpack_token"):
             getattr(_lib, name).restype = C.c_int64
     return _lib
 
@@ -257,12 +257,25 @@ def kv_quantize(kv, token0, role, lattice, snr_db, rotation, dither, seed):
     return codes, norms, clamps
 
 
-def kv_pack_head(codes, head, lattice, k, words, pos0):
+def rbits(lattice, n, k):
+    k = _karr(k)
+    return lib().hqo_rbits(lattice, C.c_int(n), _p(k))
+
+
+def kv_pack_head(codes, head, lattice, k, rem, una, upos0, t0=0):
+    """FORMAT §6: R-sections to rem at (t0+t)*Rbits, U-sections appended to una from bit upos0."""
     codes = _c(codes, np.int8); n_tok, heads, d = codes.shape; k = _karr(k)
-    lens = np.zeros(n_tok, np.uint16)
+    ulen = np.zeros(n_tok, np.uint16)
     pos = lib().hqo_kv_pack_head(_p(codes), C.c_int64(n_tok), C.c_int(heads), C.c_int(d), C.c_int(head),
-                                 lattice, _p(k), _p(words), C.c_int64(pos0), _p(lens))
-    return pos, lens
+                                 lattice, _p(k), C.c_int64(t0), _p(rem), _p(una), C.c_int64(upos0), _p(ulen))
+    return pos, ulen
+
+
+def kv_unpack_token(lattice, d, k, rem, t, una, upos):
+    k = _karr(k); codes = np.zeros(d, np.int8)
+    used = lib().hqo_kv_unpack_token(lattice, C.c_int(d), _p(k), _p(rem), C.c_int64(t), _p(una),
+                                     C.c_int64(upos), _p(codes))
+    return codes, used
 
 
 def kv_reconstruct(codes, norms, token0, role, lattice, snr_db, rotation, dither, seed):

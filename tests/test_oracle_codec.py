@@ -118,8 +118,11 @@ def test_weight_container_roundtrip(lattice, n_tile, m):
     enc = hqo.encode_weights(W, lattice, n_tile, 22.0, seed=9)
     codes, norms = hqo.unpack_weights(enc["blob"], enc["group_off"], m, 512, lattice, n_tile, enc["k"])
     assert (codes == enc["codes"]).all() and (norms == enc["norms"]).all()
-    # layout facts of FORMAT §5: headers hold the tile lengths, groups are 16-byte aligned and ordered
+    # layout facts of FORMAT §5: headers hold the U-section lengths, R-sections sit at a fixed
+    # stride, groups are 16-byte aligned and ordered
     n_kt, n_rb = 512 // n_tile, (m + 127) // 128
+    Rbits = hqo.rbits(lattice, n_tile, enc["k"])
+    r16 = (128 * Rbits + 127) // 128
     goff = enc["group_off"].astype(np.int64)
     assert len(goff) == n_rb * n_kt + 1 and (np.diff(goff) > 32).all() and goff[-1] * 16 == enc["blob"].size
     lens_total = 0
@@ -129,10 +132,38 @@ def test_weight_container_roundtrip(lattice, n_tile, m):
         assert (hdr[rows:128] == 0).all() and (hdr[128 + rows:] == 0).all()
         for i in range(rows):
             r, kt = 128 * (g // n_kt) + i, g % n_kt
-            assert hdr[i] == hqo.tile_bits(lattice, enc["codes"][r, kt * n_tile:(kt + 1) * n_tile], enc["k"])
-        assert (goff[g + 1] - goff[g] - 32) == (int(hdr[:128].sum()) + 127) // 128
-        lens_total += int(hdr[:128].sum())
+            assert hdr[i] + Rbits == hqo.tile_bits(lattice, enc["codes"][r, kt * n_tile:(kt + 1) * n_tile], enc["k"])
+        assert (goff[g + 1] - goff[g] - 32 - r16) == (int(hdr[:128].sum()) + 127) // 128
+        lens_total += int(hdr[:128].sum()) + rows * Rbits
     assert lens_total == enc["payload_bits"]
+
+
+def test_field_plane_layout_is_swar_extractable():
+    # FORMAT §4: in a full chunk of 32 symbols the w-bit field of symbols 4g..4g+3 is
+    # (V[g // (8/w)] >> (w * (g % (8/w)))) & (mask_w * 0x01010101), one symbol per byte.
+    rng = np.random.default_rng(5)
+    for k in range(1, 8):
+        zz = rng.integers(0, 1 << k, size=64)          # Z lattice: symbol = zigzag(code), q = 0
+        codes = np.where(zz & 1, -((zz + 1) >> 1), zz >> 1).astype(np.int8)
+        words = np.zeros(64, np.uint32)
+        L = hqo.write_tile(hqo.Z, codes, (k, k), words, 0)
+        assert L == 64 * (k + 1) and hqo.rbits(hqo.Z, 64, (k, k)) == 64 * k
+        wi = 0
+        for ch in range(2):
+            lo = 0
+            for wd in (1, 2, 4):
+                if not k & wd:
+                    continue
+                per = 8 // wd
+                for g in range(8):
+                    V = int(words[wi + g // per])
+                    f4 = (V >> (wd * (g % per))) & (((1 << wd) - 1) * 0x01010101)
+                    for u in range(4):
+                        assert (f4 >> (8 * u)) & 0xFF == (int(zz[32 * ch + 4 * g + u]) >> lo) & ((1 << wd) - 1)
+                wi += wd
+                lo += wd
+        # U-section: q = 0 everywhere -> 64 one bits right after the R-section
+        assert words[wi] == 0xFFFFFFFF and words[wi + 1] == 0xFFFFFFFF and words[wi + 2] == 0
 
 
 def test_auto_k_is_argmin():
@@ -287,15 +318,22 @@ def test_attend_window_covers_everything_equals_exact_attention():
 def test_kv_stream_pack_and_lengths():
     T, heads, d = 20, 2, 128
     K = hq_synth.kv_tokens(T, heads, d, seed=4)
-    codes, norms, _ = hqo.kv_quantize(K, 0, 0, hqo.E8, 9.68, 1, 1, seed=1)
-    words = np.zeros(4096, np.uint32)
-    pos, lens = hqo.kv_pack_head(codes, 1, hqo.E8, (0, 0), words, 0)
-    assert pos == lens.astype(np.int64).sum()
-    p = 0
-    for t in range(T):
-        back, used = hqo.read_tile(hqo.E8, d, (0, 0), words, p)
-        assert used == lens[t] and (back == codes[t, 1]).all()
-        p += used
-    # ~2 bps + fp16 norm: effective 2.25-2.4 bits/scalar incl. u16 length -> KV× ≈ 6.4-6.6 (L587-590)
-    eff = (lens.mean() + 32) / d
-    assert 2.0 < eff < 2.6
+    for snr, k in ((9.68, (0, 0)), (22.68, (2, 2))):
+        codes, norms, _ = hqo.kv_quantize(K, 0, 0, hqo.E8, snr, 1, 1, seed=1)
+        Rbits = hqo.rbits(hqo.E8, d, k)
+        rem = np.zeros(T * Rbits // 32 + 4, np.uint32); una = np.zeros(4096, np.uint32)
+        # appended in two calls: the second continues where the first stopped (FORMAT §6)
+        pos1, l1 = hqo.kv_pack_head(codes[:7], 1, hqo.E8, k, rem, una, 0, t0=0)
+        pos, l2 = hqo.kv_pack_head(codes[7:], 1, hqo.E8, k, rem, una, pos1, t0=7)
+        ulen = np.concatenate([l1, l2])
+        assert pos == ulen.astype(np.int64).sum()
+        p = 0
+        for t in range(T):
+            back, used = hqo.kv_unpack_token(hqo.E8, d, k, rem, t, una, p)
+            assert used == ulen[t] and (back == codes[t, 1]).all()
+            assert used + Rbits == hqo.tile_bits(hqo.E8, codes[t, 1], k)
+            p += used
+        if k[0] == 0:
+            # ~2 bps + fp16 norm: effective 2.25-2.4 bits/scalar incl. u16 length -> KV× ≈ 6.4-6.6 (L587-590)
+            eff = (ulen.mean() + Rbits + 32) / d
+            assert 2.0 < eff < 2.6
