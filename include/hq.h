@@ -1,0 +1,173 @@
+/*
+ * hq.h — C ABI of libhq.so: HyperQuant's inference-time hot path on one NVIDIA B200 (sm_100a).
+ *
+ * Citations are /root/reference/PAPER.md line numbers (arxiv/paper_2606_23406); "FORMAT" is
+ * docs/FORMAT.md (bitstream layout and the canonical fp32 arithmetic); "G<n>" are the readings of
+ * the paper listed in DESIGN.md §3.
+ *
+ * Conventions
+ *  - Every pointer says "dev" (CUDA device memory on the context's device) or "host".
+ *  - Caller-owned buffers are never retained past the call; work is enqueued on `stream`
+ *    (a cudaStream_t passed as void*) and is asynchronous unless the call says it synchronizes.
+ *  - Handles (hq_ctx, hq_weight, hq_kv) own only memory obtained from the hq_allocator given to
+ *    hq_create; the library never calls cudaMalloc itself.
+ *  - Every call returns an hq_status; nothing throws or aborts.  hq_last_error() gives the text.
+ *  - There is no CPU fallback: a device that is not compute capability 10.x gives HQ_ERR_UNSUPPORTED.
+ */
+#ifndef HQ_H_
+#define HQ_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    HQ_OK = 0,
+    HQ_ERR_INVALID_ARG = 1, /* NULL pointer, bad enum, bad handle */
+    HQ_ERR_SHAPE = 2,       /* n_in not a multiple of n_tile, head_dim not a supported tile, batch too large ... */
+    HQ_ERR_UNSUPPORTED = 3, /* not an sm_100 device, rotation qjl, ... */
+    HQ_ERR_ALLOC = 4,       /* the caller's allocator returned NULL */
+    HQ_ERR_CUDA = 5,        /* a CUDA runtime call failed; text in hq_last_error */
+    HQ_ERR_FORMAT = 6       /* a tile's U-section does not fit the u16 length field (FORMAT §4) */
+} hq_status;
+
+typedef enum { HQ_Z = 1, HQ_A2 = 2, HQ_D4 = 4, HQ_E8 = 8 } hq_lattice;     /* §3.2, §4.5; value = dimension */
+typedef enum { HQ_F32 = 0, HQ_BF16 = 1 } hq_dtype;
+typedef enum { HQ_ROT_NONE = 0, HQ_ROT_SIGNS = 1 } hq_rotation;              /* §4.2 L216 (qjl: not built) */
+
+/* Device-memory allocator supplied by the caller (the Python binding backs it with torch). */
+typedef struct {
+    void* (*alloc)(void* user, size_t bytes); /* returns a dev pointer aligned to >= 256 bytes, or NULL */
+    void (*free)(void* user, void* dev_ptr);
+    void* user;
+} hq_allocator;
+
+/* The codec operating point (Table 4). */
+typedef struct {
+    int32_t lattice;   /* hq_lattice */
+    int32_t n_tile;    /* RHT tile = normalization tile: 64, 128 or 256 (§4.1, §7.2) */
+    float snr_db;      /* target SNR; alpha = sqrt(10^(snr/10) * G V^(2/N)), eq.(9) */
+    int32_t rice_k[2]; /* Rice parameter per symbol class (FORMAT §3); -1 = auto (argmin of total bits) */
+    uint64_t seed;     /* seeds the RHT signs D (and, for KV, the rotation S and the dither) — FORMAT §1 */
+} hq_codec_config;
+
+typedef struct hq_ctx hq_ctx;
+typedef struct hq_weight hq_weight;
+typedef struct hq_kv hq_kv;
+
+/* ---- context ------------------------------------------------------------------------------- */
+hq_status hq_create(hq_ctx** out, const hq_allocator* alloc, int cuda_device);
+void hq_destroy(hq_ctx* ctx);
+const char* hq_last_error(const hq_ctx* ctx); /* never NULL; valid until the next call on ctx */
+
+/* alpha of eq.(9) L871 for (lattice, snr_db), as the library computes it (host, double). */
+double hq_alpha(int32_t lattice, double snr_db);
+
+/* ---- weights: encode (§5.1; SURVEY §8(a) B1,B3,B5-B7) ------------------------------ */
+/*
+ * Quantize W [m_out, n_in] (row-major, leading dimension ld elements, dev, F32 or BF16): per
+ * (row, column tile) RHT -> l2-normalize to radius alpha*sqrt(n) (norm stored as fp16) -> nearest
+ * lattice point -> strip + zig-zag -> Rice code, packed into the FORMAT §5 container with per-tile
+ * lengths and per-group offsets from a device prefix sum.  Synchronizes `stream` (the container
+ * size is data dependent).  *out owns its device memory; free with hq_weight_free.
+ */
+hq_status hq_encode_weights(hq_ctx* ctx, const void* W_dev, int32_t dtype, int64_t m_out, int64_t n_in,
+                            int64_t ld, const hq_codec_config* cfg, void* stream, hq_weight** out);
+void hq_weight_free(hq_ctx* ctx, hq_weight* w);
+
+typedef struct {
+    int64_t m_out, n_in;
+    int32_t lattice, n_tile, rice_k[2];
+    float snr_db;
+    double alpha;
+    uint64_t seed;
+    int64_t payload_bits;  /* sum over tiles of Rbits + ulen = the Rice code's length */
+    int64_t norm_bits;     /* 16 per tile (L500) */
+    int64_t length_bits;   /* 16 per tile (G12) */
+    int64_t blob_bytes;    /* whole container incl. padding */
+    int64_t n_groups;      /* ceil(m_out/128) * n_in/n_tile */
+    int64_t clamp_count;   /* quantizer inputs limited by the INT8 pre-clamp (G8, L236) */
+} hq_weight_info;
+hq_status hq_weight_get_info(const hq_weight* w, hq_weight_info* out);
+
+/* dev pointers into the handle (valid until hq_weight_free): the FORMAT §5 blob and group_off[G+1]. */
+hq_status hq_weight_export(const hq_weight* w, const void** blob_dev, const uint32_t** group_off_dev);
+
+/* Parity / debug: the INT8 lattice points c [m_out, n_in] (row-major, dev) and fp16 norms
+ * [m_out, n_in/n_tile] (dev, may be NULL) decoded from the container (O2; §4.5-4.7 inverse). */
+hq_status hq_decode_int8(hq_ctx* ctx, const hq_weight* w, int8_t* codes_dev, uint16_t* norms_dev, void* stream);
+
+/* ---- activations (FORMAT R1, R7) ---------------------------------------- */
+/*
+ * x [batch, n_in] (dev, leading dimension ldx) -> per (row, tile): u = RHT(x) with the weight's sign
+ * vector (§3.1 eq.(1)), amax-scaled INT8 cast q = rint(u*127/amax), s_x = amax/127.
+ * q [batch, n_in] int8, s_x [batch, n_in/n_tile] f32, u (optional, may be NULL) [batch, n_in] f32.
+ */
+hq_status hq_act_quant(hq_ctx* ctx, const hq_weight* w, const void* x_dev, int32_t dtype, int64_t batch,
+                       int64_t ldx, int8_t* q_dev, float* s_x_dev, float* u_dev_or_null, void* stream);
+
+/* ---- linear: fused Rice decode -> INT8 points -> tcgen05 INT8 MMA ------- */
+/*
+ * y[b, r] = sum_kt (rho[r,kt] / (alpha sqrt(n))) * s_x[b,kt] * acc[kt,b,r],
+ * acc[kt,b,r] = sum_{i in tile kt} c[r,i] * q[b,i]  (INT32, tcgen05.mma kind::i8).
+ * x [batch, n_in] dev (ldx), y [batch, m_out] bf16 dev (ldy).  Optional debug outputs (dev, may be
+ * NULL): y_f32 [batch, m_out] (the value before the bf16 cast), acc_i32 [n_kt, batch, m_out].
+ * The decoded weights exist only in shared memory.  Any batch >= 1 (tiles of up to 256 rows of x).
+ */
+hq_status hq_linear(hq_ctx* ctx, const hq_weight* w, const void* x_dev, int32_t dtype, int64_t batch,
+                    int64_t ldx, void* y_bf16_dev, int64_t ldy, float* y_f32_dev_or_null,
+                    int32_t* acc_i32_dev_or_null, void* stream);
+
+/* bytes of scratch hq_linear needs for this (weight, batch); it is taken from the ctx allocator and cached. */
+hq_status hq_linear_workspace_bytes(const hq_weight* w, int64_t batch, size_t* bytes);
+
+/* ---- KV cache (§5.2, attend C1-C5) ------------------------------ */
+typedef struct {
+    int32_t kv_heads, head_dim; /* head_dim is the RHT tile (L639): 64, 128 or 256 */
+    int64_t max_tokens;
+    hq_codec_config codec;      /* n_tile must equal head_dim; rice_k must be given (>= 0) */
+    int32_t rotation;           /* hq_rotation: S applied after the RHT (§4.2, G14) */
+    int32_t dither;             /* 1: subtractive dither U ~ Unif(V(Lambda)) per token (§4.4, A.6 L843) */
+    int32_t window;             /* exact bf16 residual window, tokens (§6.7.2); 0 = none */
+} hq_kv_config;
+
+hq_status hq_kv_create(hq_ctx* ctx, const hq_kv_config* cfg, hq_kv** out);
+void hq_kv_free(hq_ctx* ctx, hq_kv* kv);
+
+/* Append n_tok tokens: k, v [n_tok, kv_heads, head_dim] bf16 dev.  Encodes every vector (RHT ->
+ * rotate -> normalize -> dither -> nearest point -> strip -> Rice) into the FORMAT §6 container and
+ * writes the bf16 ring.  Token indices continue from the tokens already held. */
+hq_status hq_kv_append(hq_ctx* ctx, hq_kv* kv, const void* k_dev, const void* v_dev, int64_t n_tok, void* stream);
+
+/* One decode step of attention (L178) for q [q_heads, head_dim] bf16 dev over all held tokens:
+ * tokens [0, T-window) from the bitstream (decoded in the code domain), [T-window, T) from the ring.
+ * out [q_heads, head_dim] bf16 dev; out_f32 optional. q_heads must be a multiple of kv_heads. */
+hq_status hq_attend(hq_ctx* ctx, const hq_kv* kv, const void* q_dev, int32_t q_heads, void* out_bf16_dev,
+                    float* out_f32_dev_or_null, void* stream);
+
+typedef struct {
+    int64_t n_tokens;
+    int64_t rbits;               /* R-section bits per vector */
+    const uint32_t* rem_dev;     /* [2][kv_heads][rem_words]   */
+    const uint32_t* una_dev;     /* [2][kv_heads][una_words]   */
+    const uint16_t* ulen_dev;    /* [2][kv_heads][max_tokens]  */
+    const uint16_t* norm_dev;    /* [2][kv_heads][max_tokens]  */
+    const uint32_t* blk_off_dev; /* [2][kv_heads][max_tokens/128 + 1] */
+    const uint32_t* upos_dev;    /* [2][kv_heads] current U-stream length in bits */
+    int64_t rem_words, una_words;
+    int64_t clamp_count;
+} hq_kv_view;
+/* Synchronizes the device. Pointers stay valid until hq_kv_free. */
+hq_status hq_kv_export(hq_ctx* ctx, const hq_kv* kv, hq_kv_view* out);
+
+/* Parity / debug: decode tokens [t0, t0+n) of one role to INT8 codes [n, kv_heads, head_dim] (dev). */
+hq_status hq_kv_decode_int8(hq_ctx* ctx, const hq_kv* kv, int32_t role, int64_t t0, int64_t n,
+                            int8_t* codes_dev, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HQ_H_ */

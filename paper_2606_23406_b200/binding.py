@@ -1,0 +1,289 @@
+"""ctypes binding of libhq.so (include/hq.h).  Argument marshalling only."""
+import ctypes as C
+import os
+
+import torch
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+HQ_F32, HQ_BF16 = 0, 1
+
+
+class Lattice:
+    Z, A2, D4, E8 = 1, 2, 4, 8
+    BY_NAME = {"Z": 1, "A2": 2, "D4": 4, "E8": 8}
+
+
+class HQError(RuntimeError):
+    pass
+
+
+_ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_void_p, C.c_size_t)
+_FREE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p)
+
+
+class _Allocator(C.Structure):
+    _fields_ = [("alloc", _ALLOC_FN), ("free", _FREE_FN), ("user", C.c_void_p)]
+
+
+class _CodecConfig(C.Structure):
+    _fields_ = [("lattice", C.c_int32), ("n_tile", C.c_int32), ("snr_db", C.c_float), ("rice_k", C.c_int32 * 2),
+                ("seed", C.c_uint64)]
+
+
+class _KVConfig(C.Structure):
+    _fields_ = [("kv_heads", C.c_int32), ("head_dim", C.c_int32), ("max_tokens", C.c_int64), ("codec", _CodecConfig),
+                ("rotation", C.c_int32), ("dither", C.c_int32), ("window", C.c_int32)]
+
+
+class _WeightInfo(C.Structure):
+    _fields_ = [("m_out", C.c_int64), ("n_in", C.c_int64), ("lattice", C.c_int32), ("n_tile", C.c_int32),
+                ("rice_k", C.c_int32 * 2), ("snr_db", C.c_float), ("alpha", C.c_double), ("seed", C.c_uint64),
+                ("payload_bits", C.c_int64), ("norm_bits", C.c_int64), ("length_bits", C.c_int64),
+                ("blob_bytes", C.c_int64), ("n_groups", C.c_int64), ("clamp_count", C.c_int64)]
+
+
+class _KVView(C.Structure):
+    _fields_ = [("n_tokens", C.c_int64), ("rbits", C.c_int64), ("rem_dev", C.c_void_p), ("una_dev", C.c_void_p),
+                ("ulen_dev", C.c_void_p), ("norm_dev", C.c_void_p), ("blk_off_dev", C.c_void_p),
+                ("upos_dev", C.c_void_p), ("rem_words", C.c_int64), ("una_words", C.c_int64),
+                ("clamp_count", C.c_int64)]
+
+
+def lib_path() -> str:
+    return os.path.join(HERE, "libhq.so")
+
+
+_lib = None
+
+EXPORTS = ["hq_create", "hq_destroy", "hq_last_error", "hq_alpha", "hq_encode_weights", "hq_weight_free",
+           "hq_weight_get_info", "hq_weight_export", "hq_decode_int8", "hq_act_quant", "hq_linear",
+           "hq_linear_workspace_bytes", "hq_kv_create", "hq_kv_free", "hq_kv_append", "hq_attend", "hq_kv_export",
+           "hq_kv_decode_int8"]
+
+
+def load_library():
+    """dlopen libhq.so; fails loudly if it has not been built (python -m paper_2606_23406_b200.build)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = lib_path()
+    if not os.path.exists(path):
+        raise HQError(f"{path} is missing: build it with `python -m paper_2606_23406_b200.build` (no CPU fallback)")
+    lib = C.CDLL(path)
+    vp, i32, i64 = C.c_void_p, C.c_int32, C.c_int64
+    lib.hq_create.argtypes = [C.POINTER(vp), C.POINTER(_Allocator), C.c_int]
+    lib.hq_destroy.argtypes = [vp]; lib.hq_destroy.restype = None
+    lib.hq_last_error.argtypes = [vp]; lib.hq_last_error.restype = C.c_char_p
+    lib.hq_alpha.argtypes = [i32, C.c_double]; lib.hq_alpha.restype = C.c_double
+    lib.hq_encode_weights.argtypes = [vp, vp, i32, i64, i64, i64, C.POINTER(_CodecConfig), vp, C.POINTER(vp)]
+    lib.hq_weight_free.argtypes = [vp, vp]; lib.hq_weight_free.restype = None
+    lib.hq_weight_get_info.argtypes = [vp, C.POINTER(_WeightInfo)]
+    lib.hq_weight_export.argtypes = [vp, C.POINTER(vp), C.POINTER(vp)]
+    lib.hq_decode_int8.argtypes = [vp, vp, vp, vp, vp]
+    lib.hq_act_quant.argtypes = [vp, vp, vp, i32, i64, i64, vp, vp, vp, vp]
+    lib.hq_linear.argtypes = [vp, vp, vp, i32, i64, i64, vp, i64, vp, vp, vp]
+    lib.hq_linear_workspace_bytes.argtypes = [vp, i64, C.POINTER(C.c_size_t)]
+    lib.hq_kv_create.argtypes = [vp, C.POINTER(_KVConfig), C.POINTER(vp)]
+    lib.hq_kv_free.argtypes = [vp, vp]; lib.hq_kv_free.restype = None
+    lib.hq_kv_append.argtypes = [vp, vp, vp, vp, i64, vp]
+    lib.hq_attend.argtypes = [vp, vp, vp, i32, vp, vp, vp]
+    lib.hq_kv_export.argtypes = [vp, vp, C.POINTER(_KVView)]
+    lib.hq_kv_decode_int8.argtypes = [vp, vp, i32, i64, i64, vp, vp]
+    _lib = lib
+    return lib
+
+
+def alpha(lattice: int, snr_db: float) -> float:
+    return load_library().hq_alpha(lattice, float(snr_db))
+
+
+def _dtype_code(t: torch.Tensor) -> int:
+    if t.dtype == torch.float32:
+        return HQ_F32
+    if t.dtype == torch.bfloat16:
+        return HQ_BF16
+    raise HQError(f"unsupported dtype {t.dtype}")
+
+
+def _stream_ptr(device) -> int:
+    return torch.cuda.current_stream(device).cuda_stream
+
+
+class Context:
+    """hq_ctx with device memory lent by torch's caching allocator."""
+
+    def __init__(self, device: int = 0):
+        if not torch.cuda.is_available():
+            raise HQError("no CUDA device: libhq has no CPU fallback")
+        self.lib = load_library()
+        self.device = torch.device("cuda", device)
+        self._live = {}
+
+        def _alloc(user, nbytes):
+            try:
+                t = torch.empty(int(nbytes), dtype=torch.uint8, device=self.device)
+            except Exception:
+                return None
+            self._live[t.data_ptr()] = t
+            return t.data_ptr()
+
+        def _free(user, ptr):
+            self._live.pop(ptr, None)
+
+        self._alloc_cb, self._free_cb = _ALLOC_FN(_alloc), _FREE_FN(_free)
+        self._allocator = _Allocator(self._alloc_cb, self._free_cb, None)
+        h = C.c_void_p()
+        st = self.lib.hq_create(C.byref(h), C.byref(self._allocator), device)
+        if st != 0:
+            raise HQError(f"hq_create failed with status {st} (needs an sm_100 device)")
+        self.h = h
+
+    def check(self, st: int):
+        if st != 0:
+            raise HQError(f"libhq status {st}: {self.lib.hq_last_error(self.h).decode()}")
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.lib.hq_destroy(self.h)
+            self.h = None
+
+    # ---- weights ----
+    def encode_weights(self, W: torch.Tensor, lattice: int, n_tile: int, snr_db: float, seed: int, rice_k=(-1, -1)):
+        assert W.is_cuda and W.dim() == 2 and W.stride(1) == 1
+        cfg = _CodecConfig(lattice, n_tile, float(snr_db), (C.c_int32 * 2)(int(rice_k[0]), int(rice_k[1])), seed)
+        h = C.c_void_p()
+        self.check(self.lib.hq_encode_weights(self.h, W.data_ptr(), _dtype_code(W), W.shape[0], W.shape[1],
+                                              W.stride(0), C.byref(cfg), _stream_ptr(self.device), C.byref(h)))
+        return Weight(self, h)
+
+    # ---- KV ----
+    def kv_create(self, kv_heads, head_dim, max_tokens, lattice, snr_db, rice_k, seed, rotation=1, dither=1,
+                  window=32):
+        codec = _CodecConfig(lattice, head_dim, float(snr_db), (C.c_int32 * 2)(int(rice_k[0]), int(rice_k[1])), seed)
+        cfg = _KVConfig(kv_heads, head_dim, max_tokens, codec, rotation, dither, window)
+        h = C.c_void_p()
+        self.check(self.lib.hq_kv_create(self.h, C.byref(cfg), C.byref(h)))
+        return KVCache(self, h, kv_heads, head_dim, max_tokens)
+
+
+class Weight:
+    def __init__(self, ctx: Context, h):
+        self.ctx, self.h = ctx, h
+        info = _WeightInfo()
+        ctx.check(ctx.lib.hq_weight_get_info(h, C.byref(info)))
+        self.info = info
+        self.m, self.n_in, self.n_tile = info.m_out, info.n_in, info.n_tile
+        self.k = (info.rice_k[0], info.rice_k[1])
+
+    def free(self):
+        if self.h:
+            self.ctx.lib.hq_weight_free(self.ctx.h, self.h)
+            self.h = None
+
+    def export(self):
+        """(blob uint8 [blob_bytes], group_off uint32 [G+1]) as host numpy arrays."""
+        blob_p, goff_p = C.c_void_p(), C.c_void_p()
+        self.ctx.check(self.ctx.lib.hq_weight_export(self.h, C.byref(blob_p), C.byref(goff_p)))
+        torch.cuda.synchronize(self.ctx.device)
+        blob = _wrap(blob_p.value, self.info.blob_bytes, self.ctx.device).cpu().numpy()
+        goff = _wrap(goff_p.value, (self.info.n_groups + 1) * 4, self.ctx.device).cpu().numpy().view("uint32")
+        return blob, goff
+
+    def decode_int8(self):
+        dev = self.ctx.device
+        codes = torch.empty((self.m, self.n_in), dtype=torch.int8, device=dev)
+        norms = torch.empty((self.m, self.n_in // self.n_tile), dtype=torch.int16, device=dev)
+        self.ctx.check(self.ctx.lib.hq_decode_int8(self.ctx.h, self.h, codes.data_ptr(), norms.data_ptr(),
+                                                   _stream_ptr(dev)))
+        return codes, norms
+
+    def act_quant(self, x: torch.Tensor, want_u=False):
+        dev = self.ctx.device
+        assert x.is_cuda and x.dim() == 2 and x.shape[1] == self.n_in and x.stride(1) == 1
+        B = x.shape[0]
+        q = torch.empty((B, self.n_in), dtype=torch.int8, device=dev)
+        s_x = torch.empty((B, self.n_in // self.n_tile), dtype=torch.float32, device=dev)
+        u = torch.empty((B, self.n_in), dtype=torch.float32, device=dev) if want_u else None
+        self.ctx.check(self.ctx.lib.hq_act_quant(self.ctx.h, self.h, x.data_ptr(), _dtype_code(x), B, x.stride(0),
+                                                 q.data_ptr(), s_x.data_ptr(), u.data_ptr() if want_u else None,
+                                                 _stream_ptr(dev)))
+        return (q, s_x, u) if want_u else (q, s_x)
+
+    def linear(self, x: torch.Tensor, y: torch.Tensor = None, want_f32=False, want_acc=False):
+        """y = Ŵ x through the fused decode + INT8 MMA kernel. x [B, n_in] (bf16 or f32) -> y [B, m] bf16."""
+        dev = self.ctx.device
+        assert x.is_cuda and x.dim() == 2 and x.shape[1] == self.n_in and x.stride(1) == 1
+        B = x.shape[0]
+        if y is None:
+            y = torch.empty((B, self.m), dtype=torch.bfloat16, device=dev)
+        y32 = torch.empty((B, self.m), dtype=torch.float32, device=dev) if want_f32 else None
+        acc = torch.empty((self.n_in // self.n_tile, B, self.m), dtype=torch.int32, device=dev) if want_acc else None
+        self.ctx.check(self.ctx.lib.hq_linear(self.ctx.h, self.h, x.data_ptr(), _dtype_code(x), B, x.stride(0),
+                                              y.data_ptr(), y.stride(0), y32.data_ptr() if want_f32 else None,
+                                              acc.data_ptr() if want_acc else None, _stream_ptr(dev)))
+        if want_f32 or want_acc:
+            return y, y32, acc
+        return y
+
+
+class KVCache:
+    def __init__(self, ctx: Context, h, kv_heads, head_dim, max_tokens):
+        self.ctx, self.h = ctx, h
+        self.kv_heads, self.head_dim, self.max_tokens = kv_heads, head_dim, max_tokens
+
+    def free(self):
+        if self.h:
+            self.ctx.lib.hq_kv_free(self.ctx.h, self.h)
+            self.h = None
+
+    def append(self, k: torch.Tensor, v: torch.Tensor):
+        assert k.is_cuda and k.dtype == torch.bfloat16 and k.is_contiguous() and v.is_contiguous() and k.shape == v.shape
+        assert tuple(k.shape[1:]) == (self.kv_heads, self.head_dim)
+        self.ctx.check(self.ctx.lib.hq_kv_append(self.ctx.h, self.h, k.data_ptr(), v.data_ptr(), k.shape[0],
+                                                 _stream_ptr(self.ctx.device)))
+
+    def attend(self, q: torch.Tensor, out: torch.Tensor = None, want_f32=False):
+        dev = self.ctx.device
+        assert q.is_cuda and q.dtype == torch.bfloat16 and q.is_contiguous() and q.shape[1] == self.head_dim
+        if out is None:
+            out = torch.empty_like(q)
+        o32 = torch.empty(q.shape, dtype=torch.float32, device=dev) if want_f32 else None
+        self.ctx.check(self.ctx.lib.hq_attend(self.ctx.h, self.h, q.data_ptr(), q.shape[0], out.data_ptr(),
+                                              o32.data_ptr() if want_f32 else None, _stream_ptr(dev)))
+        return (out, o32) if want_f32 else out
+
+    def export(self):
+        """Host copies of the FORMAT §6 container: dict of numpy arrays."""
+        v = _KVView()
+        self.ctx.check(self.ctx.lib.hq_kv_export(self.ctx.h, self.h, C.byref(v)))
+        dev, H, mt = self.ctx.device, self.kv_heads, self.max_tokens
+        n_blk = (mt + 127) // 128
+
+        def arr(ptr, count, np_dtype, itemsize):
+            return _wrap(ptr, count * itemsize, dev).cpu().numpy().view(np_dtype)
+
+        return dict(
+            n_tokens=v.n_tokens, rbits=v.rbits, clamp_count=v.clamp_count,
+            rem=arr(v.rem_dev, 2 * H * v.rem_words, "uint32", 4).reshape(2, H, v.rem_words),
+            una=arr(v.una_dev, 2 * H * v.una_words, "uint32", 4).reshape(2, H, v.una_words),
+            ulen=arr(v.ulen_dev, 2 * H * mt, "uint16", 2).reshape(2, H, mt),
+            norm=arr(v.norm_dev, 2 * H * mt, "uint16", 2).reshape(2, H, mt),
+            blk_off=arr(v.blk_off_dev, 2 * H * (n_blk + 1), "uint32", 4).reshape(2, H, n_blk + 1),
+            upos=arr(v.upos_dev, 2 * H, "uint32", 4).reshape(2, H))
+
+    def decode_int8(self, role, t0, n):
+        codes = torch.empty((n, self.kv_heads, self.head_dim), dtype=torch.int8, device=self.ctx.device)
+        self.ctx.check(self.ctx.lib.hq_kv_decode_int8(self.ctx.h, self.h, role, t0, n, codes.data_ptr(),
+                                                      _stream_ptr(self.ctx.device)))
+        return codes
+
+
+class _DevMem:
+    """__cuda_array_interface__ view of raw device memory (no ownership)."""
+
+    def __init__(self, ptr, nbytes):
+        self.__cuda_array_interface__ = {"shape": (nbytes,), "typestr": "|u1", "data": (ptr, False), "version": 2}
+
+
+def _wrap(ptr, nbytes, device):
+    return torch.as_tensor(_DevMem(ptr, int(nbytes)), device=device)

@@ -1,0 +1,426 @@
+// hq_api.cu — the C ABI of libhq.so (include/hq.h): argument checking, memory through the caller's
+// allocator, kernel sequencing.  No compute happens on the host; there is no CPU fallback.
+#include <math.h>
+#include <string.h>
+
+#include <new>
+#include <vector>
+
+#include "hq_common.cuh"
+#include "hq_internal.h"
+
+using namespace hq;
+
+namespace {
+
+bool valid_lattice(int l) { return l == HQ_Z || l == HQ_A2 || l == HQ_D4 || l == HQ_E8; }
+bool valid_tile(int n) { return n == 64 || n == 128 || n == 256; }
+
+void* ctx_alloc(hq_ctx* ctx, size_t bytes) {
+    if (bytes == 0) bytes = 16;
+    void* p = ctx->alloc.alloc(ctx->alloc.user, bytes);
+    if (!p) ctx->err = "allocator returned NULL for " + std::to_string(bytes) + " bytes";
+    return p;
+}
+void ctx_free(hq_ctx* ctx, void* p) {
+    if (p) ctx->alloc.free(ctx->alloc.user, p);
+}
+
+hq_status fail(hq_ctx* ctx, hq_status s, const char* msg) {
+    if (ctx) ctx->err = msg;
+    return s;
+}
+
+}  // namespace
+
+extern "C" {
+
+hq_status hq_create(hq_ctx** out, const hq_allocator* alloc, int cuda_device) {
+    if (!out || !alloc || !alloc->alloc || !alloc->free) return HQ_ERR_INVALID_ARG;
+    *out = nullptr;
+    int count = 0;
+    if (cudaGetDeviceCount(&count) != cudaSuccess || cuda_device < 0 || cuda_device >= count) return HQ_ERR_UNSUPPORTED;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, cuda_device) != cudaSuccess) return HQ_ERR_CUDA;
+    if (prop.major != 10) return HQ_ERR_UNSUPPORTED;  // tcgen05 / TMEM: sm_100a only, no fallback
+    if (cudaSetDevice(cuda_device) != cudaSuccess) return HQ_ERR_CUDA;
+    hq_ctx* ctx = new (std::nothrow) hq_ctx();
+    if (!ctx) return HQ_ERR_ALLOC;
+    ctx->alloc = *alloc;
+    ctx->device = cuda_device;
+    ctx->sm_count = prop.multiProcessorCount;
+    ctx->err = "";
+    *out = ctx;
+    return HQ_OK;
+}
+
+void hq_destroy(hq_ctx* ctx) {
+    if (!ctx) return;
+    ctx_free(ctx, ctx->ws);
+    delete ctx;
+}
+
+const char* hq_last_error(const hq_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+
+double hq_alpha(int32_t lattice, double snr_db) {
+    if (!valid_lattice(lattice)) return 0.0;
+    return sqrt(pow(10.0, snr_db / 10.0) * second_moment(lattice));
+}
+
+// ---------------------------------------------------------------------------------------------
+hq_status hq_encode_weights(hq_ctx* ctx, const void* W_dev, int32_t dtype, int64_t m_out, int64_t n_in, int64_t ld,
+                            const hq_codec_config* cfg, void* stream, hq_weight** out) {
+    if (!ctx) return HQ_ERR_INVALID_ARG;
+    if (!W_dev || !cfg || !out) return fail(ctx, HQ_ERR_INVALID_ARG, "null argument");
+    *out = nullptr;
+    if (!valid_lattice(cfg->lattice) || (dtype != HQ_F32 && dtype != HQ_BF16))
+        return fail(ctx, HQ_ERR_INVALID_ARG, "bad lattice or dtype");
+    if (!valid_tile(cfg->n_tile) || m_out <= 0 || n_in <= 0 || n_in % cfg->n_tile != 0 || ld < n_in)
+        return fail(ctx, HQ_ERR_SHAPE, "n_tile must be 64/128/256 and divide n_in (the paper auto-shrinks, Table 4 L322; we reject)");
+    for (int a = 0; a < 2; ++a)
+        if (cfg->rice_k[a] < -1 || cfg->rice_k[a] > 7) return fail(ctx, HQ_ERR_INVALID_ARG, "rice_k must be -1 or 0..7");
+    cudaStream_t st = (cudaStream_t)stream;
+    HQ_CUDA_CHECK(ctx, cudaSetDevice(ctx->device));
+
+    hq_weight* w = new (std::nothrow) hq_weight();
+    if (!w) return HQ_ERR_ALLOC;
+    memset((void*)w, 0, sizeof(*w));
+    w->ctx = ctx;
+    w->m = m_out; w->n_in = n_in; w->lattice = cfg->lattice; w->n = cfg->n_tile; w->snr_db = cfg->snr_db;
+    w->seed = cfg->seed;
+    w->alpha = hq_alpha(cfg->lattice, (double)cfg->snr_db);
+    w->A = (float)(w->alpha * sqrt((double)w->n));
+    w->n_kt = n_in / w->n; w->n_rb = (m_out + 127) / 128; w->G = w->n_rb * w->n_kt;
+
+    int8_t* codes = nullptr;
+    uint16_t *norms = nullptr, *ulen_tmp = nullptr;
+    unsigned long long* counters = nullptr;  // [0] clamps, [1..16] auto-k totals, [17] ubits total, [18] err flag, [19] max group
+    hq_status rc = HQ_OK;
+    auto cleanup = [&]() {
+        ctx_free(ctx, codes); ctx_free(ctx, norms); ctx_free(ctx, ulen_tmp); ctx_free(ctx, counters);
+    };
+    auto bail = [&](hq_status s) {
+        cleanup();
+        hq_weight_free(ctx, w);
+        return s;
+    };
+    w->dsign = (int8_t*)ctx_alloc(ctx, (size_t)n_in);
+    codes = (int8_t*)ctx_alloc(ctx, (size_t)(m_out * n_in));
+    norms = (uint16_t*)ctx_alloc(ctx, (size_t)(m_out * w->n_kt) * 2);
+    ulen_tmp = (uint16_t*)ctx_alloc(ctx, (size_t)w->G * 128 * 2);
+    counters = (unsigned long long*)ctx_alloc(ctx, 32 * sizeof(unsigned long long));
+    w->group_off = (uint32_t*)ctx_alloc(ctx, (size_t)(w->G + 1) * 4);
+    if (!w->dsign || !codes || !norms || !ulen_tmp || !counters || !w->group_off) return bail(HQ_ERR_ALLOC);
+
+#define HQ_TRY(call)                                                                 \
+    do {                                                                             \
+        cudaError_t e__ = (call);                                                    \
+        if (e__ != cudaSuccess) {                                                    \
+            ctx->err = std::string(#call) + ": " + cudaGetErrorString(e__);          \
+            return bail(HQ_ERR_CUDA);                                                \
+        }                                                                            \
+    } while (0)
+
+    HQ_TRY(cudaMemsetAsync(counters, 0, 32 * sizeof(unsigned long long), st));
+    launch_signs(w->seed, 1u, n_in, w->dsign, st);
+    launch_quantize_weights(W_dev, dtype, m_out, n_in, ld, w->lattice, w->n, w->A, w->dsign, codes, norms, counters, st);
+    HQ_TRY(cudaGetLastError());
+    unsigned long long hc[32];
+    HQ_TRY(cudaMemcpyAsync(hc, counters, sizeof(hc), cudaMemcpyDeviceToHost, st));
+    HQ_TRY(cudaStreamSynchronize(st));
+    w->clamp_count = (int64_t)hc[0];
+    // Rice parameters (FORMAT §3): argmin of total bits, ties -> smaller; D4 ties k_t = max(k_s-1, 0)
+    int k0 = cfg->rice_k[0], k1 = cfg->rice_k[1];
+    if (k0 < 0 || (k1 < 0 && (w->lattice == HQ_D4 || w->lattice == HQ_A2))) {
+        const unsigned long long* t0 = hc + 1;
+        const unsigned long long* t1 = hc + 9;
+        if (w->lattice == HQ_D4) {
+            int best = 0;
+            unsigned long long bv = ~0ull;
+            for (int ks = 0; ks < 8; ++ks) {
+                unsigned long long v = t0[ks] + t1[ks > 0 ? ks - 1 : 0];
+                if (v < bv) { bv = v; best = ks; }
+            }
+            k0 = best; k1 = best > 0 ? best - 1 : 0;
+        } else {
+            int b0 = 0, b1 = 0;
+            for (int kk = 1; kk < 8; ++kk) {
+                if (t0[kk] < t0[b0]) b0 = kk;
+                if (t1[kk] < t1[b1]) b1 = kk;
+            }
+            k0 = b0; k1 = (w->lattice == HQ_A2) ? b1 : b0;
+        }
+    }
+    if (k1 < 0) k1 = k0;
+    if (w->lattice == HQ_Z || w->lattice == HQ_E8) k1 = k0;
+    w->k0 = k0; w->k1 = k1;
+    w->rbits = rbits_of(w->lattice, w->n, k0, k1);
+
+    int* err_flag = (int*)(counters + 18);
+    uint32_t* maxg = (uint32_t*)(counters + 19);
+    launch_tile_ulen(codes, m_out, n_in, w->lattice, w->n, k0, k1, ulen_tmp, err_flag, st);
+    launch_group_offsets(ulen_tmp, w->G, w->rbits, w->group_off, counters + 17, maxg, st);
+    HQ_TRY(cudaGetLastError());
+    uint32_t total16 = 0;
+    HQ_TRY(cudaMemcpyAsync(&total16, w->group_off + w->G, 4, cudaMemcpyDeviceToHost, st));
+    HQ_TRY(cudaMemcpyAsync(hc, counters, sizeof(hc), cudaMemcpyDeviceToHost, st));
+    HQ_TRY(cudaStreamSynchronize(st));
+    if (*(int*)(hc + 18) != 0) {
+        ctx->err = "a tile's U-section exceeds 65535 bits (FORMAT §4)";
+        return bail(HQ_ERR_FORMAT);
+    }
+    w->max_group16 = *(uint32_t*)(hc + 19);
+    w->blob_bytes = (int64_t)total16 * 16;
+    w->payload_bits = (int64_t)hc[17] + m_out * w->n_kt * (int64_t)w->rbits;
+    w->blob = (uint8_t*)ctx_alloc(ctx, (size_t)w->blob_bytes + 64);  // +64: decoders read one word ahead
+    if (!w->blob) return bail(HQ_ERR_ALLOC);
+    HQ_TRY(cudaMemsetAsync(w->blob, 0, (size_t)w->blob_bytes + 64, st));
+    launch_pack_groups(codes, norms, ulen_tmp, m_out, n_in, w->lattice, w->n, k0, k1, w->group_off, w->blob, st);
+    HQ_TRY(cudaGetLastError());
+    HQ_TRY(cudaStreamSynchronize(st));
+#undef HQ_TRY
+    cleanup();
+    *out = w;
+    return rc;
+}
+
+void hq_weight_free(hq_ctx* ctx, hq_weight* w) {
+    if (!w) return;
+    if (!ctx) ctx = w->ctx;
+    ctx_free(ctx, w->blob);
+    ctx_free(ctx, w->group_off);
+    ctx_free(ctx, w->dsign);
+    delete w;
+}
+
+hq_status hq_weight_get_info(const hq_weight* w, hq_weight_info* out) {
+    if (!w || !out) return HQ_ERR_INVALID_ARG;
+    out->m_out = w->m; out->n_in = w->n_in; out->lattice = w->lattice; out->n_tile = w->n;
+    out->rice_k[0] = w->k0; out->rice_k[1] = w->k1; out->snr_db = w->snr_db; out->alpha = w->alpha;
+    out->seed = w->seed; out->payload_bits = w->payload_bits;
+    out->norm_bits = 16 * w->m * w->n_kt; out->length_bits = 16 * w->m * w->n_kt;
+    out->blob_bytes = w->blob_bytes; out->n_groups = w->G; out->clamp_count = w->clamp_count;
+    return HQ_OK;
+}
+
+hq_status hq_weight_export(const hq_weight* w, const void** blob_dev, const uint32_t** group_off_dev) {
+    if (!w || !blob_dev || !group_off_dev) return HQ_ERR_INVALID_ARG;
+    *blob_dev = w->blob;
+    *group_off_dev = w->group_off;
+    return HQ_OK;
+}
+
+hq_status hq_decode_int8(hq_ctx* ctx, const hq_weight* w, int8_t* codes_dev, uint16_t* norms_dev, void* stream) {
+    if (!ctx) return HQ_ERR_INVALID_ARG;
+    if (!w || !codes_dev) return fail(ctx, HQ_ERR_INVALID_ARG, "null argument");
+    launch_decode_int8(w, codes_dev, norms_dev, (cudaStream_t)stream);
+    HQ_CUDA_CHECK(ctx, cudaGetLastError());
+    return HQ_OK;
+}
+
+hq_status hq_act_quant(hq_ctx* ctx, const hq_weight* w, const void* x_dev, int32_t dtype, int64_t batch, int64_t ldx,
+                       int8_t* q_dev, float* s_x_dev, float* u_dev_or_null, void* stream) {
+    if (!ctx) return HQ_ERR_INVALID_ARG;
+    if (!w || !x_dev || !q_dev || !s_x_dev) return fail(ctx, HQ_ERR_INVALID_ARG, "null argument");
+    if (batch <= 0 || ldx < w->n_in) return fail(ctx, HQ_ERR_SHAPE, "bad batch / ldx");
+    launch_act_quant(x_dev, dtype, batch, w->n_in, ldx, w->lattice, w->n, w->dsign, q_dev, s_x_dev, u_dev_or_null,
+                     (cudaStream_t)stream);
+    HQ_CUDA_CHECK(ctx, cudaGetLastError());
+    return HQ_OK;
+}
+
+static size_t linear_ws_bytes(const hq_ctx* ctx, const hq_weight* w, int64_t B, int* n_split_out) {
+    int ns = linear_choose_split(ctx, w, B);
+    if (n_split_out) *n_split_out = ns;
+    size_t q = ((size_t)(B * w->n_in) + 255) & ~(size_t)255;
+    size_t sx = ((size_t)(B * w->n_kt) * 4 + 255) & ~(size_t)255;
+    size_t part = (size_t)ns * B * w->m * 4;
+    return q + sx + part + 256;
+}
+
+hq_status hq_linear_workspace_bytes(const hq_weight* w, int64_t batch, size_t* bytes) {
+    if (!w || !bytes || batch <= 0) return HQ_ERR_INVALID_ARG;
+    *bytes = linear_ws_bytes(w->ctx, w, batch, nullptr);
+    return HQ_OK;
+}
+
+hq_status hq_linear(hq_ctx* ctx, const hq_weight* w, const void* x_dev, int32_t dtype, int64_t batch, int64_t ldx,
+                    void* y_bf16_dev, int64_t ldy, float* y_f32_dev_or_null, int32_t* acc_i32_dev_or_null, void* stream) {
+    if (!ctx) return HQ_ERR_INVALID_ARG;
+    if (!w || !x_dev || (!y_bf16_dev && !y_f32_dev_or_null)) return fail(ctx, HQ_ERR_INVALID_ARG, "null argument");
+    if (batch <= 0 || ldx < w->n_in || (y_bf16_dev && ldy < w->m)) return fail(ctx, HQ_ERR_SHAPE, "bad batch / ldx / ldy");
+    if (dtype != HQ_F32 && dtype != HQ_BF16) return fail(ctx, HQ_ERR_INVALID_ARG, "bad dtype");
+    cudaStream_t st = (cudaStream_t)stream;
+    int n_split = 1;
+    size_t need = linear_ws_bytes(ctx, w, batch, &n_split);
+    if (need > ctx->ws_bytes) {
+        // the old buffer may still be in use by work already enqueued
+        if (ctx->ws) { HQ_CUDA_CHECK(ctx, cudaDeviceSynchronize()); ctx_free(ctx, ctx->ws); ctx->ws = nullptr; ctx->ws_bytes = 0; }
+        ctx->ws = ctx_alloc(ctx, need);
+        if (!ctx->ws) return HQ_ERR_ALLOC;
+        ctx->ws_bytes = need;
+    }
+    uint8_t* base = (uint8_t*)ctx->ws;
+    int8_t* q = (int8_t*)base;
+    size_t qb = ((size_t)(batch * w->n_in) + 255) & ~(size_t)255;
+    float* s_x = (float*)(base + qb);
+    size_t sb = ((size_t)(batch * w->n_kt) * 4 + 255) & ~(size_t)255;
+    float* partials = (float*)(base + qb + sb);
+    launch_act_quant(x_dev, dtype, batch, w->n_in, ldx, w->lattice, w->n, w->dsign, q, s_x, nullptr, st);
+    HQ_CUDA_CHECK(ctx, cudaGetLastError());
+    return launch_linear(ctx, w, q, s_x, batch, y_bf16_dev, ldy, y_f32_dev_or_null, acc_i32_dev_or_null, partials,
+                         n_split, st);
+}
+
+// ---------------------------------------------------------------------------------------------
+hq_status hq_kv_create(hq_ctx* ctx, const hq_kv_config* cfg, hq_kv** out) {
+    if (!ctx) return HQ_ERR_INVALID_ARG;
+    if (!cfg || !out) return fail(ctx, HQ_ERR_INVALID_ARG, "null argument");
+    *out = nullptr;
+    if (!valid_lattice(cfg->codec.lattice)) return fail(ctx, HQ_ERR_INVALID_ARG, "bad lattice");
+    if (!valid_tile(cfg->head_dim) || cfg->codec.n_tile != cfg->head_dim || cfg->kv_heads <= 0 || cfg->max_tokens <= 0)
+        return fail(ctx, HQ_ERR_SHAPE, "head_dim must be 64/128/256 and equal codec.n_tile");
+    if (cfg->rotation != HQ_ROT_NONE && cfg->rotation != HQ_ROT_SIGNS)
+        return fail(ctx, HQ_ERR_UNSUPPORTED, "rotation qjl is not built (SURVEY §8(f))");
+    if (cfg->codec.rice_k[0] < 0 || cfg->codec.rice_k[0] > 7 || cfg->codec.rice_k[1] > 7)
+        return fail(ctx, HQ_ERR_INVALID_ARG, "KV needs explicit rice_k");
+    if (cfg->window < 0 || cfg->window > cfg->head_dim) return fail(ctx, HQ_ERR_SHAPE, "window must be in [0, head_dim]");
+    hq_kv* kv = new (std::nothrow) hq_kv();
+    if (!kv) return HQ_ERR_ALLOC;
+    memset((void*)kv, 0, sizeof(*kv));
+    kv->ctx = ctx;
+    kv->cfg = *cfg;
+    int H = cfg->kv_heads, d = cfg->head_dim, lat = cfg->codec.lattice;
+    kv->k0 = cfg->codec.rice_k[0];
+    kv->k1 = (lat == HQ_Z || lat == HQ_E8 || cfg->codec.rice_k[1] < 0) ? kv->k0 : cfg->codec.rice_k[1];
+    kv->rbits = rbits_of(lat, d, kv->k0, kv->k1);
+    kv->alpha = hq_alpha(lat, (double)cfg->codec.snr_db);
+    kv->A = (float)(kv->alpha * sqrt((double)d));
+    int64_t mt = cfg->max_tokens;
+    if ((double)mt * (kv->rbits > 0 ? kv->rbits : 1) > 4.0e9) { delete kv; return fail(ctx, HQ_ERR_SHAPE, "max_tokens too large for 32-bit bit offsets"); }
+    kv->n_blk = (mt + 127) / 128;
+    kv->rem_words = (mt * kv->rbits + 31) / 32 + 4;
+    // U-stream capacity: 4 unary bits per scalar on average (E[q] ~ 1 at the calibrated k, FORMAT §3)
+    int64_t una_bits = mt * (int64_t)d * 4 + 4096;
+    if (una_bits > 0xffff0000ll) una_bits = 0xffff0000ll;
+    kv->una_words = una_bits / 32 + 4;
+    size_t n_rh = (size_t)2 * H;
+    kv->rem = (uint32_t*)ctx_alloc(ctx, n_rh * kv->rem_words * 4);
+    kv->una = (uint32_t*)ctx_alloc(ctx, n_rh * kv->una_words * 4);
+    kv->ulen = (uint16_t*)ctx_alloc(ctx, n_rh * mt * 2 + 512);
+    kv->norm = (uint16_t*)ctx_alloc(ctx, n_rh * mt * 2 + 512);
+    kv->blk_off = (uint32_t*)ctx_alloc(ctx, n_rh * (kv->n_blk + 1) * 4);
+    kv->upos = (uint32_t*)ctx_alloc(ctx, n_rh * 4 + 64);
+    kv->ring = (__nv_bfloat16*)ctx_alloc(ctx, (size_t)2 * (cfg->window > 0 ? cfg->window : 1) * H * d * 2);
+    kv->dsign = (int8_t*)ctx_alloc(ctx, d);
+    kv->ssign = (int8_t*)ctx_alloc(ctx, d);
+    kv->counters = (unsigned long long*)ctx_alloc(ctx, 64);
+    kv->att_ws_bytes = attend_workspace_bytes(kv, 64);
+    kv->att_ws = (float*)ctx_alloc(ctx, kv->att_ws_bytes);
+    if (!kv->rem || !kv->una || !kv->ulen || !kv->norm || !kv->blk_off || !kv->upos || !kv->ring || !kv->dsign ||
+        !kv->ssign || !kv->counters || !kv->att_ws) {
+        hq_kv_free(ctx, kv);
+        return HQ_ERR_ALLOC;
+    }
+    cudaMemset(kv->rem, 0, n_rh * kv->rem_words * 4);
+    cudaMemset(kv->una, 0, n_rh * kv->una_words * 4);
+    cudaMemset(kv->ulen, 0, n_rh * mt * 2 + 512);
+    cudaMemset(kv->norm, 0, n_rh * mt * 2 + 512);
+    cudaMemset(kv->blk_off, 0, n_rh * (kv->n_blk + 1) * 4);
+    cudaMemset(kv->upos, 0, n_rh * 4 + 64);
+    cudaMemset(kv->counters, 0, 64);
+    launch_signs(cfg->codec.seed, 1u, d, kv->dsign, 0);
+    launch_signs(cfg->codec.seed, 2u, d, kv->ssign, 0);
+    cudaError_t e = cudaDeviceSynchronize();
+    if (e != cudaSuccess) {
+        ctx->err = cudaGetErrorString(e);
+        hq_kv_free(ctx, kv);
+        return HQ_ERR_CUDA;
+    }
+    *out = kv;
+    return HQ_OK;
+}
+
+void hq_kv_free(hq_ctx* ctx, hq_kv* kv) {
+    if (!kv) return;
+    if (!ctx) ctx = kv->ctx;
+    ctx_free(ctx, kv->rem); ctx_free(ctx, kv->una); ctx_free(ctx, kv->ulen); ctx_free(ctx, kv->norm);
+    ctx_free(ctx, kv->blk_off); ctx_free(ctx, kv->upos); ctx_free(ctx, kv->ring); ctx_free(ctx, kv->dsign);
+    ctx_free(ctx, kv->ssign); ctx_free(ctx, kv->counters); ctx_free(ctx, kv->scratch_codes); ctx_free(ctx, kv->att_ws);
+    delete kv;
+}
+
+hq_status hq_kv_append(hq_ctx* ctx, hq_kv* kv, const void* k_dev, const void* v_dev, int64_t n_tok, void* stream) {
+    if (!ctx) return HQ_ERR_INVALID_ARG;
+    if (!kv || !k_dev || !v_dev) return fail(ctx, HQ_ERR_INVALID_ARG, "null argument");
+    if (n_tok <= 0 || kv->n_tokens + n_tok > kv->cfg.max_tokens) return fail(ctx, HQ_ERR_SHAPE, "n_tok out of range");
+    cudaStream_t st = (cudaStream_t)stream;
+    int H = kv->cfg.kv_heads, d = kv->cfg.head_dim;
+    const int64_t CHUNK = 4096;
+    int64_t chunk = n_tok < CHUNK ? n_tok : CHUNK;
+    if (chunk > kv->scratch_tokens) {
+        if (kv->scratch_codes) { HQ_CUDA_CHECK(ctx, cudaDeviceSynchronize()); ctx_free(ctx, kv->scratch_codes); kv->scratch_codes = nullptr; }
+        int64_t cap = chunk < 64 ? 64 : chunk;
+        kv->scratch_codes = (int8_t*)ctx_alloc(ctx, (size_t)2 * cap * H * (d + 4));
+        if (!kv->scratch_codes) { kv->scratch_tokens = 0; return HQ_ERR_ALLOC; }
+        kv->scratch_tokens = cap;
+    }
+    int* err_flag = (int*)(kv->counters + 1);
+    for (int64_t c0 = 0; c0 < n_tok; c0 += chunk) {
+        int64_t nt = n_tok - c0 < chunk ? n_tok - c0 : chunk;
+        int64_t token0 = kv->n_tokens + c0;
+        for (int role = 0; role < 2; ++role) {
+            const __nv_bfloat16* src = (const __nv_bfloat16*)(role ? v_dev : k_dev) + c0 * H * d;
+            int8_t* codes = kv->scratch_codes + (size_t)role * kv->scratch_tokens * H * (d + 4);
+            uint16_t* norm_r = kv->norm + (int64_t)role * H * kv->cfg.max_tokens;
+            launch_quantize_kv(src, nt, H, d, token0, role, kv->cfg.codec.lattice, kv->A, kv->cfg.rotation,
+                               kv->cfg.dither, kv->cfg.codec.seed, kv->dsign, kv->ssign, codes, norm_r,
+                               kv->cfg.max_tokens, kv->counters, st);
+            launch_kv_pack(codes, nt, H, d, token0, role, kv->cfg.codec.lattice, kv->k0, kv->k1, kv->rbits,
+                           kv->cfg.max_tokens, kv->rem_words, kv->una_words, kv->n_blk, kv->rem, kv->una, kv->ulen,
+                           kv->blk_off, kv->upos, err_flag, st);
+        }
+    }
+    launch_kv_ring(k_dev, v_dev, n_tok, H, d, kv->n_tokens, kv->cfg.window, kv->ring, st);
+    HQ_CUDA_CHECK(ctx, cudaGetLastError());
+    kv->n_tokens += n_tok;
+    return HQ_OK;
+}
+
+hq_status hq_attend(hq_ctx* ctx, const hq_kv* kv, const void* q_dev, int32_t q_heads, void* out_bf16_dev,
+                    float* out_f32_dev_or_null, void* stream) {
+    if (!ctx) return HQ_ERR_INVALID_ARG;
+    if (!kv || !q_dev || (!out_bf16_dev && !out_f32_dev_or_null)) return fail(ctx, HQ_ERR_INVALID_ARG, "null argument");
+    if (q_heads <= 0 || q_heads % kv->cfg.kv_heads != 0 || q_heads / kv->cfg.kv_heads > 8 || q_heads > 64)
+        return fail(ctx, HQ_ERR_SHAPE, "q_heads must be a multiple of kv_heads, group size <= 8, q_heads <= 64");
+    if (kv->n_tokens <= 0) return fail(ctx, HQ_ERR_SHAPE, "empty cache");
+    return launch_attend(ctx, kv, q_dev, q_heads, out_bf16_dev, out_f32_dev_or_null, (cudaStream_t)stream);
+}
+
+hq_status hq_kv_export(hq_ctx* ctx, const hq_kv* kv, hq_kv_view* out) {
+    if (!ctx) return HQ_ERR_INVALID_ARG;
+    if (!kv || !out) return fail(ctx, HQ_ERR_INVALID_ARG, "null argument");
+    HQ_CUDA_CHECK(ctx, cudaDeviceSynchronize());
+    unsigned long long hc[8];
+    HQ_CUDA_CHECK(ctx, cudaMemcpy(hc, kv->counters, sizeof(hc), cudaMemcpyDeviceToHost));
+    if (*(int*)(hc + 1) == 1) return fail(ctx, HQ_ERR_FORMAT, "a vector's U-section exceeds 65535 bits (FORMAT §4)");
+    if (*(int*)(hc + 1) == 2) return fail(ctx, HQ_ERR_FORMAT, "U-stream capacity exceeded");
+    out->n_tokens = kv->n_tokens; out->rbits = kv->rbits;
+    out->rem_dev = kv->rem; out->una_dev = kv->una; out->ulen_dev = kv->ulen; out->norm_dev = kv->norm;
+    out->blk_off_dev = kv->blk_off; out->upos_dev = kv->upos;
+    out->rem_words = kv->rem_words; out->una_words = kv->una_words;
+    out->clamp_count = (int64_t)hc[0];
+    return HQ_OK;
+}
+
+hq_status hq_kv_decode_int8(hq_ctx* ctx, const hq_kv* kv, int32_t role, int64_t t0, int64_t n, int8_t* codes_dev,
+                            void* stream) {
+    if (!ctx) return HQ_ERR_INVALID_ARG;
+    if (!kv || !codes_dev || role < 0 || role > 1) return fail(ctx, HQ_ERR_INVALID_ARG, "bad argument");
+    if (t0 < 0 || n <= 0 || t0 + n > kv->n_tokens) return fail(ctx, HQ_ERR_SHAPE, "token range out of bounds");
+    launch_kv_decode_int8(kv, role, t0, n, codes_dev, (cudaStream_t)stream);
+    HQ_CUDA_CHECK(ctx, cudaGetLastError());
+    return HQ_OK;
+}
+
+}  // extern "C"

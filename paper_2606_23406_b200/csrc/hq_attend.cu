@@ -1,0 +1,370 @@
+// hq_attend.cu — attention over the compressed KV cache (§5.2,
+// L178).  Scores and the P·V sum are taken in the CODE domain: RHT and S are orthogonal, so
+//   <q, k̂> = (rho/(alpha sqrt n)) <S RHT q, c - U>                         (Prop. 1)
+// and the V accumulation is un-rotated once at the end.  Tokens of the residual window are read
+// exactly from the bf16 ring (§6.7.2).
+#include "hq_common.cuh"
+#include "hq_internal.h"
+
+namespace hq {
+
+// U-section start of token t of (role, head): blk_off + sum of the block's earlier ulen (FORMAT §6)
+__device__ inline uint32_t kv_ustart_serial(const uint16_t* ulen_h, const uint32_t* blk_h, int64_t t) {
+    int64_t t0 = t & ~(int64_t)127;
+    uint32_t s = blk_h[t >> 7];
+    for (int64_t i = t0; i < t; ++i) s += ulen_h[i];
+    return s;
+}
+
+template <int LAT>
+__global__ void k_kv_decode_int8(const uint32_t* rem, const uint32_t* una, const uint16_t* ulen,
+                                 const uint32_t* blk_off, int H, int d, int k0, int k1, int rbits,
+                                 int64_t max_tokens, int64_t rem_words, int64_t una_words, int64_t n_blk,
+                                 int64_t t0, int64_t n, int8_t* codes) {
+    int64_t idx = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (idx >= n * H) return;
+    int64_t t = t0 + idx / H;
+    int h = (int)(idx % H);
+    uint32_t us = kv_ustart_serial(ulen + h * max_tokens, blk_off + h * (n_blk + 1), t);
+    int8_t* out = codes + idx * d;
+    decode_row_generic<LAT>(rem + h * rem_words, (uint32_t)(t * rbits), una + h * una_words, us, d, k0, k1,
+                            [&](int b, const int* c) {
+#pragma unroll
+                                for (int e = 0; e < LAT; ++e) out[b * LAT + e] = (int8_t)c[e];
+                            });
+}
+
+void launch_kv_decode_int8(const hq_kv* kv, int role, int64_t t0, int64_t n, int8_t* codes, cudaStream_t st) {
+    int H = kv->cfg.kv_heads, d = kv->cfg.head_dim;
+    int64_t mt = kv->cfg.max_tokens;
+    const uint32_t* rem = kv->rem + (int64_t)role * H * kv->rem_words;
+    const uint32_t* una = kv->una + (int64_t)role * H * kv->una_words;
+    const uint16_t* ulen = kv->ulen + (int64_t)role * H * mt;
+    const uint32_t* blk = kv->blk_off + (int64_t)role * H * (kv->n_blk + 1);
+    unsigned blocks = (unsigned)((n * H + 63) / 64);
+#define HQ_KD(L)                                                                                                  \
+    k_kv_decode_int8<L><<<blocks, 64, 0, st>>>(rem, una, ulen, blk, H, d, kv->k0, kv->k1, kv->rbits, mt,          \
+                                               kv->rem_words, kv->una_words, kv->n_blk, t0, n, codes)
+    switch (kv->cfg.codec.lattice) {
+        case LAT_Z: HQ_KD(LAT_Z); break;
+        case LAT_A2: HQ_KD(LAT_A2); break;
+        case LAT_D4: HQ_KD(LAT_D4); break;
+        default: HQ_KD(LAT_E8); break;
+    }
+#undef HQ_KD
+}
+
+// ---------------------------------------------------------------------------------------------
+// Split attention over the bitstream part.  CTA = (kv head h, split s), 128 threads.
+// Per block of 128 tokens (thread = token):
+//   K: decode the token's code vector block by block, regenerate the dither, dot with q'_g (G query
+//      heads of this kv head) -> score; block max / exp -> p_g[t] in smem.
+//   V: decode, write v' = (rho/A)(c - U) to smem [token][d]; then thread j (= coordinate) sums
+//      p_g[t] v'[t][j] over the block into its running accumulators (online softmax rescale).
+// Output per (h, split): m_g, l_g, acc_g[d] in the code domain.
+// ---------------------------------------------------------------------------------------------
+constexpr int ATT_MAXG = 8;
+
+struct AttendParams {
+    const uint32_t *rem, *una, *blk_off;
+    const uint16_t *ulen, *norm;
+    int H, d, k0, k1, rbits, G, dither, rotation;
+    int64_t max_tokens, rem_words, una_words, n_blk;
+    int64_t Tc;      // tokens served from the bitstream: [0, Tc)
+    int n_split;
+    float inv_A, inv_sqrt_d;
+    uint64_t seed;
+    const __nv_bfloat16* q;  // [q_heads, d]
+    const int8_t *dsign, *ssign;
+    float* ws;               // [H][n_split][G][d + 2]
+};
+
+// q' = S * RHT(q) for one head, in smem (fp32), by one warp (FORMAT R1 order; any order would do here)
+__device__ inline void warp_query_transform(float* s, int d, const int8_t* dsign, const int8_t* ssign, int rotation,
+                                            int lane) {
+    for (int i = lane; i < d; i += 32)
+        if (dsign[i] < 0) s[i] = -s[i];
+    for (int h = 1; h < d; h <<= 1) {
+        __syncwarp();
+        for (int p = lane; p < d / 2; p += 32) {
+            int i = ((p / h) * 2 * h) + (p % h);
+            float a = s[i], b = s[i + h];
+            s[i] = a + b;
+            s[i + h] = a - b;
+        }
+    }
+    __syncwarp();
+    float cn = rsqrtf((float)d);
+    for (int i = lane; i < d; i += 32) {
+        float v = s[i] * cn;
+        s[i] = (rotation == HQ_ROT_SIGNS && ssign[i] < 0) ? -v : v;
+    }
+    __syncwarp();
+}
+
+template <int LAT>
+__global__ void __launch_bounds__(128)
+k_attend_split(AttendParams p) {
+    extern __shared__ float sm[];
+    const int d = p.d, G = p.G;
+    float* qs = sm;                    // [G][d]
+    float* vt = qs + G * d;            // [128][d+1]
+    float* ps = vt + 128 * (d + 1);    // [G][128]
+    float* red = ps + G * 128;         // [G][4] block reductions
+    __shared__ uint32_t scan[4];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int h = blockIdx.x / p.n_split, split = blockIdx.x % p.n_split;
+
+    for (int i = tid; i < G * d; i += 128) qs[i] = __bfloat162float(p.q[(h * G) * d + i]);
+    __syncthreads();
+    for (int g = warp; g < G; g += 4) warp_query_transform(qs + g * d, d, p.dsign, p.ssign, p.rotation, lane);
+    __syncthreads();
+
+    const int64_t nblk_total = (p.Tc + 127) / 128;
+    const int64_t per = (nblk_total + p.n_split - 1) / p.n_split;
+    const int64_t blk0 = split * per, blk1 = min(nblk_total, blk0 + per);
+
+    float m_run[ATT_MAXG], l_run[ATT_MAXG], acc[ATT_MAXG];  // thread j owns coordinate(s) j (d <= 128 -> one)
+#pragma unroll
+    for (int g = 0; g < ATT_MAXG; ++g) { m_run[g] = -INFINITY; l_run[g] = 0.0f; acc[g] = 0.0f; }
+    float acc2[ATT_MAXG];  // second coordinate when d == 256
+#pragma unroll
+    for (int g = 0; g < ATT_MAXG; ++g) acc2[g] = 0.0f;
+
+    for (int64_t blk = blk0; blk < blk1; ++blk) {
+        const int64_t t = blk * 128 + tid;
+        const bool valid = t < p.Tc;
+        float pg[ATT_MAXG];
+        for (int role = 0; role < 2; ++role) {
+            const uint32_t* rem = p.rem + ((int64_t)role * p.H + h) * p.rem_words;
+            const uint32_t* una = p.una + ((int64_t)role * p.H + h) * p.una_words;
+            const uint16_t* ulen = p.ulen + ((int64_t)role * p.H + h) * p.max_tokens;
+            const uint16_t* norm = p.norm + ((int64_t)role * p.H + h) * p.max_tokens;
+            const uint32_t* blkoff = p.blk_off + ((int64_t)role * p.H + h) * (p.n_blk + 1);
+            // every token of the block has been appended (t < T), those >= Tc are simply masked
+            uint32_t ul = (blk * 128 + tid < p.max_tokens) ? ulen[blk * 128 + tid] : 0;
+            uint32_t us = blkoff[blk] + row_ustart_128(ul, scan, tid);
+            float scale = valid ? f16_bits_to_f32(norm[t]) * p.inv_A : 0.0f;
+            if (role == 0) {
+                float dot[ATT_MAXG];
+#pragma unroll
+                for (int g = 0; g < ATT_MAXG; ++g) dot[g] = 0.0f;
+                if (valid) {
+                    decode_row_generic<LAT>(rem, (uint32_t)(t * p.rbits), una, us, d, p.k0, p.k1,
+                                            [&](int b, const int* c) {
+                                                float U[LAT];
+                                                if (p.dither) dither_block<LAT>(p.seed, (uint32_t)b, (uint32_t)t, (uint32_t)h, 0u, U);
+#pragma unroll
+                                                for (int e = 0; e < LAT; ++e) {
+                                                    float v = (float)c[e];
+                                                    if (LAT == LAT_A2 && e == 0) v *= HQ_S3;
+                                                    if (p.dither) v -= U[e];
+#pragma unroll
+                                                    for (int g = 0; g < ATT_MAXG; ++g)
+                                                        if (g < G) dot[g] += qs[g * d + b * LAT + e] * v;
+                                                }
+                                            });
+                }
+                // scores, block max, p
+#pragma unroll
+                for (int g = 0; g < ATT_MAXG; ++g) {
+                    if (g >= G) break;
+                    float s = valid ? dot[g] * scale * p.inv_sqrt_d : -INFINITY;
+                    float mx = s;
+                    for (int o = 16; o; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+                    if (lane == 0) red[g * 4 + warp] = mx;
+                    pg[g] = s;
+                }
+                __syncthreads();
+#pragma unroll
+                for (int g = 0; g < ATT_MAXG; ++g) {
+                    if (g >= G) break;
+                    float mb = fmaxf(fmaxf(red[g * 4], red[g * 4 + 1]), fmaxf(red[g * 4 + 2], red[g * 4 + 3]));
+                    float m_new = fmaxf(m_run[g], mb);
+                    float corr = (m_run[g] == -INFINITY) ? 0.0f : __expf(m_run[g] - m_new);
+                    float pe = valid ? __expf(pg[g] - m_new) : 0.0f;
+                    ps[g * 128 + tid] = pe;
+                    // every thread keeps the same running stats; l gets the block sum below
+                    acc[g] *= corr; acc2[g] *= corr; l_run[g] *= corr; m_run[g] = m_new;
+                }
+                __syncthreads();
+            } else {
+                // V: write v' rows to smem
+                float* row = vt + tid * (d + 1);
+                if (valid) {
+                    decode_row_generic<LAT>(rem, (uint32_t)(t * p.rbits), una, us, d, p.k0, p.k1,
+                                            [&](int b, const int* c) {
+                                                float U[LAT];
+                                                if (p.dither) dither_block<LAT>(p.seed, (uint32_t)b, (uint32_t)t, (uint32_t)h, 1u, U);
+#pragma unroll
+                                                for (int e = 0; e < LAT; ++e) {
+                                                    float v = (float)c[e];
+                                                    if (LAT == LAT_A2 && e == 0) v *= HQ_S3;
+                                                    if (p.dither) v -= U[e];
+                                                    row[b * LAT + e] = v * scale;
+                                                }
+                                            });
+                } else {
+                    for (int j = 0; j < d; ++j) row[j] = 0.0f;
+                }
+                __syncthreads();
+                for (int j = tid, jj = 0; j < d; j += 128, ++jj) {
+#pragma unroll
+                    for (int g = 0; g < ATT_MAXG; ++g) {
+                        if (g >= G) break;
+                        float a = 0.0f, lsum = 0.0f;
+                        for (int tt = 0; tt < 128; ++tt) {
+                            float pe = ps[g * 128 + tt];
+                            a += pe * vt[tt * (d + 1) + j];
+                            lsum += pe;
+                        }
+                        if (jj == 0) { acc[g] += a; l_run[g] += lsum; } else acc2[g] += a;
+                    }
+                }
+                __syncthreads();
+            }
+        }
+    }
+    // write partials: [h][split][g][d + 2] = acc..., m, l   (threads with tid < d hold valid m/l)
+    float* out = p.ws + ((int64_t)(h * p.n_split + split) * G) * (d + 2);
+    for (int g = 0; g < G; ++g) {
+        if (tid < d) out[g * (d + 2) + tid] = acc[g];
+        if (d > 128) out[g * (d + 2) + tid + 128] = acc2[g];
+        if (tid == 0) { out[g * (d + 2) + d] = m_run[g]; out[g * (d + 2) + d + 1] = l_run[g]; }
+    }
+}
+
+// Combine the splits, add the exact window tokens, un-rotate: one block per query head, d threads.
+__global__ void k_attend_combine(AttendParams p, const __nv_bfloat16* ring, int window, int64_t T,
+                                 __nv_bfloat16* out_bf16, float* out_f32) {
+    extern __shared__ float sm[];
+    const int d = p.d, G = p.G;
+    float* code = sm;        // [d] code-domain accumulator
+    float* sc = code + d;    // [window] window scores
+    float* qf = sc + (window > 0 ? window : 1);  // [d]
+    __shared__ float s_m, s_l;
+    const int qh = blockIdx.x, h = qh / G, g = qh % G, j = threadIdx.x;
+    // global max over splits
+    float m = -INFINITY;
+    for (int s = 0; s < p.n_split; ++s) {
+        const float* w = p.ws + ((int64_t)(h * p.n_split + s) * G + g) * (d + 2);
+        if (w[d + 1] > 0.0f) m = fmaxf(m, w[d]);
+    }
+    // window scores (original domain, exact bf16 K)
+    qf[j] = __bfloat162float(p.q[qh * d + j]);
+    __syncthreads();
+    const int64_t w0 = p.Tc;
+    const int nw = (int)(T - w0);
+    if (j < nw) {
+        int64_t t = w0 + j;
+        const __nv_bfloat16* kr = ring + ((int64_t)(0 * window + (t % window)) * p.H + h) * d;
+        float dot = 0.0f;
+        for (int i = 0; i < d; ++i) dot += qf[i] * __bfloat162float(kr[i]);
+        sc[j] = dot * p.inv_sqrt_d;
+    }
+    __syncthreads();
+    if (j == 0) {
+        float mm = m;
+        for (int i = 0; i < nw; ++i) mm = fmaxf(mm, sc[i]);
+        s_m = mm;
+    }
+    __syncthreads();
+    m = s_m;
+    float a = 0.0f, l = 0.0f;
+    for (int s = 0; s < p.n_split; ++s) {
+        const float* w = p.ws + ((int64_t)(h * p.n_split + s) * G + g) * (d + 2);
+        if (w[d + 1] > 0.0f) {
+            float f = __expf(w[d] - m);
+            a += f * w[j];
+            l += f * w[d + 1];
+        }
+    }
+    // un-rotate the code-domain sum: x = D H (S u) / sqrt(d)
+    code[j] = (p.rotation == HQ_ROT_SIGNS && p.ssign[j] < 0) ? -a : a;
+    __syncthreads();
+    for (int hh = 1; hh < d; hh <<= 1) {
+        float x = 0.0f, y = 0.0f;
+        int i = 0;
+        if (j < d / 2) {
+            i = ((j / hh) * 2 * hh) + (j % hh);
+            x = code[i];
+            y = code[i + hh];
+        }
+        __syncthreads();
+        if (j < d / 2) {
+            code[i] = x + y;
+            code[i + hh] = x - y;
+        }
+        __syncthreads();
+    }
+    float o = code[j] * rsqrtf((float)d) * (p.dsign[j] < 0 ? -1.0f : 1.0f);
+    // window tokens: exact V
+    for (int i = 0; i < nw; ++i) {
+        int64_t t = w0 + i;
+        float pe = __expf(sc[i] - m);
+        const __nv_bfloat16* vr = ring + ((int64_t)(1 * window + (t % window)) * p.H + h) * d;
+        o += pe * __bfloat162float(vr[j]);
+        l += pe;
+    }
+    if (j == 0) s_l = l;
+    __syncthreads();
+    o /= s_l;
+    if (out_bf16) out_bf16[qh * d + j] = __float2bfloat16_rn(o);
+    if (out_f32) out_f32[qh * d + j] = o;
+}
+
+static int attend_n_split(const hq_ctx* ctx, const hq_kv* kv) {
+    int64_t window = kv->cfg.window;
+    int64_t Tc = kv->n_tokens > window ? kv->n_tokens - window : 0;
+    int64_t nblk = (Tc + 127) / 128;
+    int64_t want = (ctx->sm_count * 4) / kv->cfg.kv_heads;
+    if (want < 1) want = 1;
+    int64_t ns = nblk < want ? nblk : want;
+    return (int)(ns < 1 ? 1 : ns);
+}
+
+size_t attend_workspace_bytes(const hq_kv* kv, int q_heads) {
+    // sized for the worst case split count (4 CTAs per SM)
+    return (size_t)(148 * 8) * (size_t)q_heads * (kv->cfg.head_dim + 2) * sizeof(float);
+}
+
+hq_status launch_attend(hq_ctx* ctx, const hq_kv* kv, const void* q, int q_heads, void* out_bf16, float* out_f32,
+                        cudaStream_t st) {
+    AttendParams p;
+    int H = kv->cfg.kv_heads, d = kv->cfg.head_dim;
+    p.rem = kv->rem; p.una = kv->una; p.blk_off = kv->blk_off; p.ulen = kv->ulen; p.norm = kv->norm;
+    p.H = H; p.d = d; p.k0 = kv->k0; p.k1 = kv->k1; p.rbits = kv->rbits; p.G = q_heads / H;
+    p.dither = kv->cfg.dither; p.rotation = kv->cfg.rotation;
+    p.max_tokens = kv->cfg.max_tokens; p.rem_words = kv->rem_words; p.una_words = kv->una_words; p.n_blk = kv->n_blk;
+    int64_t window = kv->cfg.window;
+    p.Tc = kv->n_tokens > window ? kv->n_tokens - window : 0;
+    p.n_split = attend_n_split(ctx, kv);
+    p.inv_A = (float)(1.0 / (kv->alpha * sqrt((double)d)));
+    p.inv_sqrt_d = (float)(1.0 / sqrt((double)d));
+    p.seed = kv->cfg.codec.seed;
+    p.q = (const __nv_bfloat16*)q; p.dsign = kv->dsign; p.ssign = kv->ssign; p.ws = kv->att_ws;
+    size_t smem = ((size_t)p.G * d + 128 * (size_t)(d + 1) + (size_t)p.G * 128 + (size_t)p.G * 4) * sizeof(float);
+#define HQ_AT(L)                                                                                                   \
+    do {                                                                                                           \
+        HQ_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_attend_split<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+        k_attend_split<L><<<H * p.n_split, 128, smem, st>>>(p);                                                    \
+    } while (0)
+    if (p.Tc > 0) {
+        switch (kv->cfg.codec.lattice) {
+            case LAT_Z: HQ_AT(LAT_Z); break;
+            case LAT_A2: HQ_AT(LAT_A2); break;
+            case LAT_D4: HQ_AT(LAT_D4); break;
+            default: HQ_AT(LAT_E8); break;
+        }
+        HQ_CUDA_CHECK(ctx, cudaGetLastError());
+    } else {
+        p.n_split = 0;
+    }
+#undef HQ_AT
+    size_t smem2 = (size_t)(2 * d + (window > 0 ? window : 1)) * sizeof(float);
+    k_attend_combine<<<q_heads, d, smem2, st>>>(p, kv->ring, (int)window, kv->n_tokens, (__nv_bfloat16*)out_bf16, out_f32);
+    HQ_CUDA_CHECK(ctx, cudaGetLastError());
+    return HQ_OK;
+}
+
+}  // namespace hq

@@ -1,0 +1,641 @@
+// hq_encode.cu — the encode half of HyperQuant's hot path:
+//   RHT (§3.1 eq.(1), §4.1) -> rotate (§4.2, KV) -> l2-normalize (§4.3) ->
+//   subtractive dither (§4.4, KV) -> nearest lattice point (§4.5) -> strip + zig-zag
+//   (§4.6) -> Rice code (§3.3, §4.7) into the FORMAT §5/§6 containers,
+//   and the activation path RHT -> amax INT8 cast (FORMAT R7).
+// All float arithmetic that decides an integer uses __f*_rn intrinsics (no FMA contraction) in
+// the fixed operation order of docs/FORMAT.md §2.
+#include "hq_common.cuh"
+#include "hq_internal.h"
+
+namespace hq {
+
+// ---------------------------------------------------------------------------------------------
+__global__ void k_signs(uint64_t seed, uint32_t stream_id, int64_t n, int8_t* out) {
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i < n) out[i] = sign_bit(seed, stream_id, (uint32_t)i) ? -1 : 1;
+}
+void launch_signs(uint64_t seed, uint32_t stream_id, int64_t n, int8_t* out, cudaStream_t st) {
+    k_signs<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(seed, stream_id, n, out);
+}
+
+// ---------------------------------------------------------------------------------------------
+// One warp transforms one tile held in shared memory: FORMAT R1 (butterflies, ascending stride).
+// ---------------------------------------------------------------------------------------------
+__device__ inline void warp_rht_inplace(float* s, int n, int lane) {
+    for (int h = 1; h < n; h <<= 1) {
+        __syncwarp();
+        for (int p = lane; p < n / 2; p += 32) {
+            int i = ((p / h) * 2 * h) + (p % h);
+            float a = s[i], b = s[i + h];
+            s[i] = __fadd_rn(a, b);
+            s[i + h] = __fsub_rn(a, b);
+        }
+    }
+    __syncwarp();
+    float cn = (float)(1.0 / sqrt((double)n));
+    for (int i = lane; i < n; i += 32) s[i] = __fmul_rn(s[i], cn);
+    __syncwarp();
+}
+
+// FORMAT R2 tree sum of t[0..n) (destroys t); all lanes return the result.
+__device__ inline float warp_treesum(float* t, int n, int lane) {
+    for (int h = 1; h < n; h <<= 1) {
+        __syncwarp();
+        for (int p = lane; p * 2 * h < n; p += 32) {
+            int i = p * 2 * h;
+            t[i] = __fadd_rn(t[i], t[i + h]);
+        }
+    }
+    __syncwarp();
+    return t[0];
+}
+
+__device__ inline float load_elem(const void* p, int dtype, int64_t idx) {
+    if (dtype == HQ_BF16) return __bfloat162float(((const __nv_bfloat16*)p)[idx]);
+    return ((const float*)p)[idx];
+}
+
+// quantize the normalized tile u[0..n) (smem) into codes; lanes take lattice blocks round-robin.
+// Returns per-lane clamp count; accumulates per-lane auto-k totals into tot[2][8] if tot != nullptr.
+template <int LAT>
+__device__ inline int quantize_blocks(const float* u, int n, float g, bool with_dither, uint64_t seed,
+                                      uint32_t token, uint32_t head, uint32_t role, int8_t* codes, int lane,
+                                      unsigned long long* tot) {
+    int clamps = 0;
+    for (int b = lane; b < n / LAT; b += 32) {
+        float y[LAT];
+        int c[LAT];
+#pragma unroll
+        for (int i = 0; i < LAT; ++i) y[i] = __fmul_rn(u[b * LAT + i], g);
+        if (with_dither) {
+            float U[LAT];
+            dither_block<LAT>(seed, (uint32_t)b, token, head, role, U);
+#pragma unroll
+            for (int i = 0; i < LAT; ++i) y[i] = __fadd_rn(y[i], U[i]);
+        }
+        clamps += clamp_block<LAT>(y);
+        nearest_noclamp<LAT>(y, c);
+#pragma unroll
+        for (int i = 0; i < LAT; ++i) codes[b * LAT + i] = (int8_t)c[i];
+        if (tot) {
+            int z[LAT];
+            strip<LAT>(c, z);
+#pragma unroll
+            for (int i = 0; i < LAT; ++i) {
+                int a = sym_class(LAT, i);
+#pragma unroll
+                for (int kk = 0; kk < 8; ++kk) tot[a * 8 + kk] += (unsigned long long)(kk + 1 + (z[i] >> kk));
+            }
+        }
+    }
+    return clamps;
+}
+
+constexpr int QW_WARPS = 4;
+
+// mode 0: weights (tile = (row, kt));  mode 1: KV (tile = (token, head), rotation, dither)
+template <int LAT, int MODE>
+__global__ void __launch_bounds__(QW_WARPS * 32)
+k_quantize(const void* X, int dtype, int64_t n_tiles, int64_t n_kt, int64_t ld, int n, float A,
+           const int8_t* dsign, const int8_t* ssign, int rotation, int dither, uint64_t seed, int64_t token0,
+           int role, int H, int64_t max_tokens, int8_t* codes, uint16_t* norms, unsigned long long* counters,
+           int want_totals) {
+    extern __shared__ float smem[];
+    int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    float* u = smem + warp * 2 * n;
+    float* t = u + n;
+    unsigned long long tot[16];
+    if (want_totals)
+        for (int i = 0; i < 16; ++i) tot[i] = 0;
+    unsigned long long clamps = 0;
+    for (int64_t tile = blockIdx.x * (int64_t)QW_WARPS + warp; tile < n_tiles; tile += (int64_t)gridDim.x * QW_WARPS) {
+        int64_t row = tile / n_kt, kt = tile % n_kt;  // KV: row = token, kt = head, n_kt = H
+        int64_t src = (MODE == 0) ? row * ld + kt * n : tile * (int64_t)n;
+        int64_t sgn0 = (MODE == 0) ? kt * n : 0;
+        for (int i = lane; i < n; i += 32) {
+            float x = load_elem(X, dtype, src + i);
+            u[i] = (dsign[sgn0 + i] < 0) ? -x : x;
+        }
+        warp_rht_inplace(u, n, lane);
+        if (MODE == 1 && rotation == HQ_ROT_SIGNS)
+            for (int i = lane; i < n; i += 32)
+                if (ssign[i] < 0) u[i] = -u[i];
+        for (int i = lane; i < n; i += 32) t[i] = __fmul_rn(u[i], u[i]);
+        float ss = warp_treesum(t, n, lane);
+        float rho32 = __fsqrt_rn(ss);
+        uint16_t hb = f32_to_f16_bits_sat(rho32);
+        float rho = f16_bits_to_f32(hb);
+        int8_t* out = codes + tile * (int64_t)n;
+        if (MODE == 0) out = codes + row * (n_kt * n) + kt * n;
+        if (lane == 0) {
+            if (MODE == 0) norms[row * n_kt + kt] = hb;
+            else norms[kt * max_tokens + token0 + row] = hb;
+        }
+        if (rho == 0.0f) {  // G18
+            for (int i = lane; i < n; i += 32) out[i] = 0;
+            if (want_totals && lane == 0)  // n zero symbols: k+1 bits each
+                for (int j = 0; j < n; ++j)
+                    for (int kk = 0; kk < 8; ++kk) tot[sym_class(LAT, j % LAT) * 8 + kk] += kk + 1;
+        } else {
+            float g = __fdiv_rn(A, rho);
+            clamps += quantize_blocks<LAT>(u, n, g, MODE == 1 && dither, seed, (uint32_t)(token0 + row),
+                                           (uint32_t)kt, (uint32_t)role, out, lane, want_totals ? tot : nullptr);
+        }
+        __syncwarp();
+    }
+    // reduce counters over the warp, one atomic per warp per counter
+    for (int o = 16; o; o >>= 1) clamps += __shfl_xor_sync(0xffffffffu, clamps, o);
+    if (lane == 0 && clamps) atomicAdd(&counters[0], clamps);
+    if (want_totals) {
+        for (int i = 0; i < 16; ++i) {
+            unsigned long long v = tot[i];
+            for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+            if (lane == 0 && v) atomicAdd(&counters[1 + i], v);
+        }
+    }
+}
+
+template <int MODE>
+static void launch_quantize_any(int lattice, dim3 grid, size_t smem, cudaStream_t st, const void* X, int dtype,
+                                int64_t n_tiles, int64_t n_kt, int64_t ld, int n, float A, const int8_t* dsign,
+                                const int8_t* ssign, int rotation, int dither, uint64_t seed, int64_t token0,
+                                int role, int H, int64_t max_tokens, int8_t* codes, uint16_t* norms,
+                                unsigned long long* counters, int want_totals) {
+#define HQ_LAUNCH_Q(L)                                                                                        \
+    k_quantize<L, MODE><<<grid, QW_WARPS * 32, smem, st>>>(X, dtype, n_tiles, n_kt, ld, n, A, dsign, ssign,   \
+                                                           rotation, dither, seed, token0, role, H,           \
+                                                           max_tokens, codes, norms, counters, want_totals)
+    switch (lattice) {
+        case LAT_Z: HQ_LAUNCH_Q(LAT_Z); break;
+        case LAT_A2: HQ_LAUNCH_Q(LAT_A2); break;
+        case LAT_D4: HQ_LAUNCH_Q(LAT_D4); break;
+        default: HQ_LAUNCH_Q(LAT_E8); break;
+    }
+#undef HQ_LAUNCH_Q
+}
+
+void launch_quantize_weights(const void* W, int dtype, int64_t m, int64_t n_in, int64_t ld, int lattice, int n,
+                             float A, const int8_t* dsign, int8_t* codes, uint16_t* norms,
+                             unsigned long long* counters, cudaStream_t st) {
+    int64_t n_kt = n_in / n, n_tiles = m * n_kt;
+    int64_t blocks = (n_tiles + QW_WARPS - 1) / QW_WARPS;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    launch_quantize_any<0>(lattice, dim3((unsigned)blocks), QW_WARPS * 2 * n * sizeof(float), st, W, dtype, n_tiles,
+                           n_kt, ld, n, A, dsign, nullptr, 0, 0, 0, 0, 0, 0, 0, codes, norms, counters, 1);
+}
+
+void launch_quantize_kv(const void* x, int64_t n_tok, int H, int d, int64_t token0, int role, int lattice,
+                        float A, int rotation, int dither, uint64_t seed, const int8_t* dsign,
+                        const int8_t* ssign, int8_t* codes, uint16_t* norm_out, int64_t max_tokens,
+                        unsigned long long* counters, cudaStream_t st) {
+    int64_t n_tiles = n_tok * H;
+    int64_t blocks = (n_tiles + QW_WARPS - 1) / QW_WARPS;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    launch_quantize_any<1>(lattice, dim3((unsigned)blocks), QW_WARPS * 2 * d * sizeof(float), st, x, HQ_BF16,
+                           n_tiles, H, 0, d, A, dsign, ssign, rotation, dither, seed, token0, role, H, max_tokens,
+                           codes, norm_out, counters, 0);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Activations (FORMAT R7): RHT, amax, INT8 cast.  One warp per (row, tile).
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(QW_WARPS * 32)
+k_act_quant(const void* X, int dtype, int64_t n_tiles, int64_t n_kt, int64_t ldx, int lattice, int n,
+            const int8_t* dsign, int8_t* q, float* s_x, float* u_out) {
+    extern __shared__ float smem[];
+    int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    float* u = smem + warp * n;
+    for (int64_t tile = blockIdx.x * (int64_t)QW_WARPS + warp; tile < n_tiles; tile += (int64_t)gridDim.x * QW_WARPS) {
+        int64_t b = tile / n_kt, kt = tile % n_kt;
+        for (int i = lane; i < n; i += 32) {
+            float x = load_elem(X, dtype, b * ldx + kt * n + i);
+            u[i] = (dsign[kt * n + i] < 0) ? -x : x;
+        }
+        warp_rht_inplace(u, n, lane);
+        int64_t o = b * (n_kt * n) + kt * n;
+        if (u_out)
+            for (int i = lane; i < n; i += 32) u_out[o + i] = u[i];
+        float amax = 0.0f;
+        for (int i = lane; i < n; i += 32) {
+            float v = u[i];
+            if (lattice == LAT_A2 && (i & 1) == 0) { v = __fmul_rn(v, HQ_S3); u[i] = v; }
+            amax = fmaxf(amax, fabsf(v));
+        }
+        for (int s = 16; s; s >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, s));
+        __syncwarp();
+        if (amax == 0.0f) {
+            for (int i = lane; i < n; i += 32) q[o + i] = 0;
+            if (lane == 0) s_x[b * n_kt + kt] = 0.0f;
+        } else {
+            float inv = __fdiv_rn(127.0f, amax);
+            for (int i = lane; i < n; i += 32) {
+                float v = rintf(__fmul_rn(u[i], inv));
+                v = fminf(fmaxf(v, -127.0f), 127.0f);
+                q[o + i] = (int8_t)(int)v;
+            }
+            if (lane == 0) s_x[b * n_kt + kt] = __fdiv_rn(amax, 127.0f);
+        }
+        __syncwarp();
+    }
+}
+
+void launch_act_quant(const void* x, int dtype, int64_t B, int64_t n_in, int64_t ldx, int lattice, int n,
+                      const int8_t* dsign, int8_t* q, float* s_x, float* u, cudaStream_t st) {
+    int64_t n_kt = n_in / n, n_tiles = B * n_kt;
+    int64_t blocks = (n_tiles + QW_WARPS - 1) / QW_WARPS;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    k_act_quant<<<(unsigned)blocks, QW_WARPS * 32, QW_WARPS * n * sizeof(float), st>>>(x, dtype, n_tiles, n_kt, ldx,
+                                                                                      lattice, n, dsign, q, s_x, u);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Tile lengths: thread per tile; symbols from the codes, ulen = n + sum q_j (FORMAT §4).
+// ---------------------------------------------------------------------------------------------
+template <int LAT>
+__device__ inline uint32_t tile_ulen(const int8_t* codes, int n, int k0, int k1) {
+    uint32_t L = (uint32_t)n;
+    for (int b = 0; b < n / LAT; ++b) {
+        int c[LAT], z[LAT];
+#pragma unroll
+        for (int i = 0; i < LAT; ++i) c[i] = codes[b * LAT + i];
+        strip<LAT>(c, z);
+#pragma unroll
+        for (int i = 0; i < LAT; ++i) L += (uint32_t)(z[i] >> (sym_class(LAT, i) ? k1 : k0));
+    }
+    return L;
+}
+
+template <int LAT>
+__global__ void k_tile_ulen(const int8_t* codes, int64_t m, int64_t n_kt, int n, int k0, int k1, int64_t G,
+                            uint16_t* ulen_tmp, int* err_flag) {
+    int64_t idx = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;  // g*128 + i
+    if (idx >= G * 128) return;
+    int64_t g = idx >> 7;
+    int i = (int)(idx & 127);
+    int64_t rb = g / n_kt, kt = g % n_kt, r = rb * 128 + i;
+    uint32_t L = 0;
+    if (r < m) {
+        L = tile_ulen<LAT>(codes + r * (n_kt * n) + kt * n, n, k0, k1);
+        if (L > 65535u) { atomicExch(err_flag, 1); L = 65535u; }
+    }
+    ulen_tmp[idx] = (uint16_t)L;
+}
+
+void launch_tile_ulen(const int8_t* codes, int64_t m, int64_t n_in, int lattice, int n, int k0, int k1,
+                      uint16_t* ulen_tmp, int* err_flag, cudaStream_t st) {
+    int64_t n_kt = n_in / n, n_rb = (m + 127) / 128, G = n_rb * n_kt;
+    unsigned blocks = (unsigned)((G * 128 + 127) / 128);
+    switch (lattice) {
+        case LAT_Z: k_tile_ulen<LAT_Z><<<blocks, 128, 0, st>>>(codes, m, n_kt, n, k0, k1, G, ulen_tmp, err_flag); break;
+        case LAT_A2: k_tile_ulen<LAT_A2><<<blocks, 128, 0, st>>>(codes, m, n_kt, n, k0, k1, G, ulen_tmp, err_flag); break;
+        case LAT_D4: k_tile_ulen<LAT_D4><<<blocks, 128, 0, st>>>(codes, m, n_kt, n, k0, k1, G, ulen_tmp, err_flag); break;
+        default: k_tile_ulen<LAT_E8><<<blocks, 128, 0, st>>>(codes, m, n_kt, n, k0, k1, G, ulen_tmp, err_flag); break;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Group offsets: device prefix sum over the groups' sizes (north_star (a); FORMAT §5).
+// One block; each thread sums its groups' 128 ulen, block scan in chunks of 1024 groups.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(1024)
+k_group_offsets(const uint16_t* ulen_tmp, int64_t G, int rbits, uint32_t* group_off, unsigned long long* totals,
+                uint32_t* max_group16) {
+    __shared__ uint32_t warp_sums[32];
+    __shared__ uint32_t carry_s;
+    __shared__ unsigned long long ubits_total;
+    __shared__ uint32_t maxg;
+    int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid == 0) { carry_s = 0; ubits_total = 0; maxg = 0; }
+    __syncthreads();
+    uint32_t r16 = (uint32_t)((128 * (int64_t)rbits + 127) / 128);
+    for (int64_t base = 0; base < G; base += 1024) {
+        int64_t g = base + tid;
+        uint32_t size16 = 0, ub = 0;
+        if (g < G) {
+            const uint4* p = (const uint4*)(ulen_tmp + g * 128);  // 256 bytes
+            for (int v = 0; v < 16; ++v) {
+                uint4 w = p[v];
+                uint32_t ws[4] = {w.x, w.y, w.z, w.w};
+#pragma unroll
+                for (int e = 0; e < 4; ++e) ub += (ws[e] & 0xffffu) + (ws[e] >> 16);
+            }
+            size16 = 32 + r16 + (ub + 127) / 128;
+        }
+        // inclusive scan of size16 over the block
+        uint32_t x = size16;
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t y = __shfl_up_sync(0xffffffffu, x, o);
+            if (lane >= o) x += y;
+        }
+        if (lane == 31) warp_sums[warp] = x;
+        __syncthreads();
+        if (warp == 0) {
+            uint32_t s = warp_sums[lane];
+            for (int o = 1; o < 32; o <<= 1) {
+                uint32_t y = __shfl_up_sync(0xffffffffu, s, o);
+                if (lane >= o) s += y;
+            }
+            warp_sums[lane] = s;
+        }
+        __syncthreads();
+        uint32_t incl = x + (warp ? warp_sums[warp - 1] : 0) + carry_s;
+        if (g < G) {
+            group_off[g] = incl - size16;
+            atomicAdd(&ubits_total, (unsigned long long)ub);
+            atomicMax(&maxg, size16);
+        }
+        __syncthreads();
+        if (tid == 1023) carry_s = incl;
+        __syncthreads();
+    }
+    if (tid == 0) {
+        group_off[G] = carry_s;
+        totals[0] = ubits_total;
+        *max_group16 = maxg;
+    }
+}
+
+void launch_group_offsets(const uint16_t* ulen_tmp, int64_t G, int rbits, uint32_t* group_off,
+                          unsigned long long* totals, uint32_t* max_group16, cudaStream_t st) {
+    k_group_offsets<<<1, 1024, 0, st>>>(ulen_tmp, G, rbits, group_off, totals, max_group16);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Bit packing.  A per-thread writer that assembles 32-bit words of an MSB-first stream and ORs
+// them into a zero-initialized area (neighbouring rows share boundary words -> atomicOr).
+// ---------------------------------------------------------------------------------------------
+struct BitWriter {
+    uint32_t* area;
+    uint32_t pos;   // next stream bit
+    uint32_t cur;   // bits of the current word accumulated so far (already positioned)
+    __device__ BitWriter(uint32_t* a, uint32_t p) : area(a), pos(p), cur(0) {}
+    __device__ inline void flush_word() {
+        if (cur) atomicOr(&area[(pos - 1) >> 5], cur);
+        cur = 0;
+    }
+    // append nb (1..32) bits, value MSB-first
+    __device__ inline void put(uint32_t v, int nb) {
+        int s = pos & 31;
+        int room = 32 - s;
+        if (nb <= room) {
+            cur |= (nb == 32) ? v : (v << (room - nb));
+            pos += nb;
+            if ((pos & 31) == 0) flush_word();
+        } else {
+            cur |= v >> (nb - room);
+            pos += room;
+            flush_word();
+            int rest = nb - room;
+            cur = v << (32 - rest);
+            pos += rest;
+        }
+    }
+    __device__ inline void skip(uint32_t nzeros) {  // append zeros
+        uint32_t np = pos + nzeros;
+        if ((np >> 5) != (pos >> 5)) {
+            if (pos & 31) { pos = (pos | 31) + 1; flush_word(); }
+        }
+        pos = np;
+    }
+    __device__ inline void finish() {
+        if (pos & 31) { if (cur) atomicOr(&area[pos >> 5], cur); cur = 0; }
+    }
+};
+
+// R-section of a tile (FORMAT §4 field planes) from its symbols z[0..n) (smem/local pointer).
+template <int LAT>
+__device__ inline void write_R(BitWriter& bw, const uint8_t* z, int n, int k0, int k1) {
+    const int nclass = (LAT == LAT_D4 || LAT == LAT_A2) ? 2 : 1;
+    for (int a = 0; a < nclass; ++a) {
+        int ka = a ? k1 : k0;
+        if (ka == 0) continue;
+        int na = class_count(LAT, n, a);
+        // j of the m-th symbol of class a
+        auto sym_at = [&](int mi) -> uint32_t {
+            int j;
+            if (LAT == LAT_D4) j = a ? 4 * mi + 3 : (mi / 3) * 4 + (mi % 3);
+            else if (LAT == LAT_A2) j = 2 * mi + a;
+            else j = mi;
+            return (uint32_t)z[j] & ((1u << ka) - 1u);
+        };
+        for (int ch = 0; ch * 32 < na; ++ch) {
+            int cnt = min(32, na - ch * 32);
+            int lo = 0;
+            for (int b = 0; b < 3; ++b) {
+                int wd = 1 << b;
+                if (!(ka & wd)) continue;
+                if (cnt == 32) {
+                    int per = 8 / wd;
+                    for (int i = 0; i < wd; ++i) {
+                        uint32_t V = 0;
+                        for (int u = 0; u < 32; ++u) {
+                            int g = u >> 2;
+                            if (g / per != i) continue;
+                            uint32_t f = (sym_at(ch * 32 + u) >> lo) & ((1u << wd) - 1u);
+                            V |= f << (8 * (u & 3) + wd * (g % per));
+                        }
+                        bw.put(V, 32);
+                    }
+                } else {
+                    for (int u = 0; u < cnt; ++u) bw.put((sym_at(ch * 32 + u) >> lo) & ((1u << wd) - 1u), wd);
+                }
+                lo += wd;
+            }
+        }
+    }
+    bw.finish();
+}
+
+template <int LAT>
+__device__ inline void write_U(BitWriter& bw, const uint8_t* z, int n, int k0, int k1) {
+    for (int j = 0; j < n; ++j) {
+        uint32_t q = (uint32_t)z[j] >> (sym_class(LAT, j) ? k1 : k0);
+        bw.skip(q);
+        bw.put(1u, 1);
+    }
+    bw.finish();
+}
+
+template <int LAT>
+__device__ inline void tile_symbols(const int8_t* codes, int n, uint8_t* z) {
+    for (int b = 0; b < n / LAT; ++b) {
+        int c[LAT], zz[LAT];
+#pragma unroll
+        for (int i = 0; i < LAT; ++i) c[i] = codes[b * LAT + i];
+        strip<LAT>(c, zz);
+#pragma unroll
+        for (int i = 0; i < LAT; ++i) z[b * LAT + i] = (uint8_t)zz[i];  // <= 255 by the INT8 pre-clamp (G8)
+    }
+}
+
+// one block (128 threads = 128 rows) per group; blob zero-initialized by the caller
+template <int LAT>
+__global__ void __launch_bounds__(128)
+k_pack_groups(const int8_t* codes, const uint16_t* norms, const uint16_t* ulen_tmp, int64_t m, int64_t n_kt,
+              int n, int k0, int k1, const uint32_t* group_off, uint8_t* blob) {
+    extern __shared__ uint8_t zs[];  // [128][n+4]  (+4: de-conflict banks)
+    __shared__ uint32_t scan[128];
+    int64_t g = blockIdx.x;
+    int i = threadIdx.x;
+    int64_t rb = g / n_kt, kt = g % n_kt, r = rb * 128 + i;
+    int rbits = rbits_of(LAT, n, k0, k1);
+    uint32_t r16 = (uint32_t)((128 * (int64_t)rbits + 127) / 128);
+    uint8_t* base = blob + 16 * (int64_t)group_off[g];
+    uint16_t* h_ulen = (uint16_t*)base;
+    uint16_t* h_norm = h_ulen + 128;
+    uint32_t* rarea = (uint32_t*)(base + 512);
+    uint32_t* uarea = (uint32_t*)(base + 512 + 16 * (int64_t)r16);
+    uint32_t ul = ulen_tmp[g * 128 + i];
+    h_ulen[i] = (uint16_t)ul;
+    h_norm[i] = (r < m) ? norms[r * n_kt + kt] : (uint16_t)0;
+    // exclusive prefix of ulen over the group's rows
+    scan[i] = ul;
+    __syncthreads();
+    for (int o = 1; o < 128; o <<= 1) {
+        uint32_t v = (i >= o) ? scan[i - o] : 0;
+        __syncthreads();
+        scan[i] += v;
+        __syncthreads();
+    }
+    uint32_t ustart = scan[i] - ul;
+    if (r >= m) return;
+    uint8_t* z = zs + i * (n + 4);
+    tile_symbols<LAT>(codes + r * (n_kt * n) + kt * n, n, z);
+    BitWriter bwr(rarea, (uint32_t)i * (uint32_t)rbits);
+    write_R<LAT>(bwr, z, n, k0, k1);
+    BitWriter bwu(uarea, ustart);
+    write_U<LAT>(bwu, z, n, k0, k1);
+}
+
+void launch_pack_groups(const int8_t* codes, const uint16_t* norms, const uint16_t* ulen_tmp, int64_t m,
+                        int64_t n_in, int lattice, int n, int k0, int k1, const uint32_t* group_off,
+                        uint8_t* blob, cudaStream_t st) {
+    int64_t n_kt = n_in / n, n_rb = (m + 127) / 128, G = n_rb * n_kt;
+    size_t smem = 128 * (size_t)(n + 4);
+#define HQ_LAUNCH_P(L)                                                                                          \
+    k_pack_groups<L><<<(unsigned)G, 128, smem, st>>>(codes, norms, ulen_tmp, m, n_kt, n, k0, k1, group_off, blob)
+    switch (lattice) {
+        case LAT_Z: HQ_LAUNCH_P(LAT_Z); break;
+        case LAT_A2: HQ_LAUNCH_P(LAT_A2); break;
+        case LAT_D4: HQ_LAUNCH_P(LAT_D4); break;
+        default: HQ_LAUNCH_P(LAT_E8); break;
+    }
+#undef HQ_LAUNCH_P
+}
+
+// ---------------------------------------------------------------------------------------------
+// KV container (FORMAT §6).  Phase 1: per-vector ulen; phase 2: per (role, head) sequential-chunk
+// prefix over the new tokens (one warp per head), block offsets; phase 3: bit packing.
+// ---------------------------------------------------------------------------------------------
+template <int LAT>
+__global__ void k_kv_ulen(const int8_t* codes, int64_t n_tok, int H, int d, int64_t token0, int k0, int k1,
+                          int64_t max_tokens, uint16_t* ulen /*[H][max_tokens] of this role*/, int* err_flag) {
+    int64_t idx = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;  // t*H + h
+    if (idx >= n_tok * H) return;
+    int64_t t = idx / H;
+    int h = (int)(idx % H);
+    uint32_t L = tile_ulen<LAT>(codes + idx * d, d, k0, k1);
+    if (L > 65535u) { atomicExch(err_flag, 1); L = 65535u; }
+    ulen[h * max_tokens + token0 + t] = (uint16_t)L;
+}
+
+// one warp per head: ustart_tmp[h*n_tok + t] = U-stream bit position of token token0+t;
+// updates upos[h], writes blk_off for every 128-token block that starts inside the range.
+__global__ void k_kv_offsets(const uint16_t* ulen, int64_t n_tok, int H, int64_t token0, int64_t max_tokens,
+                             int64_t n_blk, uint32_t* upos, uint32_t* blk_off, uint32_t* ustart_tmp,
+                             int64_t una_bits, int* err_flag) {
+    int h = blockIdx.x;
+    int lane = threadIdx.x;
+    uint32_t pos = upos[h];
+    for (int64_t t0 = 0; t0 < n_tok; t0 += 32) {
+        int64_t t = t0 + lane;
+        uint32_t L = (t < n_tok) ? ulen[h * max_tokens + token0 + t] : 0;
+        uint32_t x = L;
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t y = __shfl_up_sync(0xffffffffu, x, o);
+            if (lane >= o) x += y;
+        }
+        uint32_t start = pos + x - L;
+        if (t < n_tok) {
+            ustart_tmp[h * n_tok + t] = start;
+            if (((token0 + t) & 127) == 0) blk_off[h * (n_blk + 1) + ((token0 + t) >> 7)] = start;
+        }
+        pos += __shfl_sync(0xffffffffu, x, 31);
+    }
+    if (lane == 0) {
+        if ((int64_t)pos > una_bits) atomicExch(err_flag, 2);
+        upos[h] = pos;
+    }
+}
+
+template <int LAT>
+__global__ void __launch_bounds__(128)
+k_kv_pack(const int8_t* codes, int64_t n_tok, int H, int d, int64_t token0, int k0, int k1, int rbits,
+          int64_t rem_words, int64_t una_words, uint32_t* rem, uint32_t* una, const uint32_t* ustart_tmp) {
+    extern __shared__ uint8_t zs[];
+    int64_t idx = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;  // t*H + h
+    if (idx >= n_tok * H) return;
+    int64_t t = idx / H;
+    int h = (int)(idx % H);
+    uint8_t* z = zs + threadIdx.x * (d + 4);
+    tile_symbols<LAT>(codes + idx * d, d, z);
+    BitWriter bwr(rem + h * rem_words, (uint32_t)((token0 + t) * rbits));
+    write_R<LAT>(bwr, z, d, k0, k1);
+    BitWriter bwu(una + h * una_words, ustart_tmp[h * n_tok + t]);
+    write_U<LAT>(bwu, z, d, k0, k1);
+}
+
+void launch_kv_pack(const int8_t* codes, int64_t n_tok, int H, int d, int64_t token0, int role, int lattice,
+                    int k0, int k1, int rbits, int64_t max_tokens, int64_t rem_words, int64_t una_words,
+                    int64_t n_blk, uint32_t* rem, uint32_t* una, uint16_t* ulen, uint32_t* blk_off, uint32_t* upos,
+                    int* err_flag, cudaStream_t st) {
+    // role slices
+    uint32_t* rem_r = rem + (int64_t)role * H * rem_words;
+    uint32_t* una_r = una + (int64_t)role * H * una_words;
+    uint16_t* ulen_r = ulen + (int64_t)role * H * max_tokens;
+    uint32_t* blk_r = blk_off + (int64_t)role * H * (n_blk + 1);
+    uint32_t* upos_r = upos + (int64_t)role * H;
+    // ustart scratch lives right after the codes scratch (caller reserves n_tok*H u32 per role): we
+    // reuse the tail of the codes buffer: codes is [n_tok*H*d] int8 and d >= 64, so allocate separately.
+    uint32_t* ustart_tmp = (uint32_t*)(codes + n_tok * (int64_t)H * d);
+    unsigned blocks = (unsigned)((n_tok * H + 127) / 128);
+    size_t smem = 128 * (size_t)(d + 4);
+#define HQ_KV(L)                                                                                                  \
+    k_kv_ulen<L><<<blocks, 128, 0, st>>>(codes, n_tok, H, d, token0, k0, k1, max_tokens, ulen_r, err_flag);       \
+    k_kv_offsets<<<H, 32, 0, st>>>(ulen_r, n_tok, H, token0, max_tokens, n_blk, upos_r, blk_r, ustart_tmp,        \
+                                   una_words * 32 - 64, err_flag);                                                \
+    k_kv_pack<L><<<blocks, 128, smem, st>>>(codes, n_tok, H, d, token0, k0, k1, rbits, rem_words, una_words,      \
+                                            rem_r, una_r, ustart_tmp)
+    switch (lattice) {
+        case LAT_Z: HQ_KV(LAT_Z); break;
+        case LAT_A2: HQ_KV(LAT_A2); break;
+        case LAT_D4: HQ_KV(LAT_D4); break;
+        default: HQ_KV(LAT_E8); break;
+    }
+#undef HQ_KV
+}
+
+__global__ void k_kv_ring(const __nv_bfloat16* k, const __nv_bfloat16* v, int64_t n_tok, int H, int d,
+                          int64_t token0, int window, __nv_bfloat16* ring) {
+    int64_t per = (int64_t)H * d;
+    int64_t idx = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (idx >= n_tok * per) return;
+    int64_t t = idx / per, e = idx % per;
+    if (n_tok - t > window) return;  // only the last `window` tokens of this call can survive
+    int64_t slot = (token0 + t) % window;
+    ring[(0 * (int64_t)window + slot) * per + e] = k[idx];
+    ring[(1 * (int64_t)window + slot) * per + e] = v[idx];
+}
+void launch_kv_ring(const void* k, const void* v, int64_t n_tok, int H, int d, int64_t token0, int window,
+                    __nv_bfloat16* ring, cudaStream_t st) {
+    if (window <= 0) return;
+    int64_t t_first = n_tok > window ? n_tok - window : 0;
+    int64_t cnt = (n_tok - t_first) * H * d;
+    const __nv_bfloat16* kk = (const __nv_bfloat16*)k + t_first * H * d;
+    const __nv_bfloat16* vv = (const __nv_bfloat16*)v + t_first * H * d;
+    k_kv_ring<<<(unsigned)((cnt + 255) / 256), 256, 0, st>>>(kk, vv, n_tok - t_first, H, d, token0 + t_first, window,
+                                                            ring);
+}
+
+}  // namespace hq

@@ -1,0 +1,117 @@
+// hq_internal.h — host-side declarations shared by the translation units of libhq.so (not installed).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+
+#include "../../include/hq.h"
+
+struct hq_ctx {
+    hq_allocator alloc;
+    int device;
+    int sm_count;
+    std::string err;
+    // cached scratch for hq_linear (q, s_x, split-K partials)
+    void* ws = nullptr;
+    size_t ws_bytes = 0;
+};
+
+struct hq_weight {
+    hq_ctx* ctx;
+    int64_t m, n_in;
+    int lattice, n, k0, k1;
+    float snr_db;
+    double alpha;
+    float A;  // (float)(alpha*sqrt(n))
+    uint64_t seed;
+    int64_t n_kt, n_rb, G;
+    int rbits;
+    uint8_t* blob;        // dev
+    uint32_t* group_off;  // dev [G+1]
+    int8_t* dsign;        // dev [n_in]  RHT signs (+1/-1)
+    int64_t blob_bytes, payload_bits, clamp_count;
+    uint32_t max_group16;  // largest group size in 16-byte units
+};
+
+struct hq_kv {
+    hq_ctx* ctx;
+    hq_kv_config cfg;
+    int k0, k1, rbits;
+    double alpha;
+    float A;
+    int64_t n_tokens;  // host-side count
+    int64_t rem_words, una_words, n_blk;
+    uint32_t* rem;      // [2][H][rem_words]
+    uint32_t* una;      // [2][H][una_words]
+    uint16_t* ulen;     // [2][H][max_tokens]
+    uint16_t* norm;     // [2][H][max_tokens]
+    uint32_t* blk_off;  // [2][H][n_blk+1]
+    uint32_t* upos;     // [2][H]
+    __nv_bfloat16* ring;  // [2][window][H][d]
+    int8_t* dsign;      // [d]
+    int8_t* ssign;      // [d]
+    unsigned long long* counters;  // [1] clamp count
+    int8_t* scratch_codes;         // [2][chunk][H][d]
+    int64_t scratch_tokens;
+    float* att_ws;                 // split partials
+    size_t att_ws_bytes;
+};
+
+namespace hq {
+
+#define HQ_CUDA_CHECK(ctx, call)                                                        \
+    do {                                                                                \
+        cudaError_t e__ = (call);                                                       \
+        if (e__ != cudaSuccess) {                                                       \
+            (ctx)->err = std::string(#call) + ": " + cudaGetErrorString(e__);           \
+            return HQ_ERR_CUDA;                                                         \
+        }                                                                               \
+    } while (0)
+
+// ---- encode (hq_encode.cu) ----
+void launch_signs(uint64_t seed, uint32_t stream_id, int64_t n, int8_t* out, cudaStream_t st);
+// weights: W [m, n_in] -> codes [m, n_in] int8, norms [m, n_kt] u16; counters[0] += clamps,
+// counters[1 + a*8 + k] += total bits of class a at Rice parameter k (auto-k, FORMAT §3)
+void launch_quantize_weights(const void* W, int dtype, int64_t m, int64_t n_in, int64_t ld, int lattice, int n,
+                             float A, const int8_t* dsign, int8_t* codes, uint16_t* norms,
+                             unsigned long long* counters, cudaStream_t st);
+// KV: x [n_tok, H, d] bf16 -> codes [n_tok, H, d], norm written to norm_out[h*max_tokens + token0 + t]
+void launch_quantize_kv(const void* x, int64_t n_tok, int H, int d, int64_t token0, int role, int lattice,
+                        float A, int rotation, int dither, uint64_t seed, const int8_t* dsign,
+                        const int8_t* ssign, int8_t* codes, uint16_t* norm_out, int64_t max_tokens,
+                        unsigned long long* counters, cudaStream_t st);
+// activations: x [B, n_in] -> q int8 [B, n_in], s_x [B, n_kt], optional u
+void launch_act_quant(const void* x, int dtype, int64_t B, int64_t n_in, int64_t ldx, int lattice, int n,
+                      const int8_t* dsign, int8_t* q, float* s_x, float* u, cudaStream_t st);
+// ulen_tmp[g*128 + i] for all groups (0 for absent rows); err_flag set if a tile overflows u16
+void launch_tile_ulen(const int8_t* codes, int64_t m, int64_t n_in, int lattice, int n, int k0, int k1,
+                      uint16_t* ulen_tmp, int* err_flag, cudaStream_t st);
+// group_off[G+1] (16-byte units) by a device prefix sum; totals[0] = sum of ulen over all tiles
+void launch_group_offsets(const uint16_t* ulen_tmp, int64_t G, int rbits, uint32_t* group_off,
+                          unsigned long long* totals, uint32_t* max_group16, cudaStream_t st);
+void launch_pack_groups(const int8_t* codes, const uint16_t* norms, const uint16_t* ulen_tmp, int64_t m,
+                        int64_t n_in, int lattice, int n, int k0, int k1, const uint32_t* group_off,
+                        uint8_t* blob, cudaStream_t st);
+// KV pack: per (role, head) prefix over the new tokens' ulen, then bit-pack into rem/una
+void launch_kv_pack(const int8_t* codes /*[n_tok,H,d]*/, int64_t n_tok, int H, int d, int64_t token0, int role,
+                    int lattice, int k0, int k1, int rbits, int64_t max_tokens, int64_t rem_words,
+                    int64_t una_words, int64_t n_blk, uint32_t* rem, uint32_t* una, uint16_t* ulen,
+                    uint32_t* blk_off, uint32_t* upos, int* err_flag, cudaStream_t st);
+void launch_kv_ring(const void* k, const void* v, int64_t n_tok, int H, int d, int64_t token0, int window,
+                    __nv_bfloat16* ring, cudaStream_t st);
+
+// ---- decode + linear (hq_linear.cu) ----
+void launch_decode_int8(const hq_weight* w, int8_t* codes, uint16_t* norms, cudaStream_t st);
+hq_status launch_linear(hq_ctx* ctx, const hq_weight* w, const int8_t* q, const float* s_x, int64_t B,
+                        void* y_bf16, int64_t ldy, float* y_f32, int32_t* acc_i32, float* partials,
+                        int n_split, cudaStream_t st);
+int linear_choose_split(const hq_ctx* ctx, const hq_weight* w, int64_t B);
+
+// ---- KV decode + attend (hq_attend.cu) ----
+void launch_kv_decode_int8(const hq_kv* kv, int role, int64_t t0, int64_t n, int8_t* codes, cudaStream_t st);
+hq_status launch_attend(hq_ctx* ctx, const hq_kv* kv, const void* q, int q_heads, void* out_bf16,
+                        float* out_f32, cudaStream_t st);
+size_t attend_workspace_bytes(const hq_kv* kv, int q_heads);
+
+}  // namespace hq

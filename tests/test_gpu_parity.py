@@ -1,0 +1,206 @@
+"""GPU parity: libhq.so (through the C ABI / Python binding) against the oracle, element by element.
+
+Bars (BASELINE.json north_star): bit-exact bitstreams, lattice indices, INT8 points, INT32
+accumulators; fp32 RHT outputs within 1e-5; fp32 outputs within 1e-3 (G16) and bf16 within one bf16 ulp.
+"""
+import numpy as np
+import pytest
+
+import hq_synth
+from oracle import hqo
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+def f32(v):
+    """hq_codec_config.snr_db is a C float: hand both sides the same representable value."""
+    return float(np.float32(v))
+
+
+SNR_4BPS = {hqo.E8: f32(22.68), hqo.D4: f32(22.5), hqo.A2: f32(22.2), hqo.Z: f32(21.9)}
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    import paper_2606_23406_b200 as hq
+    c = hq.Context(0)
+    yield c
+    c.close()
+
+
+def _dev(a, dtype=None):
+    t = torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    return t.to(dtype) if dtype is not None else t
+
+
+def _rel_err(y, ref):
+    ref = np.asarray(ref, np.float64)
+    rms = np.sqrt((ref ** 2).mean())
+    return np.max(np.abs(np.asarray(y, np.float64) - ref) / np.maximum(np.abs(ref), 1e-3 * rms + 1e-30))
+
+
+def _assert_bf16_close(y, ref):
+    """bf16 output within one bf16 ulp of bf16(ref), plus the fp32 tolerance near zero (G16)."""
+    ref = np.asarray(ref, np.float64)
+    ref_bf16 = torch.from_numpy(ref.astype(np.float32)).to(torch.bfloat16).float().numpy()
+    tol = np.abs(ref_bf16) * 2.0 ** -7 + 1e-3 * np.sqrt((ref ** 2).mean())
+    assert (np.abs(y.float().cpu().numpy() - ref_bf16) <= tol).all()
+
+
+def _check_weight_bitstream(ctx, W, lattice, n_tile, snr, seed, k=(-1, -1), bf16=False):
+    snr = f32(snr)
+    enc = hqo.encode_weights(W, lattice, n_tile, snr, seed, k)
+    w = ctx.encode_weights(_dev(W, torch.bfloat16 if bf16 else None), lattice, n_tile, snr, seed, k)
+    assert tuple(w.k) == tuple(int(v) for v in enc["k"])
+    blob, goff = w.export()
+    assert (goff == enc["group_off"]).all()
+    assert blob.size == enc["blob"].size
+    if not (blob == enc["blob"]).all():
+        bad = np.flatnonzero(blob != enc["blob"])
+        raise AssertionError(f"bitstream differs at {bad.size} bytes, first {bad[:8]}")
+    codes, norms = w.decode_int8()
+    assert (codes.cpu().numpy() == enc["codes"]).all()
+    assert (norms.cpu().numpy().view(np.uint16) == enc["norms"]).all()
+    assert w.info.payload_bits == enc["payload_bits"] and w.info.clamp_count == enc["clamps"]
+    return w, enc
+
+
+def test_config1_bitstream_codes_linear(ctx):
+    """BASELINE config 1: W 256x256 fp32 N(0,0.02^2) seed 0, tile 64, E8 at 4 bps, x fp32 N(0,1)."""
+    W, x = hq_synth.c1_weight()
+    snr, seed = SNR_4BPS[hqo.E8], 1234
+    w, enc = _check_weight_bitstream(ctx, W, hqo.E8, 64, snr, seed)
+    q_o, sx_o, u_o = hqo.act_quant(x, hqo.E8, 64, seed, want_u=True)
+    q, s_x, u = w.act_quant(_dev(x), want_u=True)
+    assert (q.cpu().numpy() == q_o).all() and (s_x.cpu().numpy() == sx_o).all()
+    assert (u.cpu().numpy() == u_o).all()                       # canonical butterfly: identical bits
+    d = hqo.signs(seed, 1, 256)
+    for kt in range(4):                                          # fp32 RHT output within 1e-5 of the definition
+        ref = hqo.rht_dense_f64(x[0, kt * 64:(kt + 1) * 64].astype(np.float64), d[kt * 64:(kt + 1) * 64])
+        assert np.max(np.abs(u.cpu().numpy()[0, kt * 64:(kt + 1) * 64] - ref)) < 1e-5 * np.abs(ref).max()
+    acc_o, y_o = hqo.linear(enc["codes"], enc["norms"], hqo.E8, 64, snr, q_o, sx_o)
+    y, y32, acc = w.linear(_dev(x), want_f32=True, want_acc=True)
+    assert (acc.cpu().numpy() == acc_o).all()
+    assert _rel_err(y32.cpu().numpy(), y_o) < 1e-3
+    _assert_bf16_close(y, y_o)
+    w.free()
+
+
+@pytest.mark.parametrize("lattice", [hqo.E8, hqo.D4, hqo.A2, hqo.Z])
+@pytest.mark.parametrize("n_tile,m,bps_snr", [(64, 200, 16.5), (128, 384, 22.7), (256, 130, 28.7)])
+def test_bitstream_all_lattices_tiles_ragged_rows(ctx, lattice, n_tile, m, bps_snr):
+    W = hq_synth.gaussian_weight(m, 1024, seed=11 * lattice + m, outliers=True)
+    w, enc = _check_weight_bitstream(ctx, W, lattice, n_tile, bps_snr, seed=77, bf16=True)
+    w.free()
+
+
+def test_explicit_k_and_degenerate_tiles(ctx):
+    W = hq_synth.gaussian_weight(256, 512, seed=5)
+    W[3] = 0.0                                  # zero rows -> rho = 0 (G18)
+    W[:, 128:256] = 0.0                         # a zero K-tile for every row
+    W[7, :] = 0.0; W[7, 300] = 3.0              # all energy in one coordinate -> INT8 pre-clamp (G8)
+    for k in ((0, 0), (3, 1)):
+        w, enc = _check_weight_bitstream(ctx, W, hqo.E8, 128, 28.7, seed=3, k=k)
+        assert enc["clamps"] > 0
+        w.free()
+    w, enc = _check_weight_bitstream(ctx, W, hqo.D4, 64, 28.7, seed=3, k=(2, 1))   # partial R chunks
+    w.free()
+
+
+@pytest.mark.parametrize("lattice,n_tile", [(hqo.E8, 128), (hqo.E8, 256), (hqo.D4, 128), (hqo.A2, 64), (hqo.Z, 128)])
+@pytest.mark.parametrize("B", [1, 16, 40])
+def test_linear_acc_exact_and_outputs(ctx, lattice, n_tile, B):
+    m, n_in, snr, seed = 300, 1024, SNR_4BPS[lattice], 21
+    W = hq_synth.gaussian_weight(m, n_in, seed=lattice + 100, outliers=True)
+    x = hq_synth.activations(B, n_in, seed=B + 7)
+    enc = hqo.encode_weights(W, lattice, n_tile, snr, seed)
+    w = ctx.encode_weights(_dev(W, torch.bfloat16), lattice, n_tile, snr, seed)
+    q_o, sx_o = hqo.act_quant(x, lattice, n_tile, seed)
+    acc_o, y_o = hqo.linear(enc["codes"], enc["norms"], lattice, n_tile, snr, q_o, sx_o)
+    y, y32, acc = w.linear(_dev(x, torch.bfloat16), want_f32=True, want_acc=True)
+    assert (acc.cpu().numpy() == acc_o).all()
+    assert _rel_err(y32.cpu().numpy(), y_o) < 1e-3
+    _assert_bf16_close(y, y_o)
+    w.free()
+
+
+# ------------------------------------------------------------------------------------------ KV
+def _oracle_kv_container(K, V, lattice, snr, k, rotation, dither, seed, chunks):
+    """Oracle-side container for tokens appended in `chunks` (list of token counts)."""
+    T, H, d = K.shape
+    Rbits = hqo.rbits(lattice, d, k)
+    rem = np.zeros((2, H, T * Rbits // 32 + 8), np.uint32)
+    una = np.zeros((2, H, T * d * 4 // 32 + 64), np.uint32)
+    ulen = np.zeros((2, H, T), np.uint16); norm = np.zeros((2, H, T), np.uint16)
+    codes_all = np.zeros((2, T, H, d), np.int8)
+    upos = np.zeros((2, H), np.int64)
+    t0 = 0
+    for n in chunks:
+        for role, X in enumerate((K, V)):
+            codes, norms, _ = hqo.kv_quantize(X[t0:t0 + n], t0, role, lattice, snr, rotation, dither, seed)
+            codes_all[role, t0:t0 + n] = codes
+            norm[role, :, t0:t0 + n] = norms.T
+            for h in range(H):
+                pos, ul = hqo.kv_pack_head(codes, h, lattice, k, rem[role, h], una[role, h], int(upos[role, h]), t0=t0)
+                ulen[role, h, t0:t0 + n] = ul
+                upos[role, h] = pos
+        t0 += n
+    return dict(rem=rem, una=una, ulen=ulen, norm=norm, codes=codes_all, upos=upos)
+
+
+@pytest.mark.parametrize("lattice,snr,k,dither,rotation", [
+    (hqo.E8, 9.68, (0, 0), 1, 1),      # config 4: E8 at 2 bps, signs rotation, dither on
+    (hqo.E8, 22.68, (2, 2), 0, 0),
+    (hqo.D4, 16.3, (1, 0), 1, 1),
+    (hqo.A2, 16.0, (1, 1), 1, 0),
+    (hqo.Z, 15.7, (1, 1), 1, 1),
+])
+def test_kv_append_container_exact(ctx, lattice, snr, k, dither, rotation):
+    T, H, d, seed, snr = 300, 2, 128, 99, f32(snr)
+    K = hq_synth.kv_tokens(T, H, d, seed=4); V = hq_synth.kv_tokens(T, H, d, seed=5)
+    chunks = [257, 1, 1, 41]                                       # bulk prefill, single-token steps, ragged
+    ora = _oracle_kv_container(K, V, lattice, snr, k, rotation, dither, seed, chunks)
+    kv = ctx.kv_create(H, d, 512, lattice, snr, k, seed, rotation=rotation, dither=dither, window=32)
+    t0 = 0
+    for n in chunks:
+        kv.append(_dev(K[t0:t0 + n], torch.bfloat16), _dev(V[t0:t0 + n], torch.bfloat16))
+        t0 += n
+    ex = kv.export()
+    assert ex["n_tokens"] == T
+    assert (ex["ulen"][:, :, :T] == ora["ulen"]).all()
+    assert (ex["norm"][:, :, :T] == ora["norm"]).all()
+    assert (ex["upos"] == ora["upos"]).all()
+    nr = min(ex["rem"].shape[2], ora["rem"].shape[2]); nu = min(ex["una"].shape[2], ora["una"].shape[2])
+    assert (ex["rem"][:, :, :nr] == ora["rem"][:, :, :nr]).all()
+    assert (ex["una"][:, :, :nu] == ora["una"][:, :, :nu]).all()
+    for role in range(2):
+        for h in range(H):                                         # block offsets = prefix sums of ulen
+            cs = np.concatenate([[0], np.cumsum(ora["ulen"][role, h].astype(np.int64))])
+            for b in range((T + 127) // 128):
+                assert ex["blk_off"][role, h, b] == cs[128 * b]
+        codes = kv.decode_int8(role, 0, T).cpu().numpy()
+        assert (codes == ora["codes"][role]).all()
+    kv.free()
+
+
+@pytest.mark.parametrize("lattice,snr,k,dither,T,window", [
+    (hqo.E8, 9.68, (0, 0), 1, 700, 32),
+    (hqo.E8, 22.68, (2, 2), 0, 200, 0),
+    (hqo.A2, 16.0, (1, 1), 1, 130, 32),
+    (hqo.E8, 9.68, (0, 0), 1, 20, 32),       # everything inside the window: exact bf16 attention (G15)
+])
+def test_attend_matches_oracle_long_way(ctx, lattice, snr, k, dither, T, window):
+    H, d, QH, seed, rotation, snr = 2, 128, 8, 5, 1, f32(snr)
+    K = hq_synth.kv_tokens(T, H, d, seed=14); V = hq_synth.kv_tokens(T, H, d, seed=15)
+    q = hq_synth.activations(QH, d, seed=16)
+    kv = ctx.kv_create(H, d, 1024, lattice, snr, k, seed, rotation=rotation, dither=dither, window=window)
+    kv.append(_dev(K, torch.bfloat16), _dev(V, torch.bfloat16))
+    out, o32 = kv.attend(_dev(q, torch.bfloat16), want_f32=True)
+    ck, nk, _ = hqo.kv_quantize(K, 0, 0, lattice, snr, rotation, dither, seed)
+    cv, nv, _ = hqo.kv_quantize(V, 0, 1, lattice, snr, rotation, dither, seed)
+    Kh = hqo.kv_reconstruct(ck, nk, 0, 0, lattice, snr, rotation, dither, seed)
+    Vh = hqo.kv_reconstruct(cv, nv, 0, 1, lattice, snr, rotation, dither, seed)
+    ref = hqo.attend(Kh, Vh, K, V, window=window, q=q)
+    assert _rel_err(o32.cpu().numpy(), ref) < 1e-3
+    _assert_bf16_close(out, ref)
+    kv.free()
