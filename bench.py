@@ -1,0 +1,301 @@
+#!/usr/bin/env python
+"""bench.py — HyperQuant hot path on B200: fused Rice-decode + tcgen05 INT8 GEMV over one Llama-3.1-8B-shaped
+decoder layer's linears (BASELINE.json configs[1]: E8, 4 bps, RHT tile 128, batch 1), seeded synthetic weights.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--layers L] [--impl reference]
+
+A step = the seven linears (q,k,v,o,gate,up,down) of one layer at batch 1 through hq_linear (activation RHT +
+INT8 cast, fused decode+MMA, split-K finalize).  L distinct layers (L x ~116 MB compressed > the 126 MB L2) are
+cycled so no step re-reads its weights from L2.  One JSON line on stdout (rank 0).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import hq_synth  # noqa: E402
+
+METRIC = "fused decode+INT8 GEMV % of HBM roofline; large-M INT8 TOPS vs peak"
+UNIT = "GB/s of compressed weight bytes (batch-1 GEMV, whole layer)"
+SNR_E8_4BPS = float(np.float32(22.68))   # E8 at 4.0 bps on iid Gaussian tiles (B.1 L857)
+NAMES = list(hq_synth.LLAMA_SHAPES)
+WORKLOAD = "llama3.1-8b decoder-layer linears q/k/v/o/gate/up/down, E8 4 bps, RHT tile 128, batch 1 (BASELINE configs[1])"
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler(threading.Thread):
+    def __init__(self, index=0):
+        super().__init__(daemon=True)
+        self.index, self.stop_flag, self.rows = index, False, []
+
+    def run(self):
+        q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+            "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+        while not self.stop_flag:
+            try:
+                out = subprocess.run(["nvidia-smi", f"--query-gpu={q}", "--format=csv,noheader,nounits", "-i",
+                                      str(self.index)], capture_output=True, text=True, timeout=5).stdout.strip()
+                if out:
+                    self.rows.append([c.strip() for c in out.split(",")])
+            except Exception:
+                pass
+            time.sleep(0.05)
+
+    def summary(self):
+        if not self.rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unsampled"]}
+        sm = sorted(int(r[0]) for r in self.rows if r[0].isdigit())
+        mx = max(int(r[1]) for r in self.rows if r[1].isdigit())
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(r[2 + i].lower().startswith("active") for r in self.rows)]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": mx, "reasons": reasons, "samples": len(sm)}
+
+
+def oracle_sample(threads_note=True):
+    """The oracle (as it stands) on a bounded sample of the workload: the 'k' projection (1024 x 4096) of
+    layer 0 — decode the container (O2) + activation cast + INT8 contraction (O3) at batch 1."""
+    from oracle import hqo
+    W = hq_synth.llama_weight(0, "k")
+    x = hq_synth.activations(1, W.shape[1], seed=1000)
+    enc = hqo.encode_weights(W, hqo.E8, 128, SNR_E8_4BPS, seed=0)          # untimed: building the sample
+    nbytes = (enc["payload_bits"] + 32 * enc["norms"].size) / 8.0
+
+    def one_pass():
+        codes, norms = hqo.unpack_weights(enc["blob"], enc["group_off"], W.shape[0], W.shape[1], hqo.E8, 128, enc["k"])
+        q, s_x = hqo.act_quant(x, hqo.E8, 128, seed=0)
+        hqo.linear(codes, norms, hqo.E8, 128, SNR_E8_4BPS, q, s_x, want_acc=False)
+
+    return one_pass, nbytes, "oracle decode (O2) + act cast + INT8 contraction (O3) on layer-0 'k' 1024x4096, batch 1"
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, same metric/unit/config, bounded sample per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    one_pass, nbytes, sample = oracle_sample()
+    for _ in range(max(1, min(args.warmup, 2))):
+        one_pass()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        one_pass()
+    dt = time.perf_counter() - t0
+    val = nbytes * args.steps / dt / 1e9
+    cores = len(os.sched_getaffinity(0))
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "int8", "data": "synthetic",
+            "config": {"workload": WORKLOAD, "lattice": "E8", "bps": 4.0, "n_tile": 128, "batch": 1},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=4)
+    ap.add_argument("--layers", type=int, default=4)
+    ap.add_argument("--impl", default="ours")
+    ap.add_argument("--skip-extras", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import paper_2606_23406_b200 as hq
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    ctx = hq.Context(local)
+
+    # ---- build the workload (untimed): L layers x 7 compressed matrices, replicas on every rank
+    layers, alg_bytes = [], []
+    for l in range(args.layers):
+        ws, nb = {}, 0.0
+        for name in NAMES:
+            W = torch.from_numpy(hq_synth.llama_weight(l, name)).to(dev).to(torch.bfloat16)
+            w = ctx.encode_weights(W, hq.Lattice.E8, 128, SNR_E8_4BPS, seed=l)
+            del W
+            ws[name] = w
+            nb += (w.info.payload_bits + w.info.norm_bits + w.info.length_bits) / 8.0 + 2 * (w.n_in + w.m)
+        layers.append(ws)
+        alg_bytes.append(nb)
+    bytes_per_step = float(np.mean(alg_bytes))
+    scalars_per_step = sum(m * n for m, n in hq_synth.LLAMA_SHAPES.values())
+    bps_total = 8.0 * np.mean([sum((w.info.payload_bits + w.info.norm_bits + w.info.length_bits) / 8.0
+                                   for w in ws.values()) for ws in layers]) / scalars_per_step
+    bps_payload = np.mean([sum(w.info.payload_bits for w in ws.values()) for ws in layers]) / scalars_per_step
+
+    def make_io(B):
+        xs = {n_in: torch.from_numpy(hq_synth.activations(B, n_in, seed=77 + n_in)).to(dev).to(torch.bfloat16)
+              for n_in in (4096, 14336)}
+        ys = {name: torch.empty((B, hq_synth.LLAMA_SHAPES[name][0]), dtype=torch.bfloat16, device=dev) for name in NAMES}
+        return xs, ys
+
+    def step(i, xs, ys):
+        ws = layers[i % args.layers]
+        for name in NAMES:
+            w = ws[name]
+            w.linear(xs[w.n_in], y=ys[name])
+
+    def barrier():
+        if world > 1:
+            import torch.distributed as dist
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(B, steps, warmup, profile=False):
+        xs, ys = make_io(B)
+        for i in range(warmup):
+            step(i, xs, ys)
+        barrier()
+        ctx.profile(profile)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for i in range(steps):
+            step(warmup + i, xs, ys)
+        e1.record()
+        barrier()
+        ms = e0.elapsed_time(e1)
+        kern = ctx.profile_read() if profile else (0.0, 0)
+        ctx.profile(False)
+        if world > 1:
+            import torch.distributed as dist
+            t = torch.tensor([ms], device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        return ms, kern
+
+    # ---- headline: batch 1, device-resident inputs
+    sampler = ClockSampler(local)
+    sampler.start()
+    ms, _ = timed(1, args.steps, args.warmup)
+    sampler.stop_flag = True
+    sampler.join()
+    ms_per_step = ms / args.steps
+    value = world * bytes_per_step / (ms_per_step * 1e-3) / 1e9
+
+    # ---- roofline of the dominant kernel (fused decode+MMA), CUDA events around each launch
+    ms_p, (kern_ms, kern_n) = timed(1, args.steps, 2, profile=True)
+    weight_bytes_per_step = bytes_per_step
+    achieved = weight_bytes_per_step * args.steps / (kern_ms * 1e-3) / 1e9 if kern_ms > 0 else 0.0
+    peak, peak_src = peaks()
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": None, "kernel": "k_linear_generic<E8,16>", "peak_source": peak_src,
+                "kernel_share_of_step": kern_ms / ms_p if ms_p > 0 else None,
+                "launches_timed": kern_n, "avg_launch_us": 1e3 * kern_ms / max(kern_n, 1),
+                "alg_bytes_per_scalar": bytes_per_step / scalars_per_step,
+                "frac_of_nominal_8TBs": achieved / 8000.0}
+
+    # ---- end to end: host (pinned) x -> device, linears, y -> host, every step
+    xs, ys = make_io(1)
+    hx = {k: v.cpu().pin_memory() for k, v in xs.items()}
+    hy = {k: torch.empty_like(v, device="cpu").pin_memory() for k, v in ys.items()}
+    h2d = sum(hx[layers[0][n].n_in].numel() * 2 for n in NAMES)
+    d2h = sum(v.numel() * 2 for v in hy.values())
+
+    def e2e_step(i):
+        ws = layers[i % args.layers]
+        for name in NAMES:
+            w = ws[name]
+            xs[w.n_in].copy_(hx[w.n_in], non_blocking=True)
+            w.linear(xs[w.n_in], y=ys[name])
+            hy[name].copy_(ys[name], non_blocking=True)
+    for i in range(3):
+        e2e_step(i)
+    barrier()
+    t0 = time.perf_counter()
+    for i in range(args.steps):
+        e2e_step(3 + i)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    if world > 1:
+        import torch.distributed as dist
+        t = torch.tensor([e2e_s], device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    e2e = {"value": world * bytes_per_step * args.steps / e2e_s / 1e9, "unit": UNIT, "h2d_bytes_per_step": h2d,
+           "d2h_bytes_per_step": d2h}
+
+    extras = {}
+    if not args.skip_extras and rank == 0:
+        # batch 16 on the same weights
+        ms16, _ = timed(16, max(4, args.steps // 2), 2)
+        extras["batch16"] = {"ms_per_step": ms16 / max(4, args.steps // 2),
+                             "GBps_compressed": bytes_per_step / (ms16 / max(4, args.steps // 2) * 1e-3) / 1e9}
+        # practical baseline on the same box: bf16 GEMV by cuBLAS on uncompressed weights (one layer, cycled 4x)
+        try:
+            dense = [{n: torch.randn(hq_synth.LLAMA_SHAPES[n], device=dev, dtype=torch.bfloat16) * 0.02 for n in NAMES}
+                     for _ in range(2)]
+            xs1, _ = make_io(1)
+            for i in range(3):
+                for n in NAMES:
+                    torch.matmul(xs1[dense[0][n].shape[1]], dense[i % 2][n].t())
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for i in range(10):
+                for n in NAMES:
+                    torch.matmul(xs1[dense[0][n].shape[1]], dense[i % 2][n].t())
+            e1.record()
+            torch.cuda.synchronize()
+            extras["cublas_bf16_gemv_ms_per_layer"] = e0.elapsed_time(e1) / 10
+            del dense
+        except Exception as ex:  # noqa: BLE001
+            extras["cublas_bf16_gemv_ms_per_layer"] = f"failed: {ex}"
+
+    # ---- CPU baseline: the oracle on a bounded sample, rank 0, N=1 only
+    cpu = None
+    if rank == 0 and world == 1:
+        one_pass, nbytes, sample = oracle_sample()
+        one_pass()
+        reps, t0 = 0, time.perf_counter()
+        while time.perf_counter() - t0 < 10.0 and reps < 50:
+            one_pass()
+            reps += 1
+        dt = time.perf_counter() - t0
+        cpu = {"value": nbytes * reps / dt / 1e9, "unit": UNIT, "cores": len(os.sched_getaffinity(0)), "kind": "oracle",
+               "sample": f"{sample}; {reps} passes in {dt:.1f} s"}
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "int8", "data": "synthetic",
+                "config": {"workload": WORKLOAD, "lattice": "E8", "snr_db": SNR_E8_4BPS, "n_tile": 128, "batch": 1,
+                           "layers_cycled": args.layers, "l2_policy": "inputs larger than L2 (layers cycled)",
+                           "scalars_per_step": scalars_per_step, "bits_per_scalar_payload": bps_payload,
+                           "bits_per_scalar_total": bps_total, "parallelism": "replicas only"},
+                "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": args.steps * len(NAMES) * 3,
+                "roofline": roofline, "cpu_baseline": cpu, "extras": extras}
+        print(json.dumps(line))
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -63,6 +63,12 @@ hq_status hq_create(hq_ctx** out, const hq_allocator* alloc, int cuda_device);
 void hq_destroy(hq_ctx* ctx);
 const char* hq_last_error(const hq_ctx* ctx); /* never NULL; valid until the next call on ctx */
 
+/* Measurement aid: when enabled, hq_linear and hq_attend bracket their dominant kernel (the fused
+ * decode+MMA kernel / the split attention kernel) with CUDA events on the caller's stream.
+ * hq_profile_read synchronizes those events, returns their summed duration and count, and clears them. */
+hq_status hq_profile_enable(hq_ctx* ctx, int32_t on);
+hq_status hq_profile_read(hq_ctx* ctx, double* total_ms, int64_t* launches);
+
 /* alpha of eq.(9) L871 for (lattice, snr_db), as the library computes it (host, double). */
 double hq_alpha(int32_t lattice, double snr_db);
 

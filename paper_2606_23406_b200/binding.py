@@ -55,7 +55,7 @@ def lib_path() -> str:
 
 _lib = None
 
-EXPORTS = ["hq_create", "hq_destroy", "hq_last_error", "hq_alpha", "hq_encode_weights", "hq_weight_free",
+EXPORTS = ["hq_create", "hq_destroy", "hq_last_error", "hq_alpha", "hq_profile_enable", "hq_profile_read", "hq_encode_weights", "hq_weight_free",
            "hq_weight_get_info", "hq_weight_export", "hq_decode_int8", "hq_act_quant", "hq_linear",
            "hq_linear_workspace_bytes", "hq_kv_create", "hq_kv_free", "hq_kv_append", "hq_attend", "hq_kv_export",
            "hq_kv_decode_int8"]
@@ -75,6 +75,8 @@ def load_library():
     lib.hq_destroy.argtypes = [vp]; lib.hq_destroy.restype = None
     lib.hq_last_error.argtypes = [vp]; lib.hq_last_error.restype = C.c_char_p
     lib.hq_alpha.argtypes = [i32, C.c_double]; lib.hq_alpha.restype = C.c_double
+    lib.hq_profile_enable.argtypes = [vp, i32]
+    lib.hq_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(i64)]
     lib.hq_encode_weights.argtypes = [vp, vp, i32, i64, i64, i64, C.POINTER(_CodecConfig), vp, C.POINTER(vp)]
     lib.hq_weight_free.argtypes = [vp, vp]; lib.hq_weight_free.restype = None
     lib.hq_weight_get_info.argtypes = [vp, C.POINTER(_WeightInfo)]
@@ -141,6 +143,15 @@ class Context:
     def check(self, st: int):
         if st != 0:
             raise HQError(f"libhq status {st}: {self.lib.hq_last_error(self.h).decode()}")
+
+    def profile(self, on: bool):
+        self.check(self.lib.hq_profile_enable(self.h, 1 if on else 0))
+
+    def profile_read(self):
+        """(summed ms of the bracketed dominant kernels, their count) since the last read."""
+        ms, n = C.c_double(), C.c_int64()
+        self.check(self.lib.hq_profile_read(self.h, C.byref(ms), C.byref(n)))
+        return ms.value, n.value
 
     def close(self):
         if getattr(self, "h", None):

@@ -62,6 +62,31 @@ void hq_destroy(hq_ctx* ctx) {
 
 const char* hq_last_error(const hq_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
 
+hq_status hq_profile_enable(hq_ctx* ctx, int32_t on) {
+    if (!ctx) return HQ_ERR_INVALID_ARG;
+    ctx->prof = on != 0;
+    return HQ_OK;
+}
+
+hq_status hq_profile_read(hq_ctx* ctx, double* total_ms, int64_t* launches) {
+    if (!ctx || !total_ms || !launches) return HQ_ERR_INVALID_ARG;
+    double ms = 0.0;
+    int64_t n = 0;
+    for (size_t i = 0; i + 1 < ctx->prof_ev.size(); i += 2) {
+        HQ_CUDA_CHECK(ctx, cudaEventSynchronize(ctx->prof_ev[i + 1]));
+        float t = 0.0f;
+        HQ_CUDA_CHECK(ctx, cudaEventElapsedTime(&t, ctx->prof_ev[i], ctx->prof_ev[i + 1]));
+        ms += t;
+        ++n;
+        cudaEventDestroy(ctx->prof_ev[i]);
+        cudaEventDestroy(ctx->prof_ev[i + 1]);
+    }
+    ctx->prof_ev.clear();
+    *total_ms = ms;
+    *launches = n;
+    return HQ_OK;
+}
+
 double hq_alpha(int32_t lattice, double snr_db) {
     if (!valid_lattice(lattice)) return 0.0;
     return sqrt(pow(10.0, snr_db / 10.0) * second_moment(lattice));

@@ -349,6 +349,12 @@ hq_status launch_attend(hq_ctx* ctx, const hq_kv* kv, const void* q, int q_heads
         HQ_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_attend_split<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
         k_attend_split<L><<<H * p.n_split, 128, smem, st>>>(p);                                                    \
     } while (0)
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (ctx->prof && p.Tc > 0) {
+        HQ_CUDA_CHECK(ctx, cudaEventCreate(&e0));
+        HQ_CUDA_CHECK(ctx, cudaEventCreate(&e1));
+        HQ_CUDA_CHECK(ctx, cudaEventRecord(e0, st));
+    }
     if (p.Tc > 0) {
         switch (kv->cfg.codec.lattice) {
             case LAT_Z: HQ_AT(LAT_Z); break;
@@ -357,6 +363,11 @@ hq_status launch_attend(hq_ctx* ctx, const hq_kv* kv, const void* q, int q_heads
             default: HQ_AT(LAT_E8); break;
         }
         HQ_CUDA_CHECK(ctx, cudaGetLastError());
+        if (e0) {
+            HQ_CUDA_CHECK(ctx, cudaEventRecord(e1, st));
+            ctx->prof_ev.push_back(e0);
+            ctx->prof_ev.push_back(e1);
+        }
     } else {
         p.n_split = 0;
     }

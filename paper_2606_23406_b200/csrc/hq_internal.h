@@ -4,6 +4,7 @@
 #include <stdint.h>
 
 #include <string>
+#include <vector>
 
 #include "../../include/hq.h"
 
@@ -15,6 +16,9 @@ struct hq_ctx {
     // cached scratch for hq_linear (q, s_x, split-K partials)
     void* ws = nullptr;
     size_t ws_bytes = 0;
+    // optional kernel timing (hq_profile_*): event pairs around the dominant kernel of each call
+    bool prof = false;
+    std::vector<cudaEvent_t> prof_ev;
 };
 
 struct hq_weight {

@@ -266,8 +266,19 @@ hq_status launch_linear(hq_ctx* ctx, const hq_weight* w, const int8_t* q, const 
     p.inv_A = (float)(1.0 / (w->alpha * sqrt((double)w->n)));
     p.q = q; p.s_x = s_x; p.B = B; p.n_split = n_split; p.partials = partials; p.acc_i32 = acc_i32;
     p.stage_bytes = stage_bytes_for(w);
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (ctx->prof) {
+        HQ_CUDA_CHECK(ctx, cudaEventCreate(&e0));
+        HQ_CUDA_CHECK(ctx, cudaEventCreate(&e1));
+        HQ_CUDA_CHECK(ctx, cudaEventRecord(e0, st));
+    }
     hq_status s = (B <= 16) ? launch_linear_nb<16>(ctx, w, p, st) : launch_linear_nb<64>(ctx, w, p, st);
     if (s != HQ_OK) return s;
+    if (ctx->prof) {
+        HQ_CUDA_CHECK(ctx, cudaEventRecord(e1, st));
+        ctx->prof_ev.push_back(e0);
+        ctx->prof_ev.push_back(e1);
+    }
     int64_t tot = B * w->m;
     k_linear_finalize<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(partials, n_split, B, w->m, (__nv_bfloat16*)y_bf16,
                                                                     ldy, y_f32);

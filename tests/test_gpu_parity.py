@@ -98,8 +98,10 @@ def test_explicit_k_and_degenerate_tiles(ctx):
     W = hq_synth.gaussian_weight(256, 512, seed=5)
     W[3] = 0.0                                  # zero rows -> rho = 0 (G18)
     W[:, 128:256] = 0.0                         # a zero K-tile for every row
-    W[7, :] = 0.0; W[7, 300] = 3.0              # all energy in one coordinate -> INT8 pre-clamp (G8)
-    for k in ((0, 0), (3, 1)):
+    d = hqo.signs(3, 1, 512)[256:384].astype(np.float32)      # a row whose RHT is n*e_5: all energy in one
+    had = np.array([(-1.0) ** bin(i & 5).count("1") for i in range(128)], np.float32)
+    W[7, :] = 0.0; W[7, 256:384] = d * had * 0.5                # coordinate -> INT8 pre-clamp (G8)
+    for k in ((0, 0), (3, 3)):
         w, enc = _check_weight_bitstream(ctx, W, hqo.E8, 128, 28.7, seed=3, k=k)
         assert enc["clamps"] > 0
         w.free()
