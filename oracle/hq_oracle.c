@@ -378,10 +378,10 @@ static int64_t write_tile_R(int lattice, const int8_t* codes, int n, const int* 
                     for (int i = 0; i < wd; ++i) {
                         uint32_t V = 0;
                         for (int u = 0; u < 32; ++u) {
-                            int g = u >> 2;
+                            int g = 2 * (u >> 3) + (u & 1), lane = (u & 7) >> 1;
                             if (g / per != i) continue;
                             uint32_t f = (uint32_t)(r[ch * 32 + u] >> lo[pl]) & ((1u << wd) - 1u);
-                            V |= f << (8 * (u & 3) + wd * (g % per));
+                            V |= f << (8 * lane + wd * (g % per));
                         }
                         put_word(words, p, V, 32);
                         p += 32;
@@ -432,9 +432,9 @@ static int64_t read_tile_RU(int lattice, int n, const int* k, const uint32_t* rw
                 if (cnt == 32) {
                     for (int i = 0; i < wd; ++i) {
                         for (int u = 0; u < 32; ++u) {
-                            int g = u >> 2;
+                            int g = 2 * (u >> 3) + (u & 1), lane = (u & 7) >> 1;
                             if (g / per != i) continue;
-                            int sh = 8 * (u & 3) + wd * (g % per); /* field's bit 0 in V */
+                            int sh = 8 * lane + wd * (g % per); /* field's bit 0 in V */
                             for (int b = 0; b < wd; ++b)
                                 rem[idx[ch * 32 + u]] |= (int32_t)get_bit(rwords, p + (31 - (sh + b))) << (lo[pl] + b);
                         }

@@ -298,9 +298,9 @@ __device__ inline uint32_t get_remainder(const uint32_t* rarea, uint32_t rpos, i
         int wd = 1 << b;
         if (!(ka & wd)) continue;
         if (cnt == 32) {
-            int per = 8 / wd, g = u >> 2;
+            int per = 8 / wd, g = 2 * (u >> 3) + (u & 1), bl = (u & 7) >> 1;
             uint32_t V = get32(rarea, base + (uint32_t)(32 * lo + 32 * (g / per)));
-            r |= ((V >> (8 * (u & 3) + wd * (g % per))) & ((1u << wd) - 1u)) << lo;
+            r |= ((V >> (8 * bl + wd * (g % per))) & ((1u << wd) - 1u)) << lo;
         } else {
             r |= get_bits(rarea, base + (uint32_t)(cnt * lo + u * wd), wd) << lo;
         }

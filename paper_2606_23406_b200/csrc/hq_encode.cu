@@ -430,10 +430,10 @@ __device__ inline void write_R(BitWriter& bw, const uint8_t* z, int n, int k0, i
                     for (int i = 0; i < wd; ++i) {
                         uint32_t V = 0;
                         for (int u = 0; u < 32; ++u) {
-                            int g = u >> 2;
+                            int g = 2 * (u >> 3) + (u & 1), lane = (u & 7) >> 1;
                             if (g / per != i) continue;
                             uint32_t f = (sym_at(ch * 32 + u) >> lo) & ((1u << wd) - 1u);
-                            V |= f << (8 * (u & 3) + wd * (g % per));
+                            V |= f << (8 * lane + wd * (g % per));
                         }
                         bw.put(V, 32);
                     }

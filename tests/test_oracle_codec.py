@@ -139,8 +139,9 @@ def test_weight_container_roundtrip(lattice, n_tile, m):
 
 
 def test_field_plane_layout_is_swar_extractable():
-    # FORMAT §4: in a full chunk of 32 symbols the w-bit field of symbols 4g..4g+3 is
-    # (V[g // (8/w)] >> (w * (g % (8/w)))) & (mask_w * 0x01010101), one symbol per byte.
+    # FORMAT §4: in a full chunk of 32 symbols (four blocks of 8), group g = 2*block + parity holds the
+    # w-bit fields of the block's even (parity 0) or odd (parity 1) symbols, one symbol per byte:
+    # (V[g // (8/w)] >> (w * (g % (8/w)))) & (mask_w * 0x01010101).
     rng = np.random.default_rng(5)
     for k in range(1, 8):
         zz = rng.integers(0, 1 << k, size=64)          # Z lattice: symbol = zigzag(code), q = 0
@@ -159,7 +160,8 @@ def test_field_plane_layout_is_swar_extractable():
                     V = int(words[wi + g // per])
                     f4 = (V >> (wd * (g % per))) & (((1 << wd) - 1) * 0x01010101)
                     for u in range(4):
-                        assert (f4 >> (8 * u)) & 0xFF == (int(zz[32 * ch + 4 * g + u]) >> lo) & ((1 << wd) - 1)
+                        sym = 32 * ch + 8 * (g // 2) + 2 * u + (g % 2)
+                        assert (f4 >> (8 * u)) & 0xFF == (int(zz[sym]) >> lo) & ((1 << wd) - 1)
                 wi += wd
                 lo += wd
         # U-section: q = 0 everywhere -> 64 one bits right after the R-section
