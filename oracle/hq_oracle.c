@@ -306,15 +306,40 @@ static int sym_class(int lattice, int j) {
     if (lattice == HQO_A2) return j & 1;
     return 0;
 }
-/* symbols of a whole tile of n codes (block-major) */
+/* Stream order of a tile's symbols (FORMAT §3).  Position p of the tile stream holds the symbol of
+ * lattice block blk, coordinate i, returned as the block-major index blk*dim + i.  D4, A2, Z:
+ * block-major (identity).  E8: inside each run of 32 symbols (4 blocks) the order is coordinate-pair
+ * major: p = 32c + 8w + 2b + e  <->  block 4c + b, coordinate 2w + e  (w = 0..3, b = 0..3, e = 0..1),
+ * so that four consecutive even (odd) positions hold one coordinate of four consecutive blocks. */
+static int stream_to_blockmajor(int lattice, int p) {
+    if (lattice != HQO_E8) return p;
+    int c = p >> 5, w = (p >> 3) & 3, b = (p >> 1) & 3, e = p & 1;
+    return 8 * (4 * c + b) + 2 * w + e;
+}
+/* symbols of a whole tile of n codes, in stream order; cls[p] = Rice class of position p */
 static void tile_symbols(int lattice, const int8_t* codes, int n, int32_t* z) {
     int dim = lattice;
+    int32_t zb[1024];
     for (int b = 0; b < n / dim; ++b) {
         int32_t c[8];
         for (int i = 0; i < dim; ++i) c[i] = codes[b * dim + i];
-        hqo_strip(lattice, c, z + b * dim);
+        hqo_strip(lattice, c, zb + b * dim);
+    }
+    for (int p = 0; p < n; ++p) z[p] = zb[stream_to_blockmajor(lattice, p)];
+}
+/* inverse: stream-order symbols -> codes */
+static void tile_codes(int lattice, const int32_t* z, int n, int8_t* codes) {
+    int dim = lattice;
+    int32_t zb[1024];
+    for (int p = 0; p < n; ++p) zb[stream_to_blockmajor(lattice, p)] = z[p];
+    for (int b = 0; b < n / dim; ++b) {
+        int32_t c[8];
+        hqo_unstrip(lattice, zb + b * dim, c);
+        for (int i = 0; i < dim; ++i) codes[b * dim + i] = (int8_t)c[i];
     }
 }
+/* Rice class of stream position p: a function of the symbol's coordinate inside its block */
+static int pos_class(int lattice, int p) { return sym_class(lattice, stream_to_blockmajor(lattice, p)); }
 
 /* ------------------------------------------------------------------------------------------ */
 /* Rice coding of a tile into the split-plane tile stream (§3.3, §4.7; FORMAT §3-4).   */
@@ -335,7 +360,7 @@ int64_t hqo_tile_bits(int lattice, const int8_t* codes, int n, const int* k) {
     tile_symbols(lattice, codes, n, z);
     int64_t L = 0;
     for (int j = 0; j < n; ++j) {
-        int kk = k[sym_class(lattice, j)];
+        int kk = k[pos_class(lattice, j)];
         L += kk + 1 + (z[j] >> kk);
     }
     return L;
@@ -369,7 +394,7 @@ static int64_t write_tile_R(int lattice, const int8_t* codes, int n, const int* 
         int na = 0, ka = k[a], w[3], lo[3];
         int np = field_planes(ka, w, lo);
         for (int j = 0; j < n; ++j)
-            if (sym_class(lattice, j) == a) r[na++] = z[j] & ((1 << ka) - 1);
+            if (pos_class(lattice, j) == a) r[na++] = z[j] & ((1 << ka) - 1);
         for (int ch = 0; ch * 32 < na; ++ch) {
             int cnt = na - ch * 32 < 32 ? na - ch * 32 : 32;
             for (int pl = 0; pl < np; ++pl) {
@@ -406,7 +431,7 @@ static int64_t write_tile_U(int lattice, const int8_t* codes, int n, const int* 
     uint64_t p = pos;
     tile_symbols(lattice, codes, n, z);
     for (int j = 0; j < n; ++j) {
-        int q = z[j] >> k[sym_class(lattice, j)];
+        int q = z[j] >> k[pos_class(lattice, j)];
         p += q;
         put_bit(words, p, 1u);
         p += 1;
@@ -424,7 +449,7 @@ static int64_t read_tile_RU(int lattice, int n, const int* k, const uint32_t* rw
         int idx[1024], na = 0, ka = k[a], w[3], lo[3];
         int np = field_planes(ka, w, lo);
         for (int j = 0; j < n; ++j)
-            if (sym_class(lattice, j) == a) { idx[na++] = j; rem[j] = 0; }
+            if (pos_class(lattice, j) == a) { idx[na++] = j; rem[j] = 0; }
         for (int ch = 0; ch * 32 < na; ++ch) {
             int cnt = na - ch * 32 < 32 ? na - ch * 32 : 32;
             for (int pl = 0; pl < np; ++pl) {
@@ -455,14 +480,9 @@ static int64_t read_tile_RU(int lattice, int n, const int* k, const uint32_t* rw
         int q = 0;
         while (!get_bit(uwords, p)) { ++q; ++p; }
         ++p;
-        z[j] = (q << k[sym_class(lattice, j)]) | rem[j];
+        z[j] = (q << k[pos_class(lattice, j)]) | rem[j];
     }
-    int dim = lattice;
-    for (int b = 0; b < n / dim; ++b) {
-        int32_t c[8];
-        hqo_unstrip(lattice, z + b * dim, c);
-        for (int i = 0; i < dim; ++i) codes[b * dim + i] = (int8_t)c[i];
-    }
+    tile_codes(lattice, z, n, codes);
     return (int64_t)(p - upos);
 }
 
@@ -496,7 +516,7 @@ int64_t hqo_rice_reference_bits(int lattice, const int8_t* codes, int n, const i
     uint64_t p = 0;
     tile_symbols(lattice, codes, n, z);
     for (int j = 0; j < n; ++j) {
-        int kk = k[sym_class(lattice, j)], q = z[j] >> kk;
+        int kk = k[pos_class(lattice, j)], q = z[j] >> kk;
         p += q;
         put_bit(words, p++, 1u);
         put_word(words, p, (uint32_t)(z[j] & ((1 << kk) - 1)), kk);
@@ -512,7 +532,7 @@ void hqo_symbol_histogram(int lattice, const int8_t* codes, int64_t ntiles, int 
     int32_t z[1024];
     for (int64_t t = 0; t < ntiles; ++t) {
         tile_symbols(lattice, codes + t * n, n, z);
-        for (int j = 0; j < n; ++j) hist[(j % dim) * 512 + z[j]]++;
+        for (int j = 0; j < n; ++j) hist[(stream_to_blockmajor(lattice, j) % dim) * 512 + z[j]]++;
     }
 }
 
@@ -585,7 +605,7 @@ void hqo_choose_k(const int8_t* codes, int64_t ntiles, int lattice, int n, int* 
         int32_t z[1024];
         tile_symbols(lattice, codes + t * n, n, z);
         for (int j = 0; j < n; ++j)
-            for (int kk = 0; kk < 8; ++kk) tot[sym_class(lattice, j)][kk] += kk + 1 + (z[j] >> kk);
+            for (int kk = 0; kk < 8; ++kk) tot[pos_class(lattice, j)][kk] += kk + 1 + (z[j] >> kk);
     }
     if (lattice == HQO_D4) { /* k_t = max(k_s - 1, 0), minimize the sum (L272, L295) */
         int best = 0;
@@ -611,43 +631,61 @@ void hqo_choose_k(const int8_t* codes, int64_t ntiles, int lattice, int n, int* 
 /* ------------------------------------------------------------------------------------------ */
 /* Weight container (FORMAT §5): pack / unpack.                                                */
 /* ------------------------------------------------------------------------------------------ */
-/* returns blob size in bytes; if blob == NULL only sizes (group_off) are computed. */
+/* Sub-group sg = (rb * n_kt + kt) * 4 + w holds rows [128 rb + 32 w, +32) of K-tile kt:
+ *   u16 ulen[32] | u16 norm[32] | u32 rarea[RW*32] | u32 uarea[sum_i nw_i] | zero pad to 16 bytes
+ * RW = ceil(Rbits/32); word j of row i's R-section at rarea[j*32 + i]; row i's U-section starts at
+ * bit 0 of its own word 0 and takes nw_i = ceil(ulen_i/32) words; "word-row" t of uarea holds word t
+ * of every row with nw_i > t, in increasing row order.  Absent rows (>= m): ulen = 0, norm = 0.
+ * returns blob size in bytes; if blob == NULL only sizes (group_off[4G+1], 16-byte units) are computed. */
 int64_t hqo_pack_weights(const int8_t* codes, const uint16_t* norms, int64_t m, int64_t n_in,
                          int lattice, int n, const int* k, uint8_t* blob,
-                         uint32_t* group_off /*[G+1]*/) {
+                         uint32_t* group_off /*[4G+1]*/) {
     int64_t n_kt = n_in / n, n_rb = (m + 127) / 128, off16 = 0;
-    int64_t Rbits = rbits_of(lattice, n, k), r16 = (128 * Rbits + 127) / 128;
+    int64_t Rbits = rbits_of(lattice, n, k), RW = (Rbits + 31) / 32;
     for (int64_t rb = 0; rb < n_rb; ++rb)
-        for (int64_t kt = 0; kt < n_kt; ++kt) {
-            int64_t g = rb * n_kt + kt, ubits = 0;
-            group_off[g] = (uint32_t)off16;
-            uint16_t* ulen = blob ? (uint16_t*)(blob + 16 * off16) : NULL;
-            uint16_t* nrm = ulen ? ulen + 128 : NULL;
-            uint32_t* rarea = blob ? (uint32_t*)(blob + 16 * (off16 + 32)) : NULL;
-            uint32_t* uarea = blob ? (uint32_t*)(blob + 16 * (off16 + 32 + r16)) : NULL;
-            for (int i = 0; i < 128; ++i) {
-                int64_t r = rb * 128 + i;
-                int64_t U = (r < m) ? hqo_tile_bits(lattice, codes + r * n_in + kt * n, n, k) - Rbits : 0;
+        for (int64_t kt = 0; kt < n_kt; ++kt)
+            for (int w = 0; w < 4; ++w) {
+                int64_t sg = (rb * n_kt + kt) * 4 + w, uwords = 0;
+                int64_t U[32], nw[32], maxnw = 0;
+                group_off[sg] = (uint32_t)off16;
+                for (int i = 0; i < 32; ++i) {
+                    int64_t r = rb * 128 + w * 32 + i;
+                    U[i] = (r < m) ? hqo_tile_bits(lattice, codes + r * n_in + kt * n, n, k) - Rbits : 0;
+                    nw[i] = (U[i] + 31) / 32;
+                    uwords += nw[i];
+                    if (nw[i] > maxnw) maxnw = nw[i];
+                }
+                int64_t bytes = 128 + 4 * (RW * 32 + uwords);
+                int64_t sz16 = (bytes + 15) / 16;
                 if (blob) {
-                    ulen[i] = (uint16_t)U;
-                    nrm[i] = (r < m) ? norms[r * n_kt + kt] : 0;
+                    uint8_t* base = blob + 16 * off16;
+                    memset(base, 0, (size_t)sz16 * 16);
+                    uint16_t* ulen = (uint16_t*)base;
+                    uint16_t* nrm = ulen + 32;
+                    uint32_t* rarea = (uint32_t*)(base + 128);
+                    uint32_t* uarea = rarea + RW * 32;
+                    uint32_t tmp[32][256]; /* row streams: FORMAT §5 bounds a U-section by 8160 bits = 255 words */
+                    for (int i = 0; i < 32; ++i) {
+                        int64_t r = rb * 128 + w * 32 + i;
+                        ulen[i] = (uint16_t)U[i];
+                        nrm[i] = (r < m) ? norms[r * n_kt + kt] : 0;
+                        if (r >= m) continue;
+                        uint32_t rw[64];
+                        memset(rw, 0, sizeof rw);
+                        write_tile_R(lattice, codes + r * n_in + kt * n, n, k, rw, 0);
+                        for (int64_t j = 0; j < RW; ++j) rarea[j * 32 + i] = rw[j];
+                        if (nw[i] > 255) return -1; /* FORMAT error (the CUDA side reports HQ_ERR_FORMAT) */
+                        memset(tmp[i], 0, sizeof tmp[i]);
+                        write_tile_U(lattice, codes + r * n_in + kt * n, n, k, tmp[i], 0);
+                    }
+                    int64_t at = 0;
+                    for (int64_t t = 0; t < maxnw; ++t)
+                        for (int i = 0; i < 32; ++i)
+                            if (nw[i] > t) uarea[at++] = tmp[i][t];
                 }
-                ubits += U;
+                off16 += sz16;
             }
-            int64_t u16 = (ubits + 127) / 128;
-            if (blob) {
-                memset(rarea, 0, (size_t)(r16 + u16) * 16);
-                uint64_t p = 0;
-                for (int i = 0; i < 128; ++i) {
-                    int64_t r = rb * 128 + i;
-                    if (r >= m) break;
-                    write_tile_R(lattice, codes + r * n_in + kt * n, n, k, rarea, (uint64_t)(i * Rbits));
-                    p += (uint64_t)write_tile_U(lattice, codes + r * n_in + kt * n, n, k, uarea, p);
-                }
-            }
-            off16 += 32 + r16 + u16;
-        }
-    group_off[n_rb * n_kt] = (uint32_t)off16;
+    group_off[n_rb * n_kt * 4] = (uint32_t)off16;
     return off16 * 16;
 }
 
@@ -655,22 +693,35 @@ int64_t hqo_pack_weights(const int8_t* codes, const uint16_t* norms, int64_t m, 
 void hqo_unpack_weights(const uint8_t* blob, const uint32_t* group_off, int64_t m, int64_t n_in,
                         int lattice, int n, const int* k, int8_t* codes, uint16_t* norms) {
     int64_t n_kt = n_in / n, n_rb = (m + 127) / 128;
-    int64_t Rbits = rbits_of(lattice, n, k), r16 = (128 * Rbits + 127) / 128;
+    int64_t Rbits = rbits_of(lattice, n, k), RW = (Rbits + 31) / 32;
 #pragma omp parallel for schedule(static)
-    for (int64_t g = 0; g < n_rb * n_kt; ++g) {
-        int64_t rb = g / n_kt, kt = g % n_kt;
-        const uint8_t* base = blob + 16 * (int64_t)group_off[g];
+    for (int64_t sg = 0; sg < n_rb * n_kt * 4; ++sg) {
+        int64_t g = sg / 4, w = sg % 4, rb = g / n_kt, kt = g % n_kt;
+        const uint8_t* base = blob + 16 * (int64_t)group_off[sg];
         const uint16_t* ulen = (const uint16_t*)base;
-        const uint16_t* nrm = ulen + 128;
-        const uint32_t* rarea = (const uint32_t*)(base + 512);
-        const uint32_t* uarea = (const uint32_t*)(base + 512 + 16 * r16);
-        uint64_t p = 0;
-        for (int i = 0; i < 128; ++i) {
-            int64_t r = rb * 128 + i;
-            if (r >= m) break;
+        const uint16_t* nrm = ulen + 32;
+        const uint32_t* rarea = (const uint32_t*)(base + 128);
+        const uint32_t* uarea = rarea + RW * 32;
+        int64_t nw[32], maxnw = 0;
+        for (int i = 0; i < 32; ++i) {
+            nw[i] = (ulen[i] + 31) / 32;
+            if (nw[i] > maxnw) maxnw = nw[i];
+        }
+        for (int i = 0; i < 32; ++i) {
+            int64_t r = rb * 128 + w * 32 + i;
+            if (r >= m) continue;
             norms[r * n_kt + kt] = nrm[i];
-            read_tile_RU(lattice, n, k, rarea, (uint64_t)(i * Rbits), uarea, p, codes + r * n_in + kt * n);
-            p += ulen[i];
+            uint32_t rw[64], uw[258];
+            for (int64_t j = 0; j < RW; ++j) rw[j] = rarea[j * 32 + i];
+            int64_t at = 0;
+            for (int64_t t = 0; t < maxnw; ++t)
+                for (int i2 = 0; i2 < 32; ++i2)
+                    if (nw[i2] > t) {
+                        if (i2 == i) uw[t] = uarea[at];
+                        ++at;
+                    }
+            uw[nw[i]] = 0xffffffffu; /* guard: a corrupt stream stops here */
+            read_tile_RU(lattice, n, k, rw, 0, uw, 0, codes + r * n_in + kt * n);
         }
     }
 }

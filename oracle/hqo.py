@@ -180,10 +180,12 @@ def choose_k(codes, lattice, n_tile):
 def pack_weights(codes, norms, lattice, n_tile, k):
     codes = _c(codes, np.int8); norms = _c(norms, np.uint16); k = _karr(k)
     m, n_in = codes.shape
-    G = ((m + 127) // 128) * (n_in // n_tile)
-    goff = np.zeros(G + 1, np.uint32)
+    G4 = 4 * ((m + 127) // 128) * (n_in // n_tile)          # sub-groups of 32 rows x one K-tile (FORMAT §5)
+    goff = np.zeros(G4 + 1, np.uint32)
     args = (_p(codes), _p(norms), C.c_int64(m), C.c_int64(n_in), lattice, C.c_int(n_tile), _p(k))
     size = lib().hqo_pack_weights(*args, None, _p(goff))
+    if size < 0:
+        raise ValueError("a tile's U-section exceeds 8160 bits (FORMAT §5)")
     blob = np.zeros(size, np.uint8)
     lib().hqo_pack_weights(*args, _p(blob), _p(goff))
     return blob, goff

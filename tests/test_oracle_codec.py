@@ -118,24 +118,59 @@ def test_weight_container_roundtrip(lattice, n_tile, m):
     enc = hqo.encode_weights(W, lattice, n_tile, 22.0, seed=9)
     codes, norms = hqo.unpack_weights(enc["blob"], enc["group_off"], m, 512, lattice, n_tile, enc["k"])
     assert (codes == enc["codes"]).all() and (norms == enc["norms"]).all()
-    # layout facts of FORMAT §5: headers hold the U-section lengths, R-sections sit at a fixed
-    # stride, groups are 16-byte aligned and ordered
+    # layout facts of FORMAT §5, re-derived here from the codes alone: sub-groups of 32 rows x one K-tile,
+    # header = ulen[32] | norm[32], R words interleaved over rows, U word-rows compacted in row order
     n_kt, n_rb = 512 // n_tile, (m + 127) // 128
     Rbits = hqo.rbits(lattice, n_tile, enc["k"])
-    r16 = (128 * Rbits + 127) // 128
+    RW = (Rbits + 31) // 32
     goff = enc["group_off"].astype(np.int64)
-    assert len(goff) == n_rb * n_kt + 1 and (np.diff(goff) > 32).all() and goff[-1] * 16 == enc["blob"].size
+    assert len(goff) == 4 * n_rb * n_kt + 1 and goff[-1] * 16 == enc["blob"].size
     lens_total = 0
-    for g in range(n_rb * n_kt):
-        hdr = enc["blob"][16 * goff[g]: 16 * goff[g] + 512].view(np.uint16)
-        rows = min(128, m - 128 * (g // n_kt))
-        assert (hdr[rows:128] == 0).all() and (hdr[128 + rows:] == 0).all()
+    for sg in range(4 * n_rb * n_kt):
+        g, w = sg // 4, sg % 4
+        rb, kt = g // n_kt, g % n_kt
+        base = 16 * goff[sg]
+        hdr = enc["blob"][base: base + 128].view(np.uint16)
+        rows = int(np.clip(m - (128 * rb + 32 * w), 0, 32))
+        assert (hdr[rows:32] == 0).all() and (hdr[32 + rows:] == 0).all()
+        nw = (hdr[:32].astype(np.int64) + 31) // 32
+        size = 128 + 4 * (RW * 32 + int(nw.sum()))
+        assert goff[sg + 1] - goff[sg] == (size + 15) // 16
+        area = enc["blob"][base + 128: base + size].view(np.uint32)
+        uarea = area[RW * 32:]
         for i in range(rows):
-            r, kt = 128 * (g // n_kt) + i, g % n_kt
-            assert hdr[i] + Rbits == hqo.tile_bits(lattice, enc["codes"][r, kt * n_tile:(kt + 1) * n_tile], enc["k"])
-        assert (goff[g + 1] - goff[g] - 32 - r16) == (int(hdr[:128].sum()) + 127) // 128
-        lens_total += int(hdr[:128].sum()) + rows * Rbits
+            r = 128 * rb + 32 * w + i
+            tile = enc["codes"][r, kt * n_tile:(kt + 1) * n_tile]
+            assert hdr[i] + Rbits == hqo.tile_bits(lattice, tile, enc["k"])
+            # the row's logical stream, written on its own, is what the container interleaves
+            words = np.zeros(RW + int(nw[i]) + 2, np.uint32)
+            hqo.write_tile(lattice, tile, enc["k"], words, 0)
+            if Rbits % 32 == 0:
+                assert (area[np.arange(RW) * 32 + i] == words[:RW]).all()
+                for t in range(int(nw[i])):
+                    at = int(np.minimum(nw, t).sum()) + int((nw[:i] > t).sum())   # earlier word-rows + earlier rows
+                    assert uarea[at] == words[RW + t]
+        lens_total += int(hdr[:32].sum()) + rows * Rbits
     assert lens_total == enc["payload_bits"]
+
+
+def test_e8_stream_order_groups_coordinates_of_four_blocks():
+    # FORMAT §3: stream position p = 32c + 8w + 2b + e holds coordinate 2w+e of block 4c+b.  A tile whose only
+    # non-zero code sits in (block, coordinate) must put its only non-zero symbol at that stream position:
+    # with k = 0 the U-section is "1" per zero symbol and q zeros + "1" for the non-zero one.
+    n = 64
+    for blk in range(8):
+        for coord in range(7):                       # coordinates 0..6 carry zigzag(s_i) themselves (L261-270)
+            codes = np.zeros(n, np.int8)
+            codes[8 * blk + coord] = 2                # even coset, s = 1 -> zigzag 2; parity of the block flips s_7:
+            codes[8 * blk + 7] = 2                    # keep the point in 2E8: s_7 = 1 = 2*0 + parity(1)
+            words = np.zeros(8, np.uint32)
+            hqo.write_tile(hqo.E8, codes, (0, 0), words, 0)
+            bits = "".join(format(int(x), "032b") for x in words)
+            c, b = blk // 4, blk % 4
+            p = 32 * c + 8 * (coord // 2) + 2 * b + (coord % 2)
+            assert bits[:p] == "1" * p and bits[p:p + 3] == "001"
+            assert (hqo.read_tile(hqo.E8, n, (0, 0), words, 0)[0] == codes).all()
 
 
 def test_field_plane_layout_is_swar_extractable():
