@@ -31,7 +31,7 @@ typedef enum {
     HQ_ERR_UNSUPPORTED = 3, /* not an sm_100 device, rotation qjl, ... */
     HQ_ERR_ALLOC = 4,       /* the caller's allocator returned NULL */
     HQ_ERR_CUDA = 5,        /* a CUDA runtime call failed; text in hq_last_error */
-    HQ_ERR_FORMAT = 6       /* a tile's U-section does not fit the u16 length field (FORMAT §4) */
+    HQ_ERR_FORMAT = 6       /* a tile's U-section exceeds the container's bound (FORMAT §4, §5) */
 } hq_status;
 
 typedef enum { HQ_Z = 1, HQ_A2 = 2, HQ_D4 = 4, HQ_E8 = 8 } hq_lattice;     /* §3.2, §4.5; value = dimension */
@@ -94,12 +94,12 @@ typedef struct {
     int64_t norm_bits;     /* 16 per tile (L500) */
     int64_t length_bits;   /* 16 per tile (G12) */
     int64_t blob_bytes;    /* whole container incl. padding */
-    int64_t n_groups;      /* ceil(m_out/128) * n_in/n_tile */
+    int64_t n_groups;      /* sub-groups of 32 rows x one tile: 4 * ceil(m_out/128) * n_in/n_tile (FORMAT §5) */
     int64_t clamp_count;   /* quantizer inputs limited by the INT8 pre-clamp (G8, L236) */
 } hq_weight_info;
 hq_status hq_weight_get_info(const hq_weight* w, hq_weight_info* out);
 
-/* dev pointers into the handle (valid until hq_weight_free): the FORMAT §5 blob and group_off[G+1]. */
+/* dev pointers into the handle (valid until hq_weight_free): the FORMAT §5 blob and sub_off[n_groups+1]. */
 hq_status hq_weight_export(const hq_weight* w, const void** blob_dev, const uint32_t** group_off_dev);
 
 /* Parity / debug: the INT8 lattice points c [m_out, n_in] (row-major, dev) and fp16 norms

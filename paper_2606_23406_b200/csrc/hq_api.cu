@@ -134,7 +134,7 @@ hq_status hq_encode_weights(hq_ctx* ctx, const void* W_dev, int32_t dtype, int64
     norms = (uint16_t*)ctx_alloc(ctx, (size_t)(m_out * w->n_kt) * 2);
     ulen_tmp = (uint16_t*)ctx_alloc(ctx, (size_t)w->G * 128 * 2);
     counters = (unsigned long long*)ctx_alloc(ctx, 32 * sizeof(unsigned long long));
-    w->group_off = (uint32_t*)ctx_alloc(ctx, (size_t)(w->G + 1) * 4);
+    w->group_off = (uint32_t*)ctx_alloc(ctx, (size_t)(4 * w->G + 1) * 4);
     if (!w->dsign || !codes || !norms || !ulen_tmp || !counters || !w->group_off) return bail(HQ_ERR_ALLOC);
 
 #define HQ_TRY(call)                                                                 \
@@ -184,14 +184,14 @@ hq_status hq_encode_weights(hq_ctx* ctx, const void* W_dev, int32_t dtype, int64
     int* err_flag = (int*)(counters + 18);
     uint32_t* maxg = (uint32_t*)(counters + 19);
     launch_tile_ulen(codes, m_out, n_in, w->lattice, w->n, k0, k1, ulen_tmp, err_flag, st);
-    launch_group_offsets(ulen_tmp, w->G, w->rbits, w->group_off, counters + 17, maxg, st);
+    launch_group_offsets(ulen_tmp, 4 * w->G, (w->rbits + 31) / 32, w->group_off, counters + 17, maxg, st);
     HQ_TRY(cudaGetLastError());
     uint32_t total16 = 0;
-    HQ_TRY(cudaMemcpyAsync(&total16, w->group_off + w->G, 4, cudaMemcpyDeviceToHost, st));
+    HQ_TRY(cudaMemcpyAsync(&total16, w->group_off + 4 * w->G, 4, cudaMemcpyDeviceToHost, st));
     HQ_TRY(cudaMemcpyAsync(hc, counters, sizeof(hc), cudaMemcpyDeviceToHost, st));
     HQ_TRY(cudaStreamSynchronize(st));
     if (*(int*)(hc + 18) != 0) {
-        ctx->err = "a tile's U-section exceeds 65535 bits (FORMAT §4)";
+        ctx->err = "a tile's U-section exceeds 8160 bits (FORMAT §5)";
         return bail(HQ_ERR_FORMAT);
     }
     w->max_group16 = *(uint32_t*)(hc + 19);
@@ -224,7 +224,7 @@ hq_status hq_weight_get_info(const hq_weight* w, hq_weight_info* out) {
     out->rice_k[0] = w->k0; out->rice_k[1] = w->k1; out->snr_db = w->snr_db; out->alpha = w->alpha;
     out->seed = w->seed; out->payload_bits = w->payload_bits;
     out->norm_bits = 16 * w->m * w->n_kt; out->length_bits = 16 * w->m * w->n_kt;
-    out->blob_bytes = w->blob_bytes; out->n_groups = w->G; out->clamp_count = w->clamp_count;
+    out->blob_bytes = w->blob_bytes; out->n_groups = 4 * w->G; out->clamp_count = w->clamp_count;
     return HQ_OK;
 }
 

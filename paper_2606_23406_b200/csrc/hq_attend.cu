@@ -27,7 +27,7 @@ __global__ void k_kv_decode_int8(const uint32_t* rem, const uint32_t* una, const
     int h = (int)(idx % H);
     uint32_t us = kv_ustart_serial(ulen + h * max_tokens, blk_off + h * (n_blk + 1), t);
     int8_t* out = codes + idx * d;
-    decode_row_generic<LAT>(rem + h * rem_words, (uint32_t)(t * rbits), una + h * una_words, us, d, k0, k1,
+    decode_row_generic<LAT>(WordsContig{rem + h * rem_words}, (uint32_t)(t * rbits), WordsContig{una + h * una_words}, us, d, k0, k1,
                             [&](int b, const int* c) {
 #pragma unroll
                                 for (int e = 0; e < LAT; ++e) out[b * LAT + e] = (int8_t)c[e];
@@ -150,7 +150,7 @@ k_attend_split(AttendParams p) {
 #pragma unroll
                 for (int g = 0; g < ATT_MAXG; ++g) dot[g] = 0.0f;
                 if (valid) {
-                    decode_row_generic<LAT>(rem, (uint32_t)(t * p.rbits), una, us, d, p.k0, p.k1,
+                    decode_row_generic<LAT>(WordsContig{rem}, (uint32_t)(t * p.rbits), WordsContig{una}, us, d, p.k0, p.k1,
                                             [&](int b, const int* c) {
                                                 float U[LAT];
                                                 if (p.dither) dither_block<LAT>(p.seed, (uint32_t)b, (uint32_t)t, (uint32_t)h, 0u, U);
@@ -192,7 +192,7 @@ k_attend_split(AttendParams p) {
                 // V: write v' rows to smem
                 float* row = vt + tid * (d + 1);
                 if (valid) {
-                    decode_row_generic<LAT>(rem, (uint32_t)(t * p.rbits), una, us, d, p.k0, p.k1,
+                    decode_row_generic<LAT>(WordsContig{rem}, (uint32_t)(t * p.rbits), WordsContig{una}, us, d, p.k0, p.k1,
                                             [&](int b, const int* c) {
                                                 float U[LAT];
                                                 if (p.dither) dither_block<LAT>(p.seed, (uint32_t)b, (uint32_t)t, (uint32_t)h, 1u, U);

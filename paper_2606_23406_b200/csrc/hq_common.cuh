@@ -268,22 +268,39 @@ __device__ inline void unstrip(const int* z, int* c) {
 }
 
 // ---------------------------------------------------------------------------------------------
-// MSB-first bit streams over little-endian u32 words (FORMAT §4).
+// Stream order of a tile's symbols (FORMAT §3): position p -> block-major index blk*dim + i.
+// E8: p = 32c + 8w + 2b + e  <->  block 4c + b, coordinate 2w + e; other lattices: identity.
 // ---------------------------------------------------------------------------------------------
-// 32 stream bits starting at bit position p (reads words p>>5 and (p>>5)+1: areas are padded).
-__device__ inline uint32_t get32(const uint32_t* w, uint32_t p) {
-    uint32_t i = p >> 5, s = p & 31;
-    uint32_t hi = w[i], lo = w[i + 1];
-    return __funnelshift_l(lo, hi, s);
-}
-__device__ inline uint32_t get_bits(const uint32_t* w, uint32_t p, int nb) {  // nb in [1,32], value MSB-first
-    return get32(w, p) >> (32 - nb);
+__host__ __device__ inline int stream_to_blockmajor(int lattice, int p) {
+    if (lattice != LAT_E8) return p;
+    int c = p >> 5, w = (p >> 3) & 3, b = (p >> 1) & 3, e = p & 1;
+    return 8 * (4 * c + b) + 2 * w + e;
 }
 
-// the k-bit remainder of class-a symbol number m_idx (index within its class) of a tile whose
-// R-section starts at stream bit rpos (FORMAT §4 field planes). Generic (slow) path.
-__device__ inline uint32_t get_remainder(const uint32_t* rarea, uint32_t rpos, int lattice, int n, int k0,
-                                         int k1, int a, int m_idx) {
+// ---------------------------------------------------------------------------------------------
+// MSB-first bit streams over little-endian u32 words (FORMAT §4), read through a word accessor
+// `word(i) -> uint32_t` (must return 0 past the end of the stream).
+// ---------------------------------------------------------------------------------------------
+struct WordsContig {  // a contiguous, padded word array
+    const uint32_t* w;
+    __device__ inline uint32_t operator()(uint32_t i) const { return w[i]; }
+};
+template <class W>
+__device__ inline uint32_t get32(const W& word, uint32_t p) {  // 32 stream bits starting at bit p
+    uint32_t i = p >> 5, s = p & 31;
+    uint32_t hi = word(i), lo = word(i + 1);
+    return __funnelshift_l(lo, hi, s);
+}
+template <class W>
+__device__ inline uint32_t get_bits(const W& word, uint32_t p, int nb) {  // nb in [1,32], value MSB-first
+    return get32(word, p) >> (32 - nb);
+}
+
+// the k-bit remainder of class-a symbol number m_idx (index within its class, stream order) of a tile
+// whose R-section starts at stream bit rpos of `rword` (FORMAT §4 field planes). Generic (slow) path.
+template <class W>
+__device__ inline uint32_t get_remainder(const W& rword, uint32_t rpos, int lattice, int n, int k0, int k1, int a,
+                                         int m_idx) {
     int ka = a ? k1 : k0;
     if (ka == 0) return 0;
     int na = class_count(lattice, n, a);
@@ -299,10 +316,10 @@ __device__ inline uint32_t get_remainder(const uint32_t* rarea, uint32_t rpos, i
         if (!(ka & wd)) continue;
         if (cnt == 32) {
             int per = 8 / wd, g = 2 * (u >> 3) + (u & 1), bl = (u & 7) >> 1;
-            uint32_t V = get32(rarea, base + (uint32_t)(32 * lo + 32 * (g / per)));
+            uint32_t V = get32(rword, base + (uint32_t)(32 * lo + 32 * (g / per)));
             r |= ((V >> (8 * bl + wd * (g % per))) & ((1u << wd) - 1u)) << lo;
         } else {
-            r |= get_bits(rarea, base + (uint32_t)(cnt * lo + u * wd), wd) << lo;
+            r |= get_bits(rword, base + (uint32_t)(cnt * lo + u * wd), wd) << lo;
         }
         lo += wd;
     }
@@ -311,49 +328,136 @@ __device__ inline uint32_t get_remainder(const uint32_t* rarea, uint32_t rpos, i
 
 // ---------------------------------------------------------------------------------------------
 // Generic row decoder (any lattice / tile / k): U-section walked with clz, remainders by
-// get_remainder, un-strip per lattice block; emits INT8 codes per block through `out(b, c[LAT])`.
+// get_remainder, un-strip per lattice block; emits INT8 codes per block through `out(blk, c[LAT])`
+// (blk = block-major block index).  Symbols arrive in stream order (FORMAT §3).
 // ---------------------------------------------------------------------------------------------
-template <int LAT, class Out>
-__device__ inline void decode_row_generic(const uint32_t* rarea, uint32_t rpos, const uint32_t* uarea,
-                                          uint32_t upos, int n, int k0, int k1, Out out) {
-    uint32_t p = upos;
-    uint32_t x = get32(uarea, p);
-    int avail = 32;
-    int cls_idx[2] = {0, 0};
-    for (int b = 0; b < n / LAT; ++b) {
-        int z[LAT], c[LAT];
-#pragma unroll
-        for (int i = 0; i < LAT; ++i) {
-            int j = b * LAT + i;
-            int q = 0;
-            while (true) {  // count zeros up to the terminating one
-                if (x == 0) {
-                    q += avail;
-                    p += avail;
-                    x = get32(uarea, p);
-                    avail = 32;
-                    if (q > 70000) break;  // corrupt stream guard: stay bounded
-                    continue;
-                }
-                int lz = __clz(x);
-                q += lz;
-                int used = lz + 1;
-                x = (used >= 32) ? 0u : (x << used);
-                avail -= used;
-                p += used;
-                if (avail == 0) { x = get32(uarea, p); avail = 32; }
-                break;
+template <class W>
+struct UnaryReader {
+    const W& word;
+    uint32_t p, x;
+    int avail;
+    __device__ UnaryReader(const W& w, uint32_t p0) : word(w), p(p0), x(get32(w, p0)), avail(32) {}
+    __device__ inline int next() {  // zeros up to the terminating one
+        int q = 0;
+        while (true) {
+            if (x == 0) {
+                q += avail; p += avail;
+                x = get32(word, p); avail = 32;
+                if (q > 70000) break;  // corrupt stream guard: stay bounded
+                continue;
             }
-            int a = sym_class(LAT, j);
-            int ka = a ? k1 : k0;
-            uint32_t r = get_remainder(rarea, rpos, LAT, n, k0, k1, a, cls_idx[a]);
-            cls_idx[a]++;
-            z[i] = (q << ka) | (int)r;
+            int lz = __clz(x);
+            q += lz;
+            int used = lz + 1;
+            x = (used >= 32) ? 0u : (x << used);
+            avail -= used; p += used;
+            if (avail == 0) { x = get32(word, p); avail = 32; }
+            break;
         }
-        unstrip<LAT>(z, c);
-        out(b, c);
+        return q;
+    }
+};
+
+template <int LAT, class RW, class UW, class Out>
+__device__ inline void decode_row_generic(const RW& rword, uint32_t rpos, const UW& uword, uint32_t upos, int n,
+                                          int k0, int k1, Out out) {
+    UnaryReader<UW> ur(uword, upos);
+    int cls_idx[2] = {0, 0};
+    if (LAT == LAT_E8) {
+        for (int ch = 0; ch < n / 32; ++ch) {
+            int zc[32];
+            for (int u = 0; u < 32; ++u) {
+                int q = ur.next();
+                uint32_t r = get_remainder(rword, rpos, LAT_E8, n, k0, k1, 0, ch * 32 + u);
+                zc[u] = (q << k0) | (int)r;
+            }
+#pragma unroll
+            for (int b = 0; b < 4; ++b) {
+                int z[8], c[8];
+#pragma unroll
+                for (int i = 0; i < 8; ++i) z[i] = zc[8 * (i >> 1) + 2 * b + (i & 1)];
+                unstrip<LAT_E8>(z, c);
+                out(4 * ch + b, c);
+            }
+        }
+    } else {
+        for (int b = 0; b < n / LAT; ++b) {
+            int z[LAT], c[LAT];
+#pragma unroll
+            for (int i = 0; i < LAT; ++i) {
+                int j = b * LAT + i;
+                int q = ur.next();
+                int a = sym_class(LAT, j);
+                int ka = a ? k1 : k0;
+                uint32_t r = get_remainder(rword, rpos, LAT, n, k0, k1, a, cls_idx[a]);
+                cls_idx[a]++;
+                z[i] = (q << ka) | (int)r;
+            }
+            unstrip<LAT>(z, c);
+            out(b, c);
+        }
     }
 }
+
+// ---------------------------------------------------------------------------------------------
+// Weight sub-group access (FORMAT §5): 32 rows, lane i = row i.
+// ---------------------------------------------------------------------------------------------
+struct SubGroup {
+    const uint16_t* ulen;   // [32]
+    const uint16_t* norm;   // [32]
+    const uint32_t* rarea;  // [RW*32], word j of row i at j*32 + i
+    const uint32_t* uarea;  // compacted word-rows
+};
+__device__ inline SubGroup sub_group(const uint8_t* base, int rw_words) {
+    SubGroup s;
+    s.ulen = (const uint16_t*)base;
+    s.norm = s.ulen + 32;
+    s.rarea = (const uint32_t*)(base + 128);
+    s.uarea = s.rarea + rw_words * 32;
+    return s;
+}
+// index (in uarea) of word t of row i, by scanning the header: sum_i' min(nw_i', t) + #{i' < i : nw_i' > t}
+__device__ inline uint32_t u_word_index_slow(const uint16_t* ulen_hdr, int i, uint32_t t) {
+    uint32_t at = 0;
+    for (int r = 0; r < 32; ++r) {
+        uint32_t nw = ((uint32_t)ulen_hdr[r] + 31u) >> 5;
+        at += min(nw, t);
+        if (r < i && nw > t) ++at;
+    }
+    return at;
+}
+// Warp-synchronous gather of every lane's first min(nw, cap) U words into row[0..cap) (row = this lane's
+// scratch, any memory space).  All 32 lanes must call it.
+__device__ inline void gather_u_words(const uint32_t* uarea, uint32_t nw, int lane, uint32_t* row, uint32_t cap) {
+    uint32_t maxnw = nw;
+#pragma unroll
+    for (int o = 16; o; o >>= 1) maxnw = max(maxnw, __shfl_xor_sync(0xffffffffu, maxnw, o));
+    uint32_t base = 0;
+    for (uint32_t t = 0; t < min(maxnw, cap); ++t) {
+        const bool has = nw > t;
+        const uint32_t m = __ballot_sync(0xffffffffu, has);
+        if (has) row[t] = uarea[base + __popc(m & ((1u << lane) - 1u))];
+        base += __popc(m);
+    }
+}
+// word accessor of a weight row: the first `cap` words from the gathered scratch, later ones by the slow index
+struct WordsRowU {
+    const uint32_t* row;     // gathered words
+    const uint32_t* uarea;
+    const uint16_t* ulen_hdr;
+    uint32_t nw, cap;
+    int lane;
+    __device__ inline uint32_t operator()(uint32_t t) const {
+        if (t >= nw) return 0u;
+        if (t < cap) return row[t];
+        return uarea[u_word_index_slow(ulen_hdr, lane, t)];
+    }
+};
+struct WordsRowR {  // R words of row `lane`, interleaved over the 32 rows
+    const uint32_t* rarea;
+    int lane, rw_words;
+    __device__ inline uint32_t operator()(uint32_t j) const { return j < (uint32_t)rw_words ? rarea[j * 32 + lane] : 0u; }
+};
 
 // exclusive prefix sum of the 128 ulen of a group; thread i gets its row's U-section start.
 // scan_smem: 4 words. All 128 threads of the (sub)block call it; 

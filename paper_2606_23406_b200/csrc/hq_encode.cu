@@ -266,10 +266,13 @@ __device__ inline uint32_t tile_ulen(const int8_t* codes, int n, int k0, int k1)
     return L;
 }
 
+constexpr uint32_t W_ULEN_MAX = 8160;  // FORMAT §5: 255 words per row
+
+// ulen_tmp[sg*32 + i], sg = (rb*n_kt + kt)*4 + w, row = 128 rb + 32 w + i (0 for absent rows)
 template <int LAT>
 __global__ void k_tile_ulen(const int8_t* codes, int64_t m, int64_t n_kt, int n, int k0, int k1, int64_t G,
                             uint16_t* ulen_tmp, int* err_flag) {
-    int64_t idx = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;  // g*128 + i
+    int64_t idx = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;  // g*128 + (w*32 + i)
     if (idx >= G * 128) return;
     int64_t g = idx >> 7;
     int i = (int)(idx & 127);
@@ -277,7 +280,7 @@ __global__ void k_tile_ulen(const int8_t* codes, int64_t m, int64_t n_kt, int n,
     uint32_t L = 0;
     if (r < m) {
         L = tile_ulen<LAT>(codes + r * (n_kt * n) + kt * n, n, k0, k1);
-        if (L > 65535u) { atomicExch(err_flag, 1); L = 65535u; }
+        if (L > W_ULEN_MAX) { atomicExch(err_flag, 1); L = W_ULEN_MAX; }
     }
     ulen_tmp[idx] = (uint16_t)L;
 }
@@ -295,11 +298,11 @@ void launch_tile_ulen(const int8_t* codes, int64_t m, int64_t n_in, int lattice,
 }
 
 // ---------------------------------------------------------------------------------------------
-// Group offsets: device prefix sum over the groups' sizes (north_star (a); FORMAT §5).
-// One block; each thread sums its groups' 128 ulen, block scan in chunks of 1024 groups.
+// Sub-group offsets: device prefix sum over the sub-groups' sizes (north_star (a); FORMAT §5).
+// One block; each thread sizes one sub-group from its 32 ulen, block scan in chunks of 1024.
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(1024)
-k_group_offsets(const uint16_t* ulen_tmp, int64_t G, int rbits, uint32_t* group_off, unsigned long long* totals,
+k_group_offsets(const uint16_t* ulen_tmp, int64_t G4, int rw_words, uint32_t* group_off, unsigned long long* totals,
                 uint32_t* max_group16) {
     __shared__ uint32_t warp_sums[32];
     __shared__ uint32_t carry_s;
@@ -308,21 +311,23 @@ k_group_offsets(const uint16_t* ulen_tmp, int64_t G, int rbits, uint32_t* group_
     int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid == 0) { carry_s = 0; ubits_total = 0; maxg = 0; }
     __syncthreads();
-    uint32_t r16 = (uint32_t)((128 * (int64_t)rbits + 127) / 128);
-    for (int64_t base = 0; base < G; base += 1024) {
+    for (int64_t base = 0; base < G4; base += 1024) {
         int64_t g = base + tid;
-        uint32_t size16 = 0, ub = 0;
-        if (g < G) {
-            const uint4* p = (const uint4*)(ulen_tmp + g * 128);  // 256 bytes
-            for (int v = 0; v < 16; ++v) {
+        uint32_t size16 = 0, ub = 0, uw = 0;
+        if (g < G4) {
+            const uint4* p = (const uint4*)(ulen_tmp + g * 32);  // 64 bytes
+            for (int v = 0; v < 4; ++v) {
                 uint4 w = p[v];
                 uint32_t ws[4] = {w.x, w.y, w.z, w.w};
 #pragma unroll
-                for (int e = 0; e < 4; ++e) ub += (ws[e] & 0xffffu) + (ws[e] >> 16);
+                for (int e = 0; e < 4; ++e) {
+                    uint32_t a = ws[e] & 0xffffu, b = ws[e] >> 16;
+                    ub += a + b;
+                    uw += ((a + 31) >> 5) + ((b + 31) >> 5);
+                }
             }
-            size16 = 32 + r16 + (ub + 127) / 128;
+            size16 = (128 + 4 * ((uint32_t)rw_words * 32 + uw) + 15) / 16;
         }
-        // inclusive scan of size16 over the block
         uint32_t x = size16;
         for (int o = 1; o < 32; o <<= 1) {
             uint32_t y = __shfl_up_sync(0xffffffffu, x, o);
@@ -331,16 +336,16 @@ k_group_offsets(const uint16_t* ulen_tmp, int64_t G, int rbits, uint32_t* group_
         if (lane == 31) warp_sums[warp] = x;
         __syncthreads();
         if (warp == 0) {
-            uint32_t s = warp_sums[lane];
+            uint32_t sv = warp_sums[lane];
             for (int o = 1; o < 32; o <<= 1) {
-                uint32_t y = __shfl_up_sync(0xffffffffu, s, o);
-                if (lane >= o) s += y;
+                uint32_t y = __shfl_up_sync(0xffffffffu, sv, o);
+                if (lane >= o) sv += y;
             }
-            warp_sums[lane] = s;
+            warp_sums[lane] = sv;
         }
         __syncthreads();
         uint32_t incl = x + (warp ? warp_sums[warp - 1] : 0) + carry_s;
-        if (g < G) {
+        if (g < G4) {
             group_off[g] = incl - size16;
             atomicAdd(&ubits_total, (unsigned long long)ub);
             atomicMax(&maxg, size16);
@@ -350,34 +355,35 @@ k_group_offsets(const uint16_t* ulen_tmp, int64_t G, int rbits, uint32_t* group_
         __syncthreads();
     }
     if (tid == 0) {
-        group_off[G] = carry_s;
+        group_off[G4] = carry_s;
         totals[0] = ubits_total;
         *max_group16 = maxg;
     }
 }
 
-void launch_group_offsets(const uint16_t* ulen_tmp, int64_t G, int rbits, uint32_t* group_off,
+void launch_group_offsets(const uint16_t* ulen_tmp, int64_t G4, int rw_words, uint32_t* group_off,
                           unsigned long long* totals, uint32_t* max_group16, cudaStream_t st) {
-    k_group_offsets<<<1, 1024, 0, st>>>(ulen_tmp, G, rbits, group_off, totals, max_group16);
+    k_group_offsets<<<1, 1024, 0, st>>>(ulen_tmp, G4, rw_words, group_off, totals, max_group16);
 }
 
 // ---------------------------------------------------------------------------------------------
-// Bit packing.  A per-thread writer that assembles 32-bit words of an MSB-first stream and ORs
-// them into a zero-initialized area (neighbouring rows share boundary words -> atomicOr).
+// Bit packing.  A per-thread writer that assembles the 32-bit words of an MSB-first stream and hands
+// every non-zero word to `store(word_index, value)` exactly once (destinations are zero-initialized).
 // ---------------------------------------------------------------------------------------------
+template <class Store>
 struct BitWriter {
-    uint32_t* area;
+    Store store;
     uint32_t pos;   // next stream bit
     uint32_t cur;   // bits of the current word accumulated so far (already positioned)
-    __device__ BitWriter(uint32_t* a, uint32_t p) : area(a), pos(p), cur(0) {}
+    __device__ BitWriter(Store s, uint32_t p) : store(s), pos(p), cur(0) {}
     __device__ inline void flush_word() {
-        if (cur) atomicOr(&area[(pos - 1) >> 5], cur);
+        if (cur) store((pos - 1) >> 5, cur);
         cur = 0;
     }
     // append nb (1..32) bits, value MSB-first
     __device__ inline void put(uint32_t v, int nb) {
-        int s = pos & 31;
-        int room = 32 - s;
+        int sft = pos & 31;
+        int room = 32 - sft;
         if (nb <= room) {
             cur |= (nb == 32) ? v : (v << (room - nb));
             pos += nb;
@@ -399,19 +405,23 @@ struct BitWriter {
         pos = np;
     }
     __device__ inline void finish() {
-        if (pos & 31) { if (cur) atomicOr(&area[pos >> 5], cur); cur = 0; }
+        if (pos & 31) { if (cur) store(pos >> 5, cur); cur = 0; }
     }
 };
+struct StoreAtomicOr {  // streams that share boundary words with their neighbours (KV container, FORMAT §6)
+    uint32_t* area;
+    __device__ inline void operator()(uint32_t i, uint32_t v) const { atomicOr(&area[i], v); }
+};
 
-// R-section of a tile (FORMAT §4 field planes) from its symbols z[0..n) (smem/local pointer).
-template <int LAT>
-__device__ inline void write_R(BitWriter& bw, const uint8_t* z, int n, int k0, int k1) {
+// R-section of a tile (FORMAT §4 field planes) from its symbols z[0..n) in stream order.
+template <int LAT, class BW>
+__device__ inline void write_R(BW& bw, const uint8_t* z, int n, int k0, int k1) {
     const int nclass = (LAT == LAT_D4 || LAT == LAT_A2) ? 2 : 1;
     for (int a = 0; a < nclass; ++a) {
         int ka = a ? k1 : k0;
         if (ka == 0) continue;
         int na = class_count(LAT, n, a);
-        // j of the m-th symbol of class a
+        // stream position of the m-th symbol of class a
         auto sym_at = [&](int mi) -> uint32_t {
             int j;
             if (LAT == LAT_D4) j = a ? 4 * mi + 3 : (mi / 3) * 4 + (mi % 3);
@@ -447,8 +457,8 @@ __device__ inline void write_R(BitWriter& bw, const uint8_t* z, int n, int k0, i
     bw.finish();
 }
 
-template <int LAT>
-__device__ inline void write_U(BitWriter& bw, const uint8_t* z, int n, int k0, int k1) {
+template <int LAT, class BW>
+__device__ inline void write_U(BW& bw, const uint8_t* z, int n, int k0, int k1) {
     for (int j = 0; j < n; ++j) {
         uint32_t q = (uint32_t)z[j] >> (sym_class(LAT, j) ? k1 : k0);
         bw.skip(q);
@@ -457,6 +467,7 @@ __device__ inline void write_U(BitWriter& bw, const uint8_t* z, int n, int k0, i
     bw.finish();
 }
 
+// symbols of a tile in stream order (FORMAT §3)
 template <int LAT>
 __device__ inline void tile_symbols(const int8_t* codes, int n, uint8_t* z) {
     for (int b = 0; b < n / LAT; ++b) {
@@ -465,54 +476,69 @@ __device__ inline void tile_symbols(const int8_t* codes, int n, uint8_t* z) {
         for (int i = 0; i < LAT; ++i) c[i] = codes[b * LAT + i];
         strip<LAT>(c, zz);
 #pragma unroll
-        for (int i = 0; i < LAT; ++i) z[b * LAT + i] = (uint8_t)zz[i];  // <= 255 by the INT8 pre-clamp (G8)
+        for (int i = 0; i < LAT; ++i) {  // <= 255 by the INT8 pre-clamp (G8)
+            int p = (LAT == LAT_E8) ? 32 * (b >> 2) + 8 * (i >> 1) + 2 * (b & 3) + (i & 1) : b * LAT + i;
+            z[p] = (uint8_t)zz[i];
+        }
     }
 }
 
-// one block (128 threads = 128 rows) per group; blob zero-initialized by the caller
+// one block (128 threads = 128 rows = four sub-groups, one per warp) per (rb, kt); blob zero-initialized
+constexpr uint32_t PACK_UCAP = 24;  // U words per row gathered through shared memory; longer rows go the slow way
 template <int LAT>
 __global__ void __launch_bounds__(128)
 k_pack_groups(const int8_t* codes, const uint16_t* norms, const uint16_t* ulen_tmp, int64_t m, int64_t n_kt,
               int n, int k0, int k1, const uint32_t* group_off, uint8_t* blob) {
-    extern __shared__ uint8_t zs[];  // [128][n+4]  (+4: de-conflict banks)
-    __shared__ uint32_t scan[128];
+    extern __shared__ uint8_t zs[];  // [128][n+4] symbols (+4: de-conflict banks) | [128][PACK_UCAP+1] U words
     int64_t g = blockIdx.x;
-    int i = threadIdx.x;
-    int64_t rb = g / n_kt, kt = g % n_kt, r = rb * 128 + i;
+    int t = threadIdx.x, lane = t & 31, warp = t >> 5;
+    int64_t rb = g / n_kt, kt = g % n_kt, r = rb * 128 + t;
     int rbits = rbits_of(LAT, n, k0, k1);
-    uint32_t r16 = (uint32_t)((128 * (int64_t)rbits + 127) / 128);
-    uint8_t* base = blob + 16 * (int64_t)group_off[g];
+    int rw_words = (rbits + 31) / 32;
+    uint8_t* base = blob + 16 * (int64_t)group_off[g * 4 + warp];
     uint16_t* h_ulen = (uint16_t*)base;
-    uint16_t* h_norm = h_ulen + 128;
-    uint32_t* rarea = (uint32_t*)(base + 512);
-    uint32_t* uarea = (uint32_t*)(base + 512 + 16 * (int64_t)r16);
-    uint32_t ul = ulen_tmp[g * 128 + i];
-    h_ulen[i] = (uint16_t)ul;
-    h_norm[i] = (r < m) ? norms[r * n_kt + kt] : (uint16_t)0;
-    // exclusive prefix of ulen over the group's rows
-    scan[i] = ul;
-    __syncthreads();
-    for (int o = 1; o < 128; o <<= 1) {
-        uint32_t v = (i >= o) ? scan[i - o] : 0;
-        __syncthreads();
-        scan[i] += v;
-        __syncthreads();
+    uint16_t* h_norm = h_ulen + 32;
+    uint32_t* rarea = (uint32_t*)(base + 128);
+    uint32_t* uarea = rarea + rw_words * 32;
+    const uint16_t* ulen_sg = ulen_tmp + (g * 4 + warp) * 32;
+    uint32_t ul = ulen_sg[lane];
+    uint32_t nw = (ul + 31) >> 5;
+    h_ulen[lane] = (uint16_t)ul;
+    h_norm[lane] = (r < m) ? norms[r * n_kt + kt] : (uint16_t)0;
+    uint32_t* urow = (uint32_t*)(zs + 128 * (size_t)(n + 4)) + t * (PACK_UCAP + 1);
+    for (uint32_t i = 0; i < PACK_UCAP; ++i) urow[i] = 0;
+    if (r < m) {
+        uint8_t* z = zs + t * (n + 4);
+        tile_symbols<LAT>(codes + r * (n_kt * n) + kt * n, n, z);
+        auto store_r = [&](uint32_t i, uint32_t v) { rarea[i * 32 + lane] = v; };
+        BitWriter<decltype(store_r)> bwr(store_r, 0u);
+        write_R<LAT>(bwr, z, n, k0, k1);
+        auto store_u = [&](uint32_t i, uint32_t v) {
+            if (i < PACK_UCAP) urow[i] = v;
+            else uarea[u_word_index_slow(ulen_sg, lane, i)] = v;
+        };
+        BitWriter<decltype(store_u)> bwu(store_u, 0u);
+        write_U<LAT>(bwu, z, n, k0, k1);
     }
-    uint32_t ustart = scan[i] - ul;
-    if (r >= m) return;
-    uint8_t* z = zs + i * (n + 4);
-    tile_symbols<LAT>(codes + r * (n_kt * n) + kt * n, n, z);
-    BitWriter bwr(rarea, (uint32_t)i * (uint32_t)rbits);
-    write_R<LAT>(bwr, z, n, k0, k1);
-    BitWriter bwu(uarea, ustart);
-    write_U<LAT>(bwu, z, n, k0, k1);
+    __syncwarp();
+    // scatter the gathered words into the compacted word-rows
+    uint32_t maxnw = nw;
+#pragma unroll
+    for (int o = 16; o; o >>= 1) maxnw = max(maxnw, __shfl_xor_sync(0xffffffffu, maxnw, o));
+    uint32_t at = 0;
+    for (uint32_t w = 0; w < min(maxnw, PACK_UCAP); ++w) {
+        const bool has = nw > w;
+        const uint32_t mk = __ballot_sync(0xffffffffu, has);
+        if (has) uarea[at + __popc(mk & ((1u << lane) - 1u))] = urow[w];
+        at += __popc(mk);
+    }
 }
 
 void launch_pack_groups(const int8_t* codes, const uint16_t* norms, const uint16_t* ulen_tmp, int64_t m,
                         int64_t n_in, int lattice, int n, int k0, int k1, const uint32_t* group_off,
                         uint8_t* blob, cudaStream_t st) {
     int64_t n_kt = n_in / n, n_rb = (m + 127) / 128, G = n_rb * n_kt;
-    size_t smem = 128 * (size_t)(n + 4);
+    size_t smem = 128 * (size_t)(n + 4) + 128 * (size_t)(PACK_UCAP + 1) * 4;
 #define HQ_LAUNCH_P(L)                                                                                          \
     k_pack_groups<L><<<(unsigned)G, 128, smem, st>>>(codes, norms, ulen_tmp, m, n_kt, n, k0, k1, group_off, blob)
     switch (lattice) {
@@ -580,9 +606,9 @@ k_kv_pack(const int8_t* codes, int64_t n_tok, int H, int d, int64_t token0, int 
     int h = (int)(idx % H);
     uint8_t* z = zs + threadIdx.x * (d + 4);
     tile_symbols<LAT>(codes + idx * d, d, z);
-    BitWriter bwr(rem + h * rem_words, (uint32_t)((token0 + t) * rbits));
+    BitWriter<StoreAtomicOr> bwr(StoreAtomicOr{rem + h * rem_words}, (uint32_t)((token0 + t) * rbits));
     write_R<LAT>(bwr, z, d, k0, k1);
-    BitWriter bwu(una + h * una_words, ustart_tmp[h * n_tok + t]);
+    BitWriter<StoreAtomicOr> bwu(StoreAtomicOr{una + h * una_words}, ustart_tmp[h * n_tok + t]);
     write_U<LAT>(bwu, z, d, k0, k1);
 }
 

@@ -32,7 +32,7 @@ struct hq_weight {
     int64_t n_kt, n_rb, G;
     int rbits;
     uint8_t* blob;        // dev
-    uint32_t* group_off;  // dev [G+1]
+    uint32_t* group_off;  // dev [4G+1]  sub-group offsets (FORMAT §5)
     int8_t* dsign;        // dev [n_in]  RHT signs (+1/-1)
     int64_t blob_bytes, payload_bits, clamp_count;
     uint32_t max_group16;  // largest group size in 16-byte units
@@ -88,11 +88,11 @@ void launch_quantize_kv(const void* x, int64_t n_tok, int H, int d, int64_t toke
 // activations: x [B, n_in] -> q int8 [B, n_in], s_x [B, n_kt], optional u
 void launch_act_quant(const void* x, int dtype, int64_t B, int64_t n_in, int64_t ldx, int lattice, int n,
                       const int8_t* dsign, int8_t* q, float* s_x, float* u, cudaStream_t st);
-// ulen_tmp[g*128 + i] for all groups (0 for absent rows); err_flag set if a tile overflows u16
+// ulen_tmp[sg*32 + i] for all sub-groups (0 for absent rows); err_flag set if a tile exceeds 8160 bits
 void launch_tile_ulen(const int8_t* codes, int64_t m, int64_t n_in, int lattice, int n, int k0, int k1,
                       uint16_t* ulen_tmp, int* err_flag, cudaStream_t st);
-// group_off[G+1] (16-byte units) by a device prefix sum; totals[0] = sum of ulen over all tiles
-void launch_group_offsets(const uint16_t* ulen_tmp, int64_t G, int rbits, uint32_t* group_off,
+// group_off[G4+1] (sub-group offsets, 16-byte units) by a device prefix sum; totals[0] = sum of ulen over all tiles
+void launch_group_offsets(const uint16_t* ulen_tmp, int64_t G4, int rw_words, uint32_t* group_off,
                           unsigned long long* totals, uint32_t* max_group16, cudaStream_t st);
 void launch_pack_groups(const int8_t* codes, const uint16_t* norms, const uint16_t* ulen_tmp, int64_t m,
                         int64_t n_in, int lattice, int n, int k0, int k1, const uint32_t* group_off,
