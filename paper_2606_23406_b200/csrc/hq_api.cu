@@ -7,6 +7,7 @@
 #include <vector>
 
 #include "hq_common.cuh"
+#include "hq_e8_decode.cuh"
 #include "hq_internal.h"
 
 using namespace hq;
@@ -50,6 +51,18 @@ hq_status hq_create(hq_ctx** out, const hq_allocator* alloc, int cuda_device) {
     ctx->device = cuda_device;
     ctx->sm_count = prop.multiProcessorCount;
     ctx->err = "";
+    // phase-1 table of the E8 fast decoder: [parity][byte][copy] (hq_e8_decode.cuh)
+    std::vector<uint32_t> lut(E8_LUT_WORDS);
+    for (int par = 0; par < 2; ++par)
+        for (int b = 0; b < 256; ++b)
+            for (int c = 0; c < E8_LUT_COPIES; ++c) lut[(par * 256 + b) * E8_LUT_COPIES + c] = unary_lut_entry(b, par);
+    ctx->e8_lut = (uint32_t*)ctx_alloc(ctx, E8_LUT_BYTES);
+    if (!ctx->e8_lut) { delete ctx; return HQ_ERR_ALLOC; }
+    if (cudaMemcpy(ctx->e8_lut, lut.data(), E8_LUT_BYTES, cudaMemcpyHostToDevice) != cudaSuccess) {
+        ctx_free(ctx, ctx->e8_lut);
+        delete ctx;
+        return HQ_ERR_CUDA;
+    }
     *out = ctx;
     return HQ_OK;
 }
@@ -57,6 +70,7 @@ hq_status hq_create(hq_ctx** out, const hq_allocator* alloc, int cuda_device) {
 void hq_destroy(hq_ctx* ctx) {
     if (!ctx) return;
     ctx_free(ctx, ctx->ws);
+    ctx_free(ctx, ctx->e8_lut);
     delete ctx;
 }
 
@@ -254,18 +268,9 @@ hq_status hq_act_quant(hq_ctx* ctx, const hq_weight* w, const void* x_dev, int32
     return HQ_OK;
 }
 
-static size_t linear_ws_bytes(const hq_ctx* ctx, const hq_weight* w, int64_t B, int* n_split_out) {
-    int ns = linear_choose_split(ctx, w, B);
-    if (n_split_out) *n_split_out = ns;
-    size_t q = ((size_t)(B * w->n_in) + 255) & ~(size_t)255;
-    size_t sx = ((size_t)(B * w->n_kt) * 4 + 255) & ~(size_t)255;
-    size_t part = (size_t)ns * B * w->m * 4;
-    return q + sx + part + 256;
-}
-
 hq_status hq_linear_workspace_bytes(const hq_weight* w, int64_t batch, size_t* bytes) {
     if (!w || !bytes || batch <= 0) return HQ_ERR_INVALID_ARG;
-    *bytes = linear_ws_bytes(w->ctx, w, batch, nullptr);
+    *bytes = linear_workspace_bytes(w->ctx, w, batch);
     return HQ_OK;
 }
 
@@ -276,8 +281,7 @@ hq_status hq_linear(hq_ctx* ctx, const hq_weight* w, const void* x_dev, int32_t 
     if (batch <= 0 || ldx < w->n_in || (y_bf16_dev && ldy < w->m)) return fail(ctx, HQ_ERR_SHAPE, "bad batch / ldx / ldy");
     if (dtype != HQ_F32 && dtype != HQ_BF16) return fail(ctx, HQ_ERR_INVALID_ARG, "bad dtype");
     cudaStream_t st = (cudaStream_t)stream;
-    int n_split = 1;
-    size_t need = linear_ws_bytes(ctx, w, batch, &n_split);
+    size_t need = linear_workspace_bytes(ctx, w, batch);
     if (need > ctx->ws_bytes) {
         // the old buffer may still be in use by work already enqueued
         if (ctx->ws) { HQ_CUDA_CHECK(ctx, cudaDeviceSynchronize()); ctx_free(ctx, ctx->ws); ctx->ws = nullptr; ctx->ws_bytes = 0; }
@@ -285,16 +289,8 @@ hq_status hq_linear(hq_ctx* ctx, const hq_weight* w, const void* x_dev, int32_t 
         if (!ctx->ws) return HQ_ERR_ALLOC;
         ctx->ws_bytes = need;
     }
-    uint8_t* base = (uint8_t*)ctx->ws;
-    int8_t* q = (int8_t*)base;
-    size_t qb = ((size_t)(batch * w->n_in) + 255) & ~(size_t)255;
-    float* s_x = (float*)(base + qb);
-    size_t sb = ((size_t)(batch * w->n_kt) * 4 + 255) & ~(size_t)255;
-    float* partials = (float*)(base + qb + sb);
-    launch_act_quant(x_dev, dtype, batch, w->n_in, ldx, w->lattice, w->n, w->dsign, q, s_x, nullptr, st);
-    HQ_CUDA_CHECK(ctx, cudaGetLastError());
-    return launch_linear(ctx, w, q, s_x, batch, y_bf16_dev, ldy, y_f32_dev_or_null, acc_i32_dev_or_null, partials,
-                         n_split, st);
+    return launch_linear(ctx, w, x_dev, dtype, batch, ldx, y_bf16_dev, ldy, y_f32_dev_or_null, acc_i32_dev_or_null,
+                         (uint8_t*)ctx->ws, st);
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -1,0 +1,111 @@
+// hq_e8_decode.cuh — the fast E8 tile decoder (hard part H1).
+//
+// One lane owns one row of a sub-group (FORMAT §5): its U words and R words arrive in registers by
+// coalesced loads.  Two phases, both branch-free in the common case:
+//
+//  phase 1 (unary, §3.3): the row's U-section is walked 8 stream bits at a time.  A 256-entry table
+//    maps a byte to the positions (mod 16, one nibble each, in order) of its one bits — every one bit
+//    terminates a symbol.  The nibbles are appended to a per-row nibble stream in shared memory
+//    (8 symbols per 32-bit word); no per-symbol loop, no clz.
+//  phase 2 (remainders + un-strip, §4.6): per run of 32 symbols = four E8 blocks in FORMAT §3's
+//    coordinate-pair order.  The unary quotient of a symbol is the gap between consecutive terminators,
+//    q_j = (e_j - e_{j-1} - 1) mod 16 (exact for q <= 15); all further steps are SWAR on one register of
+//    four bytes = ONE coordinate of FOUR blocks: z = (q << k) | r with r from the R-section field planes
+//    (one shift + one mask per 4 symbols), c_i = (z ^ signfill) | coset, the block parity as a 7-input
+//    XOR, the comb symbol (coordinate 7) as one more register.
+//  A row with a quotient >= 16 or more than NW words is flagged and re-decoded by the generic decoder.
+//
+// Output: per run c, registers C[0..7], byte b of C[i] = code c_i of block 4c + b: the A operand's K
+// index inside the tile is 32c + 4i + b, and the activation operand is stored in the same order.
+#pragma once
+#include "hq_common.cuh"
+
+namespace hq {
+
+constexpr int E8_LUT_COPIES = 16;                                  // replicas per entry: lane l uses copy l & 15
+constexpr int E8_LUT_WORDS = 2 * 256 * E8_LUT_COPIES;              // [parity][byte][copy]
+constexpr int E8_LUT_BYTES = E8_LUT_WORDS * 4;                     // 32 KB
+
+// table entry for stream byte `b` (bit 7 first) and byte parity: nibble j = position of the j-th one + 8*par
+__host__ __device__ inline uint32_t unary_lut_entry(uint32_t b, uint32_t par) {
+    uint32_t v = 0, j = 0;
+    for (int pos = 0; pos < 8; ++pos)
+        if (b & (0x80u >> pos)) { v |= (uint32_t)(pos + 8 * par) << (4 * j); ++j; }
+    return v;
+}
+
+// phase 1 for one stream word x (4 bytes, byte 0 = bits 31..24).  `lut_lane` = this lane's copy of entry 0 /
+// parity 0 in shared memory.  State: acc (partial nibble word), fs (bits used in acc, 0..28), wo (next nibble
+// word of this row in shared memory).
+__device__ __forceinline__ void e8_unary_word(uint32_t x, const uint32_t* lut_lane, uint32_t& acc, uint32_t& fs,
+                                              uint32_t*& wo) {
+    uint32_t N[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const uint32_t sel = (i < 3) ? ((x >> (18 - 8 * i)) & 0x3fc0u) : ((x << 6) & 0x3fc0u);   // byte * 64
+        N[i] = *(const uint32_t*)((const char*)lut_lane + sel + ((i & 1) ? 256 * E8_LUT_COPIES * 4 : 0));
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const uint32_t c4 = 4u * (uint32_t)__popc(x & (0xff000000u >> (8 * i)));
+        const uint32_t out0 = acc | (N[i] << fs);
+        const uint32_t out1 = __funnelshift_l(N[i], 0u, fs);  // the bits of N shifted out past bit 31 (fs < 32)
+        const uint32_t fs2 = fs + c4;
+        const bool full = fs2 >= 32u;
+        if (full) *wo++ = out0;
+        acc = full ? out1 : out0;
+        fs = fs2 & 31u;
+    }
+}
+
+// the K-bit remainders of symbol group g (0..7 = coordinate) of a 32-symbol run whose K field-plane words are
+// V[0..K)  (FORMAT §4): byte b = block b of the run
+template <int K>
+__device__ __forceinline__ uint32_t e8_rem4(const uint32_t* V, int g) {
+    uint32_t r = 0;
+    int lo = 0;
+#pragma unroll
+    for (int b = 0; b < 3; ++b) {
+        const int wd = 1 << b;
+        if (!(K & wd)) continue;
+        const int per = 8 / wd;
+        const uint32_t mask = ((1u << wd) - 1u) * 0x01010101u;
+        r |= ((V[lo + g / per] >> (wd * (g % per))) & mask) << lo;
+        lo += wd;
+    }
+    return r;
+}
+
+// phase 2 for one run of 32 symbols: nibble words W[0..3], remainder words V[0..K) -> C[0..7].
+// prevWo carries the last odd-position word (for the gap of the next even positions); qsum accumulates
+// all quotients of the row byte-wise (caller widens).
+template <int K>
+__device__ __forceinline__ void e8_run(const uint32_t* W, const uint32_t* V, uint32_t& prevWo, uint32_t& qsum, uint32_t* C) {
+    uint32_t Z[8];
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+        const uint32_t We = W[w] & 0x0f0f0f0fu, Wo = (W[w] >> 4) & 0x0f0f0f0fu;
+        const uint32_t prev = __funnelshift_l(prevWo, Wo, 8);  // (Wo << 8) | (prevWo >> 24)
+        const uint32_t qe = (We + 0x1f1f1f1fu - prev) & 0x0f0f0f0fu;
+        const uint32_t qo = (Wo + 0x1f1f1f1fu - We) & 0x0f0f0f0fu;
+        prevWo = Wo;
+        qsum += qe + qo;
+        Z[2 * w] = qe * (1u << K) + e8_rem4<K>(V, 2 * w);
+        Z[2 * w + 1] = qo * (1u << K) + e8_rem4<K>(V, 2 * w + 1);
+    }
+    // un-strip (§4.6): Z[7] is comb = 2*zigzag(t) + coset (L274); every other Z[i] is zigzag(s_i)
+    const uint32_t coset4 = Z[7] & 0x01010101u;
+    uint32_t P = 0;
+#pragma unroll
+    for (int i = 0; i < 7; ++i) {
+        const uint32_t fill = (Z[i] & 0x01010101u) * 0xffu;
+        const uint32_t c2 = Z[i] ^ fill;  // 2 s_i (bit 0 clear)
+        P ^= c2;
+        C[i] = c2 | coset4;               // c_i = 2 s_i + coset
+    }
+    const uint32_t zt = (Z[7] >> 1) & 0x7f7f7f7fu;            // zigzag(t)
+    const uint32_t t2 = zt ^ ((zt & 0x01010101u) * 0xffu);     // 2 t
+    C[7] = ((t2 << 1) & 0xfefefefeu) | (P & 0x02020202u) | coset4;  // c_7 = 4 t + 2 parity + coset
+}
+
+}  // namespace hq

@@ -240,6 +240,60 @@ k_act_quant(const void* X, int dtype, int64_t n_tiles, int64_t n_kt, int64_t ldx
     }
 }
 
+// Same arithmetic as k_act_quant, output as the B operand tiles of the E8 fused kernel: for batch tile bt and
+// K-tile kt a blob of NB rows x 128 bytes in K-major SWIZZLE_128B order, the K index permuted like the decoded
+// weights (e8_kcol: 32c + 4i + b for block 4c+b, coordinate i), followed by NB fp32 scales s_x.  n = 128.
+__global__ void __launch_bounds__(QW_WARPS * 32)
+k_act_blob(const void* X, int dtype, int64_t B, int64_t n_kt, int64_t ldx, const int8_t* dsign, int NB,
+           uint8_t* bblob) {
+    extern __shared__ float smem[];
+    const int n = 128;
+    int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    float* u = smem + warp * n;
+    const int64_t n_bt = (B + NB - 1) / NB, n_tiles = n_bt * NB * n_kt;
+    const uint32_t blob_bytes = (uint32_t)(NB * 128 + NB * 4);
+    for (int64_t tile = blockIdx.x * (int64_t)QW_WARPS + warp; tile < n_tiles; tile += (int64_t)gridDim.x * QW_WARPS) {
+        int64_t b = tile / n_kt, kt = tile % n_kt;   // b runs over the padded batch n_bt*NB
+        int64_t bt = b / NB;
+        int bb = (int)(b % NB);
+        uint8_t* blob = bblob + (bt * n_kt + kt) * (int64_t)blob_bytes;
+        float* sx = (float*)(blob + NB * 128);
+        float amax = 0.0f;
+        if (b < B) {
+            for (int i = lane; i < n; i += 32) {
+                float x = load_elem(X, dtype, b * ldx + kt * n + i);
+                u[i] = (dsign[kt * n + i] < 0) ? -x : x;
+            }
+            warp_rht_inplace(u, n, lane);
+            for (int i = lane; i < n; i += 32) amax = fmaxf(amax, fabsf(u[i]));
+            for (int s = 16; s; s >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, s));
+        }
+        __syncwarp();
+        const float inv = (amax == 0.0f) ? 0.0f : __fdiv_rn(127.0f, amax);
+        for (int i = lane; i < n; i += 32) {
+            int qv = 0;
+            if (amax != 0.0f) {
+                float v = rintf(__fmul_rn(u[i], inv));
+                v = fminf(fmaxf(v, -127.0f), 127.0f);
+                qv = (int)v;
+            }
+            const int blk = i >> 3, ci = i & 7;
+            const int col = 32 * (blk >> 2) + 4 * ci + (blk & 3);
+            blob[(bb >> 3) * 1024 + (bb & 7) * 128 + ((((col >> 4) ^ (bb & 7)) << 4) | (col & 15))] = (uint8_t)(int8_t)qv;
+        }
+        if (lane == 0) sx[bb] = (amax == 0.0f) ? 0.0f : __fdiv_rn(amax, 127.0f);
+        __syncwarp();
+    }
+}
+
+void launch_act_blob(const void* x, int dtype, int64_t B, int64_t n_in, int64_t ldx, const int8_t* dsign, int NB,
+                     uint8_t* bblob, cudaStream_t st) {
+    int64_t n_kt = n_in / 128, n_bt = (B + NB - 1) / NB, n_tiles = n_bt * NB * n_kt;
+    int64_t blocks = (n_tiles + QW_WARPS - 1) / QW_WARPS;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    k_act_blob<<<(unsigned)blocks, QW_WARPS * 32, QW_WARPS * 128 * sizeof(float), st>>>(x, dtype, B, n_kt, ldx, dsign, NB, bblob);
+}
+
 void launch_act_quant(const void* x, int dtype, int64_t B, int64_t n_in, int64_t ldx, int lattice, int n,
                       const int8_t* dsign, int8_t* q, float* s_x, float* u, cudaStream_t st) {
     int64_t n_kt = n_in / n, n_tiles = B * n_kt;

@@ -13,9 +13,10 @@ struct hq_ctx {
     int device;
     int sm_count;
     std::string err;
-    // cached scratch for hq_linear (q, s_x, split-K partials)
+    // cached scratch for hq_linear (activation operand, split-K partials)
     void* ws = nullptr;
     size_t ws_bytes = 0;
+    uint32_t* e8_lut = nullptr;  // dev: phase-1 table of the E8 fast decoder (hq_e8_decode.cuh)
     // optional kernel timing (hq_profile_*): event pairs around the dominant kernel of each call
     bool prof = false;
     std::vector<cudaEvent_t> prof_ev;
@@ -88,6 +89,9 @@ void launch_quantize_kv(const void* x, int64_t n_tok, int H, int d, int64_t toke
 // activations: x [B, n_in] -> q int8 [B, n_in], s_x [B, n_kt], optional u
 void launch_act_quant(const void* x, int dtype, int64_t B, int64_t n_in, int64_t ldx, int lattice, int n,
                       const int8_t* dsign, int8_t* q, float* s_x, float* u, cudaStream_t st);
+// activations as the E8 fused kernel's B operand tiles (UMMA layout, permuted K, + scales); n_tile = 128
+void launch_act_blob(const void* x, int dtype, int64_t B, int64_t n_in, int64_t ldx, const int8_t* dsign, int NB,
+                     uint8_t* bblob, cudaStream_t st);
 // ulen_tmp[sg*32 + i] for all sub-groups (0 for absent rows); err_flag set if a tile exceeds 8160 bits
 void launch_tile_ulen(const int8_t* codes, int64_t m, int64_t n_in, int lattice, int n, int k0, int k1,
                       uint16_t* ulen_tmp, int* err_flag, cudaStream_t st);
@@ -107,10 +111,11 @@ void launch_kv_ring(const void* k, const void* v, int64_t n_tok, int H, int d, i
 
 // ---- decode + linear (hq_linear.cu) ----
 void launch_decode_int8(const hq_weight* w, int8_t* codes, uint16_t* norms, cudaStream_t st);
-hq_status launch_linear(hq_ctx* ctx, const hq_weight* w, const int8_t* q, const float* s_x, int64_t B,
-                        void* y_bf16, int64_t ldy, float* y_f32, int32_t* acc_i32, float* partials,
-                        int n_split, cudaStream_t st);
-int linear_choose_split(const hq_ctx* ctx, const hq_weight* w, int64_t B);
+// the whole of hq_linear after argument checks: activation cast, fused decode + MMA, split-K finalize
+hq_status launch_linear(hq_ctx* ctx, const hq_weight* w, const void* x, int dtype, int64_t B, int64_t ldx,
+                        void* y_bf16, int64_t ldy, float* y_f32, int32_t* acc_i32, uint8_t* ws, cudaStream_t st);
+size_t linear_workspace_bytes(const hq_ctx* ctx, const hq_weight* w, int64_t B);
+bool linear_uses_e8_fast(const hq_weight* w);
 
 // ---- KV decode + attend (hq_attend.cu) ----
 void launch_kv_decode_int8(const hq_kv* kv, int role, int64_t t0, int64_t n, int8_t* codes, cudaStream_t st);

@@ -6,6 +6,7 @@
 // §4.3).  Decoded weights never leave shared memory.
 #include "hq_common.cuh"
 #include "hq_internal.h"
+#include "hq_linear_e8.cuh"
 #include "hq_tc.cuh"
 
 namespace hq {
@@ -197,7 +198,7 @@ __global__ void k_linear_finalize(const float* partials, int n_split, int64_t B,
     if (y_f32) y_f32[idx] = s;
 }
 
-int linear_choose_split(const hq_ctx* ctx, const hq_weight* w, int64_t B) {
+static int generic_split(const hq_ctx* ctx, const hq_weight* w, int64_t B) {
     int NB = B <= 16 ? 16 : 64;
     int64_t n_bt = (B + NB - 1) / NB;
     int64_t items = w->n_rb * n_bt;
@@ -208,7 +209,7 @@ int linear_choose_split(const hq_ctx* ctx, const hq_weight* w, int64_t B) {
 }
 
 template <int NB>
-static hq_status launch_linear_nb(hq_ctx* ctx, const hq_weight* w, LinearParams& p, cudaStream_t st) {
+static hq_status launch_generic_nb(hq_ctx* ctx, const hq_weight* w, LinearParams& p, cudaStream_t st) {
     int n_atoms = (w->n + 127) / 128;
     int64_t n_bt = (p.B + NB - 1) / NB;
     int64_t grid = w->n_rb * n_bt * p.n_split;
@@ -230,22 +231,97 @@ static hq_status launch_linear_nb(hq_ctx* ctx, const hq_weight* w, LinearParams&
     return HQ_OK;
 }
 
-hq_status launch_linear(hq_ctx* ctx, const hq_weight* w, const int8_t* q, const float* s_x, int64_t B,
-                        void* y_bf16, int64_t ldy, float* y_f32, int32_t* acc_i32, float* partials, int n_split,
-                        cudaStream_t st) {
-    LinearParams p;
-    p.blob = w->blob; p.group_off = w->group_off; p.m = w->m; p.n_kt = w->n_kt;
-    p.n = w->n; p.k0 = w->k0; p.k1 = w->k1; p.rbits = w->rbits;
-    p.inv_A = (float)(1.0 / (w->alpha * sqrt((double)w->n)));
-    p.q = q; p.s_x = s_x; p.B = B; p.n_split = n_split; p.partials = partials; p.acc_i32 = acc_i32;
-    cudaEvent_t e0 = nullptr, e1 = nullptr;
-    if (ctx->prof) {
-        HQ_CUDA_CHECK(ctx, cudaEventCreate(&e0));
-        HQ_CUDA_CHECK(ctx, cudaEventCreate(&e1));
-        HQ_CUDA_CHECK(ctx, cudaEventRecord(e0, st));
+// ---- E8 fast path -----------------------------------------------------------------------------
+bool linear_uses_e8_fast(const hq_weight* w) { return w->lattice == LAT_E8 && w->n == 128 && w->k0 <= 3; }
+
+struct E8Plan { int NB, n_bt, n_split, L, n_items, grid; };
+static E8Plan e8_plan(const hq_ctx* ctx, const hq_weight* w, int64_t B) {
+    E8Plan pl;
+    pl.NB = B <= 16 ? 16 : 64;
+    pl.n_bt = (int)((B + pl.NB - 1) / pl.NB);
+    const int64_t GW = (int64_t)ctx->sm_count * E8_NWG;
+    const int n_kt = (int)w->n_kt;
+    int split = n_kt;  // the smallest divisor of n_kt that gives every warp group at least two items
+    for (int d = 1; d <= n_kt; ++d)
+        if (n_kt % d == 0 && w->n_rb * pl.n_bt * d >= 2 * GW) { split = d; break; }
+    pl.n_split = split;
+    pl.L = n_kt / split;
+    pl.n_items = (int)(w->n_rb * pl.n_bt * split);
+    int64_t ctas = (pl.n_items + E8_NWG - 1) / E8_NWG;
+    pl.grid = (int)(ctas < ctx->sm_count ? ctas : ctx->sm_count);
+    return pl;
+}
+
+template <int NB>
+static hq_status launch_e8_nb(hq_ctx* ctx, const hq_weight* w, E8Params& p, int grid, cudaStream_t st) {
+    const size_t smem = e8_smem_bytes<NB>();
+#define HQ_LE(KK)                                                                                                   \
+    case KK:                                                                                                        \
+        HQ_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_linear_e8<KK, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+        k_linear_e8<KK, NB><<<grid, E8_NWG * 128, smem, st>>>(p);                                                   \
+        break
+    switch (w->k0) {
+        HQ_LE(0); HQ_LE(1); HQ_LE(2); HQ_LE(3);
     }
-    hq_status s = (B <= 16) ? launch_linear_nb<16>(ctx, w, p, st) : launch_linear_nb<64>(ctx, w, p, st);
-    if (s != HQ_OK) return s;
+#undef HQ_LE
+    HQ_CUDA_CHECK(ctx, cudaGetLastError());
+    return HQ_OK;
+}
+
+static size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
+
+size_t linear_workspace_bytes(const hq_ctx* ctx, const hq_weight* w, int64_t B) {
+    if (linear_uses_e8_fast(w)) {
+        E8Plan pl = e8_plan(ctx, w, B);
+        return align256((size_t)pl.n_bt * w->n_kt * e8_bblob_bytes(pl.NB)) + (size_t)pl.n_split * B * w->m * 4 + 256;
+    }
+    int ns = generic_split(ctx, w, B);
+    return align256((size_t)(B * w->n_in)) + align256((size_t)(B * w->n_kt) * 4) + (size_t)ns * B * w->m * 4 + 256;
+}
+
+hq_status launch_linear(hq_ctx* ctx, const hq_weight* w, const void* x, int dtype, int64_t B, int64_t ldx,
+                        void* y_bf16, int64_t ldy, float* y_f32, int32_t* acc_i32, uint8_t* ws, cudaStream_t st) {
+    const float inv_A = (float)(1.0 / (w->alpha * sqrt((double)w->n)));
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    float* partials = nullptr;
+    int n_split = 1;
+    if (linear_uses_e8_fast(w)) {
+        E8Plan pl = e8_plan(ctx, w, B);
+        uint8_t* bblob = ws;
+        partials = (float*)(ws + align256((size_t)pl.n_bt * w->n_kt * e8_bblob_bytes(pl.NB)));
+        n_split = pl.n_split;
+        launch_act_blob(x, dtype, B, w->n_in, ldx, w->dsign, pl.NB, bblob, st);
+        HQ_CUDA_CHECK(ctx, cudaGetLastError());
+        E8Params p;
+        p.blob = w->blob; p.sub_off = w->group_off; p.lut = ctx->e8_lut; p.m = w->m;
+        p.n_kt = (int)w->n_kt; p.n_rb = (int)w->n_rb; p.n_bt = pl.n_bt; p.n_split = pl.n_split; p.L = pl.L;
+        p.n_items = pl.n_items; p.inv_A = inv_A; p.bblob = bblob; p.B = B; p.partials = partials; p.acc_i32 = acc_i32;
+        if (ctx->prof) {
+            HQ_CUDA_CHECK(ctx, cudaEventCreate(&e0));
+            HQ_CUDA_CHECK(ctx, cudaEventCreate(&e1));
+            HQ_CUDA_CHECK(ctx, cudaEventRecord(e0, st));
+        }
+        hq_status s = (pl.NB == 16) ? launch_e8_nb<16>(ctx, w, p, pl.grid, st) : launch_e8_nb<64>(ctx, w, p, pl.grid, st);
+        if (s != HQ_OK) return s;
+    } else {
+        int8_t* q = (int8_t*)ws;
+        float* s_x = (float*)(ws + align256((size_t)(B * w->n_in)));
+        partials = (float*)((uint8_t*)s_x + align256((size_t)(B * w->n_kt) * 4));
+        n_split = generic_split(ctx, w, B);
+        launch_act_quant(x, dtype, B, w->n_in, ldx, w->lattice, w->n, w->dsign, q, s_x, nullptr, st);
+        HQ_CUDA_CHECK(ctx, cudaGetLastError());
+        LinearParams p;
+        p.blob = w->blob; p.group_off = w->group_off; p.m = w->m; p.n_kt = w->n_kt;
+        p.n = w->n; p.k0 = w->k0; p.k1 = w->k1; p.rbits = w->rbits; p.inv_A = inv_A;
+        p.q = q; p.s_x = s_x; p.B = B; p.n_split = n_split; p.partials = partials; p.acc_i32 = acc_i32;
+        if (ctx->prof) {
+            HQ_CUDA_CHECK(ctx, cudaEventCreate(&e0));
+            HQ_CUDA_CHECK(ctx, cudaEventCreate(&e1));
+            HQ_CUDA_CHECK(ctx, cudaEventRecord(e0, st));
+        }
+        hq_status s = (B <= 16) ? launch_generic_nb<16>(ctx, w, p, st) : launch_generic_nb<64>(ctx, w, p, st);
+        if (s != HQ_OK) return s;
+    }
     if (ctx->prof) {
         HQ_CUDA_CHECK(ctx, cudaEventRecord(e1, st));
         ctx->prof_ev.push_back(e0);
