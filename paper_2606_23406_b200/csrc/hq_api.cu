@@ -209,6 +209,7 @@ hq_status hq_encode_weights(hq_ctx* ctx, const void* W_dev, int32_t dtype, int64
         return bail(HQ_ERR_FORMAT);
     }
     w->max_group16 = *(uint32_t*)(hc + 19);
+    w->min_ulen = 65535u - ((uint32_t*)(hc + 18))[4];
     w->blob_bytes = (int64_t)total16 * 16;
     w->payload_bits = (int64_t)hc[17] + m_out * w->n_kt * (int64_t)w->rbits;
     w->blob = (uint8_t*)ctx_alloc(ctx, (size_t)w->blob_bytes + 64);  // +64: decoders read one word ahead

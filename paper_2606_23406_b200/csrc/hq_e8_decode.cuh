@@ -19,6 +19,7 @@
 // index inside the tile is 32c + 4i + b, and the activation operand is stored in the same order.
 #pragma once
 #include "hq_common.cuh"
+#include "hq_tc.cuh"
 
 namespace hq {
 
@@ -34,16 +35,15 @@ __host__ __device__ inline uint32_t unary_lut_entry(uint32_t b, uint32_t par) {
     return v;
 }
 
-// phase 1 for one stream word x (4 bytes, byte 0 = bits 31..24).  `lut_lane` = this lane's copy of entry 0 /
-// parity 0 in shared memory.  State: acc (partial nibble word), fs (bits used in acc, 0..28), wo (next nibble
-// word of this row in shared memory).
-__device__ __forceinline__ void e8_unary_word(uint32_t x, const uint32_t* lut_lane, uint32_t& acc, uint32_t& fs,
-                                              uint32_t*& wo) {
+// phase 1 for one stream word x (4 bytes, byte 0 = bits 31..24).  `lut_lane` = shared-space address of this
+// lane's copy of entry 0 / parity 0.  State: acc (partial nibble word), fs (bits used in acc, 0..28), wo
+// (shared-space address of the next nibble word of this row).
+__device__ __forceinline__ void e8_unary_word(uint32_t x, uint32_t lut_lane, uint32_t& acc, uint32_t& fs, uint32_t& wo) {
     uint32_t N[4];
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
         const uint32_t sel = (i < 3) ? ((x >> (18 - 8 * i)) & 0x3fc0u) : ((x << 6) & 0x3fc0u);   // byte * 64
-        N[i] = *(const uint32_t*)((const char*)lut_lane + sel + ((i & 1) ? 256 * E8_LUT_COPIES * 4 : 0));
+        N[i] = lds32_ro(lut_lane + sel + ((i & 1) ? 256 * E8_LUT_COPIES * 4 : 0));
     }
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
@@ -52,7 +52,7 @@ __device__ __forceinline__ void e8_unary_word(uint32_t x, const uint32_t* lut_la
         const uint32_t out1 = __funnelshift_l(N[i], 0u, fs);  // the bits of N shifted out past bit 31 (fs < 32)
         const uint32_t fs2 = fs + c4;
         const bool full = fs2 >= 32u;
-        if (full) *wo++ = out0;
+        if (full) { sts32(wo, out0); wo += 4; }
         acc = full ? out1 : out0;
         fs = fs2 & 31u;
     }

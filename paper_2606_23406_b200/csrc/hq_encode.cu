@@ -335,6 +335,10 @@ __global__ void k_tile_ulen(const int8_t* codes, int64_t m, int64_t n_kt, int n,
     if (r < m) {
         L = tile_ulen<LAT>(codes + r * (n_kt * n) + kt * n, n, k0, k1);
         if (L > W_ULEN_MAX) { atomicExch(err_flag, 1); L = W_ULEN_MAX; }
+        // err_flag[4] tracks 65535 - (shortest U-section of a present row), warp-aggregated
+        uint32_t inv = 65535u - L;
+        inv = __reduce_max_sync(__activemask(), inv);
+        if ((threadIdx.x & 31) == (__ffs(__activemask()) - 1)) atomicMax((unsigned int*)err_flag + 4, inv);
     }
     ulen_tmp[idx] = (uint16_t)L;
 }

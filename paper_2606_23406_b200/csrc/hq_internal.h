@@ -36,7 +36,8 @@ struct hq_weight {
     uint32_t* group_off;  // dev [4G+1]  sub-group offsets (FORMAT §5)
     int8_t* dsign;        // dev [n_in]  RHT signs (+1/-1)
     int64_t blob_bytes, payload_bits, clamp_count;
-    uint32_t max_group16;  // largest group size in 16-byte units
+    uint32_t max_group16;  // largest sub-group size in 16-byte units
+    uint32_t min_ulen;     // shortest U-section (bits) over the present rows of all tiles
 };
 
 struct hq_kv {
@@ -92,7 +93,8 @@ void launch_act_quant(const void* x, int dtype, int64_t B, int64_t n_in, int64_t
 // activations as the E8 fused kernel's B operand tiles (UMMA layout, permuted K, + scales); n_tile = 128
 void launch_act_blob(const void* x, int dtype, int64_t B, int64_t n_in, int64_t ldx, const int8_t* dsign, int NB,
                      uint8_t* bblob, cudaStream_t st);
-// ulen_tmp[sg*32 + i] for all sub-groups (0 for absent rows); err_flag set if a tile exceeds 8160 bits
+// ulen_tmp[sg*32 + i] for all sub-groups (0 for absent rows); err_flag[0] set if a tile exceeds 8160 bits,
+// err_flag[4] = max over present rows of 65535 - ulen
 void launch_tile_ulen(const int8_t* codes, int64_t m, int64_t n_in, int lattice, int n, int k0, int k1,
                       uint16_t* ulen_tmp, int* err_flag, cudaStream_t st);
 // group_off[G4+1] (sub-group offsets, 16-byte units) by a device prefix sum; totals[0] = sum of ulen over all tiles

@@ -234,31 +234,35 @@ static hq_status launch_generic_nb(hq_ctx* ctx, const hq_weight* w, LinearParams
 // ---- E8 fast path -----------------------------------------------------------------------------
 bool linear_uses_e8_fast(const hq_weight* w) { return w->lattice == LAT_E8 && w->n == 128 && w->k0 <= 3; }
 
-struct E8Plan { int NB, n_bt, n_split, L, n_items, grid; };
+struct E8Plan { int NB, BC, NWG, n_bt, n_split, L, n_items, grid; };
 static E8Plan e8_plan(const hq_ctx* ctx, const hq_weight* w, int64_t B) {
     E8Plan pl;
     pl.NB = B <= 16 ? 16 : 64;
+    pl.BC = B == 1 ? 1 : pl.NB;
+    pl.NWG = B == 1 ? 6 : (B <= 16 ? 5 : 4);
     pl.n_bt = (int)((B + pl.NB - 1) / pl.NB);
-    const int64_t GW = (int64_t)ctx->sm_count * E8_NWG;
     const int n_kt = (int)w->n_kt;
-    int split = n_kt;  // the smallest divisor of n_kt that gives every warp group at least two items
+    // K split: the largest divisor of n_kt whose fp32 partial sums (written + read back) stay below a quarter of
+    // the compressed weight bytes; batch 1 therefore splits down to single tiles (finest load balance)
+    const double budget = 0.25 * 0.53 * (double)w->n_in / (8.0 * (double)B);
+    int split = 1;
     for (int d = 1; d <= n_kt; ++d)
-        if (n_kt % d == 0 && w->n_rb * pl.n_bt * d >= 2 * GW) { split = d; break; }
+        if (n_kt % d == 0 && (double)d <= budget) split = d;
     pl.n_split = split;
     pl.L = n_kt / split;
-    pl.n_items = (int)(w->n_rb * pl.n_bt * split);
-    int64_t ctas = (pl.n_items + E8_NWG - 1) / E8_NWG;
-    pl.grid = (int)(ctas < ctx->sm_count ? ctas : ctx->sm_count);
+    pl.n_items = (int)(w->n_rb * split);
+    pl.grid = pl.n_items < ctx->sm_count ? pl.n_items : ctx->sm_count;
     return pl;
 }
 
-template <int NB>
-static hq_status launch_e8_nb(hq_ctx* ctx, const hq_weight* w, E8Params& p, int grid, cudaStream_t st) {
-    const size_t smem = e8_smem_bytes<NB>();
+template <int NB, int BC, int NWG>
+static hq_status launch_e8_v(hq_ctx* ctx, const hq_weight* w, E8Params& p, const E8Plan& pl, cudaStream_t st) {
+    const size_t smem = e8_smem_bytes<NB, NWG>();
+    dim3 grid((unsigned)pl.grid, (unsigned)pl.n_bt);
 #define HQ_LE(KK)                                                                                                   \
     case KK:                                                                                                        \
-        HQ_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_linear_e8<KK, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
-        k_linear_e8<KK, NB><<<grid, E8_NWG * 128, smem, st>>>(p);                                                   \
+        HQ_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_linear_e8<KK, NB, BC, NWG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+        k_linear_e8<KK, NB, BC, NWG><<<grid, NWG * 128, smem, st>>>(p);                                             \
         break
     switch (w->k0) {
         HQ_LE(0); HQ_LE(1); HQ_LE(2); HQ_LE(3);
@@ -294,14 +298,17 @@ hq_status launch_linear(hq_ctx* ctx, const hq_weight* w, const void* x, int dtyp
         HQ_CUDA_CHECK(ctx, cudaGetLastError());
         E8Params p;
         p.blob = w->blob; p.sub_off = w->group_off; p.lut = ctx->e8_lut; p.m = w->m;
-        p.n_kt = (int)w->n_kt; p.n_rb = (int)w->n_rb; p.n_bt = pl.n_bt; p.n_split = pl.n_split; p.L = pl.L;
+        p.n_kt = (int)w->n_kt; p.n_rb = (int)w->n_rb; p.n_split = pl.n_split; p.L = pl.L;
         p.n_items = pl.n_items; p.inv_A = inv_A; p.bblob = bblob; p.B = B; p.partials = partials; p.acc_i32 = acc_i32;
+        p.u_dense = (int)(((w->min_ulen + 31) >> 5) < (uint32_t)E8_NW ? ((w->min_ulen + 31) >> 5) : (uint32_t)E8_NW);
         if (ctx->prof) {
             HQ_CUDA_CHECK(ctx, cudaEventCreate(&e0));
             HQ_CUDA_CHECK(ctx, cudaEventCreate(&e1));
             HQ_CUDA_CHECK(ctx, cudaEventRecord(e0, st));
         }
-        hq_status s = (pl.NB == 16) ? launch_e8_nb<16>(ctx, w, p, pl.grid, st) : launch_e8_nb<64>(ctx, w, p, pl.grid, st);
+        hq_status s = (B == 1)    ? launch_e8_v<16, 1, 6>(ctx, w, p, pl, st)
+                      : (B <= 16) ? launch_e8_v<16, 16, 5>(ctx, w, p, pl, st)
+                                  : launch_e8_v<64, 64, 4>(ctx, w, p, pl, st);
         if (s != HQ_OK) return s;
     } else {
         int8_t* q = (int8_t*)ws;
