@@ -36,26 +36,28 @@ __host__ __device__ inline uint32_t unary_lut_entry(uint32_t b, uint32_t par) {
 }
 
 // phase 1 for one stream word x (4 bytes, byte 0 = bits 31..24).  `lut_lane` = shared-space address of this
-// lane's copy of entry 0 / parity 0.  State: acc (partial nibble word), fs (bits used in acc, 0..28), wo
-// (shared-space address of the next nibble word of this row).
-__device__ __forceinline__ void e8_unary_word(uint32_t x, uint32_t lut_lane, uint32_t& acc, uint32_t& fs, uint32_t& wo) {
-    uint32_t N[4];
+// lane's copy of entry 0 / parity 0.  State: T = 4 * (terminators seen so far in the row) = bit position in the
+// nibble stream, acc = the partial nibble word, wo = shared-space address of the next nibble word of this row.
+// Every shift amount and every "word completed" predicate comes from prefix popcounts of x, so the only
+// loop-carried values are acc (one select per byte) and wo (one predicated add per byte).
+__device__ __forceinline__ void e8_unary_word(uint32_t x, uint32_t lut_lane, uint32_t& T, uint32_t& acc, uint32_t& wo) {
+    uint32_t N[4], Te[4];
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
         const uint32_t sel = (i < 3) ? ((x >> (18 - 8 * i)) & 0x3fc0u) : ((x << 6) & 0x3fc0u);   // byte * 64
         N[i] = lds32_ro(lut_lane + sel + ((i & 1) ? 256 * E8_LUT_COPIES * 4 : 0));
+        Te[i] = T + 4u * (uint32_t)__popc(i < 3 ? (x >> (24 - 8 * i)) : x);   // nibble-stream position after byte i
     }
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
-        const uint32_t c4 = 4u * (uint32_t)__popc(x & (0xff000000u >> (8 * i)));
-        const uint32_t out0 = acc | (N[i] << fs);
-        const uint32_t out1 = __funnelshift_l(N[i], 0u, fs);  // the bits of N shifted out past bit 31 (fs < 32)
-        const uint32_t fs2 = fs + c4;
-        const bool full = fs2 >= 32u;
+        const uint32_t Tb = i ? Te[i - 1] : T;                  // position before byte i
+        const uint32_t out0 = acc | __funnelshift_l(0u, N[i], Tb);   // N << (Tb & 31)
+        const uint32_t out1 = __funnelshift_l(N[i], 0u, Tb);         // the bits of N shifted out past bit 31
+        const bool full = ((Te[i] ^ Tb) & 32u) != 0u;                // this byte completed a 32-bit nibble word
         if (full) { sts32(wo, out0); wo += 4; }
         acc = full ? out1 : out0;
-        fs = fs2 & 31u;
     }
+    T = Te[3];
 }
 
 // the K-bit remainders of symbol group g (0..7 = coordinate) of a 32-symbol run whose K field-plane words are

@@ -7,6 +7,7 @@
 // the fixed operation order of docs/FORMAT.md §2.
 #include "hq_common.cuh"
 #include "hq_internal.h"
+#include "hq_tc.cuh"
 
 namespace hq {
 
@@ -248,6 +249,8 @@ k_act_blob(const void* X, int dtype, int64_t B, int64_t n_kt, int64_t ldx, const
            uint8_t* bblob) {
     extern __shared__ float smem[];
     const int n = 128;
+    griddep_launch();
+    griddep_wait();   // x comes from the previous kernel; the blob area is read by the previous hq_linear
     int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     float* u = smem + warp * n;
     const int64_t n_bt = (B + NB - 1) / NB, n_tiles = n_bt * NB * n_kt;
@@ -291,7 +294,8 @@ void launch_act_blob(const void* x, int dtype, int64_t B, int64_t n_in, int64_t 
     int64_t n_kt = n_in / 128, n_bt = (B + NB - 1) / NB, n_tiles = n_bt * NB * n_kt;
     int64_t blocks = (n_tiles + QW_WARPS - 1) / QW_WARPS;
     if (blocks > 148 * 16) blocks = 148 * 16;
-    k_act_blob<<<(unsigned)blocks, QW_WARPS * 32, QW_WARPS * 128 * sizeof(float), st>>>(x, dtype, B, n_kt, ldx, dsign, NB, bblob);
+    launch_pdl(k_act_blob, dim3((unsigned)blocks), dim3(QW_WARPS * 32), QW_WARPS * 128 * sizeof(float), st, x, dtype, B, n_kt, ldx,
+               dsign, NB, bblob);
 }
 
 void launch_act_quant(const void* x, int dtype, int64_t B, int64_t n_in, int64_t ldx, int lattice, int n,

@@ -66,6 +66,19 @@ struct hq_kv {
 
 namespace hq {
 
+// launch with the programmatic-stream-serialization attribute (PDL): the kernel may begin while its
+// predecessor in the stream drains; it synchronizes with griddepcontrol.wait (hq_tc.cuh)
+template <class... KArgs, class... Args>
+inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
 #define HQ_CUDA_CHECK(ctx, call)                                                        \
     do {                                                                                \
         cudaError_t e__ = (call);                                                       \

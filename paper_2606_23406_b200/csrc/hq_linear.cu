@@ -189,6 +189,8 @@ k_linear_generic(LinearParams p) {
 // y[b, r] = sum over splits (in order) -> fp32 and bf16
 __global__ void k_linear_finalize(const float* partials, int n_split, int64_t B, int64_t m, __nv_bfloat16* y,
                                   int64_t ldy, float* y_f32) {
+    griddep_launch();
+    griddep_wait();
     int64_t idx = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (idx >= B * m) return;
     float s = 0.0f;
@@ -262,7 +264,7 @@ static hq_status launch_e8_v(hq_ctx* ctx, const hq_weight* w, E8Params& p, const
 #define HQ_LE(KK)                                                                                                   \
     case KK:                                                                                                        \
         HQ_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_linear_e8<KK, NB, BC, NWG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
-        k_linear_e8<KK, NB, BC, NWG><<<grid, NWG * 128, smem, st>>>(p);                                             \
+        HQ_CUDA_CHECK(ctx, launch_pdl(k_linear_e8<KK, NB, BC, NWG>, grid, dim3(NWG * 128), smem, st, p));           \
         break
     switch (w->k0) {
         HQ_LE(0); HQ_LE(1); HQ_LE(2); HQ_LE(3);
@@ -335,8 +337,8 @@ hq_status launch_linear(hq_ctx* ctx, const hq_weight* w, const void* x, int dtyp
         ctx->prof_ev.push_back(e1);
     }
     int64_t tot = B * w->m;
-    k_linear_finalize<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(partials, n_split, B, w->m, (__nv_bfloat16*)y_bf16,
-                                                                    ldy, y_f32);
+    HQ_CUDA_CHECK(ctx, launch_pdl(k_linear_finalize, dim3((unsigned)((tot + 255) / 256)), dim3(256), 0, st, (const float*)partials,
+                                  n_split, B, w->m, (__nv_bfloat16*)y_bf16, ldy, y_f32));
     HQ_CUDA_CHECK(ctx, cudaGetLastError());
     return HQ_OK;
 }

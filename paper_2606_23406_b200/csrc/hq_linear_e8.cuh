@@ -126,6 +126,7 @@ k_linear_e8(E8Params p) {
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
+    griddep_launch();
     if (tid == 0) {  // the phase-1 table arrives by one TMA bulk copy while the first loads are in flight
         mbar_arrive_expect_tx(bar_lut, E8_LUT_BYTES);
         bulk_g2s(smem, p.lut, E8_LUT_BYTES, bar_lut);
@@ -147,7 +148,6 @@ k_linear_e8(E8Params p) {
     E8Desc q0 = it.get(p); it.next(p);
     E8Desc q1 = it.get(p); it.next(p);
     E8Desc q2 = it.get(p); it.next(p);
-    E8Desc q3 = it.get(p); it.next(p);
     if (!q0.valid()) {   // nothing to do for this warp group (the CTA still joins the final barrier)
         __syncthreads();
         if (tid < 32) tmem_dealloc(*tmem_slot, TCOLS);
@@ -164,17 +164,22 @@ k_linear_e8(E8Params p) {
     };
     // a sub-group whose 32 rows are all present has at least p.u_dense words in every row: those word-rows are
     // dense (no rank needed); the rest are compacted (FORMAT §5)
-    auto load_u = [&](const uint8_t* sgp, uint32_t ul, bool full_rows, uint32_t* U) {
+    auto load_u_dense = [&](const uint8_t* sgp, bool full_rows, uint32_t* U) {   // needs only the offset
+        const uint32_t* uarea = (const uint32_t*)(sgp + 128) + KW * 32;
+        const uint32_t dense = full_rows ? (uint32_t)p.u_dense : 0u;
+#pragma unroll
+        for (int w = 0; w < E8_NW; ++w)
+            if ((uint32_t)w < dense) U[w] = __ldg(uarea + w * 32 + lane);
+    };
+    auto load_u_ragged = [&](const uint8_t* sgp, uint32_t ul, bool full_rows, uint32_t* U) {   // needs the header
         const uint32_t* uarea = (const uint32_t*)(sgp + 128) + KW * 32;
         const uint32_t nw = (ul + 31) >> 5;
         const uint32_t dense = full_rows ? (uint32_t)p.u_dense : 0u;
         uint32_t base = dense * 32;
 #pragma unroll
         for (int w = 0; w < E8_NW; ++w) {
-            const bool has = nw > (uint32_t)w;
-            if ((uint32_t)w < dense) {
-                U[w] = __ldg(uarea + w * 32 + lane);
-            } else {
+            if ((uint32_t)w >= dense) {
+                const bool has = nw > (uint32_t)w;
                 const uint32_t mk = __ballot_sync(0xffffffffu, has);
                 U[w] = has ? __ldg(uarea + base + __popc(mk & lane_lt)) : 0u;
                 base += __popc(mk);
@@ -189,15 +194,15 @@ k_linear_e8(E8Params p) {
     auto rows_full = [&](const E8Desc& d) -> bool { return (int64_t)d.rb * 128 + warp * 32 + 32 <= p.m; };
 
     uint32_t Uw[E8_NW], Rw[KW > 0 ? KW : 1];
+    // prologue: offsets of tiles 0 and 1 together, then everything of tile 0 that needs only its offset
+    uint32_t off_n1 = load_off(q1);
     const uint8_t* sgp_c = p.blob + 16 * (size_t)load_off(q0);
     uint32_t ul_c = __ldg((const uint16_t*)sgp_c + lane), nrm_c = __ldg((const uint16_t*)sgp_c + 32 + lane);
-    load_u(sgp_c, ul_c, rows_full(q0), Uw);
+    load_u_dense(sgp_c, rows_full(q0), Uw);
     load_r(sgp_c, Rw);
-    const uint8_t* sgp_n1 = p.blob + 16 * (size_t)load_off(q1);
+    load_u_ragged(sgp_c, ul_c, rows_full(q0), Uw);
+    const uint8_t* sgp_n1 = nullptr;
     uint32_t ul_n1 = 0, nrm_n1 = 0;
-    if (q1.valid()) { ul_n1 = __ldg((const uint16_t*)sgp_n1 + lane); nrm_n1 = __ldg((const uint16_t*)sgp_n1 + 32 + lane); }
-    uint32_t off_n2 = load_off(q2);
-    if (t == 0) issue_b(q0, 0);
 
     float yacc[BC];
 #pragma unroll
@@ -246,26 +251,25 @@ k_linear_e8(E8Params p) {
     mbar_wait(bar_lut, 0u);
 
     for (int tau = 0;; ++tau) {
-        // ---- move the pipeline: header of tau+2 (offset known), offset of tau+3
-        const uint8_t* sgp_n2 = p.blob + 16 * (size_t)off_n2;
-        uint32_t ul_n2 = 0, nrm_n2 = 0;
-        if (q2.valid()) {
-            ul_n2 = __ldg((const uint16_t*)sgp_n2 + lane);
-            nrm_n2 = __ldg((const uint16_t*)sgp_n2 + 32 + lane);
-        }
-        const uint32_t off_n3 = load_off(q3);
+        // ---- move the pipeline: offset of tile tau+2
+        const uint32_t off_n2 = load_off(q2);
 
         // ---- phase 1: unary section -> nibble words (A4)
         const uint32_t nw = (ul_c + 31) >> 5;
         const uint32_t maxnw = __reduce_max_sync(0xffffffffu, nw);
         {
-            uint32_t acc = 0, fs = 0, wo = scr_a;
+            uint32_t T = 0, acc = 0, wo = scr_a;
 #pragma unroll
             for (int w = 0; w < E8_NW; ++w)
-                if ((uint32_t)w < maxnw) e8_unary_word(Uw[w], lut_lane, acc, fs, wo);
+                if ((uint32_t)w < maxnw) e8_unary_word(Uw[w], lut_lane, T, acc, wo);
         }
-        // the U registers are free: words of tile tau+1 (its header arrived during the previous iteration)
-        if (q1.valid()) load_u(sgp_n1, ul_n1, rows_full(q1), Uw);
+        // the U registers are free: header and dense U words of tile tau+1 (its offset arrived an iteration ago)
+        sgp_n1 = p.blob + 16 * (size_t)off_n1;
+        if (q1.valid()) {
+            ul_n1 = __ldg((const uint16_t*)sgp_n1 + lane);
+            nrm_n1 = __ldg((const uint16_t*)sgp_n1 + 32 + lane);
+            load_u_dense(sgp_n1, rows_full(q1), Uw);
+        }
 
         // ---- the previous tile's MMA must be done before its accumulators are read and the A tile is rewritten
         if (tau > 0) {
@@ -308,11 +312,20 @@ k_linear_e8(E8Params p) {
                 }
             });
         }
-        // the R registers are free: remainder words of tile tau+1
-        if (q1.valid()) load_r(sgp_n1, Rw);
+        // the R registers are free: remainder words of tile tau+1, and its ragged U words (the header has arrived)
+        if (q1.valid()) {
+            load_r(sgp_n1, Rw);
+            load_u_ragged(sgp_n1, ul_n1, rows_full(q1), Uw);
+        }
         const float sw_cur = f16_bits_to_f32((uint16_t)nrm_c) * p.inv_A;
         fence_proxy_async_smem();
         tc_fence_before();
+        if (tau == 0) {
+            // everything up to here touched only the weights; the activation operand, the partial sums and the debug
+            // outputs belong to the stream order: join it (no-op unless launched with PDL)
+            griddep_wait();
+            if (t == 0) issue_b(q0, 0);
+        }
         asm volatile("bar.sync %0, 128;" ::"r"(wg + 1) : "memory");
         if (t == 0) {
             issue_b(q1, (tau + 1) & 1);   // that slot's last reader, the epilogue of tile tau-1, is behind the barrier
@@ -334,10 +347,9 @@ k_linear_e8(E8Params p) {
             break;
         }
         sgp_c = sgp_n1; ul_c = ul_n1; nrm_c = nrm_n1;
-        sgp_n1 = sgp_n2; ul_n1 = ul_n2; nrm_n1 = nrm_n2;
-        off_n2 = off_n3;
-        q0 = q1; q1 = q2; q2 = q3;
-        q3 = it.get(p); it.next(p);
+        off_n1 = off_n2;
+        q0 = q1; q1 = q2;
+        q2 = it.get(p); it.next(p);
     }
     tc_fence_before();
     __syncthreads();
