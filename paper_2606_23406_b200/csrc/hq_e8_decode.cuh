@@ -41,19 +41,23 @@ __host__ __device__ inline uint32_t unary_lut_entry(uint32_t b, uint32_t par) {
 // Every shift amount and every "word completed" predicate comes from prefix popcounts of x, so the only
 // loop-carried values are acc (one select per byte) and wo (one predicated add per byte).
 __device__ __forceinline__ void e8_unary_word(uint32_t x, uint32_t lut_lane, uint32_t& T, uint32_t& acc, uint32_t& wo) {
+    // The ALU pipe (LOP3 / SHF / SEL, half rate) is the busiest unit of this kernel: the byte-prefix shift, shared by
+    // the table index and the prefix popcount, is taken as the high half of a multiply (FMA pipe).  (Doing the
+    // variable shifts of the append as multiplies too was measured slower: IMAD.HI is quarter rate.)
     uint32_t N[4], Te[4];
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
-        const uint32_t sel = (i < 3) ? ((x >> (18 - 8 * i)) & 0x3fc0u) : ((x << 6) & 0x3fc0u);   // byte * 64
+        const uint32_t pre = (i < 3) ? __umulhi(x, 1u << (8 + 8 * i)) : x;   // x >> (24 - 8i): bytes 0..i
+        const uint32_t sel = (pre * 64u) & 0x3fc0u;                          // byte i * 64
         N[i] = lds32_ro(lut_lane + sel + ((i & 1) ? 256 * E8_LUT_COPIES * 4 : 0));
-        Te[i] = T + 4u * (uint32_t)__popc(i < 3 ? (x >> (24 - 8 * i)) : x);   // nibble-stream position after byte i
+        Te[i] = T + 4u * (uint32_t)__popc(pre);   // nibble-stream position after byte i
     }
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
         const uint32_t Tb = i ? Te[i - 1] : T;                  // position before byte i
         const uint32_t out0 = acc | __funnelshift_l(0u, N[i], Tb);   // N << (Tb & 31)
         const uint32_t out1 = __funnelshift_l(N[i], 0u, Tb);         // the bits of N shifted out past bit 31
-        const bool full = ((Te[i] ^ Tb) & 32u) != 0u;                // this byte completed a 32-bit nibble word
+        const bool full = ((Te[i] ^ Tb) & 32u) != 0u;           // this byte completed a 32-bit nibble word
         if (full) { sts32(wo, out0); wo += 4; }
         acc = full ? out1 : out0;
     }
@@ -80,7 +84,7 @@ __device__ __forceinline__ uint32_t e8_rem4(const uint32_t* V, int g) {
 
 // phase 2 for one run of 32 symbols: nibble words W[0..3], remainder words V[0..K) -> C[0..7].
 // prevWo carries the last odd-position word (for the gap of the next even positions); qsum accumulates
-// all quotients of the row byte-wise (caller widens).
+// the quotients of the row.
 template <int K>
 __device__ __forceinline__ void e8_run(const uint32_t* W, const uint32_t* V, uint32_t& prevWo, uint32_t& qsum, uint32_t* C) {
     uint32_t Z[8];
@@ -91,7 +95,8 @@ __device__ __forceinline__ void e8_run(const uint32_t* W, const uint32_t* V, uin
         const uint32_t qe = (We + 0x1f1f1f1fu - prev) & 0x0f0f0f0fu;
         const uint32_t qo = (Wo + 0x1f1f1f1fu - We) & 0x0f0f0f0fu;
         prevWo = Wo;
-        qsum += qe + qo;
+        qsum = __dp4a(qe, 0x01010101u, qsum);
+        qsum = __dp4a(qo, 0x01010101u, qsum);
         Z[2 * w] = qe * (1u << K) + e8_rem4<K>(V, 2 * w);
         Z[2 * w + 1] = qo * (1u << K) + e8_rem4<K>(V, 2 * w + 1);
     }

@@ -285,11 +285,10 @@ k_linear_e8(E8Params p) {
             uint32_t prevWo = 15u << 24;  // e_{-1} = -1 mod 16
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
-                uint32_t W[4], C[8], qsum = 0;
+                uint32_t W[4], C[8];
 #pragma unroll
                 for (int w = 0; w < 4; ++w) W[w] = lds32(scr_a + (c * 4 + w) * 4);
-                e8_run<K>(W, Rw + c * K, prevWo, qsum, C);
-                total += __dp4a(qsum, 0x01010101u, 0u);
+                e8_run<K>(W, Rw + c * K, prevWo, total, C);
                 if (!present) {
 #pragma unroll
                     for (int i = 0; i < 8; ++i) C[i] = 0u;
