@@ -110,6 +110,124 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def _time_cuda(fn, reps, warm=1):
+    import torch
+    for _ in range(warm):
+        fn()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(reps):
+        fn()
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / reps
+
+
+def run_extras(ctx, hq, dev, peak_gbs):
+    """The other BASELINE configs, each a bounded, seeded, synthetic run through the public API (parity for the
+    same code paths is in tests/): config 5 (large-M INT8 TOPS), config 4 (KV append / attend), config 3 (reduced
+    lattice / rate / tile sweep at batch 1)."""
+    import torch
+    out = {}
+    # ---- config 5: 8192 tokens x (4096 -> 16384), E8 4 bps, tile 128, INT8 MMA
+    try:
+        W = torch.from_numpy(hq_synth.gaussian_weight(16384, 4096, seed=5)).to(dev).to(torch.bfloat16)
+        w = ctx.encode_weights(W, hq.Lattice.E8, 128, SNR_E8_4BPS, seed=5)
+        del W
+        X = torch.from_numpy(hq_synth.activations(8192, 4096, seed=6)).to(dev).to(torch.bfloat16)
+        y = torch.empty((8192, 16384), dtype=torch.bfloat16, device=dev)
+        ms = _time_cuda(lambda: w.linear(X, y=y), reps=3)
+        ops = 2.0 * 8192 * 16384 * 4096
+        c5 = {"workload": "8192 tokens x 4096->16384, E8 4 bps, tile 128", "ms": ms, "int8_TOPS": ops / (ms * 1e-3) / 1e12,
+              "nominal_dense_int8_TOPS": 4500.0}
+        try:
+            a = torch.randint(-127, 127, (8192, 8192), dtype=torch.int8, device=dev)
+            b = torch.randint(-127, 127, (8192, 8192), dtype=torch.int8, device=dev)
+            ms_mm = _time_cuda(lambda: torch._int_mm(a, b), reps=5, warm=2)
+            c5["measured_int8_peak_TOPS_torch_int_mm_8192"] = 2.0 * 8192 ** 3 / (ms_mm * 1e-3) / 1e12
+            c5["frac_of_measured_int8_peak"] = c5["int8_TOPS"] / c5["measured_int8_peak_TOPS_torch_int_mm_8192"]
+            del a, b
+        except Exception as ex:  # noqa: BLE001
+            c5["measured_int8_peak_TOPS_torch_int_mm_8192"] = f"unavailable: {ex}"
+        c5["frac_of_nominal_int8_peak"] = c5["int8_TOPS"] / 4500.0
+        out["config5_large_m"] = c5
+        w.free(); del X, y
+    except Exception as ex:  # noqa: BLE001
+        out["config5_large_m"] = f"failed: {ex}"
+    # ---- config 4: KV cache, 8 heads x 128, 32768 tokens, E8 2 bps, signs rotation, dither, window 32
+    try:
+        T, H, d, QH = 32768, 8, 128, 32
+        snr_kv = float(np.float32(9.68))
+        K = torch.from_numpy(hq_synth.kv_tokens(T + 16, H, d, seed=4)).to(dev).to(torch.bfloat16)
+        V = torch.from_numpy(hq_synth.kv_tokens(T + 16, H, d, seed=5)).to(dev).to(torch.bfloat16)
+        q = torch.from_numpy(hq_synth.activations(QH, d, seed=6)).to(dev).to(torch.bfloat16)
+        kv = ctx.kv_create(H, d, T + 64, hq.Lattice.E8, snr_kv, (0, 0), 4, rotation=1, dither=1, window=32)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        kv.append(K[:T], V[:T])
+        torch.cuda.synchronize()
+        bulk_s = time.perf_counter() - t0
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for i in range(16):
+            kv.append(K[T + i:T + i + 1], V[T + i:T + i + 1])
+        e1.record()
+        torch.cuda.synchronize()
+        app_us = 1e3 * e0.elapsed_time(e1) / 16
+        o = torch.empty_like(q)
+        att_ms = _time_cuda(lambda: kv.attend(q, out=o), reps=5)
+        ex = kv.export()
+        Tn = int(ex["n_tokens"])
+        payload_bits = float(ex["upos"].astype(np.int64).sum()) + 2.0 * H * Tn * float(ex["rbits"])
+        scal = 2.0 * H * Tn * d
+        alg_bytes = (payload_bits + 32.0 * 2 * H * Tn) / 8.0
+        out["config4_kv"] = {"workload": "8 KV heads x 128, 32768 tokens, E8 2 bps, signs rotation, dither, window 32; 32 query heads",
+                             "bulk_append_Mscalars_per_s": 2.0 * H * T * d / bulk_s / 1e6, "append_us_per_token": app_us,
+                             "attend_ms": att_ms, "attend_GBps_compressed": alg_bytes / (att_ms * 1e-3) / 1e9,
+                             "attend_frac_of_hbm_roofline": alg_bytes / (att_ms * 1e-3) / 1e9 / peak_gbs,
+                             "bits_per_scalar_payload": payload_bits / scal, "bits_per_scalar_total": 8.0 * alg_bytes / scal,
+                             "kv_compression_vs_bf16": 16.0 / (8.0 * alg_bytes / scal)}
+        kv.free(); del K, V
+    except Exception as ex:  # noqa: BLE001
+        out["config4_kv"] = f"failed: {ex}"
+    # ---- config 3 (reduced): one 14336 x 4096 Gaussian weight; lattice x rate at tile 128, E8 4 bps at tiles 64 / 256
+    try:
+        Wn = hq_synth.gaussian_weight(14336, 4096, seed=3)
+        W = torch.from_numpy(Wn).to(dev).to(torch.bfloat16)
+        x = torch.from_numpy(hq_synth.activations(1, 4096, seed=9)).to(dev).to(torch.bfloat16)
+        snr = {"E8": (16.50, 22.68, 28.73), "D4": (16.4, 22.5, 28.6), "A2": (16.02, 22.21, 28.26), "Z": (15.8, 21.9, 27.9)}
+        combos = [(lat, s, 128) for lat in ("E8", "D4", "A2", "Z") for s in snr[lat]] + [("E8", 22.68, 64), ("E8", 22.68, 256)]
+        rows = []
+        for lat, s, n_tile in combos:
+            s32 = float(np.float32(s))
+            w = ctx.encode_weights(W, hq.Lattice.BY_NAME[lat], n_tile, s32, seed=3)
+            info = w.info
+            sc = float(info.m_out * info.n_in)
+            yv = torch.empty((1, 14336), dtype=torch.bfloat16, device=dev)
+            ms = _time_cuda(lambda: w.linear(x, y=yv), reps=5, warm=2)
+            nbytes = (info.payload_bits + info.norm_bits + info.length_bits) / 8.0
+            # MSE of the reconstruction, measured in the rotated domain (the RHT is orthonormal) on the first 512 rows
+            R = 512
+            _, _, u = w.act_quant(W[:R], want_u=True)
+            codes, norms = w.decode_int8()
+            c = codes[:R].float().view(R, -1, n_tile)
+            if lat == "A2":
+                c[..., 0::2] *= 3.0 ** 0.5
+            rho = norms[:R].view(torch.float16).float()
+            scale = rho / (info.alpha * n_tile ** 0.5)
+            mse = float(((u.view(R, -1, n_tile) - scale[..., None] * c) ** 2).mean())
+            pred = float((rho ** 2).mean() / n_tile / 10 ** (s32 / 10))
+            rows.append({"lattice": lat, "snr_db": s, "n_tile": n_tile, "k": [info.rice_k[0], info.rice_k[1]],
+                         "bits_payload": info.payload_bits / sc, "bits_total": 8.0 * nbytes / sc,
+                         "mse": mse, "mse_predicted": pred, "gemv_us": 1e3 * ms, "GBps_compressed": nbytes / (ms * 1e-3) / 1e9})
+            w.free()
+        out["config3_sweep"] = rows
+    except Exception as ex:  # noqa: BLE001
+        out["config3_sweep"] = f"failed: {ex}"
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -290,6 +408,8 @@ def main():
             del dense
         except Exception as ex:  # noqa: BLE001
             extras["cublas_bf16_gemv_ms_per_layer"] = f"failed: {ex}"
+        if world == 1:
+            extras.update(run_extras(ctx, hq, dev, peaks()[0]))
 
     # ---- CPU baseline: the oracle on a bounded sample, rank 0, N=1 only
     cpu = None
