@@ -4,8 +4,8 @@ decoder layer's linears (BASELINE.json configs[1]: E8, 4 bps, RHT tile 128, batc
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--layers L] [--impl reference]
 
-A step = the seven linears (q,k,v,o,gate,up,down) of one layer at batch 1 through hq_linear (activation RHT +
-INT8 cast, fused decode+MMA, split-K finalize).  L distinct layers (L x ~116 MB compressed > the 126 MB L2) are
+A step = the seven linears (q,k,v,o,gate,up,down) of one layer at batch 1 through hq_linear_group (matrices that
+share an input share a launch: activation RHT + INT8 cast, fused decode+MMA, split-K finalize).  L distinct layers (L x ~116 MB compressed > the 126 MB L2) are
 cycled so no step re-reads its weights from L2.  One JSON line on stdout (rank 0).
 """
 import argparse
@@ -277,11 +277,12 @@ def main():
         ys = {name: torch.empty((B, hq_synth.LLAMA_SHAPES[name][0]), dtype=torch.bfloat16, device=dev) for name in NAMES}
         return xs, ys
 
+    GROUPS = [["q", "k", "v"], ["o"], ["gate", "up"], ["down"]]   # matrices that share an input share a launch
+
     def step(i, xs, ys):
         ws = layers[i % args.layers]
-        for name in NAMES:
-            w = ws[name]
-            w.linear(xs[w.n_in], y=ys[name])
+        for g in GROUPS:
+            ctx.linear_group([ws[n] for n in g], xs[ws[g[0]].n_in], ys=[ys[n] for n in g])
 
     def barrier():
         if world > 1:
@@ -345,7 +346,7 @@ def main():
     achieved = weight_bytes_per_step * args.steps / (kern_ms * 1e-3) / 1e9 if kern_ms > 0 else 0.0
     peak, peak_src = peaks()
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": NCU_DRAM_BYTES_PER_STEP / len(NAMES), "alg_bytes_per_launch": bytes_per_step / len(NAMES),
+                "traffic": NCU_DRAM_BYTES_PER_STEP / len(GROUPS), "alg_bytes_per_launch": bytes_per_step / len(GROUPS),
                 "traffic_source": "ncu --set full, profiles/r01b_e8_warpgroup_kernel.md", "kernel": "k_linear_e8<K=2,NB=16,BC=1,NWG=6>", "peak_source": peak_src,
                 "kernel_share_of_step": kern_ms / ms_p if ms_p > 0 else None,
                 "launches_timed": kern_n, "avg_launch_us": 1e3 * kern_ms / max(kern_n, 1),
@@ -356,16 +357,17 @@ def main():
     xs, ys = make_io(1)
     hx = {k: v.cpu().pin_memory() for k, v in xs.items()}
     hy = {k: torch.empty_like(v, device="cpu").pin_memory() for k, v in ys.items()}
-    h2d = sum(hx[layers[0][n].n_in].numel() * 2 for n in NAMES)
+    h2d = sum(hx[layers[0][g[0]].n_in].numel() * 2 for g in GROUPS)
     d2h = sum(v.numel() * 2 for v in hy.values())
 
     def e2e_step(i):
         ws = layers[i % args.layers]
-        for name in NAMES:
-            w = ws[name]
-            xs[w.n_in].copy_(hx[w.n_in], non_blocking=True)
-            w.linear(xs[w.n_in], y=ys[name])
-            hy[name].copy_(ys[name], non_blocking=True)
+        for g in GROUPS:
+            n_in = ws[g[0]].n_in
+            xs[n_in].copy_(hx[n_in], non_blocking=True)
+            ctx.linear_group([ws[n] for n in g], xs[n_in], ys=[ys[n] for n in g])
+            for n in g:
+                hy[n].copy_(ys[n], non_blocking=True)
     for i in range(3):
         e2e_step(i)
     barrier()
@@ -429,10 +431,10 @@ def main():
                 "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "int8", "data": "synthetic",
                 "config": {"workload": WORKLOAD, "lattice": "E8", "snr_db": SNR_E8_4BPS, "n_tile": 128, "batch": 1,
-                           "layers_cycled": args.layers, "l2_policy": "inputs larger than L2 (layers cycled)", "launch": "one CUDA graph per layer (7 x hq_linear)",
+                           "layers_cycled": args.layers, "l2_policy": "inputs larger than L2 (layers cycled)", "launch": "one CUDA graph per layer: hq_linear_group x 4 (q+k+v, o, gate+up, down)",
                            "scalars_per_step": scalars_per_step, "bits_per_scalar_payload": bps_payload,
                            "bits_per_scalar_total": bps_total, "parallelism": "replicas only"},
-                "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": args.steps * len(NAMES) * 3,
+                "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": args.steps * (len(GROUPS) * 2 + len(NAMES)),
                 "roofline": roofline, "cpu_baseline": cpu, "extras": extras}
         print(json.dumps(line))
     if world > 1:

@@ -127,6 +127,17 @@ hq_status hq_linear(hq_ctx* ctx, const hq_weight* w, const void* x_dev, int32_t 
                     int64_t ldx, void* y_bf16_dev, int64_t ldy, float* y_f32_dev_or_null,
                     int32_t* acc_i32_dev_or_null, void* stream);
 
+/*
+ * Several weights applied to the SAME x in one fused launch (q/k/v or gate/up of a decoder layer: §5.1 L309 quantizes
+ * every nn.Linear separately, the forward shares the input).  ws[i] -> ys_bf16[i] [batch, m_i] (leading dimension
+ * ldys[i]).  Results are bit-identical to n_w separate hq_linear calls.  1 <= n_w <= 4.  Weights that cannot share
+ * a launch (different n_in / lattice / tile / Rice k / seed / snr_db, or not on the E8 fast path) are run one by one.
+ * ys_f32_or_null: optional array of n_w dev pointers (entries may be NULL) for the fp32 pre-cast outputs.
+ */
+hq_status hq_linear_group(hq_ctx* ctx, const hq_weight* const* ws, int32_t n_w, const void* x_dev, int32_t dtype,
+                          int64_t batch, int64_t ldx, void* const* ys_bf16_dev, const int64_t* ldys,
+                          float* const* ys_f32_or_null, void* stream);
+
 /* bytes of scratch hq_linear needs for this (weight, batch); it is taken from the ctx allocator and cached. */
 hq_status hq_linear_workspace_bytes(const hq_weight* w, int64_t batch, size_t* bytes);
 

@@ -57,7 +57,7 @@ _lib = None
 
 EXPORTS = ["hq_create", "hq_destroy", "hq_last_error", "hq_alpha", "hq_profile_enable", "hq_profile_read", "hq_encode_weights", "hq_weight_free",
            "hq_weight_get_info", "hq_weight_export", "hq_decode_int8", "hq_act_quant", "hq_linear",
-           "hq_linear_workspace_bytes", "hq_kv_create", "hq_kv_free", "hq_kv_append", "hq_attend", "hq_kv_export",
+           "hq_linear_group", "hq_linear_workspace_bytes", "hq_kv_create", "hq_kv_free", "hq_kv_append", "hq_attend", "hq_kv_export",
            "hq_kv_decode_int8"]
 
 
@@ -84,6 +84,7 @@ def load_library():
     lib.hq_decode_int8.argtypes = [vp, vp, vp, vp, vp]
     lib.hq_act_quant.argtypes = [vp, vp, vp, i32, i64, i64, vp, vp, vp, vp]
     lib.hq_linear.argtypes = [vp, vp, vp, i32, i64, i64, vp, i64, vp, vp, vp]
+    lib.hq_linear_group.argtypes = [vp, C.POINTER(vp), i32, vp, i32, i64, i64, C.POINTER(vp), C.POINTER(i64), C.POINTER(vp), vp]
     lib.hq_linear_workspace_bytes.argtypes = [vp, i64, C.POINTER(C.c_size_t)]
     lib.hq_kv_create.argtypes = [vp, C.POINTER(_KVConfig), C.POINTER(vp)]
     lib.hq_kv_free.argtypes = [vp, vp]; lib.hq_kv_free.restype = None
@@ -166,6 +167,22 @@ class Context:
         self.check(self.lib.hq_encode_weights(self.h, W.data_ptr(), _dtype_code(W), W.shape[0], W.shape[1],
                                               W.stride(0), C.byref(cfg), _stream_ptr(self.device), C.byref(h)))
         return Weight(self, h)
+
+    def linear_group(self, weights, x: torch.Tensor, ys=None, want_f32=False):
+        """[w_i x for w_i in weights] in one fused launch (weights that share x: q/k/v, gate/up)."""
+        n = len(weights)
+        assert 1 <= n <= 4 and x.is_cuda and x.dim() == 2 and x.stride(1) == 1
+        B = x.shape[0]
+        if ys is None:
+            ys = [torch.empty((B, w.m), dtype=torch.bfloat16, device=self.device) for w in weights]
+        y32 = [torch.empty((B, w.m), dtype=torch.float32, device=self.device) for w in weights] if want_f32 else None
+        wa = (C.c_void_p * n)(*[w.h for w in weights])
+        ya = (C.c_void_p * n)(*[y.data_ptr() for y in ys])
+        la = (C.c_int64 * n)(*[y.stride(0) for y in ys])
+        fa = (C.c_void_p * n)(*[t.data_ptr() for t in y32]) if want_f32 else None
+        self.check(self.lib.hq_linear_group(self.h, wa, n, x.data_ptr(), _dtype_code(x), B, x.stride(0), ya, la, fa,
+                                            _stream_ptr(self.device)))
+        return (ys, y32) if want_f32 else ys
 
     # ---- KV ----
     def kv_create(self, kv_heads, head_dim, max_tokens, lattice, snr_db, rice_k, seed, rotation=1, dither=1,

@@ -212,9 +212,9 @@ hq_status hq_encode_weights(hq_ctx* ctx, const void* W_dev, int32_t dtype, int64
     w->min_ulen = 65535u - ((uint32_t*)(hc + 18))[4];
     w->blob_bytes = (int64_t)total16 * 16;
     w->payload_bits = (int64_t)hc[17] + m_out * w->n_kt * (int64_t)w->rbits;
-    w->blob = (uint8_t*)ctx_alloc(ctx, (size_t)w->blob_bytes + 64);  // +64: decoders read one word ahead
+    w->blob = (uint8_t*)ctx_alloc(ctx, (size_t)w->blob_bytes + 4096);  // slack: decoders read a word ahead, the fused kernel prefetches whole lines
     if (!w->blob) return bail(HQ_ERR_ALLOC);
-    HQ_TRY(cudaMemsetAsync(w->blob, 0, (size_t)w->blob_bytes + 64, st));
+    HQ_TRY(cudaMemsetAsync(w->blob, 0, (size_t)w->blob_bytes + 4096, st));
     launch_pack_groups(codes, norms, ulen_tmp, m_out, n_in, w->lattice, w->n, k0, k1, w->group_off, w->blob, st);
     HQ_TRY(cudaGetLastError());
     HQ_TRY(cudaStreamSynchronize(st));
@@ -292,6 +292,37 @@ hq_status hq_linear(hq_ctx* ctx, const hq_weight* w, const void* x_dev, int32_t 
     }
     return launch_linear(ctx, w, x_dev, dtype, batch, ldx, y_bf16_dev, ldy, y_f32_dev_or_null, acc_i32_dev_or_null,
                          (uint8_t*)ctx->ws, st);
+}
+
+hq_status hq_linear_group(hq_ctx* ctx, const hq_weight* const* ws, int32_t n_w, const void* x_dev, int32_t dtype,
+                          int64_t batch, int64_t ldx, void* const* ys_bf16_dev, const int64_t* ldys,
+                          float* const* ys_f32_or_null, void* stream) {
+    if (!ctx) return HQ_ERR_INVALID_ARG;
+    if (!ws || !x_dev || !ys_bf16_dev || !ldys || n_w < 1 || n_w > 4) return fail(ctx, HQ_ERR_INVALID_ARG, "bad group arguments");
+    for (int i = 0; i < n_w; ++i) {
+        if (!ws[i] || !ys_bf16_dev[i]) return fail(ctx, HQ_ERR_INVALID_ARG, "null weight or output in group");
+        if (ws[i]->n_in != ws[0]->n_in) return fail(ctx, HQ_ERR_SHAPE, "the weights of a group must share n_in");
+        if (ldys[i] < ws[i]->m) return fail(ctx, HQ_ERR_SHAPE, "bad ldy");
+    }
+    if (batch <= 0 || ldx < ws[0]->n_in) return fail(ctx, HQ_ERR_SHAPE, "bad batch / ldx");
+    if (dtype != HQ_F32 && dtype != HQ_BF16) return fail(ctx, HQ_ERR_INVALID_ARG, "bad dtype");
+    if (!linear_group_compatible(ws, n_w)) {   // one by one: same results, more launches
+        for (int i = 0; i < n_w; ++i) {
+            hq_status s = hq_linear(ctx, ws[i], x_dev, dtype, batch, ldx, ys_bf16_dev[i], ldys[i],
+                                    ys_f32_or_null ? ys_f32_or_null[i] : nullptr, nullptr, stream);
+            if (s != HQ_OK) return s;
+        }
+        return HQ_OK;
+    }
+    size_t need = linear_group_workspace_bytes(ctx, ws, n_w, batch);
+    if (need > ctx->ws_bytes) {
+        if (ctx->ws) { HQ_CUDA_CHECK(ctx, cudaDeviceSynchronize()); ctx_free(ctx, ctx->ws); ctx->ws = nullptr; ctx->ws_bytes = 0; }
+        ctx->ws = ctx_alloc(ctx, need);
+        if (!ctx->ws) return HQ_ERR_ALLOC;
+        ctx->ws_bytes = need;
+    }
+    return launch_linear_group(ctx, ws, n_w, x_dev, dtype, batch, ldx, ys_bf16_dev, ldys, ys_f32_or_null, nullptr,
+                               (uint8_t*)ctx->ws, (cudaStream_t)stream);
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -130,6 +130,12 @@ void launch_decode_int8(const hq_weight* w, int8_t* codes, uint16_t* norms, cuda
 hq_status launch_linear(hq_ctx* ctx, const hq_weight* w, const void* x, int dtype, int64_t B, int64_t ldx,
                         void* y_bf16, int64_t ldy, float* y_f32, int32_t* acc_i32, uint8_t* ws, cudaStream_t st);
 size_t linear_workspace_bytes(const hq_ctx* ctx, const hq_weight* w, int64_t B);
+// several weights that share x in ONE fused launch (hq_linear_group)
+bool linear_group_compatible(const hq_weight* const* ws, int n_w);
+size_t linear_group_workspace_bytes(const hq_ctx* ctx, const hq_weight* const* ws, int n_w, int64_t B);
+hq_status launch_linear_group(hq_ctx* ctx, const hq_weight* const* ws, int n_w, const void* x, int dtype, int64_t B,
+                              int64_t ldx, void* const* ys_bf16, const int64_t* ldys, float* const* ys_f32,
+                              int32_t* acc_i32, uint8_t* wsbuf, cudaStream_t st);
 bool linear_uses_e8_fast(const hq_weight* w);
 
 // ---- KV decode + attend (hq_attend.cu) ----

@@ -4,6 +4,8 @@
 // K-major SWIZZLE_128B layout and contract with the INT8 activations on the tensor core
 // (A6, tcgen05.mma kind::i8 -> INT32 in TMEM, §4.8), then rescale per K-tile and accumulate (A7,
 // §4.3).  Decoded weights never leave shared memory.
+#include <string.h>
+
 #include "hq_common.cuh"
 #include "hq_internal.h"
 #include "hq_linear_e8.cuh"
@@ -237,28 +239,29 @@ static hq_status launch_generic_nb(hq_ctx* ctx, const hq_weight* w, LinearParams
 bool linear_uses_e8_fast(const hq_weight* w) { return w->lattice == LAT_E8 && w->n == 128 && w->k0 <= 3; }
 
 struct E8Plan { int NB, BC, NWG, n_bt, n_split, L, n_items, grid; };
-static E8Plan e8_plan(const hq_ctx* ctx, const hq_weight* w, int64_t B) {
+// plan for a group of weights that share n_in (their row blocks are stacked into one item space)
+static E8Plan e8_plan(const hq_ctx* ctx, int64_t n_rb_total, int64_t n_kt64, int64_t n_in, int64_t B) {
     E8Plan pl;
     pl.NB = B <= 16 ? 16 : 64;
     pl.BC = B == 1 ? 1 : pl.NB;
     pl.NWG = B == 1 ? 6 : (B <= 16 ? 5 : 4);
     pl.n_bt = (int)((B + pl.NB - 1) / pl.NB);
-    const int n_kt = (int)w->n_kt;
+    const int n_kt = (int)n_kt64;
     // K split: the largest divisor of n_kt whose fp32 partial sums (written + read back) stay below a quarter of
     // the compressed weight bytes; batch 1 therefore splits down to single tiles (finest load balance)
-    const double budget = 0.25 * 0.53 * (double)w->n_in / (8.0 * (double)B);
+    const double budget = 0.25 * 0.53 * (double)n_in / (8.0 * (double)B);
     int split = 1;
     for (int d = 1; d <= n_kt; ++d)
         if (n_kt % d == 0 && (double)d <= budget) split = d;
     pl.n_split = split;
     pl.L = n_kt / split;
-    pl.n_items = (int)(w->n_rb * split);
+    pl.n_items = (int)(n_rb_total * split);
     pl.grid = pl.n_items < ctx->sm_count ? pl.n_items : ctx->sm_count;
     return pl;
 }
 
 template <int NB, int BC, int NWG>
-static hq_status launch_e8_v(hq_ctx* ctx, const hq_weight* w, E8Params& p, const E8Plan& pl, cudaStream_t st) {
+static hq_status launch_e8_v(hq_ctx* ctx, int k0, E8Params& p, const E8Plan& pl, cudaStream_t st) {
     const size_t smem = e8_smem_bytes<NB, NWG>();
     dim3 grid((unsigned)pl.grid, (unsigned)pl.n_bt);
 #define HQ_LE(KK)                                                                                                   \
@@ -266,7 +269,7 @@ static hq_status launch_e8_v(hq_ctx* ctx, const hq_weight* w, E8Params& p, const
         HQ_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_linear_e8<KK, NB, BC, NWG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
         HQ_CUDA_CHECK(ctx, launch_pdl(k_linear_e8<KK, NB, BC, NWG>, grid, dim3(NWG * 128), smem, st, p));           \
         break
-    switch (w->k0) {
+    switch (k0) {
         HQ_LE(0); HQ_LE(1); HQ_LE(2); HQ_LE(3);
     }
 #undef HQ_LE
@@ -276,61 +279,109 @@ static hq_status launch_e8_v(hq_ctx* ctx, const hq_weight* w, E8Params& p, const
 
 static size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
 
-size_t linear_workspace_bytes(const hq_ctx* ctx, const hq_weight* w, int64_t B) {
-    if (linear_uses_e8_fast(w)) {
-        E8Plan pl = e8_plan(ctx, w, B);
-        return align256((size_t)pl.n_bt * w->n_kt * e8_bblob_bytes(pl.NB)) + (size_t)pl.n_split * B * w->m * 4 + 256;
+// weights that may share one launch: the E8 fast path, same n_in / k / seed (= same RHT signs) / operating point
+bool linear_group_compatible(const hq_weight* const* ws, int n_w) {
+    if (n_w < 1 || n_w > E8_MAXW) return false;
+    for (int i = 0; i < n_w; ++i) {
+        if (!linear_uses_e8_fast(ws[i])) return false;
+        if (ws[i]->n_in != ws[0]->n_in || ws[i]->k0 != ws[0]->k0 || ws[i]->seed != ws[0]->seed ||
+            ws[i]->snr_db != ws[0]->snr_db)
+            return false;
     }
+    return true;
+}
+
+size_t linear_group_workspace_bytes(const hq_ctx* ctx, const hq_weight* const* ws, int n_w, int64_t B) {
+    int64_t n_rb = 0;
+    for (int i = 0; i < n_w; ++i) n_rb += ws[i]->n_rb;
+    E8Plan pl = e8_plan(ctx, n_rb, ws[0]->n_kt, ws[0]->n_in, B);
+    size_t bytes = align256((size_t)pl.n_bt * ws[0]->n_kt * e8_bblob_bytes(pl.NB));
+    for (int i = 0; i < n_w; ++i) bytes += align256((size_t)pl.n_split * B * ws[i]->m * 4);
+    return bytes + 256;
+}
+
+size_t linear_workspace_bytes(const hq_ctx* ctx, const hq_weight* w, int64_t B) {
+    if (linear_uses_e8_fast(w)) return linear_group_workspace_bytes(ctx, &w, 1, B);
     int ns = generic_split(ctx, w, B);
     return align256((size_t)(B * w->n_in)) + align256((size_t)(B * w->n_kt) * 4) + (size_t)ns * B * w->m * 4 + 256;
 }
 
+// one activation cast, ONE fused decode + MMA launch over the stacked row blocks of all weights, one finalize each
+hq_status launch_linear_group(hq_ctx* ctx, const hq_weight* const* ws, int n_w, const void* x, int dtype, int64_t B,
+                              int64_t ldx, void* const* ys_bf16, const int64_t* ldys, float* const* ys_f32,
+                              int32_t* acc_i32, uint8_t* wsbuf, cudaStream_t st) {
+    const hq_weight* w0 = ws[0];
+    int64_t n_rb = 0;
+    for (int i = 0; i < n_w; ++i) n_rb += ws[i]->n_rb;
+    E8Plan pl = e8_plan(ctx, n_rb, w0->n_kt, w0->n_in, B);
+    uint8_t* bblob = wsbuf;
+    uint8_t* at = wsbuf + align256((size_t)pl.n_bt * w0->n_kt * e8_bblob_bytes(pl.NB));
+    launch_act_blob(x, dtype, B, w0->n_in, ldx, w0->dsign, pl.NB, bblob, st);
+    HQ_CUDA_CHECK(ctx, cudaGetLastError());
+    E8Params p;
+    memset(&p, 0, sizeof(p));
+    uint32_t min_ulen = 0xffffffffu;
+    p.rb_base[0] = 0;
+    for (int i = 0; i < n_w; ++i) {
+        p.blob[i] = ws[i]->blob; p.sub_off[i] = ws[i]->group_off; p.m[i] = ws[i]->m;
+        p.partials[i] = (float*)at;
+        at += align256((size_t)pl.n_split * B * ws[i]->m * 4);
+        p.inv_A[i] = (float)(1.0 / (ws[i]->alpha * sqrt((double)ws[i]->n)));
+        p.rb_base[i + 1] = p.rb_base[i] + (int)ws[i]->n_rb;
+        if (ws[i]->min_ulen < min_ulen) min_ulen = ws[i]->min_ulen;
+    }
+    for (int i = n_w; i < E8_MAXW; ++i) p.rb_base[i + 1] = p.rb_base[n_w];
+    p.n_w = n_w; p.lut = ctx->e8_lut;
+    p.n_kt = (int)w0->n_kt; p.n_split = pl.n_split; p.L = pl.L; p.n_items = pl.n_items;
+    p.u_dense = (int)(((min_ulen + 31) >> 5) < (uint32_t)E8_NW ? ((min_ulen + 31) >> 5) : (uint32_t)E8_NW);
+    p.bblob = bblob; p.B = B; p.acc_i32 = (n_w == 1) ? acc_i32 : nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (ctx->prof) {
+        HQ_CUDA_CHECK(ctx, cudaEventCreate(&e0));
+        HQ_CUDA_CHECK(ctx, cudaEventCreate(&e1));
+        HQ_CUDA_CHECK(ctx, cudaEventRecord(e0, st));
+    }
+    hq_status s = (B == 1)    ? launch_e8_v<16, 1, 6>(ctx, w0->k0, p, pl, st)
+                  : (B <= 16) ? launch_e8_v<16, 16, 5>(ctx, w0->k0, p, pl, st)
+                              : launch_e8_v<64, 64, 4>(ctx, w0->k0, p, pl, st);
+    if (s != HQ_OK) return s;
+    if (ctx->prof) {
+        HQ_CUDA_CHECK(ctx, cudaEventRecord(e1, st));
+        ctx->prof_ev.push_back(e0);
+        ctx->prof_ev.push_back(e1);
+    }
+    for (int i = 0; i < n_w; ++i) {
+        int64_t tot = B * ws[i]->m;
+        HQ_CUDA_CHECK(ctx, launch_pdl(k_linear_finalize, dim3((unsigned)((tot + 255) / 256)), dim3(256), 0, st,
+                                      (const float*)p.partials[i], pl.n_split, B, ws[i]->m, (__nv_bfloat16*)ys_bf16[i],
+                                      ldys[i], ys_f32 ? ys_f32[i] : (float*)nullptr));
+    }
+    return HQ_OK;
+}
+
 hq_status launch_linear(hq_ctx* ctx, const hq_weight* w, const void* x, int dtype, int64_t B, int64_t ldx,
                         void* y_bf16, int64_t ldy, float* y_f32, int32_t* acc_i32, uint8_t* ws, cudaStream_t st) {
+    if (linear_uses_e8_fast(w))
+        return launch_linear_group(ctx, &w, 1, x, dtype, B, ldx, &y_bf16, &ldy, &y_f32, acc_i32, ws, st);
     const float inv_A = (float)(1.0 / (w->alpha * sqrt((double)w->n)));
     cudaEvent_t e0 = nullptr, e1 = nullptr;
-    float* partials = nullptr;
-    int n_split = 1;
-    if (linear_uses_e8_fast(w)) {
-        E8Plan pl = e8_plan(ctx, w, B);
-        uint8_t* bblob = ws;
-        partials = (float*)(ws + align256((size_t)pl.n_bt * w->n_kt * e8_bblob_bytes(pl.NB)));
-        n_split = pl.n_split;
-        launch_act_blob(x, dtype, B, w->n_in, ldx, w->dsign, pl.NB, bblob, st);
-        HQ_CUDA_CHECK(ctx, cudaGetLastError());
-        E8Params p;
-        p.blob = w->blob; p.sub_off = w->group_off; p.lut = ctx->e8_lut; p.m = w->m;
-        p.n_kt = (int)w->n_kt; p.n_rb = (int)w->n_rb; p.n_split = pl.n_split; p.L = pl.L;
-        p.n_items = pl.n_items; p.inv_A = inv_A; p.bblob = bblob; p.B = B; p.partials = partials; p.acc_i32 = acc_i32;
-        p.u_dense = (int)(((w->min_ulen + 31) >> 5) < (uint32_t)E8_NW ? ((w->min_ulen + 31) >> 5) : (uint32_t)E8_NW);
-        if (ctx->prof) {
-            HQ_CUDA_CHECK(ctx, cudaEventCreate(&e0));
-            HQ_CUDA_CHECK(ctx, cudaEventCreate(&e1));
-            HQ_CUDA_CHECK(ctx, cudaEventRecord(e0, st));
-        }
-        hq_status s = (B == 1)    ? launch_e8_v<16, 1, 6>(ctx, w, p, pl, st)
-                      : (B <= 16) ? launch_e8_v<16, 16, 5>(ctx, w, p, pl, st)
-                                  : launch_e8_v<64, 64, 4>(ctx, w, p, pl, st);
-        if (s != HQ_OK) return s;
-    } else {
-        int8_t* q = (int8_t*)ws;
-        float* s_x = (float*)(ws + align256((size_t)(B * w->n_in)));
-        partials = (float*)((uint8_t*)s_x + align256((size_t)(B * w->n_kt) * 4));
-        n_split = generic_split(ctx, w, B);
-        launch_act_quant(x, dtype, B, w->n_in, ldx, w->lattice, w->n, w->dsign, q, s_x, nullptr, st);
-        HQ_CUDA_CHECK(ctx, cudaGetLastError());
-        LinearParams p;
-        p.blob = w->blob; p.group_off = w->group_off; p.m = w->m; p.n_kt = w->n_kt;
-        p.n = w->n; p.k0 = w->k0; p.k1 = w->k1; p.rbits = w->rbits; p.inv_A = inv_A;
-        p.q = q; p.s_x = s_x; p.B = B; p.n_split = n_split; p.partials = partials; p.acc_i32 = acc_i32;
-        if (ctx->prof) {
-            HQ_CUDA_CHECK(ctx, cudaEventCreate(&e0));
-            HQ_CUDA_CHECK(ctx, cudaEventCreate(&e1));
-            HQ_CUDA_CHECK(ctx, cudaEventRecord(e0, st));
-        }
-        hq_status s = (B <= 16) ? launch_generic_nb<16>(ctx, w, p, st) : launch_generic_nb<64>(ctx, w, p, st);
-        if (s != HQ_OK) return s;
+    int8_t* q = (int8_t*)ws;
+    float* s_x = (float*)(ws + align256((size_t)(B * w->n_in)));
+    float* partials = (float*)((uint8_t*)s_x + align256((size_t)(B * w->n_kt) * 4));
+    const int n_split = generic_split(ctx, w, B);
+    launch_act_quant(x, dtype, B, w->n_in, ldx, w->lattice, w->n, w->dsign, q, s_x, nullptr, st);
+    HQ_CUDA_CHECK(ctx, cudaGetLastError());
+    LinearParams p;
+    p.blob = w->blob; p.group_off = w->group_off; p.m = w->m; p.n_kt = w->n_kt;
+    p.n = w->n; p.k0 = w->k0; p.k1 = w->k1; p.rbits = w->rbits; p.inv_A = inv_A;
+    p.q = q; p.s_x = s_x; p.B = B; p.n_split = n_split; p.partials = partials; p.acc_i32 = acc_i32;
+    if (ctx->prof) {
+        HQ_CUDA_CHECK(ctx, cudaEventCreate(&e0));
+        HQ_CUDA_CHECK(ctx, cudaEventCreate(&e1));
+        HQ_CUDA_CHECK(ctx, cudaEventRecord(e0, st));
     }
+    hq_status s = (B <= 16) ? launch_generic_nb<16>(ctx, w, p, st) : launch_generic_nb<64>(ctx, w, p, st);
+    if (s != HQ_OK) return s;
     if (ctx->prof) {
         HQ_CUDA_CHECK(ctx, cudaEventRecord(e1, st));
         ctx->prof_ev.push_back(e0);
@@ -339,7 +390,6 @@ hq_status launch_linear(hq_ctx* ctx, const hq_weight* w, const void* x, int dtyp
     int64_t tot = B * w->m;
     HQ_CUDA_CHECK(ctx, launch_pdl(k_linear_finalize, dim3((unsigned)((tot + 255) / 256)), dim3(256), 0, st, (const float*)partials,
                                   n_split, B, w->m, (__nv_bfloat16*)y_bf16, ldy, y_f32));
-    HQ_CUDA_CHECK(ctx, cudaGetLastError());
     return HQ_OK;
 }
 

@@ -38,18 +38,21 @@ __host__ __device__ inline int e8_kcol(int j) {  // j = 8*blk + i (natural order
     return 32 * (blk >> 2) + 4 * i + (blk & 3);
 }
 
+constexpr int E8_MAXW = 4;   // weights per launch (hq_linear_group: matrices that share x, e.g. q/k/v or gate/up)
 struct E8Params {
-    const uint8_t* blob;
-    const uint32_t* sub_off;
-    const uint32_t* lut;     // global copy of the phase-1 table, E8_LUT_WORDS words
-    int64_t m;
-    int n_kt, n_rb, n_split, L, n_items;   // item = (rb, split): L = n_kt / n_split consecutive tiles
-    int u_dense;             // every present row of the tensor has at least this many U words
-    float inv_A;
-    const uint8_t* bblob;    // [n_bt][n_kt][e8_bblob_bytes(NB)]
+    const uint8_t* blob[E8_MAXW];
+    const uint32_t* sub_off[E8_MAXW];
+    int64_t m[E8_MAXW];
+    float* partials[E8_MAXW];   // [n_split][B][m_w]
+    float inv_A[E8_MAXW];
+    int rb_base[E8_MAXW + 1];   // the weights' row blocks stacked: weight w owns global row blocks [rb_base[w], rb_base[w+1])
+    int n_w;
+    const uint32_t* lut;        // global copy of the phase-1 table, E8_LUT_WORDS words
+    int n_kt, n_split, L, n_items;   // item = (global row block, split): L = n_kt / n_split consecutive tiles
+    int u_dense;                // every present row of the tensors has at least this many U words
+    const uint8_t* bblob;       // [n_bt][n_kt][e8_bblob_bytes(NB)]
     int64_t B;
-    float* partials;         // [n_split][B][m]
-    int32_t* acc_i32;        // [n_kt][B][m] or null
+    int32_t* acc_i32;           // [n_kt][B][m] or null (single weight only)
 };
 
 // Tile descriptor, three registers: the stream of tiles of one warp group is item = gw, gw + GW, ... each
@@ -57,7 +60,9 @@ struct E8Params {
 struct E8Desc {
     uint32_t gk;      // rb * n_kt + kt, bit 31 = valid
     uint32_t ks;      // kt | split << 12 | last-of-item << 31
-    uint32_t rb;
+    uint32_t rb;      // row block inside its weight | weight index << 28
+    __device__ __forceinline__ uint32_t rbl() const { return rb & 0x0fffffffu; }
+    __device__ __forceinline__ uint32_t w() const { return rb >> 28; }
     __device__ __forceinline__ bool valid() const { return (gk >> 31) != 0; }
     __device__ __forceinline__ uint32_t kt() const { return ks & 0xfffu; }
     __device__ __forceinline__ uint32_t split() const { return (ks >> 12) & 0xfffu; }
@@ -78,9 +83,14 @@ struct E8Iter {
         E8Desc d;
         const bool v = item < end;
         const int kt = split * p.L + j;
-        d.gk = (uint32_t)(rb * p.n_kt + kt) | 0x80000000u;
+        int w = 0;
+#pragma unroll
+        for (int i = 1; i < E8_MAXW; ++i)
+            if (i < p.n_w && rb >= p.rb_base[i]) w = i;
+        const int rbl = rb - p.rb_base[w];
+        d.gk = (uint32_t)(rbl * p.n_kt + kt) | 0x80000000u;
         d.ks = (uint32_t)kt | ((uint32_t)split << 12) | ((j == p.L - 1) ? 0x80000000u : 0u);
-        d.rb = (uint32_t)rb;
+        d.rb = (uint32_t)rbl | ((uint32_t)w << 28);
         if (!v) { d.gk = 0; d.ks = 0; d.rb = 0; }
         return d;
     }
@@ -154,7 +164,7 @@ k_linear_e8(E8Params p) {
         return;
     }
     auto load_off = [&](const E8Desc& d) -> uint32_t {
-        return d.valid() ? __ldg(p.sub_off + ((size_t)d.g() * 4 + warp)) : 0u;
+        return d.valid() ? __ldg(p.sub_off[d.w()] + ((size_t)d.g() * 4 + warp)) : 0u;
     };
     auto issue_b = [&](const E8Desc& d, int slot) {  // wg thread 0: TMA bulk copy of a tile's activation operand
         if (!d.valid()) return;
@@ -191,12 +201,12 @@ k_linear_e8(E8Params p) {
 #pragma unroll
         for (int j = 0; j < KW; ++j) R[j] = __ldg(rarea + j * 32 + lane);
     };
-    auto rows_full = [&](const E8Desc& d) -> bool { return (int64_t)d.rb * 128 + warp * 32 + 32 <= p.m; };
+    auto rows_full = [&](const E8Desc& d) -> bool { return (int64_t)d.rbl() * 128 + warp * 32 + 32 <= p.m[d.w()]; };
 
     uint32_t Uw[E8_NW], Rw[KW > 0 ? KW : 1];
     // prologue: offsets of tiles 0 and 1 together, then everything of tile 0 that needs only its offset
     uint32_t off_n1 = load_off(q1);
-    const uint8_t* sgp_c = p.blob + 16 * (size_t)load_off(q0);
+    const uint8_t* sgp_c = p.blob[q0.w()] + 16 * (size_t)load_off(q0);
     uint32_t ul_c = __ldg((const uint16_t*)sgp_c + lane), nrm_c = __ldg((const uint16_t*)sgp_c + 32 + lane);
     load_u_dense(sgp_c, rows_full(q0), Uw);
     load_r(sgp_c, Rw);
@@ -212,7 +222,8 @@ k_linear_e8(E8Params p) {
 
     // epilogue of tile `x` = tile number tau (its MMA has completed): drain the accumulator row, rescale, accumulate (A7)
     auto epilogue = [&](const E8Desc& x, int tau) {
-        const int64_t r = (int64_t)x.rb * 128 + t;
+        const int64_t r = (int64_t)x.rbl() * 128 + t;
+        const int64_t mw = p.m[x.w()];
         mbar_wait(&bar_b[tau & 1], (uint32_t)((tau >> 1) & 1));   // the TMA-written scales are visible to this thread
         const uint32_t sx_a = sB_a + (tau & 1) * BSLOT + NB * 128;
         const uint32_t taddr = tmem_acc + ((uint32_t)(warp * 32) << 16);
@@ -220,7 +231,7 @@ k_linear_e8(E8Params p) {
             uint32_t v;
             tmem_ld1(taddr, v);
             tmem_ld_wait();
-            if (p.acc_i32 && r < p.m) p.acc_i32[((int64_t)x.kt() * p.B + b0) * p.m + r] = (int)v;
+            if (p.acc_i32 && r < mw) p.acc_i32[((int64_t)x.kt() * p.B + b0) * mw + r] = (int)v;
             yacc[0] += (sw_prev * lds_f32(sx_a)) * (float)(int)v;
         } else {
 #pragma unroll
@@ -231,17 +242,18 @@ k_linear_e8(E8Params p) {
 #pragma unroll
                 for (int e = 0; e < 16; ++e) {
                     const int a = (int)v[e];
-                    if (p.acc_i32 && r < p.m && b0 + c0 + e < p.B) p.acc_i32[((int64_t)x.kt() * p.B + b0 + c0 + e) * p.m + r] = a;
+                    if (p.acc_i32 && r < mw && b0 + c0 + e < p.B) p.acc_i32[((int64_t)x.kt() * p.B + b0 + c0 + e) * mw + r] = a;
                     yacc[c0 + e] += (sw_prev * lds_f32(sx_a + (c0 + e) * 4)) * (float)a;
                 }
             }
         }
         tc_fence_before();
         if (x.last()) {
-            if (r < p.m) {
+            if (r < mw) {
+                float* part = p.partials[x.w()];
 #pragma unroll
                 for (int b = 0; b < BC; ++b)
-                    if (b0 + b < p.B) p.partials[((int64_t)x.split() * p.B + b0 + b) * p.m + r] = yacc[b];
+                    if (b0 + b < p.B) part[((int64_t)x.split() * p.B + b0 + b) * mw + r] = yacc[b];
             }
 #pragma unroll
             for (int b = 0; b < BC; ++b) yacc[b] = 0.0f;
@@ -264,7 +276,7 @@ k_linear_e8(E8Params p) {
                 if ((uint32_t)w < maxnw) e8_unary_word(Uw[w], lut_lane, T, acc, wo);
         }
         // the U registers are free: header and dense U words of tile tau+1 (its offset arrived an iteration ago)
-        sgp_n1 = p.blob + 16 * (size_t)off_n1;
+        sgp_n1 = p.blob[q1.w()] + 16 * (size_t)off_n1;
         if (q1.valid()) {
             ul_n1 = __ldg((const uint16_t*)sgp_n1 + lane);
             nrm_n1 = __ldg((const uint16_t*)sgp_n1 + 32 + lane);
@@ -278,8 +290,8 @@ k_linear_e8(E8Params p) {
             epilogue(prev, tau - 1);
         }
         // ---- phase 2: nibble words + remainders -> INT8 points in the A tile (A5)
-        const int64_t r = (int64_t)q0.rb * 128 + t;
-        const bool present = r < p.m && ul_c > 0;
+        const int64_t r = (int64_t)q0.rbl() * 128 + t;
+        const bool present = r < p.m[q0.w()] && ul_c > 0;
         uint32_t total = 0;
         {
             uint32_t prevWo = 15u << 24;  // e_{-1} = -1 mod 16
@@ -316,7 +328,7 @@ k_linear_e8(E8Params p) {
             load_r(sgp_n1, Rw);
             load_u_ragged(sgp_n1, ul_n1, rows_full(q1), Uw);
         }
-        const float sw_cur = f16_bits_to_f32((uint16_t)nrm_c) * p.inv_A;
+        const float sw_cur = f16_bits_to_f32((uint16_t)nrm_c) * p.inv_A[q0.w()];
         fence_proxy_async_smem();
         tc_fence_before();
         if (tau == 0) {
@@ -346,6 +358,9 @@ k_linear_e8(E8Params p) {
             break;
         }
         sgp_c = sgp_n1; ul_c = ul_n1; nrm_c = nrm_n1;
+        // pull the sub-group of tile tau+2 into L2 (no registers held): its demand loads are issued an iteration from now
+        if (q2.valid() && lane < 18)
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(p.blob[q2.w()] + 16 * (size_t)off_n2 + lane * 128));
         off_n1 = off_n2;
         q0 = q1; q1 = q2;
         q2 = it.get(p); it.next(p);

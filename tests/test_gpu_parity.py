@@ -126,6 +126,56 @@ def test_linear_acc_exact_and_outputs(ctx, lattice, n_tile, B):
     w.free()
 
 
+def test_e8_fast_kernel_falls_back_on_long_quotients_and_ragged_blocks(ctx):
+    """E8 / tile 128 runs the SWAR decoder; rows with a unary quotient >= 16 or more U words than it holds in
+    registers must come out identical through its generic fallback.  k = 0 at 5 bps makes such rows the rule;
+    the clamp row (all energy in one coordinate, G8) has a quotient near 250; m = 200 leaves absent rows."""
+    m, n_in, snr, seed = 200, 512, f32(28.73), 3
+    W = hq_synth.gaussian_weight(m, n_in, seed=5)
+    W[3] = 0.0
+    d = hqo.signs(seed, 1, n_in)[256:384].astype(np.float32)
+    had = np.array([(-1.0) ** bin(i & 5).count("1") for i in range(128)], np.float32)
+    W[7, :] = 0.0; W[7, 256:384] = d * had * 0.5
+    for k in ((0, 0), (1, 1), (3, 3)):
+        enc = hqo.encode_weights(W, hqo.E8, 128, snr, seed, k)
+        w = ctx.encode_weights(_dev(W), hqo.E8, 128, snr, seed, k)
+        for B in (1, 5):
+            x = hq_synth.activations(B, n_in, seed=40 + B)
+            q_o, sx_o = hqo.act_quant(x, hqo.E8, 128, seed)
+            acc_o, y_o = hqo.linear(enc["codes"], enc["norms"], hqo.E8, 128, snr, q_o, sx_o)
+            y, y32, acc = w.linear(_dev(x, torch.bfloat16), want_f32=True, want_acc=True)
+            assert (acc.cpu().numpy() == acc_o).all()
+            assert _rel_err(y32.cpu().numpy(), y_o) < 1e-3
+        w.free()
+
+
+def test_linear_group_is_bit_identical_to_separate_calls(ctx):
+    """hq_linear_group (q/k/v-style: several weights, one x, one fused launch) against hq_linear per weight and
+    against the oracle for the first weight."""
+    n_in, snr, seed = 1024, SNR_4BPS[hqo.E8], 11
+    shapes = [384, 130, 256]
+    Ws = [hq_synth.gaussian_weight(m, n_in, seed=70 + i, outliers=True) for i, m in enumerate(shapes)]
+    ws = [ctx.encode_weights(_dev(W, torch.bfloat16), hqo.E8, 128, snr, seed, (2, 2)) for W in Ws]
+    for B in (1, 16, 33):
+        x = _dev(hq_synth.activations(B, n_in, seed=B), torch.bfloat16)
+        ys, y32s = ctx.linear_group(ws, x, want_f32=True)
+        for w, y, y32 in zip(ws, ys, y32s):
+            y1, y1_32, _ = w.linear(x, want_f32=True)
+            assert torch.equal(y, y1) and torch.equal(y32, y1_32)
+    enc = hqo.encode_weights(Ws[0], hqo.E8, 128, snr, seed, (2, 2))
+    xh = hq_synth.activations(4, n_in, seed=3)
+    q_o, sx_o = hqo.act_quant(xh, hqo.E8, 128, seed)
+    _, y_o = hqo.linear(enc["codes"], enc["norms"], hqo.E8, 128, snr, q_o, sx_o)
+    ys, y32s = ctx.linear_group(ws, _dev(xh, torch.bfloat16), want_f32=True)
+    assert _rel_err(y32s[0].cpu().numpy(), y_o) < 1e-3
+    # weights that cannot share a launch (different seed -> different RHT signs) still give the right answers
+    w_other = ctx.encode_weights(_dev(Ws[1], torch.bfloat16), hqo.E8, 128, snr, seed + 1, (2, 2))
+    ys = ctx.linear_group([ws[0], w_other], _dev(xh, torch.bfloat16))
+    assert torch.equal(ys[1], w_other.linear(_dev(xh, torch.bfloat16)))
+    for w in ws + [w_other]:
+        w.free()
+
+
 # ------------------------------------------------------------------------------------------ KV
 def _oracle_kv_container(K, V, lattice, snr, k, rotation, dither, seed, chunks):
     """Oracle-side container for tokens appended in `chunks` (list of token counts)."""
