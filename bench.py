@@ -110,6 +110,22 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def max_over_ranks(value, device=None):
+    """Replicas only: the job's time is the slowest rank's.  No-op without a process group."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(value)
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(bytes_per_step_per_rank, ms_per_step_max, world):
+    """Whole-job throughput of N independent replicas (weak scaling): all ranks' bytes over the slowest rank's time."""
+    return world * bytes_per_step_per_rank / (ms_per_step_max * 1e-3) / 1e9
+
+
 def _time_cuda(fn, reps, warm=1):
     import torch
     for _ in range(warm):
@@ -324,11 +340,7 @@ def main():
         ms = e0.elapsed_time(e1)
         kern = ctx.profile_read() if profile else (0.0, 0)
         ctx.profile(False)
-        if world > 1:
-            import torch.distributed as dist
-            t = torch.tensor([ms], device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
+        ms = max_over_ranks(ms, dev)
         return ms, kern
 
     # ---- headline: batch 1, device-resident inputs
@@ -338,7 +350,7 @@ def main():
     sampler.stop_flag = True
     sampler.join()
     ms_per_step = ms / args.steps
-    value = world * bytes_per_step / (ms_per_step * 1e-3) / 1e9
+    value = aggregate_value(bytes_per_step, ms_per_step, world)
 
     # ---- roofline of the dominant kernel (fused decode+MMA), CUDA events around each launch
     ms_p, (kern_ms, kern_n) = timed(1, args.steps, 2, profile=True)
@@ -376,11 +388,7 @@ def main():
         e2e_step(3 + i)
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
-    if world > 1:
-        import torch.distributed as dist
-        t = torch.tensor([e2e_s], device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = max_over_ranks(e2e_s, dev)
     e2e = {"value": world * bytes_per_step * args.steps / e2e_s / 1e9, "unit": UNIT, "h2d_bytes_per_step": h2d,
            "d2h_bytes_per_step": d2h}
 

@@ -244,7 +244,7 @@ static E8Plan e8_plan(const hq_ctx* ctx, int64_t n_rb_total, int64_t n_kt64, int
     E8Plan pl;
     pl.NB = B <= 16 ? 16 : 64;
     pl.BC = B == 1 ? 1 : pl.NB;
-    pl.NWG = B == 1 ? 6 : (B <= 16 ? 5 : 4);
+    pl.NWG = B == 1 ? 6 : (B <= 16 ? 5 : 3);
     pl.n_bt = (int)((B + pl.NB - 1) / pl.NB);
     const int n_kt = (int)n_kt64;
     // K split: the largest divisor of n_kt whose fp32 partial sums (written + read back) stay below a quarter of
@@ -343,7 +343,7 @@ hq_status launch_linear_group(hq_ctx* ctx, const hq_weight* const* ws, int n_w, 
     }
     hq_status s = (B == 1)    ? launch_e8_v<16, 1, 6>(ctx, w0->k0, p, pl, st)
                   : (B <= 16) ? launch_e8_v<16, 16, 5>(ctx, w0->k0, p, pl, st)
-                              : launch_e8_v<64, 64, 4>(ctx, w0->k0, p, pl, st);
+                              : launch_e8_v<64, 64, 3>(ctx, w0->k0, p, pl, st);
     if (s != HQ_OK) return s;
     if (ctx->prof) {
         HQ_CUDA_CHECK(ctx, cudaEventRecord(e1, st));

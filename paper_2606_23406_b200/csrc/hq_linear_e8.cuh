@@ -239,11 +239,17 @@ k_linear_e8(E8Params p) {
                 uint32_t v[16];
                 tmem_ld16(taddr + c0, v);
                 tmem_ld_wait();
+                if (p.acc_i32 && r < mw) {   // parity / debug output, off the hot path
+                    for (int e = 0; e < 16; ++e)
+                        if (b0 + c0 + e < p.B) p.acc_i32[((int64_t)x.kt() * p.B + b0 + c0 + e) * mw + r] = (int)v[e];
+                }
 #pragma unroll
-                for (int e = 0; e < 16; ++e) {
-                    const int a = (int)v[e];
-                    if (p.acc_i32 && r < mw && b0 + c0 + e < p.B) p.acc_i32[((int64_t)x.kt() * p.B + b0 + c0 + e) * mw + r] = a;
-                    yacc[c0 + e] += (sw_prev * lds_f32(sx_a + (c0 + e) * 4)) * (float)a;
+                for (int e = 0; e < 4; ++e) {
+                    const uint4 s4 = lds128(sx_a + (c0 + 4 * e) * 4);
+                    yacc[c0 + 4 * e + 0] += (sw_prev * __uint_as_float(s4.x)) * (float)(int)v[4 * e + 0];
+                    yacc[c0 + 4 * e + 1] += (sw_prev * __uint_as_float(s4.y)) * (float)(int)v[4 * e + 1];
+                    yacc[c0 + 4 * e + 2] += (sw_prev * __uint_as_float(s4.z)) * (float)(int)v[4 * e + 2];
+                    yacc[c0 + 4 * e + 3] += (sw_prev * __uint_as_float(s4.w)) * (float)(int)v[4 * e + 3];
                 }
             }
         }
