@@ -4,6 +4,7 @@
 // and the V accumulation is un-rotated once at the end.  Tokens of the residual window are read
 // exactly from the bf16 ring (§6.7.2).
 #include "hq_common.cuh"
+#include "hq_e8_decode.cuh"
 #include "hq_internal.h"
 
 namespace hq {
@@ -52,6 +53,24 @@ void launch_kv_decode_int8(const hq_kv* kv, int role, int64_t t0, int64_t n, int
         default: HQ_KD(LAT_E8); break;
     }
 #undef HQ_KD
+}
+
+// one cached vector -> out(blk, c[LAT]) per lattice block: the SWAR E8 decoder of hq_e8_decode.cuh when it applies
+// (E8, head_dim 128, k <= 3), the generic decoder otherwise and for the rare rows the fast one declines
+template <int LAT, class Out>
+__device__ __forceinline__ void decode_token(const uint32_t* rem, uint32_t rpos, const uint32_t* una, uint32_t us,
+                                             uint32_t ul, int d, int k0, int k1, uint32_t lut, uint32_t scr_a, Out out) {
+    bool ok = false;
+    if (LAT == LAT_E8 && d == 128 && k0 <= 3) {
+        const uint32_t* rrow = rem + (rpos >> 5);   // rbits = 128 k: word aligned
+        switch (k0) {
+            case 0: ok = e8_decode_row_kv<0>(una, us, ul, rrow, lut, scr_a, out); break;
+            case 1: ok = e8_decode_row_kv<1>(una, us, ul, rrow, lut, scr_a, out); break;
+            case 2: ok = e8_decode_row_kv<2>(una, us, ul, rrow, lut, scr_a, out); break;
+            default: ok = e8_decode_row_kv<3>(una, us, ul, rrow, lut, scr_a, out); break;
+        }
+    }
+    if (!ok) decode_row_generic<LAT>(WordsContig{rem}, rpos, WordsContig{una}, us, d, k0, k1, out);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -103,7 +122,7 @@ __device__ inline void warp_query_transform(float* s, int d, const int8_t* dsign
 }
 
 template <int LAT>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(128, 3)
 k_attend_split(AttendParams p) {
     extern __shared__ float sm[];
     const int d = p.d, G = p.G;
@@ -112,8 +131,13 @@ k_attend_split(AttendParams p) {
     float* ps = vt + 128 * (d + 1);    // [G][128]
     float* red = ps + G * 128;         // [G][4] block reductions
     __shared__ uint32_t scan[4];
+    __shared__ uint32_t lut_s[512];    // phase-1 table of the E8 decoder, [parity][byte]
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int h = blockIdx.x / p.n_split, split = blockIdx.x % p.n_split;
+    for (int i = tid; i < 512; i += 128) lut_s[i] = unary_lut_entry(i & 255, i >> 8);
+    const uint32_t lut_a = smem_u32(lut_s);
+    // nibble scratch of the E8 decoder: the last 17 words of this thread's (otherwise idle at that time) vt row
+    const uint32_t scr_a = smem_u32(vt + tid * (d + 1) + (d - 17));
 
     for (int i = tid; i < G * d; i += 128) qs[i] = __bfloat162float(p.q[(h * G) * d + i]);
     __syncthreads();
@@ -150,7 +174,7 @@ k_attend_split(AttendParams p) {
 #pragma unroll
                 for (int g = 0; g < ATT_MAXG; ++g) dot[g] = 0.0f;
                 if (valid) {
-                    decode_row_generic<LAT>(WordsContig{rem}, (uint32_t)(t * p.rbits), WordsContig{una}, us, d, p.k0, p.k1,
+                    decode_token<LAT>(rem, (uint32_t)(t * p.rbits), una, us, ul, d, p.k0, p.k1, lut_a, scr_a,
                                             [&](int b, const int* c) {
                                                 float U[LAT];
                                                 if (p.dither) dither_block<LAT>(p.seed, (uint32_t)b, (uint32_t)t, (uint32_t)h, 0u, U);
@@ -192,7 +216,7 @@ k_attend_split(AttendParams p) {
                 // V: write v' rows to smem
                 float* row = vt + tid * (d + 1);
                 if (valid) {
-                    decode_row_generic<LAT>(WordsContig{rem}, (uint32_t)(t * p.rbits), WordsContig{una}, us, d, p.k0, p.k1,
+                    decode_token<LAT>(rem, (uint32_t)(t * p.rbits), una, us, ul, d, p.k0, p.k1, lut_a, scr_a,
                                             [&](int b, const int* c) {
                                                 float U[LAT];
                                                 if (p.dither) dither_block<LAT>(p.seed, (uint32_t)b, (uint32_t)t, (uint32_t)h, 1u, U);

@@ -40,6 +40,7 @@ __host__ __device__ inline uint32_t unary_lut_entry(uint32_t b, uint32_t par) {
 // nibble stream, acc = the partial nibble word, wo = shared-space address of the next nibble word of this row.
 // Every shift amount and every "word completed" predicate comes from prefix popcounts of x, so the only
 // loop-carried values are acc (one select per byte) and wo (one predicated add per byte).
+template <int COPIES = E8_LUT_COPIES>
 __device__ __forceinline__ void e8_unary_word(uint32_t x, uint32_t lut_lane, uint32_t& T, uint32_t& acc, uint32_t& wo) {
     // The ALU pipe (LOP3 / SHF / SEL, half rate) is the busiest unit of this kernel: the byte-prefix shift, shared by
     // the table index and the prefix popcount, is taken as the high half of a multiply (FMA pipe).  (Doing the
@@ -48,8 +49,8 @@ __device__ __forceinline__ void e8_unary_word(uint32_t x, uint32_t lut_lane, uin
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
         const uint32_t pre = (i < 3) ? __umulhi(x, 1u << (8 + 8 * i)) : x;   // x >> (24 - 8i): bytes 0..i
-        const uint32_t sel = (pre * 64u) & 0x3fc0u;                          // byte i * 64
-        N[i] = lds32_ro(lut_lane + sel + ((i & 1) ? 256 * E8_LUT_COPIES * 4 : 0));
+        const uint32_t sel = (pre * (uint32_t)(COPIES * 4)) & (uint32_t)(0xff * COPIES * 4);   // byte i * entry stride
+        N[i] = lds32_ro(lut_lane + sel + ((i & 1) ? 256 * COPIES * 4 : 0));
         Te[i] = T + 4u * (uint32_t)__popc(pre);   // nibble-stream position after byte i
     }
 #pragma unroll
@@ -113,6 +114,56 @@ __device__ __forceinline__ void e8_run(const uint32_t* W, const uint32_t* V, uin
     const uint32_t zt = (Z[7] >> 1) & 0x7f7f7f7fu;            // zigzag(t)
     const uint32_t t2 = zt ^ ((zt & 0x01010101u) * 0xffu);     // 2 t
     C[7] = ((t2 << 1) & 0xfefefefeu) | (P & 0x02020202u) | coset4;  // c_7 = 4 t + 2 parity + coset
+}
+
+// ---------------------------------------------------------------------------------------------
+// The same decoder for one KV vector (FORMAT §6): 128 symbols, U-section = `ulen` bits starting at bit `upos` of the
+// contiguous MSB-first word array `una` (the next vector's bits follow: the tail is masked), R-section = 4K words at
+// rrow.  lut = shared-space address of an un-replicated table [2][256]; scr_a = 17 words of per-thread scratch.
+// out(blk, c[8]) receives the blocks in order.  Returns false (nothing emitted) if the row needs the generic decoder.
+// ---------------------------------------------------------------------------------------------
+template <int K, class Out>
+__device__ __forceinline__ bool e8_decode_row_kv(const uint32_t* __restrict__ una, uint32_t upos, uint32_t ulen,
+                                                 const uint32_t* __restrict__ rrow, uint32_t lut, uint32_t scr_a, Out out) {
+    const uint32_t nw = (ulen + 31) >> 5;
+    if (nw > 16u) return false;
+    uint32_t T = 0, acc = 0, wo = scr_a;
+    {
+        const uint32_t wi = upos >> 5, sh = upos & 31;
+        uint32_t hi = __ldg(una + wi);
+        for (uint32_t w = 0; w < nw; ++w) {
+            const uint32_t lo = __ldg(una + wi + w + 1);
+            uint32_t x = __funnelshift_l(lo, hi, sh);
+            hi = lo;
+            const uint32_t rem = ulen - 32u * w;
+            if (rem < 32u) x &= ~(0xffffffffu >> rem);
+            e8_unary_word<1>(x, lut, T, acc, wo);
+        }
+    }
+    if (T != 4u * 128u) return false;   // a valid row has exactly 128 terminators
+    uint32_t V[4 * (K > 0 ? K : 1)];
+#pragma unroll
+    for (int j = 0; j < 4 * K; ++j) V[j] = __ldg(rrow + j);
+    uint32_t prevWo = 15u << 24, total = 0;
+    uint32_t Cs[4][8];
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+        uint32_t W[4];
+#pragma unroll
+        for (int w = 0; w < 4; ++w) W[w] = lds32(scr_a + (c * 4 + w) * 4);
+        e8_run<K>(W, V + c * K, prevWo, total, Cs[c]);
+    }
+    if (total + 128u != ulen) return false;   // a quotient >= 16 aliased
+#pragma unroll
+    for (int c = 0; c < 4; ++c)
+#pragma unroll
+        for (int b = 0; b < 4; ++b) {
+            int cc[8];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) cc[i] = (int)(int8_t)(Cs[c][i] >> (8 * b));
+            out(4 * c + b, cc);
+        }
+    return true;
 }
 
 }  // namespace hq
