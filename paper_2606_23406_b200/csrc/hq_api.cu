@@ -71,6 +71,7 @@ void hq_destroy(hq_ctx* ctx) {
     if (!ctx) return;
     ctx_free(ctx, ctx->ws);
     ctx_free(ctx, ctx->e8_lut);
+    ctx_free(ctx, ctx->e8_cnt);
     delete ctx;
 }
 

@@ -17,6 +17,10 @@ struct hq_ctx {
     void* ws = nullptr;
     size_t ws_bytes = 0;
     uint32_t* e8_lut = nullptr;  // dev: phase-1 table of the E8 fast decoder (hq_e8_decode.cuh)
+    // dev: split-arrival counters of the E8 kernel's in-kernel split-K reduction; all zero whenever no hq_linear is
+    // in flight (the last arrival resets its counter), cleared when (re)allocated
+    unsigned int* e8_cnt = nullptr;
+    size_t e8_cnt_bytes = 0;
     // optional kernel timing (hq_profile_*): event pairs around the dominant kernel of each call
     bool prof = false;
     std::vector<cudaEvent_t> prof_ev;

@@ -331,6 +331,20 @@ hq_status launch_linear_group(hq_ctx* ctx, const hq_weight* const* ws, int n_w, 
         if (ws[i]->min_ulen < min_ulen) min_ulen = ws[i]->min_ulen;
     }
     for (int i = n_w; i < E8_MAXW; ++i) p.rb_base[i + 1] = p.rb_base[n_w];
+    for (int i = 0; i < n_w; ++i) {
+        p.y_bf16[i] = (__nv_bfloat16*)ys_bf16[i]; p.ldy[i] = ldys[i]; p.y_f32[i] = ys_f32 ? ys_f32[i] : nullptr;
+    }
+    // split-arrival counters: zero whenever the kernel is not running (the last arrival resets its counter)
+    const size_t cnt_need = (size_t)n_rb * pl.n_bt * 4 * sizeof(unsigned int);
+    if (cnt_need > ctx->e8_cnt_bytes) {
+        if (ctx->e8_cnt) { HQ_CUDA_CHECK(ctx, cudaDeviceSynchronize()); ctx->alloc.free(ctx->alloc.user, ctx->e8_cnt); ctx->e8_cnt = nullptr; ctx->e8_cnt_bytes = 0; }
+        const size_t cap = cnt_need < (1u << 16) ? (1u << 16) : 2 * cnt_need;
+        ctx->e8_cnt = (unsigned int*)ctx->alloc.alloc(ctx->alloc.user, cap);
+        if (!ctx->e8_cnt) { ctx->err = "allocator returned NULL for the split counters"; return HQ_ERR_ALLOC; }
+        ctx->e8_cnt_bytes = cap;
+        HQ_CUDA_CHECK(ctx, cudaMemsetAsync(ctx->e8_cnt, 0, cap, st));
+    }
+    p.counters = ctx->e8_cnt;
     p.n_w = n_w; p.lut = ctx->e8_lut;
     p.n_kt = (int)w0->n_kt; p.n_split = pl.n_split; p.L = pl.L; p.n_items = pl.n_items;
     p.u_dense = (int)(((min_ulen + 31) >> 5) < (uint32_t)E8_NW ? ((min_ulen + 31) >> 5) : (uint32_t)E8_NW);
@@ -349,12 +363,6 @@ hq_status launch_linear_group(hq_ctx* ctx, const hq_weight* const* ws, int n_w, 
         HQ_CUDA_CHECK(ctx, cudaEventRecord(e1, st));
         ctx->prof_ev.push_back(e0);
         ctx->prof_ev.push_back(e1);
-    }
-    for (int i = 0; i < n_w; ++i) {
-        int64_t tot = B * ws[i]->m;
-        HQ_CUDA_CHECK(ctx, launch_pdl(k_linear_finalize, dim3((unsigned)((tot + 255) / 256)), dim3(256), 0, st,
-                                      (const float*)p.partials[i], pl.n_split, B, ws[i]->m, (__nv_bfloat16*)ys_bf16[i],
-                                      ldys[i], ys_f32 ? ys_f32[i] : (float*)nullptr));
     }
     return HQ_OK;
 }

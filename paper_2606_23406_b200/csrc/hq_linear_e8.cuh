@@ -10,7 +10,8 @@
 //   A6  one thread issues 4 x tcgen05.mma kind::i8 (M=128, N=NB, K=32) per tile; the activation operand tile
 //       arrives by a TMA bulk copy (already in UMMA layout, written by k_act_blob); accumulators sit in TMEM;
 //   A7  the next iteration drains the accumulator row (tcgen05.ld) and rescales by rho/(alpha sqrt n) * s_x.
-// The MMA of tile t overlaps phase 1 of tile t+1; the A tile is single-buffered per warp group.
+// The MMA of tile t overlaps phase 1 of tile t+1; the A tile is single-buffered per warp group.  The four warps of a
+// warp group never meet at a barrier: the last one to finish its rows issues the MMA.
 // blockIdx.y = batch tile (NB activation rows); blockIdx.x strides over items (rb, split).
 #pragma once
 #include "hq_common.cuh"
@@ -30,7 +31,7 @@ __host__ __device__ constexpr uint32_t e8_wg_bytes(int NB) {
 }
 template <int NB, int NWG>
 constexpr size_t e8_smem_bytes() {
-    return 1024 + (size_t)E8_LUT_BYTES + (size_t)NWG * e8_wg_bytes(NB) + 8 * (NWG * 3 + 1) + 16;
+    return 1024 + (size_t)E8_LUT_BYTES + (size_t)NWG * e8_wg_bytes(NB) + 8 * (NWG * 3 + 1) + 16 + 4 * NWG + 16;
 }
 // K index inside a tile of the code of (block blk, coordinate i) in the A / B operand tiles
 __host__ __device__ inline int e8_kcol(int j) {  // j = 8*blk + i (natural order)
@@ -44,6 +45,10 @@ struct E8Params {
     const uint32_t* sub_off[E8_MAXW];
     int64_t m[E8_MAXW];
     float* partials[E8_MAXW];   // [n_split][B][m_w]
+    __nv_bfloat16* y_bf16[E8_MAXW];   // outputs [B][ldy_w] (may be null)
+    float* y_f32[E8_MAXW];      // optional fp32 outputs [B][m_w]
+    int64_t ldy[E8_MAXW];
+    unsigned int* counters;     // [global row block][batch tile][4 warps], zero between launches: split arrivals
     float inv_A[E8_MAXW];
     int rb_base[E8_MAXW + 1];   // the weights' row blocks stacked: weight w owns global row blocks [rb_base[w], rb_base[w+1])
     int n_w;
@@ -124,12 +129,14 @@ k_linear_e8(E8Params p) {
     uint64_t* bar_mma = bars + wg * 3 + 2;  // MMA of the current tile done
     uint64_t* bar_lut = bars + NWG * 3;
     uint32_t* tmem_slot = (uint32_t*)(bars + NWG * 3 + 1);
+    uint32_t* arrive_cnt = tmem_slot + 2 + wg;   // warps of this warp group that finished their part of the A tile
 
     constexpr uint32_t TCOLS_WG = NB < 32 ? 32 : NB;
     constexpr uint32_t TCOLS = TCOLS_WG * NWG <= 128 ? 128 : (TCOLS_WG * NWG <= 256 ? 256 : 512);
     if (tid < 32) tmem_alloc(tmem_slot, TCOLS);
     if (t == 0) {
         mbar_init(&bar_b[0], 1); mbar_init(&bar_b[1], 1); mbar_init(bar_mma, 1);
+        *arrive_cnt = 0;
         if (wg == 0) mbar_init(bar_lut, 1);
         mbar_fence_init();
     }
@@ -151,6 +158,7 @@ k_linear_e8(E8Params p) {
     const int64_t b0 = (int64_t)bt * NB;
     const uint8_t* bblob_bt = p.bblob + (size_t)bt * p.n_kt * e8_bblob_bytes(NB);
     const uint32_t lane_lt = (1u << lane) - 1u;
+    const uint32_t cnt_a = smem_u32(arrive_cnt);
 
     // ---- tile queue (tau .. tau+3) and software pipeline registers
     E8Iter it;
@@ -255,14 +263,48 @@ k_linear_e8(E8Params p) {
         }
         tc_fence_before();
         if (x.last()) {
+            // split-K: this item's partial sums go to the workspace; the LAST split to arrive for these 32 rows (a
+            // per-warp counter, no block barrier) adds all of them in split order - deterministic - and writes y (A7)
+            float* part = p.partials[x.w()];
             if (r < mw) {
-                float* part = p.partials[x.w()];
 #pragma unroll
                 for (int b = 0; b < BC; ++b)
                     if (b0 + b < p.B) part[((int64_t)x.split() * p.B + b0 + b) * mw + r] = yacc[b];
             }
 #pragma unroll
             for (int b = 0; b < BC; ++b) yacc[b] = 0.0f;
+            __syncwarp();
+            unsigned int last = 0;
+            if (lane == 0) {
+                unsigned int* cnt = p.counters + (((size_t)(p.rb_base[x.w()] + x.rbl()) * gridDim.y + bt) * 4 + warp);
+                __threadfence();
+                last = atomicAdd(cnt, 1u) == (unsigned int)(p.n_split - 1);
+                if (last) *cnt = 0u;
+            }
+            last = __shfl_sync(0xffffffffu, last, 0);
+            if (last) {
+                __threadfence();
+                if (r < mw) {
+                    __nv_bfloat16* yb = p.y_bf16[x.w()];
+                    float* yf = p.y_f32[x.w()];
+                    const int64_t ldy = p.ldy[x.w()];
+                    for (int b = 0; b < BC; ++b) {
+                        if (b0 + b >= p.B) break;
+                        float sum = 0.0f;   // split order, eight loads in flight
+                        const float* pp = part + (b0 + b) * mw + r;
+                        const int64_t sstride = p.B * mw;
+                        for (int sp0 = 0; sp0 < p.n_split; sp0 += 8) {
+                            float v[8];
+#pragma unroll
+                            for (int u = 0; u < 8; ++u) v[u] = (sp0 + u < p.n_split) ? __ldcg(pp + (sp0 + u) * sstride) : 0.0f;
+#pragma unroll
+                            for (int u = 0; u < 8; ++u) sum += v[u];
+                        }
+                        if (yb) yb[(b0 + b) * ldy + r] = __float2bfloat16_rn(sum);
+                        if (yf) yf[(b0 + b) * mw + r] = sum;
+                    }
+                }
+            }
         }
     };
 
@@ -343,9 +385,18 @@ k_linear_e8(E8Params p) {
             griddep_wait();
             if (t == 0) issue_b(q0, 0);
         }
-        asm volatile("bar.sync %0, 128;" ::"r"(wg + 1) : "memory");
-        if (t == 0) {
-            issue_b(q1, (tau + 1) & 1);   // that slot's last reader, the epilogue of tile tau-1, is behind the barrier
+        // No block barrier: the last of the four warps to finish the tile issues the MMA.  (A warp cannot arrive for tile
+        // tau+1 before the MMA of tile tau was issued - it waits for its commit before phase 2 - so the arrivals of a
+        // tile are the counter values 4 tau .. 4 tau + 3.)
+        __syncwarp();
+        bool issuer = false;
+        if (lane == 0) {
+            uint32_t old;
+            asm volatile("atom.acq_rel.cta.shared::cta.add.u32 %0, [%1], 1;" : "=r"(old) : "r"(cnt_a) : "memory");
+            issuer = (old & 3u) == 3u;
+        }
+        if (issuer) {
+            issue_b(q1, (tau + 1) & 1);   // that slot's last reader, the epilogue of tile tau-1, precedes every arrival
             mbar_wait(&bar_b[tau & 1], (uint32_t)((tau >> 1) & 1));
             tc_fence_after();
             const uint32_t b0s = sB_a + (tau & 1) * BSLOT;
