@@ -247,12 +247,19 @@ static E8Plan e8_plan(const hq_ctx* ctx, int64_t n_rb_total, int64_t n_kt64, int
     pl.NWG = B == 1 ? 6 : (B <= 16 ? 5 : 3);
     pl.n_bt = (int)((B + pl.NB - 1) / pl.NB);
     const int n_kt = (int)n_kt64;
-    // K split: the largest divisor of n_kt whose fp32 partial sums (written + read back) stay below a quarter of
-    // the compressed weight bytes; batch 1 therefore splits down to single tiles (finest load balance)
-    const double budget = 0.25 * 0.53 * (double)n_in / (8.0 * (double)B);
-    int split = 1;
+    // K split.  Every item end costs a release fence + an arrival atomic per warp and one fp32 partial per row, so
+    // items should be long, but the Llama-shaped matrices have too few row blocks to fill 148 x NWG warp groups
+    // without splitting K finely.  Measured at batch 1: items of two tiles beat one and four.
+    // Never more partial-sum traffic than a quarter of the compressed weight bytes (matters for batch > 1).
+    int split = n_kt;
     for (int d = 1; d <= n_kt; ++d)
-        if (n_kt % d == 0 && (double)d <= budget) split = d;
+        if (n_kt % d == 0 && n_kt / d <= 2) { split = d; break; }
+    const double budget = 0.25 * 0.53 * (double)n_in / (8.0 * (double)B);
+    while (split > 1 && (double)split > budget) {   // next smaller divisor
+        int d = split - 1;
+        while (d > 1 && n_kt % d != 0) --d;
+        split = d;
+    }
     pl.n_split = split;
     pl.L = n_kt / split;
     pl.n_items = (int)(n_rb_total * split);

@@ -262,9 +262,7 @@ k_linear_e8(E8Params p) {
             }
         }
         tc_fence_before();
-        if (x.last()) {
-            // split-K: this item's partial sums go to the workspace; the LAST split to arrive for these 32 rows (a
-            // per-warp counter, no block barrier) adds all of them in split order - deterministic - and writes y (A7)
+        if (x.last()) {   // split-K: this item's partial sums go to the workspace (reduced after the tile loop)
             float* part = p.partials[x.w()];
             if (r < mw) {
 #pragma unroll
@@ -273,36 +271,53 @@ k_linear_e8(E8Params p) {
             }
 #pragma unroll
             for (int b = 0; b < BC; ++b) yacc[b] = 0.0f;
-            __syncwarp();
-            unsigned int last = 0;
-            if (lane == 0) {
-                unsigned int* cnt = p.counters + (((size_t)(p.rb_base[x.w()] + x.rbl()) * gridDim.y + bt) * 4 + warp);
-                __threadfence();
-                last = atomicAdd(cnt, 1u) == (unsigned int)(p.n_split - 1);
-                if (last) *cnt = 0u;
+        }
+    };
+    // split-K reduction inside the kernel: after its last tile a warp publishes its partial sums (one fence) and
+    // arrives once per item on a per-(row block, batch tile, warp) counter; the LAST of the n_split arrivals adds the
+    // partials in split order - deterministic - and writes y (A7).  No block barrier, no extra launch.
+    auto arrive = [&](const E8Desc& x) {
+        const int64_t r = (int64_t)x.rbl() * 128 + t;
+        const int64_t mw = p.m[x.w()];
+        float* part = p.partials[x.w()];
+        unsigned int last = 0;
+        if (lane == 0) {
+            unsigned int* cnt = p.counters + (((size_t)(p.rb_base[x.w()] + x.rbl()) * gridDim.y + bt) * 4 + warp);
+            last = atomicAdd(cnt, 1u) == (unsigned int)(p.n_split - 1);
+            if (last) *cnt = 0u;
+        }
+        last = __shfl_sync(0xffffffffu, last, 0);
+        if (!last) return;
+        __threadfence();
+        if (r >= mw) return;
+        __nv_bfloat16* yb = p.y_bf16[x.w()];
+        float* yf = p.y_f32[x.w()];
+        const int64_t ldy = p.ldy[x.w()];
+        constexpr int CB = BC < 4 ? BC : 4;   // columns summed together: CB x 8 loads in flight
+        const int64_t sstride = p.B * mw;
+        for (int bb = 0; bb < BC; bb += CB) {
+            if (b0 + bb >= p.B) break;
+            float sum[CB];
+#pragma unroll
+            for (int c = 0; c < CB; ++c) sum[c] = 0.0f;
+            for (int sp0 = 0; sp0 < p.n_split; sp0 += 8) {   // split order per column
+                float v[CB][8];
+#pragma unroll
+                for (int c = 0; c < CB; ++c)
+#pragma unroll
+                    for (int u = 0; u < 8; ++u)
+                        v[c][u] = (sp0 + u < p.n_split && b0 + bb + c < p.B)
+                                      ? __ldcg(part + (b0 + bb + c) * mw + r + (sp0 + u) * sstride) : 0.0f;
+#pragma unroll
+                for (int c = 0; c < CB; ++c)
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) sum[c] += v[c][u];
             }
-            last = __shfl_sync(0xffffffffu, last, 0);
-            if (last) {
-                __threadfence();
-                if (r < mw) {
-                    __nv_bfloat16* yb = p.y_bf16[x.w()];
-                    float* yf = p.y_f32[x.w()];
-                    const int64_t ldy = p.ldy[x.w()];
-                    for (int b = 0; b < BC; ++b) {
-                        if (b0 + b >= p.B) break;
-                        float sum = 0.0f;   // split order, eight loads in flight
-                        const float* pp = part + (b0 + b) * mw + r;
-                        const int64_t sstride = p.B * mw;
-                        for (int sp0 = 0; sp0 < p.n_split; sp0 += 8) {
-                            float v[8];
 #pragma unroll
-                            for (int u = 0; u < 8; ++u) v[u] = (sp0 + u < p.n_split) ? __ldcg(pp + (sp0 + u) * sstride) : 0.0f;
-#pragma unroll
-                            for (int u = 0; u < 8; ++u) sum += v[u];
-                        }
-                        if (yb) yb[(b0 + b) * ldy + r] = __float2bfloat16_rn(sum);
-                        if (yf) yf[(b0 + b) * mw + r] = sum;
-                    }
+            for (int c = 0; c < CB; ++c) {
+                if (b0 + bb + c < p.B) {
+                    if (yb) yb[(b0 + bb + c) * ldy + r] = __float2bfloat16_rn(sum[c]);
+                    if (yf) yf[(b0 + bb + c) * mw + r] = sum[c];
                 }
             }
         }
@@ -421,6 +436,19 @@ k_linear_e8(E8Params p) {
         off_n1 = off_n2;
         q0 = q1; q1 = q2;
         q2 = it.get(p); it.next(p);
+    }
+    // publish this thread's partial sums, then arrive for every item this warp group went through
+    __threadfence();
+    __syncwarp();
+    {
+        E8Iter it2;
+        it2.init(p, it_first, it_end, NWG);
+        for (;;) {
+            const E8Desc d = it2.get(p);
+            if (!d.valid()) break;
+            if (d.last()) arrive(d);
+            it2.next(p);
+        }
     }
     tc_fence_before();
     __syncthreads();
