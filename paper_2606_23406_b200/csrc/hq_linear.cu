@@ -238,13 +238,14 @@ static hq_status launch_generic_nb(hq_ctx* ctx, const hq_weight* w, LinearParams
 // ---- E8 fast path -----------------------------------------------------------------------------
 bool linear_uses_e8_fast(const hq_weight* w) { return w->lattice == LAT_E8 && w->n == 128 && w->k0 <= 3; }
 
-struct E8Plan { int NB, BC, NWG, n_bt, n_split, L, n_items, grid; };
+struct E8Plan { int NB, BC, NWG, CPS, n_bt, n_split, L, n_items, grid; };
 // plan for a group of weights that share n_in (their row blocks are stacked into one item space)
 static E8Plan e8_plan(const hq_ctx* ctx, int64_t n_rb_total, int64_t n_kt64, int64_t n_in, int64_t B) {
     E8Plan pl;
     pl.NB = B <= 16 ? 16 : 64;
     pl.BC = B == 1 ? 1 : pl.NB;
     pl.NWG = B == 1 ? 6 : (B <= 16 ? 5 : 3);
+    pl.CPS = 1;   // (two half-size CTAs per SM, to overlap launches, measured 2 % slower: DESIGN.md §6.1)
     pl.n_bt = (int)((B + pl.NB - 1) / pl.NB);
     const int n_kt = (int)n_kt64;
     // K split.  Every item end costs a release fence + an arrival atomic per warp and one fp32 partial per row, so
@@ -263,18 +264,19 @@ static E8Plan e8_plan(const hq_ctx* ctx, int64_t n_rb_total, int64_t n_kt64, int
     pl.n_split = split;
     pl.L = n_kt / split;
     pl.n_items = (int)(n_rb_total * split);
-    pl.grid = pl.n_items < ctx->sm_count ? pl.n_items : ctx->sm_count;
+    const int ctas = ctx->sm_count * pl.CPS;
+    pl.grid = pl.n_items < ctas ? pl.n_items : ctas;
     return pl;
 }
 
-template <int NB, int BC, int NWG>
+template <int NB, int BC, int NWG, int CPS>
 static hq_status launch_e8_v(hq_ctx* ctx, int k0, E8Params& p, const E8Plan& pl, cudaStream_t st) {
     const size_t smem = e8_smem_bytes<NB, NWG>();
     dim3 grid((unsigned)pl.grid, (unsigned)pl.n_bt);
 #define HQ_LE(KK)                                                                                                   \
     case KK:                                                                                                        \
-        HQ_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_linear_e8<KK, NB, BC, NWG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
-        HQ_CUDA_CHECK(ctx, launch_pdl(k_linear_e8<KK, NB, BC, NWG>, grid, dim3(NWG * 128), smem, st, p));           \
+        HQ_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_linear_e8<KK, NB, BC, NWG, CPS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+        HQ_CUDA_CHECK(ctx, launch_pdl(k_linear_e8<KK, NB, BC, NWG, CPS>, grid, dim3(NWG * 128), smem, st, p));           \
         break
     switch (k0) {
         HQ_LE(0); HQ_LE(1); HQ_LE(2); HQ_LE(3);
@@ -362,9 +364,9 @@ hq_status launch_linear_group(hq_ctx* ctx, const hq_weight* const* ws, int n_w, 
         HQ_CUDA_CHECK(ctx, cudaEventCreate(&e1));
         HQ_CUDA_CHECK(ctx, cudaEventRecord(e0, st));
     }
-    hq_status s = (B == 1)    ? launch_e8_v<16, 1, 6>(ctx, w0->k0, p, pl, st)
-                  : (B <= 16) ? launch_e8_v<16, 16, 5>(ctx, w0->k0, p, pl, st)
-                              : launch_e8_v<64, 64, 3>(ctx, w0->k0, p, pl, st);
+    hq_status s = (B == 1)    ? launch_e8_v<16, 1, 6, 1>(ctx, w0->k0, p, pl, st)
+                  : (B <= 16) ? launch_e8_v<16, 16, 5, 1>(ctx, w0->k0, p, pl, st)
+                              : launch_e8_v<64, 64, 3, 1>(ctx, w0->k0, p, pl, st);
     if (s != HQ_OK) return s;
     if (ctx->prof) {
         HQ_CUDA_CHECK(ctx, cudaEventRecord(e1, st));

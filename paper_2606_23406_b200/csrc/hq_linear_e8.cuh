@@ -109,9 +109,10 @@ struct E8Iter {
 };
 
 // K = Rice parameter, NB = MMA N (activation rows per batch tile), BC = accumulator columns drained per row
-// (1 when batch == 1, else NB), NWG = warp groups per CTA.
-template <int K, int NB, int BC, int NWG>
-__global__ void __launch_bounds__(NWG * 128, 1)
+// (1 when batch == 1, else NB), NWG = warp groups per CTA, CPS = CTAs per SM (two half-size CTAs per SM let the
+// tail of one launch overlap the prologue of the next under PDL).
+template <int K, int NB, int BC, int NWG, int CPS>
+__global__ void __launch_bounds__(NWG * 128, CPS)
 k_linear_e8(E8Params p) {
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
@@ -265,9 +266,22 @@ k_linear_e8(E8Params p) {
         if (x.last()) {   // split-K: this item's partial sums go to the workspace (reduced after the tile loop)
             float* part = p.partials[x.w()];
             if (r < mw) {
+                if (p.n_split == 1) {   // the item covered all of K: yacc is y
+                    __nv_bfloat16* yb = p.y_bf16[x.w()];
+                    float* yf = p.y_f32[x.w()];
+                    const int64_t ldy = p.ldy[x.w()];
 #pragma unroll
-                for (int b = 0; b < BC; ++b)
-                    if (b0 + b < p.B) part[((int64_t)x.split() * p.B + b0 + b) * mw + r] = yacc[b];
+                    for (int b = 0; b < BC; ++b) {
+                        if (b0 + b < p.B) {
+                            if (yb) yb[(b0 + b) * ldy + r] = __float2bfloat16_rn(yacc[b]);
+                            if (yf) yf[(b0 + b) * mw + r] = yacc[b];
+                        }
+                    }
+                } else {
+#pragma unroll
+                    for (int b = 0; b < BC; ++b)
+                        if (b0 + b < p.B) part[((int64_t)x.split() * p.B + b0 + b) * mw + r] = yacc[b];
+                }
             }
 #pragma unroll
             for (int b = 0; b < BC; ++b) yacc[b] = 0.0f;
@@ -440,7 +454,7 @@ k_linear_e8(E8Params p) {
     // publish this thread's partial sums, then arrive for every item this warp group went through
     __threadfence();
     __syncwarp();
-    {
+    if (p.n_split > 1) {
         E8Iter it2;
         it2.init(p, it_first, it_end, NWG);
         for (;;) {
