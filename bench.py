@@ -28,9 +28,9 @@ METRIC = "fused decode+INT8 GEMV % of HBM roofline; large-M INT8 TOPS vs peak"
 UNIT = "GB/s of compressed weight bytes (batch-1 GEMV, whole layer)"
 SNR_E8_4BPS = float(np.float32(22.68))   # E8 at 4.0 bps on iid Gaussian tiles (B.1 L857)
 NAMES = list(hq_synth.LLAMA_SHAPES)
-# dram__bytes_read.sum + dram__bytes_write.sum of the seven k_linear_e8 launches of one step, from the ncu --set full
-# capture summarised in profiles/r01b_e8_warpgroup_kernel.md §3 (9.39+2.48+2.48+9.40+32.44+32.45+32.61 MB)
-NCU_DRAM_BYTES_PER_STEP = 121.25e6
+# dram__bytes_read.sum + dram__bytes_write.sum of the four k_linear_e8 launches of one step, from the ncu --set full
+# capture summarised in profiles/r01c_e8_grouped_kernel.md §3 (14.02 + 9.41 + 64.73+1.66 + 32.62 MB)
+NCU_DRAM_BYTES_PER_STEP = 122.44e6
 WORKLOAD = "llama3.1-8b decoder-layer linears q/k/v/o/gate/up/down, E8 4 bps, RHT tile 128, batch 1 (BASELINE configs[1])"
 
 
@@ -359,7 +359,7 @@ def main():
     peak, peak_src = peaks()
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": NCU_DRAM_BYTES_PER_STEP / len(GROUPS), "alg_bytes_per_launch": bytes_per_step / len(GROUPS),
-                "traffic_source": "ncu --set full, profiles/r01b_e8_warpgroup_kernel.md", "kernel": "k_linear_e8<K=2,NB=16,BC=1,NWG=6>", "peak_source": peak_src,
+                "traffic_source": "ncu --set full, profiles/r01c_e8_grouped_kernel.md", "kernel": "k_linear_e8<K=2,NB=16,BC=1,NWG=6,CPS=1> (one launch per hq_linear_group)", "peak_source": peak_src,
                 "kernel_share_of_step": kern_ms / ms_p if ms_p > 0 else None,
                 "launches_timed": kern_n, "avg_launch_us": 1e3 * kern_ms / max(kern_n, 1),
                 "alg_bytes_per_scalar": bytes_per_step / scalars_per_step,
