@@ -410,6 +410,12 @@ hq_status hq_kv_append(hq_ctx* ctx, hq_kv* kv, const void* k_dev, const void* v_
     if (n_tok <= 0 || kv->n_tokens + n_tok > kv->cfg.max_tokens) return fail(ctx, HQ_ERR_SHAPE, "n_tok out of range");
     cudaStream_t st = (cudaStream_t)stream;
     int H = kv->cfg.kv_heads, d = kv->cfg.head_dim;
+    if (n_tok == 1) {   // the decode step: one fused launch
+        launch_kv_append1(kv, k_dev, v_dev, st);
+        HQ_CUDA_CHECK(ctx, cudaGetLastError());
+        kv->n_tokens += 1;
+        return HQ_OK;
+    }
     const int64_t CHUNK = 4096;
     int64_t chunk = n_tok < CHUNK ? n_tok : CHUNK;
     if (chunk > kv->scratch_tokens) {

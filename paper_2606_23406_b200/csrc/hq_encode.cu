@@ -726,4 +726,116 @@ void launch_kv_ring(const void* k, const void* v, int64_t n_tok, int H, int d, i
                                                             ring);
 }
 
+
+// ---------------------------------------------------------------------------------------------
+// One appended token, one launch (the decode-step case of hq_kv_append; a 1-token append is launch-latency
+// bound).  One warp per (head, role) runs the whole chain B1-B7 with the same device functions as the bulk kernels
+// (bit-identical container): RHT -> rotate -> normalize -> dither -> nearest point -> strip -> U length -> running
+// offset of the head's U stream -> pack R and U -> bf16 ring.
+// ---------------------------------------------------------------------------------------------
+struct KvAppend1 {
+    const __nv_bfloat16 *k, *v;    // [H][d] of the new token
+    int H, d, rotation, dither, k0, k1, rbits, window;
+    int64_t token, max_tokens, rem_words, una_words, n_blk;
+    float A;
+    uint64_t seed;
+    const int8_t *dsign, *ssign;
+    uint32_t *rem, *una, *blk_off, *upos;
+    uint16_t *ulen, *norm;
+    __nv_bfloat16* ring;
+    unsigned long long* counters;   // [0] clamps, [1] (as int) error flag
+};
+
+template <int LAT>
+__global__ void __launch_bounds__(32)
+k_kv_append1(KvAppend1 p) {
+    extern __shared__ float smf[];   // u[d] | t[d] | codes[d] (int8) | z[d] (u8)
+    const int lane = threadIdx.x, h = blockIdx.x, role = blockIdx.y, d = p.d, H = p.H;
+    float* u = smf;
+    float* t = u + d;
+    int8_t* codes = (int8_t*)(t + d);
+    uint8_t* z = (uint8_t*)(codes + d);
+    const __nv_bfloat16* x = (role ? p.v : p.k) + (int64_t)h * d;
+    for (int i = lane; i < d; i += 32) {
+        const float xv = __bfloat162float(x[i]);
+        u[i] = (p.dsign[i] < 0) ? -xv : xv;
+        if (p.window > 0) p.ring[((int64_t)(role * p.window + (p.token % p.window)) * H + h) * d + i] = x[i];
+    }
+    warp_rht_inplace(u, d, lane);
+    if (p.rotation == HQ_ROT_SIGNS)
+        for (int i = lane; i < d; i += 32)
+            if (p.ssign[i] < 0) u[i] = -u[i];
+    for (int i = lane; i < d; i += 32) t[i] = __fmul_rn(u[i], u[i]);
+    const float ss = warp_treesum(t, d, lane);
+    const uint16_t hb = f32_to_f16_bits_sat(__fsqrt_rn(ss));
+    const float rho = f16_bits_to_f32(hb);
+    const int64_t rh = (int64_t)role * H + h;
+    if (lane == 0) p.norm[rh * p.max_tokens + p.token] = hb;
+    unsigned long long clamps = 0;
+    if (rho == 0.0f) {
+        for (int i = lane; i < d; i += 32) codes[i] = 0;
+    } else {
+        const float g = __fdiv_rn(p.A, rho);
+        clamps = (unsigned long long)quantize_blocks<LAT>(u, d, g, p.dither != 0, p.seed, (uint32_t)p.token, (uint32_t)h,
+                                                          (uint32_t)role, codes, lane, nullptr);
+    }
+    for (int o = 16; o; o >>= 1) clamps += __shfl_xor_sync(0xffffffffu, clamps, o);
+    if (lane == 0 && clamps) atomicAdd(&p.counters[0], clamps);
+    __syncwarp();
+    // symbols in stream order, U length
+    uint32_t L = 0;
+    for (int b = lane; b < d / LAT; b += 32) {
+        int c[LAT], zz[LAT];
+#pragma unroll
+        for (int i = 0; i < LAT; ++i) c[i] = codes[b * LAT + i];
+        strip<LAT>(c, zz);
+#pragma unroll
+        for (int i = 0; i < LAT; ++i) {
+            const int pos = (LAT == LAT_E8) ? 32 * (b >> 2) + 8 * (i >> 1) + 2 * (b & 3) + (i & 1) : b * LAT + i;
+            z[pos] = (uint8_t)zz[i];
+            L += 1u + ((uint32_t)zz[i] >> (sym_class(LAT, i) ? p.k1 : p.k0));
+        }
+    }
+    for (int o = 16; o; o >>= 1) L += __shfl_xor_sync(0xffffffffu, L, o);
+    __syncwarp();
+    int* err_flag = (int*)(p.counters + 1);
+    if (L > 65535u) { if (lane == 0) atomicExch(err_flag, 1); L = 65535u; }
+    uint32_t ustart = 0;
+    if (lane == 0) {
+        ustart = p.upos[rh];
+        if ((p.token & 127) == 0) p.blk_off[rh * (p.n_blk + 1) + (p.token >> 7)] = ustart;
+        if ((int64_t)ustart + L > p.una_words * 32 - 64) atomicExch(err_flag, 2);
+        p.upos[rh] = ustart + L;
+        p.ulen[rh * p.max_tokens + p.token] = (uint16_t)L;
+    }
+    // pack: lane 0 writes the R-section, lane 1 the U-section (serial bit writers; 2 x 128 symbols)
+    ustart = __shfl_sync(0xffffffffu, ustart, 0);
+    if (lane == 0) {
+        BitWriter<StoreAtomicOr> bwr(StoreAtomicOr{p.rem + rh * p.rem_words}, (uint32_t)(p.token * p.rbits));
+        write_R<LAT>(bwr, z, d, p.k0, p.k1);
+    } else if (lane == 1) {
+        BitWriter<StoreAtomicOr> bwu(StoreAtomicOr{p.una + rh * p.una_words}, ustart);
+        write_U<LAT>(bwu, z, d, p.k0, p.k1);
+    }
+}
+
+void launch_kv_append1(const hq_kv* kv, const void* k, const void* v, cudaStream_t st) {
+    KvAppend1 p;
+    p.k = (const __nv_bfloat16*)k; p.v = (const __nv_bfloat16*)v;
+    p.H = kv->cfg.kv_heads; p.d = kv->cfg.head_dim; p.rotation = kv->cfg.rotation; p.dither = kv->cfg.dither;
+    p.k0 = kv->k0; p.k1 = kv->k1; p.rbits = kv->rbits; p.window = kv->cfg.window;
+    p.token = kv->n_tokens; p.max_tokens = kv->cfg.max_tokens; p.rem_words = kv->rem_words; p.una_words = kv->una_words;
+    p.n_blk = kv->n_blk; p.A = kv->A; p.seed = kv->cfg.codec.seed; p.dsign = kv->dsign; p.ssign = kv->ssign;
+    p.rem = kv->rem; p.una = kv->una; p.blk_off = kv->blk_off; p.upos = kv->upos; p.ulen = kv->ulen; p.norm = kv->norm;
+    p.ring = kv->ring; p.counters = kv->counters;
+    const size_t smem = (size_t)p.d * (4 + 4 + 1 + 1);
+    dim3 grid((unsigned)p.H, 2);
+    switch (kv->cfg.codec.lattice) {
+        case LAT_Z: k_kv_append1<LAT_Z><<<grid, 32, smem, st>>>(p); break;
+        case LAT_A2: k_kv_append1<LAT_A2><<<grid, 32, smem, st>>>(p); break;
+        case LAT_D4: k_kv_append1<LAT_D4><<<grid, 32, smem, st>>>(p); break;
+        default: k_kv_append1<LAT_E8><<<grid, 32, smem, st>>>(p); break;
+    }
+}
+
 }  // namespace hq

@@ -125,6 +125,8 @@ void launch_kv_pack(const int8_t* codes /*[n_tok,H,d]*/, int64_t n_tok, int H, i
                     int lattice, int k0, int k1, int rbits, int64_t max_tokens, int64_t rem_words,
                     int64_t una_words, int64_t n_blk, uint32_t* rem, uint32_t* una, uint16_t* ulen,
                     uint32_t* blk_off, uint32_t* upos, int* err_flag, cudaStream_t st);
+// one token, one launch: the whole append chain incl. the ring (bit-identical to the bulk kernels)
+void launch_kv_append1(const hq_kv* kv, const void* k, const void* v, cudaStream_t st);
 void launch_kv_ring(const void* k, const void* v, int64_t n_tok, int H, int d, int64_t token0, int window,
                     __nv_bfloat16* ring, cudaStream_t st);
 
