@@ -121,7 +121,8 @@ hq_status hq_act_quant(hq_ctx* ctx, const hq_weight* w, const void* x_dev, int32
  * acc[kt,b,r] = sum_{i in tile kt} c[r,i] * q[b,i]  (INT32, tcgen05.mma kind::i8).
  * x [batch, n_in] dev (ldx), y [batch, m_out] bf16 dev (ldy).  Optional debug outputs (dev, may be
  * NULL): y_f32 [batch, m_out] (the value before the bf16 cast), acc_i32 [n_kt, batch, m_out].
- * The decoded weights exist only in shared memory.  Any batch >= 1 (tiles of up to 256 rows of x).
+ * The decoded weights exist only in shared memory.  Any batch >= 1 (x is processed in tiles of 16 or 64 rows).
+ * E8 / tile 128 / k <= 3 runs the SWAR kernel with the split-K reduction inside; everything else the generic kernel.
  */
 hq_status hq_linear(hq_ctx* ctx, const hq_weight* w, const void* x_dev, int32_t dtype, int64_t batch,
                     int64_t ldx, void* y_bf16_dev, int64_t ldy, float* y_f32_dev_or_null,

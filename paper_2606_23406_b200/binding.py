@@ -209,7 +209,7 @@ class Weight:
             self.h = None
 
     def export(self):
-        """(blob uint8 [blob_bytes], group_off uint32 [G+1]) as host numpy arrays."""
+        """(blob uint8 [blob_bytes], sub_off uint32 [n_groups+1]) as host numpy arrays (FORMAT §5)."""
         blob_p, goff_p = C.c_void_p(), C.c_void_p()
         self.ctx.check(self.ctx.lib.hq_weight_export(self.h, C.byref(blob_p), C.byref(goff_p)))
         torch.cuda.synchronize(self.ctx.device)

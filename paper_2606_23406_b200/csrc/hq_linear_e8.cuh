@@ -3,16 +3,19 @@
 // Persistent CTA of NWG independent warp groups (128 threads each, one CTA per SM).  A warp group owns a
 // stream of tiles (row block rb, K-tile kt); lane = weight row, warp = sub-group (FORMAT §5):
 //   A3  coalesced 128-byte loads of the sub-group's U / R words straight into registers, software pipeline
-//       offset(t+3) -> header(t+2) -> words(t+1), no shared-memory staging of the bitstream;
+//       offset(t+2) -> header + dense words(t+1) -> ragged words(t+1), L2 prefetch of t+2, no shared-memory staging
+//       of the bitstream;
 //   A4  phase 1 of hq_e8_decode.cuh: unary section -> nibble stream (shared-memory scratch, conflict-free);
 //   A5  phase 2: gaps + remainders -> INT8 lattice points, SWAR over four blocks, written with 128-bit stores into
 //       the K-major SWIZZLE_128B A operand tile (decoded weights never leave shared memory);
 //   A6  one thread issues 4 x tcgen05.mma kind::i8 (M=128, N=NB, K=32) per tile; the activation operand tile
 //       arrives by a TMA bulk copy (already in UMMA layout, written by k_act_blob); accumulators sit in TMEM;
-//   A7  the next iteration drains the accumulator row (tcgen05.ld) and rescales by rho/(alpha sqrt n) * s_x.
+//   A7  the next iteration drains the accumulator row (tcgen05.ld) and rescales by rho/(alpha sqrt n) * s_x; split-K
+//       partial sums are reduced in-kernel by the last split to arrive (deterministic order).
 // The MMA of tile t overlaps phase 1 of tile t+1; the A tile is single-buffered per warp group.  The four warps of a
 // warp group never meet at a barrier: the last one to finish its rows issues the MMA.
-// blockIdx.y = batch tile (NB activation rows); blockIdx.x strides over items (rb, split).
+// blockIdx.y = batch tile (NB activation rows); CTA blockIdx.x owns a contiguous range of items (row block, split);
+// up to E8_MAXW weights that share x are stacked into one item space (hq_linear_group).
 #pragma once
 #include "hq_common.cuh"
 #include "hq_e8_decode.cuh"
@@ -60,8 +63,7 @@ struct E8Params {
     int32_t* acc_i32;           // [n_kt][B][m] or null (single weight only)
 };
 
-// Tile descriptor, three registers: the stream of tiles of one warp group is item = gw, gw + GW, ... each
-// with L consecutive K-tiles; advanced without divisions.
+// Tile descriptor, three registers; the stream of tiles of one warp group is advanced without divisions.
 struct E8Desc {
     uint32_t gk;      // rb * n_kt + kt, bit 31 = valid
     uint32_t ks;      // kt | split << 12 | last-of-item << 31
@@ -161,7 +163,7 @@ k_linear_e8(E8Params p) {
     const uint32_t lane_lt = (1u << lane) - 1u;
     const uint32_t cnt_a = smem_u32(arrive_cnt);
 
-    // ---- tile queue (tau .. tau+3) and software pipeline registers
+    // ---- tile queue (tau .. tau+2) and software pipeline registers
     E8Iter it;
     it.init(p, it_first, it_end, NWG);
     E8Desc q0 = it.get(p); it.next(p);
