@@ -356,7 +356,7 @@ hq_status launch_linear_group(hq_ctx* ctx, const hq_weight* const* ws, int n_w, 
     p.counters = ctx->e8_cnt;
     p.n_w = n_w; p.lut = ctx->e8_lut;
     p.n_kt = (int)w0->n_kt; p.n_split = pl.n_split; p.L = pl.L; p.n_items = pl.n_items;
-    p.u_dense = (int)(((min_ulen + 31) >> 5) < (uint32_t)E8_NW ? ((min_ulen + 31) >> 5) : (uint32_t)E8_NW);
+    p.u_dense = ((min_ulen + 31) >> 5) >= (uint32_t)E8_DENSE ? E8_DENSE : 0;
     p.bblob = bblob; p.B = B; p.acc_i32 = (n_w == 1) ? acc_i32 : nullptr;
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     if (ctx->prof) {

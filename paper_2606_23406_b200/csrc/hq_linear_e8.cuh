@@ -24,6 +24,7 @@
 
 namespace hq {
 
+constexpr int E8_DENSE = 8;        // U word-rows assumed present in every row of a full sub-group when u_dense says so
 constexpr int E8_NW = 10;          // U words per row handled by the fast path (tile 128: 8.1 on average at 4 bps)
 constexpr int E8_SCR_STRIDE = 17;  // nibble words per row + 1 (bank-conflict-free)
 
@@ -185,21 +186,32 @@ k_linear_e8(E8Params p) {
     };
     // a sub-group whose 32 rows are all present has at least p.u_dense words in every row: those word-rows are
     // dense (no rank needed); the rest are compacted (FORMAT §5)
-    auto load_u_dense = [&](const uint8_t* sgp, bool full_rows, uint32_t* U) {   // needs only the offset
-        const uint32_t* uarea = (const uint32_t*)(sgp + 128) + KW * 32;
-        const uint32_t dense = full_rows ? (uint32_t)p.u_dense : 0u;
+    // U word-rows.  In a sub-group whose 32 rows are all present every row has at least p.u_dense words; the launcher
+    // passes u_dense = E8_DENSE (8: the common case at tile 128, 2 unary bits per symbol) or 0.  Dense word-rows need
+    // only the sub-group offset; the rest are compacted (FORMAT §5) and need the header.
+    auto is_dense = [&](bool full_rows) -> bool { return full_rows && p.u_dense >= E8_DENSE; };   // warp-uniform
+    auto load_u_dense = [&](const uint8_t* sgp, bool full_rows, uint32_t* U) {
+        if (!is_dense(full_rows)) return;
+        const uint32_t* ua = (const uint32_t*)(sgp + 128) + KW * 32 + lane;
 #pragma unroll
-        for (int w = 0; w < E8_NW; ++w)
-            if ((uint32_t)w < dense) U[w] = __ldg(uarea + w * 32 + lane);
+        for (int w = 0; w < E8_DENSE; ++w) U[w] = __ldg(ua + w * 32);
     };
-    auto load_u_ragged = [&](const uint8_t* sgp, uint32_t ul, bool full_rows, uint32_t* U) {   // needs the header
+    auto load_u_ragged = [&](const uint8_t* sgp, uint32_t ul, bool full_rows, uint32_t* U) {
         const uint32_t* uarea = (const uint32_t*)(sgp + 128) + KW * 32;
         const uint32_t nw = (ul + 31) >> 5;
-        const uint32_t dense = full_rows ? (uint32_t)p.u_dense : 0u;
-        uint32_t base = dense * 32;
+        if (is_dense(full_rows)) {
+            uint32_t base = E8_DENSE * 32;
 #pragma unroll
-        for (int w = 0; w < E8_NW; ++w) {
-            if ((uint32_t)w >= dense) {
+            for (int w = E8_DENSE; w < E8_NW; ++w) {
+                const bool has = nw > (uint32_t)w;
+                const uint32_t mk = __ballot_sync(0xffffffffu, has);
+                U[w] = has ? __ldg(uarea + base + __popc(mk & lane_lt)) : 0u;
+                base += __popc(mk);
+            }
+        } else {
+            uint32_t base = 0;
+#pragma unroll
+            for (int w = 0; w < E8_NW; ++w) {
                 const bool has = nw > (uint32_t)w;
                 const uint32_t mk = __ballot_sync(0xffffffffu, has);
                 U[w] = has ? __ldg(uarea + base + __popc(mk & lane_lt)) : 0u;
@@ -351,8 +363,8 @@ k_linear_e8(E8Params p) {
         {
             uint32_t T = 0, acc = 0, wo = scr_a;
 #pragma unroll
-            for (int w = 0; w < E8_NW; ++w)
-                if ((uint32_t)w < maxnw) e8_unary_word(Uw[w], lut_lane, T, acc, wo);
+            for (int w = 0; w < E8_NW; ++w)   // an absent word is zero: no terminators, nothing appended
+                if (w < E8_DENSE || (uint32_t)w < maxnw) e8_unary_word(Uw[w], lut_lane, T, acc, wo);
         }
         // the U registers are free: header and dense U words of tile tau+1 (its offset arrived an iteration ago)
         sgp_n1 = p.blob[q1.w()] + 16 * (size_t)off_n1;
