@@ -40,12 +40,34 @@ __host__ __device__ inline uint32_t unary_lut_entry(uint32_t b, uint32_t par) {
 // nibble stream, acc = the partial nibble word, wo = shared-space address of the next nibble word of this row.
 // Every shift amount and every "word completed" predicate comes from prefix popcounts of x, so the only
 // loop-carried values are acc (one select per byte) and wo (one predicated add per byte).
+// nbytes (warp-uniform, 1..4): only the first nbytes stream bytes of x can hold terminators (the tail words of a row)
 template <int COPIES = E8_LUT_COPIES>
-__device__ __forceinline__ void e8_unary_word(uint32_t x, uint32_t lut_lane, uint32_t& T, uint32_t& acc, uint32_t& wo) {
+__device__ __forceinline__ void e8_unary_word(uint32_t x, uint32_t lut_lane, uint32_t& T, uint32_t& acc, uint32_t& wo,
+                                              int nbytes = 4) {
     // The ALU pipe (LOP3 / SHF / SEL, half rate) is the busiest unit of this kernel: the byte-prefix shift, shared by
     // the table index and the prefix popcount, is taken as the high half of a multiply (FMA pipe).  (Doing the
     // variable shifts of the append as multiplies too was measured slower: IMAD.HI is quarter rate.)
     uint32_t N[4], Te[4];
+    if (nbytes < 4) {   // tail word: byte by byte (a skipped byte is zero: it would append nothing)
+        uint32_t Tb = T;
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+            if (i < nbytes) {
+                const uint32_t pre = __umulhi(x, 1u << (8 + 8 * i));
+                const uint32_t sel = (pre * (uint32_t)(COPIES * 4)) & (uint32_t)(0xff * COPIES * 4);
+                const uint32_t Ni = lds32_ro(lut_lane + sel + ((i & 1) ? 256 * COPIES * 4 : 0));
+                const uint32_t Tei = T + 4u * (uint32_t)__popc(pre);
+                const uint32_t out0 = acc | __funnelshift_l(0u, Ni, Tb);
+                const uint32_t out1 = __funnelshift_l(Ni, 0u, Tb);
+                const bool full = ((Tei ^ Tb) & 32u) != 0u;
+                if (full) { sts32(wo, out0); wo += 4; }
+                acc = full ? out1 : out0;
+                Tb = Tei;
+            }
+        }
+        T = Tb;
+        return;
+    }
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
         const uint32_t pre = (i < 3) ? __umulhi(x, 1u << (8 + 8 * i)) : x;   // x >> (24 - 8i): bytes 0..i

@@ -359,12 +359,19 @@ k_linear_e8(E8Params p) {
 
         // ---- phase 1: unary section -> nibble words (A4)
         const uint32_t nw = (ul_c + 31) >> 5;
-        const uint32_t maxnw = __reduce_max_sync(0xffffffffu, nw);
+        const uint32_t maxul = __reduce_max_sync(0xffffffffu, ul_c);   // longest U-section of the sub-group, bits
+        const uint32_t maxnw = (maxul + 31) >> 5;
         {
             uint32_t T = 0, acc = 0, wo = scr_a;
 #pragma unroll
-            for (int w = 0; w < E8_NW; ++w)   // an absent word is zero: no terminators, nothing appended
-                if (w < E8_DENSE || (uint32_t)w < maxnw) e8_unary_word(Uw[w], lut_lane, T, acc, wo);
+            for (int w = 0; w < E8_NW; ++w) {   // an absent word is zero: no terminators, nothing appended
+                if (w < E8_DENSE) {
+                    e8_unary_word(Uw[w], lut_lane, T, acc, wo);
+                } else if ((uint32_t)w < maxnw) {   // tail words: only the bytes some row of the warp still uses
+                    const int nb = (int)min(4u, (maxul - 32u * (uint32_t)w + 7u) >> 3);
+                    e8_unary_word(Uw[w], lut_lane, T, acc, wo, nb);
+                }
+            }
         }
         // the U registers are free: header and dense U words of tile tau+1 (its offset arrived an iteration ago)
         sgp_n1 = p.blob[q1.w()] + 16 * (size_t)off_n1;
