@@ -29,8 +29,8 @@ UNIT = "GB/s of compressed weight bytes (batch-1 GEMV, whole layer)"
 SNR_E8_4BPS = float(np.float32(22.68))   # E8 at 4.0 bps on iid Gaussian tiles (B.1 L857)
 NAMES = list(hq_synth.LLAMA_SHAPES)
 # dram__bytes_read.sum + dram__bytes_write.sum of the four k_linear_e8 launches of one step, from the ncu --set full
-# capture summarised in profiles/r01c_e8_grouped_kernel.md §3 (14.02 + 9.41 + 64.73+1.66 + 32.62 MB)
-NCU_DRAM_BYTES_PER_STEP = 122.44e6
+# capture summarised in profiles/r01c_e8_grouped_kernel.md §3 (14.01 + 9.40 + 64.73+0.57 + 32.62 MB)
+NCU_DRAM_BYTES_PER_STEP = 121.34e6
 WORKLOAD = "llama3.1-8b decoder-layer linears q/k/v/o/gate/up/down, E8 4 bps, RHT tile 128, batch 1 (BASELINE configs[1])"
 
 
