@@ -13,6 +13,10 @@
  *    hq_create; the library never calls cudaMalloc itself.
  *  - Every call returns an hq_status; nothing throws or aborts.  hq_last_error() gives the text.
  *  - There is no CPU fallback: a device that is not compute capability 10.x gives HQ_ERR_UNSUPPORTED.
+ *  - A context serializes its work: hq_linear / hq_linear_group share one context-owned workspace (activation
+ *    operand tiles, split-K partial sums, arrival counters), so calls on one hq_ctx must be issued to one stream at a
+ *    time.  The workspace grows on demand (which synchronizes the device): call each shape once eagerly before
+ *    capturing the calls into a CUDA graph.  Results are deterministic (fixed summation order).
  */
 #ifndef HQ_H_
 #define HQ_H_
