@@ -31,6 +31,8 @@ NAMES = list(hq_synth.LLAMA_SHAPES)
 # dram__bytes_read.sum + dram__bytes_write.sum of the four k_linear_e8 launches of one step, from the ncu --set full
 # capture summarised in profiles/r01c_e8_grouped_kernel.md §3 (14.01 + 9.40 + 64.73+0.57 + 32.62 MB)
 NCU_DRAM_BYTES_PER_STEP = 121.34e6
+# smsp__inst_executed.sum of the same four launches (10.24 + 7.17 + 43.85 + 22.43 M warp-instructions)
+NCU_WARP_INSTR_PER_STEP = 83.69e6
 WORKLOAD = "llama3.1-8b decoder-layer linears q/k/v/o/gate/up/down, E8 4 bps, RHT tile 128, batch 1 (BASELINE configs[1])"
 
 
@@ -364,6 +366,16 @@ def main():
                 "launches_timed": kern_n, "avg_launch_us": 1e3 * kern_ms / max(kern_n, 1),
                 "alg_bytes_per_scalar": bytes_per_step / scalars_per_step,
                 "frac_of_nominal_8TBs": achieved / 8000.0}
+    # co-bound: the kernel is limited by the ALU work of the Rice decode.  Issue rate achieved =
+    # warp-instructions of the four launches (ncu) / (their summed duration x SMs x SM clock); peak = 4 warp-instr/clk/SM
+    sm_clock_hz, n_sms = 1.965e9, 148
+    kern_s_per_step = kern_ms * 1e-3 / args.steps if kern_ms > 0 else float("nan")
+    ipc = NCU_WARP_INSTR_PER_STEP / (kern_s_per_step * n_sms * sm_clock_hz)
+    roofline["co_bound"] = {"bound": "alu", "achieved": ipc, "peak": 4.0, "unit": "warp-instr/clk/SM", "frac": ipc / 4.0,
+                            "lane_instr_per_scalar": NCU_WARP_INSTR_PER_STEP * 32 / scalars_per_step,
+                            "budget_for_70pct_hbm_lane_instr_per_scalar": n_sms * 128 * sm_clock_hz /
+                            (0.70 * peak * 1e9 / (bytes_per_step / scalars_per_step)),
+                            "source": "instruction count: ncu, profiles/r01c_e8_grouped_kernel.md; peak: profiles/r01_issue_rates.md"}
 
     # ---- end to end: host (pinned) x -> device, linears, y -> host, every step.  The step's two activation vectors
     # live in one pinned buffer and its seven outputs in one device / one pinned buffer, so a step is ONE H2D copy,
