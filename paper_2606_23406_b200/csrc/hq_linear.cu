@@ -263,7 +263,7 @@ static E8Plan e8_plan(const hq_ctx* ctx, int64_t n_rb_total, int64_t n_kt64, int
     }
     pl.n_split = split;
     pl.L = n_kt / split;
-    pl.n_items = (int)(n_rb_total * split);
+    pl.n_items = (int)(n_rb_total * pl.n_bt * split);
     const int ctas = ctx->sm_count * pl.CPS;
     pl.grid = pl.n_items < ctas ? pl.n_items : ctas;
     return pl;
@@ -272,7 +272,7 @@ static E8Plan e8_plan(const hq_ctx* ctx, int64_t n_rb_total, int64_t n_kt64, int
 template <int NB, int BC, int NWG, int CPS>
 static hq_status launch_e8_v(hq_ctx* ctx, int k0, E8Params& p, const E8Plan& pl, cudaStream_t st) {
     const size_t smem = e8_smem_bytes<NB, NWG>();
-    dim3 grid((unsigned)pl.grid, (unsigned)pl.n_bt);
+    dim3 grid((unsigned)pl.grid);
 #define HQ_LE(KK)                                                                                                   \
     case KK:                                                                                                        \
         HQ_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_linear_e8<KK, NB, BC, NWG, CPS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
@@ -355,7 +355,7 @@ hq_status launch_linear_group(hq_ctx* ctx, const hq_weight* const* ws, int n_w, 
     }
     p.counters = ctx->e8_cnt;
     p.n_w = n_w; p.lut = ctx->e8_lut;
-    p.n_kt = (int)w0->n_kt; p.n_split = pl.n_split; p.L = pl.L; p.n_items = pl.n_items;
+    p.n_kt = (int)w0->n_kt; p.n_split = pl.n_split; p.L = pl.L; p.n_items = pl.n_items; p.n_bt = pl.n_bt;
     p.u_dense = ((min_ulen + 31) >> 5) >= (uint32_t)E8_DENSE ? E8_DENSE : 0;
     p.bblob = bblob; p.B = B; p.acc_i32 = (n_w == 1) ? acc_i32 : nullptr;
     cudaEvent_t e0 = nullptr, e1 = nullptr;

@@ -14,7 +14,7 @@
 //       partial sums are reduced in-kernel by the last split to arrive (deterministic order).
 // The MMA of tile t overlaps phase 1 of tile t+1; the A tile is single-buffered per warp group.  The four warps of a
 // warp group never meet at a barrier: the last one to finish its rows issues the MMA.
-// blockIdx.y = batch tile (NB activation rows); CTA blockIdx.x owns a contiguous range of items (row block, split);
+// CTA blockIdx.x owns a contiguous range of items (row block, batch tile of NB activation rows, split);
 // up to E8_MAXW weights that share x are stacked into one item space (hq_linear_group).
 #pragma once
 #include "hq_common.cuh"
@@ -57,7 +57,8 @@ struct E8Params {
     int rb_base[E8_MAXW + 1];   // the weights' row blocks stacked: weight w owns global row blocks [rb_base[w], rb_base[w+1])
     int n_w;
     const uint32_t* lut;        // global copy of the phase-1 table, E8_LUT_WORDS words
-    int n_kt, n_split, L, n_items;   // item = (global row block, split): L = n_kt / n_split consecutive tiles
+    int n_kt, n_split, L, n_items;   // item = (global row block, batch tile, split): L = n_kt / n_split consecutive tiles
+    int n_bt;                   // batch tiles of NB activation rows; adjacent items share the row block (weights stay hot)
     int u_dense;                // every present row of the tensors has at least this many U words
     const uint8_t* bblob;       // [n_bt][n_kt][e8_bblob_bytes(NB)]
     int64_t B;
@@ -68,8 +69,9 @@ struct E8Params {
 struct E8Desc {
     uint32_t gk;      // rb * n_kt + kt, bit 31 = valid
     uint32_t ks;      // kt | split << 12 | last-of-item << 31
-    uint32_t rb;      // row block inside its weight | weight index << 28
-    __device__ __forceinline__ uint32_t rbl() const { return rb & 0x0fffffffu; }
+    uint32_t rb;      // row block inside its weight (16 bits) | batch tile << 16 (12 bits) | weight index << 28
+    __device__ __forceinline__ uint32_t rbl() const { return rb & 0xffffu; }
+    __device__ __forceinline__ uint32_t bt() const { return (rb >> 16) & 0xfffu; }
     __device__ __forceinline__ uint32_t w() const { return rb >> 28; }
     __device__ __forceinline__ bool valid() const { return (gk >> 31) != 0; }
     __device__ __forceinline__ uint32_t kt() const { return ks & 0xfffu; }
@@ -91,14 +93,16 @@ struct E8Iter {
         E8Desc d;
         const bool v = item < end;
         const int kt = split * p.L + j;
+        int rbg = rb, bt = 0;                                  // `rb` counts (global row block, batch tile) pairs
+        if (p.n_bt > 1) { rbg = rb / p.n_bt; bt = rb - rbg * p.n_bt; }
         int w = 0;
 #pragma unroll
         for (int i = 1; i < E8_MAXW; ++i)
-            if (i < p.n_w && rb >= p.rb_base[i]) w = i;
-        const int rbl = rb - p.rb_base[w];
+            if (i < p.n_w && rbg >= p.rb_base[i]) w = i;
+        const int rbl = rbg - p.rb_base[w];
         d.gk = (uint32_t)(rbl * p.n_kt + kt) | 0x80000000u;
         d.ks = (uint32_t)kt | ((uint32_t)split << 12) | ((j == p.L - 1) ? 0x80000000u : 0u);
-        d.rb = (uint32_t)rbl | ((uint32_t)w << 28);
+        d.rb = (uint32_t)rbl | ((uint32_t)bt << 16) | ((uint32_t)w << 28);
         if (!v) { d.gk = 0; d.ks = 0; d.rb = 0; }
         return d;
     }
@@ -158,9 +162,6 @@ k_linear_e8(E8Params p) {
     const uint32_t sA_a = sA_base + (uint32_t)((t >> 3) * 1024 + (t & 7) * 128);   // this row of the A tile
     const int it_first = (int)(((int64_t)blockIdx.x * p.n_items) / gridDim.x) + wg;
     const int it_end = (int)(((int64_t)(blockIdx.x + 1) * p.n_items) / gridDim.x);
-    const int bt = blockIdx.y;
-    const int64_t b0 = (int64_t)bt * NB;
-    const uint8_t* bblob_bt = p.bblob + (size_t)bt * p.n_kt * e8_bblob_bytes(NB);
     const uint32_t lane_lt = (1u << lane) - 1u;
     const uint32_t cnt_a = smem_u32(arrive_cnt);
 
@@ -182,7 +183,7 @@ k_linear_e8(E8Params p) {
         if (!d.valid()) return;
         mbar_arrive_expect_tx(&bar_b[slot], e8_bblob_bytes(NB));
         bulk_g2s(smem + E8_LUT_BYTES + (size_t)wg * WG_BYTES + 16384 + slot * BSLOT,
-                 bblob_bt + (size_t)d.kt() * e8_bblob_bytes(NB), e8_bblob_bytes(NB), &bar_b[slot]);
+                 p.bblob + ((size_t)d.bt() * p.n_kt + d.kt()) * e8_bblob_bytes(NB), e8_bblob_bytes(NB), &bar_b[slot]);
     };
     // a sub-group whose 32 rows are all present has at least p.u_dense words in every row: those word-rows are
     // dense (no rank needed); the rest are compacted (FORMAT §5)
@@ -247,6 +248,7 @@ k_linear_e8(E8Params p) {
     auto epilogue = [&](const E8Desc& x, int tau) {
         const int64_t r = (int64_t)x.rbl() * 128 + t;
         const int64_t mw = p.m[x.w()];
+        const int64_t b0 = (int64_t)x.bt() * NB;
         mbar_wait(&bar_b[tau & 1], (uint32_t)((tau >> 1) & 1));   // the TMA-written scales are visible to this thread
         const uint32_t sx_a = sB_a + (tau & 1) * BSLOT + NB * 128;
         const uint32_t taddr = tmem_acc + ((uint32_t)(warp * 32) << 16);
@@ -307,10 +309,11 @@ k_linear_e8(E8Params p) {
     auto arrive = [&](const E8Desc& x) {
         const int64_t r = (int64_t)x.rbl() * 128 + t;
         const int64_t mw = p.m[x.w()];
+        const int64_t b0 = (int64_t)x.bt() * NB;
         float* part = p.partials[x.w()];
         unsigned int last = 0;
         if (lane == 0) {
-            unsigned int* cnt = p.counters + (((size_t)(p.rb_base[x.w()] + x.rbl()) * gridDim.y + bt) * 4 + warp);
+            unsigned int* cnt = p.counters + (((size_t)(p.rb_base[x.w()] + x.rbl()) * p.n_bt + x.bt()) * 4 + warp);
             last = atomicAdd(cnt, 1u) == (unsigned int)(p.n_split - 1);
             if (last) *cnt = 0u;
         }

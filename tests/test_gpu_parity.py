@@ -110,7 +110,7 @@ def test_explicit_k_and_degenerate_tiles(ctx):
 
 
 @pytest.mark.parametrize("lattice,n_tile", [(hqo.E8, 128), (hqo.E8, 256), (hqo.D4, 128), (hqo.A2, 64), (hqo.Z, 128)])
-@pytest.mark.parametrize("B", [1, 16, 40])
+@pytest.mark.parametrize("B", [1, 16, 40, 130])
 def test_linear_acc_exact_and_outputs(ctx, lattice, n_tile, B):
     m, n_in, snr, seed = 300, 1024, SNR_4BPS[lattice], 21
     W = hq_synth.gaussian_weight(m, n_in, seed=lattice + 100, outliers=True)
@@ -156,7 +156,7 @@ def test_linear_group_is_bit_identical_to_separate_calls(ctx):
     shapes = [384, 130, 256]
     Ws = [hq_synth.gaussian_weight(m, n_in, seed=70 + i, outliers=True) for i, m in enumerate(shapes)]
     ws = [ctx.encode_weights(_dev(W, torch.bfloat16), hqo.E8, 128, snr, seed, (2, 2)) for W in Ws]
-    for B in (1, 16, 33):
+    for B in (1, 16, 33, 130):
         x = _dev(hq_synth.activations(B, n_in, seed=B), torch.bfloat16)
         ys, y32s = ctx.linear_group(ws, x, want_f32=True)
         for w, y, y32 in zip(ws, ys, y32s):
