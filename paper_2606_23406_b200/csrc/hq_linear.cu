@@ -251,11 +251,11 @@ static E8Plan e8_plan(const hq_ctx* ctx, int64_t n_rb_total, int64_t n_kt64, int
     // K split.  Every item end costs a release fence + an arrival atomic per warp and one fp32 partial per row, so
     // items should be long, but the Llama-shaped matrices have too few row blocks to fill 148 x NWG warp groups
     // without splitting K finely.  Measured at batch 1: items of two tiles beat one and four.
-    // Never more partial-sum traffic than a quarter of the compressed weight bytes (matters for batch > 1).
+    // Never more partial-sum traffic than half of the compressed weight bytes (matters for batch > 1; measured at batch 16).
     int split = n_kt;
     for (int d = 1; d <= n_kt; ++d)
         if (n_kt % d == 0 && n_kt / d <= 2) { split = d; break; }
-    const double budget = 0.25 * 0.53 * (double)n_in / (8.0 * (double)B);
+    const double budget = 0.50 * 0.53 * (double)n_in / (8.0 * (double)B);
     while (split > 1 && (double)split > budget) {   // next smaller divisor
         int d = split - 1;
         while (d > 1 && n_kt % d != 0) --d;
