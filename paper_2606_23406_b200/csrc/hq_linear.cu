@@ -9,6 +9,7 @@
 #include "hq_common.cuh"
 #include "hq_internal.h"
 #include "hq_linear_e8.cuh"
+#include "hq_linear_large.cuh"
 #include "hq_tc.cuh"
 
 namespace hq {
@@ -238,6 +239,7 @@ static hq_status launch_generic_nb(hq_ctx* ctx, const hq_weight* w, LinearParams
 // ---- E8 fast path -----------------------------------------------------------------------------
 bool linear_uses_e8_fast(const hq_weight* w) { return w->lattice == LAT_E8 && w->n == 128 && w->k0 <= 3; }
 
+constexpr int64_t LG_MIN_B = 512;   // activation rows from which the decode-once large-M path is used
 struct E8Plan { int NB, BC, NWG, CPS, n_bt, n_split, L, n_items, grid; };
 // plan for a group of weights that share n_in (their row blocks are stacked into one item space)
 static E8Plan e8_plan(const hq_ctx* ctx, int64_t n_rb_total, int64_t n_kt64, int64_t n_in, int64_t B) {
@@ -305,7 +307,13 @@ size_t linear_group_workspace_bytes(const hq_ctx* ctx, const hq_weight* const* w
     for (int i = 0; i < n_w; ++i) n_rb += ws[i]->n_rb;
     E8Plan pl = e8_plan(ctx, n_rb, ws[0]->n_kt, ws[0]->n_in, B);
     size_t bytes = align256((size_t)pl.n_bt * ws[0]->n_kt * e8_bblob_bytes(pl.NB));
-    for (int i = 0; i < n_w; ++i) bytes += align256((size_t)pl.n_split * B * ws[i]->m * 4);
+    if (pl.n_split > 1)
+        for (int i = 0; i < n_w; ++i) bytes += align256((size_t)pl.n_split * B * ws[i]->m * 4);
+    if (B >= LG_MIN_B) {   // the large-M path: activation blob of 256-row tiles + the decoded copy of the largest weight
+        int64_t rb_max = 0;
+        for (int i = 0; i < n_w; ++i) rb_max = ws[i]->n_rb > rb_max ? ws[i]->n_rb : rb_max;
+        bytes += align256((size_t)((B + LG_NB - 1) / LG_NB) * ws[0]->n_kt * LG_BBLOB) + align256((size_t)rb_max * ws[0]->n_kt * LG_ABLOB);
+    }
     return bytes + 256;
 }
 
@@ -315,6 +323,59 @@ size_t linear_workspace_bytes(const hq_ctx* ctx, const hq_weight* w, int64_t B) 
     return align256((size_t)(B * w->n_in)) + align256((size_t)(B * w->n_kt) * 4) + (size_t)ns * B * w->m * 4 + 256;
 }
 
+// Large-M path (hq_linear_large.cuh): activation blob of 256-row tiles, then per weight one decode into the operand-layout
+// scratch copy and one warp-specialised GEMM.  The scratch copy is reused by the weights of a group (stream order).
+static hq_status launch_large(hq_ctx* ctx, const hq_weight* const* ws, int n_w, const void* x, int dtype, int64_t B,
+                              int64_t ldx, void* const* ys_bf16, const int64_t* ldys, float* const* ys_f32, uint8_t* wsbuf,
+                              cudaStream_t st) {
+    const hq_weight* w0 = ws[0];
+    const int64_t n_bt = (B + LG_NB - 1) / LG_NB;
+    uint8_t* bblob = wsbuf;
+    uint8_t* ablob = wsbuf + align256((size_t)n_bt * w0->n_kt * LG_BBLOB);
+    launch_act_blob(x, dtype, B, w0->n_in, ldx, w0->dsign, LG_NB, bblob, st);
+    HQ_CUDA_CHECK(ctx, cudaGetLastError());
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (ctx->prof) {
+        HQ_CUDA_CHECK(ctx, cudaEventCreate(&e0));
+        HQ_CUDA_CHECK(ctx, cudaEventCreate(&e1));
+        HQ_CUDA_CHECK(ctx, cudaEventRecord(e0, st));
+    }
+    for (int i = 0; i < n_w; ++i) {
+        const hq_weight* w = ws[i];
+        E8AblobParams d;
+        d.blob = w->blob; d.sub_off = w->group_off; d.lut = ctx->e8_lut; d.ablob = ablob; d.m = w->m;
+        d.n_kt = (int)w->n_kt;
+        d.inv_A = (float)(1.0 / (w->alpha * sqrt((double)w->n)));
+        int ky = 1;   // enough CTAs for ~8 per SM, each amortising its table load over several tiles
+        while (ky < d.n_kt && (int64_t)w->n_rb * ky < (int64_t)ctx->sm_count * 8) ky *= 2;
+        d.kt_per_cta = (d.n_kt + ky - 1) / ky;
+        dim3 dgrid((unsigned)w->n_rb, (unsigned)((d.n_kt + d.kt_per_cta - 1) / d.kt_per_cta));
+        const size_t dsmem = E8_LUT_BYTES + 128 * E8_SCR_STRIDE * 4;
+#define HQ_LD(KK)                                                                                                          \
+    case KK:                                                                                                               \
+        HQ_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_e8_decode_ablob<KK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dsmem)); \
+        k_e8_decode_ablob<KK><<<dgrid, 128, dsmem, st>>>(d);                                                               \
+        break
+        switch (w->k0) { HQ_LD(0); HQ_LD(1); HQ_LD(2); HQ_LD(3); }
+#undef HQ_LD
+        HQ_CUDA_CHECK(ctx, cudaGetLastError());
+        E8LargeParams g;
+        g.ablob = ablob; g.bblob = bblob; g.y_bf16 = (__nv_bfloat16*)ys_bf16[i]; g.y_f32 = ys_f32 ? ys_f32[i] : nullptr;
+        g.ldy = ldys[i]; g.m = w->m; g.B = B; g.n_rb = (int)w->n_rb; g.n_bt = (int)n_bt; g.n_kt = (int)w->n_kt;
+        const int64_t tiles = (int64_t)g.n_rb * g.n_bt;
+        const unsigned grid = (unsigned)(tiles < ctx->sm_count ? tiles : ctx->sm_count);
+        HQ_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_e8_gemm_large, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LG_SMEM));
+        k_e8_gemm_large<<<grid, 384, LG_SMEM, st>>>(g);
+        HQ_CUDA_CHECK(ctx, cudaGetLastError());
+    }
+    if (ctx->prof) {
+        HQ_CUDA_CHECK(ctx, cudaEventRecord(e1, st));
+        ctx->prof_ev.push_back(e0);
+        ctx->prof_ev.push_back(e1);
+    }
+    return HQ_OK;
+}
+
 // one activation cast, ONE fused decode + MMA launch over the stacked row blocks of all weights, one finalize each
 hq_status launch_linear_group(hq_ctx* ctx, const hq_weight* const* ws, int n_w, const void* x, int dtype, int64_t B,
                               int64_t ldx, void* const* ys_bf16, const int64_t* ldys, float* const* ys_f32,
@@ -322,6 +383,7 @@ hq_status launch_linear_group(hq_ctx* ctx, const hq_weight* const* ws, int n_w, 
     const hq_weight* w0 = ws[0];
     int64_t n_rb = 0;
     for (int i = 0; i < n_w; ++i) n_rb += ws[i]->n_rb;
+    if (B >= LG_MIN_B && !acc_i32) return launch_large(ctx, ws, n_w, x, dtype, B, ldx, ys_bf16, ldys, ys_f32, wsbuf, st);
     E8Plan pl = e8_plan(ctx, n_rb, w0->n_kt, w0->n_in, B);
     uint8_t* bblob = wsbuf;
     uint8_t* at = wsbuf + align256((size_t)pl.n_bt * w0->n_kt * e8_bblob_bytes(pl.NB));
@@ -334,7 +396,7 @@ hq_status launch_linear_group(hq_ctx* ctx, const hq_weight* const* ws, int n_w, 
     for (int i = 0; i < n_w; ++i) {
         p.blob[i] = ws[i]->blob; p.sub_off[i] = ws[i]->group_off; p.m[i] = ws[i]->m;
         p.partials[i] = (float*)at;
-        at += align256((size_t)pl.n_split * B * ws[i]->m * 4);
+        if (pl.n_split > 1) at += align256((size_t)pl.n_split * B * ws[i]->m * 4);
         p.inv_A[i] = (float)(1.0 / (ws[i]->alpha * sqrt((double)ws[i]->n)));
         p.rb_base[i + 1] = p.rb_base[i] + (int)ws[i]->n_rb;
         if (ws[i]->min_ulen < min_ulen) min_ulen = ws[i]->min_ulen;

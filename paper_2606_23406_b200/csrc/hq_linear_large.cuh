@@ -1,0 +1,243 @@
+// hq_linear_large.cuh — the large-M path of hq_linear for E8 tiles of 128 (north_star (e); BASELINE config 5).
+//
+// At thousands of activation rows the Rice decode must not be repeated per batch tile: the weights are decoded ONCE per
+// call into a scratch copy that already has the tensor-core operand layout, and a warp-specialised GEMM streams it.
+//   k_e8_decode_ablob : sub-group (FORMAT §5) -> 128 x 128 INT8 tile, K-major SWIZZLE_128B, K permuted by e8_kcol, followed
+//                       by the 128 row scales rho / (alpha sqrt n) (§4.8).  Same two-phase SWAR decoder as the fused
+//                       kernel (hq_e8_decode.cuh), same fallback.
+//   k_e8_gemm_large   : persistent CTA per SM, tile = 128 weight rows x 256 activation rows.  Warp 0 = TMA producer
+//                       (1-D bulk copies of the A and B blobs into a 4-stage ring), warp 1 = MMA issuer
+//                       (4 x tcgen05.mma kind::i8 M=128 N=256 K=32 per K-tile into one of two TMEM accumulators),
+//                       warps 4..11 = epilogue: per K-tile the INT32 accumulator is drained (tcgen05.ld), scaled by
+//                       rho_tile * s_x,tile (both scales are per tile of 128, so the INT32 sum cannot run across tiles:
+//                       §4.8) and added to fp32 registers; y is written once per output tile.
+// The epilogue (I2F + FMUL + FFMA per accumulator) is the co-bound of this path: DESIGN.md §6.3.
+#pragma once
+#include "hq_common.cuh"
+#include "hq_e8_decode.cuh"
+#include "hq_linear_e8.cuh"
+#include "hq_tc.cuh"
+
+namespace hq {
+
+constexpr int LG_NB = 256;                                   // activation rows per tile = MMA N
+constexpr uint32_t LG_ABLOB = 16384u + 512u;                 // INT8 tile + 128 fp32 row scales
+constexpr uint32_t LG_BBLOB = LG_NB * 128u + LG_NB * 4u;     // = e8_bblob_bytes(256)
+constexpr uint32_t LG_STAGE = (LG_ABLOB + LG_BBLOB + 1023u) & ~1023u;
+constexpr int LG_NST = 4;
+constexpr size_t LG_SMEM = 1024 + (size_t)LG_NST * LG_STAGE + 8 * (2 * LG_NST + 4) + 16;
+
+struct E8AblobParams {
+    const uint8_t* blob;
+    const uint32_t* sub_off;
+    const uint32_t* lut;
+    uint8_t* ablob;       // [n_rb][n_kt][LG_ABLOB]
+    int64_t m;
+    int n_kt, kt_per_cta;
+    float inv_A;
+};
+
+template <int K>
+__global__ void __launch_bounds__(128) k_e8_decode_ablob(E8AblobParams p) {
+    extern __shared__ __align__(16) uint8_t smem_raw[];
+    constexpr int KW = 4 * K;
+    const int t = threadIdx.x, warp = t >> 5, lane = t & 31;
+    uint32_t* lut_s = (uint32_t*)smem_raw;
+    for (int i = t; i < E8_LUT_WORDS; i += 128) lut_s[i] = __ldg(p.lut + i);
+    __syncthreads();
+    const uint32_t smem_a = smem_u32(smem_raw);
+    const uint32_t lut_lane = smem_a + (uint32_t)(lane & (E8_LUT_COPIES - 1)) * 4;
+    const uint32_t scr_a = smem_a + E8_LUT_BYTES + (uint32_t)t * E8_SCR_STRIDE * 4;
+    const uint32_t lane_lt = (1u << lane) - 1u;
+    const int rb = blockIdx.x;
+    const int kt0 = blockIdx.y * p.kt_per_cta;
+    const int64_t r = (int64_t)rb * 128 + t;
+    for (int kt = kt0; kt < kt0 + p.kt_per_cta && kt < p.n_kt; ++kt) {
+        const size_t g = (size_t)rb * p.n_kt + kt;
+        const uint8_t* sgp = p.blob + 16 * (size_t)__ldg(p.sub_off + g * 4 + warp);
+        const uint32_t ul = __ldg((const uint16_t*)sgp + lane), nrm = __ldg((const uint16_t*)sgp + 32 + lane);
+        const uint32_t* rarea = (const uint32_t*)(sgp + 128);
+        const uint32_t* uarea = rarea + KW * 32;
+        uint32_t Rw[KW > 0 ? KW : 1], Uw[E8_NW];
+#pragma unroll
+        for (int j = 0; j < KW; ++j) Rw[j] = __ldg(rarea + j * 32 + lane);
+        const uint32_t nw = (ul + 31) >> 5;
+        {
+            uint32_t base = 0;
+#pragma unroll
+            for (int w = 0; w < E8_NW; ++w) {
+                const bool has = nw > (uint32_t)w;
+                const uint32_t mk = __ballot_sync(0xffffffffu, has);
+                Uw[w] = has ? __ldg(uarea + base + __popc(mk & lane_lt)) : 0u;
+                base += __popc(mk);
+            }
+        }
+        {
+            uint32_t T = 0, acc = 0, wo = scr_a;
+#pragma unroll
+            for (int w = 0; w < E8_NW; ++w) e8_unary_word(Uw[w], lut_lane, T, acc, wo);
+        }
+        uint8_t* tile = p.ablob + g * LG_ABLOB;
+        uint8_t* rowp = tile + (t >> 3) * 1024 + (t & 7) * 128;
+        const bool present = r < p.m && ul > 0;
+        uint32_t total = 0, prevWo = 15u << 24;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            uint32_t W[4], C[8];
+#pragma unroll
+            for (int w = 0; w < 4; ++w) W[w] = lds32(scr_a + (c * 4 + w) * 4);
+            e8_run<K>(W, Rw + c * K, prevWo, total, C);
+            if (!present) {
+#pragma unroll
+                for (int i = 0; i < 8; ++i) C[i] = 0u;
+            }
+            *(uint4*)(rowp + (((2 * c) ^ (t & 7)) << 4)) = make_uint4(C[0], C[1], C[2], C[3]);
+            *(uint4*)(rowp + (((2 * c + 1) ^ (t & 7)) << 4)) = make_uint4(C[4], C[5], C[6], C[7]);
+        }
+        if (present && (nw > (uint32_t)E8_NW || total + 128u != ul)) {   // a quotient >= 16 or a long row: generic decoder
+            SubGroup sg = sub_group(sgp, KW);
+            WordsRowU uw{nullptr, sg.uarea, sg.ulen, nw, 0u, lane};
+            WordsRowR rw{sg.rarea, lane, KW};
+            decode_row_generic<LAT_E8>(rw, 0u, uw, 0u, 128, K, K, [&](int bk, const int* c) {
+#pragma unroll
+                for (int e = 0; e < 8; ++e) {
+                    const int col = e8_kcol(8 * bk + e);
+                    rowp[(((col >> 4) ^ (t & 7)) << 4) | (col & 15)] = (uint8_t)(int8_t)c[e];
+                }
+            });
+        }
+        ((float*)(tile + 16384))[t] = present ? f16_bits_to_f32((uint16_t)nrm) * p.inv_A : 0.0f;
+    }
+}
+
+struct E8LargeParams {
+    const uint8_t* ablob;   // [n_rb][n_kt][LG_ABLOB]
+    const uint8_t* bblob;   // [n_bt][n_kt][LG_BBLOB]
+    __nv_bfloat16* y_bf16;  // [B][ldy] or null
+    float* y_f32;           // [B][m] or null
+    int64_t ldy, m, B;
+    int n_rb, n_bt, n_kt;
+};
+
+__global__ void __launch_bounds__(384, 1) k_e8_gemm_large(E8LargeParams p) {
+    extern __shared__ __align__(1024) uint8_t smem_raw[];
+    uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+    const uint32_t smem_a = smem_u32(smem);
+    uint64_t* full = (uint64_t*)(smem + (size_t)LG_NST * LG_STAGE);
+    uint64_t* empty = full + LG_NST;
+    uint64_t* acc_full = empty + LG_NST;
+    uint64_t* acc_empty = acc_full + 2;
+    uint32_t* tmem_slot = (uint32_t*)(acc_empty + 2);
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+
+    if (warp == 0) tmem_alloc(tmem_slot, 512);
+    if (tid == 32) {
+        for (int s = 0; s < LG_NST; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1 + 8); }
+        for (int a = 0; a < 2; ++a) { mbar_init(&acc_full[a], 1); mbar_init(&acc_empty[a], 8); }
+        mbar_fence_init();
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = *tmem_slot;
+    const int n_tiles = p.n_rb * p.n_bt;
+
+    if (warp < 4) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
+        if (tid == 0) {   // ---- TMA producer
+            uint32_t it = 0;
+            for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+                const int bt = tile / p.n_rb, rb = tile - bt * p.n_rb;
+                const uint8_t* ag = p.ablob + (size_t)rb * p.n_kt * LG_ABLOB;
+                const uint8_t* bg = p.bblob + (size_t)bt * p.n_kt * LG_BBLOB;
+                for (int kt = 0; kt < p.n_kt; ++kt, ++it) {
+                    const uint32_t s = it % LG_NST, ph = (it / LG_NST) & 1u;
+                    mbar_wait(&empty[s], ph ^ 1u);
+                    mbar_arrive_expect_tx(&full[s], LG_ABLOB + LG_BBLOB);
+                    uint8_t* st = smem + (size_t)s * LG_STAGE;
+                    bulk_g2s(st, bg + (size_t)kt * LG_BBLOB, LG_BBLOB, &full[s]);
+                    bulk_g2s(st + LG_BBLOB, ag + (size_t)kt * LG_ABLOB, LG_ABLOB, &full[s]);
+                }
+            }
+        } else if (tid == 32) {   // ---- MMA issuer
+            const uint32_t idesc = make_idesc_i8(128, LG_NB);
+            uint32_t it = 0;
+            for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+                for (int kt = 0; kt < p.n_kt; ++kt, ++it) {
+                    const uint32_t s = it % LG_NST, ph = (it / LG_NST) & 1u, a = it & 1u;
+                    mbar_wait(&acc_empty[a], ((it >> 1) & 1u) ^ 1u);
+                    mbar_wait(&full[s], ph);
+                    tc_fence_after();
+                    const uint32_t sb = smem_a + s * LG_STAGE, sa = sb + LG_BBLOB;
+#pragma unroll
+                    for (int ks = 0; ks < 4; ++ks)
+                        mma_i8(tmem + a * LG_NB, make_desc_sw128(sa + ks * 32), make_desc_sw128(sb + ks * 32), idesc, ks > 0);
+                    mma_commit(&empty[s]);
+                    mma_commit(&acc_full[a]);
+                }
+            }
+        }
+    } else {
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 232;");
+        // ---- epilogue: TMEM lane quarter q = warp % 4, column half = (warp - 4) / 4
+        const int q = warp & 3, half = (warp - 4) >> 2;
+        const int row = q * 32 + lane;
+        float yacc[128];
+#pragma unroll
+        for (int i = 0; i < 128; ++i) yacc[i] = 0.0f;
+        uint32_t it = 0;
+        for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+            const int bt = tile / p.n_rb, rb = tile - bt * p.n_rb;
+            for (int kt = 0; kt < p.n_kt; ++kt, ++it) {
+                const uint32_t s = it % LG_NST, ph = (it / LG_NST) & 1u, a = it & 1u;
+                mbar_wait(&full[s], ph);            // the TMA-written scales are visible to this thread
+                mbar_wait(&acc_full[a], (it >> 1) & 1u);
+                tc_fence_after();
+                const uint32_t sb = smem_a + s * LG_STAGE;
+                const float sw = lds_f32(sb + LG_BBLOB + 16384 + row * 4);
+                const uint32_t sx_a = sb + LG_NB * 128 + half * 512;
+                const uint32_t taddr = tmem + a * LG_NB + half * 128 + ((uint32_t)(q * 32) << 16);
+#pragma unroll
+                for (int c0 = 0; c0 < 128; c0 += 32) {
+                    uint32_t v[32];
+                    tmem_ld16(taddr + c0, v);
+                    tmem_ld16(taddr + c0 + 16, v + 16);
+                    tmem_ld_wait();
+                    if (c0 == 96) {   // the accumulator is in registers: hand the TMEM buffer back to the MMA warp
+                        tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(&acc_empty[a]);
+                    }
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) {
+                        const uint4 s4 = lds128(sx_a + (c0 + 4 * e) * 4);
+                        yacc[c0 + 4 * e + 0] = fmaf((float)(int)v[4 * e + 0] * sw, __uint_as_float(s4.x), yacc[c0 + 4 * e + 0]);
+                        yacc[c0 + 4 * e + 1] = fmaf((float)(int)v[4 * e + 1] * sw, __uint_as_float(s4.y), yacc[c0 + 4 * e + 1]);
+                        yacc[c0 + 4 * e + 2] = fmaf((float)(int)v[4 * e + 2] * sw, __uint_as_float(s4.z), yacc[c0 + 4 * e + 2]);
+                        yacc[c0 + 4 * e + 3] = fmaf((float)(int)v[4 * e + 3] * sw, __uint_as_float(s4.w), yacc[c0 + 4 * e + 3]);
+                    }
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&empty[s]);   // the scales of this stage have been read
+            }
+            const int64_t r = (int64_t)rb * 128 + row;
+            const int64_t b0 = (int64_t)bt * LG_NB + half * 128;
+            if (r < p.m) {
+#pragma unroll
+                for (int c = 0; c < 128; ++c) {
+                    if (b0 + c < p.B) {
+                        if (p.y_bf16) p.y_bf16[(b0 + c) * p.ldy + r] = __float2bfloat16_rn(yacc[c]);
+                        if (p.y_f32) p.y_f32[(b0 + c) * p.m + r] = yacc[c];
+                    }
+                }
+            }
+#pragma unroll
+            for (int c = 0; c < 128; ++c) yacc[c] = 0.0f;
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 0) tmem_dealloc(tmem, 512);
+}
+
+}  // namespace hq

@@ -149,6 +149,35 @@ def test_e8_fast_kernel_falls_back_on_long_quotients_and_ragged_blocks(ctx):
         w.free()
 
 
+@pytest.mark.parametrize("B,m,k", [(600, 300, (-1, -1)), (512, 200, (0, 0)), (1030, 130, (3, 3))])
+def test_linear_large_m_path(ctx, B, m, k):
+    """From 512 activation rows hq_linear decodes the weights once into an operand-layout scratch copy and runs the
+    warp-specialised GEMM (hq_linear_large.cuh): ragged row block, ragged batch tile, several tiles per CTA, rows that
+    take the decoder's generic fallback (k = 0 at 5 bps; a clamp row), an absent row; and the weights of a group."""
+    n_in, seed = 1024, 17
+    snr = f32(28.73) if k == (0, 0) else SNR_4BPS[hqo.E8]
+    W = hq_synth.gaussian_weight(m, n_in, seed=m, outliers=True)
+    W[3] = 0.0
+    d = hqo.signs(seed, 1, n_in)[256:384].astype(np.float32)
+    had = np.array([(-1.0) ** bin(i & 5).count("1") for i in range(128)], np.float32)
+    W[7, :] = 0.0; W[7, 256:384] = d * had * 0.5
+    x = hq_synth.activations(B, n_in, seed=B)
+    enc = hqo.encode_weights(W, hqo.E8, 128, snr, seed, k)
+    w = ctx.encode_weights(_dev(W), hqo.E8, 128, snr, seed, k)
+    q_o, sx_o = hqo.act_quant(x, hqo.E8, 128, seed)
+    _, y_o = hqo.linear(enc["codes"], enc["norms"], hqo.E8, 128, snr, q_o, sx_o)
+    xd = _dev(x, torch.bfloat16)
+    y, y32, _ = w.linear(xd, want_f32=True)
+    assert _rel_err(y32.cpu().numpy(), y_o) < 1e-3
+    _assert_bf16_close(y, y_o)
+    # the fused kernel (the one that also returns the accumulators) gives the same outputs to fp32 rounding order
+    y_f, y32_f, _ = w.linear(xd, want_f32=True, want_acc=True)
+    assert _rel_err(y32.cpu().numpy(), y32_f.cpu().numpy().astype(np.float64)) < 1e-3
+    ys, y32s = ctx.linear_group([w, w], xd, want_f32=True)
+    assert torch.equal(y32s[0], y32) and torch.equal(y32s[1], y32) and torch.equal(ys[1], y)
+    w.free()
+
+
 def test_linear_group_is_bit_identical_to_separate_calls(ctx):
     """hq_linear_group (q/k/v-style: several weights, one x, one fused launch) against hq_linear per weight and
     against the oracle for the first weight."""
