@@ -110,6 +110,26 @@ __global__ void __launch_bounds__(128) k_e8_decode_ablob(E8AblobParams p) {
     }
 }
 
+// packed fp32 pairs (sm_100 f32x2 arithmetic): one instruction for two accumulators
+__device__ __forceinline__ uint64_t pack_u32x2(uint32_t lo, uint32_t hi) {
+    uint64_t r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "r"(lo), "r"(hi));
+    return r;
+}
+__device__ __forceinline__ uint64_t pack_f32x2(float lo, float hi) { return pack_u32x2(__float_as_uint(lo), __float_as_uint(hi)); }
+__device__ __forceinline__ float f32x2_lo(uint64_t v) { return __uint_as_float((uint32_t)v); }
+__device__ __forceinline__ float f32x2_hi(uint64_t v) { return __uint_as_float((uint32_t)(v >> 32)); }
+__device__ __forceinline__ uint64_t mul_f32x2(uint64_t a, uint64_t b) {
+    uint64_t r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ uint64_t fma_f32x2(uint64_t a, uint64_t b, uint64_t c) {
+    uint64_t r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+
 struct E8LargeParams {
     const uint8_t* ablob;   // [n_rb][n_kt][LG_ABLOB]
     const uint8_t* bblob;   // [n_bt][n_kt][LG_BBLOB]
@@ -182,9 +202,10 @@ __global__ void __launch_bounds__(384, 1) k_e8_gemm_large(E8LargeParams p) {
         // ---- epilogue: TMEM lane quarter q = warp % 4, column half = (warp - 4) / 4
         const int q = warp & 3, half = (warp - 4) >> 2;
         const int row = q * 32 + lane;
-        float yacc[128];
+        // fp32 accumulators as packed pairs: the rescale is two packed instructions (mul.f32x2, fma.f32x2) per pair
+        uint64_t yacc[64];
 #pragma unroll
-        for (int i = 0; i < 128; ++i) yacc[i] = 0.0f;
+        for (int i = 0; i < 64; ++i) yacc[i] = 0ull;
         uint32_t it = 0;
         for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
             const int bt = tile / p.n_rb, rb = tile - bt * p.n_rb;
@@ -195,26 +216,32 @@ __global__ void __launch_bounds__(384, 1) k_e8_gemm_large(E8LargeParams p) {
                 tc_fence_after();
                 const uint32_t sb = smem_a + s * LG_STAGE;
                 const float sw = lds_f32(sb + LG_BBLOB + 16384 + row * 4);
+                const uint64_t sw2 = pack_f32x2(sw, sw);
                 const uint32_t sx_a = sb + LG_NB * 128 + half * 512;
                 const uint32_t taddr = tmem + a * LG_NB + half * 128 + ((uint32_t)(q * 32) << 16);
+                uint32_t v[2][32];
+                tmem_ld16(taddr, v[0]);
+                tmem_ld16(taddr + 16, v[0] + 16);
 #pragma unroll
-                for (int c0 = 0; c0 < 128; c0 += 32) {
-                    uint32_t v[32];
-                    tmem_ld16(taddr + c0, v);
-                    tmem_ld16(taddr + c0 + 16, v + 16);
+                for (int ch = 0; ch < 4; ++ch) {
+                    const int c0 = ch * 32;
                     tmem_ld_wait();
-                    if (c0 == 96) {   // the accumulator is in registers: hand the TMEM buffer back to the MMA warp
+                    if (ch < 3) {   // the next chunk's accumulators fly while this one is rescaled
+                        tmem_ld16(taddr + c0 + 32, v[(ch + 1) & 1]);
+                        tmem_ld16(taddr + c0 + 48, v[(ch + 1) & 1] + 16);
+                    } else {        // the accumulator is in registers: hand the TMEM buffer back to the MMA warp
                         tc_fence_before();
                         __syncwarp();
                         if (lane == 0) mbar_arrive(&acc_empty[a]);
                     }
+                    const uint32_t* vc = v[ch & 1];
 #pragma unroll
                     for (int e = 0; e < 8; ++e) {
                         const uint4 s4 = lds128(sx_a + (c0 + 4 * e) * 4);
-                        yacc[c0 + 4 * e + 0] = fmaf((float)(int)v[4 * e + 0] * sw, __uint_as_float(s4.x), yacc[c0 + 4 * e + 0]);
-                        yacc[c0 + 4 * e + 1] = fmaf((float)(int)v[4 * e + 1] * sw, __uint_as_float(s4.y), yacc[c0 + 4 * e + 1]);
-                        yacc[c0 + 4 * e + 2] = fmaf((float)(int)v[4 * e + 2] * sw, __uint_as_float(s4.z), yacc[c0 + 4 * e + 2]);
-                        yacc[c0 + 4 * e + 3] = fmaf((float)(int)v[4 * e + 3] * sw, __uint_as_float(s4.w), yacc[c0 + 4 * e + 3]);
+                        const uint64_t f01 = pack_f32x2((float)(int)vc[4 * e + 0], (float)(int)vc[4 * e + 1]);
+                        const uint64_t f23 = pack_f32x2((float)(int)vc[4 * e + 2], (float)(int)vc[4 * e + 3]);
+                        yacc[(c0 >> 1) + 2 * e + 0] = fma_f32x2(mul_f32x2(f01, sw2), pack_u32x2(s4.x, s4.y), yacc[(c0 >> 1) + 2 * e + 0]);
+                        yacc[(c0 >> 1) + 2 * e + 1] = fma_f32x2(mul_f32x2(f23, sw2), pack_u32x2(s4.z, s4.w), yacc[(c0 >> 1) + 2 * e + 1]);
                     }
                 }
                 __syncwarp();
@@ -223,16 +250,31 @@ __global__ void __launch_bounds__(384, 1) k_e8_gemm_large(E8LargeParams p) {
             const int64_t r = (int64_t)rb * 128 + row;
             const int64_t b0 = (int64_t)bt * LG_NB + half * 128;
             if (r < p.m) {
+                const int64_t nc = p.B - b0 < 128 ? p.B - b0 : 128;   // columns of this half inside the batch
+                if (p.y_bf16) {
+                    __nv_bfloat16* yp = p.y_bf16 + b0 * p.ldy + r;
+                    if (nc == 128) {
 #pragma unroll
-                for (int c = 0; c < 128; ++c) {
-                    if (b0 + c < p.B) {
-                        if (p.y_bf16) p.y_bf16[(b0 + c) * p.ldy + r] = __float2bfloat16_rn(yacc[c]);
-                        if (p.y_f32) p.y_f32[(b0 + c) * p.m + r] = yacc[c];
+                        for (int c = 0; c < 64; ++c) {
+                            yp[0] = __float2bfloat16_rn(f32x2_lo(yacc[c]));
+                            yp[p.ldy] = __float2bfloat16_rn(f32x2_hi(yacc[c]));
+                            yp += 2 * p.ldy;
+                        }
+                    } else {
+#pragma unroll
+                        for (int c = 0; c < 128; ++c)
+                            if (c < nc) yp[c * p.ldy] = __float2bfloat16_rn((c & 1) ? f32x2_hi(yacc[c >> 1]) : f32x2_lo(yacc[c >> 1]));
                     }
+                }
+                if (p.y_f32) {
+                    float* yp = p.y_f32 + b0 * p.m + r;
+#pragma unroll
+                    for (int c = 0; c < 128; ++c)
+                        if (c < nc) yp[c * p.m] = (c & 1) ? f32x2_hi(yacc[c >> 1]) : f32x2_lo(yacc[c >> 1]);
                 }
             }
 #pragma unroll
-            for (int c = 0; c < 128; ++c) yacc[c] = 0.0f;
+            for (int c = 0; c < 64; ++c) yacc[c] = 0ull;
         }
     }
     tc_fence_before();
