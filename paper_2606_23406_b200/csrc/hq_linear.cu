@@ -8,6 +8,7 @@
 
 #include "hq_common.cuh"
 #include "hq_internal.h"
+#include <stdlib.h>
 #include "hq_linear_e8.cuh"
 #include "hq_linear_large.cuh"
 #include "hq_tc.cuh"
@@ -239,7 +240,15 @@ static hq_status launch_generic_nb(hq_ctx* ctx, const hq_weight* w, LinearParams
 // ---- E8 fast path -----------------------------------------------------------------------------
 bool linear_uses_e8_fast(const hq_weight* w) { return w->lattice == LAT_E8 && w->n == 128 && w->k0 <= 3; }
 
-constexpr int64_t LG_MIN_B = 512;   // activation rows from which the decode-once large-M path is used
+// activation rows from which the decode-once large-M path is used; HQ_LARGE_MIN_B overrides it (tuning)
+static int64_t lg_min_b() {
+    static const int64_t v = [] {
+        const char* e = getenv("HQ_LARGE_MIN_B");
+        return e && *e ? (int64_t)atoll(e) : (int64_t)64;
+    }();
+    return v;
+}
+#define LG_MIN_B lg_min_b()
 struct E8Plan { int NB, BC, NWG, CPS, n_bt, n_split, L, n_items, grid; };
 // plan for a group of weights that share n_in (their row blocks are stacked into one item space)
 static E8Plan e8_plan(const hq_ctx* ctx, int64_t n_rb_total, int64_t n_kt64, int64_t n_in, int64_t B) {
