@@ -247,44 +247,88 @@ k_act_quant(const void* X, int dtype, int64_t n_tiles, int64_t n_kt, int64_t ldx
 __global__ void __launch_bounds__(QW_WARPS * 32)
 k_act_blob(const void* X, int dtype, int64_t B, int64_t n_kt, int64_t ldx, const int8_t* dsign, int NB,
            uint8_t* bblob) {
+    // The tile lives in registers: lane l holds elements 4l .. 4l+3.  FORMAT R1's butterflies (ascending stride, a+b to
+    // the lower index, a-b to the upper) are two in-register stages and five shuffle stages: the same additions on the
+    // same pairs as warp_rht_inplace, so the result is bit-identical to k_act_quant.
     extern __shared__ float smem[];
-    const int n = 128;
     griddep_launch();
     griddep_wait();   // x comes from the previous kernel; the blob area is read by the previous hq_linear
-    int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    float* u = smem + warp * n;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    uint8_t* srow = (uint8_t*)smem + warp * 128;          // one operand row, K order of the operand (e8_kcol)
     const int64_t n_bt = (B + NB - 1) / NB, n_tiles = n_bt * NB * n_kt;
     const uint32_t blob_bytes = (uint32_t)(NB * 128 + NB * 4);
+    const float cn = (float)(1.0 / sqrt(128.0));
+    const bool vec = dtype == HQ_BF16 ? ((((uintptr_t)X) | (uintptr_t)(ldx * 2)) & 7) == 0
+                                      : ((((uintptr_t)X) | (uintptr_t)(ldx * 4)) & 15) == 0;
+    // the four codes of this lane go to operand columns colb + 4j (block l>>1, coordinates 4(l&1) .. +3)
+    const int blk = lane >> 1;
+    const int colb = 32 * (blk >> 2) + 16 * (lane & 1) + (blk & 3);
     for (int64_t tile = blockIdx.x * (int64_t)QW_WARPS + warp; tile < n_tiles; tile += (int64_t)gridDim.x * QW_WARPS) {
-        int64_t b = tile / n_kt, kt = tile % n_kt;   // b runs over the padded batch n_bt*NB
-        int64_t bt = b / NB;
-        int bb = (int)(b % NB);
+        const int64_t b = tile / n_kt, kt = tile - b * n_kt;   // b runs over the padded batch n_bt*NB
+        const int64_t bt = b / NB;
+        const int bb = (int)(b - bt * NB);
         uint8_t* blob = bblob + (bt * n_kt + kt) * (int64_t)blob_bytes;
-        float* sx = (float*)(blob + NB * 128);
+        float x[4] = {0.0f, 0.0f, 0.0f, 0.0f};
         float amax = 0.0f;
         if (b < B) {
-            for (int i = lane; i < n; i += 32) {
-                float x = load_elem(X, dtype, b * ldx + kt * n + i);
-                u[i] = (dsign[kt * n + i] < 0) ? -x : x;
+            const int64_t base = b * ldx + kt * 128 + 4 * lane;
+            if (vec && dtype == HQ_BF16) {
+                const uint2 v = __ldg((const uint2*)((const __nv_bfloat16*)X + base));
+                x[0] = __uint_as_float(v.x << 16); x[1] = __uint_as_float(v.x & 0xffff0000u);
+                x[2] = __uint_as_float(v.y << 16); x[3] = __uint_as_float(v.y & 0xffff0000u);
+            } else if (vec) {
+                const float4 v = __ldg((const float4*)((const float*)X + base));
+                x[0] = v.x; x[1] = v.y; x[2] = v.z; x[3] = v.w;
+            } else {
+#pragma unroll
+                for (int j = 0; j < 4; ++j) x[j] = load_elem(X, dtype, base + j);
             }
-            warp_rht_inplace(u, n, lane);
-            for (int i = lane; i < n; i += 32) amax = fmaxf(amax, fabsf(u[i]));
-            for (int s = 16; s; s >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, s));
+            const uint32_t sg = __ldg((const uint32_t*)(dsign + kt * 128) + lane);
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+                if ((sg >> (8 * j)) & 0x80u) x[j] = -x[j];
+            {   // strides 1 and 2: inside the lane
+                float a = x[0], c = x[1];
+                x[0] = __fadd_rn(a, c); x[1] = __fsub_rn(a, c);
+                a = x[2]; c = x[3];
+                x[2] = __fadd_rn(a, c); x[3] = __fsub_rn(a, c);
+                a = x[0]; c = x[2];
+                x[0] = __fadd_rn(a, c); x[2] = __fsub_rn(a, c);
+                a = x[1]; c = x[3];
+                x[1] = __fadd_rn(a, c); x[3] = __fsub_rn(a, c);
+            }
+#pragma unroll
+            for (int m = 1; m < 32; m <<= 1) {   // strides 4 .. 64: lane ^ m holds the partner
+                const bool upper = (lane & m) != 0;
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const float o = __shfl_xor_sync(0xffffffffu, x[j], m);
+                    x[j] = upper ? __fsub_rn(o, x[j]) : __fadd_rn(x[j], o);
+                }
+            }
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                x[j] = __fmul_rn(x[j], cn);
+                amax = fmaxf(amax, fabsf(x[j]));
+            }
+            for (int sft = 16; sft; sft >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, sft));
         }
-        __syncwarp();
         const float inv = (amax == 0.0f) ? 0.0f : __fdiv_rn(127.0f, amax);
-        for (int i = lane; i < n; i += 32) {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
             int qv = 0;
             if (amax != 0.0f) {
-                float v = rintf(__fmul_rn(u[i], inv));
+                float v = rintf(__fmul_rn(x[j], inv));
                 v = fminf(fmaxf(v, -127.0f), 127.0f);
                 qv = (int)v;
             }
-            const int blk = i >> 3, ci = i & 7;
-            const int col = 32 * (blk >> 2) + 4 * ci + (blk & 3);
-            blob[(bb >> 3) * 1024 + (bb & 7) * 128 + ((((col >> 4) ^ (bb & 7)) << 4) | (col & 15))] = (uint8_t)(int8_t)qv;
+            srow[colb + 4 * j] = (uint8_t)(int8_t)qv;
         }
-        if (lane == 0) sx[bb] = (amax == 0.0f) ? 0.0f : __fdiv_rn(amax, 127.0f);
+        __syncwarp();
+        // one coalesced 128-byte row: lane l owns operand columns 4l .. 4l+3 = 16-byte chunk l>>2 (swizzled), word l&3
+        const uint32_t w4 = ((const uint32_t*)srow)[lane];
+        *(uint32_t*)(blob + (bb >> 3) * 1024 + (bb & 7) * 128 + ((((lane >> 2) ^ (bb & 7)) << 4) | ((lane & 3) << 2))) = w4;
+        if (lane == 0) ((float*)(blob + NB * 128))[bb] = (amax == 0.0f) ? 0.0f : __fdiv_rn(amax, 127.0f);
         __syncwarp();
     }
 }
