@@ -207,21 +207,29 @@ __global__ void __launch_bounds__(384, 1) k_e8_gemm_large(E8LargeParams p) {
 #pragma unroll
         for (int i = 0; i < 64; ++i) yacc[i] = 0ull;
         uint32_t it = 0;
+        uint32_t v[2][32];
+        const uint32_t tlane = tmem + half * 128 + ((uint32_t)(q * 32) << 16);
+        // first chunk of K-step `i`: wait for its operands (scales) and its accumulator, start the TMEM load
+        auto begin_step = [&](uint32_t i) {
+            mbar_wait(&full[i % LG_NST], (i / LG_NST) & 1u);   // the TMA-written scales are visible to this thread
+            mbar_wait(&acc_full[i & 1u], (i >> 1) & 1u);
+            tc_fence_after();
+            const uint32_t ta = tlane + (i & 1u) * LG_NB;
+            tmem_ld16(ta, v[0]);
+            tmem_ld16(ta + 16, v[0] + 16);
+        };
+        const int my_tiles = blockIdx.x < n_tiles ? (n_tiles - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
+        const uint32_t n_steps = (uint32_t)my_tiles * (uint32_t)p.n_kt;
+        if (n_steps) begin_step(0);
         for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
             const int bt = tile / p.n_rb, rb = tile - bt * p.n_rb;
             for (int kt = 0; kt < p.n_kt; ++kt, ++it) {
-                const uint32_t s = it % LG_NST, ph = (it / LG_NST) & 1u, a = it & 1u;
-                mbar_wait(&full[s], ph);            // the TMA-written scales are visible to this thread
-                mbar_wait(&acc_full[a], (it >> 1) & 1u);
-                tc_fence_after();
+                const uint32_t s = it % LG_NST, a = it & 1u;
                 const uint32_t sb = smem_a + s * LG_STAGE;
                 const float sw = lds_f32(sb + LG_BBLOB + 16384 + row * 4);
                 const uint64_t sw2 = pack_f32x2(sw, sw);
                 const uint32_t sx_a = sb + LG_NB * 128 + half * 512;
-                const uint32_t taddr = tmem + a * LG_NB + half * 128 + ((uint32_t)(q * 32) << 16);
-                uint32_t v[2][32];
-                tmem_ld16(taddr, v[0]);
-                tmem_ld16(taddr + 16, v[0] + 16);
+                const uint32_t taddr = tlane + a * LG_NB;
 #pragma unroll
                 for (int ch = 0; ch < 4; ++ch) {
                     const int c0 = ch * 32;
@@ -229,10 +237,11 @@ __global__ void __launch_bounds__(384, 1) k_e8_gemm_large(E8LargeParams p) {
                     if (ch < 3) {   // the next chunk's accumulators fly while this one is rescaled
                         tmem_ld16(taddr + c0 + 32, v[(ch + 1) & 1]);
                         tmem_ld16(taddr + c0 + 48, v[(ch + 1) & 1] + 16);
-                    } else {        // the accumulator is in registers: hand the TMEM buffer back to the MMA warp
-                        tc_fence_before();
+                    } else {        // the accumulator is in registers: hand the TMEM buffer back to the MMA warp,
+                        tc_fence_before();   // and start on the next K-step's accumulator while this chunk is rescaled
                         __syncwarp();
                         if (lane == 0) mbar_arrive(&acc_empty[a]);
+                        if (it + 1 < n_steps) begin_step(it + 1);
                     }
                     const uint32_t* vc = v[ch & 1];
 #pragma unroll
