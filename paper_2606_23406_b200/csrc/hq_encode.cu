@@ -263,10 +263,12 @@ k_act_blob(const void* X, int dtype, int64_t B, int64_t n_kt, int64_t ldx, const
     // the four codes of this lane go to operand columns colb + 4j (block l>>1, coordinates 4(l&1) .. +3)
     const int blk = lane >> 1;
     const int colb = 32 * (blk >> 2) + 16 * (lane & 1) + (blk & 3);
+    const uint32_t n_kt32 = (uint32_t)n_kt, NB32 = (uint32_t)NB;   // n_tiles < 2^32 (see launch_act_blob)
     for (int64_t tile = blockIdx.x * (int64_t)QW_WARPS + warp; tile < n_tiles; tile += (int64_t)gridDim.x * QW_WARPS) {
-        const int64_t b = tile / n_kt, kt = tile - b * n_kt;   // b runs over the padded batch n_bt*NB
-        const int64_t bt = b / NB;
-        const int bb = (int)(b - bt * NB);
+        const uint32_t b32 = (uint32_t)tile / n_kt32;            // b runs over the padded batch n_bt*NB
+        const int64_t b = b32, kt = (uint32_t)tile - b32 * n_kt32;
+        const int64_t bt = b32 / NB32;
+        const int bb = (int)(b32 - (uint32_t)bt * NB32);
         uint8_t* blob = bblob + (bt * n_kt + kt) * (int64_t)blob_bytes;
         float x[4] = {0.0f, 0.0f, 0.0f, 0.0f};
         float amax = 0.0f;
@@ -299,11 +301,11 @@ k_act_blob(const void* X, int dtype, int64_t B, int64_t n_kt, int64_t ldx, const
             }
 #pragma unroll
             for (int m = 1; m < 32; m <<= 1) {   // strides 4 .. 64: lane ^ m holds the partner
-                const bool upper = (lane & m) != 0;
+                const float sg1 = (lane & m) ? -1.0f : 1.0f;   // upper index of the pair: a - b = o - x, else x + o
 #pragma unroll
                 for (int j = 0; j < 4; ++j) {
                     const float o = __shfl_xor_sync(0xffffffffu, x[j], m);
-                    x[j] = upper ? __fsub_rn(o, x[j]) : __fadd_rn(x[j], o);
+                    x[j] = __fmaf_rn(x[j], sg1, o);            // the product is exact: one rounding, that of the sum
                 }
             }
 #pragma unroll
@@ -338,6 +340,7 @@ void launch_act_blob(const void* x, int dtype, int64_t B, int64_t n_in, int64_t 
     int64_t n_kt = n_in / 128, n_bt = (B + NB - 1) / NB, n_tiles = n_bt * NB * n_kt;
     int64_t blocks = (n_tiles + QW_WARPS - 1) / QW_WARPS;
     if (blocks > 148 * 16) blocks = 148 * 16;
+    // n_tiles < 2^32 always: 2^32 tiles of 128 bf16 activations would be 1.1 TB of x
     launch_pdl(k_act_blob, dim3((unsigned)blocks), dim3(QW_WARPS * 32), QW_WARPS * 128 * sizeof(float), st, x, dtype, B, n_kt, ldx,
                dsign, NB, bblob);
 }
