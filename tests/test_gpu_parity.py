@@ -285,3 +285,39 @@ def test_attend_matches_oracle_long_way(ctx, lattice, snr, k, dither, T, window)
     assert _rel_err(o32.cpu().numpy(), ref) < 1e-3
     _assert_bf16_close(out, ref)
     kv.free()
+
+
+def test_empty_and_out_of_range_arguments_fail_loudly_and_leave_the_context_usable(ctx):
+    """include/hq.h error behaviour: empty batches, ragged K, an empty or overfull cache are HQ_ERR_SHAPE, never a
+    silent no-op; the next valid call on the same context is still bit-exact against the oracle."""
+    import paper_2606_23406_b200 as hq
+    snr = SNR_4BPS[hqo.E8]
+    W = hq_synth.gaussian_weight(64, 256, seed=21)
+    with pytest.raises(hq.HQError):                                # n_in not a multiple of the RHT tile
+        ctx.encode_weights(_dev(W[:, :200].copy()), hqo.E8, 128, snr, 1)
+    w, enc = _check_weight_bitstream(ctx, W, hqo.E8, 128, snr, 1)
+    with pytest.raises(hq.HQError):                                # empty batch
+        w.linear(torch.empty((0, 256), dtype=torch.bfloat16, device="cuda"))
+    with pytest.raises(hq.HQError):
+        ctx.linear_group([w], torch.empty((0, 256), dtype=torch.bfloat16, device="cuda"))
+    kv = ctx.kv_create(1, 128, 4, hqo.E8, f32(9.68), (0, 0), 5)
+    q = _dev(hq_synth.kv_tokens(1, 2, 128, seed=8)[0], torch.bfloat16)
+    with pytest.raises(hq.HQError):                                # attend on an empty cache
+        kv.attend(q)
+    K = _dev(hq_synth.kv_tokens(5, 1, 128, seed=6), torch.bfloat16)
+    with pytest.raises(hq.HQError):                                # 5 tokens into a cache of 4
+        kv.append(K, K)
+    with pytest.raises(hq.HQError):                                # zero tokens
+        kv.append(K[:0], K[:0])
+    kv.append(K[:4], K[:4])
+    assert kv.export()["n_tokens"] == 4
+    with pytest.raises(hq.HQError):                                # full
+        kv.append(K[:1], K[:1])
+    kv.free()
+    # the context still computes: accumulators bit-exact after the failed calls
+    x = hq_synth.activations(3, 256, seed=22)
+    q_o, sx_o = hqo.act_quant(x, hqo.E8, 128, 1)
+    acc_o, _ = hqo.linear(enc["codes"], enc["norms"], hqo.E8, 128, snr, q_o, sx_o)
+    _, _, acc = w.linear(_dev(x, torch.bfloat16), want_acc=True)
+    assert (acc.cpu().numpy() == acc_o).all()
+    w.free()
