@@ -264,10 +264,16 @@ k_act_blob(const void* X, int dtype, int64_t B, int64_t n_kt, int64_t ldx, const
     const int blk = lane >> 1;
     const int colb = 32 * (blk >> 2) + 16 * (lane & 1) + (blk & 3);
     const uint32_t n_kt32 = (uint32_t)n_kt, NB32 = (uint32_t)NB;   // n_tiles < 2^32 (see launch_act_blob)
-    for (int64_t tile = blockIdx.x * (int64_t)QW_WARPS + warp; tile < n_tiles; tile += (int64_t)gridDim.x * QW_WARPS) {
-        const uint32_t b32 = (uint32_t)tile / n_kt32;            // b runs over the padded batch n_bt*NB
-        const int64_t b = b32, kt = (uint32_t)tile - b32 * n_kt32;
-        const int64_t bt = b32 / NB32;
+    // (row, K-tile) of the tile advances by the grid stride without a division per tile
+    const uint32_t stride = gridDim.x * (uint32_t)QW_WARPS;
+    const uint32_t st_b = stride / n_kt32, st_k = stride - st_b * n_kt32;
+    const int nb_sh = (NB32 & (NB32 - 1u)) == 0u ? __ffs((int)NB32) - 1 : -1;
+    uint32_t b32 = (blockIdx.x * (uint32_t)QW_WARPS + warp) / n_kt32;   // b runs over the padded batch n_bt*NB
+    uint32_t kt32 = (blockIdx.x * (uint32_t)QW_WARPS + warp) - b32 * n_kt32;
+    for (int64_t tile = blockIdx.x * (int64_t)QW_WARPS + warp; tile < n_tiles; tile += stride,
+                 kt32 += st_k, b32 += st_b + (kt32 >= n_kt32 ? 1u : 0u), kt32 -= (kt32 >= n_kt32 ? n_kt32 : 0u)) {
+        const int64_t b = b32, kt = kt32;
+        const int64_t bt = nb_sh >= 0 ? (b32 >> nb_sh) : (b32 / NB32);
         const int bb = (int)(b32 - (uint32_t)bt * NB32);
         uint8_t* blob = bblob + (bt * n_kt + kt) * (int64_t)blob_bytes;
         float x[4] = {0.0f, 0.0f, 0.0f, 0.0f};
