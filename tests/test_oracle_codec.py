@@ -314,7 +314,7 @@ def test_subtractive_dither_is_unbiased_per_vector():
     heads, d, snr = 1, 128, 9.68                       # E8 at ~2 bps
     x = hq_synth.kv_tokens(1, heads, d, seed=4)
     qv = np.random.default_rng(3).standard_normal(d)
-    N = 100000 // 8
+    N = 100000                                         # north_star: 1e5 dithers per rotation
     for rotation in (0, 1):
         # the same vector presented as tokens 0..N-1: a fresh dither per token (L190)
         X = np.repeat(x, N, axis=0)
