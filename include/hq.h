@@ -35,12 +35,14 @@ typedef enum {
     HQ_ERR_UNSUPPORTED = 3, /* not an sm_100 device, rotation qjl, ... */
     HQ_ERR_ALLOC = 4,       /* the caller's allocator returned NULL */
     HQ_ERR_CUDA = 5,        /* a CUDA runtime call failed; text in hq_last_error */
-    HQ_ERR_FORMAT = 6       /* a tile's U-section exceeds the container's bound (FORMAT §4, §5) */
+    HQ_ERR_FORMAT = 6       /* a tile's U-section exceeds the container's bound (FORMAT §4, §5); a KV cache whose U stream
+                               ran out of capacity (sticky: every later call on that cache returns it); a blob that fails
+                               hq_weight_import's layout checks */
 } hq_status;
 
 typedef enum { HQ_Z = 1, HQ_A2 = 2, HQ_D4 = 4, HQ_E8 = 8 } hq_lattice;     /* §3.2, §4.5; value = dimension */
 typedef enum { HQ_F32 = 0, HQ_BF16 = 1 } hq_dtype;
-typedef enum { HQ_ROT_NONE = 0, HQ_ROT_SIGNS = 1 } hq_rotation;              /* §4.2 L216 (qjl: not built) */
+typedef enum { HQ_ROT_NONE = 0, HQ_ROT_SIGNS = 1, HQ_ROT_QJL = 2 } hq_rotation; /* §4.2, §3.4; QJL (Haar) -> HQ_ERR_UNSUPPORTED */
 
 /* Device-memory allocator supplied by the caller (the Python binding backs it with torch). */
 typedef struct {
@@ -76,6 +78,16 @@ hq_status hq_profile_read(hq_ctx* ctx, double* total_ms, int64_t* launches);
 /* alpha of eq.(9) L871 for (lattice, snr_db), as the library computes it (host, double). */
 double hq_alpha(int32_t lattice, double snr_db);
 
+/*
+ * Calibration lookup (§5.4, App. B.1, reading G17): the SNR at which `lattice` realizes
+ * `target_bps` payload bits per scalar (Rice code at the best k, no metadata) on iid Gaussian tiles of 128, by linear
+ * interpolation in a cached table b(SNR) (1e5 tiles, seed 42, 0.25 dB grid over 5..35 dB).  The table is data, committed
+ * as csrc/hq_calib_table.inc and written by oracle/make_calib_table.py (which calls only oracle/); the paper's printed
+ * anchors pin it (tests/test_abi.py).  Pure host function: ctx may be NULL.  target_bps outside the table's range ->
+ * HQ_ERR_INVALID_ARG.  rice_k_out (may be NULL) receives the table's best k-set at the grid point below the answer.
+ */
+hq_status hq_snr_for_bps(const hq_ctx* ctx, int32_t lattice, double target_bps, float* snr_db_out, int32_t* rice_k_out);
+
 /* ---- weights: encode (§5.1; SURVEY §8(a) B1,B3,B5-B7) ------------------------------ */
 /*
  * Quantize W [m_out, n_in] (row-major, leading dimension ld elements, dev, F32 or BF16): per
@@ -105,6 +117,43 @@ hq_status hq_weight_get_info(const hq_weight* w, hq_weight_info* out);
 
 /* dev pointers into the handle (valid until hq_weight_free): the FORMAT §5 blob and sub_off[n_groups+1]. */
 hq_status hq_weight_export(const hq_weight* w, const void** blob_dev, const uint32_t** group_off_dev);
+
+/* Rate and range statistics of an encoded weight (SURVEY §5 "metrics": Figs 10-11 report realized bps and overflow).
+ * Host values recorded at encode / import time; no device work. */
+typedef struct {
+    int64_t payload_bits, norm_bits, length_bits;  /* as hq_weight_info */
+    int64_t offset_bits;                           /* 32 per sub-group (sub_off, FORMAT §5) */
+    int64_t padding_bits;                          /* 8 * blob_bytes - payload - norm - length: word / 16-byte alignment */
+    int64_t clamp_count;                           /* INT8 pre-clamp events (G8) */
+    int64_t n_tiles;                               /* m_out * n_in / n_tile */
+    int32_t tile_bits_min, tile_bits_max;          /* Rice code length of the shortest / longest tile (Rbits + ulen) */
+    double bits_per_scalar_payload, bits_per_scalar_total; /* total = payload + norm + length */
+} hq_stats;
+hq_status hq_weight_stats(const hq_weight* w, hq_stats* out);
+
+/*
+ * The encoded weight as a host artefact ("store integer codes and per-tile scales", §5.1; SURVEY §5 checkpoint).
+ * hq_weight_export_host copies the FORMAT §5 container to caller-owned HOST buffers (blob_host: header.blob_bytes
+ * bytes, sub_off_host: header.n_groups + 1 words; pass both NULL to get the header and the sizes only) and
+ * synchronizes `stream`.  hq_weight_import rebuilds a handle from them: it checks the header, that sub_off is
+ * increasing and ends at blob_bytes / 16, and that every sub-group's size equals what its ulen header implies
+ * (HQ_ERR_FORMAT otherwise, nothing is launched on a bad blob), uploads on `stream`, regenerates the RHT signs from
+ * the seed.  An imported handle gives bit-identical hq_linear / hq_decode_int8 results.
+ */
+typedef struct {
+    uint32_t magic, version;      /* 'HQW1', 2 */
+    int64_t m_out, n_in;
+    int32_t lattice, n_tile, rice_k[2];
+    float snr_db;
+    uint64_t seed;
+    int64_t blob_bytes, n_groups;
+    int64_t payload_bits, clamp_count;
+    int32_t ulen_min, ulen_max;   /* shortest / longest U-section over the present rows, bits */
+} hq_weight_header;
+hq_status hq_weight_export_host(hq_ctx* ctx, const hq_weight* w, hq_weight_header* header, void* blob_host,
+                                uint32_t* sub_off_host, void* stream);
+hq_status hq_weight_import(hq_ctx* ctx, const hq_weight_header* header, const void* blob_host,
+                           const uint32_t* sub_off_host, void* stream, hq_weight** out);
 
 /* Parity / debug: the INT8 lattice points c [m_out, n_in] (row-major, dev) and fp16 norms
  * [m_out, n_in/n_tile] (dev, may be NULL) decoded from the container (O2; §4.5-4.7 inverse). */
@@ -153,7 +202,10 @@ typedef struct {
     hq_codec_config codec;      /* n_tile must equal head_dim; rice_k must be given (>= 0) */
     int32_t rotation;           /* hq_rotation: S applied after the RHT (§4.2, G14) */
     int32_t dither;             /* 1: subtractive dither U ~ Unif(V(Lambda)) per token (§4.4, A.6 L843) */
-    int32_t window;             /* exact bf16 residual window, tokens (§6.7.2); 0 = none */
+    int32_t window;             /* exact bf16 residual window, tokens (§6.7.2); 0 <= window <= head_dim */
+    int64_t una_capacity_bits;  /* capacity of each (role, head) U stream; 0 = auto: max_tokens * head_dim *
+                                   max(4, 1.3 * (1 + (0.8 alpha + 0.5) / 2^k)) bits (E|zz| ~ 0.8 alpha on a normalized vector).
+                                   A vector that does not fit is NOT written; the cache turns sticky HQ_ERR_FORMAT. */
 } hq_kv_config;
 
 hq_status hq_kv_create(hq_ctx* ctx, const hq_kv_config* cfg, hq_kv** out);
@@ -166,7 +218,8 @@ hq_status hq_kv_append(hq_ctx* ctx, hq_kv* kv, const void* k_dev, const void* v_
 
 /* One decode step of attention (L178) for q [q_heads, head_dim] bf16 dev over all held tokens:
  * tokens [0, T-window) from the bitstream (decoded in the code domain), [T-window, T) from the ring.
- * out [q_heads, head_dim] bf16 dev; out_f32 optional. q_heads must be a multiple of kv_heads. */
+ * out [q_heads, head_dim] bf16 dev; out_f32 optional. q_heads must be a multiple of kv_heads, q_heads <= 64,
+ * q_heads / kv_heads <= 8 (HQ_ERR_SHAPE otherwise). */
 hq_status hq_attend(hq_ctx* ctx, const hq_kv* kv, const void* q_dev, int32_t q_heads, void* out_bf16_dev,
                     float* out_f32_dev_or_null, void* stream);
 

@@ -32,7 +32,7 @@ class _CodecConfig(C.Structure):
 
 class _KVConfig(C.Structure):
     _fields_ = [("kv_heads", C.c_int32), ("head_dim", C.c_int32), ("max_tokens", C.c_int64), ("codec", _CodecConfig),
-                ("rotation", C.c_int32), ("dither", C.c_int32), ("window", C.c_int32)]
+                ("rotation", C.c_int32), ("dither", C.c_int32), ("window", C.c_int32), ("una_capacity_bits", C.c_int64)]
 
 
 class _WeightInfo(C.Structure):
@@ -40,6 +40,21 @@ class _WeightInfo(C.Structure):
                 ("rice_k", C.c_int32 * 2), ("snr_db", C.c_float), ("alpha", C.c_double), ("seed", C.c_uint64),
                 ("payload_bits", C.c_int64), ("norm_bits", C.c_int64), ("length_bits", C.c_int64),
                 ("blob_bytes", C.c_int64), ("n_groups", C.c_int64), ("clamp_count", C.c_int64)]
+
+
+class _Stats(C.Structure):
+    _fields_ = [("payload_bits", C.c_int64), ("norm_bits", C.c_int64), ("length_bits", C.c_int64),
+                ("offset_bits", C.c_int64), ("padding_bits", C.c_int64), ("clamp_count", C.c_int64),
+                ("n_tiles", C.c_int64), ("tile_bits_min", C.c_int32), ("tile_bits_max", C.c_int32),
+                ("bits_per_scalar_payload", C.c_double), ("bits_per_scalar_total", C.c_double)]
+
+
+class WeightHeader(C.Structure):
+    _fields_ = [("magic", C.c_uint32), ("version", C.c_uint32), ("m_out", C.c_int64), ("n_in", C.c_int64),
+                ("lattice", C.c_int32), ("n_tile", C.c_int32), ("rice_k", C.c_int32 * 2), ("snr_db", C.c_float),
+                ("seed", C.c_uint64), ("blob_bytes", C.c_int64), ("n_groups", C.c_int64),
+                ("payload_bits", C.c_int64), ("clamp_count", C.c_int64), ("ulen_min", C.c_int32),
+                ("ulen_max", C.c_int32)]
 
 
 class _KVView(C.Structure):
@@ -55,8 +70,9 @@ def lib_path() -> str:
 
 _lib = None
 
-EXPORTS = ["hq_create", "hq_destroy", "hq_last_error", "hq_alpha", "hq_profile_enable", "hq_profile_read", "hq_encode_weights", "hq_weight_free",
-           "hq_weight_get_info", "hq_weight_export", "hq_decode_int8", "hq_act_quant", "hq_linear",
+EXPORTS = ["hq_create", "hq_destroy", "hq_last_error", "hq_alpha", "hq_snr_for_bps", "hq_profile_enable", "hq_profile_read",
+           "hq_encode_weights", "hq_weight_free", "hq_weight_get_info", "hq_weight_stats", "hq_weight_export",
+           "hq_weight_export_host", "hq_weight_import", "hq_decode_int8", "hq_act_quant", "hq_linear",
            "hq_linear_group", "hq_linear_workspace_bytes", "hq_kv_create", "hq_kv_free", "hq_kv_append", "hq_attend", "hq_kv_export",
            "hq_kv_decode_int8"]
 
@@ -75,6 +91,10 @@ def load_library():
     lib.hq_destroy.argtypes = [vp]; lib.hq_destroy.restype = None
     lib.hq_last_error.argtypes = [vp]; lib.hq_last_error.restype = C.c_char_p
     lib.hq_alpha.argtypes = [i32, C.c_double]; lib.hq_alpha.restype = C.c_double
+    lib.hq_snr_for_bps.argtypes = [vp, i32, C.c_double, C.POINTER(C.c_float), C.POINTER(i32)]
+    lib.hq_weight_stats.argtypes = [vp, C.POINTER(_Stats)]
+    lib.hq_weight_export_host.argtypes = [vp, vp, C.POINTER(WeightHeader), vp, vp, vp]
+    lib.hq_weight_import.argtypes = [vp, C.POINTER(WeightHeader), vp, vp, vp, C.POINTER(vp)]
     lib.hq_profile_enable.argtypes = [vp, i32]
     lib.hq_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(i64)]
     lib.hq_encode_weights.argtypes = [vp, vp, i32, i64, i64, i64, C.POINTER(_CodecConfig), vp, C.POINTER(vp)]
@@ -98,6 +118,15 @@ def load_library():
 
 def alpha(lattice: int, snr_db: float) -> float:
     return load_library().hq_alpha(lattice, float(snr_db))
+
+
+def snr_for_bps(lattice: int, target_bps: float):
+    """(snr_db as the float32 the codec config carries, (k0, k1)) from the library's calibration table (host only)."""
+    snr, k = C.c_float(), (C.c_int32 * 2)()
+    st = load_library().hq_snr_for_bps(None, lattice, float(target_bps), C.byref(snr), k)
+    if st != 0:
+        raise HQError(f"hq_snr_for_bps: status {st} (target outside the table's range?)")
+    return float(snr.value), (int(k[0]), int(k[1]))
 
 
 def _dtype_code(t: torch.Tensor) -> int:
@@ -184,11 +213,20 @@ class Context:
                                             _stream_ptr(self.device)))
         return (ys, y32) if want_f32 else ys
 
+    def import_weight(self, header: "WeightHeader", blob, sub_off):
+        """hq_weight_import from host numpy arrays (the pair Weight.export_host returns)."""
+        import numpy as np
+        blob = np.ascontiguousarray(blob, dtype=np.uint8); sub_off = np.ascontiguousarray(sub_off, dtype=np.uint32)
+        h = C.c_void_p()
+        self.check(self.lib.hq_weight_import(self.h, C.byref(header), blob.ctypes.data, sub_off.ctypes.data,
+                                             _stream_ptr(self.device), C.byref(h)))
+        return Weight(self, h)
+
     # ---- KV ----
     def kv_create(self, kv_heads, head_dim, max_tokens, lattice, snr_db, rice_k, seed, rotation=1, dither=1,
-                  window=32):
+                  window=32, una_capacity_bits=0):
         codec = _CodecConfig(lattice, head_dim, float(snr_db), (C.c_int32 * 2)(int(rice_k[0]), int(rice_k[1])), seed)
-        cfg = _KVConfig(kv_heads, head_dim, max_tokens, codec, rotation, dither, window)
+        cfg = _KVConfig(kv_heads, head_dim, max_tokens, codec, rotation, dither, window, int(una_capacity_bits))
         h = C.c_void_p()
         self.check(self.lib.hq_kv_create(self.h, C.byref(cfg), C.byref(h)))
         return KVCache(self, h, kv_heads, head_dim, max_tokens)
@@ -216,6 +254,21 @@ class Weight:
         blob = _wrap(blob_p.value, self.info.blob_bytes, self.ctx.device).cpu().numpy()
         goff = _wrap(goff_p.value, (self.info.n_groups + 1) * 4, self.ctx.device).cpu().numpy().view("uint32")
         return blob, goff
+
+    def stats(self):
+        st = _Stats()
+        self.ctx.check(self.ctx.lib.hq_weight_stats(self.h, C.byref(st)))
+        return st
+
+    def export_host(self):
+        """(header, blob uint8, sub_off uint32): the encoded weight as host data (hq_weight_export_host)."""
+        import numpy as np
+        hd = WeightHeader()
+        self.ctx.check(self.ctx.lib.hq_weight_export_host(self.ctx.h, self.h, C.byref(hd), None, None, None))
+        blob = np.empty(hd.blob_bytes, np.uint8); goff = np.empty(hd.n_groups + 1, np.uint32)
+        self.ctx.check(self.ctx.lib.hq_weight_export_host(self.ctx.h, self.h, C.byref(hd), blob.ctypes.data,
+                                                          goff.ctypes.data, _stream_ptr(self.ctx.device)))
+        return hd, blob, goff
 
     def decode_int8(self):
         dev = self.ctx.device

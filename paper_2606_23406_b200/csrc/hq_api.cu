@@ -32,6 +32,25 @@ hq_status fail(hq_ctx* ctx, hq_status s, const char* msg) {
     return s;
 }
 
+// every entry point that launches work makes the context's device current (two contexts on two GPUs in one process)
+#define HQ_ENTER(ctx) HQ_CUDA_CHECK(ctx, cudaSetDevice((ctx)->device))
+
+// sticky error state of a KV cache: the append kernels raise the flag in mapped host memory (no synchronization here)
+hq_status kv_flag_status(hq_ctx* ctx, const hq_kv* kv) {
+    const int f = *(volatile int*)kv->flag_host;
+    if (f == 1) return fail(ctx, HQ_ERR_FORMAT, "a vector's U-section exceeds 65534 bits (FORMAT §4); the cache is unusable");
+    if (f == 2) return fail(ctx, HQ_ERR_FORMAT, "U-stream capacity exceeded (hq_kv_config.una_capacity_bits); the cache is unusable");
+    return HQ_OK;
+}
+
+// calibration table b(SNR) written by oracle/make_calib_table.py (G17): HQ_CALIB_N grid points from HQ_CALIB_SNR0 in
+// steps of HQ_CALIB_STEP dB; per lattice (Z, A2, D4, E8) the payload bits per scalar and the best k-set
+#include "hq_calib_table.inc"
+int calib_index(int lattice) { return lattice == HQ_Z ? 0 : lattice == HQ_A2 ? 1 : lattice == HQ_D4 ? 2 : 3; }
+
+constexpr uint32_t HQW_MAGIC = 0x31575148u;   // "HQW1"
+constexpr uint32_t HQW_VERSION = 2u;           // FORMAT v2 (sub-group container)
+
 }  // namespace
 
 extern "C" {
@@ -105,6 +124,22 @@ hq_status hq_profile_read(hq_ctx* ctx, double* total_ms, int64_t* launches) {
 double hq_alpha(int32_t lattice, double snr_db) {
     if (!valid_lattice(lattice)) return 0.0;
     return sqrt(pow(10.0, snr_db / 10.0) * second_moment(lattice));
+}
+
+hq_status hq_snr_for_bps(const hq_ctx* ctx, int32_t lattice, double target_bps, float* snr_db_out, int32_t* rice_k_out) {
+    (void)ctx;   // a host table lookup
+    if (!valid_lattice(lattice) || !snr_db_out) return HQ_ERR_INVALID_ARG;
+    const float* b = HQ_CALIB_BPS[calib_index(lattice)];
+    if (!(target_bps >= b[0]) || !(target_bps <= b[HQ_CALIB_N - 1])) return HQ_ERR_INVALID_ARG;
+    int i = 0;
+    while (i + 2 < HQ_CALIB_N && (double)b[i + 1] <= target_bps) ++i;   // b is increasing in SNR (checked by the generator)
+    const double f = (double)b[i + 1] > (double)b[i] ? (target_bps - b[i]) / ((double)b[i + 1] - (double)b[i]) : 0.0;
+    *snr_db_out = (float)(HQ_CALIB_SNR0 + HQ_CALIB_STEP * ((double)i + f));
+    if (rice_k_out) {
+        rice_k_out[0] = HQ_CALIB_K[calib_index(lattice)][i][0];
+        rice_k_out[1] = HQ_CALIB_K[calib_index(lattice)][i][1];
+    }
+    return HQ_OK;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -211,6 +246,7 @@ hq_status hq_encode_weights(hq_ctx* ctx, const void* W_dev, int32_t dtype, int64
     }
     w->max_group16 = *(uint32_t*)(hc + 19);
     w->min_ulen = 65535u - ((uint32_t*)(hc + 18))[4];
+    w->max_ulen = ((uint32_t*)(hc + 18))[5];
     w->blob_bytes = (int64_t)total16 * 16;
     w->payload_bits = (int64_t)hc[17] + m_out * w->n_kt * (int64_t)w->rbits;
     w->blob = (uint8_t*)ctx_alloc(ctx, (size_t)w->blob_bytes + 4096);  // slack: decoders read a word ahead, the fused kernel prefetches whole lines
@@ -251,9 +287,113 @@ hq_status hq_weight_export(const hq_weight* w, const void** blob_dev, const uint
     return HQ_OK;
 }
 
+hq_status hq_weight_stats(const hq_weight* w, hq_stats* out) {
+    if (!w || !out) return HQ_ERR_INVALID_ARG;
+    const int64_t tiles = w->m * w->n_kt;
+    out->payload_bits = w->payload_bits; out->norm_bits = 16 * tiles; out->length_bits = 16 * tiles;
+    out->offset_bits = 32 * 4 * w->G;
+    out->padding_bits = 8 * w->blob_bytes - out->payload_bits - out->norm_bits - out->length_bits;
+    out->clamp_count = w->clamp_count; out->n_tiles = tiles;
+    out->tile_bits_min = (int32_t)(w->rbits + w->min_ulen); out->tile_bits_max = (int32_t)(w->rbits + w->max_ulen);
+    const double sc = (double)w->m * (double)w->n_in;
+    out->bits_per_scalar_payload = (double)out->payload_bits / sc;
+    out->bits_per_scalar_total = (double)(out->payload_bits + out->norm_bits + out->length_bits) / sc;
+    return HQ_OK;
+}
+
+hq_status hq_weight_export_host(hq_ctx* ctx, const hq_weight* w, hq_weight_header* hd, void* blob_host,
+                                uint32_t* sub_off_host, void* stream) {
+    if (!ctx) return HQ_ERR_INVALID_ARG;
+    if (!w || !hd || ((blob_host == nullptr) != (sub_off_host == nullptr))) return fail(ctx, HQ_ERR_INVALID_ARG, "null argument");
+    if (w->ctx != ctx) return fail(ctx, HQ_ERR_INVALID_ARG, "the weight belongs to another context");
+    HQ_ENTER(ctx);
+    memset(hd, 0, sizeof(*hd));
+    hd->magic = HQW_MAGIC; hd->version = HQW_VERSION;
+    hd->m_out = w->m; hd->n_in = w->n_in; hd->lattice = w->lattice; hd->n_tile = w->n;
+    hd->rice_k[0] = w->k0; hd->rice_k[1] = w->k1; hd->snr_db = w->snr_db; hd->seed = w->seed;
+    hd->blob_bytes = w->blob_bytes; hd->n_groups = 4 * w->G;
+    hd->payload_bits = w->payload_bits; hd->clamp_count = w->clamp_count;
+    hd->ulen_min = (int32_t)w->min_ulen; hd->ulen_max = (int32_t)w->max_ulen;
+    if (!blob_host) return HQ_OK;
+    cudaStream_t st = (cudaStream_t)stream;
+    HQ_CUDA_CHECK(ctx, cudaMemcpyAsync(blob_host, w->blob, (size_t)w->blob_bytes, cudaMemcpyDeviceToHost, st));
+    HQ_CUDA_CHECK(ctx, cudaMemcpyAsync(sub_off_host, w->group_off, (size_t)(4 * w->G + 1) * 4, cudaMemcpyDeviceToHost, st));
+    HQ_CUDA_CHECK(ctx, cudaStreamSynchronize(st));
+    return HQ_OK;
+}
+
+hq_status hq_weight_import(hq_ctx* ctx, const hq_weight_header* hd, const void* blob_host, const uint32_t* sub_off_host,
+                           void* stream, hq_weight** out) {
+    if (!ctx) return HQ_ERR_INVALID_ARG;
+    if (!hd || !blob_host || !sub_off_host || !out) return fail(ctx, HQ_ERR_INVALID_ARG, "null argument");
+    *out = nullptr;
+    if (hd->magic != HQW_MAGIC || hd->version != HQW_VERSION) return fail(ctx, HQ_ERR_FORMAT, "not an HQW1 v2 header");
+    if (!valid_lattice(hd->lattice) || !valid_tile(hd->n_tile) || hd->m_out <= 0 || hd->n_in <= 0 || hd->n_in % hd->n_tile != 0)
+        return fail(ctx, HQ_ERR_FORMAT, "bad lattice / tile / shape in the header");
+    for (int a = 0; a < 2; ++a)
+        if (hd->rice_k[a] < 0 || hd->rice_k[a] > 7) return fail(ctx, HQ_ERR_FORMAT, "bad rice_k in the header");
+    const int64_t n_kt = hd->n_in / hd->n_tile, n_rb = (hd->m_out + 127) / 128, G = n_rb * n_kt;
+    if (hd->n_groups != 4 * G || hd->blob_bytes <= 0 || hd->blob_bytes % 16 != 0) return fail(ctx, HQ_ERR_FORMAT, "group count / blob size do not match the shape");
+    const int rbits = rbits_of(hd->lattice, hd->n_tile, hd->rice_k[0], hd->rice_k[1]);
+    const int64_t rw_words = (rbits + 31) / 32;
+    // layout checks (FORMAT §5): offsets increasing, inside the blob, and each sub-group exactly as long as its
+    // ulen header implies; present rows' ulen in [n_tile, 8160], absent rows' 0.  A decoder never leaves a checked blob.
+    const uint8_t* blob = (const uint8_t*)blob_host;
+    uint32_t umin = 65535u, umax = 0u;
+    int64_t usum = 0;
+    if (sub_off_host[0] != 0 || (int64_t)sub_off_host[4 * G] * 16 != hd->blob_bytes) return fail(ctx, HQ_ERR_FORMAT, "sub_off does not span the blob");
+    for (int64_t sg = 0; sg < 4 * G; ++sg) {
+        const int64_t o0 = (int64_t)sub_off_host[sg] * 16, o1 = (int64_t)sub_off_host[sg + 1] * 16;
+        if (o1 <= o0 || o1 > hd->blob_bytes || o1 - o0 < 128 + rw_words * 128) return fail(ctx, HQ_ERR_FORMAT, "sub_off is not increasing / a sub-group is truncated");
+        const uint16_t* ul = (const uint16_t*)(blob + o0);
+        const int64_t rb = (sg / 4) / n_kt, row0 = rb * 128 + (sg % 4) * 32;
+        int64_t words = 0;
+        for (int i = 0; i < 32; ++i) {
+            const uint32_t L = ul[i];
+            const bool present = row0 + i < hd->m_out;
+            if (present ? (L < (uint32_t)hd->n_tile || L > 8160u) : (L != 0u)) return fail(ctx, HQ_ERR_FORMAT, "a tile's ulen is out of range");
+            if (present) { umin = L < umin ? L : umin; umax = L > umax ? L : umax; usum += L; }
+            words += (L + 31) / 32;
+        }
+        const int64_t need = (128 + rw_words * 128 + words * 4 + 15) / 16 * 16;
+        if (need != o1 - o0) return fail(ctx, HQ_ERR_FORMAT, "a sub-group's size does not match its ulen header");
+    }
+    if (usum + hd->m_out * n_kt * (int64_t)rbits != hd->payload_bits) return fail(ctx, HQ_ERR_FORMAT, "payload_bits does not match the blob");
+    HQ_ENTER(ctx);
+    cudaStream_t st = (cudaStream_t)stream;
+    hq_weight* w = new (std::nothrow) hq_weight();
+    if (!w) return HQ_ERR_ALLOC;
+    memset((void*)w, 0, sizeof(*w));
+    w->ctx = ctx;
+    w->m = hd->m_out; w->n_in = hd->n_in; w->lattice = hd->lattice; w->n = hd->n_tile; w->snr_db = hd->snr_db;
+    w->seed = hd->seed; w->k0 = hd->rice_k[0]; w->k1 = hd->rice_k[1]; w->rbits = rbits;
+    w->alpha = hq_alpha(hd->lattice, (double)hd->snr_db);
+    w->A = (float)(w->alpha * sqrt((double)w->n));
+    w->n_kt = n_kt; w->n_rb = n_rb; w->G = G;
+    w->blob_bytes = hd->blob_bytes; w->payload_bits = hd->payload_bits; w->clamp_count = hd->clamp_count;
+    w->min_ulen = umin; w->max_ulen = umax;
+    w->dsign = (int8_t*)ctx_alloc(ctx, (size_t)w->n_in);
+    w->group_off = (uint32_t*)ctx_alloc(ctx, (size_t)(4 * G + 1) * 4);
+    w->blob = (uint8_t*)ctx_alloc(ctx, (size_t)w->blob_bytes + 4096);
+    if (!w->dsign || !w->group_off || !w->blob) { hq_weight_free(ctx, w); return HQ_ERR_ALLOC; }
+    cudaError_t e = cudaMemsetAsync(w->blob + w->blob_bytes, 0, 4096, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(w->blob, blob_host, (size_t)w->blob_bytes, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(w->group_off, sub_off_host, (size_t)(4 * G + 1) * 4, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) { launch_signs(w->seed, 1u, w->n_in, w->dsign, st); e = cudaGetLastError(); }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);   // the host buffers are the caller's again on return
+    if (e != cudaSuccess) {
+        ctx->err = std::string("hq_weight_import: ") + cudaGetErrorString(e);
+        hq_weight_free(ctx, w);
+        return HQ_ERR_CUDA;
+    }
+    *out = w;
+    return HQ_OK;
+}
+
 hq_status hq_decode_int8(hq_ctx* ctx, const hq_weight* w, int8_t* codes_dev, uint16_t* norms_dev, void* stream) {
     if (!ctx) return HQ_ERR_INVALID_ARG;
     if (!w || !codes_dev) return fail(ctx, HQ_ERR_INVALID_ARG, "null argument");
+    HQ_ENTER(ctx);
     launch_decode_int8(w, codes_dev, norms_dev, (cudaStream_t)stream);
     HQ_CUDA_CHECK(ctx, cudaGetLastError());
     return HQ_OK;
@@ -264,6 +404,7 @@ hq_status hq_act_quant(hq_ctx* ctx, const hq_weight* w, const void* x_dev, int32
     if (!ctx) return HQ_ERR_INVALID_ARG;
     if (!w || !x_dev || !q_dev || !s_x_dev) return fail(ctx, HQ_ERR_INVALID_ARG, "null argument");
     if (batch <= 0 || ldx < w->n_in) return fail(ctx, HQ_ERR_SHAPE, "bad batch / ldx");
+    HQ_ENTER(ctx);
     launch_act_quant(x_dev, dtype, batch, w->n_in, ldx, w->lattice, w->n, w->dsign, q_dev, s_x_dev, u_dev_or_null,
                      (cudaStream_t)stream);
     HQ_CUDA_CHECK(ctx, cudaGetLastError());
@@ -282,6 +423,8 @@ hq_status hq_linear(hq_ctx* ctx, const hq_weight* w, const void* x_dev, int32_t 
     if (!w || !x_dev || (!y_bf16_dev && !y_f32_dev_or_null)) return fail(ctx, HQ_ERR_INVALID_ARG, "null argument");
     if (batch <= 0 || ldx < w->n_in || (y_bf16_dev && ldy < w->m)) return fail(ctx, HQ_ERR_SHAPE, "bad batch / ldx / ldy");
     if (dtype != HQ_F32 && dtype != HQ_BF16) return fail(ctx, HQ_ERR_INVALID_ARG, "bad dtype");
+    if (w->ctx != ctx) return fail(ctx, HQ_ERR_INVALID_ARG, "the weight belongs to another context");
+    HQ_ENTER(ctx);
     cudaStream_t st = (cudaStream_t)stream;
     size_t need = linear_workspace_bytes(ctx, w, batch);
     if (need > ctx->ws_bytes) {
@@ -304,7 +447,9 @@ hq_status hq_linear_group(hq_ctx* ctx, const hq_weight* const* ws, int32_t n_w, 
         if (!ws[i] || !ys_bf16_dev[i]) return fail(ctx, HQ_ERR_INVALID_ARG, "null weight or output in group");
         if (ws[i]->n_in != ws[0]->n_in) return fail(ctx, HQ_ERR_SHAPE, "the weights of a group must share n_in");
         if (ldys[i] < ws[i]->m) return fail(ctx, HQ_ERR_SHAPE, "bad ldy");
+        if (ws[i]->ctx != ctx) return fail(ctx, HQ_ERR_INVALID_ARG, "a weight belongs to another context");
     }
+    HQ_ENTER(ctx);
     if (batch <= 0 || ldx < ws[0]->n_in) return fail(ctx, HQ_ERR_SHAPE, "bad batch / ldx");
     if (dtype != HQ_F32 && dtype != HQ_BF16) return fail(ctx, HQ_ERR_INVALID_ARG, "bad dtype");
     if (!linear_group_compatible(ws, n_w)) {   // one by one: same results, more launches
@@ -334,8 +479,10 @@ hq_status hq_kv_create(hq_ctx* ctx, const hq_kv_config* cfg, hq_kv** out) {
     if (!valid_lattice(cfg->codec.lattice)) return fail(ctx, HQ_ERR_INVALID_ARG, "bad lattice");
     if (!valid_tile(cfg->head_dim) || cfg->codec.n_tile != cfg->head_dim || cfg->kv_heads <= 0 || cfg->max_tokens <= 0)
         return fail(ctx, HQ_ERR_SHAPE, "head_dim must be 64/128/256 and equal codec.n_tile");
-    if (cfg->rotation != HQ_ROT_NONE && cfg->rotation != HQ_ROT_SIGNS)
-        return fail(ctx, HQ_ERR_UNSUPPORTED, "rotation qjl is not built (SURVEY §8(f))");
+    if (cfg->rotation == HQ_ROT_QJL) return fail(ctx, HQ_ERR_UNSUPPORTED, "rotation qjl is not built (SURVEY §8(f)1)");
+    if (cfg->rotation != HQ_ROT_NONE && cfg->rotation != HQ_ROT_SIGNS) return fail(ctx, HQ_ERR_INVALID_ARG, "bad rotation");
+    if (cfg->una_capacity_bits < 0) return fail(ctx, HQ_ERR_INVALID_ARG, "una_capacity_bits must be >= 0");
+    HQ_ENTER(ctx);
     if (cfg->codec.rice_k[0] < 0 || cfg->codec.rice_k[0] > 7 || cfg->codec.rice_k[1] > 7)
         return fail(ctx, HQ_ERR_INVALID_ARG, "KV needs explicit rice_k");
     if (cfg->window < 0 || cfg->window > cfg->head_dim) return fail(ctx, HQ_ERR_SHAPE, "window must be in [0, head_dim]");
@@ -354,8 +501,16 @@ hq_status hq_kv_create(hq_ctx* ctx, const hq_kv_config* cfg, hq_kv** out) {
     if ((double)mt * (kv->rbits > 0 ? kv->rbits : 1) > 4.0e9) { delete kv; return fail(ctx, HQ_ERR_SHAPE, "max_tokens too large for 32-bit bit offsets"); }
     kv->n_blk = (mt + 127) / 128;
     kv->rem_words = (mt * kv->rbits + 31) / 32 + 4;
-    // U-stream capacity: 4 unary bits per scalar on average (E[q] ~ 1 at the calibrated k, FORMAT §3)
-    int64_t una_bits = mt * (int64_t)d * 4 + 4096;
+    // U-stream capacity per (role, head): the caller's figure, else an estimate with margin.  On a vector normalized to
+    // radius alpha sqrt(d), E|zz| ~ E|c| <= alpha (0.8 alpha if Gaussian), so a class-a symbol costs about
+    // 1 + (0.8 alpha + 0.5) / 2^k_a unary bits; x 1.3, at least 4 per scalar.  Overflow is detected, never written.
+    int64_t una_bits = cfg->una_capacity_bits;
+    if (una_bits == 0) {
+        const int kmin = kv->k0 < kv->k1 ? kv->k0 : kv->k1;
+        double per = 1.3 * (1.0 + (0.8 * kv->alpha + 0.5) / (double)(1 << kmin));
+        if (per < 4.0) per = 4.0;
+        una_bits = (int64_t)((double)mt * d * per) + 4096;
+    }
     if (una_bits > 0xffff0000ll) una_bits = 0xffff0000ll;
     kv->una_words = una_bits / 32 + 4;
     size_t n_rh = (size_t)2 * H;
@@ -369,8 +524,14 @@ hq_status hq_kv_create(hq_ctx* ctx, const hq_kv_config* cfg, hq_kv** out) {
     kv->dsign = (int8_t*)ctx_alloc(ctx, d);
     kv->ssign = (int8_t*)ctx_alloc(ctx, d);
     kv->counters = (unsigned long long*)ctx_alloc(ctx, 64);
-    kv->att_ws_bytes = attend_workspace_bytes(kv, 64);
+    kv->att_ws_bytes = attend_workspace_bytes(ctx, kv);
     kv->att_ws = (float*)ctx_alloc(ctx, kv->att_ws_bytes);
+    if (cudaHostAlloc((void**)&kv->flag_host, 64, cudaHostAllocMapped) != cudaSuccess ||
+        cudaHostGetDevicePointer((void**)&kv->flag_dev, kv->flag_host, 0) != cudaSuccess) {
+        hq_kv_free(ctx, kv);
+        return fail(ctx, HQ_ERR_CUDA, "cudaHostAlloc for the cache's error flag failed");
+    }
+    *kv->flag_host = 0;
     if (!kv->rem || !kv->una || !kv->ulen || !kv->norm || !kv->blk_off || !kv->upos || !kv->ring || !kv->dsign ||
         !kv->ssign || !kv->counters || !kv->att_ws) {
         hq_kv_free(ctx, kv);
@@ -401,13 +562,17 @@ void hq_kv_free(hq_ctx* ctx, hq_kv* kv) {
     ctx_free(ctx, kv->rem); ctx_free(ctx, kv->una); ctx_free(ctx, kv->ulen); ctx_free(ctx, kv->norm);
     ctx_free(ctx, kv->blk_off); ctx_free(ctx, kv->upos); ctx_free(ctx, kv->ring); ctx_free(ctx, kv->dsign);
     ctx_free(ctx, kv->ssign); ctx_free(ctx, kv->counters); ctx_free(ctx, kv->scratch_codes); ctx_free(ctx, kv->att_ws);
+    if (kv->flag_host) { cudaDeviceSynchronize(); cudaFreeHost(kv->flag_host); }
     delete kv;
 }
 
 hq_status hq_kv_append(hq_ctx* ctx, hq_kv* kv, const void* k_dev, const void* v_dev, int64_t n_tok, void* stream) {
     if (!ctx) return HQ_ERR_INVALID_ARG;
     if (!kv || !k_dev || !v_dev) return fail(ctx, HQ_ERR_INVALID_ARG, "null argument");
+    if (kv->ctx != ctx) return fail(ctx, HQ_ERR_INVALID_ARG, "the cache belongs to another context");
     if (n_tok <= 0 || kv->n_tokens + n_tok > kv->cfg.max_tokens) return fail(ctx, HQ_ERR_SHAPE, "n_tok out of range");
+    if (hq_status fs = kv_flag_status(ctx, kv)) return fs;
+    HQ_ENTER(ctx);
     cudaStream_t st = (cudaStream_t)stream;
     int H = kv->cfg.kv_heads, d = kv->cfg.head_dim;
     if (n_tok == 1) {   // the decode step: one fused launch
@@ -425,7 +590,7 @@ hq_status hq_kv_append(hq_ctx* ctx, hq_kv* kv, const void* k_dev, const void* v_
         if (!kv->scratch_codes) { kv->scratch_tokens = 0; return HQ_ERR_ALLOC; }
         kv->scratch_tokens = cap;
     }
-    int* err_flag = (int*)(kv->counters + 1);
+    int* err_flag = kv->flag_dev;
     for (int64_t c0 = 0; c0 < n_tok; c0 += chunk) {
         int64_t nt = n_tok - c0 < chunk ? n_tok - c0 : chunk;
         int64_t token0 = kv->n_tokens + c0;
@@ -454,17 +619,20 @@ hq_status hq_attend(hq_ctx* ctx, const hq_kv* kv, const void* q_dev, int32_t q_h
     if (q_heads <= 0 || q_heads % kv->cfg.kv_heads != 0 || q_heads / kv->cfg.kv_heads > 8 || q_heads > 64)
         return fail(ctx, HQ_ERR_SHAPE, "q_heads must be a multiple of kv_heads, group size <= 8, q_heads <= 64");
     if (kv->n_tokens <= 0) return fail(ctx, HQ_ERR_SHAPE, "empty cache");
+    if (kv->ctx != ctx) return fail(ctx, HQ_ERR_INVALID_ARG, "the cache belongs to another context");
+    if (hq_status fs = kv_flag_status(ctx, kv)) return fs;
+    HQ_ENTER(ctx);
     return launch_attend(ctx, kv, q_dev, q_heads, out_bf16_dev, out_f32_dev_or_null, (cudaStream_t)stream);
 }
 
 hq_status hq_kv_export(hq_ctx* ctx, const hq_kv* kv, hq_kv_view* out) {
     if (!ctx) return HQ_ERR_INVALID_ARG;
     if (!kv || !out) return fail(ctx, HQ_ERR_INVALID_ARG, "null argument");
+    HQ_ENTER(ctx);
     HQ_CUDA_CHECK(ctx, cudaDeviceSynchronize());
     unsigned long long hc[8];
     HQ_CUDA_CHECK(ctx, cudaMemcpy(hc, kv->counters, sizeof(hc), cudaMemcpyDeviceToHost));
-    if (*(int*)(hc + 1) == 1) return fail(ctx, HQ_ERR_FORMAT, "a vector's U-section exceeds 65535 bits (FORMAT §4)");
-    if (*(int*)(hc + 1) == 2) return fail(ctx, HQ_ERR_FORMAT, "U-stream capacity exceeded");
+    if (hq_status fs = kv_flag_status(ctx, kv)) return fs;
     out->n_tokens = kv->n_tokens; out->rbits = kv->rbits;
     out->rem_dev = kv->rem; out->una_dev = kv->una; out->ulen_dev = kv->ulen; out->norm_dev = kv->norm;
     out->blk_off_dev = kv->blk_off; out->upos_dev = kv->upos;
@@ -478,6 +646,8 @@ hq_status hq_kv_decode_int8(hq_ctx* ctx, const hq_kv* kv, int32_t role, int64_t 
     if (!ctx) return HQ_ERR_INVALID_ARG;
     if (!kv || !codes_dev || role < 0 || role > 1) return fail(ctx, HQ_ERR_INVALID_ARG, "bad argument");
     if (t0 < 0 || n <= 0 || t0 + n > kv->n_tokens) return fail(ctx, HQ_ERR_SHAPE, "token range out of bounds");
+    if (hq_status fs = kv_flag_status(ctx, kv)) return fs;
+    HQ_ENTER(ctx);
     launch_kv_decode_int8(kv, role, t0, n, codes_dev, (cudaStream_t)stream);
     HQ_CUDA_CHECK(ctx, cudaGetLastError());
     return HQ_OK;

@@ -347,9 +347,9 @@ static int attend_n_split(const hq_ctx* ctx, const hq_kv* kv) {
     return (int)(ns < 1 ? 1 : ns);
 }
 
-size_t attend_workspace_bytes(const hq_kv* kv, int q_heads) {
-    // sized for the worst case split count (4 CTAs per SM)
-    return (size_t)(148 * 8) * (size_t)q_heads * (kv->cfg.head_dim + 2) * sizeof(float);
+size_t attend_workspace_bytes(const hq_ctx* ctx, const hq_kv* kv) {
+    // attend_n_split launches at most 4 CTAs per SM in total, each writing ATT_MAXG x (d + 2) floats
+    return (size_t)(ctx->sm_count * 4 + kv->cfg.kv_heads) * ATT_MAXG * (size_t)(kv->cfg.head_dim + 2) * sizeof(float);
 }
 
 hq_status launch_attend(hq_ctx* ctx, const hq_kv* kv, const void* q, int q_heads, void* out_bf16, float* out_f32,

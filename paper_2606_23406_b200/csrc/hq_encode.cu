@@ -393,9 +393,13 @@ __global__ void k_tile_ulen(const int8_t* codes, int64_t m, int64_t n_kt, int n,
         L = tile_ulen<LAT>(codes + r * (n_kt * n) + kt * n, n, k0, k1);
         if (L > W_ULEN_MAX) { atomicExch(err_flag, 1); L = W_ULEN_MAX; }
         // err_flag[4] tracks 65535 - (shortest U-section of a present row), warp-aggregated
-        uint32_t inv = 65535u - L;
-        inv = __reduce_max_sync(__activemask(), inv);
-        if ((threadIdx.x & 31) == (__ffs(__activemask()) - 1)) atomicMax((unsigned int*)err_flag + 4, inv);
+        const unsigned am = __activemask();
+        const uint32_t inv = __reduce_max_sync(am, 65535u - L);
+        const uint32_t mx = __reduce_max_sync(am, L);   // err_flag[5]: the longest U-section (hq_weight_stats)
+        if ((threadIdx.x & 31) == (__ffs(am) - 1)) {
+            atomicMax((unsigned int*)err_flag + 4, inv);
+            atomicMax((unsigned int*)err_flag + 5, mx);
+        }
     }
     ulen_tmp[idx] = (uint16_t)L;
 }
@@ -669,6 +673,13 @@ void launch_pack_groups(const int8_t* codes, const uint16_t* norms, const uint16
 // KV container (FORMAT §6).  Phase 1: per-vector ulen; phase 2: per (role, head) sequential-chunk
 // prefix over the new tokens (one warp per head), block offsets; phase 3: bit packing.
 // ---------------------------------------------------------------------------------------------
+// the cache's error flag lives in mapped host memory (hq_kv::flag): the host reads it without synchronizing
+__device__ inline void kv_raise(int* flag, int code) {
+    *(volatile int*)flag = code;
+    __threadfence_system();
+}
+constexpr uint32_t KV_NO_ROOM = 0xffffffffu;   // ustart of a vector whose U-section is not stored
+
 template <int LAT>
 __global__ void k_kv_ulen(const int8_t* codes, int64_t n_tok, int H, int d, int64_t token0, int k0, int k1,
                           int64_t max_tokens, uint16_t* ulen /*[H][max_tokens] of this role*/, int* err_flag) {
@@ -677,7 +688,7 @@ __global__ void k_kv_ulen(const int8_t* codes, int64_t n_tok, int H, int d, int6
     int64_t t = idx / H;
     int h = (int)(idx % H);
     uint32_t L = tile_ulen<LAT>(codes + idx * d, d, k0, k1);
-    if (L > 65535u) { atomicExch(err_flag, 1); L = 65535u; }
+    if (L >= 65535u) { kv_raise(err_flag, 1); L = 65535u; }   // 65535 marks "does not fit" for k_kv_offsets
     ulen[h * max_tokens + token0 + t] = (uint16_t)L;
 }
 
@@ -688,26 +699,28 @@ __global__ void k_kv_offsets(const uint16_t* ulen, int64_t n_tok, int H, int64_t
                              int64_t una_bits, int* err_flag) {
     int h = blockIdx.x;
     int lane = threadIdx.x;
-    uint32_t pos = upos[h];
+    uint64_t pos = upos[h];
+    bool bad = false;
     for (int64_t t0 = 0; t0 < n_tok; t0 += 32) {
         int64_t t = t0 + lane;
         uint32_t L = (t < n_tok) ? ulen[h * max_tokens + token0 + t] : 0;
-        uint32_t x = L;
+        uint64_t x = L;
         for (int o = 1; o < 32; o <<= 1) {
-            uint32_t y = __shfl_up_sync(0xffffffffu, x, o);
+            uint64_t y = __shfl_up_sync(0xffffffffu, x, o);
             if (lane >= o) x += y;
         }
-        uint32_t start = pos + x - L;
+        const uint64_t start = pos + x - L;
         if (t < n_tok) {
-            ustart_tmp[h * n_tok + t] = start;
-            if (((token0 + t) & 127) == 0) blk_off[h * (n_blk + 1) + ((token0 + t) >> 7)] = start;
+            // a vector that does not fit (stream capacity, or a U-section past 65534 bits) is not written at all
+            const bool fits = L < 65535u && start + L <= (uint64_t)una_bits;
+            bad |= !fits;
+            ustart_tmp[h * n_tok + t] = fits ? (uint32_t)start : KV_NO_ROOM;
+            if (((token0 + t) & 127) == 0) blk_off[h * (n_blk + 1) + ((token0 + t) >> 7)] = (uint32_t)min(start, (uint64_t)una_bits);
         }
         pos += __shfl_sync(0xffffffffu, x, 31);
     }
-    if (lane == 0) {
-        if ((int64_t)pos > una_bits) atomicExch(err_flag, 2);
-        upos[h] = pos;
-    }
+    if (__any_sync(0xffffffffu, bad) && lane == 0) kv_raise(err_flag, 2);
+    if (lane == 0) upos[h] = (uint32_t)min(pos, (uint64_t)una_bits + 1u);
 }
 
 template <int LAT>
@@ -723,7 +736,9 @@ k_kv_pack(const int8_t* codes, int64_t n_tok, int H, int d, int64_t token0, int 
     tile_symbols<LAT>(codes + idx * d, d, z);
     BitWriter<StoreAtomicOr> bwr(StoreAtomicOr{rem + h * rem_words}, (uint32_t)((token0 + t) * rbits));
     write_R<LAT>(bwr, z, d, k0, k1);
-    BitWriter<StoreAtomicOr> bwu(StoreAtomicOr{una + h * una_words}, ustart_tmp[h * n_tok + t]);
+    const uint32_t ustart = ustart_tmp[h * n_tok + t];
+    if (ustart == KV_NO_ROOM) return;   // flagged by k_kv_offsets: nothing is written past the stream's capacity
+    BitWriter<StoreAtomicOr> bwu(StoreAtomicOr{una + h * una_words}, ustart);
     write_U<LAT>(bwu, z, d, k0, k1);
 }
 
@@ -796,7 +811,8 @@ struct KvAppend1 {
     uint32_t *rem, *una, *blk_off, *upos;
     uint16_t *ulen, *norm;
     __nv_bfloat16* ring;
-    unsigned long long* counters;   // [0] clamps, [1] (as int) error flag
+    unsigned long long* counters;   // [0] clamps
+    int* flag;                      // mapped host memory: error flag of the cache
 };
 
 template <int LAT>
@@ -851,14 +867,13 @@ k_kv_append1(KvAppend1 p) {
     }
     for (int o = 16; o; o >>= 1) L += __shfl_xor_sync(0xffffffffu, L, o);
     __syncwarp();
-    int* err_flag = (int*)(p.counters + 1);
-    if (L > 65535u) { if (lane == 0) atomicExch(err_flag, 1); L = 65535u; }
     uint32_t ustart = 0;
     if (lane == 0) {
         ustart = p.upos[rh];
         if ((p.token & 127) == 0) p.blk_off[rh * (p.n_blk + 1) + (p.token >> 7)] = ustart;
-        if ((int64_t)ustart + L > p.una_words * 32 - 64) atomicExch(err_flag, 2);
-        p.upos[rh] = ustart + L;
+        if (L >= 65535u) { kv_raise(p.flag, 1); L = 65535u; ustart = KV_NO_ROOM; }
+        else if ((int64_t)ustart + L > p.una_words * 32 - 64) { kv_raise(p.flag, 2); ustart = KV_NO_ROOM; }
+        else p.upos[rh] = ustart + L;
         p.ulen[rh * p.max_tokens + p.token] = (uint16_t)L;
     }
     // pack: lane 0 writes the R-section, lane 1 the U-section (serial bit writers; 2 x 128 symbols)
@@ -866,7 +881,7 @@ k_kv_append1(KvAppend1 p) {
     if (lane == 0) {
         BitWriter<StoreAtomicOr> bwr(StoreAtomicOr{p.rem + rh * p.rem_words}, (uint32_t)(p.token * p.rbits));
         write_R<LAT>(bwr, z, d, p.k0, p.k1);
-    } else if (lane == 1) {
+    } else if (lane == 1 && ustart != KV_NO_ROOM) {   // a vector that does not fit is not written (flag raised)
         BitWriter<StoreAtomicOr> bwu(StoreAtomicOr{p.una + rh * p.una_words}, ustart);
         write_U<LAT>(bwu, z, d, p.k0, p.k1);
     }
@@ -880,7 +895,7 @@ void launch_kv_append1(const hq_kv* kv, const void* k, const void* v, cudaStream
     p.token = kv->n_tokens; p.max_tokens = kv->cfg.max_tokens; p.rem_words = kv->rem_words; p.una_words = kv->una_words;
     p.n_blk = kv->n_blk; p.A = kv->A; p.seed = kv->cfg.codec.seed; p.dsign = kv->dsign; p.ssign = kv->ssign;
     p.rem = kv->rem; p.una = kv->una; p.blk_off = kv->blk_off; p.upos = kv->upos; p.ulen = kv->ulen; p.norm = kv->norm;
-    p.ring = kv->ring; p.counters = kv->counters;
+    p.ring = kv->ring; p.counters = kv->counters; p.flag = kv->flag_dev;
     const size_t smem = (size_t)p.d * (4 + 4 + 1 + 1);
     dim3 grid((unsigned)p.H, 2);
     switch (kv->cfg.codec.lattice) {

@@ -42,6 +42,7 @@ struct hq_weight {
     int64_t blob_bytes, payload_bits, clamp_count;
     uint32_t max_group16;  // largest sub-group size in 16-byte units
     uint32_t min_ulen;     // shortest U-section (bits) over the present rows of all tiles
+    uint32_t max_ulen;     // longest
 };
 
 struct hq_kv {
@@ -61,7 +62,9 @@ struct hq_kv {
     __nv_bfloat16* ring;  // [2][window][H][d]
     int8_t* dsign;      // [d]
     int8_t* ssign;      // [d]
-    unsigned long long* counters;  // [1] clamp count
+    unsigned long long* counters;  // [0] clamp count
+    int* flag_host;                // mapped pinned host word: 0 ok, 1 a U-section past 65534 bits, 2 U stream full (sticky)
+    int* flag_dev;                 // its device alias (the append kernels raise it, the host polls it without a sync)
     int8_t* scratch_codes;         // [2][chunk][H][d]
     int64_t scratch_tokens;
     float* att_ws;                 // split partials
@@ -111,7 +114,7 @@ void launch_act_quant(const void* x, int dtype, int64_t B, int64_t n_in, int64_t
 void launch_act_blob(const void* x, int dtype, int64_t B, int64_t n_in, int64_t ldx, const int8_t* dsign, int NB,
                      uint8_t* bblob, cudaStream_t st);
 // ulen_tmp[sg*32 + i] for all sub-groups (0 for absent rows); err_flag[0] set if a tile exceeds 8160 bits,
-// err_flag[4] = max over present rows of 65535 - ulen
+// err_flag[4] = max over present rows of 65535 - ulen, err_flag[5] = max over present rows of ulen
 void launch_tile_ulen(const int8_t* codes, int64_t m, int64_t n_in, int lattice, int n, int k0, int k1,
                       uint16_t* ulen_tmp, int* err_flag, cudaStream_t st);
 // group_off[G4+1] (sub-group offsets, 16-byte units) by a device prefix sum; totals[0] = sum of ulen over all tiles
@@ -148,6 +151,6 @@ bool linear_uses_e8_fast(const hq_weight* w);
 void launch_kv_decode_int8(const hq_kv* kv, int role, int64_t t0, int64_t n, int8_t* codes, cudaStream_t st);
 hq_status launch_attend(hq_ctx* ctx, const hq_kv* kv, const void* q, int q_heads, void* out_bf16,
                         float* out_f32, cudaStream_t st);
-size_t attend_workspace_bytes(const hq_kv* kv, int q_heads);
+size_t attend_workspace_bytes(const hq_ctx* ctx, const hq_kv* kv);
 
 }  // namespace hq

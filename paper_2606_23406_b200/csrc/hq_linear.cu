@@ -8,7 +8,6 @@
 
 #include "hq_common.cuh"
 #include "hq_internal.h"
-#include <stdlib.h>
 #include "hq_linear_e8.cuh"
 #include "hq_linear_large.cuh"
 #include "hq_tc.cuh"
@@ -240,15 +239,8 @@ static hq_status launch_generic_nb(hq_ctx* ctx, const hq_weight* w, LinearParams
 // ---- E8 fast path -----------------------------------------------------------------------------
 bool linear_uses_e8_fast(const hq_weight* w) { return w->lattice == LAT_E8 && w->n == 128 && w->k0 <= 3; }
 
-// activation rows from which the decode-once large-M path is used; HQ_LARGE_MIN_B overrides it (tuning)
-static int64_t lg_min_b() {
-    static const int64_t v = [] {
-        const char* e = getenv("HQ_LARGE_MIN_B");
-        return e && *e ? (int64_t)atoll(e) : (int64_t)64;
-    }();
-    return v;
-}
-#define LG_MIN_B lg_min_b()
+// activation rows from which the decode-once large-M path is used (measured crossover)
+constexpr int64_t LG_MIN_B = 64;
 struct E8Plan { int NB, BC, NWG, CPS, n_bt, n_split, L, n_items, grid; };
 // plan for a group of weights that share n_in (their row blocks are stacked into one item space)
 static E8Plan e8_plan(const hq_ctx* ctx, int64_t n_rb_total, int64_t n_kt64, int64_t n_in, int64_t B) {
@@ -335,8 +327,8 @@ size_t linear_workspace_bytes(const hq_ctx* ctx, const hq_weight* w, int64_t B) 
 // Large-M path (hq_linear_large.cuh): activation blob of 256-row tiles, then per weight one decode into the operand-layout
 // scratch copy and one warp-specialised GEMM.  The scratch copy is reused by the weights of a group (stream order).
 static hq_status launch_large(hq_ctx* ctx, const hq_weight* const* ws, int n_w, const void* x, int dtype, int64_t B,
-                              int64_t ldx, void* const* ys_bf16, const int64_t* ldys, float* const* ys_f32, uint8_t* wsbuf,
-                              cudaStream_t st) {
+                              int64_t ldx, void* const* ys_bf16, const int64_t* ldys, float* const* ys_f32, int32_t* acc_i32,
+                              uint8_t* wsbuf, cudaStream_t st) {
     const hq_weight* w0 = ws[0];
     const int64_t n_bt = (B + LG_NB - 1) / LG_NB;
     uint8_t* bblob = wsbuf;
@@ -371,6 +363,7 @@ static hq_status launch_large(hq_ctx* ctx, const hq_weight* const* ws, int n_w, 
         E8LargeParams g;
         g.ablob = ablob; g.bblob = bblob; g.y_bf16 = (__nv_bfloat16*)ys_bf16[i]; g.y_f32 = ys_f32 ? ys_f32[i] : nullptr;
         g.ldy = ldys[i]; g.m = w->m; g.B = B; g.n_rb = (int)w->n_rb; g.n_bt = (int)n_bt; g.n_kt = (int)w->n_kt;
+        g.acc_i32 = (n_w == 1) ? acc_i32 : nullptr;
         const int64_t tiles = (int64_t)g.n_rb * g.n_bt;
         const unsigned grid = (unsigned)(tiles < ctx->sm_count ? tiles : ctx->sm_count);
         HQ_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_e8_gemm_large, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LG_SMEM));
@@ -392,8 +385,12 @@ hq_status launch_linear_group(hq_ctx* ctx, const hq_weight* const* ws, int n_w, 
     const hq_weight* w0 = ws[0];
     int64_t n_rb = 0;
     for (int i = 0; i < n_w; ++i) n_rb += ws[i]->n_rb;
-    if (B >= LG_MIN_B && !acc_i32) return launch_large(ctx, ws, n_w, x, dtype, B, ldx, ys_bf16, ldys, ys_f32, wsbuf, st);
+    if (B >= LG_MIN_B) return launch_large(ctx, ws, n_w, x, dtype, B, ldx, ys_bf16, ldys, ys_f32, acc_i32, wsbuf, st);
     E8Plan pl = e8_plan(ctx, n_rb, w0->n_kt, w0->n_in, B);
+    // the tile descriptor of the fused kernel packs its fields (hq_linear_e8.cuh E8Desc): reject shapes that would alias
+    for (int i = 0; i < n_w; ++i)
+        if (ws[i]->n_rb >= 65536 || ws[i]->n_rb * w0->n_kt >= (1ll << 31)) { ctx->err = "m_out too large for the fused kernel (< 8388608 rows, row blocks x K-tiles < 2^31)"; return HQ_ERR_SHAPE; }
+    if (w0->n_kt >= 4096 || pl.n_bt >= 4096 || pl.n_split >= 4096) { ctx->err = "n_in / n_tile and batch tiles must be below 4096 on the fused path"; return HQ_ERR_SHAPE; }
     uint8_t* bblob = wsbuf;
     uint8_t* at = wsbuf + align256((size_t)pl.n_bt * w0->n_kt * e8_bblob_bytes(pl.NB));
     launch_act_blob(x, dtype, B, w0->n_in, ldx, w0->dsign, pl.NB, bblob, st);

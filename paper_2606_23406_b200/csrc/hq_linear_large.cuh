@@ -137,6 +137,7 @@ struct E8LargeParams {
     float* y_f32;           // [B][m] or null
     int64_t ldy, m, B;
     int n_rb, n_bt, n_kt;
+    int32_t* acc_i32;       // [n_kt][B][m] or null: parity / debug copy of every K-tile's INT32 accumulator
 };
 
 __global__ void __launch_bounds__(384, 1) k_e8_gemm_large(E8LargeParams p) {
@@ -244,6 +245,13 @@ __global__ void __launch_bounds__(384, 1) k_e8_gemm_large(E8LargeParams p) {
                         if (it + 1 < n_steps) begin_step(it + 1);
                     }
                     const uint32_t* vc = v[ch & 1];
+                    if (p.acc_i32) {   // parity / debug output, off the hot path
+                        const int64_t rr = (int64_t)rb * 128 + row;
+                        const int64_t bb = (int64_t)bt * LG_NB + half * 128 + c0;
+                        if (rr < p.m)
+                            for (int e = 0; e < 32; ++e)
+                                if (bb + e < p.B) p.acc_i32[((int64_t)kt * p.B + bb + e) * p.m + rr] = (int)vc[e];
+                    }
 #pragma unroll
                     for (int e = 0; e < 8; ++e) {
                         const uint4 s4 = lds128(sx_a + (c0 + 4 * e) * 4);

@@ -165,14 +165,15 @@ def test_linear_large_m_path(ctx, B, m, k):
     enc = hqo.encode_weights(W, hqo.E8, 128, snr, seed, k)
     w = ctx.encode_weights(_dev(W), hqo.E8, 128, snr, seed, k)
     q_o, sx_o = hqo.act_quant(x, hqo.E8, 128, seed)
-    _, y_o = hqo.linear(enc["codes"], enc["norms"], hqo.E8, 128, snr, q_o, sx_o)
+    acc_o, y_o = hqo.linear(enc["codes"], enc["norms"], hqo.E8, 128, snr, q_o, sx_o)
     xd = _dev(x, torch.bfloat16)
     y, y32, _ = w.linear(xd, want_f32=True)
     assert _rel_err(y32.cpu().numpy(), y_o) < 1e-3
     _assert_bf16_close(y, y_o)
-    # the fused kernel (the one that also returns the accumulators) gives the same outputs to fp32 rounding order
-    y_f, y32_f, _ = w.linear(xd, want_f32=True, want_acc=True)
-    assert _rel_err(y32.cpu().numpy(), y32_f.cpu().numpy().astype(np.float64)) < 1e-3
+    # the INT32 accumulators of THIS path (every K-tile's TMEM tile as the epilogue drains it), bit for bit
+    y_f, y32_f, acc = w.linear(xd, want_f32=True, want_acc=True)
+    assert (acc.cpu().numpy() == acc_o).all()
+    assert torch.equal(y32_f, y32) and torch.equal(y_f, y)
     ys, y32s = ctx.linear_group([w, w], xd, want_f32=True)
     assert torch.equal(y32s[0], y32) and torch.equal(y32s[1], y32) and torch.equal(ys[1], y)
     w.free()
@@ -285,6 +286,131 @@ def test_attend_matches_oracle_long_way(ctx, lattice, snr, k, dither, T, window)
     assert _rel_err(o32.cpu().numpy(), ref) < 1e-3
     _assert_bf16_close(out, ref)
     kv.free()
+
+
+def test_attend_several_blocks_per_split_matches_oracle(ctx):
+    """64 KV heads leave 148*4/64 = 9 splits per head: 3600 tokens = 28 blocks of 128 -> 4 blocks per split, so the
+    running-max rescale INSIDE a split (online softmax, L178) is compared with the oracle's long way round."""
+    T, H, d, QH, seed, snr = 3600, 64, 128, 64, 6, f32(9.68)
+    K = hq_synth.kv_tokens(T, H, d, seed=24); V = hq_synth.kv_tokens(T, H, d, seed=25)
+    K[1500:1510] *= 6.0                                            # a late block raises the running max
+    K = hq_synth.to_bf16_f32(K)
+    q = hq_synth.activations(QH, d, seed=26)
+    kv = ctx.kv_create(H, d, 4096, hqo.E8, snr, (0, 0), seed, rotation=1, dither=1, window=32)
+    kv.append(_dev(K, torch.bfloat16), _dev(V, torch.bfloat16))
+    out, o32 = kv.attend(_dev(q, torch.bfloat16), want_f32=True)
+    ck, nk, _ = hqo.kv_quantize(K, 0, 0, hqo.E8, snr, 1, 1, seed)
+    cv, nv, _ = hqo.kv_quantize(V, 0, 1, hqo.E8, snr, 1, 1, seed)
+    Kh = hqo.kv_reconstruct(ck, nk, 0, 0, hqo.E8, snr, 1, 1, seed)
+    Vh = hqo.kv_reconstruct(cv, nv, 0, 1, hqo.E8, snr, 1, 1, seed)
+    ref = hqo.attend(Kh, Vh, K, V, window=32, q=q)
+    assert _rel_err(o32.cpu().numpy(), ref) < 1e-3
+    _assert_bf16_close(out, ref)
+    kv.free()
+
+
+def test_kv_u_stream_overflow_is_detected_never_written_and_sticky(ctx):
+    """a legal config whose unary bits outrun the U stream.  E8 at 22.68 dB with k = (0, 0) costs ~6.4 unary
+    bits per scalar.  (i) the default capacity holds a full cache of it, container bit-exact; (ii) with a small
+    caller-given capacity the vectors that do not fit are not written (the neighbouring head's stream and the words
+    past the stream stay as the oracle has them), and the cache turns HQ_ERR_FORMAT on the next call and stays so."""
+    import paper_2606_23406_b200 as hq
+    T, H, d, seed, snr, k = 256, 2, 128, 31, f32(22.68), (0, 0)
+    K = hq_synth.kv_tokens(T, H, d, seed=4); V = hq_synth.kv_tokens(T, H, d, seed=5)
+    ora = _oracle_kv_container(K, V, hqo.E8, snr, k, 1, 1, seed, [T])
+    assert ora["upos"].min() > 5.0 * T * d                          # really more than the old 4 bits / scalar
+    kv = ctx.kv_create(H, d, T, hqo.E8, snr, k, seed, rotation=1, dither=1, window=0)
+    kv.append(_dev(K, torch.bfloat16), _dev(V, torch.bfloat16))
+    ex = kv.export()
+    assert (ex["upos"] == ora["upos"]).all()
+    nu = min(ex["una"].shape[2], ora["una"].shape[2])
+    assert (ex["una"][:, :, :nu] == ora["una"][:, :, :nu]).all()
+    kv.free()
+    cap = int(ora["upos"].min()) // 2 // 32 * 32                    # room for about half of the tokens
+    for chunks in ([T], [1] * 200):                                 # the bulk kernels and the one-token kernel
+        kv = ctx.kv_create(H, d, T, hqo.E8, snr, k, seed, rotation=1, dither=1, window=0, una_capacity_bits=cap)
+        t0, raised = 0, False
+        try:
+            for n in chunks:
+                kv.append(_dev(K[t0:t0 + n], torch.bfloat16), _dev(V[t0:t0 + n], torch.bfloat16))
+                t0 += n
+                torch.cuda.synchronize()
+        except hq.HQError:
+            raised = True
+        torch.cuda.synchronize()
+        if not raised:                                              # the bulk call itself is asynchronous: the NEXT call reports
+            with pytest.raises(hq.HQError):
+                kv.attend(_dev(hq_synth.activations(8, d, seed=1), torch.bfloat16))
+        with pytest.raises(hq.HQError):                             # sticky
+            kv.append(_dev(K[:1], torch.bfloat16), _dev(V[:1], torch.bfloat16))
+        with pytest.raises(hq.HQError):
+            kv.export()
+        # nothing was written outside [0, cap) of any stream: compare raw memory with the oracle's prefix
+        una_words = cap // 32 + 4
+        raw = None                                                  # the cache's `una` allocation, found by its size
+        for obj in list(ctx._live.values()):
+            if obj.numel() == 2 * H * una_words * 4:
+                raw = obj.cpu().numpy().view(np.uint32).reshape(2, H, una_words)
+        assert raw is not None
+        for role in range(2):
+            for h in range(H):
+                cs = np.concatenate([[0], np.cumsum(ora["ulen"][role, h].astype(np.int64))])
+                n_fit = int(np.searchsorted(cs, cap - 64, side="right")) - 1      # tokens whose U-section ends inside
+                full_words = int(cs[n_fit]) // 32
+                assert (raw[role, h, :full_words] == ora["una"][role, h, :full_words]).all()
+                assert (raw[role, h, (cap - 64) // 32 + 1:] == 0).all()          # the guard zone is untouched
+        kv.free()
+
+
+def test_weight_export_host_import_round_trip_and_layout_checks(ctx):
+    """SURVEY §5 checkpoint: the encoded weight leaves the process as host data and comes back; the imported handle
+    is bit-identical in hq_linear / hq_decode_int8; a blob that fails the layout checks is HQ_ERR_FORMAT."""
+    import paper_2606_23406_b200 as hq
+    for lattice, n_tile, m in ((hqo.E8, 128, 300), (hqo.D4, 64, 130)):
+        snr, seed = SNR_4BPS[lattice], 9
+        W = hq_synth.gaussian_weight(m, 512, seed=m, outliers=True)
+        w, enc = _check_weight_bitstream(ctx, W, lattice, n_tile, snr, seed)
+        hd, blob, goff = w.export_host()
+        assert (blob == enc["blob"]).all() and (goff == enc["group_off"]).all()
+        assert hd.payload_bits == enc["payload_bits"] and (hd.rice_k[0], hd.rice_k[1]) == tuple(int(v) for v in enc["k"])
+        w2 = ctx.import_weight(hd, blob.copy(), goff.copy())
+        c1, n1 = w.decode_int8(); c2, n2 = w2.decode_int8()
+        assert torch.equal(c1, c2) and torch.equal(n1, n2)
+        for B in (1, 16, 70):
+            x = _dev(hq_synth.activations(B, 512, seed=B), torch.bfloat16)
+            a = w.linear(x, want_f32=True, want_acc=True); b = w2.linear(x, want_f32=True, want_acc=True)
+            assert all(torch.equal(u, v) for u, v in zip(a, b))
+        st1, st2 = w.stats(), w2.stats()
+        tb = [hqo.tile_bits(lattice, enc["codes"][r, t * n_tile:(t + 1) * n_tile], enc["k"])
+              for r in range(m) for t in range(512 // n_tile)]
+        for st in (st1, st2):
+            assert (st.tile_bits_min, st.tile_bits_max) == (min(tb), max(tb))
+            assert st.payload_bits == sum(tb) and st.n_tiles == len(tb) and st.clamp_count == enc["clamps"]
+            assert st.padding_bits == 8 * blob.size - st.payload_bits - 32 * len(tb) and st.padding_bits >= 0
+        bad = goff.copy(); bad[3] += 1
+        with pytest.raises(hq.HQError):
+            ctx.import_weight(hd, blob, bad)
+        bad = blob.copy(); bad[int(goff[2]) * 16] ^= 0x40           # a ulen that no longer matches its sub-group's size
+        with pytest.raises(hq.HQError):
+            ctx.import_weight(hd, bad, goff)
+        hd2 = hq.WeightHeader.from_buffer_copy(hd); hd2.n_tile = 96
+        with pytest.raises(hq.HQError):
+            ctx.import_weight(hd2, blob, goff)
+        w.free(); w2.free()
+
+
+def test_snr_for_bps_operating_points_realize_their_rate_on_the_gpu_encoder(ctx):
+    """§5.4: target bps -> table SNR -> the GPU encoder on iid Gaussian tiles realizes the rate within
+    ~0.01 bps of the target (L295, L381)."""
+    import paper_2606_23406_b200 as hq
+    tiles = hq_synth.calib_tiles(4096, 128, seed=43)                # fresh tiles, not the table's
+    W = _dev(tiles.reshape(512, 1024).copy())
+    for lat in (hqo.E8, hqo.D4, hqo.A2, hqo.Z):
+        for bps in (3.0, 4.0, 5.0):
+            snr, k = hq.snr_for_bps(lat, bps)
+            w = ctx.encode_weights(W, lat, 128, snr, seed=1)
+            assert abs(w.stats().bits_per_scalar_payload - bps) < 0.015, (lat, bps)
+            w.free()
 
 
 def test_empty_and_out_of_range_arguments_fail_loudly_and_leave_the_context_usable(ctx):
