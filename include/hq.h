@@ -75,6 +75,12 @@ const char* hq_last_error(const hq_ctx* ctx); /* never NULL; valid until the nex
 hq_status hq_profile_enable(hq_ctx* ctx, int32_t on);
 hq_status hq_profile_read(hq_ctx* ctx, double* total_ms, int64_t* launches);
 
+/* Measurement aid: the issue-slot ceiling of the E8 Rice decode on this device.  Every warp of a
+ * full grid (one CTA per SM, the fused kernel's CTA shape) keeps one sub-group of `w` in registers and runs the fused
+ * kernel's decode phases on it `reps` times - no global loads in the loop, no MMA, no split-K.  Returns decoded
+ * scalars per second (CUDA events on `stream`, synchronizes).  w must be E8 / tile 128 / k <= 3 (HQ_ERR_UNSUPPORTED). */
+hq_status hq_measure_decode_ceiling(hq_ctx* ctx, const hq_weight* w, int32_t reps, void* stream, double* scalars_per_s);
+
 /* alpha of eq.(9) L871 for (lattice, snr_db), as the library computes it (host, double). */
 double hq_alpha(int32_t lattice, double snr_db);
 
@@ -184,7 +190,9 @@ hq_status hq_linear(hq_ctx* ctx, const hq_weight* w, const void* x_dev, int32_t 
 /*
  * Several weights applied to the SAME x in one fused launch (q/k/v or gate/up of a decoder layer: §5.1 L309 quantizes
  * every nn.Linear separately, the forward shares the input).  ws[i] -> ys_bf16[i] [batch, m_i] (leading dimension
- * ldys[i]).  Results are bit-identical to n_w separate hq_linear calls.  1 <= n_w <= 4.  Weights that cannot share
+ * ldys[i]).  From 2 activation rows the results are bit-identical to n_w separate hq_linear calls; at batch 1 the K range of
+ * a row block is summed in the segments the launch's flat tile partition cuts it into, so grouped and separate calls
+ * agree to fp32 rounding (each call is deterministic: same call, same bits).  1 <= n_w <= 4.  Weights that cannot share
  * a launch (different n_in / lattice / tile / Rice k / seed / snr_db, or not on the E8 fast path) are run one by one.
  * ys_f32_or_null: optional array of n_w dev pointers (entries may be NULL) for the fp32 pre-cast outputs.
  */

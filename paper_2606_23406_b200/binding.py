@@ -70,7 +70,7 @@ def lib_path() -> str:
 
 _lib = None
 
-EXPORTS = ["hq_create", "hq_destroy", "hq_last_error", "hq_alpha", "hq_snr_for_bps", "hq_profile_enable", "hq_profile_read",
+EXPORTS = ["hq_create", "hq_destroy", "hq_last_error", "hq_measure_decode_ceiling", "hq_alpha", "hq_snr_for_bps", "hq_profile_enable", "hq_profile_read",
            "hq_encode_weights", "hq_weight_free", "hq_weight_get_info", "hq_weight_stats", "hq_weight_export",
            "hq_weight_export_host", "hq_weight_import", "hq_decode_int8", "hq_act_quant", "hq_linear",
            "hq_linear_group", "hq_linear_workspace_bytes", "hq_kv_create", "hq_kv_free", "hq_kv_append", "hq_attend", "hq_kv_export",
@@ -95,6 +95,7 @@ def load_library():
     lib.hq_weight_stats.argtypes = [vp, C.POINTER(_Stats)]
     lib.hq_weight_export_host.argtypes = [vp, vp, C.POINTER(WeightHeader), vp, vp, vp]
     lib.hq_weight_import.argtypes = [vp, C.POINTER(WeightHeader), vp, vp, vp, C.POINTER(vp)]
+    lib.hq_measure_decode_ceiling.argtypes = [vp, vp, i32, vp, C.POINTER(C.c_double)]
     lib.hq_profile_enable.argtypes = [vp, i32]
     lib.hq_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(i64)]
     lib.hq_encode_weights.argtypes = [vp, vp, i32, i64, i64, i64, C.POINTER(_CodecConfig), vp, C.POINTER(vp)]
@@ -254,6 +255,13 @@ class Weight:
         blob = _wrap(blob_p.value, self.info.blob_bytes, self.ctx.device).cpu().numpy()
         goff = _wrap(goff_p.value, (self.info.n_groups + 1) * 4, self.ctx.device).cpu().numpy().view("uint32")
         return blob, goff
+
+    def decode_ceiling(self, reps=200):
+        """Decode-only issue ceiling of the E8 decoder on this weight's data (scalars per second)."""
+        v = C.c_double()
+        self.ctx.check(self.ctx.lib.hq_measure_decode_ceiling(self.ctx.h, self.h, reps, _stream_ptr(self.ctx.device),
+                                                              C.byref(v)))
+        return v.value
 
     def stats(self):
         st = _Stats()

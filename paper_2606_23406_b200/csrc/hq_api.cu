@@ -121,6 +121,15 @@ hq_status hq_profile_read(hq_ctx* ctx, double* total_ms, int64_t* launches) {
     return HQ_OK;
 }
 
+hq_status hq_measure_decode_ceiling(hq_ctx* ctx, const hq_weight* w, int32_t reps, void* stream, double* scalars_per_s) {
+    if (!ctx) return HQ_ERR_INVALID_ARG;
+    if (!w || !scalars_per_s || reps == 0) return fail(ctx, HQ_ERR_INVALID_ARG, "bad argument");
+    if (w->ctx != ctx) return fail(ctx, HQ_ERR_INVALID_ARG, "the weight belongs to another context");
+    if (!linear_uses_e8_fast(w) || w->m < 128) return fail(ctx, HQ_ERR_UNSUPPORTED, "needs an E8 / tile 128 / k <= 3 weight with a full row block");
+    HQ_ENTER(ctx);
+    return launch_decode_ceiling(ctx, w, reps, (cudaStream_t)stream, scalars_per_s);
+}
+
 double hq_alpha(int32_t lattice, double snr_db) {
     if (!valid_lattice(lattice)) return 0.0;
     return sqrt(pow(10.0, snr_db / 10.0) * second_moment(lattice));

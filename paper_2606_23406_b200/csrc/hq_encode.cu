@@ -6,6 +6,7 @@
 // All float arithmetic that decides an integer uses __f*_rn intrinsics (no FMA contraction) in
 // the fixed operation order of docs/FORMAT.md §2.
 #include "hq_common.cuh"
+#include "hq_act.cuh"
 #include "hq_internal.h"
 #include "hq_tc.cuh"
 
@@ -257,12 +258,10 @@ k_act_blob(const void* X, int dtype, int64_t B, int64_t n_kt, int64_t ldx, const
     uint8_t* srow = (uint8_t*)smem + warp * 128;          // one operand row, K order of the operand (e8_kcol)
     const int64_t n_bt = (B + NB - 1) / NB, n_tiles = n_bt * NB * n_kt;
     const uint32_t blob_bytes = (uint32_t)(NB * 128 + NB * 4);
-    const float cn = (float)(1.0 / sqrt(128.0));
     const bool vec = dtype == HQ_BF16 ? ((((uintptr_t)X) | (uintptr_t)(ldx * 2)) & 7) == 0
                                       : ((((uintptr_t)X) | (uintptr_t)(ldx * 4)) & 15) == 0;
     // the four codes of this lane go to operand columns colb + 4j (block l>>1, coordinates 4(l&1) .. +3)
-    const int blk = lane >> 1;
-    const int colb = 32 * (blk >> 2) + 16 * (lane & 1) + (blk & 3);
+    const int colb = act_col0(lane);
     const uint32_t n_kt32 = (uint32_t)n_kt, NB32 = (uint32_t)NB;   // n_tiles < 2^32 (see launch_act_blob)
     // (row, K-tile) of the tile advances by the grid stride without a division per tile
     const uint32_t stride = gridDim.x * (uint32_t)QW_WARPS;
@@ -277,7 +276,8 @@ k_act_blob(const void* X, int dtype, int64_t B, int64_t n_kt, int64_t ldx, const
         const int bb = (int)(b32 - (uint32_t)bt * NB32);
         uint8_t* blob = bblob + (bt * n_kt + kt) * (int64_t)blob_bytes;
         float x[4] = {0.0f, 0.0f, 0.0f, 0.0f};
-        float amax = 0.0f;
+        int qv4[4] = {0, 0, 0, 0};
+        float sx = 0.0f;
         if (b < B) {
             const int64_t base = b * ldx + kt * 128 + 4 * lane;
             if (vec && dtype == HQ_BF16) {
@@ -295,48 +295,15 @@ k_act_blob(const void* X, int dtype, int64_t B, int64_t n_kt, int64_t ldx, const
 #pragma unroll
             for (int j = 0; j < 4; ++j)
                 if ((sg >> (8 * j)) & 0x80u) x[j] = -x[j];
-            {   // strides 1 and 2: inside the lane
-                float a = x[0], c = x[1];
-                x[0] = __fadd_rn(a, c); x[1] = __fsub_rn(a, c);
-                a = x[2]; c = x[3];
-                x[2] = __fadd_rn(a, c); x[3] = __fsub_rn(a, c);
-                a = x[0]; c = x[2];
-                x[0] = __fadd_rn(a, c); x[2] = __fsub_rn(a, c);
-                a = x[1]; c = x[3];
-                x[1] = __fadd_rn(a, c); x[3] = __fsub_rn(a, c);
-            }
-#pragma unroll
-            for (int m = 1; m < 32; m <<= 1) {   // strides 4 .. 64: lane ^ m holds the partner
-                const float sg1 = (lane & m) ? -1.0f : 1.0f;   // upper index of the pair: a - b = o - x, else x + o
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    const float o = __shfl_xor_sync(0xffffffffu, x[j], m);
-                    x[j] = __fmaf_rn(x[j], sg1, o);            // the product is exact: one rounding, that of the sum
-                }
-            }
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                x[j] = __fmul_rn(x[j], cn);
-                amax = fmaxf(amax, fabsf(x[j]));
-            }
-            for (int sft = 16; sft; sft >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, sft));
+            sx = warp_act_tile128(x, lane, qv4);
         }
-        const float inv = (amax == 0.0f) ? 0.0f : __fdiv_rn(127.0f, amax);
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            int qv = 0;
-            if (amax != 0.0f) {
-                float v = rintf(__fmul_rn(x[j], inv));
-                v = fminf(fmaxf(v, -127.0f), 127.0f);
-                qv = (int)v;
-            }
-            srow[colb + 4 * j] = (uint8_t)(int8_t)qv;
-        }
+        for (int j = 0; j < 4; ++j) srow[colb + 4 * j] = (uint8_t)(int8_t)qv4[j];
         __syncwarp();
         // one coalesced 128-byte row: lane l owns operand columns 4l .. 4l+3 = 16-byte chunk l>>2 (swizzled), word l&3
         const uint32_t w4 = ((const uint32_t*)srow)[lane];
         *(uint32_t*)(blob + (bb >> 3) * 1024 + (bb & 7) * 128 + ((((lane >> 2) ^ (bb & 7)) << 4) | ((lane & 3) << 2))) = w4;
-        if (lane == 0) ((float*)(blob + NB * 128))[bb] = (amax == 0.0f) ? 0.0f : __fdiv_rn(amax, 127.0f);
+        if (lane == 0) ((float*)(blob + NB * 128))[bb] = sx;
         __syncwarp();
     }
 }

@@ -146,6 +146,7 @@ hq_status launch_linear_group(hq_ctx* ctx, const hq_weight* const* ws, int n_w, 
                               int64_t ldx, void* const* ys_bf16, const int64_t* ldys, float* const* ys_f32,
                               int32_t* acc_i32, uint8_t* wsbuf, cudaStream_t st);
 bool linear_uses_e8_fast(const hq_weight* w);
+hq_status launch_decode_ceiling(hq_ctx* ctx, const hq_weight* w, int reps, cudaStream_t st, double* scalars_per_s);
 
 // ---- KV decode + attend (hq_attend.cu) ----
 void launch_kv_decode_int8(const hq_kv* kv, int role, int64_t t0, int64_t n, int8_t* codes, cudaStream_t st);

@@ -10,6 +10,8 @@
 #include "hq_internal.h"
 #include "hq_linear_e8.cuh"
 #include "hq_linear_large.cuh"
+#include "hq_e8_ceiling.cuh"
+#include "hq_gemv_e8.cuh"
 #include "hq_tc.cuh"
 
 namespace hq {
@@ -289,7 +291,34 @@ static hq_status launch_e8_v(hq_ctx* ctx, int k0, E8Params& p, const E8Plan& pl,
     return HQ_OK;
 }
 
+// batch 1: k_gemv_e8 (decoded rows through tensor memory, independent warps, activations quantized in-kernel)
+constexpr int GV_NWG = 5;   // measured: 4 .. 8 warp groups run the big launches within 5 %, 5 is the best whole layer
+template <int NWG>
+static hq_status launch_gemv(hq_ctx* ctx, int k0, E8Params& p, const E8Plan& pl, cudaStream_t st) {
+    const size_t smem = gv_smem_bytes<NWG>(p.n_kt);
+    dim3 grid((unsigned)ctx->sm_count);   // flat partition of the items over all warp groups of the device
+#define HQ_LG(KK)                                                                                                   \
+    case KK:                                                                                                        \
+        HQ_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_gemv_e8<KK, NWG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+        HQ_CUDA_CHECK(ctx, launch_pdl(k_gemv_e8<KK, NWG>, grid, dim3(NWG * 128), smem, st, p));                      \
+        break
+    switch (k0) {
+        HQ_LG(0); HQ_LG(1); HQ_LG(2); HQ_LG(3);
+    }
+#undef HQ_LG
+    HQ_CUDA_CHECK(ctx, cudaGetLastError());
+    return HQ_OK;
+}
+
 static size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
+// partial-sum slots per row block of the batch-1 kernel: the segments a row block's K range can be cut into by the flat
+// tile partition over G warp groups (hq_gemv_e8.cuh); sized for the largest G the launcher may use
+static int64_t gv_slots(const hq_ctx* ctx, int64_t n_rb_total, int64_t n_kt) {
+    const int64_t T = n_rb_total * n_kt, G = (int64_t)ctx->sm_count * GV_NWG;
+    const int64_t per = T / G > 0 ? T / G : 1;
+    const int64_t s = (n_kt + per - 1) / per + 1;
+    return s < n_kt + 1 ? s : n_kt + 1;
+}
 
 // weights that may share one launch: the E8 fast path, same n_in / k / seed (= same RHT signs) / operating point
 bool linear_group_compatible(const hq_weight* const* ws, int n_w) {
@@ -308,8 +337,9 @@ size_t linear_group_workspace_bytes(const hq_ctx* ctx, const hq_weight* const* w
     for (int i = 0; i < n_w; ++i) n_rb += ws[i]->n_rb;
     E8Plan pl = e8_plan(ctx, n_rb, ws[0]->n_kt, ws[0]->n_in, B);
     size_t bytes = align256((size_t)pl.n_bt * ws[0]->n_kt * e8_bblob_bytes(pl.NB));
-    if (pl.n_split > 1)
-        for (int i = 0; i < n_w; ++i) bytes += align256((size_t)pl.n_split * B * ws[i]->m * 4);
+    const int64_t slots = B == 1 ? gv_slots(ctx, n_rb, ws[0]->n_kt) : 0;
+    if (pl.n_split > 1 || B == 1)
+        for (int i = 0; i < n_w; ++i) bytes += align256((size_t)(slots > pl.n_split ? slots : pl.n_split) * B * ws[i]->m * 4);
     if (B >= LG_MIN_B) {   // the large-M path: activation blob of 256-row tiles + the decoded copy of the largest weight
         int64_t rb_max = 0;
         for (int i = 0; i < n_w; ++i) rb_max = ws[i]->n_rb > rb_max ? ws[i]->n_rb : rb_max;
@@ -393,8 +423,11 @@ hq_status launch_linear_group(hq_ctx* ctx, const hq_weight* const* ws, int n_w, 
     if (w0->n_kt >= 4096 || pl.n_bt >= 4096 || pl.n_split >= 4096) { ctx->err = "n_in / n_tile and batch tiles must be below 4096 on the fused path"; return HQ_ERR_SHAPE; }
     uint8_t* bblob = wsbuf;
     uint8_t* at = wsbuf + align256((size_t)pl.n_bt * w0->n_kt * e8_bblob_bytes(pl.NB));
-    launch_act_blob(x, dtype, B, w0->n_in, ldx, w0->dsign, pl.NB, bblob, st);
-    HQ_CUDA_CHECK(ctx, cudaGetLastError());
+    const bool gemv = B == 1 && w0->n_kt <= GV_MAX_KT;   // the batch-1 kernel quantizes x itself
+    if (!gemv) {
+        launch_act_blob(x, dtype, B, w0->n_in, ldx, w0->dsign, pl.NB, bblob, st);
+        HQ_CUDA_CHECK(ctx, cudaGetLastError());
+    }
     E8Params p;
     memset(&p, 0, sizeof(p));
     uint32_t min_ulen = 0xffffffffu;
@@ -402,7 +435,8 @@ hq_status launch_linear_group(hq_ctx* ctx, const hq_weight* const* ws, int n_w, 
     for (int i = 0; i < n_w; ++i) {
         p.blob[i] = ws[i]->blob; p.sub_off[i] = ws[i]->group_off; p.m[i] = ws[i]->m;
         p.partials[i] = (float*)at;
-        if (pl.n_split > 1) at += align256((size_t)pl.n_split * B * ws[i]->m * 4);
+        const int64_t slots = B == 1 ? gv_slots(ctx, n_rb, w0->n_kt) : 0;
+        if (pl.n_split > 1 || B == 1) at += align256((size_t)(slots > pl.n_split ? slots : pl.n_split) * B * ws[i]->m * 4);
         p.inv_A[i] = (float)(1.0 / (ws[i]->alpha * sqrt((double)ws[i]->n)));
         p.rb_base[i + 1] = p.rb_base[i] + (int)ws[i]->n_rb;
         if (ws[i]->min_ulen < min_ulen) min_ulen = ws[i]->min_ulen;
@@ -426,13 +460,16 @@ hq_status launch_linear_group(hq_ctx* ctx, const hq_weight* const* ws, int n_w, 
     p.n_kt = (int)w0->n_kt; p.n_split = pl.n_split; p.L = pl.L; p.n_items = pl.n_items; p.n_bt = pl.n_bt;
     p.u_dense = ((min_ulen + 31) >> 5) >= (uint32_t)E8_DENSE ? E8_DENSE : 0;
     p.bblob = bblob; p.B = B; p.acc_i32 = (n_w == 1) ? acc_i32 : nullptr;
+    p.x = x; p.dtype = dtype; p.dsign = w0->dsign;
+    if (gemv) p.n_items = (int)(n_rb * w0->n_kt);   // the batch-1 kernel partitions tiles, not items
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     if (ctx->prof) {
         HQ_CUDA_CHECK(ctx, cudaEventCreate(&e0));
         HQ_CUDA_CHECK(ctx, cudaEventCreate(&e1));
         HQ_CUDA_CHECK(ctx, cudaEventRecord(e0, st));
     }
-    hq_status s = (B == 1)    ? launch_e8_v<16, 1, 6, 1>(ctx, w0->k0, p, pl, st)
+    hq_status s = gemv        ? launch_gemv<GV_NWG>(ctx, w0->k0, p, pl, st)
+                  : (B == 1)  ? launch_e8_v<16, 1, 6, 1>(ctx, w0->k0, p, pl, st)
                   : (B <= 16) ? launch_e8_v<16, 16, 5, 1>(ctx, w0->k0, p, pl, st)
                               : launch_e8_v<64, 64, 3, 1>(ctx, w0->k0, p, pl, st);
     if (s != HQ_OK) return s;
@@ -442,6 +479,43 @@ hq_status launch_linear_group(hq_ctx* ctx, const hq_weight* const* ws, int n_w, 
         ctx->prof_ev.push_back(e1);
     }
     return HQ_OK;
+}
+
+// decode-only ceiling measurement (hq_e8_ceiling.cuh)
+template <int NWG>
+static hq_status decode_ceiling_nwg(hq_ctx* ctx, const hq_weight* w, int reps, cudaStream_t st, double* scalars_per_s) {
+    E8CeilParams p;
+    p.blob = w->blob; p.sub_off = w->group_off; p.lut = ctx->e8_lut; p.n_groups = 4 * w->G; p.reps = reps;
+    const size_t threads = (size_t)ctx->sm_count * NWG * 128;
+    p.sink = (unsigned int*)ctx->alloc.alloc(ctx->alloc.user, threads * 4);
+    if (!p.sink) { ctx->err = "allocator returned NULL"; return HQ_ERR_ALLOC; }
+    const size_t smem = 1024 + E8_LUT_BYTES + (size_t)NWG * (16384 + 128 * E8_SCR_STRIDE * 4);
+    cudaEvent_t e0, e1;
+    HQ_CUDA_CHECK(ctx, cudaEventCreate(&e0));
+    HQ_CUDA_CHECK(ctx, cudaEventCreate(&e1));
+    float ms = 0.0f;
+#define HQ_CE(KK)                                                                                                       \
+    case KK:                                                                                                            \
+        HQ_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_e8_decode_ceiling<KK, NWG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+        p.reps = 2; k_e8_decode_ceiling<KK, NWG><<<ctx->sm_count, NWG * 128, smem, st>>>(p);   /* warm-up */                \
+        p.reps = reps;                                                                                                  \
+        HQ_CUDA_CHECK(ctx, cudaEventRecord(e0, st));                                                                    \
+        k_e8_decode_ceiling<KK, NWG><<<ctx->sm_count, NWG * 128, smem, st>>>(p);                                        \
+        HQ_CUDA_CHECK(ctx, cudaEventRecord(e1, st));                                                                    \
+        break
+    switch (w->k0) { HQ_CE(0); HQ_CE(1); HQ_CE(2); HQ_CE(3); }
+#undef HQ_CE
+    HQ_CUDA_CHECK(ctx, cudaGetLastError());
+    HQ_CUDA_CHECK(ctx, cudaEventSynchronize(e1));
+    HQ_CUDA_CHECK(ctx, cudaEventElapsedTime(&ms, e0, e1));
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    ctx->alloc.free(ctx->alloc.user, p.sink);
+    *scalars_per_s = (double)threads * 128.0 * reps / (ms * 1e-3);
+    return HQ_OK;
+}
+// reps < 0: |reps| repetitions with 4 warp groups (16 warps per SM) instead of the fused kernel's 6
+hq_status launch_decode_ceiling(hq_ctx* ctx, const hq_weight* w, int reps, cudaStream_t st, double* scalars_per_s) {
+    return reps > 0 ? decode_ceiling_nwg<6>(ctx, w, reps, st, scalars_per_s) : decode_ceiling_nwg<4>(ctx, w, -reps, st, scalars_per_s);
 }
 
 hq_status launch_linear(hq_ctx* ctx, const hq_weight* w, const void* x, int dtype, int64_t B, int64_t ldx,

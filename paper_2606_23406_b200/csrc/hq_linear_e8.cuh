@@ -63,6 +63,10 @@ struct E8Params {
     const uint8_t* bblob;       // [n_bt][n_kt][e8_bblob_bytes(NB)]
     int64_t B;
     int32_t* acc_i32;           // [n_kt][B][m] or null (single weight only)
+    // batch 1 (k_gemv_e8, hq_gemv_e8.cuh): the kernel quantizes the activation vector itself
+    const void* x;              // [n_in] bf16 or f32
+    int dtype;
+    const int8_t* dsign;        // [n_in] RHT signs
 };
 
 // Tile descriptor, three registers; the stream of tiles of one warp group is advanced without divisions.

