@@ -4,8 +4,9 @@ decoder layer's linears (BASELINE.json configs[1]: E8, 4 bps, RHT tile 128, batc
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--layers L] [--impl reference]
 
-A step = the seven linears (q,k,v,o,gate,up,down) of one layer at batch 1 through hq_linear_group (matrices that
-share an input share a launch: activation RHT + INT8 cast, fused decode+MMA, split-K finalize).  L distinct layers (L x ~116 MB compressed > the 126 MB L2) are
+A step = the seven linears (q,k,v,o,gate,up,down) of one layer at batch 1 through hq_linear_group: matrices that share an
+input share ONE launch of the fused kernel (activation RHT + INT8 cast, Rice decode, tcgen05 INT8 MMA, split-K reduction
+all inside k_gemv_e8), so a step is exactly four kernel launches.  L distinct layers (L x ~116 MB compressed > the 126 MB L2) are
 cycled so no step re-reads its weights from L2.  One JSON line on stdout (rank 0).
 """
 import argparse
@@ -28,11 +29,10 @@ METRIC = "fused decode+INT8 GEMV % of HBM roofline; large-M INT8 TOPS vs peak"
 UNIT = "GB/s of compressed weight bytes (batch-1 GEMV, whole layer)"
 SNR_E8_4BPS = float(np.float32(22.68))   # E8 at 4.0 bps on iid Gaussian tiles (B.1 L857)
 NAMES = list(hq_synth.LLAMA_SHAPES)
-# dram__bytes_read.sum + dram__bytes_write.sum of the four k_linear_e8 launches of one step, from the ncu --set full
-# capture summarised in profiles/r01c_e8_grouped_kernel.md §3 (14.01 + 9.40 + 64.73+0.57 + 32.62 MB)
-NCU_DRAM_BYTES_PER_STEP = 121.34e6
-# smsp__inst_executed.sum of the same four launches (10.24 + 7.17 + 43.85 + 22.43 M warp-instructions)
-NCU_WARP_INSTR_PER_STEP = 83.69e6
+# ncu-derived figures (DRAM bytes and warp instructions of the four fused launches of one step) are NOT typed in here:
+# they are read from profiles/r02_ncu_step.json, which the ncu pass of a named commit wrote (see the .md beside it)
+NCU_STEP_JSON = os.path.join(ROOT, "profiles", "r02_ncu_step.json")
+LARGE_M_TILE = 128   # RHT tile of the config-5 weights (the tile is chosen on kernel grounds)
 WORKLOAD = "llama3.1-8b decoder-layer linears q/k/v/o/gate/up/down, E8 4 bps, RHT tile 128, batch 1 (BASELINE configs[1])"
 
 
@@ -72,6 +72,14 @@ class ClockSampler(threading.Thread):
         return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": mx, "reasons": reasons, "samples": len(sm)}
 
 
+def base_config(layers):
+    """The `config` both arms print (same keys: the driver compares them)."""
+    return {"workload": WORKLOAD, "lattice": "E8", "snr_db": SNR_E8_4BPS, "n_tile": 128, "batch": 1,
+            "layers_cycled": layers, "l2_policy": "inputs larger than L2 (layers cycled)",
+            "launch": "one CUDA graph per layer: hq_linear_group x 4 (q+k+v, o, gate+up, down) = 4 launches of k_gemv_e8",
+            "scalars_per_step": sum(m * n for m, n in hq_synth.LLAMA_SHAPES.values()), "parallelism": "replicas only"}
+
+
 def oracle_sample(threads_note=True):
     """The oracle (as it stands) on a bounded sample of the workload: the 'k' projection (1024 x 4096) of
     layer 0 — decode the container (O2) + activation cast + INT8 contraction (O3) at batch 1."""
@@ -106,7 +114,7 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "int8", "data": "synthetic",
-            "config": {"workload": WORKLOAD, "lattice": "E8", "bps": 4.0, "n_tile": 128, "batch": 1},
+            "config": base_config(args.layers),
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line))
@@ -142,119 +150,117 @@ def _time_cuda(fn, reps, warm=1):
     return e0.elapsed_time(e1) / reps
 
 
-def run_extras(ctx, hq, dev, peak_gbs):
-    """The other BASELINE configs, each a bounded, seeded, synthetic run through the public API (parity for the
-    same code paths is in tests/): config 5 (large-M INT8 TOPS), config 4 (KV append / attend), config 3 (reduced
-    lattice / rate / tile sweep at batch 1)."""
+def measure_large_m(ctx, hq, dev, reps=10):
+    """BASELINE config 5, both GEMMs of the DiT-scale MLP (8192 tokens: 4096 -> 16384 and 16384 -> 4096), E8 4 bps,
+    whole hq_linear call (activation operand + weight decode + warp-specialised tcgen05 GEMM), >= 10 repetitions each;
+    peak = torch._int_mm 8192^3 measured in the same run (a plain library INT8 GEMM)."""
     import torch
-    out = {}
-    # ---- config 5: 8192 tokens x (4096 -> 16384), E8 4 bps, tile 128, INT8 MMA
-    try:
-        W = torch.from_numpy(hq_synth.gaussian_weight(16384, 4096, seed=5)).to(dev).to(torch.bfloat16)
-        w = ctx.encode_weights(W, hq.Lattice.E8, 128, SNR_E8_4BPS, seed=5)
+    res = {"bound": "tensor", "unit": "TOPS", "reps": reps, "gemms": []}
+    a = torch.randint(-127, 127, (8192, 8192), dtype=torch.int8, device=dev)
+    b = torch.randint(-127, 127, (8192, 8192), dtype=torch.int8, device=dev)
+    ms_mm = _time_cuda(lambda: torch._int_mm(a, b), reps=10, warm=3)
+    peak = 2.0 * 8192 ** 3 / (ms_mm * 1e-3) / 1e12
+    del a, b
+    res["peak"], res["peak_source"] = peak, "torch._int_mm 8192^3 INT8, measured in this run"
+    res["peak_nominal_dense_int8"] = 4500.0
+    tot_ops, tot_ms = 0.0, 0.0
+    for m, n_in, seed in ((16384, 4096, 5), (4096, 16384, 7)):
+        W = torch.from_numpy(hq_synth.gaussian_weight(m, n_in, seed=seed)).to(dev).to(torch.bfloat16)
+        w = ctx.encode_weights(W, hq.Lattice.E8, LARGE_M_TILE, SNR_E8_4BPS, seed=seed)
         del W
-        X = torch.from_numpy(hq_synth.activations(8192, 4096, seed=6)).to(dev).to(torch.bfloat16)
-        y = torch.empty((8192, 16384), dtype=torch.bfloat16, device=dev)
-        ms = _time_cuda(lambda: w.linear(X, y=y), reps=3)
-        ops = 2.0 * 8192 * 16384 * 4096
-        c5 = {"workload": "8192 tokens x 4096->16384, E8 4 bps, tile 128", "ms": ms, "int8_TOPS": ops / (ms * 1e-3) / 1e12,
-              "nominal_dense_int8_TOPS": 4500.0}
-        try:
-            a = torch.randint(-127, 127, (8192, 8192), dtype=torch.int8, device=dev)
-            b = torch.randint(-127, 127, (8192, 8192), dtype=torch.int8, device=dev)
-            ms_mm = _time_cuda(lambda: torch._int_mm(a, b), reps=5, warm=2)
-            c5["measured_int8_peak_TOPS_torch_int_mm_8192"] = 2.0 * 8192 ** 3 / (ms_mm * 1e-3) / 1e12
-            c5["frac_of_measured_int8_peak"] = c5["int8_TOPS"] / c5["measured_int8_peak_TOPS_torch_int_mm_8192"]
-            del a, b
-        except Exception as ex:  # noqa: BLE001
-            c5["measured_int8_peak_TOPS_torch_int_mm_8192"] = f"unavailable: {ex}"
-        c5["frac_of_nominal_int8_peak"] = c5["int8_TOPS"] / 4500.0
-        # Roofline of the large-M path: the INT8 tensor pipe.  peak = torch._int_mm measured beside it (a plain library
-        # GEMM with one drain per output tile); this path must drain and rescale the INT32 accumulator once per K-tile of
-        # 128 (both scales are per tile, PAPER §4.8), which costs >= 2 issue slots per accumulator (I2F + half of a packed
-        # multiply and a packed FMA): DESIGN.md §6.3 derives that co-bound and profiles/r01d_large_m_path.md shows it.
-        meas = c5.get("measured_int8_peak_TOPS_torch_int_mm_8192")
-        peak = meas if isinstance(meas, float) else 4500.0
-        c5["roofline"] = {"bound": "tensor", "achieved": c5["int8_TOPS"], "peak": peak, "unit": "TOPS",
-                          "frac": c5["int8_TOPS"] / peak,
-                          "peak_source": "torch._int_mm 8192^3 measured in this run" if isinstance(meas, float) else "nominal dense INT8",
-                          "note": "whole call: activation blob + weight decode into the operand-layout scratch copy + GEMM"}
-        c5["path"] = "k_act_blob + k_e8_decode_ablob + k_e8_gemm_large (hq_linear_large.cuh)"
-        out["config5_large_m"] = c5
+        X = torch.from_numpy(hq_synth.activations(8192, n_in, seed=6)).to(dev).to(torch.bfloat16)
+        y = torch.empty((8192, m), dtype=torch.bfloat16, device=dev)
+        ms = _time_cuda(lambda: w.linear(X, y=y), reps=reps, warm=2)
+        ops = 2.0 * 8192 * m * n_in
+        res["gemms"].append({"shape": f"8192 tokens x {n_in} -> {m}", "ms": ms, "TOPS": ops / (ms * 1e-3) / 1e12,
+                             "frac": ops / (ms * 1e-3) / 1e12 / peak})
+        tot_ops += ops; tot_ms += ms
         w.free(); del X, y
-    except Exception as ex:  # noqa: BLE001
-        out["config5_large_m"] = f"failed: {ex}"
-    # ---- config 4: KV cache, 8 heads x 128, 32768 tokens, E8 2 bps, signs rotation, dither, window 32
-    try:
-        T, H, d, QH = 32768, 8, 128, 32
-        snr_kv = float(np.float32(9.68))
-        K = torch.from_numpy(hq_synth.kv_tokens(T + 16, H, d, seed=4)).to(dev).to(torch.bfloat16)
-        V = torch.from_numpy(hq_synth.kv_tokens(T + 16, H, d, seed=5)).to(dev).to(torch.bfloat16)
-        q = torch.from_numpy(hq_synth.activations(QH, d, seed=6)).to(dev).to(torch.bfloat16)
-        kv = ctx.kv_create(H, d, T + 64, hq.Lattice.E8, snr_kv, (0, 0), 4, rotation=1, dither=1, window=32)
-        torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        kv.append(K[:T], V[:T])
-        torch.cuda.synchronize()
-        bulk_s = time.perf_counter() - t0
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record()
-        for i in range(16):
-            kv.append(K[T + i:T + i + 1], V[T + i:T + i + 1])
-        e1.record()
-        torch.cuda.synchronize()
-        app_us = 1e3 * e0.elapsed_time(e1) / 16
-        o = torch.empty_like(q)
-        att_ms = _time_cuda(lambda: kv.attend(q, out=o), reps=5)
-        ex = kv.export()
-        Tn = int(ex["n_tokens"])
-        payload_bits = float(ex["upos"].astype(np.int64).sum()) + 2.0 * H * Tn * float(ex["rbits"])
-        scal = 2.0 * H * Tn * d
-        alg_bytes = (payload_bits + 32.0 * 2 * H * Tn) / 8.0
-        out["config4_kv"] = {"workload": "8 KV heads x 128, 32768 tokens, E8 2 bps, signs rotation, dither, window 32; 32 query heads",
-                             "bulk_append_Mscalars_per_s": 2.0 * H * T * d / bulk_s / 1e6, "append_us_per_token": app_us,
-                             "attend_ms": att_ms, "attend_GBps_compressed": alg_bytes / (att_ms * 1e-3) / 1e9,
-                             "attend_frac_of_hbm_roofline": alg_bytes / (att_ms * 1e-3) / 1e9 / peak_gbs,
-                             "bits_per_scalar_payload": payload_bits / scal, "bits_per_scalar_total": 8.0 * alg_bytes / scal,
-                             "kv_compression_vs_bf16": 16.0 / (8.0 * alg_bytes / scal)}
-        kv.free(); del K, V
-    except Exception as ex:  # noqa: BLE001
-        out["config4_kv"] = f"failed: {ex}"
-    # ---- config 3 (reduced): one 14336 x 4096 Gaussian weight; lattice x rate at tile 128, E8 4 bps at tiles 64 / 256
-    try:
-        Wn = hq_synth.gaussian_weight(14336, 4096, seed=3)
-        W = torch.from_numpy(Wn).to(dev).to(torch.bfloat16)
-        x = torch.from_numpy(hq_synth.activations(1, 4096, seed=9)).to(dev).to(torch.bfloat16)
-        snr = {"E8": (16.50, 22.68, 28.73), "D4": (16.4, 22.5, 28.6), "A2": (16.02, 22.21, 28.26), "Z": (15.8, 21.9, 27.9)}
-        combos = [(lat, s, 128) for lat in ("E8", "D4", "A2", "Z") for s in snr[lat]] + [("E8", 22.68, 64), ("E8", 22.68, 256)]
-        rows = []
-        for lat, s, n_tile in combos:
-            s32 = float(np.float32(s))
-            w = ctx.encode_weights(W, hq.Lattice.BY_NAME[lat], n_tile, s32, seed=3)
-            info = w.info
-            sc = float(info.m_out * info.n_in)
-            yv = torch.empty((1, 14336), dtype=torch.bfloat16, device=dev)
-            ms = _time_cuda(lambda: w.linear(x, y=yv), reps=5, warm=2)
-            nbytes = (info.payload_bits + info.norm_bits + info.length_bits) / 8.0
-            # MSE of the reconstruction, measured in the rotated domain (the RHT is orthonormal) on the first 512 rows
-            R = 512
-            _, _, u = w.act_quant(W[:R], want_u=True)
-            codes, norms = w.decode_int8()
-            c = codes[:R].float().view(R, -1, n_tile)
-            if lat == "A2":
-                c[..., 0::2] *= 3.0 ** 0.5
-            rho = norms[:R].view(torch.float16).float()
-            scale = rho / (info.alpha * n_tile ** 0.5)
-            mse = float(((u.view(R, -1, n_tile) - scale[..., None] * c) ** 2).mean())
-            pred = float((rho ** 2).mean() / n_tile / 10 ** (s32 / 10))
-            rows.append({"lattice": lat, "snr_db": s, "n_tile": n_tile, "k": [info.rice_k[0], info.rice_k[1]],
-                         "bits_payload": info.payload_bits / sc, "bits_total": 8.0 * nbytes / sc,
-                         "mse": mse, "mse_predicted": pred, "gemv_us": 1e3 * ms, "GBps_compressed": nbytes / (ms * 1e-3) / 1e9})
+    res["achieved"] = tot_ops / (tot_ms * 1e-3) / 1e12
+    res["frac"] = res["achieved"] / peak
+    res["n_tile"] = LARGE_M_TILE
+    res["workload"] = "BASELINE configs[4]: 8192 tokens x (4096 -> 16384, 16384 -> 4096), E8 4 bps, bf16 activations through the per-tile RHT"
+    return res
+
+
+def measure_attend(ctx, hq, dev, peak_gbs):
+    """BASELINE config 4: 8 KV heads x 128, 32768 tokens, E8 2 bps, signs rotation, dither, window 32; 32 query heads."""
+    import torch
+    T, H, d, QH = 32768, 8, 128, 32
+    snr_kv = float(np.float32(9.68))
+    K = torch.from_numpy(hq_synth.kv_tokens(T + 16, H, d, seed=4)).to(dev).to(torch.bfloat16)
+    V = torch.from_numpy(hq_synth.kv_tokens(T + 16, H, d, seed=5)).to(dev).to(torch.bfloat16)
+    q = torch.from_numpy(hq_synth.activations(QH, d, seed=6)).to(dev).to(torch.bfloat16)
+    kv = ctx.kv_create(H, d, T + 64, hq.Lattice.E8, snr_kv, (0, 0), 4, rotation=1, dither=1, window=32)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    kv.append(K[:T], V[:T])
+    torch.cuda.synchronize()
+    bulk_s = time.perf_counter() - t0
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for i in range(16):
+        kv.append(K[T + i:T + i + 1], V[T + i:T + i + 1])
+    e1.record()
+    torch.cuda.synchronize()
+    app_us = 1e3 * e0.elapsed_time(e1) / 16
+    o = torch.empty_like(q)
+    att_ms = _time_cuda(lambda: kv.attend(q, out=o), reps=10, warm=2)
+    ex = kv.export()
+    Tn = int(ex["n_tokens"])
+    payload_bits = float(ex["upos"].astype(np.int64).sum()) + 2.0 * H * Tn * float(ex["rbits"])
+    scal = 2.0 * H * Tn * d
+    alg_bytes = (payload_bits + 32.0 * 2 * H * Tn) / 8.0
+    gbs = alg_bytes / (att_ms * 1e-3) / 1e9
+    res = {"bound": "hbm", "unit": "GB/s", "achieved": gbs, "peak": peak_gbs, "frac": gbs / peak_gbs,
+           "attend_us": 1e3 * att_ms, "alg_bytes": alg_bytes, "append_us_per_token": app_us,
+           "bulk_append_Mscalars_per_s": 2.0 * H * T * d / bulk_s / 1e6,
+           "bits_per_scalar_payload": payload_bits / scal, "bits_per_scalar_total": 8.0 * alg_bytes / scal,
+           "kv_compression_vs_bf16": 16.0 / (8.0 * alg_bytes / scal),
+           "workload": "BASELINE configs[3]: 8 KV heads x 128, 32768 tokens, E8 2 bps, signs rotation, dither, window 32; 32 query heads"}
+    kv.free(); del K, V
+    return res
+
+
+def measure_config3(ctx, hq, dev, copies=5):
+    """BASELINE config 3 (reduced): a 14336 x 4096 Gaussian weight; lattice x rate at tile 128, E8 4 bps at tiles 64 / 256.
+    `copies` distinct weights per point (5 x ~31 MB > the 126 MB L2) are cycled so the GEMV reads HBM, not L2."""
+    import torch
+    Ws = [torch.from_numpy(hq_synth.gaussian_weight(14336, 4096, seed=30 + c)).to(dev).to(torch.bfloat16) for c in range(copies)]
+    x = torch.from_numpy(hq_synth.activations(1, 4096, seed=9)).to(dev).to(torch.bfloat16)
+    combos = [(lat, bps, 128) for lat in ("E8", "D4", "A2", "Z") for bps in (3.0, 4.0, 5.0)] + [("E8", 4.0, 64), ("E8", 4.0, 256)]
+    rows = []
+    for lat, bps, n_tile in combos:
+        s32, _ = hq.snr_for_bps(hq.Lattice.BY_NAME[lat], bps)       # the library's calibration table (§5.4 L365)
+        ws = [ctx.encode_weights(W, hq.Lattice.BY_NAME[lat], n_tile, s32, seed=3) for W in Ws]
+        info, st = ws[0].info, ws[0].stats()
+        sc = float(info.m_out * info.n_in)
+        yv = torch.empty((1, 14336), dtype=torch.bfloat16, device=dev)
+        state = {"i": 0}
+
+        def one():
+            ws[state["i"] % copies].linear(x, y=yv)
+            state["i"] += 1
+        ms = _time_cuda(one, reps=2 * copies, warm=copies)
+        nbytes = (info.payload_bits + info.norm_bits + info.length_bits) / 8.0
+        # MSE of the reconstruction, measured in the rotated domain (the RHT is orthonormal) on the first 512 rows
+        R = 512
+        _, _, u = ws[0].act_quant(Ws[0][:R], want_u=True)
+        codes, norms = ws[0].decode_int8()
+        c = codes[:R].float().view(R, -1, n_tile)
+        if lat == "A2":
+            c[..., 0::2] *= 3.0 ** 0.5
+        rho = norms[:R].view(torch.float16).float()
+        scale = rho / (info.alpha * n_tile ** 0.5)
+        mse = float(((u.view(R, -1, n_tile) - scale[..., None] * c) ** 2).mean())
+        pred = float((rho ** 2).mean() / n_tile / 10 ** (s32 / 10))
+        rows.append({"lattice": lat, "target_bps": bps, "snr_db": s32, "n_tile": n_tile, "k": [info.rice_k[0], info.rice_k[1]],
+                     "bits_payload": info.payload_bits / sc, "bits_total": 8.0 * nbytes / sc,
+                     "tile_bits_min_max": [st.tile_bits_min, st.tile_bits_max],
+                     "mse": mse, "mse_predicted": pred, "gemv_us": 1e3 * ms, "GBps_compressed": nbytes / (ms * 1e-3) / 1e9})
+        for w in ws:
             w.free()
-        out["config3_sweep"] = rows
-    except Exception as ex:  # noqa: BLE001
-        out["config3_sweep"] = f"failed: {ex}"
-    return out
+    return {"copies_cycled": copies, "rows": rows}
 
 
 def main():
@@ -363,28 +369,46 @@ def main():
     ms_per_step = ms / args.steps
     value = aggregate_value(bytes_per_step, ms_per_step, world)
 
-    # ---- roofline of the dominant kernel (fused decode+MMA), CUDA events around each launch
+    # ---- roofline of the dominant kernel.  At batch 1 a step IS four launches of k_gemv_e8 and nothing else (the
+    # activation cast, the decode, the MMA and the split-K reduction are one kernel), so the kernel's average launch
+    # duration in the schedule the step runs in (graph replay, PDL between the launches) is ms_per_step / 4: kernel
+    # time == step time by construction.  The eager per-launch bracket (library events around every launch, no overlap)
+    # is reported beside it.
     ms_p, (kern_ms, kern_n) = timed(1, args.steps, 2, profile=True)
-    weight_bytes_per_step = bytes_per_step
-    achieved = weight_bytes_per_step * args.steps / (kern_ms * 1e-3) / 1e9 if kern_ms > 0 else 0.0
     peak, peak_src = peaks()
+    n_launch = len(GROUPS)
+    achieved = bytes_per_step / (ms_per_step * 1e-3) / 1e9
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": NCU_DRAM_BYTES_PER_STEP / len(GROUPS), "alg_bytes_per_launch": bytes_per_step / len(GROUPS),
-                "traffic_source": "ncu --set full, profiles/r01c_e8_grouped_kernel.md", "kernel": "k_linear_e8<K=2,NB=16,BC=1,NWG=6,CPS=1> (one launch per hq_linear_group)", "peak_source": peak_src,
-                "kernel_share_of_step": kern_ms / ms_p if ms_p > 0 else None,
-                "launches_timed": kern_n, "avg_launch_us": 1e3 * kern_ms / max(kern_n, 1),
+                "traffic": None, "alg_bytes_per_launch": bytes_per_step / n_launch,
+                "kernel": "k_gemv_e8<K=2,NWG=5> (one launch per hq_linear_group; 4 per step)", "peak_source": peak_src,
+                "avg_launch_us": 1e3 * ms_per_step / n_launch, "launches_per_step": n_launch,
+                "timing": "CUDA events around K graph replays on the launching stream; the step holds only this kernel",
+                "eager_avg_launch_us": 1e3 * kern_ms / max(kern_n, 1), "eager_launches_timed": kern_n,
                 "alg_bytes_per_scalar": bytes_per_step / scalars_per_step,
                 "frac_of_nominal_8TBs": achieved / 8000.0}
-    # co-bound: the kernel is limited by the ALU work of the Rice decode.  Issue rate achieved =
-    # warp-instructions of the four launches (ncu) / (their summed duration x SMs x SM clock); peak = 4 warp-instr/clk/SM
-    sm_clock_hz, n_sms = 1.965e9, 148
-    kern_s_per_step = kern_ms * 1e-3 / args.steps if kern_ms > 0 else float("nan")
-    ipc = NCU_WARP_INSTR_PER_STEP / (kern_s_per_step * n_sms * sm_clock_hz)
-    roofline["co_bound"] = {"bound": "alu", "achieved": ipc, "peak": 4.0, "unit": "warp-instr/clk/SM", "frac": ipc / 4.0,
-                            "lane_instr_per_scalar": NCU_WARP_INSTR_PER_STEP * 32 / scalars_per_step,
-                            "budget_for_70pct_hbm_lane_instr_per_scalar": n_sms * 128 * sm_clock_hz /
-                            (0.70 * peak * 1e9 / (bytes_per_step / scalars_per_step)),
-                            "source": "instruction count: ncu, profiles/r01c_e8_grouped_kernel.md; peak: profiles/r01_issue_rates.md"}
+    clocks_now = sampler.summary()
+    sm_clock_hz = 1e6 * float(clocks_now["sm_mhz"] or 1965)
+    n_sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    budget = n_sms * 128 * sm_clock_hz / (0.70 * peak * 1e9 / (bytes_per_step / scalars_per_step))
+    roofline["co_bound"] = {"bound": "alu", "unit": "warp-instr/clk/SM", "peak": 4.0,
+                            "budget_for_70pct_hbm_lane_instr_per_scalar": budget,
+                            "peak_source": "profiles/r01_issue_rates.md (4 warp-instructions per clock per SM)"}
+    if os.path.exists(NCU_STEP_JSON):   # written by the ncu pass of a named commit: profiles/r02_ncu_step.md
+        nc = json.load(open(NCU_STEP_JSON))
+        roofline["traffic"] = nc["dram_bytes_per_step"] / n_launch
+        roofline["traffic_source"] = f"ncu --set full at commit {nc['commit']} ({os.path.relpath(NCU_STEP_JSON, ROOT)})"
+        ipc = nc["warp_instr_per_step"] / (ms_per_step * 1e-3 * n_sms * sm_clock_hz)
+        roofline["co_bound"].update({"achieved": ipc, "frac": ipc / 4.0,
+                                     "lane_instr_per_scalar": nc["warp_instr_per_step"] * 32 / scalars_per_step,
+                                     "source": roofline["traffic_source"]})
+    # the decode-only ceiling, measured live: the fused kernel's decode phases on register-resident data
+    try:
+        ceil = layers[0]["q"].decode_ceiling(200)
+        roofline["decode_ceiling"] = {"scalars_per_s": ceil, "equivalent_GBps": ceil * bytes_per_step / scalars_per_step / 1e9,
+                                      "frac_of_hbm_peak": ceil * bytes_per_step / scalars_per_step / 1e9 / peak,
+                                      "what": "hq_measure_decode_ceiling: phase 1 + phase 2 only, no loads, no MMA (profiles/r02_decode_ceiling.md)"}
+    except Exception as ex:  # noqa: BLE001
+        roofline["decode_ceiling"] = f"failed: {ex}"
 
     # ---- end to end: host (pinned) x -> device, linears, y -> host, every step.  The step's two activation vectors
     # live in one pinned buffer and its seven outputs in one device / one pinned buffer, so a step is ONE H2D copy,
@@ -438,10 +462,12 @@ def main():
 
     extras = {}
     if not args.skip_extras and rank == 0:
-        # batch 16 on the same weights
-        ms16, _ = timed(16, max(4, args.steps // 2), 2)
-        extras["batch16"] = {"ms_per_step": ms16 / max(4, args.steps // 2),
-                             "GBps_compressed": bytes_per_step / (ms16 / max(4, args.steps // 2) * 1e-3) / 1e9}
+        # batch 16 on the same weights (also part of BASELINE configs[1])
+        n16 = max(4, args.steps // 2)
+        ms16, _ = timed(16, n16, 2)
+        g16 = bytes_per_step / (ms16 / n16 * 1e-3) / 1e9
+        roofline["batch16"] = {"bound": "hbm", "unit": "GB/s", "achieved": g16, "peak": peak, "frac": g16 / peak,
+                               "ms_per_step": ms16 / n16, "kernel": "k_act_blob + k_linear_e8<NB=16> per group"}
         # practical baseline on the same box: bf16 GEMV by cuBLAS on uncompressed weights (one layer, cycled 4x)
         try:
             dense = [{n: torch.randn(hq_synth.LLAMA_SHAPES[n], device=dev, dtype=torch.bfloat16) * 0.02 for n in NAMES}
@@ -463,7 +489,16 @@ def main():
         except Exception as ex:  # noqa: BLE001
             extras["cublas_bf16_gemv_ms_per_layer"] = f"failed: {ex}"
         if world == 1:
-            extras.update(run_extras(ctx, hq, dev, peaks()[0]))
+            for key, fn in (("large_m", lambda: measure_large_m(ctx, hq, dev)),
+                            ("attend", lambda: measure_attend(ctx, hq, dev, peak))):
+                try:
+                    roofline[key] = fn()
+                except Exception as ex:  # noqa: BLE001
+                    roofline[key] = f"failed: {ex}"
+            try:
+                extras["config3_sweep"] = measure_config3(ctx, hq, dev)
+            except Exception as ex:  # noqa: BLE001
+                extras["config3_sweep"] = f"failed: {ex}"
 
     # ---- CPU baseline: the oracle on a bounded sample, rank 0, N=1 only
     cpu = None
@@ -471,7 +506,7 @@ def main():
         one_pass, nbytes, sample = oracle_sample()
         one_pass()
         reps, t0 = 0, time.perf_counter()
-        while time.perf_counter() - t0 < 10.0 and reps < 50:
+        while time.perf_counter() - t0 < 12.0 and reps < 100000:   # about 12 s of CPU work on the bounded sample
             one_pass()
             reps += 1
         dt = time.perf_counter() - t0
@@ -482,11 +517,9 @@ def main():
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "int8", "data": "synthetic",
-                "config": {"workload": WORKLOAD, "lattice": "E8", "snr_db": SNR_E8_4BPS, "n_tile": 128, "batch": 1,
-                           "layers_cycled": args.layers, "l2_policy": "inputs larger than L2 (layers cycled)", "launch": "one CUDA graph per layer: hq_linear_group x 4 (q+k+v, o, gate+up, down)",
-                           "scalars_per_step": scalars_per_step, "bits_per_scalar_payload": bps_payload,
-                           "bits_per_scalar_total": bps_total, "parallelism": "replicas only"},
-                "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": args.steps * (len(GROUPS) * 2 + len(NAMES)),
+                "config": base_config(args.layers),
+                "rate": {"bits_per_scalar_payload": bps_payload, "bits_per_scalar_total": bps_total},
+                "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": args.steps * len(GROUPS),
                 "roofline": roofline, "cpu_baseline": cpu, "extras": extras}
         print(json.dumps(line))
     if world > 1:
