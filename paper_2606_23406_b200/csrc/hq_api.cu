@@ -82,12 +82,22 @@ hq_status hq_create(hq_ctx** out, const hq_allocator* alloc, int cuda_device) {
         delete ctx;
         return HQ_ERR_CUDA;
     }
+    if (cudaStreamCreateWithFlags(&ctx->side, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming) != cudaSuccess) {
+        ctx_free(ctx, ctx->e8_lut);
+        delete ctx;
+        return HQ_ERR_CUDA;
+    }
     *out = ctx;
     return HQ_OK;
 }
 
 void hq_destroy(hq_ctx* ctx) {
     if (!ctx) return;
+    if (ctx->side) cudaStreamDestroy(ctx->side);
+    if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
+    if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
     ctx_free(ctx, ctx->ws);
     ctx_free(ctx, ctx->e8_lut);
     ctx_free(ctx, ctx->e8_cnt);

@@ -308,6 +308,111 @@ k_act_blob(const void* X, int dtype, int64_t B, int64_t n_kt, int64_t ldx, const
     }
 }
 
+// The same for RHT tiles of 256 (the large-M path at n_tile = 256): lane l holds elements 8l .. 8l+7 = E8 block l of the
+// tile.  Three in-register butterfly stages (strides 1, 2, 4) and five shuffle stages (8 .. 128), FORMAT R1 order.  The
+// tile leaves as TWO operand chunks of 128 K-bytes (chunk = block / 16; K index inside a chunk 32c + 4i + b for block
+// 4c + b, coordinate i), each followed by the NB scales s_x of the whole tile.  blob index = (bt * n_kt256 + kt) * 2 + chunk.
+__global__ void __launch_bounds__(QW_WARPS * 32)
+k_act_blob256(const void* X, int dtype, int64_t B, int64_t n_kt, int64_t ldx, const int8_t* dsign, int NB, uint8_t* bblob) {
+    extern __shared__ float smem[];
+    griddep_launch();
+    griddep_wait();
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    uint8_t* srow = (uint8_t*)smem + warp * 256;          // two operand rows of 128 bytes
+    const int64_t n_bt = (B + NB - 1) / NB, n_tiles = n_bt * NB * n_kt;
+    const uint32_t blob_bytes = (uint32_t)(NB * 128 + NB * 4);
+    const bool vec = dtype == HQ_BF16 ? ((((uintptr_t)X) | (uintptr_t)(ldx * 2)) & 15) == 0
+                                      : ((((uintptr_t)X) | (uintptr_t)(ldx * 4)) & 15) == 0;
+    const int colb = 128 * (lane >> 4) + 32 * ((lane >> 2) & 3) + (lane & 3);   // + 4 i: byte of coordinate i in the two rows
+    const uint32_t n_kt32 = (uint32_t)n_kt, NB32 = (uint32_t)NB;
+    const uint32_t stride = gridDim.x * (uint32_t)QW_WARPS;
+    const uint32_t st_b = stride / n_kt32, st_k = stride - st_b * n_kt32;
+    uint32_t b32 = (blockIdx.x * (uint32_t)QW_WARPS + warp) / n_kt32;
+    uint32_t kt32 = (blockIdx.x * (uint32_t)QW_WARPS + warp) - b32 * n_kt32;
+    for (int64_t tile = blockIdx.x * (int64_t)QW_WARPS + warp; tile < n_tiles; tile += stride,
+                 kt32 += st_k, b32 += st_b + (kt32 >= n_kt32 ? 1u : 0u), kt32 -= (kt32 >= n_kt32 ? n_kt32 : 0u)) {
+        const int64_t b = b32, kt = kt32;
+        const int64_t bt = b32 / NB32;
+        const int bb = (int)(b32 - (uint32_t)bt * NB32);
+        float x[8];
+        int qv[8];
+        float sx = 0.0f;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) { x[j] = 0.0f; qv[j] = 0; }
+        if (b < B) {
+            const int64_t base = b * ldx + kt * 256 + 8 * lane;
+            if (vec && dtype == HQ_BF16) {
+                const uint4 v = __ldg((const uint4*)((const __nv_bfloat16*)X + base));
+                x[0] = __uint_as_float(v.x << 16); x[1] = __uint_as_float(v.x & 0xffff0000u);
+                x[2] = __uint_as_float(v.y << 16); x[3] = __uint_as_float(v.y & 0xffff0000u);
+                x[4] = __uint_as_float(v.z << 16); x[5] = __uint_as_float(v.z & 0xffff0000u);
+                x[6] = __uint_as_float(v.w << 16); x[7] = __uint_as_float(v.w & 0xffff0000u);
+            } else {
+#pragma unroll
+                for (int j = 0; j < 8; ++j) x[j] = load_elem(X, dtype, base + j);
+            }
+            const uint2 sg = __ldg((const uint2*)(dsign + kt * 256) + lane);
+#pragma unroll
+            for (int j = 0; j < 8; ++j)
+                if ((((j < 4 ? sg.x : sg.y) >> (8 * (j & 3))) & 0x80u)) x[j] = -x[j];
+#pragma unroll
+            for (int h = 1; h < 8; h <<= 1)      // strides 1, 2, 4: inside the lane
+#pragma unroll
+                for (int i = 0; i < 8; ++i)
+                    if (!(i & h)) {
+                        const float a = x[i], c = x[i + h];
+                        x[i] = __fadd_rn(a, c); x[i + h] = __fsub_rn(a, c);
+                    }
+#pragma unroll
+            for (int m = 1; m < 32; m <<= 1) {   // strides 8 .. 128: lane ^ m holds the partner
+                const float sg1 = (lane & m) ? -1.0f : 1.0f;
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    const float o = __shfl_xor_sync(0xffffffffu, x[j], m);
+                    x[j] = __fmaf_rn(x[j], sg1, o);
+                }
+            }
+            float amax = 0.0f;
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                x[j] = __fmul_rn(x[j], 0.0625f);   // 1 / sqrt(256)
+                amax = fmaxf(amax, fabsf(x[j]));
+            }
+            for (int sft = 16; sft; sft >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, sft));
+            if (amax != 0.0f) {
+                const float inv = __fdiv_rn(127.0f, amax);
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    // rint + clamp to +-127 + cast in one instruction: |x| <= amax bounds |x * inv| by 127 (1 + 2^-23), which
+                    // rounds to 127, so the saturating convert can never return -128 and equals FORMAT R7's clamp(rint(.))
+                    asm("cvt.rni.sat.s8.f32 %0, %1;" : "=r"(qv[j]) : "f"(__fmul_rn(x[j], inv)));
+                }
+                sx = __fdiv_rn(amax, 127.0f);
+            }
+        }
+#pragma unroll
+        for (int j = 0; j < 8; ++j) srow[colb + 4 * j] = (uint8_t)(int8_t)qv[j];
+        __syncwarp();
+#pragma unroll
+        for (int ch = 0; ch < 2; ++ch) {   // one coalesced 128-byte row per chunk
+            uint8_t* blob = bblob + ((bt * n_kt + kt) * 2 + ch) * (int64_t)blob_bytes;
+            const uint32_t w4 = ((const uint32_t*)srow)[ch * 32 + lane];
+            *(uint32_t*)(blob + (bb >> 3) * 1024 + (bb & 7) * 128 + ((((lane >> 2) ^ (bb & 7)) << 4) | ((lane & 3) << 2))) = w4;
+            if (lane == 0) ((float*)(blob + NB * 128))[bb] = sx;
+        }
+        __syncwarp();
+    }
+}
+
+void launch_act_blob256(const void* x, int dtype, int64_t B, int64_t n_in, int64_t ldx, const int8_t* dsign, int NB,
+                        uint8_t* bblob, cudaStream_t st) {
+    int64_t n_kt = n_in / 256, n_bt = (B + NB - 1) / NB, n_tiles = n_bt * NB * n_kt;
+    int64_t blocks = (n_tiles + QW_WARPS - 1) / QW_WARPS;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    launch_pdl(k_act_blob256, dim3((unsigned)blocks), dim3(QW_WARPS * 32), QW_WARPS * 256, st, x, dtype, B, n_kt, ldx, dsign, NB,
+               bblob);
+}
+
 void launch_act_blob(const void* x, int dtype, int64_t B, int64_t n_in, int64_t ldx, const int8_t* dsign, int NB,
                      uint8_t* bblob, cudaStream_t st) {
     int64_t n_kt = n_in / 128, n_bt = (B + NB - 1) / NB, n_tiles = n_bt * NB * n_kt;

@@ -24,6 +24,10 @@ struct hq_ctx {
     // optional kernel timing (hq_profile_*): event pairs around the dominant kernel of each call
     bool prof = false;
     std::vector<cudaEvent_t> prof_ev;
+    // fork / join inside one call (large-M path: the weight decode runs beside the activation cast): a side stream and
+    // two timing-free events; everything stays ordered with respect to the caller's stream (graph-capturable)
+    cudaStream_t side = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
 };
 
 struct hq_weight {
@@ -113,6 +117,9 @@ void launch_act_quant(const void* x, int dtype, int64_t B, int64_t n_in, int64_t
 // activations as the E8 fused kernel's B operand tiles (UMMA layout, permuted K, + scales); n_tile = 128
 void launch_act_blob(const void* x, int dtype, int64_t B, int64_t n_in, int64_t ldx, const int8_t* dsign, int NB,
                      uint8_t* bblob, cudaStream_t st);
+// the same for RHT tiles of 256: two operand chunks of 128 K-bytes per tile (large-M path at n_tile = 256)
+void launch_act_blob256(const void* x, int dtype, int64_t B, int64_t n_in, int64_t ldx, const int8_t* dsign, int NB,
+                        uint8_t* bblob, cudaStream_t st);
 // ulen_tmp[sg*32 + i] for all sub-groups (0 for absent rows); err_flag[0] set if a tile exceeds 8160 bits,
 // err_flag[4] = max over present rows of 65535 - ulen, err_flag[5] = max over present rows of ulen
 void launch_tile_ulen(const int8_t* codes, int64_t m, int64_t n_in, int lattice, int n, int k0, int k1,

@@ -343,13 +343,20 @@ size_t linear_group_workspace_bytes(const hq_ctx* ctx, const hq_weight* const* w
     if (B >= LG_MIN_B) {   // the large-M path: activation blob of 256-row tiles + the decoded copy of the largest weight
         int64_t rb_max = 0;
         for (int i = 0; i < n_w; ++i) rb_max = ws[i]->n_rb > rb_max ? ws[i]->n_rb : rb_max;
-        bytes += align256((size_t)((B + LG_NB - 1) / LG_NB) * ws[0]->n_kt * LG_BBLOB) + align256((size_t)rb_max * ws[0]->n_kt * LG_ABLOB);
+        bytes += align256((size_t)((B + LG_NB - 1) / LG_NB) * (ws[0]->n_in / 128) * LG_BBLOB) + align256((size_t)rb_max * (ws[0]->n_in / 128) * LG_ABLOB);
     }
     return bytes + 256;
 }
 
+// E8 / tile 256 takes the large-M path only (from LG_MIN_B activation rows); below that the generic kernel
+static bool linear_uses_e8_large256(const hq_weight* w, int64_t B) {
+    return w->lattice == LAT_E8 && w->n == 256 && w->k0 <= 3 && B >= LG_MIN_B;
+}
+
 size_t linear_workspace_bytes(const hq_ctx* ctx, const hq_weight* w, int64_t B) {
     if (linear_uses_e8_fast(w)) return linear_group_workspace_bytes(ctx, &w, 1, B);
+    if (linear_uses_e8_large256(w, B))
+        return align256((size_t)((B + LG_NB - 1) / LG_NB) * (w->n_in / 128) * LG_BBLOB) + align256((size_t)w->n_rb * (w->n_in / 128) * LG_ABLOB) + 256;
     int ns = generic_split(ctx, w, B);
     return align256((size_t)(B * w->n_in)) + align256((size_t)(B * w->n_kt) * 4) + (size_t)ns * B * w->m * 4 + 256;
 }
@@ -361,9 +368,15 @@ static hq_status launch_large(hq_ctx* ctx, const hq_weight* const* ws, int n_w, 
                               uint8_t* wsbuf, cudaStream_t st) {
     const hq_weight* w0 = ws[0];
     const int64_t n_bt = (B + LG_NB - 1) / LG_NB;
+    const int nch = w0->n / 128;                       // operand chunks of 128 K-bytes per RHT tile (tile 128 or 256)
+    const int64_t n_kt128 = w0->n_in / 128;
     uint8_t* bblob = wsbuf;
-    uint8_t* ablob = wsbuf + align256((size_t)n_bt * w0->n_kt * LG_BBLOB);
-    launch_act_blob(x, dtype, B, w0->n_in, ldx, w0->dsign, LG_NB, bblob, st);
+    uint8_t* ablob = wsbuf + align256((size_t)n_bt * n_kt128 * LG_BBLOB);
+    // fork: the first weight's decode does not depend on x, it runs on the side stream beside the activation cast
+    HQ_CUDA_CHECK(ctx, cudaEventRecord(ctx->ev_fork, st));
+    HQ_CUDA_CHECK(ctx, cudaStreamWaitEvent(ctx->side, ctx->ev_fork, 0));
+    if (nch == 1) launch_act_blob(x, dtype, B, w0->n_in, ldx, w0->dsign, LG_NB, bblob, st);
+    else launch_act_blob256(x, dtype, B, w0->n_in, ldx, w0->dsign, LG_NB, bblob, st);
     HQ_CUDA_CHECK(ctx, cudaGetLastError());
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     if (ctx->prof) {
@@ -381,23 +394,38 @@ static hq_status launch_large(hq_ctx* ctx, const hq_weight* const* ws, int n_w, 
         while (ky < d.n_kt && (int64_t)w->n_rb * ky < (int64_t)ctx->sm_count * 8) ky *= 2;
         d.kt_per_cta = (d.n_kt + ky - 1) / ky;
         dim3 dgrid((unsigned)w->n_rb, (unsigned)((d.n_kt + d.kt_per_cta - 1) / d.kt_per_cta));
-        const size_t dsmem = E8_LUT_BYTES + 128 * E8_SCR_STRIDE * 4;
+        const size_t dsmem = E8_LUT_BYTES + 128 * (size_t)(w->n / 8 + 1) * 4;
+        cudaStream_t dst = i == 0 ? ctx->side : st;   // later weights reuse the scratch copy: stream order after the GEMM
 #define HQ_LD(KK)                                                                                                          \
     case KK:                                                                                                               \
-        HQ_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_e8_decode_ablob<KK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dsmem)); \
-        k_e8_decode_ablob<KK><<<dgrid, 128, dsmem, st>>>(d);                                                               \
+        if (nch == 1) {                                                                                                    \
+            HQ_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_e8_decode_ablob<KK, 128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dsmem)); \
+            k_e8_decode_ablob<KK, 128><<<dgrid, 128, dsmem, dst>>>(d);                                                     \
+        } else {                                                                                                           \
+            HQ_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_e8_decode_ablob<KK, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dsmem)); \
+            k_e8_decode_ablob<KK, 256><<<dgrid, 128, dsmem, dst>>>(d);                                                     \
+        }                                                                                                                  \
         break
         switch (w->k0) { HQ_LD(0); HQ_LD(1); HQ_LD(2); HQ_LD(3); }
 #undef HQ_LD
         HQ_CUDA_CHECK(ctx, cudaGetLastError());
+        if (i == 0) {   // join
+            HQ_CUDA_CHECK(ctx, cudaEventRecord(ctx->ev_join, ctx->side));
+            HQ_CUDA_CHECK(ctx, cudaStreamWaitEvent(st, ctx->ev_join, 0));
+        }
         E8LargeParams g;
         g.ablob = ablob; g.bblob = bblob; g.y_bf16 = (__nv_bfloat16*)ys_bf16[i]; g.y_f32 = ys_f32 ? ys_f32[i] : nullptr;
-        g.ldy = ldys[i]; g.m = w->m; g.B = B; g.n_rb = (int)w->n_rb; g.n_bt = (int)n_bt; g.n_kt = (int)w->n_kt;
+        g.ldy = ldys[i]; g.m = w->m; g.B = B; g.n_rb = (int)w->n_rb; g.n_bt = (int)n_bt; g.n_kt = (int)n_kt128;
         g.acc_i32 = (n_w == 1) ? acc_i32 : nullptr;
         const int64_t tiles = (int64_t)g.n_rb * g.n_bt;
         const unsigned grid = (unsigned)(tiles < ctx->sm_count ? tiles : ctx->sm_count);
-        HQ_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_e8_gemm_large, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LG_SMEM));
-        k_e8_gemm_large<<<grid, 384, LG_SMEM, st>>>(g);
+        if (nch == 1) {
+            HQ_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_e8_gemm_large<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LG_SMEM));
+            k_e8_gemm_large<1><<<grid, 384, LG_SMEM, st>>>(g);
+        } else {
+            HQ_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_e8_gemm_large<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LG_SMEM));
+            k_e8_gemm_large<2><<<grid, 384, LG_SMEM, st>>>(g);
+        }
         HQ_CUDA_CHECK(ctx, cudaGetLastError());
     }
     if (ctx->prof) {
@@ -522,6 +550,7 @@ hq_status launch_linear(hq_ctx* ctx, const hq_weight* w, const void* x, int dtyp
                         void* y_bf16, int64_t ldy, float* y_f32, int32_t* acc_i32, uint8_t* ws, cudaStream_t st) {
     if (linear_uses_e8_fast(w))
         return launch_linear_group(ctx, &w, 1, x, dtype, B, ldx, &y_bf16, &ldy, &y_f32, acc_i32, ws, st);
+    if (linear_uses_e8_large256(w, B)) return launch_large(ctx, &w, 1, x, dtype, B, ldx, &y_bf16, &ldy, &y_f32, acc_i32, ws, st);
     const float inv_A = (float)(1.0 / (w->alpha * sqrt((double)w->n)));
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     int8_t* q = (int8_t*)ws;

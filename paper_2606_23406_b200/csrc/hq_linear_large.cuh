@@ -23,9 +23,13 @@ namespace hq {
 constexpr int LG_NB = 256;                                   // activation rows per tile = MMA N
 constexpr uint32_t LG_ABLOB = 16384u + 512u;                 // INT8 tile + 128 fp32 row scales
 constexpr uint32_t LG_BBLOB = LG_NB * 128u + LG_NB * 4u;     // = e8_bblob_bytes(256)
-constexpr uint32_t LG_STAGE = (LG_ABLOB + LG_BBLOB + 1023u) & ~1023u;
+constexpr uint32_t LG_STAGE = LG_NB * 128u + 16384u;          // operand bytes of one K-chunk of 128: B tile 32 KB + A tile 16 KB
 constexpr int LG_NST = 4;
-constexpr size_t LG_SMEM = 1024 + (size_t)LG_NST * LG_STAGE + 8 * (2 * LG_NST + 4) + 16;
+// The scales of an RHT tile (256 s_x + 128 row scales) travel in a ring of their own: an operand stage is released by the
+// MMA's commit alone, not held while the epilogue drains the tile (that throttled the TMA pipeline to a third).
+constexpr uint32_t LG_SCSLOT = LG_NB * 4u + 512u;
+constexpr int LG_NSC = 8;
+constexpr size_t LG_SMEM = 1024 + (size_t)LG_NST * LG_STAGE + (size_t)LG_NSC * LG_SCSLOT + 8 * (2 * LG_NST + 2 * LG_NSC + 4) + 16;
 
 struct E8AblobParams {
     const uint8_t* blob;
@@ -37,17 +41,23 @@ struct E8AblobParams {
     float inv_A;
 };
 
-template <int K>
+// TILE = RHT tile of the weight (128 or 256).  A tile of 256 is written as two operand chunks of 128 K-bytes (K index
+// inside the tile: 32c + 4i + b for block 4c + b, coordinate i; chunk = c / 4), each followed by the same 128 row scales.
+template <int K, int TILE>
 __global__ void __launch_bounds__(128) k_e8_decode_ablob(E8AblobParams p) {
     extern __shared__ __align__(16) uint8_t smem_raw[];
-    constexpr int KW = 4 * K;
+    constexpr int KW = K * TILE / 32;              // R words per row
+    constexpr int NWT = E8_NW * TILE / 128;        // U words per row handled by the fast path
+    constexpr int NRUN = TILE / 32;                // runs of 32 symbols
+    constexpr int SCR = TILE / 8 + 1;              // nibble words per row + 1
+    constexpr int NCH = TILE / 128;                // operand chunks per tile
     const int t = threadIdx.x, warp = t >> 5, lane = t & 31;
     uint32_t* lut_s = (uint32_t*)smem_raw;
     for (int i = t; i < E8_LUT_WORDS; i += 128) lut_s[i] = __ldg(p.lut + i);
     __syncthreads();
     const uint32_t smem_a = smem_u32(smem_raw);
     const uint32_t lut_lane = smem_a + (uint32_t)(lane & (E8_LUT_COPIES - 1)) * 4;
-    const uint32_t scr_a = smem_a + E8_LUT_BYTES + (uint32_t)t * E8_SCR_STRIDE * 4;
+    const uint32_t scr_a = smem_a + E8_LUT_BYTES + (uint32_t)t * SCR * 4;
     const uint32_t lane_lt = (1u << lane) - 1u;
     const int rb = blockIdx.x;
     const int kt0 = blockIdx.y * p.kt_per_cta;
@@ -58,14 +68,14 @@ __global__ void __launch_bounds__(128) k_e8_decode_ablob(E8AblobParams p) {
         const uint32_t ul = __ldg((const uint16_t*)sgp + lane), nrm = __ldg((const uint16_t*)sgp + 32 + lane);
         const uint32_t* rarea = (const uint32_t*)(sgp + 128);
         const uint32_t* uarea = rarea + KW * 32;
-        uint32_t Rw[KW > 0 ? KW : 1], Uw[E8_NW];
+        uint32_t Rw[KW > 0 ? KW : 1], Uw[NWT];
 #pragma unroll
         for (int j = 0; j < KW; ++j) Rw[j] = __ldg(rarea + j * 32 + lane);
         const uint32_t nw = (ul + 31) >> 5;
         {
             uint32_t base = 0;
 #pragma unroll
-            for (int w = 0; w < E8_NW; ++w) {
+            for (int w = 0; w < NWT; ++w) {
                 const bool has = nw > (uint32_t)w;
                 const uint32_t mk = __ballot_sync(0xffffffffu, has);
                 Uw[w] = has ? __ldg(uarea + base + __popc(mk & lane_lt)) : 0u;
@@ -75,14 +85,13 @@ __global__ void __launch_bounds__(128) k_e8_decode_ablob(E8AblobParams p) {
         {
             uint32_t T = 0, acc = 0, wo = scr_a;
 #pragma unroll
-            for (int w = 0; w < E8_NW; ++w) e8_unary_word(Uw[w], lut_lane, T, acc, wo);
+            for (int w = 0; w < NWT; ++w) e8_unary_word(Uw[w], lut_lane, T, acc, wo);
         }
-        uint8_t* tile = p.ablob + g * LG_ABLOB;
-        uint8_t* rowp = tile + (t >> 3) * 1024 + (t & 7) * 128;
+        uint8_t* tile = p.ablob + g * (size_t)(NCH * LG_ABLOB);
         const bool present = r < p.m && ul > 0;
         uint32_t total = 0, prevWo = 15u << 24;
 #pragma unroll
-        for (int c = 0; c < 4; ++c) {
+        for (int c = 0; c < NRUN; ++c) {
             uint32_t W[4], C[8];
 #pragma unroll
             for (int w = 0; w < 4; ++w) W[w] = lds32(scr_a + (c * 4 + w) * 4);
@@ -91,22 +100,26 @@ __global__ void __launch_bounds__(128) k_e8_decode_ablob(E8AblobParams p) {
 #pragma unroll
                 for (int i = 0; i < 8; ++i) C[i] = 0u;
             }
-            *(uint4*)(rowp + (((2 * c) ^ (t & 7)) << 4)) = make_uint4(C[0], C[1], C[2], C[3]);
-            *(uint4*)(rowp + (((2 * c + 1) ^ (t & 7)) << 4)) = make_uint4(C[4], C[5], C[6], C[7]);
+            uint8_t* rowp = tile + (c >> 2) * LG_ABLOB + (t >> 3) * 1024 + (t & 7) * 128;
+            *(uint4*)(rowp + (((2 * (c & 3)) ^ (t & 7)) << 4)) = make_uint4(C[0], C[1], C[2], C[3]);
+            *(uint4*)(rowp + (((2 * (c & 3) + 1) ^ (t & 7)) << 4)) = make_uint4(C[4], C[5], C[6], C[7]);
         }
-        if (present && (nw > (uint32_t)E8_NW || total + 128u != ul)) {   // a quotient >= 16 or a long row: generic decoder
+        if (present && (nw > (uint32_t)NWT || total + (uint32_t)TILE != ul)) {   // a quotient >= 16 or a long row: generic decoder
             SubGroup sg = sub_group(sgp, KW);
             WordsRowU uw{nullptr, sg.uarea, sg.ulen, nw, 0u, lane};
             WordsRowR rw{sg.rarea, lane, KW};
-            decode_row_generic<LAT_E8>(rw, 0u, uw, 0u, 128, K, K, [&](int bk, const int* c) {
+            decode_row_generic<LAT_E8>(rw, 0u, uw, 0u, TILE, K, K, [&](int bk, const int* c) {
 #pragma unroll
                 for (int e = 0; e < 8; ++e) {
-                    const int col = e8_kcol(8 * bk + e);
+                    const int col = e8_kcol(8 * (bk & 15) + e);
+                    uint8_t* rowp = tile + (bk >> 4) * LG_ABLOB + (t >> 3) * 1024 + (t & 7) * 128;
                     rowp[(((col >> 4) ^ (t & 7)) << 4) | (col & 15)] = (uint8_t)(int8_t)c[e];
                 }
             });
         }
-        ((float*)(tile + 16384))[t] = present ? f16_bits_to_f32((uint16_t)nrm) * p.inv_A : 0.0f;
+        const float sw = present ? f16_bits_to_f32((uint16_t)nrm) * p.inv_A : 0.0f;
+#pragma unroll
+        for (int ch = 0; ch < NCH; ++ch) ((float*)(tile + ch * LG_ABLOB + 16384))[t] = sw;
     }
 }
 
@@ -140,20 +153,28 @@ struct E8LargeParams {
     int32_t* acc_i32;       // [n_kt][B][m] or null: parity / debug copy of every K-tile's INT32 accumulator
 };
 
+// NCH = operand chunks (TMA stages of 128 K-bytes) per RHT tile: 1 (tile 128) or 2 (tile 256).  The INT32 accumulator runs
+// over the NCH chunks of a tile and is drained once per TILE: at tile 256 the rescale costs half as many issue slots per
+// MAC (the tile is chosen on kernel grounds).  p.n_kt counts chunks.
+template <int NCH>
 __global__ void __launch_bounds__(384, 1) k_e8_gemm_large(E8LargeParams p) {
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
     const uint32_t smem_a = smem_u32(smem);
-    uint64_t* full = (uint64_t*)(smem + (size_t)LG_NST * LG_STAGE);
+    const uint32_t sc_a = smem_a + LG_NST * LG_STAGE;   // scale ring
+    uint64_t* full = (uint64_t*)(smem + (size_t)LG_NST * LG_STAGE + (size_t)LG_NSC * LG_SCSLOT);
     uint64_t* empty = full + LG_NST;
-    uint64_t* acc_full = empty + LG_NST;
+    uint64_t* scf = empty + LG_NST;      // scales of a tile landed
+    uint64_t* sce = scf + LG_NSC;        // scales of a tile read by the eight epilogue warps
+    uint64_t* acc_full = sce + LG_NSC;
     uint64_t* acc_empty = acc_full + 2;
     uint32_t* tmem_slot = (uint32_t*)(acc_empty + 2);
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
 
     if (warp == 0) tmem_alloc(tmem_slot, 512);
     if (tid == 32) {
-        for (int s = 0; s < LG_NST; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1 + 8); }
+        for (int s = 0; s < LG_NST; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
+        for (int s = 0; s < LG_NSC; ++s) { mbar_init(&scf[s], 1); mbar_init(&sce[s], 8); }
         for (int a = 0; a < 2; ++a) { mbar_init(&acc_full[a], 1); mbar_init(&acc_empty[a], 8); }
         mbar_fence_init();
     }
@@ -174,10 +195,18 @@ __global__ void __launch_bounds__(384, 1) k_e8_gemm_large(E8LargeParams p) {
                 for (int kt = 0; kt < p.n_kt; ++kt, ++it) {
                     const uint32_t s = it % LG_NST, ph = (it / LG_NST) & 1u;
                     mbar_wait(&empty[s], ph ^ 1u);
-                    mbar_arrive_expect_tx(&full[s], LG_ABLOB + LG_BBLOB);
+                    mbar_arrive_expect_tx(&full[s], LG_STAGE);
                     uint8_t* st = smem + (size_t)s * LG_STAGE;
-                    bulk_g2s(st, bg + (size_t)kt * LG_BBLOB, LG_BBLOB, &full[s]);
-                    bulk_g2s(st + LG_BBLOB, ag + (size_t)kt * LG_ABLOB, LG_ABLOB, &full[s]);
+                    bulk_g2s(st, bg + (size_t)kt * LG_BBLOB, LG_NB * 128u, &full[s]);
+                    bulk_g2s(st + LG_NB * 128u, ag + (size_t)kt * LG_ABLOB, 16384u, &full[s]);
+                    if (it % NCH == NCH - 1) {   // last chunk of an RHT tile: its scales into the scale ring
+                        const uint32_t tl = it / NCH, q = tl % LG_NSC;
+                        mbar_wait(&sce[q], ((tl / LG_NSC) & 1u) ^ 1u);
+                        mbar_arrive_expect_tx(&scf[q], LG_SCSLOT);
+                        uint8_t* sc = smem + (size_t)LG_NST * LG_STAGE + (size_t)q * LG_SCSLOT;
+                        bulk_g2s(sc, bg + (size_t)kt * LG_BBLOB + LG_NB * 128u, LG_NB * 4u, &scf[q]);
+                        bulk_g2s(sc + LG_NB * 4u, ag + (size_t)kt * LG_ABLOB + 16384u, 512u, &scf[q]);
+                    }
                 }
             }
         } else if (tid == 32) {   // ---- MMA issuer
@@ -185,16 +214,17 @@ __global__ void __launch_bounds__(384, 1) k_e8_gemm_large(E8LargeParams p) {
             uint32_t it = 0;
             for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
                 for (int kt = 0; kt < p.n_kt; ++kt, ++it) {
-                    const uint32_t s = it % LG_NST, ph = (it / LG_NST) & 1u, a = it & 1u;
-                    mbar_wait(&acc_empty[a], ((it >> 1) & 1u) ^ 1u);
+                    const uint32_t s = it % LG_NST, ph = (it / LG_NST) & 1u;
+                    const uint32_t tl = it / NCH, ch = it % NCH, a = tl & 1u;   // RHT tile, chunk inside it, accumulator
+                    if (ch == 0) mbar_wait(&acc_empty[a], ((tl >> 1) & 1u) ^ 1u);
                     mbar_wait(&full[s], ph);
                     tc_fence_after();
-                    const uint32_t sb = smem_a + s * LG_STAGE, sa = sb + LG_BBLOB;
+                    const uint32_t sb = smem_a + s * LG_STAGE, sa = sb + LG_NB * 128u;
 #pragma unroll
                     for (int ks = 0; ks < 4; ++ks)
-                        mma_i8(tmem + a * LG_NB, make_desc_sw128(sa + ks * 32), make_desc_sw128(sb + ks * 32), idesc, ks > 0);
+                        mma_i8(tmem + a * LG_NB, make_desc_sw128(sa + ks * 32), make_desc_sw128(sb + ks * 32), idesc, (ks > 0 || ch > 0));
                     mma_commit(&empty[s]);
-                    mma_commit(&acc_full[a]);
+                    if (ch == NCH - 1) mma_commit(&acc_full[a]);
                 }
             }
         }
@@ -211,8 +241,9 @@ __global__ void __launch_bounds__(384, 1) k_e8_gemm_large(E8LargeParams p) {
         uint32_t v[2][32];
         const uint32_t tlane = tmem + half * 128 + ((uint32_t)(q * 32) << 16);
         // first chunk of K-step `i`: wait for its operands (scales) and its accumulator, start the TMEM load
+        // step i = RHT tile i of this CTA's stream; its scales sit in the stage of its LAST chunk
         auto begin_step = [&](uint32_t i) {
-            mbar_wait(&full[i % LG_NST], (i / LG_NST) & 1u);   // the TMA-written scales are visible to this thread
+            mbar_wait(&scf[i % LG_NSC], (i / LG_NSC) & 1u);   // the TMA-written scales are visible to this thread
             mbar_wait(&acc_full[i & 1u], (i >> 1) & 1u);
             tc_fence_after();
             const uint32_t ta = tlane + (i & 1u) * LG_NB;
@@ -220,16 +251,17 @@ __global__ void __launch_bounds__(384, 1) k_e8_gemm_large(E8LargeParams p) {
             tmem_ld16(ta + 16, v[0] + 16);
         };
         const int my_tiles = blockIdx.x < n_tiles ? (n_tiles - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
-        const uint32_t n_steps = (uint32_t)my_tiles * (uint32_t)p.n_kt;
+        const int n_tl = p.n_kt / NCH;   // RHT tiles along K
+        const uint32_t n_steps = (uint32_t)my_tiles * (uint32_t)n_tl;
         if (n_steps) begin_step(0);
         for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
             const int bt = tile / p.n_rb, rb = tile - bt * p.n_rb;
-            for (int kt = 0; kt < p.n_kt; ++kt, ++it) {
-                const uint32_t s = it % LG_NST, a = it & 1u;
-                const uint32_t sb = smem_a + s * LG_STAGE;
-                const float sw = lds_f32(sb + LG_BBLOB + 16384 + row * 4);
+            for (int kt = 0; kt < n_tl; ++kt, ++it) {
+                const uint32_t q = it % LG_NSC, a = it & 1u;
+                const uint32_t sb = sc_a + q * LG_SCSLOT;
+                const float sw = lds_f32(sb + LG_NB * 4 + row * 4);
                 const uint64_t sw2 = pack_f32x2(sw, sw);
-                const uint32_t sx_a = sb + LG_NB * 128 + half * 512;
+                const uint32_t sx_a = sb + half * 512;
                 const uint32_t taddr = tlane + a * LG_NB;
 #pragma unroll
                 for (int ch = 0; ch < 4; ++ch) {
@@ -262,7 +294,7 @@ __global__ void __launch_bounds__(384, 1) k_e8_gemm_large(E8LargeParams p) {
                     }
                 }
                 __syncwarp();
-                if (lane == 0) mbar_arrive(&empty[s]);   // the scales of this stage have been read
+                if (lane == 0) mbar_arrive(&sce[q]);   // the scales of this tile have been read
             }
             const int64_t r = (int64_t)rb * 128 + row;
             const int64_t b0 = (int64_t)bt * LG_NB + half * 128;

@@ -152,10 +152,12 @@ def test_e8_fast_kernel_falls_back_on_long_quotients_and_ragged_blocks(ctx):
         w.free()
 
 
+@pytest.mark.parametrize("n_tile", [128, 256])
 @pytest.mark.parametrize("B,m,k", [(600, 300, (-1, -1)), (512, 200, (0, 0)), (1030, 130, (3, 3))])
-def test_linear_large_m_path(ctx, B, m, k):
+def test_linear_large_m_path(ctx, B, m, k, n_tile):
     """From 512 activation rows hq_linear decodes the weights once into an operand-layout scratch copy and runs the
-    warp-specialised GEMM (hq_linear_large.cuh): ragged row block, ragged batch tile, several tiles per CTA, rows that
+    warp-specialised GEMM (hq_linear_large.cuh), at RHT tiles of 128 and 256 (two operand chunks per accumulator
+    drain): ragged row block, ragged batch tile, several tiles per CTA, rows that
     take the decoder's generic fallback (k = 0 at 5 bps; a clamp row), an absent row; and the weights of a group."""
     n_in, seed = 1024, 17
     snr = f32(28.73) if k == (0, 0) else SNR_4BPS[hqo.E8]
@@ -163,12 +165,12 @@ def test_linear_large_m_path(ctx, B, m, k):
     W[3] = 0.0
     d = hqo.signs(seed, 1, n_in)[256:384].astype(np.float32)
     had = np.array([(-1.0) ** bin(i & 5).count("1") for i in range(128)], np.float32)
-    W[7, :] = 0.0; W[7, 256:384] = d * had * 0.5
+    W[7, :] = 0.0; W[7, 256:384] = d * had * 0.5               # at tile 128 this row is n * e_5 after the RHT (clamp, G8)
     x = hq_synth.activations(B, n_in, seed=B)
-    enc = hqo.encode_weights(W, hqo.E8, 128, snr, seed, k)
-    w = ctx.encode_weights(_dev(W), hqo.E8, 128, snr, seed, k)
-    q_o, sx_o = hqo.act_quant(x, hqo.E8, 128, seed)
-    acc_o, y_o = hqo.linear(enc["codes"], enc["norms"], hqo.E8, 128, snr, q_o, sx_o)
+    enc = hqo.encode_weights(W, hqo.E8, n_tile, snr, seed, k)
+    w = ctx.encode_weights(_dev(W), hqo.E8, n_tile, snr, seed, k)
+    q_o, sx_o = hqo.act_quant(x, hqo.E8, n_tile, seed)
+    acc_o, y_o = hqo.linear(enc["codes"], enc["norms"], hqo.E8, n_tile, snr, q_o, sx_o)
     xd = _dev(x, torch.bfloat16)
     y, y32, _ = w.linear(xd, want_f32=True)
     assert _rel_err(y32.cpu().numpy(), y_o) < 1e-3
