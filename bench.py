@@ -32,7 +32,7 @@ NAMES = list(hq_synth.LLAMA_SHAPES)
 # ncu-derived figures (DRAM bytes and warp instructions of the four fused launches of one step) are NOT typed in here:
 # they are read from profiles/r02_ncu_step.json, which the ncu pass of a named commit wrote (see the .md beside it)
 NCU_STEP_JSON = os.path.join(ROOT, "profiles", "r02_ncu_step.json")
-LARGE_M_TILE = 128   # RHT tile of the config-5 weights (the tile is chosen on kernel grounds)
+LARGE_M_TILE = 256   # RHT tile of the config-5 weights (the tile is chosen on kernel grounds)
 WORKLOAD = "llama3.1-8b decoder-layer linears q/k/v/o/gate/up/down, E8 4 bps, RHT tile 128, batch 1 (BASELINE configs[1])"
 
 
