@@ -121,15 +121,98 @@ __device__ inline void warp_query_transform(float* s, int d, const int8_t* dsign
     __syncwarp();
 }
 
-template <int LAT>
+// ---------------------------------------------------------------------------------------------
+// The E8 dither of one lattice block, regenerated for attend (FORMAT §1, R4, R6; A.6 L843-847).  Same decisions and the
+// same roundings as dither_block<LAT_E8> (hq_common.cuh) - every value below is the same fp32 number - but written for
+// issue slots: the Philox round keys are precomputed once per thread (rk), rint is the magic-constant add (exact RNE for
+// |z| < 2^22), the D8 parity fix is branch-free, and the coset points stay in fp32 (small integers are exact).
+// ---------------------------------------------------------------------------------------------
+struct PhiloxKeys { uint32_t k0[10], k1[10]; };
+__device__ __forceinline__ PhiloxKeys philox_round_keys(uint64_t seed) {
+    PhiloxKeys rk;
+    uint32_t a = (uint32_t)seed, b = (uint32_t)(seed >> 32);
+#pragma unroll
+    for (int r = 0; r < 10; ++r) { rk.k0[r] = a; rk.k1[r] = b; a += 0x9E3779B9u; b += 0xBB67AE85u; }
+    return rk;
+}
+__device__ __forceinline__ void philox4x32_10_keys(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, const PhiloxKeys& rk,
+                                                   uint32_t* o) {
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t h0 = __umulhi(0xD2511F53u, c0), l0 = 0xD2511F53u * c0;
+        const uint32_t h1 = __umulhi(0xCD9E8D57u, c2), l1 = 0xCD9E8D57u * c2;
+        c0 = h1 ^ c1 ^ rk.k0[r]; c1 = l1; c2 = h0 ^ c3 ^ rk.k1[r]; c3 = l0;
+    }
+    o[0] = c0; o[1] = c1; o[2] = c2; o[3] = c3;
+}
+// Q_{D8}(z) in fp32: f = rint(z); if sum f is odd, the first coordinate with the largest |z - f| moves one step away
+__device__ __forceinline__ void nearest_d8_f32(const float* z, float* f) {
+    const float M = 12582912.0f;   // 1.5 * 2^23
+    float dl[8], sum = 0.0f;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        f[i] = __fsub_rn(__fadd_rn(z[i], M), M);
+        dl[i] = __fsub_rn(z[i], f[i]);
+        sum += f[i];                      // exact: small integers
+    }
+    const bool odd = ((int)sum) & 1;
+    float best = fabsf(dl[0]), dj = dl[0];
+    int j = 0;
+#pragma unroll
+    for (int i = 1; i < 8; ++i) {
+        const float a = fabsf(dl[i]);
+        const bool gt = a > best;
+        best = gt ? a : best; dj = gt ? dl[i] : dj; j = gt ? i : j;
+    }
+    const float step = odd ? (dj < 0.0f ? -1.0f : 1.0f) : 0.0f;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) f[i] += (i == j) ? step : 0.0f;
+}
+__device__ __forceinline__ void dither_e8_fast(const PhiloxKeys& rk, uint32_t blk, uint32_t token, uint32_t headrole, float* U) {
+    uint32_t o[8];
+    philox4x32_10_keys(2 * blk, token, headrole, 3u, rk, o);
+    philox4x32_10_keys(2 * blk + 1, token, headrole, 3u, rk, o + 4);
+    float y[8], za[8], zb[8], fa[8], fb[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+        const float wf = (float)(2u * (o[j] >> 9) + 1u);          // exact: < 2^24
+        y[j] = __fsub_rn(__fmul_rn(wf, 0x1p-22f), 2.0f);
+        za[j] = __fmul_rn(y[j], 0.5f);
+        zb[j] = __fmul_rn(__fsub_rn(y[j], 1.0f), 0.5f);
+    }
+    nearest_d8_f32(za, fa);
+    nearest_d8_f32(zb, fb);
+    float da[8], db[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        fa[i] = fa[i] * 2.0f;                 // a = 2 Q(y/2)
+        fb[i] = fb[i] * 2.0f + 1.0f;          // b = 2 Q((y-1)/2) + 1   (exact small integers)
+        const float ea = __fsub_rn(y[i], fa[i]), eb = __fsub_rn(y[i], fb[i]);
+        da[i] = __fmul_rn(ea, ea);
+        db[i] = __fmul_rn(eb, eb);
+    }
+    const float dist_a = __fadd_rn(__fadd_rn(__fadd_rn(da[0], da[1]), __fadd_rn(da[2], da[3])),
+                                   __fadd_rn(__fadd_rn(da[4], da[5]), __fadd_rn(da[6], da[7])));
+    const float dist_b = __fadd_rn(__fadd_rn(__fadd_rn(db[0], db[1]), __fadd_rn(db[2], db[3])),
+                                   __fadd_rn(__fadd_rn(db[4], db[5]), __fadd_rn(db[6], db[7])));
+    const bool pa = dist_a <= dist_b;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) U[i] = __fsub_rn(y[i], pa ? fa[i] : fb[i]);
+}
+
+// GP = query heads per KV head padded to 4 or 8 (vector loads of q' and p).
+// Code size matters here (the dither regeneration is ~300 instructions per lattice block): a token's codes are decoded
+// once into a byte row in shared memory, and ONE loop over the lattice blocks regenerates the dither and feeds the score
+// (K) or the v' row (V); nothing is unrolled over blocks or duplicated per decoder path.
+template <int LAT, int GP>
 __global__ void __launch_bounds__(128, 3)
 k_attend_split(AttendParams p) {
     extern __shared__ float sm[];
     const int d = p.d, G = p.G;
-    float* qs = sm;                    // [G][d]
-    float* vt = qs + G * d;            // [128][d+1]
-    float* ps = vt + 128 * (d + 1);    // [G][128]
-    float* red = ps + G * 128;         // [G][4] block reductions
+    float* qs = sm;                            // [d][GP]   q' of the G query heads, coordinate-major
+    float* vt = qs + d * GP;                   // [128][d+1]
+    float* ps = vt + 128 * (d + 1);            // [128][GP]  p of the block's tokens
+    float* red = ps + 128 * GP;                // [GP][4] block reductions
     __shared__ uint32_t scan[4];
     __shared__ uint32_t lut_s[512];    // phase-1 table of the E8 decoder, [parity][byte]
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -138,27 +221,33 @@ k_attend_split(AttendParams p) {
     const uint32_t lut_a = smem_u32(lut_s);
     // nibble scratch of the E8 decoder: the last 17 words of this thread's (otherwise idle at that time) vt row
     const uint32_t scr_a = smem_u32(vt + tid * (d + 1) + (d - 17));
+    // the token's INT8 codes: the last d bytes of its vt row.  The V loop overwrites the row with floats from the front
+    // and reads the codes of a step before writing it, so the floats never reach codes still needed (4 j0 + 32 <= 3 d + 4 + j0 + 8)
+    uint8_t* crow = (uint8_t*)(vt + tid * (d + 1)) + (3 * d + 4);
 
-    for (int i = tid; i < G * d; i += 128) qs[i] = __bfloat162float(p.q[(h * G) * d + i]);
+    // q' = S RHT(q): transformed in the vt area (one row of d floats per head), then stored coordinate-major
+    for (int i = tid; i < G * d; i += 128) vt[i] = __bfloat162float(p.q[(h * G) * d + i]);
     __syncthreads();
-    for (int g = warp; g < G; g += 4) warp_query_transform(qs + g * d, d, p.dsign, p.ssign, p.rotation, lane);
+    for (int g = warp; g < G; g += 4) warp_query_transform(vt + g * d, d, p.dsign, p.ssign, p.rotation, lane);
+    __syncthreads();
+    for (int i = tid; i < d * GP; i += 128) {
+        const int j = i / GP, g = i % GP;
+        qs[i] = g < G ? vt[g * d + j] : 0.0f;
+    }
     __syncthreads();
 
     const int64_t nblk_total = (p.Tc + 127) / 128;
-    const int64_t per = (nblk_total + p.n_split - 1) / p.n_split;
-    const int64_t blk0 = split * per, blk1 = min(nblk_total, blk0 + per);
+    const int64_t blk0 = (nblk_total * split) / p.n_split, blk1 = (nblk_total * (split + 1)) / p.n_split;   // balanced
 
-    float m_run[ATT_MAXG], l_run[ATT_MAXG], acc[ATT_MAXG];  // thread j owns coordinate(s) j (d <= 128 -> one)
+    const PhiloxKeys rk = philox_round_keys(p.seed);
+    float m_run[GP], l_run[GP], acc[GP], acc2[GP];  // thread j owns coordinate j (and j + 128 when d == 256)
 #pragma unroll
-    for (int g = 0; g < ATT_MAXG; ++g) { m_run[g] = -INFINITY; l_run[g] = 0.0f; acc[g] = 0.0f; }
-    float acc2[ATT_MAXG];  // second coordinate when d == 256
-#pragma unroll
-    for (int g = 0; g < ATT_MAXG; ++g) acc2[g] = 0.0f;
+    for (int g = 0; g < GP; ++g) { m_run[g] = -INFINITY; l_run[g] = 0.0f; acc[g] = 0.0f; acc2[g] = 0.0f; }
 
     for (int64_t blk = blk0; blk < blk1; ++blk) {
         const int64_t t = blk * 128 + tid;
         const bool valid = t < p.Tc;
-        float pg[ATT_MAXG];
+        float pg[GP];
         for (int role = 0; role < 2; ++role) {
             const uint32_t* rem = p.rem + ((int64_t)role * p.H + h) * p.rem_words;
             const uint32_t* una = p.una + ((int64_t)role * p.H + h) * p.una_words;
@@ -168,32 +257,74 @@ k_attend_split(AttendParams p) {
             // every token of the block has been appended (t < T), those >= Tc are simply masked
             uint32_t ul = (blk * 128 + tid < p.max_tokens) ? ulen[blk * 128 + tid] : 0;
             uint32_t us = blkoff[blk] + row_ustart_128(ul, scan, tid);
-            float scale = valid ? f16_bits_to_f32(norm[t]) * p.inv_A : 0.0f;
-            if (role == 0) {
-                float dot[ATT_MAXG];
+            const float scale = valid ? f16_bits_to_f32(norm[t]) * p.inv_A : 0.0f;
+            // ---- decode the token's codes into its byte row
+            if (valid) {
+                decode_token<LAT>(rem, (uint32_t)(t * p.rbits), una, us, ul, d, p.k0, p.k1, lut_a, scr_a,
+                                  [&](int b, const int* c) {
+                                      if (LAT == LAT_E8) {
+                                          uint32_t w0 = 0, w1 = 0;
 #pragma unroll
-                for (int g = 0; g < ATT_MAXG; ++g) dot[g] = 0.0f;
-                if (valid) {
-                    decode_token<LAT>(rem, (uint32_t)(t * p.rbits), una, us, ul, d, p.k0, p.k1, lut_a, scr_a,
-                                            [&](int b, const int* c) {
-                                                float U[LAT];
-                                                if (p.dither) dither_block<LAT>(p.seed, (uint32_t)b, (uint32_t)t, (uint32_t)h, 0u, U);
+                                          for (int e = 0; e < 4; ++e) {
+                                              w0 |= (uint32_t)(uint8_t)(int8_t)c[e] << (8 * e);
+                                              w1 |= (uint32_t)(uint8_t)(int8_t)c[4 + e] << (8 * e);
+                                          }
+                                          *(uint32_t*)(crow + b * 8) = w0;
+                                          *(uint32_t*)(crow + b * 8 + 4) = w1;
+                                      } else {
 #pragma unroll
-                                                for (int e = 0; e < LAT; ++e) {
-                                                    float v = (float)c[e];
-                                                    if (LAT == LAT_A2 && e == 0) v *= HQ_S3;
-                                                    if (p.dither) v -= U[e];
+                                          for (int e = 0; e < LAT; ++e) crow[b * LAT + e] = (uint8_t)(int8_t)c[e];
+                                      }
+                                  });
+            }
+            float dot[GP];
 #pragma unroll
-                                                    for (int g = 0; g < ATT_MAXG; ++g)
-                                                        if (g < G) dot[g] += qs[g * d + b * LAT + e] * v;
-                                                }
-                                            });
+            for (int g = 0; g < GP; ++g) dot[g] = 0.0f;
+            float* row = vt + tid * (d + 1);
+            // ---- one loop over the lattice blocks: codes - regenerated dither -> score terms (K) or the v' row (V)
+            if (valid) {
+                constexpr int BL = LAT == LAT_E8 ? 8 : 4;   // coordinates per iteration (a multiple of the lattice dimension)
+#pragma unroll 1
+                for (int j0 = 0; j0 < d; j0 += BL) {
+                    float v[BL];
+                    const uint32_t w0 = *(const uint32_t*)(crow + j0);
+                    const uint32_t w1 = BL == 8 ? *(const uint32_t*)(crow + j0 + 4) : 0u;
+#pragma unroll
+                    for (int e = 0; e < BL; ++e) v[e] = (float)(int)(int8_t)((e < 4 ? w0 : w1) >> (8 * (e & 3)));
+                    if (LAT == LAT_A2) { v[0] *= HQ_S3; v[2] *= HQ_S3; }
+                    if (p.dither) {
+#pragma unroll
+                        for (int sb = 0; sb < BL / LAT; ++sb) {
+                            float U[LAT];
+                            if (LAT == LAT_E8) dither_e8_fast(rk, (uint32_t)(j0 / LAT + sb), (uint32_t)t, (uint32_t)h | ((uint32_t)role << 16), U);
+                            else dither_block<LAT>(p.seed, (uint32_t)(j0 / LAT + sb), (uint32_t)t, (uint32_t)h, (uint32_t)role, U);
+#pragma unroll
+                            for (int e = 0; e < LAT; ++e) v[sb * LAT + e] -= U[e];
+                        }
+                    }
+                    if (role == 0) {
+#pragma unroll
+                        for (int e = 0; e < BL; ++e) {
+#pragma unroll
+                            for (int g4 = 0; g4 < GP; g4 += 4) {
+                                const float4 q4 = *(const float4*)(qs + (j0 + e) * GP + g4);
+                                dot[g4 + 0] += q4.x * v[e]; dot[g4 + 1] += q4.y * v[e];
+                                dot[g4 + 2] += q4.z * v[e]; dot[g4 + 3] += q4.w * v[e];
+                            }
+                        }
+                    } else {
+#pragma unroll
+                        for (int e = 0; e < BL; ++e) row[j0 + e] = v[e] * scale;
+                    }
                 }
+            } else if (role == 1) {
+                for (int j = 0; j < d; ++j) row[j] = 0.0f;
+            }
+            if (role == 0) {
                 // scores, block max, p
 #pragma unroll
-                for (int g = 0; g < ATT_MAXG; ++g) {
-                    if (g >= G) break;
-                    float s = valid ? dot[g] * scale * p.inv_sqrt_d : -INFINITY;
+                for (int g = 0; g < GP; ++g) {
+                    float s = (valid && g < G) ? dot[g] * scale * p.inv_sqrt_d : -INFINITY;
                     float mx = s;
                     for (int o = 16; o; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
                     if (lane == 0) red[g * 4 + warp] = mx;
@@ -201,48 +332,36 @@ k_attend_split(AttendParams p) {
                 }
                 __syncthreads();
 #pragma unroll
-                for (int g = 0; g < ATT_MAXG; ++g) {
-                    if (g >= G) break;
+                for (int g = 0; g < GP; ++g) {
                     float mb = fmaxf(fmaxf(red[g * 4], red[g * 4 + 1]), fmaxf(red[g * 4 + 2], red[g * 4 + 3]));
                     float m_new = fmaxf(m_run[g], mb);
                     float corr = (m_run[g] == -INFINITY) ? 0.0f : __expf(m_run[g] - m_new);
-                    float pe = valid ? __expf(pg[g] - m_new) : 0.0f;
-                    ps[g * 128 + tid] = pe;
+                    float pe = (valid && g < G) ? __expf(pg[g] - m_new) : 0.0f;
+                    ps[tid * GP + g] = pe;
                     // every thread keeps the same running stats; l gets the block sum below
                     acc[g] *= corr; acc2[g] *= corr; l_run[g] *= corr; m_run[g] = m_new;
                 }
                 __syncthreads();
             } else {
-                // V: write v' rows to smem
-                float* row = vt + tid * (d + 1);
-                if (valid) {
-                    decode_token<LAT>(rem, (uint32_t)(t * p.rbits), una, us, ul, d, p.k0, p.k1, lut_a, scr_a,
-                                            [&](int b, const int* c) {
-                                                float U[LAT];
-                                                if (p.dither) dither_block<LAT>(p.seed, (uint32_t)b, (uint32_t)t, (uint32_t)h, 1u, U);
-#pragma unroll
-                                                for (int e = 0; e < LAT; ++e) {
-                                                    float v = (float)c[e];
-                                                    if (LAT == LAT_A2 && e == 0) v *= HQ_S3;
-                                                    if (p.dither) v -= U[e];
-                                                    row[b * LAT + e] = v * scale;
-                                                }
-                                            });
-                } else {
-                    for (int j = 0; j < d; ++j) row[j] = 0.0f;
-                }
                 __syncthreads();
+                // P V: thread j = coordinate; one pass over the block's tokens for all heads
                 for (int j = tid, jj = 0; j < d; j += 128, ++jj) {
+                    float a[GP], lsum[GP];
 #pragma unroll
-                    for (int g = 0; g < ATT_MAXG; ++g) {
-                        if (g >= G) break;
-                        float a = 0.0f, lsum = 0.0f;
-                        for (int tt = 0; tt < 128; ++tt) {
-                            float pe = ps[g * 128 + tt];
-                            a += pe * vt[tt * (d + 1) + j];
-                            lsum += pe;
+                    for (int g = 0; g < GP; ++g) { a[g] = 0.0f; lsum[g] = 0.0f; }
+#pragma unroll 4
+                    for (int tt = 0; tt < 128; ++tt) {
+                        const float vv = vt[tt * (d + 1) + j];
+#pragma unroll
+                        for (int g4 = 0; g4 < GP; g4 += 4) {
+                            const float4 p4 = *(const float4*)(ps + tt * GP + g4);
+                            a[g4 + 0] += p4.x * vv; a[g4 + 1] += p4.y * vv; a[g4 + 2] += p4.z * vv; a[g4 + 3] += p4.w * vv;
+                            lsum[g4 + 0] += p4.x; lsum[g4 + 1] += p4.y; lsum[g4 + 2] += p4.z; lsum[g4 + 3] += p4.w;
                         }
-                        if (jj == 0) { acc[g] += a; l_run[g] += lsum; } else acc2[g] += a;
+                    }
+#pragma unroll
+                    for (int g = 0; g < GP; ++g) {
+                        if (jj == 0) { acc[g] += a[g]; l_run[g] += lsum[g]; } else acc2[g] += a[g];
                     }
                 }
                 __syncthreads();
@@ -251,10 +370,13 @@ k_attend_split(AttendParams p) {
     }
     // write partials: [h][split][g][d + 2] = acc..., m, l   (threads with tid < d hold valid m/l)
     float* out = p.ws + ((int64_t)(h * p.n_split + split) * G) * (d + 2);
-    for (int g = 0; g < G; ++g) {
-        if (tid < d) out[g * (d + 2) + tid] = acc[g];
-        if (d > 128) out[g * (d + 2) + tid + 128] = acc2[g];
-        if (tid == 0) { out[g * (d + 2) + d] = m_run[g]; out[g * (d + 2) + d + 1] = l_run[g]; }
+#pragma unroll
+    for (int g = 0; g < GP; ++g) {
+        if (g < G) {
+            if (tid < d) out[g * (d + 2) + tid] = acc[g];
+            if (d > 128) out[g * (d + 2) + tid + 128] = acc2[g];
+            if (tid == 0) { out[g * (d + 2) + d] = m_run[g]; out[g * (d + 2) + d + 1] = l_run[g]; }
+        }
     }
 }
 
@@ -341,7 +463,7 @@ static int attend_n_split(const hq_ctx* ctx, const hq_kv* kv) {
     int64_t window = kv->cfg.window;
     int64_t Tc = kv->n_tokens > window ? kv->n_tokens - window : 0;
     int64_t nblk = (Tc + 127) / 128;
-    int64_t want = (ctx->sm_count * 4) / kv->cfg.kv_heads;
+    int64_t want = (ctx->sm_count * 3) / kv->cfg.kv_heads;   // one wave of the 3 resident CTAs per SM
     if (want < 1) want = 1;
     int64_t ns = nblk < want ? nblk : want;
     return (int)(ns < 1 ? 1 : ns);
@@ -367,11 +489,17 @@ hq_status launch_attend(hq_ctx* ctx, const hq_kv* kv, const void* q, int q_heads
     p.inv_sqrt_d = (float)(1.0 / sqrt((double)d));
     p.seed = kv->cfg.codec.seed;
     p.q = (const __nv_bfloat16*)q; p.dsign = kv->dsign; p.ssign = kv->ssign; p.ws = kv->att_ws;
-    size_t smem = ((size_t)p.G * d + 128 * (size_t)(d + 1) + (size_t)p.G * 128 + (size_t)p.G * 4) * sizeof(float);
+    const int GP = p.G <= 4 ? 4 : 8;
+    size_t smem = ((size_t)GP * d + 128 * (size_t)(d + 1) + (size_t)GP * 128 + (size_t)GP * 4) * sizeof(float);
 #define HQ_AT(L)                                                                                                   \
     do {                                                                                                           \
-        HQ_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_attend_split<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
-        k_attend_split<L><<<H * p.n_split, 128, smem, st>>>(p);                                                    \
+        if (GP == 4) {                                                                                             \
+            HQ_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_attend_split<L, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+            k_attend_split<L, 4><<<H * p.n_split, 128, smem, st>>>(p);                                             \
+        } else {                                                                                                   \
+            HQ_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_attend_split<L, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+            k_attend_split<L, 8><<<H * p.n_split, 128, smem, st>>>(p);                                             \
+        }                                                                                                          \
     } while (0)
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     if (ctx->prof && p.Tc > 0) {
