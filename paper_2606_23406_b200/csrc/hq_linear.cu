@@ -12,6 +12,7 @@
 #include "hq_linear_large.cuh"
 #include "hq_e8_ceiling.cuh"
 #include "hq_gemv_e8.cuh"
+#include "hq_generic_fast.cuh"
 #include "hq_tc.cuh"
 
 namespace hq {
@@ -95,6 +96,9 @@ k_linear_generic(LinearParams p) {
     float* s_sx = (float*)(urows + 128 * (GEN_UCAP + 1));    // [NB]
     uint64_t* bar = (uint64_t*)(s_sx + NB);
     uint32_t* tmem_slot = (uint32_t*)(bar + 1);
+    uint32_t* lut_s = tmem_slot + 2;                         // [2][256] phase-1 table of the fast row decoders
+    uint32_t* scr = lut_s + 512;                             // [128][n/8 + 1] nibble words
+    for (int i = threadIdx.x; i < 512; i += 128) lut_s[i] = unary_lut_entry(i & 255, i >> 8);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int64_t n_bt = (p.B + NB - 1) / NB;
@@ -142,12 +146,22 @@ k_linear_generic(LinearParams p) {
         gather_u_words(sg.uarea, nw, lane, urow, GEN_UCAP);
         __syncwarp();
         if (r < p.m) {
-            WordsRowU uw{urow, sg.uarea, sg.ulen, nw, GEN_UCAP, lane};
-            WordsRowR rw{sg.rarea, lane, rw_words};
-            decode_row_generic<LAT>(rw, 0u, uw, 0u, n, p.k0, p.k1, [&](int bk, const int* c) {
-#pragma unroll
-                for (int e = 0; e < LAT; ++e) sA[sw128_offset(128, tid, bk * LAT + e)] = (uint8_t)(int8_t)c[e];
+            // fast row decoder (hq_generic_fast.cuh): codes four per word, natural coordinate order, into the swizzled A tile
+            for (uint32_t i = nw; i < GEN_UCAP; ++i) urow[i] = 0u;
+            const uint32_t row_a = smem_u32(sA) + (uint32_t)((tid >> 3) * 1024 + (tid & 7) * 128);
+            const bool ok = decode_row_fast<LAT>(urow, GEN_UCAP, ul, sg.rarea, lane, n, p.k0, p.k1, smem_u32(lut_s),
+                                                 smem_u32(scr + tid * (n / 8 + 1)), [&](int wi, uint32_t v) {
+                const int col = 4 * wi;
+                sts32(row_a + (uint32_t)((col >> 7) * 128 * 128) + (uint32_t)(((((col & 127) >> 4) ^ (tid & 7)) << 4) | (col & 15)), v);
             });
+            if (!ok) {   // a quotient >= 16, a long row, k > 3, D4 at tile 64: the clz walker
+                WordsRowU uw{urow, sg.uarea, sg.ulen, nw, GEN_UCAP, lane};
+                WordsRowR rw{sg.rarea, lane, rw_words};
+                decode_row_generic<LAT>(rw, 0u, uw, 0u, n, p.k0, p.k1, [&](int bk, const int* c) {
+#pragma unroll
+                    for (int e = 0; e < LAT; ++e) sA[sw128_offset(128, tid, bk * LAT + e)] = (uint8_t)(int8_t)c[e];
+                });
+            }
         } else {
             for (int j = 0; j < n; j += 16) *(uint4*)(sA + sw128_offset(128, tid, j)) = make_uint4(0, 0, 0, 0);
         }
@@ -221,7 +235,7 @@ static hq_status launch_generic_nb(hq_ctx* ctx, const hq_weight* w, LinearParams
     int64_t n_bt = (p.B + NB - 1) / NB;
     int64_t grid = w->n_rb * n_bt * p.n_split;
     size_t smem = 1024 + (size_t)n_atoms * 128 * 128 + (size_t)n_atoms * NB * 128 + 128 * (size_t)(GEN_UCAP + 1) * 4 +
-                  NB * 4 + 16 + 8 + 8;
+                  NB * 4 + 16 + 8 + 8 + 2048 + 128 * (size_t)(w->n / 8 + 1) * 4;
 #define HQ_L(L)                                                                                                   \
     do {                                                                                                          \
         HQ_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_linear_generic<L, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
