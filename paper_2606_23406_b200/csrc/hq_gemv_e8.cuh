@@ -365,7 +365,11 @@ k_gemv_e8(E8Params p) {
         for (int kt = ka; kt < kb; ++kt) {
             const bool has1 = kt + 1 < kb, has2 = kt + 2 < kb;
             const uint32_t off_n2 = has2 ? __ldg(soff + (kt + 2 - ka) * 4) : 0u;
-            if (need_act) mbar_wait(bar_lut, 0u);
+            if (need_act) {   // first tile of the kernel: the activation operand, while the tile's words are still in flight
+                act_prologue();   // (all warps of the CTA meet here)
+                need_act = false;
+                mbar_wait(bar_lut, 0u);
+            }
 
             // ---- phase 1: unary section -> nibble words (A4)
             const uint32_t nw = (ul_c + 31) >> 5;
@@ -391,10 +395,6 @@ k_gemv_e8(E8Params p) {
             const uint8_t* sgp_n = blob + 16 * (size_t)off_n1;
             if (has1) load_hdr_dense(sgp_n, ul_n, nrm_n);
 
-            if (need_act) {   // first tile of the kernel: the activation operand (all warps of the CTA meet here)
-                act_prologue();
-                need_act = false;
-            }
             // ---- this warp's MMAs of the previous tile: issued a whole phase 1 ago, so this wait rarely spins
             if (kt > ka) {
                 mbar_wait(bar_w, (n_mma - 1) & 1u);
