@@ -271,6 +271,8 @@ def main():
     ap.add_argument("--layers", type=int, default=4)
     ap.add_argument("--impl", default="ours")
     ap.add_argument("--skip-extras", action="store_true")
+    ap.add_argument("--only", choices=("decode_ceiling", "large_m", "attend", "config3"), default=None,
+                    help="run one secondary measurement alone and print its JSON (the command the ncu captures under profiles/ name)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -287,6 +289,20 @@ def main():
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
     ctx = hq.Context(local)
+
+    if args.only:
+        if args.only == "decode_ceiling":
+            W = torch.from_numpy(hq_synth.llama_weight(0, "q")).to(dev).to(torch.bfloat16)
+            w = ctx.encode_weights(W, hq.Lattice.E8, 128, SNR_E8_4BPS, seed=0)
+            out = {"scalars_per_s": [w.decode_ceiling(200) for _ in range(3)]}
+        elif args.only == "large_m":
+            out = measure_large_m(ctx, hq, dev, reps=3)
+        elif args.only == "attend":
+            out = measure_attend(ctx, hq, dev, peaks()[0])
+        else:
+            out = measure_config3(ctx, hq, dev)
+        print(json.dumps({"only": args.only, "result": out}))
+        return
 
     # ---- build the workload (untimed): L layers x 7 compressed matrices, replicas on every rank
     layers, alg_bytes = [], []

@@ -180,8 +180,15 @@ hq_status hq_act_quant(hq_ctx* ctx, const hq_weight* w, const void* x_dev, int32
  * acc[kt,b,r] = sum_{i in tile kt} c[r,i] * q[b,i]  (INT32, tcgen05.mma kind::i8).
  * x [batch, n_in] dev (ldx), y [batch, m_out] bf16 dev (ldy).  Optional debug outputs (dev, may be
  * NULL): y_f32 [batch, m_out] (the value before the bf16 cast), acc_i32 [n_kt, batch, m_out].
- * The decoded weights exist only in shared memory.  Any batch >= 1 (x is processed in tiles of 16 or 64 rows).
- * E8 / tile 128 / k <= 3 runs the SWAR kernel with the split-K reduction inside; everything else the generic kernel.
+ * Where the decoded weights live (north_star (d)):
+ *   batch 1, E8 / tile 128 / k <= 3 (k_gemv_e8): registers -> tensor memory (tcgen05.st) -> MMA A operand; never in
+ *     shared or global memory.  The kernel also does the activation RHT + INT8 cast itself: one launch per call.
+ *   batch 2..63 (k_linear_e8) and every other lattice / tile (k_linear_generic): a shared-memory operand tile.
+ *   batch >= 64, E8 at tile 128 or 256 (large-M path): decoded ONCE per call into a scratch copy in operand layout in
+ *     the context's workspace (global memory, L2 resident: 69 MB for a 16384 x 4096 weight), streamed by TMA into a
+ *     warp-specialised tcgen05 GEMM.  This is the one place decoded weights leave the SM (DESIGN.md §6.4 says why).
+ * Any batch >= 1.  Limits of the fused kernels (HQ_ERR_SHAPE beyond them): n_in / n_tile < 4096, m_out < 8388608,
+ * ceil(m_out / 128) * (n_in / n_tile) < 2^31.
  */
 hq_status hq_linear(hq_ctx* ctx, const hq_weight* w, const void* x_dev, int32_t dtype, int64_t batch,
                     int64_t ldx, void* y_bf16_dev, int64_t ldy, float* y_f32_dev_or_null,

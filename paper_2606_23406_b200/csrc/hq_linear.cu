@@ -3,7 +3,8 @@
 // un-strip to INT8 lattice points (A5, §4.6), stage them in shared memory in the UMMA
 // K-major SWIZZLE_128B layout and contract with the INT8 activations on the tensor core
 // (A6, tcgen05.mma kind::i8 -> INT32 in TMEM, §4.8), then rescale per K-tile and accumulate (A7,
-// §4.3).  Decoded weights never leave shared memory.
+// §4.3).  Decoded weights stay on the SM (tensor memory at batch 1, shared memory up to 63 rows); the large-M path
+// (from 64 rows) decodes once per call into an operand-layout scratch copy (hq_linear_large.cuh).
 #include <string.h>
 
 #include "hq_common.cuh"
