@@ -27,6 +27,14 @@
 
 namespace hq {
 
+#ifdef HQ_TRACE   // phase timestamps per warp (a probe build only: never defined by build.py)
+__device__ unsigned long long g_gv_trace[8 * 148 * 32 * 12];   // slot (n_items >> 9) & 7: the four launches of the bench step differ
+__device__ __forceinline__ unsigned long long gv_now() { unsigned long long v; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(v)); return v; }
+#define GV_TR(i) do { if (lane == 0) g_gv_trace[((size_t)((p.n_items >> 9) & 7) * 148 * 32 + (size_t)blockIdx.x * 32 + wid) * 12 + (i)] = gv_now(); } while (0)
+#else
+#define GV_TR(i) do { } while (0)
+#endif
+
 constexpr int GV_TCOLS_WG = 48;   // TMEM columns per warp group: A tile (32: 128 INT8 per lane) + accumulator (16)
 constexpr int GV_MAX_KT = 128;    // n_in <= 16384: the whole activation operand stays in shared memory
 constexpr int GV_STAGE_WORDS = E8_NW + 12;   // per row: the next tile's U words and R words (K <= 3), staged by cp.async
@@ -149,69 +157,125 @@ __device__ __noinline__ float gv_segment_fallback(const uint8_t* blob, const uin
     return corr;
 }
 
-// A1-A2: the activation vector through the RHT and the INT8 cast, one warp per tile of 128 (FORMAT R1, R7), into the
-// shared operand (row kt of a K-major SWIZZLE_128B tile = the INT8 codes of K-tile kt, K order of e8_kcol) and s_x[kt].
-// Executed by every warp of the CTA once, after the first tile's weight-only work; ends with a block barrier.
-template <int NW>
-__device__ __noinline__ void gv_act_prologue(const void* xp, int dtype, const int8_t* dsign, int n_kt, uint32_t xq_a,
-                                             uint32_t sx_a, int wid, int lane) {
-    // x, the partial sums and the debug outputs belong to the stream order: join it here (no-op without PDL)
-    griddep_wait();
-    constexpr int MAXT = (GV_MAX_KT + NW - 1) / NW;   // tiles per warp: all their loads are issued before any arithmetic
-    const bool vec = dtype == HQ_BF16 ? (((uintptr_t)xp) & 7) == 0 : (((uintptr_t)xp) & 15) == 0;
-    const int col0 = act_col0(lane);
-    float x[MAXT][4];
-    uint32_t sg[MAXT];
-    bool on[MAXT];
+// The bitstream words of a tile travel global -> shared by cp.async (no register is held while they fly): U word i of
+// this lane's row at stg_a + i * 128, R word j at stg_a + (E8_NW + j) * 128.  Absent words are stored as zero.
+template <int KW>
+__device__ __forceinline__ void gv_load_hdr_dense(const uint8_t* sgp, int lane, bool dense, uint32_t stg_a, uint32_t& ul, uint32_t& nrm) {
+    ul = __ldg((const uint16_t*)sgp + lane);
+    nrm = __ldg((const uint16_t*)sgp + 32 + lane);
+    if (dense) {
+        const uint32_t* ua = (const uint32_t*)(sgp + 128) + KW * 32 + lane;
 #pragma unroll
-    for (int i = 0; i < MAXT; ++i) {
-        const int kt = wid + i * NW;
-        on[i] = kt < n_kt;   // warp-uniform
-#pragma unroll
-        for (int j = 0; j < 4; ++j) x[i][j] = 0.0f;
-        sg[i] = 0u;
-        if (on[i]) {
-            const int64_t base = (int64_t)kt * 128 + 4 * lane;
-            if (vec && dtype == HQ_BF16) {
-                const uint2 v = __ldg((const uint2*)((const __nv_bfloat16*)xp + base));
-                x[i][0] = __uint_as_float(v.x << 16); x[i][1] = __uint_as_float(v.x & 0xffff0000u);
-                x[i][2] = __uint_as_float(v.y << 16); x[i][3] = __uint_as_float(v.y & 0xffff0000u);
-            } else if (vec) {
-                const float4 v = __ldg((const float4*)((const float*)xp + base));
-                x[i][0] = v.x; x[i][1] = v.y; x[i][2] = v.z; x[i][3] = v.w;
-            } else {
-#pragma unroll
-                for (int j = 0; j < 4; ++j)
-                    x[i][j] = dtype == HQ_BF16 ? __bfloat162float(((const __nv_bfloat16*)xp)[base + j]) : ((const float*)xp)[base + j];
-            }
-            sg[i] = __ldg((const uint32_t*)(dsign + kt * 128) + lane);
-        }
+        for (int i = 0; i < E8_DENSE; ++i) cp_async4(stg_a + i * 128, ua + i * 32);
     }
+}
+template <int KW>
+__device__ __forceinline__ void gv_load_r(const uint8_t* sgp, int lane, uint32_t stg_a) {
+    const uint32_t* rarea = (const uint32_t*)(sgp + 128);
 #pragma unroll
-    for (int i = 0; i < MAXT; ++i)
+    for (int j = 0; j < KW; ++j) cp_async4(stg_a + (E8_NW + j) * 128, rarea + j * 32 + lane);
+}
+template <int KW>
+__device__ __forceinline__ void gv_load_ragged(const uint8_t* sgp, int lane, bool dense, uint32_t stg_a, uint32_t ul) {
+    const uint32_t* uarea = (const uint32_t*)(sgp + 128) + KW * 32;
+    const uint32_t nw = (ul + 31) >> 5;
+    const uint32_t lane_lt = (1u << lane) - 1u;
+    uint32_t base = dense ? E8_DENSE * 32 : 0;
+#pragma unroll
+    for (int i = 0; i < E8_NW; ++i) {
+        if (i < E8_DENSE && dense) continue;
+        const bool has = nw > (uint32_t)i;
+        const uint32_t mk = __ballot_sync(0xffffffffu, has);
+        if (has) cp_async4(stg_a + i * 128, uarea + base + __popc(mk & lane_lt));
+        else sts32(stg_a + i * 128, 0u);
+        base += __popc(mk);
+    }
+}
+
+__device__ __forceinline__ void gv_load_x(const void* xp, int dtype, bool vec, const int8_t* dsign, int kt, int lane, float* x, uint32_t& sg) {
+    const int64_t base = (int64_t)kt * 128 + 4 * lane;
+    if (vec && dtype == HQ_BF16) {
+        const uint2 v = __ldg((const uint2*)((const __nv_bfloat16*)xp + base));
+        x[0] = __uint_as_float(v.x << 16); x[1] = __uint_as_float(v.x & 0xffff0000u);
+        x[2] = __uint_as_float(v.y << 16); x[3] = __uint_as_float(v.y & 0xffff0000u);
+    } else if (vec) {
+        const float4 v = __ldg((const float4*)((const float*)xp + base));
+        x[0] = v.x; x[1] = v.y; x[2] = v.z; x[3] = v.w;
+    } else {
 #pragma unroll
         for (int j = 0; j < 4; ++j)
-            if ((sg[i] >> (8 * j)) & 0x80u) x[i][j] = -x[i][j];
-    int qv[MAXT][4];
-    float sx[MAXT];
-    warp_act_tiles128<MAXT>(x, on, lane, qv, sx);   // all of the warp's tiles stage by stage: the latency of one
-#pragma unroll
-    for (int i = 0; i < MAXT; ++i) {
-        const int kt = wid + i * NW;
-        if (on[i]) {
-            const uint32_t row_a = xq_a + (uint32_t)((kt >> 3) * 1024 + (kt & 7) * 128);
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                const int col = col0 + 4 * j;
-                sts8(row_a + ((((col >> 4) ^ (kt & 7)) << 4) | (col & 15)), (uint32_t)(uint8_t)(int8_t)qv[i][j]);
-            }
-            if (lane == 0) asm volatile("st.shared.f32 [%0], %1;" ::"r"(sx_a + kt * 4), "f"(sx[i]) : "memory");
-        }
+            x[j] = dtype == HQ_BF16 ? __bfloat162float(((const __nv_bfloat16*)xp)[base + j]) : ((const float*)xp)[base + j];
     }
-    // rows of the last 8-row groups that no K-tile fills: zero (their accumulator columns are never read)
-    for (int r = n_kt + wid; r < ((n_kt + 7) / 8 + 1) * 8; r += NW)
-        asm volatile("st.shared.u32 [%0], %1;" ::"r"(xq_a + (uint32_t)(r * 128 + lane * 4)), "r"(0u) : "memory");
+    sg = __ldg((const uint32_t*)(dsign + kt * 128) + lane);
+}
+
+// The start of a CTA, one call per warp (noinline: none of its registers count against the tile loop):
+//  * the loads of the warp's first tile, a chain of three dependent global reads (sub-group offset -> header -> ragged U
+//    words), interleaved with
+//  * A1-A2: the activation tiles the CTA's tile range touches - K-tiles kt0 + j (mod n_kt), j < nt, one warp per tile -
+//    through the RHT and the INT8 cast (FORMAT R1, R7) into the shared operand (row kt of a K-major SWIZZLE_128B tile =
+//    the INT8 codes of K-tile kt, K order of e8_kcol) and s_x[kt]; the FWHT runs while the weight loads are in flight.
+// x belongs to the stream order (griddepcontrol.wait comes before its first load); the weights do not.
+// Ends with a block barrier.  Leaves ulen, norm bits and the next tile's offset of the warp's first tile at ret_a.
+template <int K, int NW>
+__device__ __noinline__ void gv_first_prologue(const void* xp, int dtype, const int8_t* dsign, int n_kt, uint32_t xq_a,
+                                               uint32_t sx_a, int wid, int lane, int kt0, int nt, const uint8_t* blob,
+                                               const uint32_t* soff, int has, int dense_i, uint32_t stg_a, uint32_t ret_a
+#ifdef HQ_TRACE
+                                               , int tr_slot
+#endif
+) {
+    constexpr int KW = 4 * K;
+    const bool dense = dense_i != 0;
+    uint32_t off0 = 0, off1 = 0;
+    if (has) {
+        off0 = __ldg(soff);
+        if (has > 1) off1 = __ldg(soff + 4);
+    }
+    griddep_wait();
+#ifdef HQ_TRACE
+    if (lane == 0) g_gv_trace[((size_t)tr_slot * 148 * 32 + (size_t)blockIdx.x * 32 + wid) * 12 + 9] = gv_now();
+#endif
+    const bool vec = dtype == HQ_BF16 ? (((uintptr_t)xp) & 7) == 0 : (((uintptr_t)xp) & 15) == 0;
+    const int col0 = act_col0(lane);
+    float x[4], xn[4];
+    uint32_t sg = 0, sgn = 0;
+    auto tile_of = [&](int j) { const int kt = kt0 + j; return kt >= n_kt ? kt - n_kt : kt; };
+    int j = wid;
+    if (j < nt) gv_load_x(xp, dtype, vec, dsign, tile_of(j), lane, xn, sgn);
+    uint32_t ul = 0, nrm = 0;
+    const uint8_t* sgp = blob + 16 * (size_t)off0;
+    if (has) {
+        gv_load_hdr_dense<KW>(sgp, lane, dense, stg_a, ul, nrm);
+        gv_load_r<KW>(sgp, lane, stg_a);
+    }
+    bool ragged_due = has != 0;
+#pragma unroll 1
+    for (; j < nt; j += NW) {
+        const int kt = tile_of(j);
+#pragma unroll
+        for (int e = 0; e < 4; ++e) x[e] = (sgn >> (8 * e)) & 0x80u ? -xn[e] : xn[e];
+        if (j + NW < nt) gv_load_x(xp, dtype, vec, dsign, tile_of(j + NW), lane, xn, sgn);
+        int qv[4];
+        const float sx = warp_act_tile128(x, lane, qv);
+        if (ragged_due) {   // the header has arrived behind the FWHT
+            gv_load_ragged<KW>(sgp, lane, dense, stg_a, ul);
+            ragged_due = false;
+        }
+        const uint32_t row_a = xq_a + (uint32_t)((kt >> 3) * 1024 + (kt & 7) * 128);
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            const int col = col0 + 4 * e;
+            sts8(row_a + ((((col >> 4) ^ (kt & 7)) << 4) | (col & 15)), (uint32_t)(uint8_t)(int8_t)qv[e]);
+        }
+        if (lane == 0) asm volatile("st.shared.f32 [%0], %1;" ::"r"(sx_a + kt * 4), "f"(sx) : "memory");
+    }
+    if (ragged_due) gv_load_ragged<KW>(sgp, lane, dense, stg_a, ul);
+    sts32(ret_a, ul); sts32(ret_a + 4, nrm); sts32(ret_a + 8, off1); sts32(ret_a + 12, off0);
     fence_proxy_async_smem();   // the operand is read by the tensor core (async proxy)
+#ifdef HQ_TRACE
+    if (lane == 0) g_gv_trace[((size_t)tr_slot * 148 * 32 + (size_t)blockIdx.x * 32 + wid) * 12 + 10] = gv_now();
+#endif
     __syncthreads();
 }
 
@@ -233,6 +297,7 @@ k_gemv_e8(E8Params p) {
     // the warp index through a shuffle: the compiler then knows it is warp-uniform (descriptors stay in uniform registers)
     const int wid = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
     const int tid = threadIdx.x, wg = wid >> 2, warp = wid & 3, lane = tid & 31, t = warp * 32 + lane;
+    GV_TR(0);
     const uint32_t smem_a = smem_u32(smem);
     const uint32_t xq_a = smem_a + E8_LUT_BYTES;                                  // activation operand, 1024-aligned
     const uint32_t XQB = gv_xq_bytes(p.n_kt);
@@ -256,6 +321,7 @@ k_gemv_e8(E8Params p) {
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
+    GV_TR(1);
     griddep_launch();
     if (tid == 0) {  // the phase-1 table arrives by one TMA bulk copy while the first loads are in flight
         mbar_arrive_expect_tx(bar_lut, E8_LUT_BYTES);
@@ -269,7 +335,6 @@ k_gemv_e8(E8Params p) {
     const uint32_t dm0 = warp == 0 ? 0u : 0xffffffffu, dm1 = warp == 1 ? 0u : 0xffffffffu,
                    dm2 = warp == 2 ? 0u : 0xffffffffu, dm3 = warp == 3 ? 0u : 0xffffffffu;   // lanes this warp does NOT write
     const uint32_t lut_lane = smem_a + (uint32_t)(lane & (E8_LUT_COPIES - 1)) * 4;
-    const uint32_t lane_lt = (1u << lane) - 1u;
     const int n_kt = p.n_kt;
 
     // ---- this warp group's flat tile range
@@ -279,17 +344,24 @@ k_gemv_e8(E8Params p) {
     int f = f_begin;
     auto wg_of_tile = [&](int64_t ft) -> int { return (int)(((ft + 1) * GWG - 1) / T); };   // the warp group whose range holds tile ft
 
-    auto act_prologue = [&]() { gv_act_prologue<NW>(p.x, p.dtype, p.dsign, n_kt, xq_a, sx_a, wid, lane); };
+    // the K-tiles this CTA's tile range touches: kt0 + j (mod n_kt), j < nt_cta - the only activation tiles it quantizes
+    const int64_t cta_b = ((int64_t)blockIdx.x * NWG * T) / GWG, cta_e = ((int64_t)(blockIdx.x + 1) * NWG * T) / GWG;
+    const int nt_cta = (int)min((int64_t)n_kt, cta_e - cta_b), kt0_cta = (int)(cta_b % n_kt);
+#ifdef HQ_TRACE
+#define GV_TRARG , (p.n_items >> 9) & 7
+#else
+#define GV_TRARG
+#endif
 
     if (f >= f_end) {   // nothing to do for this warp group: it still helps with the activations and joins the barriers
-        act_prologue();
+        gv_first_prologue<K, NW>(p.x, p.dtype, p.dsign, n_kt, xq_a, sx_a, wid, lane, kt0_cta, nt_cta, nullptr, nullptr, 0, 0, stg_a, scr_a GV_TRARG);
         tc_fence_before();
         __syncthreads();
         if (wid == 0) tmem_dealloc(*tmem_slot, 512);
         return;
     }
     asm volatile("st.shared.v4.u32 [%0], {%1,%1,%1,%1};" ::"r"(mask_a), "r"(0u) : "memory");
-    bool need_act = true;
+    bool first_seg = true;
     uint32_t n_mma = 0;    // commits of this warp so far: the barrier's phase
     float yacc = 0.0f;
 
@@ -311,36 +383,9 @@ k_gemv_e8(E8Params p) {
         const uint32_t* soff = p.sub_off[w] + (((size_t)rbl * n_kt + ka) * 4 + warp);   // this warp's sub-group of tile ka; +4 per tile
         const float inv_A = p.inv_A[w];
 
-        // The bitstream words of a tile travel global -> shared by cp.async (no register is held while they fly): U word i of
-        // this lane's row at stg_a + i * 128, R word j at stg_a + (E8_NW + j) * 128.  Absent words are stored as zero.
-        auto load_hdr_dense = [&](const uint8_t* sgp, uint32_t& ul, uint32_t& nrm) {
-            ul = __ldg((const uint16_t*)sgp + lane);
-            nrm = __ldg((const uint16_t*)sgp + 32 + lane);
-            if (dense) {
-                const uint32_t* ua = (const uint32_t*)(sgp + 128) + KW * 32 + lane;
-#pragma unroll
-                for (int i = 0; i < E8_DENSE; ++i) cp_async4(stg_a + i * 128, ua + i * 32);
-            }
-        };
-        auto load_r = [&](const uint8_t* sgp) {
-            const uint32_t* rarea = (const uint32_t*)(sgp + 128);
-#pragma unroll
-            for (int j = 0; j < KW; ++j) cp_async4(stg_a + (E8_NW + j) * 128, rarea + j * 32 + lane);
-        };
-        auto load_ragged = [&](const uint8_t* sgp, uint32_t ul) {
-            const uint32_t* uarea = (const uint32_t*)(sgp + 128) + KW * 32;
-            const uint32_t nw = (ul + 31) >> 5;
-            uint32_t base = dense ? E8_DENSE * 32 : 0;
-#pragma unroll
-            for (int i = 0; i < E8_NW; ++i) {
-                if (i < E8_DENSE && dense) continue;
-                const bool has = nw > (uint32_t)i;
-                const uint32_t mk = __ballot_sync(0xffffffffu, has);
-                if (has) cp_async4(stg_a + i * 128, uarea + base + __popc(mk & lane_lt));
-                else sts32(stg_a + i * 128, 0u);
-                base += __popc(mk);
-            }
-        };
+        auto load_hdr_dense = [&](const uint8_t* sgp, uint32_t& ul, uint32_t& nrm) { gv_load_hdr_dense<KW>(sgp, lane, dense, stg_a, ul, nrm); };
+        auto load_r = [&](const uint8_t* sgp) { gv_load_r<KW>(sgp, lane, stg_a); };
+        auto load_ragged = [&](const uint8_t* sgp, uint32_t ul) { gv_load_ragged<KW>(sgp, lane, dense, stg_a, ul); };
         // epilogue of K-tile kt (this warp's MMAs on it have completed): drain the accumulator lane, rescale, accumulate (A7)
         auto epilogue = [&](int kt, float sw, bool ovr) {
             uint32_t v;
@@ -354,23 +399,34 @@ k_gemv_e8(E8Params p) {
 
         uint32_t ul_c, nrm_c, ul_n = 0, nrm_n = 0;
         // segment prologue: offsets of its first two tiles, then everything of the first tile
-        uint32_t off_n1 = (ka + 1 < kb) ? __ldg(soff + 4) : 0u;
-        const uint8_t* sgp_c = blob + 16 * (size_t)__ldg(soff);
-        load_hdr_dense(sgp_c, ul_c, nrm_c);
-        load_r(sgp_c);
-        load_ragged(sgp_c, ul_c);
+        uint32_t off_n1;
+        const uint8_t* sgp_c;
+        if (first_seg) {   // the kernel's first tile: its loads are interleaved with the activation prologue (all warps meet there)
+            GV_TR(2);
+            gv_first_prologue<K, NW>(p.x, p.dtype, p.dsign, n_kt, xq_a, sx_a, wid, lane, kt0_cta, nt_cta, blob, soff,
+                                     (ka + 1 < kb) ? 2 : 1, dense ? 1 : 0, stg_a, scr_a GV_TRARG);
+            first_seg = false;
+            GV_TR(3);
+            ul_c = lds32(scr_a); nrm_c = lds32(scr_a + 4); off_n1 = lds32(scr_a + 8);
+            sgp_c = blob + 16 * (size_t)lds32(scr_a + 12);
+            mbar_wait(bar_lut, 0u);
+#ifdef HQ_TRACE
+            cp_async_wait_all();
+            GV_TR(4);
+#endif
+        } else {
+            off_n1 = (ka + 1 < kb) ? __ldg(soff + 4) : 0u;
+            sgp_c = blob + 16 * (size_t)__ldg(soff);
+            load_hdr_dense(sgp_c, ul_c, nrm_c);
+            load_r(sgp_c);
+            load_ragged(sgp_c, ul_c);
+        }
         float sw_prev = 0.0f;
         bool ovr_prev = false, seg_flagged = false;
 
         for (int kt = ka; kt < kb; ++kt) {
             const bool has1 = kt + 1 < kb, has2 = kt + 2 < kb;
             const uint32_t off_n2 = has2 ? __ldg(soff + (kt + 2 - ka) * 4) : 0u;
-            if (need_act) {   // first tile of the kernel: the activation operand, while the tile's words are still in flight
-                act_prologue();   // (all warps of the CTA meet here)
-                need_act = false;
-                mbar_wait(bar_lut, 0u);
-            }
-
             // ---- phase 1: unary section -> nibble words (A4)
             const uint32_t nw = (ul_c + 31) >> 5;
             const uint32_t maxul = __reduce_max_sync(0xffffffffu, ul_c);   // longest U-section of the sub-group, bits
@@ -473,11 +529,13 @@ k_gemv_e8(E8Params p) {
         }
         yacc = 0.0f;
     }
+    GV_TR(5);
     // ---- split-K reduction inside the kernel: publish this thread's partial sums (one fence), then arrive once per cut
     // row block of the range on a per-(row block, warp) counter; the LAST of the row block's segments to arrive adds the
     // partials in slot order - deterministic - and writes y (A7).  No block barrier, no extra launch.
     __threadfence();
     __syncwarp();
+    GV_TR(6);
     for (int ff = f_begin; ff < f_end;) {
         const int rbg = ff / n_kt, ka = ff - rbg * n_kt;
         const int kb = min(n_kt, ka + (f_end - ff));
@@ -513,8 +571,10 @@ k_gemv_e8(E8Params p) {
         if (p.y_bf16[w]) p.y_bf16[w][r] = __float2bfloat16_rn(sum);
         if (p.y_f32[w]) p.y_f32[w][r] = sum;
     }
+    GV_TR(7);
     tc_fence_before();
     __syncthreads();
+    GV_TR(8);
     if (wid == 0) tmem_dealloc(*tmem_slot, 512);
 }
 

@@ -307,7 +307,15 @@ static hq_status launch_e8_v(hq_ctx* ctx, int k0, E8Params& p, const E8Plan& pl,
 }
 
 // batch 1: k_gemv_e8 (decoded rows through tensor memory, independent warps, activations quantized in-kernel)
-constexpr int GV_NWG = 5;   // measured: 4 .. 8 warp groups run the big launches within 5 %, 5 is the best whole layer
+// Warp groups per CTA: 5 or 4, whichever wastes fewer tile slots.  The flat partition gives every warp group floor or ceil
+// of T / (SMs x NWG) tiles and the launch ends with the slowest one, so its length is ~ ceil(T / (SMs x NWG)) x NWG
+// (a tile takes a warp NWG x as long when NWG groups share the SM's issue slots).
+constexpr int GV_NWG = 5;   // the largest: sizes the partial-sum slots
+static int gv_pick_nwg(const hq_ctx* ctx, int64_t T) {
+    const int64_t sm = ctx->sm_count;
+    const int64_t c5 = (T + sm * 5 - 1) / (sm * 5) * 5, c4 = (T + sm * 4 - 1) / (sm * 4) * 4;
+    return c4 < c5 ? 4 : 5;
+}
 template <int NWG>
 static hq_status launch_gemv(hq_ctx* ctx, int k0, E8Params& p, const E8Plan& pl, cudaStream_t st) {
     const size_t smem = gv_smem_bytes<NWG>(p.n_kt);
@@ -511,7 +519,7 @@ hq_status launch_linear_group(hq_ctx* ctx, const hq_weight* const* ws, int n_w, 
         HQ_CUDA_CHECK(ctx, cudaEventCreate(&e1));
         HQ_CUDA_CHECK(ctx, cudaEventRecord(e0, st));
     }
-    hq_status s = gemv        ? launch_gemv<GV_NWG>(ctx, w0->k0, p, pl, st)
+    hq_status s = gemv        ? (gv_pick_nwg(ctx, p.n_items) == 4 ? launch_gemv<4>(ctx, w0->k0, p, pl, st) : launch_gemv<5>(ctx, w0->k0, p, pl, st))
                   : (B == 1)  ? launch_e8_v<16, 1, 6, 1>(ctx, w0->k0, p, pl, st)
                   : (B <= 16) ? launch_e8_v<16, 16, 5, 1>(ctx, w0->k0, p, pl, st)
                               : launch_e8_v<64, 64, 3, 1>(ctx, w0->k0, p, pl, st);
@@ -597,3 +605,10 @@ hq_status launch_linear(hq_ctx* ctx, const hq_weight* w, const void* x, int dtyp
 }
 
 }  // namespace hq
+
+#ifdef HQ_TRACE
+extern "C" int hq_debug_trace(unsigned long long* host_out, long long n_words) {
+    cudaDeviceSynchronize();
+    return (int)cudaMemcpyFromSymbol(host_out, hq::g_gv_trace, (size_t)n_words * 8);
+}
+#endif
