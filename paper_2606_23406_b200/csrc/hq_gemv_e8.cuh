@@ -175,21 +175,30 @@ __device__ __forceinline__ void gv_load_r(const uint8_t* sgp, int lane, uint32_t
 #pragma unroll
     for (int j = 0; j < KW; ++j) cp_async4(stg_a + (E8_NW + j) * 128, rarea + j * 32 + lane);
 }
-template <int KW>
-__device__ __forceinline__ void gv_load_ragged(const uint8_t* sgp, int lane, bool dense, uint32_t stg_a, uint32_t ul) {
-    const uint32_t* uarea = (const uint32_t*)(sgp + 128) + KW * 32;
-    const uint32_t nw = (ul + 31) >> 5;
-    const uint32_t lane_lt = (1u << lane) - 1u;
-    uint32_t base = dense ? E8_DENSE * 32 : 0;
+// U words a row may or may not have (word i of the rows that have it are compacted, FORMAT §5): words [FIRST, E8_NW),
+// `base` = words of the word-rows below FIRST.  No branch: an absent word is a zero-fill copy.
+template <int FIRST>
+__device__ __forceinline__ void gv_load_ragged_from(const uint32_t* uarea, uint32_t base, uint32_t stg_a, uint32_t nw) {
+    const uint32_t lt = lanemask_lt();
 #pragma unroll
-    for (int i = 0; i < E8_NW; ++i) {
-        if (i < E8_DENSE && dense) continue;
+    for (int i = FIRST; i < E8_NW; ++i) {
         const bool has = nw > (uint32_t)i;
         const uint32_t mk = __ballot_sync(0xffffffffu, has);
-        if (has) cp_async4(stg_a + i * 128, uarea + base + __popc(mk & lane_lt));
-        else sts32(stg_a + i * 128, 0u);
+        cp_async4_zfill(stg_a + i * 128, uarea + base + __popc(mk & lt), has);
         base += __popc(mk);
     }
+}
+// a sub-group whose rows are not known to hold E8_DENSE words each (a row block's ragged edge, a low-rate stream): rare,
+// kept out of the tile loop's instruction footprint
+__device__ __noinline__ void gv_load_ragged_all(const uint32_t* uarea, uint32_t stg_a, uint32_t nw) {
+    gv_load_ragged_from<0>(uarea, 0u, stg_a, nw);
+}
+template <int KW>
+__device__ __forceinline__ void gv_load_ragged(const uint8_t* sgp, bool dense, uint32_t stg_a, uint32_t ul) {
+    const uint32_t* uarea = (const uint32_t*)(sgp + 128) + KW * 32;
+    const uint32_t nw = (ul + 31) >> 5;
+    if (dense) gv_load_ragged_from<E8_DENSE>(uarea, E8_DENSE * 32, stg_a, nw);
+    else gv_load_ragged_all(uarea, stg_a, nw);
 }
 
 __device__ __forceinline__ void gv_load_x(const void* xp, int dtype, bool vec, const int8_t* dsign, int kt, int lane, float* x, uint32_t& sg) {
@@ -259,7 +268,7 @@ __device__ __noinline__ void gv_first_prologue(const void* xp, int dtype, const 
         int qv[4];
         const float sx = warp_act_tile128(x, lane, qv);
         if (ragged_due) {   // the header has arrived behind the FWHT
-            gv_load_ragged<KW>(sgp, lane, dense, stg_a, ul);
+            gv_load_ragged<KW>(sgp, dense, stg_a, ul);
             ragged_due = false;
         }
         const uint32_t row_a = xq_a + (uint32_t)((kt >> 3) * 1024 + (kt & 7) * 128);
@@ -270,7 +279,7 @@ __device__ __noinline__ void gv_first_prologue(const void* xp, int dtype, const 
         }
         if (lane == 0) asm volatile("st.shared.f32 [%0], %1;" ::"r"(sx_a + kt * 4), "f"(sx) : "memory");
     }
-    if (ragged_due) gv_load_ragged<KW>(sgp, lane, dense, stg_a, ul);
+    if (ragged_due) gv_load_ragged<KW>(sgp, dense, stg_a, ul);
     sts32(ret_a, ul); sts32(ret_a + 4, nrm); sts32(ret_a + 8, off1); sts32(ret_a + 12, off0);
     fence_proxy_async_smem();   // the operand is read by the tensor core (async proxy)
 #ifdef HQ_TRACE
@@ -385,7 +394,7 @@ k_gemv_e8(E8Params p) {
 
         auto load_hdr_dense = [&](const uint8_t* sgp, uint32_t& ul, uint32_t& nrm) { gv_load_hdr_dense<KW>(sgp, lane, dense, stg_a, ul, nrm); };
         auto load_r = [&](const uint8_t* sgp) { gv_load_r<KW>(sgp, lane, stg_a); };
-        auto load_ragged = [&](const uint8_t* sgp, uint32_t ul) { gv_load_ragged<KW>(sgp, lane, dense, stg_a, ul); };
+        auto load_ragged = [&](const uint8_t* sgp, uint32_t ul) { gv_load_ragged<KW>(sgp, dense, stg_a, ul); };
         // epilogue of K-tile kt (this warp's MMAs on it have completed): drain the accumulator lane, rescale, accumulate (A7)
         auto epilogue = [&](int kt, float sw, bool ovr) {
             uint32_t v;

@@ -39,6 +39,11 @@ __device__ __forceinline__ void sts128(uint32_t a, uint32_t x, uint32_t y, uint3
 __device__ __forceinline__ void cp_async4(uint32_t smem_addr, const void* gptr) {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem_addr), "l"(gptr) : "memory");
 }
+// the same with a zero fill: `on` false copies nothing (the source is not touched) and stores a zero word
+__device__ __forceinline__ void cp_async4_zfill(uint32_t smem_addr, const void* gptr, bool on) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(smem_addr), "l"(gptr), "r"(on ? 4u : 0u) : "memory");
+}
+__device__ __forceinline__ uint32_t lanemask_lt() { uint32_t m; asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m)); return m; }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
 // ---- programmatic dependent launch (PDL): a kernel launched with the programmatic-stream-serialization
