@@ -308,109 +308,174 @@ k_act_blob(const void* X, int dtype, int64_t B, int64_t n_kt, int64_t ldx, const
     }
 }
 
-// The same for RHT tiles of 256 (the large-M path at n_tile = 256): lane l holds elements 8l .. 8l+7 = E8 block l of the
-// tile.  Three in-register butterfly stages (strides 1, 2, 4) and five shuffle stages (8 .. 128), FORMAT R1 order.  The
-// tile leaves as TWO operand chunks of 128 K-bytes (chunk = block / 16; K index inside a chunk 32c + 4i + b for block
-// 4c + b, coordinate i), each followed by the NB scales s_x of the whole tile.  blob index = (bt * n_kt256 + kt) * 2 + chunk.
-__global__ void __launch_bounds__(QW_WARPS * 32)
+// The same for RHT tiles of 256 (the large-M path at n_tile = 256).  A half-warp owns one tile: lane l of the half holds the
+// 16 contiguous elements 16l .. 16l+15 and runs the butterflies of strides 1, 2, 4, 8 in registers; a 16 x 16 transpose
+// through shared memory gives it elements l, 16 + l, ..., 240 + l for the strides 16 .. 128 - the same pairs in the same
+// ascending-stride order as FORMAT R1, so the fp32 results are bit-identical to the shuffle butterfly of k_act_blob.
+// Butterflies whose two operands sit in different register pairs run as packed f32x2 adds (IEEE round-to-nearest per
+// element).  The tile leaves as TWO operand chunks of 128 K-bytes (chunk = block / 16; K index inside a chunk 32c + 4i + b
+// for block 4c + b, coordinate i), each followed by the NB scales s_x of the whole tile: blob index = (bt * n_kt256 + kt) * 2
+// + chunk.  Lanes l and l ^ 8 hold the four bytes of every operand word between them: one 16-bit exchange each way.
+constexpr int A256_WARPS = 8;
+constexpr int A256_WFLOATS = 672;   // per warp: two 16 x 20 float transposition buffers, the second shifted by 16 banks
+__device__ __forceinline__ uint64_t a256_pack(float lo, float hi) {
+    uint64_t r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "r"(__float_as_uint(lo)), "r"(__float_as_uint(hi)));
+    return r;
+}
+__device__ __forceinline__ void a256_unpack(uint64_t v, float& lo, float& hi) {
+    uint32_t a, b;
+    asm("mov.b64 {%0, %1}, %2;" : "=r"(a), "=r"(b) : "l"(v));
+    lo = __uint_as_float(a); hi = __uint_as_float(b);
+}
+__device__ __forceinline__ uint64_t a256_add2(uint64_t a, uint64_t b) { uint64_t r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ uint64_t a256_sub2(uint64_t a, uint64_t b) { uint64_t r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ uint64_t a256_mul2(uint64_t a, uint64_t b) { uint64_t r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+// four butterfly stages on 16 values v[0..15]: index bits 0, 1, 2 between the pairs {v[j], v[j+8]}, bit 3 inside them
+__device__ __forceinline__ void a256_fwht16(float* v) {
+    uint64_t P[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) P[j] = a256_pack(v[j], v[j + 8]);
+#pragma unroll
+    for (int h = 1; h < 8; h <<= 1)
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+            if (!(i & h)) {
+                const uint64_t a = P[i], c = P[i + h];
+                P[i] = a256_add2(a, c); P[i + h] = a256_sub2(a, c);
+            }
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+        float a, c;
+        a256_unpack(P[j], a, c);
+        v[j] = __fadd_rn(a, c); v[j + 8] = __fsub_rn(a, c);
+    }
+}
+
+__global__ void __launch_bounds__(A256_WARPS * 32)
 k_act_blob256(const void* X, int dtype, int64_t B, int64_t n_kt, int64_t ldx, const int8_t* dsign, int NB, uint8_t* bblob) {
     extern __shared__ float smem[];
     griddep_launch();
     griddep_wait();
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    uint8_t* srow = (uint8_t*)smem + warp * 256;          // two operand rows of 128 bytes
-    const int64_t n_bt = (B + NB - 1) / NB, n_tiles = n_bt * NB * n_kt;
-    const uint32_t blob_bytes = (uint32_t)(NB * 128 + NB * 4);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, half = lane >> 4, l = lane & 15, hi8 = (l >> 3) & 1;
+    float* tr = smem + warp * A256_WFLOATS + half * 336;
+    const uint32_t n_kt32 = (uint32_t)n_kt, npr = (n_kt32 + 1u) >> 1, NB32 = (uint32_t)NB;
+    const uint32_t rows = (uint32_t)((B + NB - 1) / NB) * NB32;
+    const uint64_t n_pairs = (uint64_t)rows * npr;
+    const uint32_t blob_bytes = NB32 * 128u + NB32 * 4u;
     const bool vec = dtype == HQ_BF16 ? ((((uintptr_t)X) | (uintptr_t)(ldx * 2)) & 15) == 0
                                       : ((((uintptr_t)X) | (uintptr_t)(ldx * 4)) & 15) == 0;
-    const int colb = 128 * (lane >> 4) + 32 * ((lane >> 2) & 3) + (lane & 3);   // + 4 i: byte of coordinate i in the two rows
-    const uint32_t n_kt32 = (uint32_t)n_kt, NB32 = (uint32_t)NB;
-    const uint32_t stride = gridDim.x * (uint32_t)QW_WARPS;
-    const uint32_t st_b = stride / n_kt32, st_k = stride - st_b * n_kt32;
-    uint32_t b32 = (blockIdx.x * (uint32_t)QW_WARPS + warp) / n_kt32;
-    uint32_t kt32 = (blockIdx.x * (uint32_t)QW_WARPS + warp) - b32 * n_kt32;
-    for (int64_t tile = blockIdx.x * (int64_t)QW_WARPS + warp; tile < n_tiles; tile += stride,
-                 kt32 += st_k, b32 += st_b + (kt32 >= n_kt32 ? 1u : 0u), kt32 -= (kt32 >= n_kt32 ? n_kt32 : 0u)) {
-        const int64_t b = b32, kt = kt32;
-        const int64_t bt = b32 / NB32;
-        const int bb = (int)(b32 - (uint32_t)bt * NB32);
-        float x[8];
-        int qv[8];
-        float sx = 0.0f;
+    for (uint64_t pair = (uint64_t)blockIdx.x * A256_WARPS + warp; pair < n_pairs; pair += (uint64_t)gridDim.x * A256_WARPS) {
+        const uint32_t b32 = (uint32_t)(pair / npr);
+        const uint32_t kt = 2u * (uint32_t)(pair - (uint64_t)b32 * npr) + (uint32_t)half;
+        const bool tile_on = kt < n_kt32;                        // an odd tile count leaves the last pair's second half idle
+        const bool row_on = tile_on && (int64_t)b32 < B;         // rows past B pad the batch tile with zeros
+        float v[16];
 #pragma unroll
-        for (int j = 0; j < 8; ++j) { x[j] = 0.0f; qv[j] = 0; }
-        if (b < B) {
-            const int64_t base = b * ldx + kt * 256 + 8 * lane;
+        for (int j = 0; j < 16; ++j) v[j] = 0.0f;
+        if (row_on) {
+            const int64_t base = (int64_t)b32 * ldx + (int64_t)kt * 256 + 16 * l;
             if (vec && dtype == HQ_BF16) {
-                const uint4 v = __ldg((const uint4*)((const __nv_bfloat16*)X + base));
-                x[0] = __uint_as_float(v.x << 16); x[1] = __uint_as_float(v.x & 0xffff0000u);
-                x[2] = __uint_as_float(v.y << 16); x[3] = __uint_as_float(v.y & 0xffff0000u);
-                x[4] = __uint_as_float(v.z << 16); x[5] = __uint_as_float(v.z & 0xffff0000u);
-                x[6] = __uint_as_float(v.w << 16); x[7] = __uint_as_float(v.w & 0xffff0000u);
+#pragma unroll
+                for (int q = 0; q < 2; ++q) {
+                    const uint4 w = __ldg((const uint4*)((const __nv_bfloat16*)X + base) + q);
+                    const uint32_t ww[4] = {w.x, w.y, w.z, w.w};
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        v[8 * q + 2 * e] = __uint_as_float(ww[e] << 16);
+                        v[8 * q + 2 * e + 1] = __uint_as_float(ww[e] & 0xffff0000u);
+                    }
+                }
+            } else if (vec) {
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const float4 w = __ldg((const float4*)((const float*)X + base) + q);
+                    v[4 * q] = w.x; v[4 * q + 1] = w.y; v[4 * q + 2] = w.z; v[4 * q + 3] = w.w;
+                }
             } else {
 #pragma unroll
-                for (int j = 0; j < 8; ++j) x[j] = load_elem(X, dtype, base + j);
+                for (int j = 0; j < 16; ++j) v[j] = load_elem(X, dtype, base + j);
             }
-            const uint2 sg = __ldg((const uint2*)(dsign + kt * 256) + lane);
+            const uint4 sg = __ldg((const uint4*)(dsign + (int64_t)kt * 256) + l);   // +-1 as int8: bit 7 = negative
+            const uint32_t sw[4] = {sg.x, sg.y, sg.z, sg.w};
 #pragma unroll
-            for (int j = 0; j < 8; ++j)
-                if ((((j < 4 ? sg.x : sg.y) >> (8 * (j & 3))) & 0x80u)) x[j] = -x[j];
+            for (int j = 0; j < 16; ++j)
+                v[j] = __uint_as_float(__float_as_uint(v[j]) ^ ((sw[j >> 2] << (24 - 8 * (j & 3))) & 0x80000000u));
+        }
+        a256_fwht16(v);                                          // strides 1, 2, 4, 8
+        __syncwarp();                                            // the previous pair's reads of the buffer are done
 #pragma unroll
-            for (int h = 1; h < 8; h <<= 1)      // strides 1, 2, 4: inside the lane
+        for (int q = 0; q < 4; ++q) *(float4*)(tr + l * 20 + 4 * q) = make_float4(v[4 * q], v[4 * q + 1], v[4 * q + 2], v[4 * q + 3]);
+        __syncwarp();
 #pragma unroll
-                for (int i = 0; i < 8; ++i)
-                    if (!(i & h)) {
-                        const float a = x[i], c = x[i + h];
-                        x[i] = __fadd_rn(a, c); x[i + h] = __fsub_rn(a, c);
-                    }
-#pragma unroll
-            for (int m = 1; m < 32; m <<= 1) {   // strides 8 .. 128: lane ^ m holds the partner
-                const float sg1 = (lane & m) ? -1.0f : 1.0f;
-#pragma unroll
-                for (int j = 0; j < 8; ++j) {
-                    const float o = __shfl_xor_sync(0xffffffffu, x[j], m);
-                    x[j] = __fmaf_rn(x[j], sg1, o);
-                }
-            }
-            float amax = 0.0f;
+        for (int m = 0; m < 16; ++m) v[m] = tr[m * 20 + l];      // element 16 m + l
+        a256_fwht16(v);                                          // strides 16, 32, 64, 128
+        float amax = 0.0f;
+        {
+            const uint64_t cn = a256_pack(0.0625f, 0.0625f);     // 1 / sqrt(256)
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
-                x[j] = __fmul_rn(x[j], 0.0625f);   // 1 / sqrt(256)
-                amax = fmaxf(amax, fabsf(x[j]));
+                a256_unpack(a256_mul2(a256_pack(v[j], v[j + 8]), cn), v[j], v[j + 8]);
+                amax = fmaxf(amax, fmaxf(fabsf(v[j]), fabsf(v[j + 8])));
             }
-            for (int sft = 16; sft; sft >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, sft));
-            if (amax != 0.0f) {
-                const float inv = __fdiv_rn(127.0f, amax);
+        }
 #pragma unroll
-                for (int j = 0; j < 8; ++j) {
-                    // rint + clamp to +-127 + cast in one instruction: |x| <= amax bounds |x * inv| by 127 (1 + 2^-23), which
-                    // rounds to 127, so the saturating convert can never return -128 and equals FORMAT R7's clamp(rint(.))
-                    asm("cvt.rni.sat.s8.f32 %0, %1;" : "=r"(qv[j]) : "f"(__fmul_rn(x[j], inv)));
+        for (int sft = 8; sft; sft >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, sft));   // inside the half-warp
+        uint32_t pk[2][2] = {{0u, 0u}, {0u, 0u}};                // pk[chunk][jj]: codes of m = 8 chunk + 4 jj .. + 3, one byte each
+        float sx = 0.0f;
+        if (amax != 0.0f) {
+            const float inv = __fdiv_rn(127.0f, amax);
+            const uint64_t inv2 = a256_pack(inv, inv);
+            int q[16];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                float a, c;
+                a256_unpack(a256_mul2(a256_pack(v[j], v[j + 8]), inv2), a, c);
+                // rint + clamp to +-127 + cast in one instruction: |x| <= amax bounds |x * inv| by 127 (1 + 2^-23), which
+                // rounds to 127, so the saturating convert can never return -128 and equals FORMAT R7's clamp(rint(.))
+                asm("cvt.rni.sat.s8.f32 %0, %1;" : "=r"(q[j]) : "f"(a));
+                asm("cvt.rni.sat.s8.f32 %0, %1;" : "=r"(q[j + 8]) : "f"(c));
+            }
+#pragma unroll
+            for (int ch = 0; ch < 2; ++ch)
+#pragma unroll
+                for (int jj = 0; jj < 2; ++jj) {
+                    const int m0 = 8 * ch + 4 * jj;
+                    pk[ch][jj] = __byte_perm(__byte_perm((uint32_t)q[m0], (uint32_t)q[m0 + 1], 0x0040),
+                                             __byte_perm((uint32_t)q[m0 + 2], (uint32_t)q[m0 + 3], 0x0040), 0x5410);
                 }
-                sx = __fdiv_rn(amax, 127.0f);
+            sx = __fdiv_rn(amax, 127.0f);
+        }
+        // lane l (bit 3 clear) and lane l + 8 hold bytes {0, 2} and {1, 3} of every word: the low lane assembles chunk 0, the
+        // high lane chunk 1
+        uint32_t A[2], Bv[2];
+#pragma unroll
+        for (int jj = 0; jj < 2; ++jj) {
+            const uint32_t keep = hi8 ? pk[1][jj] : pk[0][jj], send = hi8 ? pk[0][jj] : pk[1][jj];
+            const uint32_t recv = __shfl_xor_sync(0xffffffffu, send, 8);
+            A[jj] = hi8 ? recv : keep; Bv[jj] = hi8 ? keep : recv;
+        }
+        if (tile_on) {
+            const uint32_t bt = b32 / NB32, bb = b32 - bt * NB32;
+            uint8_t* blob = bblob + (((uint64_t)bt * n_kt32 + kt) * 2 + (uint32_t)hi8) * (uint64_t)blob_bytes;
+            uint8_t* rowp = blob + (bb >> 3) * 1024 + (bb & 7) * 128 + ((l & 3) << 2);
+#pragma unroll
+            for (int pm = 0; pm < 4; ++pm) {   // word 8 pm + (l & 7) of the chunk row: 16-byte unit 2 pm + ((l & 7) >> 2)
+                const uint32_t unit = 2u * pm + ((l & 7) >> 2);
+                *(uint32_t*)(rowp + ((unit ^ (bb & 7)) << 4)) = __byte_perm(A[pm >> 1], Bv[pm >> 1], (pm & 1) ? 0x7362 : 0x5140);
             }
+            if ((l & 7) == 0) ((float*)(blob + NB32 * 128u))[bb] = sx;   // both chunks carry the tile's scale
         }
-#pragma unroll
-        for (int j = 0; j < 8; ++j) srow[colb + 4 * j] = (uint8_t)(int8_t)qv[j];
-        __syncwarp();
-#pragma unroll
-        for (int ch = 0; ch < 2; ++ch) {   // one coalesced 128-byte row per chunk
-            uint8_t* blob = bblob + ((bt * n_kt + kt) * 2 + ch) * (int64_t)blob_bytes;
-            const uint32_t w4 = ((const uint32_t*)srow)[ch * 32 + lane];
-            *(uint32_t*)(blob + (bb >> 3) * 1024 + (bb & 7) * 128 + ((((lane >> 2) ^ (bb & 7)) << 4) | ((lane & 3) << 2))) = w4;
-            if (lane == 0) ((float*)(blob + NB * 128))[bb] = sx;
-        }
-        __syncwarp();
     }
 }
 
 void launch_act_blob256(const void* x, int dtype, int64_t B, int64_t n_in, int64_t ldx, const int8_t* dsign, int NB,
                         uint8_t* bblob, cudaStream_t st) {
-    int64_t n_kt = n_in / 256, n_bt = (B + NB - 1) / NB, n_tiles = n_bt * NB * n_kt;
-    int64_t blocks = (n_tiles + QW_WARPS - 1) / QW_WARPS;
-    if (blocks > 148 * 16) blocks = 148 * 16;
-    launch_pdl(k_act_blob256, dim3((unsigned)blocks), dim3(QW_WARPS * 32), QW_WARPS * 256, st, x, dtype, B, n_kt, ldx, dsign, NB,
-               bblob);
+    const int64_t n_kt = n_in / 256, n_bt = (B + NB - 1) / NB, n_pairs = n_bt * NB * ((n_kt + 1) / 2);
+    int64_t blocks = (n_pairs + A256_WARPS - 1) / A256_WARPS;
+    if (blocks > 148 * 8) blocks = 148 * 8;
+    launch_pdl(k_act_blob256, dim3((unsigned)blocks), dim3(A256_WARPS * 32), A256_WARPS * A256_WFLOATS * sizeof(float), st, x, dtype, B,
+               n_kt, ldx, dsign, NB, bblob);
 }
 
 void launch_act_blob(const void* x, int dtype, int64_t B, int64_t n_in, int64_t ldx, const int8_t* dsign, int NB,

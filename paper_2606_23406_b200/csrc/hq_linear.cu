@@ -413,11 +413,10 @@ static hq_status launch_large(hq_ctx* ctx, const hq_weight* const* ws, int n_w, 
         d.blob = w->blob; d.sub_off = w->group_off; d.lut = ctx->e8_lut; d.ablob = ablob; d.m = w->m;
         d.n_kt = (int)w->n_kt;
         d.inv_A = (float)(1.0 / (w->alpha * sqrt((double)w->n)));
-        int ky = 1;   // enough CTAs for ~8 per SM, each amortising its table load over several tiles
-        while (ky < d.n_kt && (int64_t)w->n_rb * ky < (int64_t)ctx->sm_count * 8) ky *= 2;
-        d.kt_per_cta = (d.n_kt + ky - 1) / ky;
-        dim3 dgrid((unsigned)w->n_rb, (unsigned)((d.n_kt + d.kt_per_cta - 1) / d.kt_per_cta));
-        const size_t dsmem = E8_LUT_BYTES + 128 * (size_t)(w->n / 8 + 1) * 4;
+        d.n_rb = (int)w->n_rb;
+        const size_t dsmem = E8_LUT_BYTES + 128 * (size_t)(w->n / 8 + 1) * 4 + 16;
+        const int64_t dtiles = (int64_t)w->n_rb * d.n_kt, dmax = (int64_t)ctx->sm_count * 4;   // 4 CTAs of 128 threads per SM
+        dim3 dgrid((unsigned)(dtiles < dmax ? dtiles : dmax));
         cudaStream_t dst = i == 0 ? ctx->side : st;   // later weights reuse the scratch copy: stream order after the GEMM
 #define HQ_LD(KK)                                                                                                          \
     case KK:                                                                                                               \

@@ -37,7 +37,7 @@ struct E8AblobParams {
     const uint32_t* lut;
     uint8_t* ablob;       // [n_rb][n_kt][LG_ABLOB]
     int64_t m;
-    int n_kt, kt_per_cta;
+    int n_kt, n_rb;
     float inv_A;
 };
 
@@ -52,19 +52,29 @@ __global__ void __launch_bounds__(128) k_e8_decode_ablob(E8AblobParams p) {
     constexpr int SCR = TILE / 8 + 1;              // nibble words per row + 1
     constexpr int NCH = TILE / 128;                // operand chunks per tile
     const int t = threadIdx.x, warp = t >> 5, lane = t & 31;
-    uint32_t* lut_s = (uint32_t*)smem_raw;
-    for (int i = t; i < E8_LUT_WORDS; i += 128) lut_s[i] = __ldg(p.lut + i);
-    __syncthreads();
     const uint32_t smem_a = smem_u32(smem_raw);
+    // the phase-1 table arrives by one bulk copy; the CTA's first loads are in flight meanwhile
+    uint64_t* bar_lut = (uint64_t*)(smem_raw + E8_LUT_BYTES + 128 * SCR * 4);
+    if (t == 0) {
+        mbar_init(bar_lut, 1);
+        mbar_fence_init();
+        mbar_arrive_expect_tx(bar_lut, E8_LUT_BYTES);
+        bulk_g2s(smem_raw, p.lut, E8_LUT_BYTES, bar_lut);
+    }
+    __syncthreads();
     const uint32_t lut_lane = smem_a + (uint32_t)(lane & (E8_LUT_COPIES - 1)) * 4;
     const uint32_t scr_a = smem_a + E8_LUT_BYTES + (uint32_t)t * SCR * 4;
     const uint32_t lane_lt = (1u << lane) - 1u;
-    const int rb = blockIdx.x;
-    const int kt0 = blockIdx.y * p.kt_per_cta;
-    const int64_t r = (int64_t)rb * 128 + t;
-    for (int kt = kt0; kt < kt0 + p.kt_per_cta && kt < p.n_kt; ++kt) {
-        const size_t g = (size_t)rb * p.n_kt + kt;
-        const uint8_t* sgp = p.blob + 16 * (size_t)__ldg(p.sub_off + g * 4 + warp);
+    // contiguous range of (row block, tile) pairs per CTA: a few CTAs per SM, each amortising its table over many tiles
+    const int64_t G = (int64_t)p.n_rb * p.n_kt;
+    const int64_t g_begin = (int64_t)blockIdx.x * G / gridDim.x, g_end = (int64_t)(blockIdx.x + 1) * G / gridDim.x;
+    uint32_t off_c = g_begin < g_end ? __ldg(p.sub_off + g_begin * 4 + warp) : 0u;
+    bool lut_ready = false;
+    for (int64_t g = g_begin; g < g_end; ++g) {
+        const int rb = (int)(g / p.n_kt);
+        const int64_t r = (int64_t)rb * 128 + t;
+        const uint8_t* sgp = p.blob + 16 * (size_t)off_c;
+        const uint32_t off_n = g + 1 < g_end ? __ldg(p.sub_off + (g + 1) * 4 + warp) : 0u;
         const uint32_t ul = __ldg((const uint16_t*)sgp + lane), nrm = __ldg((const uint16_t*)sgp + 32 + lane);
         const uint32_t* rarea = (const uint32_t*)(sgp + 128);
         const uint32_t* uarea = rarea + KW * 32;
@@ -82,6 +92,10 @@ __global__ void __launch_bounds__(128) k_e8_decode_ablob(E8AblobParams p) {
                 base += __popc(mk);
             }
         }
+        // the next tile's sub-group into L2 while this one is decoded (its demand loads then hit)
+        if (g + 1 < g_end && lane < (TILE == 128 ? 18 : 34))
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(p.blob + 16 * (size_t)off_n + lane * 128));
+        if (!lut_ready) { mbar_wait(bar_lut, 0u); lut_ready = true; }
         {
             uint32_t T = 0, acc = 0, wo = scr_a;
 #pragma unroll
@@ -120,6 +134,7 @@ __global__ void __launch_bounds__(128) k_e8_decode_ablob(E8AblobParams p) {
         const float sw = present ? f16_bits_to_f32((uint16_t)nrm) * p.inv_A : 0.0f;
 #pragma unroll
         for (int ch = 0; ch < NCH; ++ch) ((float*)(tile + ch * LG_ABLOB + 16384))[t] = sw;
+        off_c = off_n;
     }
 }
 
