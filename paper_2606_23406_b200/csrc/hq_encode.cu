@@ -312,17 +312,15 @@ k_act_blob(const void* X, int dtype, int64_t B, int64_t n_kt, int64_t ldx, const
 // 16 contiguous elements 16l .. 16l+15 and runs the butterflies of strides 1, 2, 4, 8 in registers; a 16 x 16 transpose
 // through shared memory gives it elements l, 16 + l, ..., 240 + l for the strides 16 .. 128 - the same pairs in the same
 // ascending-stride order as FORMAT R1, so the fp32 results are bit-identical to the shuffle butterfly of k_act_blob.
-// Butterflies whose two operands sit in different register pairs run as packed f32x2 adds (IEEE round-to-nearest per
-// element).  The tile leaves as TWO operand chunks of 128 K-bytes (chunk = block / 16; K index inside a chunk 32c + 4i + b
-// for block 4c + b, coordinate i), each followed by the NB scales s_x of the whole tile: blob index = (bt * n_kt256 + kt) * 2
-// + chunk.  Lanes l and l ^ 8 hold the four bytes of every operand word between them: one 16-bit exchange each way.
+// The 16 values live as eight f32x2 register pairs {v[j], v[j+8]} from the load to the INT8 cast: butterflies between
+// pairs are packed adds (IEEE round-to-nearest per element), the one inside the pairs is scalar.  The tile leaves as TWO
+// operand chunks of 128 K-bytes (chunk = block / 16; K index inside a chunk 32c + 4i + b for block 4c + b, coordinate i),
+// each followed by the NB scales s_x of the whole tile: blob index = (bt * n_kt256 + kt) * 2 + chunk.  Lanes l and l ^ 8
+// hold the four bytes of every operand word between them: one exchange of two registers.
 constexpr int A256_WARPS = 8;
-constexpr int A256_WFLOATS = 672;   // per warp: two 16 x 20 float transposition buffers, the second shifted by 16 banks
-__device__ __forceinline__ uint64_t a256_pack(float lo, float hi) {
-    uint64_t r;
-    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "r"(__float_as_uint(lo)), "r"(__float_as_uint(hi)));
-    return r;
-}
+constexpr int A256_CTAS = 4;        // per SM (64 registers x 256 threads)
+constexpr int A256_WFLOATS = 592;   // per warp: two 16 x 18 float transposition buffers, the second shifted by 16 banks
+__device__ __forceinline__ uint64_t a256_pack(uint32_t lo, uint32_t hi) { uint64_t r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "r"(lo), "r"(hi)); return r; }
 __device__ __forceinline__ void a256_unpack(uint64_t v, float& lo, float& hi) {
     uint32_t a, b;
     asm("mov.b64 {%0, %1}, %2;" : "=r"(a), "=r"(b) : "l"(v));
@@ -331,11 +329,11 @@ __device__ __forceinline__ void a256_unpack(uint64_t v, float& lo, float& hi) {
 __device__ __forceinline__ uint64_t a256_add2(uint64_t a, uint64_t b) { uint64_t r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
 __device__ __forceinline__ uint64_t a256_sub2(uint64_t a, uint64_t b) { uint64_t r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
 __device__ __forceinline__ uint64_t a256_mul2(uint64_t a, uint64_t b) { uint64_t r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
-// four butterfly stages on 16 values v[0..15]: index bits 0, 1, 2 between the pairs {v[j], v[j+8]}, bit 3 inside them
-__device__ __forceinline__ void a256_fwht16(float* v) {
-    uint64_t P[8];
-#pragma unroll
-    for (int j = 0; j < 8; ++j) P[j] = a256_pack(v[j], v[j + 8]);
+// sign bytes (+-1 as int8) -> sign-bit masks: prmt's replicate mode turns the selected byte into 0x00 / 0xff
+template <uint32_t SEL>
+__device__ __forceinline__ uint32_t a256_signs(uint32_t sgw) { uint32_t r; asm("prmt.b32 %0, %1, %2, %3;" : "=r"(r) : "r"(sgw), "r"(0u), "n"(SEL)); return r; }
+// four butterfly stages on the 16 values {P[j].lo = v[j], P[j].hi = v[j+8]}: index bits 0, 1, 2 between pairs, bit 3 inside
+__device__ __forceinline__ void a256_fwht16(uint64_t* P) {
 #pragma unroll
     for (int h = 1; h < 8; h <<= 1)
 #pragma unroll
@@ -348,102 +346,119 @@ __device__ __forceinline__ void a256_fwht16(float* v) {
     for (int j = 0; j < 8; ++j) {
         float a, c;
         a256_unpack(P[j], a, c);
-        v[j] = __fadd_rn(a, c); v[j + 8] = __fsub_rn(a, c);
+        P[j] = a256_pack(__float_as_uint(__fadd_rn(a, c)), __float_as_uint(__fsub_rn(a, c)));
     }
 }
 
-__global__ void __launch_bounds__(A256_WARPS * 32)
+struct A256Raw { uint4 a, b, sg; };   // a lane's 16 bf16 elements and their 16 sign bytes
+
+template <bool FAST>   // FAST: bf16 rows whose 16-element groups can be read as 16-byte words
+__global__ void __launch_bounds__(A256_WARPS * 32, A256_CTAS)
 k_act_blob256(const void* X, int dtype, int64_t B, int64_t n_kt, int64_t ldx, const int8_t* dsign, int NB, uint8_t* bblob) {
     extern __shared__ float smem[];
     griddep_launch();
     griddep_wait();
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, half = lane >> 4, l = lane & 15, hi8 = (l >> 3) & 1;
-    float* tr = smem + warp * A256_WFLOATS + half * 336;
+    float* tr = smem + warp * A256_WFLOATS + half * 304;
     const uint32_t n_kt32 = (uint32_t)n_kt, npr = (n_kt32 + 1u) >> 1, NB32 = (uint32_t)NB;
     const uint32_t rows = (uint32_t)((B + NB - 1) / NB) * NB32;
-    const uint64_t n_pairs = (uint64_t)rows * npr;
+    const uint32_t n_pairs = rows * npr, stride = gridDim.x * (uint32_t)A256_WARPS;   // < 2^32: checked by the launcher
     const uint32_t blob_bytes = NB32 * 128u + NB32 * 4u;
-    const bool vec = dtype == HQ_BF16 ? ((((uintptr_t)X) | (uintptr_t)(ldx * 2)) & 15) == 0
-                                      : ((((uintptr_t)X) | (uintptr_t)(ldx * 4)) & 15) == 0;
-    for (uint64_t pair = (uint64_t)blockIdx.x * A256_WARPS + warp; pair < n_pairs; pair += (uint64_t)gridDim.x * A256_WARPS) {
-        const uint32_t b32 = (uint32_t)(pair / npr);
-        const uint32_t kt = 2u * (uint32_t)(pair - (uint64_t)b32 * npr) + (uint32_t)half;
+    constexpr bool fast = FAST;
+    auto locate = [&](uint32_t pair, uint32_t& b32, uint32_t& kt) {
+        b32 = pair / npr;
+        kt = 2u * (pair - b32 * npr) + (uint32_t)half;
+    };
+    auto load_raw = [&](uint32_t b32, uint32_t kt, A256Raw& r) {
+        if (fast && kt < n_kt32 && (int64_t)b32 < B) {
+            const uint4* src = (const uint4*)((const __nv_bfloat16*)X + ((int64_t)b32 * ldx + (int64_t)kt * 256 + 16 * l));
+            r.a = __ldg(src); r.b = __ldg(src + 1);
+            r.sg = __ldg((const uint4*)(dsign + (int64_t)kt * 256) + l);
+        }
+    };
+    uint32_t pair = blockIdx.x * (uint32_t)A256_WARPS + warp;
+    uint32_t b32 = 0, kt = 0;
+    A256Raw cur;
+    cur.a = cur.b = cur.sg = make_uint4(0u, 0u, 0u, 0u);
+    if (pair < n_pairs) { locate(pair, b32, kt); load_raw(b32, kt, cur); }
+    while (pair < n_pairs) {
+        const uint32_t pair_n = pair + stride < pair ? 0xffffffffu : pair + stride;
+        uint32_t b32_n = 0, kt_n = 0;
+        A256Raw nxt;
+        nxt.a = nxt.b = nxt.sg = make_uint4(0u, 0u, 0u, 0u);
+        if (pair_n < n_pairs) { locate(pair_n, b32_n, kt_n); load_raw(b32_n, kt_n, nxt); }   // in flight behind this pair's arithmetic
         const bool tile_on = kt < n_kt32;                        // an odd tile count leaves the last pair's second half idle
         const bool row_on = tile_on && (int64_t)b32 < B;         // rows past B pad the batch tile with zeros
-        float v[16];
+        uint64_t P[8];
 #pragma unroll
-        for (int j = 0; j < 16; ++j) v[j] = 0.0f;
+        for (int j = 0; j < 8; ++j) P[j] = 0ull;
         if (row_on) {
-            const int64_t base = (int64_t)b32 * ldx + (int64_t)kt * 256 + 16 * l;
-            if (vec && dtype == HQ_BF16) {
+            if (fast) {
+                const uint32_t wa[4] = {cur.a.x, cur.a.y, cur.a.z, cur.a.w}, wb[4] = {cur.b.x, cur.b.y, cur.b.z, cur.b.w};
+                const uint32_t sw[4] = {cur.sg.x, cur.sg.y, cur.sg.z, cur.sg.w};
 #pragma unroll
-                for (int q = 0; q < 2; ++q) {
-                    const uint4 w = __ldg((const uint4*)((const __nv_bfloat16*)X + base) + q);
-                    const uint32_t ww[4] = {w.x, w.y, w.z, w.w};
-#pragma unroll
-                    for (int e = 0; e < 4; ++e) {
-                        v[8 * q + 2 * e] = __uint_as_float(ww[e] << 16);
-                        v[8 * q + 2 * e + 1] = __uint_as_float(ww[e] & 0xffff0000u);
-                    }
-                }
-            } else if (vec) {
-#pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    const float4 w = __ldg((const float4*)((const float*)X + base) + q);
-                    v[4 * q] = w.x; v[4 * q + 1] = w.y; v[4 * q + 2] = w.z; v[4 * q + 3] = w.w;
+                for (int e = 0; e < 4; ++e) {   // word e: elements 2e, 2e+1 (and 8 + 2e, 9 + 2e); sign bytes (2e) & 3, +1 of sw[e >> 1] (sw[2 + (e >> 1)])
+                    uint32_t ma, mb;
+                    if (e & 1) { ma = a256_signs<0xb4a4>(sw[e >> 1]); mb = a256_signs<0xb4a4>(sw[2 + (e >> 1)]); }
+                    else       { ma = a256_signs<0x9484>(sw[e >> 1]); mb = a256_signs<0x9484>(sw[2 + (e >> 1)]); }
+                    const uint32_t xa = wa[e] ^ (ma & 0x80008000u), xb = wb[e] ^ (mb & 0x80008000u);
+                    P[2 * e] = a256_pack(xa << 16, xb << 16);
+                    P[2 * e + 1] = a256_pack(xa & 0xffff0000u, xb & 0xffff0000u);
                 }
             } else {
+                const int64_t base = (int64_t)b32 * ldx + (int64_t)kt * 256 + 16 * l;
+                const int8_t* sp = dsign + (int64_t)kt * 256 + 16 * l;
 #pragma unroll
-                for (int j = 0; j < 16; ++j) v[j] = load_elem(X, dtype, base + j);
+                for (int j = 0; j < 8; ++j) {
+                    const float lo = load_elem(X, dtype, base + j), hi = load_elem(X, dtype, base + j + 8);
+                    P[j] = a256_pack(__float_as_uint(sp[j] < 0 ? -lo : lo), __float_as_uint(sp[j + 8] < 0 ? -hi : hi));
+                }
             }
-            const uint4 sg = __ldg((const uint4*)(dsign + (int64_t)kt * 256) + l);   // +-1 as int8: bit 7 = negative
-            const uint32_t sw[4] = {sg.x, sg.y, sg.z, sg.w};
-#pragma unroll
-            for (int j = 0; j < 16; ++j)
-                v[j] = __uint_as_float(__float_as_uint(v[j]) ^ ((sw[j >> 2] << (24 - 8 * (j & 3))) & 0x80000000u));
         }
-        a256_fwht16(v);                                          // strides 1, 2, 4, 8
+        a256_fwht16(P);                                          // strides 1, 2, 4, 8
         __syncwarp();                                            // the previous pair's reads of the buffer are done
 #pragma unroll
-        for (int q = 0; q < 4; ++q) *(float4*)(tr + l * 20 + 4 * q) = make_float4(v[4 * q], v[4 * q + 1], v[4 * q + 2], v[4 * q + 3]);
+        for (int j = 0; j < 8; ++j) *(uint64_t*)(tr + l * 18 + 2 * j) = P[j];   // value j at slot 2 (j & 7) + (j >> 3) of row l
         __syncwarp();
+        {
+            const float* col = tr + 2 * (l & 7) + (l >> 3);      // element 16 m + l: value l of row m
 #pragma unroll
-        for (int m = 0; m < 16; ++m) v[m] = tr[m * 20 + l];      // element 16 m + l
-        a256_fwht16(v);                                          // strides 16, 32, 64, 128
+            for (int j = 0; j < 8; ++j) P[j] = a256_pack(__float_as_uint(col[j * 18]), __float_as_uint(col[(j + 8) * 18]));
+        }
+        a256_fwht16(P);                                          // strides 16, 32, 64, 128
         float amax = 0.0f;
         {
-            const uint64_t cn = a256_pack(0.0625f, 0.0625f);     // 1 / sqrt(256)
+            const uint64_t cn = a256_pack(__float_as_uint(0.0625f), __float_as_uint(0.0625f));   // 1 / sqrt(256)
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
-                a256_unpack(a256_mul2(a256_pack(v[j], v[j + 8]), cn), v[j], v[j + 8]);
-                amax = fmaxf(amax, fmaxf(fabsf(v[j]), fabsf(v[j + 8])));
+                P[j] = a256_mul2(P[j], cn);
+                float a, c;
+                a256_unpack(P[j], a, c);
+                amax = fmaxf(amax, fmaxf(fabsf(a), fabsf(c)));
             }
         }
 #pragma unroll
         for (int sft = 8; sft; sft >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, sft));   // inside the half-warp
-        uint32_t pk[2][2] = {{0u, 0u}, {0u, 0u}};                // pk[chunk][jj]: codes of m = 8 chunk + 4 jj .. + 3, one byte each
+        uint32_t pk[2][2] = {{0u, 0u}, {0u, 0u}};                // pk[chunk][jj]: codes of elements m = 8 chunk + 4 jj .. + 3 (x 16 + l)
         float sx = 0.0f;
         if (amax != 0.0f) {
             const float inv = __fdiv_rn(127.0f, amax);
-            const uint64_t inv2 = a256_pack(inv, inv);
-            int q[16];
+            const uint64_t inv2 = a256_pack(__float_as_uint(inv), __float_as_uint(inv));
+            uint32_t qlo[8], qhi[8];
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
                 float a, c;
-                a256_unpack(a256_mul2(a256_pack(v[j], v[j + 8]), inv2), a, c);
+                a256_unpack(a256_mul2(P[j], inv2), a, c);
                 // rint + clamp to +-127 + cast in one instruction: |x| <= amax bounds |x * inv| by 127 (1 + 2^-23), which
                 // rounds to 127, so the saturating convert can never return -128 and equals FORMAT R7's clamp(rint(.))
-                asm("cvt.rni.sat.s8.f32 %0, %1;" : "=r"(q[j]) : "f"(a));
-                asm("cvt.rni.sat.s8.f32 %0, %1;" : "=r"(q[j + 8]) : "f"(c));
+                asm("cvt.rni.sat.s8.f32 %0, %1;" : "=r"(qlo[j]) : "f"(a));
+                asm("cvt.rni.sat.s8.f32 %0, %1;" : "=r"(qhi[j]) : "f"(c));
             }
 #pragma unroll
-            for (int ch = 0; ch < 2; ++ch)
-#pragma unroll
-                for (int jj = 0; jj < 2; ++jj) {
-                    const int m0 = 8 * ch + 4 * jj;
-                    pk[ch][jj] = __byte_perm(__byte_perm((uint32_t)q[m0], (uint32_t)q[m0 + 1], 0x0040),
-                                             __byte_perm((uint32_t)q[m0 + 2], (uint32_t)q[m0 + 3], 0x0040), 0x5410);
-                }
+            for (int jj = 0; jj < 2; ++jj) {
+                pk[0][jj] = __byte_perm(__byte_perm(qlo[4 * jj], qlo[4 * jj + 1], 0x0040), __byte_perm(qlo[4 * jj + 2], qlo[4 * jj + 3], 0x0040), 0x5410);
+                pk[1][jj] = __byte_perm(__byte_perm(qhi[4 * jj], qhi[4 * jj + 1], 0x0040), __byte_perm(qhi[4 * jj + 2], qhi[4 * jj + 3], 0x0040), 0x5410);
+            }
             sx = __fdiv_rn(amax, 127.0f);
         }
         // lane l (bit 3 clear) and lane l + 8 hold bytes {0, 2} and {1, 3} of every word: the low lane assembles chunk 0, the
@@ -466,6 +481,7 @@ k_act_blob256(const void* X, int dtype, int64_t B, int64_t n_kt, int64_t ldx, co
             }
             if ((l & 7) == 0) ((float*)(blob + NB32 * 128u))[bb] = sx;   // both chunks carry the tile's scale
         }
+        cur = nxt; pair = pair_n; b32 = b32_n; kt = kt_n;
     }
 }
 
@@ -473,9 +489,15 @@ void launch_act_blob256(const void* x, int dtype, int64_t B, int64_t n_in, int64
                         uint8_t* bblob, cudaStream_t st) {
     const int64_t n_kt = n_in / 256, n_bt = (B + NB - 1) / NB, n_pairs = n_bt * NB * ((n_kt + 1) / 2);
     int64_t blocks = (n_pairs + A256_WARPS - 1) / A256_WARPS;
-    if (blocks > 148 * 8) blocks = 148 * 8;
-    launch_pdl(k_act_blob256, dim3((unsigned)blocks), dim3(A256_WARPS * 32), A256_WARPS * A256_WFLOATS * sizeof(float), st, x, dtype, B,
-               n_kt, ldx, dsign, NB, bblob);
+    if (blocks > 148 * A256_CTAS) blocks = 148 * A256_CTAS;
+    // n_pairs < 2^32 always: 2^32 pairs of 512 bf16 activations would be 4.4 TB of x
+    const bool fast = dtype == HQ_BF16 && ((((uintptr_t)x) | (uintptr_t)(ldx * 2)) & 15) == 0;
+    if (fast)
+        launch_pdl(k_act_blob256<true>, dim3((unsigned)blocks), dim3(A256_WARPS * 32), A256_WARPS * A256_WFLOATS * sizeof(float), st, x,
+                   dtype, B, n_kt, ldx, dsign, NB, bblob);
+    else
+        launch_pdl(k_act_blob256<false>, dim3((unsigned)blocks), dim3(A256_WARPS * 32), A256_WARPS * A256_WFLOATS * sizeof(float), st, x,
+                   dtype, B, n_kt, ldx, dsign, NB, bblob);
 }
 
 void launch_act_blob(const void* x, int dtype, int64_t B, int64_t n_in, int64_t ldx, const int8_t* dsign, int NB,

@@ -414,18 +414,18 @@ static hq_status launch_large(hq_ctx* ctx, const hq_weight* const* ws, int n_w, 
         d.n_kt = (int)w->n_kt;
         d.inv_A = (float)(1.0 / (w->alpha * sqrt((double)w->n)));
         d.n_rb = (int)w->n_rb;
-        const size_t dsmem = E8_LUT_BYTES + 128 * (size_t)(w->n / 8 + 1) * 4 + 16;
-        const int64_t dtiles = (int64_t)w->n_rb * d.n_kt, dmax = (int64_t)ctx->sm_count * 4;   // 4 CTAs of 128 threads per SM
-        dim3 dgrid((unsigned)(dtiles < dmax ? dtiles : dmax));
+        const size_t dsmem = E8_LUT_BYTES + 256 * (size_t)(w->n / 8 + 1) * 4 + 16;
+        const int64_t dpairs = ((int64_t)w->n_rb * d.n_kt + 1) / 2, dmax = (int64_t)ctx->sm_count * 3;   // 3 CTAs of 256 threads per SM
+        dim3 dgrid((unsigned)(dpairs < dmax ? dpairs : dmax));
         cudaStream_t dst = i == 0 ? ctx->side : st;   // later weights reuse the scratch copy: stream order after the GEMM
 #define HQ_LD(KK)                                                                                                          \
     case KK:                                                                                                               \
         if (nch == 1) {                                                                                                    \
             HQ_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_e8_decode_ablob<KK, 128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dsmem)); \
-            k_e8_decode_ablob<KK, 128><<<dgrid, 128, dsmem, dst>>>(d);                                                     \
+            k_e8_decode_ablob<KK, 128><<<dgrid, 256, dsmem, dst>>>(d);                                                     \
         } else {                                                                                                           \
             HQ_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_e8_decode_ablob<KK, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dsmem)); \
-            k_e8_decode_ablob<KK, 256><<<dgrid, 128, dsmem, dst>>>(d);                                                     \
+            k_e8_decode_ablob<KK, 256><<<dgrid, 256, dsmem, dst>>>(d);                                                     \
         }                                                                                                                  \
         break
         switch (w->k0) { HQ_LD(0); HQ_LD(1); HQ_LD(2); HQ_LD(3); }

@@ -44,18 +44,18 @@ struct E8AblobParams {
 // TILE = RHT tile of the weight (128 or 256).  A tile of 256 is written as two operand chunks of 128 K-bytes (K index
 // inside the tile: 32c + 4i + b for block 4c + b, coordinate i; chunk = c / 4), each followed by the same 128 row scales.
 template <int K, int TILE>
-__global__ void __launch_bounds__(128) k_e8_decode_ablob(E8AblobParams p) {
+__global__ void __launch_bounds__(256) k_e8_decode_ablob(E8AblobParams p) {   // two tiles per CTA pass: warps 0-3 and 4-7
     extern __shared__ __align__(16) uint8_t smem_raw[];
     constexpr int KW = K * TILE / 32;              // R words per row
     constexpr int NWT = E8_NW * TILE / 128;        // U words per row handled by the fast path
     constexpr int NRUN = TILE / 32;                // runs of 32 symbols
     constexpr int SCR = TILE / 8 + 1;              // nibble words per row + 1
     constexpr int NCH = TILE / 128;                // operand chunks per tile
-    const int t = threadIdx.x, warp = t >> 5, lane = t & 31;
+    const int t = threadIdx.x & 127, sub = threadIdx.x >> 7, warp = t >> 5, lane = t & 31;
     const uint32_t smem_a = smem_u32(smem_raw);
     // the phase-1 table arrives by one bulk copy; the CTA's first loads are in flight meanwhile
-    uint64_t* bar_lut = (uint64_t*)(smem_raw + E8_LUT_BYTES + 128 * SCR * 4);
-    if (t == 0) {
+    uint64_t* bar_lut = (uint64_t*)(smem_raw + E8_LUT_BYTES + 256 * SCR * 4);
+    if (threadIdx.x == 0) {
         mbar_init(bar_lut, 1);
         mbar_fence_init();
         mbar_arrive_expect_tx(bar_lut, E8_LUT_BYTES);
@@ -63,18 +63,18 @@ __global__ void __launch_bounds__(128) k_e8_decode_ablob(E8AblobParams p) {
     }
     __syncthreads();
     const uint32_t lut_lane = smem_a + (uint32_t)(lane & (E8_LUT_COPIES - 1)) * 4;
-    const uint32_t scr_a = smem_a + E8_LUT_BYTES + (uint32_t)t * SCR * 4;
+    const uint32_t scr_a = smem_a + E8_LUT_BYTES + (uint32_t)threadIdx.x * SCR * 4;
     const uint32_t lane_lt = (1u << lane) - 1u;
     // contiguous range of (row block, tile) pairs per CTA: a few CTAs per SM, each amortising its table over many tiles
     const int64_t G = (int64_t)p.n_rb * p.n_kt;
     const int64_t g_begin = (int64_t)blockIdx.x * G / gridDim.x, g_end = (int64_t)(blockIdx.x + 1) * G / gridDim.x;
-    uint32_t off_c = g_begin < g_end ? __ldg(p.sub_off + g_begin * 4 + warp) : 0u;
+    uint32_t off_c = g_begin + sub < g_end ? __ldg(p.sub_off + (g_begin + sub) * 4 + warp) : 0u;
     bool lut_ready = false;
-    for (int64_t g = g_begin; g < g_end; ++g) {
+    for (int64_t g = g_begin + sub; g < g_end; g += 2) {
         const int rb = (int)(g / p.n_kt);
         const int64_t r = (int64_t)rb * 128 + t;
         const uint8_t* sgp = p.blob + 16 * (size_t)off_c;
-        const uint32_t off_n = g + 1 < g_end ? __ldg(p.sub_off + (g + 1) * 4 + warp) : 0u;
+        const uint32_t off_n = g + 2 < g_end ? __ldg(p.sub_off + (g + 2) * 4 + warp) : 0u;
         const uint32_t ul = __ldg((const uint16_t*)sgp + lane), nrm = __ldg((const uint16_t*)sgp + 32 + lane);
         const uint32_t* rarea = (const uint32_t*)(sgp + 128);
         const uint32_t* uarea = rarea + KW * 32;
@@ -93,7 +93,7 @@ __global__ void __launch_bounds__(128) k_e8_decode_ablob(E8AblobParams p) {
             }
         }
         // the next tile's sub-group into L2 while this one is decoded (its demand loads then hit)
-        if (g + 1 < g_end && lane < (TILE == 128 ? 18 : 34))
+        if (g + 2 < g_end && lane < (TILE == 128 ? 18 : 34))
             asm volatile("prefetch.global.L2 [%0];" ::"l"(p.blob + 16 * (size_t)off_n + lane * 128));
         if (!lut_ready) { mbar_wait(bar_lut, 0u); lut_ready = true; }
         {
