@@ -542,7 +542,9 @@ k_gemv_e8(E8Params p) {
     // ---- split-K reduction inside the kernel: publish this thread's partial sums (one fence), then arrive once per cut
     // row block of the range on a per-(row block, warp) counter; the LAST of the row block's segments to arrive adds the
     // partials in slot order - deterministic - and writes y (A7).  No block barrier, no extra launch.
-    __threadfence();
+    // Ordering: the lanes' partial sums -> __syncwarp -> lane 0's acq_rel atomic (release: cumulative over what the barrier
+    // ordered before it; acquire: the other segments' partials) -> __syncwarp -> the lanes' L2 loads.  One atomic round trip
+    // instead of fence + atomic + fence.
     __syncwarp();
     GV_TR(6);
     for (int ff = f_begin; ff < f_end;) {
@@ -559,12 +561,14 @@ k_gemv_e8(E8Params p) {
         unsigned int last = 0;
         if (lane == 0) {
             unsigned int* cnt = p.counters + ((size_t)rbg * 4 + warp);
-            last = atomicAdd(cnt, 1u) == (unsigned int)(n_seg - 1);
+            unsigned int prev;
+            asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], %2;" : "=r"(prev) : "l"(cnt), "r"(1u) : "memory");
+            last = prev == (unsigned int)(n_seg - 1);
             if (last) *cnt = 0u;
         }
         last = __shfl_sync(0xffffffffu, last, 0);
         if (!last) continue;
-        __threadfence();
+        __syncwarp();
         const int64_t mw = p.m[w];
         const int64_t r = (int64_t)(rbg - p.rb_base[w]) * 128 + t;
         if (r >= mw) continue;
