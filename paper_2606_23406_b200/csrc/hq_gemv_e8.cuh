@@ -27,13 +27,6 @@
 
 namespace hq {
 
-#ifdef HQ_TRACE   // phase timestamps per warp (a probe build only: never defined by build.py)
-__device__ unsigned long long g_gv_trace[8 * 148 * 32 * 12];   // slot (n_items >> 9) & 7: the four launches of the bench step differ
-__device__ __forceinline__ unsigned long long gv_now() { unsigned long long v; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(v)); return v; }
-#define GV_TR(i) do { if (lane == 0) g_gv_trace[((size_t)((p.n_items >> 9) & 7) * 148 * 32 + (size_t)blockIdx.x * 32 + wid) * 12 + (i)] = gv_now(); } while (0)
-#else
-#define GV_TR(i) do { } while (0)
-#endif
 
 constexpr int GV_TCOLS_WG = 48;   // TMEM columns per warp group: A tile (32: 128 INT8 per lane) + accumulator (16)
 constexpr int GV_MAX_KT = 128;    // n_in <= 16384: the whole activation operand stays in shared memory
@@ -230,9 +223,6 @@ template <int K, int NW>
 __device__ __noinline__ void gv_first_prologue(const void* xp, int dtype, const int8_t* dsign, int n_kt, uint32_t xq_a,
                                                uint32_t sx_a, int wid, int lane, int kt0, int nt, const uint8_t* blob,
                                                const uint32_t* soff, int has, int dense_i, uint32_t stg_a, uint32_t ret_a
-#ifdef HQ_TRACE
-                                               , int tr_slot
-#endif
 ) {
     constexpr int KW = 4 * K;
     const bool dense = dense_i != 0;
@@ -242,9 +232,6 @@ __device__ __noinline__ void gv_first_prologue(const void* xp, int dtype, const 
         if (has > 1) off1 = __ldg(soff + 4);
     }
     griddep_wait();
-#ifdef HQ_TRACE
-    if (lane == 0) g_gv_trace[((size_t)tr_slot * 148 * 32 + (size_t)blockIdx.x * 32 + wid) * 12 + 9] = gv_now();
-#endif
     const bool vec = dtype == HQ_BF16 ? (((uintptr_t)xp) & 7) == 0 : (((uintptr_t)xp) & 15) == 0;
     const int col0 = act_col0(lane);
     float x[4], xn[4];
@@ -282,9 +269,6 @@ __device__ __noinline__ void gv_first_prologue(const void* xp, int dtype, const 
     if (ragged_due) gv_load_ragged<KW>(sgp, dense, stg_a, ul);
     sts32(ret_a, ul); sts32(ret_a + 4, nrm); sts32(ret_a + 8, off1); sts32(ret_a + 12, off0);
     fence_proxy_async_smem();   // the operand is read by the tensor core (async proxy)
-#ifdef HQ_TRACE
-    if (lane == 0) g_gv_trace[((size_t)tr_slot * 148 * 32 + (size_t)blockIdx.x * 32 + wid) * 12 + 10] = gv_now();
-#endif
     __syncthreads();
 }
 
@@ -306,7 +290,6 @@ k_gemv_e8(E8Params p) {
     // the warp index through a shuffle: the compiler then knows it is warp-uniform (descriptors stay in uniform registers)
     const int wid = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
     const int tid = threadIdx.x, wg = wid >> 2, warp = wid & 3, lane = tid & 31, t = warp * 32 + lane;
-    GV_TR(0);
     const uint32_t smem_a = smem_u32(smem);
     const uint32_t xq_a = smem_a + E8_LUT_BYTES;                                  // activation operand, 1024-aligned
     const uint32_t XQB = gv_xq_bytes(p.n_kt);
@@ -330,7 +313,6 @@ k_gemv_e8(E8Params p) {
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
-    GV_TR(1);
     griddep_launch();
     if (tid == 0) {  // the phase-1 table arrives by one TMA bulk copy while the first loads are in flight
         mbar_arrive_expect_tx(bar_lut, E8_LUT_BYTES);
@@ -356,14 +338,9 @@ k_gemv_e8(E8Params p) {
     // the K-tiles this CTA's tile range touches: kt0 + j (mod n_kt), j < nt_cta - the only activation tiles it quantizes
     const int64_t cta_b = ((int64_t)blockIdx.x * NWG * T) / GWG, cta_e = ((int64_t)(blockIdx.x + 1) * NWG * T) / GWG;
     const int nt_cta = (int)min((int64_t)n_kt, cta_e - cta_b), kt0_cta = (int)(cta_b % n_kt);
-#ifdef HQ_TRACE
-#define GV_TRARG , (p.n_items >> 9) & 7
-#else
-#define GV_TRARG
-#endif
 
     if (f >= f_end) {   // nothing to do for this warp group: it still helps with the activations and joins the barriers
-        gv_first_prologue<K, NW>(p.x, p.dtype, p.dsign, n_kt, xq_a, sx_a, wid, lane, kt0_cta, nt_cta, nullptr, nullptr, 0, 0, stg_a, scr_a GV_TRARG);
+        gv_first_prologue<K, NW>(p.x, p.dtype, p.dsign, n_kt, xq_a, sx_a, wid, lane, kt0_cta, nt_cta, nullptr, nullptr, 0, 0, stg_a, scr_a);
         tc_fence_before();
         __syncthreads();
         if (wid == 0) tmem_dealloc(*tmem_slot, 512);
@@ -411,18 +388,12 @@ k_gemv_e8(E8Params p) {
         uint32_t off_n1;
         const uint8_t* sgp_c;
         if (first_seg) {   // the kernel's first tile: its loads are interleaved with the activation prologue (all warps meet there)
-            GV_TR(2);
             gv_first_prologue<K, NW>(p.x, p.dtype, p.dsign, n_kt, xq_a, sx_a, wid, lane, kt0_cta, nt_cta, blob, soff,
-                                     (ka + 1 < kb) ? 2 : 1, dense ? 1 : 0, stg_a, scr_a GV_TRARG);
+                                     (ka + 1 < kb) ? 2 : 1, dense ? 1 : 0, stg_a, scr_a);
             first_seg = false;
-            GV_TR(3);
             ul_c = lds32(scr_a); nrm_c = lds32(scr_a + 4); off_n1 = lds32(scr_a + 8);
             sgp_c = blob + 16 * (size_t)lds32(scr_a + 12);
             mbar_wait(bar_lut, 0u);
-#ifdef HQ_TRACE
-            cp_async_wait_all();
-            GV_TR(4);
-#endif
         } else {
             off_n1 = (ka + 1 < kb) ? __ldg(soff + 4) : 0u;
             sgp_c = blob + 16 * (size_t)__ldg(soff);
@@ -538,7 +509,6 @@ k_gemv_e8(E8Params p) {
         }
         yacc = 0.0f;
     }
-    GV_TR(5);
     // ---- split-K reduction inside the kernel: publish this thread's partial sums (one fence), then arrive once per cut
     // row block of the range on a per-(row block, warp) counter; the LAST of the row block's segments to arrive adds the
     // partials in slot order - deterministic - and writes y (A7).  No block barrier, no extra launch.
@@ -546,7 +516,6 @@ k_gemv_e8(E8Params p) {
     // ordered before it; acquire: the other segments' partials) -> __syncwarp -> the lanes' L2 loads.  One atomic round trip
     // instead of fence + atomic + fence.
     __syncwarp();
-    GV_TR(6);
     for (int ff = f_begin; ff < f_end;) {
         const int rbg = ff / n_kt, ka = ff - rbg * n_kt;
         const int kb = min(n_kt, ka + (f_end - ff));
@@ -584,10 +553,8 @@ k_gemv_e8(E8Params p) {
         if (p.y_bf16[w]) p.y_bf16[w][r] = __float2bfloat16_rn(sum);
         if (p.y_f32[w]) p.y_f32[w][r] = sum;
     }
-    GV_TR(7);
     tc_fence_before();
     __syncthreads();
-    GV_TR(8);
     if (wid == 0) tmem_dealloc(*tmem_slot, 512);
 }
 

@@ -604,10 +604,3 @@ hq_status launch_linear(hq_ctx* ctx, const hq_weight* w, const void* x, int dtyp
 }
 
 }  // namespace hq
-
-#ifdef HQ_TRACE
-extern "C" int hq_debug_trace(unsigned long long* host_out, long long n_words) {
-    cudaDeviceSynchronize();
-    return (int)cudaMemcpyFromSymbol(host_out, hq::g_gv_trace, (size_t)n_words * 8);
-}
-#endif
