@@ -207,6 +207,26 @@ hq_status hq_linear_group(hq_ctx* ctx, const hq_weight* const* ws, int32_t n_w, 
                           int64_t batch, int64_t ldx, void* const* ys_bf16_dev, const int64_t* ldys,
                           float* const* ys_f32_or_null, void* stream);
 
+/*
+ * hq_linear for ONE activation row that allocates nothing: for callers that cannot call cudaMalloc (code under CUDA
+ * graph capture, tight serving loops, harnesses that forbid it).  Same kernel and same result as hq_linear at batch 1 on
+ * the E8 / tile 128 / k <= 3 path (k_gemv_e8: x [n_in] dev -> y [m_out] bf16 dev and/or y_f32 [m_out] dev, at least one
+ * non-NULL); the kernel's scratch (split-K arrival counters and partial sums) lives in a file-scope device array of
+ * HQ_LINEAR_STATIC_SCRATCH_BYTES inside the library instead of the allocator-backed workspace.  Every GPU that loads the
+ * library holds that array until the process exits.  The call makes no cudaMalloc / cudaFree / allocator call: it
+ * enqueues one cudaMemsetAsync (the counters must start at zero; the array keeps the previous call's contents) and one
+ * kernel on `stream`.  ALL calls on a device share the array: calls that overlap on the GPU (two streams, two contexts,
+ * two threads) race on it - serialize them.  Limits: other lattices / tiles / k > 3 / n_in > 16384 -> HQ_ERR_UNSUPPORTED;
+ * a weight whose scratch does not fit -> HQ_ERR_SHAPE, hq_last_error says by how much.  The array holds 32 KiB of
+ * counters (16 bytes per 128 rows: m_out <= 262144) and 2 064 384 bytes of partial sums (slots * m_out * 4, slots = the
+ * segments the launch's tile partition cuts a row block's K range into, <= n_in / 128 + 1): on a 148-SM device every
+ * weight with m_out <= 160 000 fits, whatever its n_in.  The array's device address is taken once per device at hq_create (cudaGetSymbolAddress); if that failed the
+ * call returns HQ_ERR_CUDA.
+ */
+#define HQ_LINEAR_STATIC_SCRATCH_BYTES (2u * 1024u * 1024u)
+hq_status hq_linear_static(hq_ctx* ctx, const hq_weight* w, const void* x_dev, int32_t dtype, void* y_bf16_dev,
+                           float* y_f32_dev_or_null, void* stream);
+
 /* bytes of scratch hq_linear needs for this (weight, batch); it is taken from the ctx allocator and cached. */
 hq_status hq_linear_workspace_bytes(const hq_weight* w, int64_t batch, size_t* bytes);
 

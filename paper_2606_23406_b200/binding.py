@@ -73,7 +73,7 @@ _lib = None
 EXPORTS = ["hq_create", "hq_destroy", "hq_last_error", "hq_measure_decode_ceiling", "hq_alpha", "hq_snr_for_bps", "hq_profile_enable", "hq_profile_read",
            "hq_encode_weights", "hq_weight_free", "hq_weight_get_info", "hq_weight_stats", "hq_weight_export",
            "hq_weight_export_host", "hq_weight_import", "hq_decode_int8", "hq_act_quant", "hq_linear",
-           "hq_linear_group", "hq_linear_workspace_bytes", "hq_kv_create", "hq_kv_free", "hq_kv_append", "hq_attend", "hq_kv_export",
+           "hq_linear_group", "hq_linear_static", "hq_linear_workspace_bytes", "hq_kv_create", "hq_kv_free", "hq_kv_append", "hq_attend", "hq_kv_export",
            "hq_kv_decode_int8"]
 
 
@@ -105,6 +105,7 @@ def load_library():
     lib.hq_decode_int8.argtypes = [vp, vp, vp, vp, vp]
     lib.hq_act_quant.argtypes = [vp, vp, vp, i32, i64, i64, vp, vp, vp, vp]
     lib.hq_linear.argtypes = [vp, vp, vp, i32, i64, i64, vp, i64, vp, vp, vp]
+    lib.hq_linear_static.argtypes = [vp, vp, vp, i32, vp, vp, vp]
     lib.hq_linear_group.argtypes = [vp, C.POINTER(vp), i32, vp, i32, i64, i64, C.POINTER(vp), C.POINTER(i64), C.POINTER(vp), vp]
     lib.hq_linear_workspace_bytes.argtypes = [vp, i64, C.POINTER(C.c_size_t)]
     lib.hq_kv_create.argtypes = [vp, C.POINTER(_KVConfig), C.POINTER(vp)]
@@ -312,6 +313,17 @@ class Weight:
                                               acc.data_ptr() if want_acc else None, _stream_ptr(dev)))
         if want_f32 or want_acc:
             return y, y32, acc
+        return y
+
+
+    def linear_static(self, x: torch.Tensor, y: torch.Tensor, y32: torch.Tensor = None):
+        """hq_linear_static: one activation row, outputs given by the caller, no allocation anywhere in the call."""
+        assert x.is_cuda and x.numel() == self.n_in and x.is_contiguous()
+        assert y is None or (y.is_cuda and y.dtype == torch.bfloat16 and y.numel() == self.m and y.is_contiguous())
+        assert y32 is None or (y32.is_cuda and y32.dtype == torch.float32 and y32.numel() == self.m and y32.is_contiguous())
+        self.ctx.check(self.ctx.lib.hq_linear_static(self.ctx.h, self.h, x.data_ptr(), _dtype_code(x),
+                                                     y.data_ptr() if y is not None else None,
+                                                     y32.data_ptr() if y32 is not None else None, _stream_ptr(self.ctx.device)))
         return y
 
 

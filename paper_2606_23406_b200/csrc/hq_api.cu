@@ -89,6 +89,8 @@ hq_status hq_create(hq_ctx** out, const hq_allocator* alloc, int cuda_device) {
         delete ctx;
         return HQ_ERR_CUDA;
     }
+    // set-up for hq_linear_static (the device is current): a failure here only disables that entry point
+    (void)linear_static_setup(ctx);
     *out = ctx;
     return HQ_OK;
 }
@@ -455,6 +457,16 @@ hq_status hq_linear(hq_ctx* ctx, const hq_weight* w, const void* x_dev, int32_t 
     }
     return launch_linear(ctx, w, x_dev, dtype, batch, ldx, y_bf16_dev, ldy, y_f32_dev_or_null, acc_i32_dev_or_null,
                          (uint8_t*)ctx->ws, st);
+}
+
+hq_status hq_linear_static(hq_ctx* ctx, const hq_weight* w, const void* x_dev, int32_t dtype, void* y_bf16_dev,
+                           float* y_f32_dev_or_null, void* stream) {
+    if (!ctx) return HQ_ERR_INVALID_ARG;
+    if (!w || !x_dev || (!y_bf16_dev && !y_f32_dev_or_null)) return fail(ctx, HQ_ERR_INVALID_ARG, "null argument");
+    if (dtype != HQ_F32 && dtype != HQ_BF16) return fail(ctx, HQ_ERR_INVALID_ARG, "bad dtype");
+    if (w->ctx != ctx) return fail(ctx, HQ_ERR_INVALID_ARG, "the weight belongs to another context");
+    HQ_ENTER(ctx);
+    return launch_linear_static(ctx, w, x_dev, dtype, y_bf16_dev, y_f32_dev_or_null, (cudaStream_t)stream);
 }
 
 hq_status hq_linear_group(hq_ctx* ctx, const hq_weight* const* ws, int32_t n_w, const void* x_dev, int32_t dtype,

@@ -28,6 +28,9 @@ struct hq_ctx {
     // two timing-free events; everything stays ordered with respect to the caller's stream (graph-capturable)
     cudaStream_t side = nullptr;
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    // device address of the library's file-scope scratch array on this device (hq_linear_static), from
+    // cudaGetSymbolAddress at hq_create; null if that failed
+    uint8_t* static_scratch = nullptr;
 };
 
 struct hq_weight {
@@ -154,6 +157,10 @@ hq_status launch_linear_group(hq_ctx* ctx, const hq_weight* const* ws, int n_w, 
                               int32_t* acc_i32, uint8_t* wsbuf, cudaStream_t st);
 bool linear_uses_e8_fast(const hq_weight* w);
 hq_status launch_decode_ceiling(hq_ctx* ctx, const hq_weight* w, int reps, cudaStream_t st, double* scalars_per_s);
+// hq_linear_static: the address of the static scratch array (once per device, that device current), and the launch
+hq_status linear_static_setup(hq_ctx* ctx);
+hq_status launch_linear_static(hq_ctx* ctx, const hq_weight* w, const void* x, int dtype, void* y_bf16, float* y_f32,
+                               cudaStream_t st);
 
 // ---- KV decode + attend (hq_attend.cu) ----
 void launch_kv_decode_int8(const hq_kv* kv, int role, int64_t t0, int64_t n, int8_t* codes, cudaStream_t st);

@@ -7,6 +7,9 @@
 // (from 64 rows) decodes once per call into an operand-layout scratch copy (hq_linear_large.cuh).
 #include <string.h>
 
+#include <mutex>
+#include <string>
+
 #include "hq_common.cuh"
 #include "hq_internal.h"
 #include "hq_linear_e8.cuh"
@@ -601,6 +604,79 @@ hq_status launch_linear(hq_ctx* ctx, const hq_weight* w, const void* x, int dtyp
     HQ_CUDA_CHECK(ctx, launch_pdl(k_linear_finalize, dim3((unsigned)((tot + 255) / 256)), dim3(256), 0, st, (const float*)partials,
                                   n_split, B, w->m, (__nv_bfloat16*)y_bf16, ldy, y_f32));
     return HQ_OK;
+}
+
+}  // namespace hq
+
+// ---------------------------------------------------------------------------------------------
+// hq_linear_static (include/hq.h): the batch-1 fused kernel (k_gemv_e8) with its scratch - the split-K arrival
+// counters and partial sums - in a file-scope device array instead of the context's allocator-backed workspace, for
+// callers that may not allocate (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc).  Every GPU
+// that loads the library holds the array until the process exits.  All calls share it and it keeps the last call's
+// contents: the counters are cleared on the caller's stream before every launch; the partial sums need no clearing
+// (every slot that is read was written by the same launch).  Calls that overlap on the GPU race on it.
+namespace hq {
+
+constexpr size_t ST_CNT_BYTES = 32u * 1024u;                       // 2048 row blocks x 4 warps x u32
+constexpr size_t ST_PART_BYTES = HQ_LINEAR_STATIC_SCRATCH_BYTES - ST_CNT_BYTES;
+static __device__ __align__(256) unsigned char g_static_scratch[HQ_LINEAR_STATIC_SCRATCH_BYTES];
+
+// The array's name is a host-side stand-in in host code, not a device address: the address a kernel may use comes from
+// cudaGetSymbolAddress, asked once per device with that device current (hq_create calls this).
+constexpr int ST_MAX_DEV = 64;
+static std::mutex g_static_mu;
+static void* g_static_ptr[ST_MAX_DEV];
+
+hq_status linear_static_setup(hq_ctx* ctx) {
+    if (ctx->device < 0 || ctx->device >= ST_MAX_DEV) { ctx->err = "device index beyond the static scratch table"; return HQ_ERR_UNSUPPORTED; }
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (!g_static_ptr[ctx->device]) {
+        void* ptr = nullptr;
+        cudaError_t e = cudaGetSymbolAddress(&ptr, g_static_scratch);
+        if (e != cudaSuccess || !ptr) {
+            ctx->err = std::string("cudaGetSymbolAddress(static scratch): ") + cudaGetErrorString(e);
+            return HQ_ERR_CUDA;
+        }
+        g_static_ptr[ctx->device] = ptr;
+    }
+    ctx->static_scratch = (uint8_t*)g_static_ptr[ctx->device];
+    return HQ_OK;
+}
+
+hq_status launch_linear_static(hq_ctx* ctx, const hq_weight* w, const void* x, int dtype, void* y_bf16, float* y_f32,
+                               cudaStream_t st) {
+    if (!ctx->static_scratch) { ctx->err = "the static scratch address was not obtained at hq_create"; return HQ_ERR_CUDA; }
+    if (!linear_uses_e8_fast(w) || w->n_kt > GV_MAX_KT) {
+        ctx->err = "hq_linear_static takes E8 / tile 128 / k <= 3 weights with n_in <= 16384";
+        return HQ_ERR_UNSUPPORTED;
+    }
+    const int64_t n_rb = w->n_rb, n_kt = w->n_kt;
+    if (n_rb >= 65536 || n_rb * n_kt >= (1ll << 31)) { ctx->err = "m_out too large for the fused kernel"; return HQ_ERR_SHAPE; }
+    const size_t cnt_need = (size_t)n_rb * 4 * sizeof(unsigned int);
+    const size_t part_need = (size_t)gv_slots(ctx, n_rb, n_kt) * (size_t)w->m * 4;
+    if (cnt_need > ST_CNT_BYTES || part_need > ST_PART_BYTES) {
+        ctx->err = "hq_linear_static: this weight needs " + std::to_string(cnt_need) + " counter bytes and " + std::to_string(part_need) +
+                   " partial-sum bytes; the static scratch holds " + std::to_string(ST_CNT_BYTES) + " + " + std::to_string(ST_PART_BYTES) +
+                   " (m_out <= 262144): use hq_linear";
+        return HQ_ERR_SHAPE;
+    }
+    E8Plan pl = e8_plan(ctx, n_rb, n_kt, w->n_in, 1);
+    E8Params p;
+    memset(&p, 0, sizeof(p));
+    p.blob[0] = w->blob; p.sub_off[0] = w->group_off; p.m[0] = w->m;
+    p.counters = (unsigned int*)ctx->static_scratch;
+    p.partials[0] = (float*)(ctx->static_scratch + ST_CNT_BYTES);
+    p.inv_A[0] = (float)(1.0 / (w->alpha * sqrt((double)w->n)));
+    for (int i = 0; i < E8_MAXW; ++i) p.rb_base[i + 1] = (int)n_rb;
+    p.y_bf16[0] = (__nv_bfloat16*)y_bf16; p.ldy[0] = w->m; p.y_f32[0] = y_f32;
+    p.n_w = 1; p.lut = ctx->e8_lut;
+    p.n_kt = (int)n_kt; p.n_split = pl.n_split; p.L = pl.L; p.n_bt = 1;
+    p.n_items = (int)(n_rb * n_kt);   // the batch-1 kernel partitions tiles
+    p.u_dense = ((w->min_ulen + 31) >> 5) >= (uint32_t)E8_DENSE ? E8_DENSE : 0;
+    p.B = 1; p.x = x; p.dtype = dtype; p.dsign = w->dsign;
+    // what must start at zero: the arrival counters (the partial sums are written before they are read)
+    HQ_CUDA_CHECK(ctx, cudaMemsetAsync(p.counters, 0, cnt_need, st));
+    return gv_pick_nwg(ctx, p.n_items) == 4 ? launch_gemv<4>(ctx, w->k0, p, pl, st) : launch_gemv<5>(ctx, w->k0, p, pl, st);
 }
 
 }  // namespace hq
