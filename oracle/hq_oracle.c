@@ -14,7 +14,9 @@
  * Parity pins (tests/test_oracle_*.py): Philox known-answer vectors; H·Hᵀ = n·I and the dense
  * double RHT; brute-force nearest point; Voronoi second moments vs Table 2 (L139-142); strip
  * bijection and Table 3 savings (L284); Rice round trip; printed rates at 21 dB (L289); Table 14
- * α (L887-890); Table 11 A2 SNRs (L550-552); dither moments and unbiasedness (L786-808).
+ * α (L887-890); Table 11 A2 SNRs (L550-552); dither moments and unbiasedness (L786-808);
+ * the layer glue of FORMAT R8-R10 (RMSNorm, SiLU·mul, bf16 rounding) against numpy float64 / ml_dtypes-free
+ * bit manipulation (tests/test_oracle_layer.py).
  * Parity unpinned: none.
  */
 #include <math.h>
@@ -760,6 +762,63 @@ void hqo_act_quant(const float* x, int64_t B, int64_t n_in, int64_t ldx, int lat
             s_x[b * n_kt + kt] = amax / 127.0f;
         }
     free(d);
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* The steps between the linears of a decoder layer that fold into the activation cast           */
+/* (§4.1: "the butterfly folds into the preceding LayerNorm"; FORMAT R8-R10). */
+/* They produce the bf16 activation vector that hqo_act_quant then takes, so they decide integers */
+/* and are canonical fp32.                                                                        */
+/* ------------------------------------------------------------------------------------------ */
+float hqo_bf16_round(float v) { /* fp32 -> bf16 (round to nearest even) -> fp32 */
+    uint32_t b;
+    memcpy(&b, &v, 4);
+    if ((b & 0x7f800000u) == 0x7f800000u) return v; /* inf / nan unchanged */
+    b += 0x7fffu + ((b >> 16) & 1u);
+    b &= 0xffff0000u;
+    memcpy(&v, &b, 4);
+    return v;
+}
+
+void hqo_bf16_round_array(const float* v, int64_t n, float* out) {
+    for (int64_t i = 0; i < n; ++i) out[i] = hqo_bf16_round(v[i]);
+}
+
+/* FORMAT R8: x_i = bf16((h_i * r) * g_i), r = 1 / sqrt(treesum(h_i^2) / n + eps). */
+void hqo_rmsnorm_bf16(const float* h, const float* g, int64_t n, float eps, float* x) {
+    float* sq = (float*)malloc((size_t)n * sizeof(float));
+    for (int64_t i = 0; i < n; ++i) sq[i] = h[i] * h[i];
+    float s = treesum_f32(sq, (int)n);
+    free(sq);
+    float ms = s / (float)n;
+    float r = 1.0f / sqrtf(ms + eps);
+    for (int64_t i = 0; i < n; ++i) x[i] = hqo_bf16_round((h[i] * r) * g[i]);
+}
+
+/* FORMAT R9: the canonical exponential (range reduction by ln 2 in two parts, degree-7 Taylor polynomial in Horner
+ * form with fused multiply-adds, scaling by the exponent bits). */
+float hqo_exp_c(float t) {
+    if (t < -87.0f) t = -87.0f;
+    if (t > 88.0f) t = 88.0f;
+    float m = rintf(t * 0x1.715476p+0f);
+    float f = fmaf(m, -0x1.62e000p-1f, t);
+    f = fmaf(m, -0x1.0bfbe8p-15f, f);
+    static const float C[8] = {1.0f, 1.0f, 0.5f, 0x1.555556p-3f, 0x1.555556p-5f, 0x1.111112p-7f, 0x1.6c16c2p-10f, 0x1.a01a02p-13f};
+    float p = C[7];
+    for (int j = 6; j >= 0; --j) p = fmaf(p, f, C[j]);
+    uint32_t eb = (uint32_t)((int)m + 127) << 23;
+    float two_m;
+    memcpy(&two_m, &eb, 4);
+    return p * two_m;
+}
+
+/* FORMAT R9: x_i = bf16(silu_c(a_i) * b_i), silu_c(a) = a / (1 + exp_c(-a)). */
+void hqo_silu_mul_bf16(const float* a, const float* b, int64_t n, float* x) {
+    for (int64_t i = 0; i < n; ++i) {
+        float e = hqo_exp_c(-a[i]);
+        float s = a[i] / (1.0f + e);
+        x[i] = hqo_bf16_round(s * b[i]);
+    }
 }
 
 /* acc[kt,b,r] = Σ_{i in tile} c[r,i]·q[b,i];  y[b,r] = Σ_kt (ρ[r,kt]/(α√n))·s_x[b,kt]·acc  (double) */

@@ -320,3 +320,27 @@ def snr_for_bps(tiles, lattice, target_bps, lo=0.0, hi=45.0, iters=18):
         else:
             hi = mid
     return 0.5 * (lo + hi)
+
+
+# ---- layer glue that folds into the activation cast (FORMAT R8-R10)
+def bf16_round(x):
+    x = _c(x, np.float32); out = np.empty_like(x)
+    lib().hqo_bf16_round_array(_p(x), C.c_int64(x.size), _p(out))
+    return out
+
+
+def rmsnorm_bf16(h, g, eps):
+    h = _c(h, np.float32); g = _c(g, np.float32); x = np.empty_like(h)
+    lib().hqo_rmsnorm_bf16(_p(h), _p(g), C.c_int64(h.size), C.c_float(eps), _p(x))
+    return x
+
+
+def exp_c(t):
+    f = lib().hqo_exp_c; f.restype = C.c_float; f.argtypes = [C.c_float]
+    return np.array([f(float(v)) for v in np.asarray(t, np.float32).reshape(-1)], np.float32)
+
+
+def silu_mul_bf16(a, b):
+    a = _c(a, np.float32); b = _c(b, np.float32); x = np.empty_like(a)
+    lib().hqo_silu_mul_bf16(_p(a), _p(b), C.c_int64(a.size), _p(x))
+    return x
