@@ -227,6 +227,60 @@ hq_status hq_linear_group(hq_ctx* ctx, const hq_weight* const* ws, int32_t n_w, 
 hq_status hq_linear_static(hq_ctx* ctx, const hq_weight* w, const void* x_dev, int32_t dtype, void* y_bf16_dev,
                            float* y_f32_dev_or_null, void* stream);
 
+/* ---- a decoder layer's decode step: the glue between the linears folded into their kernels ---- */
+/*
+ * PAPER.md:L212 (§4.1): "the butterfly folds into the preceding LayerNorm"; Table 10's decode shape
+ * (L496-511).  At batch 1 the fused kernel (k_gemv_e8) quantizes the activation vector itself, so the element-wise steps
+ * that precede a linear run inside its prologue and the residual add inside its epilogue - no kernel of their own, no
+ * round trip of the normalised vector through HBM.  Canonical arithmetic: docs/FORMAT.md R8 (RMSNorm), R9 (SiLU.mul),
+ * R10 (residual); each fold is bit-identical to a separate kernel that writes its result in bf16.
+ *   HQ_FOLD_RMSNORM : x_dev = residual stream h [n_in] bf16, aux_dev = gain g [n_in] bf16:  x_i = bf16((h_i r) g_i),
+ *                     r = 1 / sqrt(mean(h^2) + eps).  Every CTA recomputes r from the 2 n_in bytes of h (L2 hits).
+ *   HQ_FOLD_SILU_MUL: x_dev = gate a [n_in] bf16, aux_dev = up b [n_in] bf16:  x_i = bf16(silu(a_i) b_i).
+ *   residuals_dev   : NULL, or n_w device pointers (entries may be NULL): bf16 [m_i] added to output i before the bf16
+ *                     cast (y_f32 then carries the sum).  A residual may alias its output.
+ * x_dev and aux_dev must be 8-byte aligned.  Batch 1, bf16, E8 / tile 128 / k <= 3 weights that can share a launch
+ * (as hq_linear_group), n_in <= 16384: anything else -> HQ_ERR_UNSUPPORTED (there is no unfused fallback).
+ */
+typedef enum { HQ_FOLD_NONE = 0, HQ_FOLD_RMSNORM = 1, HQ_FOLD_SILU_MUL = 2 } hq_fold_mode;
+typedef struct {
+    int32_t mode;                      /* hq_fold_mode */
+    float eps;                         /* HQ_FOLD_RMSNORM */
+    const void* aux_dev;               /* gain (RMSNORM) or second factor (SILU_MUL); NULL for HQ_FOLD_NONE */
+    const void* const* residuals_dev;  /* NULL or n_w pointers */
+} hq_fold;
+hq_status hq_linear_group_fold(hq_ctx* ctx, const hq_weight* const* ws, int32_t n_w, const void* x_dev,
+                               const hq_fold* fold, void* const* ys_bf16_dev, float* const* ys_f32_or_null, void* stream);
+
+/*
+ * One decode step (one token) of a Llama-style decoder layer on compressed weights and a compressed KV cache, seven
+ * launches in stream order, no host synchronisation, no allocation after the first call at a given shape:
+ *   q,k,v = W_{q,k,v} RMSNorm(h; g_attn)      hq_linear_group_fold, RMSNorm in the prologue        (1 launch)
+ *   cache <- (k, v)                            hq_kv_append                                         (1 launch)
+ *   a = attend(q)                              hq_attend                                            (2 launches)
+ *   h2 = h + W_o a                             hq_linear_group_fold, residual in the epilogue       (1 launch)
+ *   gate, up = W_{gate,up} RMSNorm(h2; g_mlp)  hq_linear_group_fold, RMSNorm in the prologue        (1 launch)
+ *   h_out = h2 + W_down (silu(gate) * up)      hq_linear_group_fold, SiLU.mul prologue + residual   (1 launch)
+ * Rotary position embedding is not part of the paper's method and is not applied (the weights are synthetic).
+ * h_in, h_out [hidden] bf16 dev (may alias).  scratch_dev: hq_layer_scratch_bytes() bytes, 256-byte aligned, holds q, k, v,
+ * a, h2, gate, up (bf16); hq_layer_scratch_view returns their offsets for parity tests.  The token position is host state
+ * of the cache (hq_kv_append): a captured CUDA graph of this call replays the SAME position.
+ * Shapes: wq [q_heads d, hidden], wk / wv [kv_heads d, hidden], wo [hidden, q_heads d], wgate / wup [ffn, hidden],
+ * wdown [hidden, ffn]; d = the cache's head_dim.  Mismatch -> HQ_ERR_SHAPE.
+ */
+typedef struct {
+    const hq_weight *wq, *wk, *wv, *wo, *wgate, *wup, *wdown;
+    const void* g_attn_dev;   /* [hidden] bf16 */
+    const void* g_mlp_dev;    /* [hidden] bf16 */
+    float eps;
+    hq_kv* kv;
+    int32_t q_heads;
+} hq_layer;
+typedef struct { size_t q, k, v, a, h2, gate, up, total; } hq_layer_scratch;   /* byte offsets into scratch_dev */
+hq_status hq_layer_scratch_view(const hq_layer* layer, hq_layer_scratch* out);
+hq_status hq_layer_decode(hq_ctx* ctx, const hq_layer* layer, const void* h_in_dev, void* h_out_dev, void* scratch_dev,
+                          size_t scratch_bytes, void* stream);
+
 /* bytes of scratch hq_linear needs for this (weight, batch); it is taken from the ctx allocator and cached. */
 hq_status hq_linear_workspace_bytes(const hq_weight* w, int64_t batch, size_t* bytes);
 

@@ -57,6 +57,23 @@ class WeightHeader(C.Structure):
                 ("ulen_max", C.c_int32)]
 
 
+class _Fold(C.Structure):
+    _fields_ = [("mode", C.c_int32), ("eps", C.c_float), ("aux_dev", C.c_void_p), ("residuals_dev", C.POINTER(C.c_void_p))]
+
+
+class _Layer(C.Structure):
+    _fields_ = [("wq", C.c_void_p), ("wk", C.c_void_p), ("wv", C.c_void_p), ("wo", C.c_void_p), ("wgate", C.c_void_p),
+                ("wup", C.c_void_p), ("wdown", C.c_void_p), ("g_attn_dev", C.c_void_p), ("g_mlp_dev", C.c_void_p),
+                ("eps", C.c_float), ("kv", C.c_void_p), ("q_heads", C.c_int32)]
+
+
+class _LayerScratch(C.Structure):
+    _fields_ = [(n, C.c_size_t) for n in ("q", "k", "v", "a", "h2", "gate", "up", "total")]
+
+
+FOLD_NONE, FOLD_RMSNORM, FOLD_SILU_MUL = 0, 1, 2
+
+
 class _KVView(C.Structure):
     _fields_ = [("n_tokens", C.c_int64), ("rbits", C.c_int64), ("rem_dev", C.c_void_p), ("una_dev", C.c_void_p),
                 ("ulen_dev", C.c_void_p), ("norm_dev", C.c_void_p), ("blk_off_dev", C.c_void_p),
@@ -73,7 +90,7 @@ _lib = None
 EXPORTS = ["hq_create", "hq_destroy", "hq_last_error", "hq_measure_decode_ceiling", "hq_alpha", "hq_snr_for_bps", "hq_profile_enable", "hq_profile_read",
            "hq_encode_weights", "hq_weight_free", "hq_weight_get_info", "hq_weight_stats", "hq_weight_export",
            "hq_weight_export_host", "hq_weight_import", "hq_decode_int8", "hq_act_quant", "hq_linear",
-           "hq_linear_group", "hq_linear_static", "hq_linear_workspace_bytes", "hq_kv_create", "hq_kv_free", "hq_kv_append", "hq_attend", "hq_kv_export",
+           "hq_linear_group", "hq_linear_group_fold", "hq_layer_scratch_view", "hq_layer_decode", "hq_linear_static", "hq_linear_workspace_bytes", "hq_kv_create", "hq_kv_free", "hq_kv_append", "hq_attend", "hq_kv_export",
            "hq_kv_decode_int8"]
 
 
@@ -107,6 +124,9 @@ def load_library():
     lib.hq_linear.argtypes = [vp, vp, vp, i32, i64, i64, vp, i64, vp, vp, vp]
     lib.hq_linear_static.argtypes = [vp, vp, vp, i32, vp, vp, vp]
     lib.hq_linear_group.argtypes = [vp, C.POINTER(vp), i32, vp, i32, i64, i64, C.POINTER(vp), C.POINTER(i64), C.POINTER(vp), vp]
+    lib.hq_linear_group_fold.argtypes = [vp, C.POINTER(vp), i32, vp, C.POINTER(_Fold), C.POINTER(vp), C.POINTER(vp), vp]
+    lib.hq_layer_scratch_view.argtypes = [C.POINTER(_Layer), C.POINTER(_LayerScratch)]
+    lib.hq_layer_decode.argtypes = [vp, C.POINTER(_Layer), vp, vp, vp, C.c_size_t, vp]
     lib.hq_linear_workspace_bytes.argtypes = [vp, i64, C.POINTER(C.c_size_t)]
     lib.hq_kv_create.argtypes = [vp, C.POINTER(_KVConfig), C.POINTER(vp)]
     lib.hq_kv_free.argtypes = [vp, vp]; lib.hq_kv_free.restype = None
@@ -214,6 +234,26 @@ class Context:
         self.check(self.lib.hq_linear_group(self.h, wa, n, x.data_ptr(), _dtype_code(x), B, x.stride(0), ya, la, fa,
                                             _stream_ptr(self.device)))
         return (ys, y32) if want_f32 else ys
+
+    def linear_group_fold(self, weights, x: torch.Tensor, mode=FOLD_NONE, aux: torch.Tensor = None, eps=0.0,
+                          residuals=None, ys=None, want_f32=False):
+        """hq_linear_group_fold: batch-1 linears with RMSNorm / SiLU.mul folded into the prologue and an optional
+        residual add in the epilogue (x, aux, residuals: bf16 vectors)."""
+        n = len(weights)
+        assert 1 <= n <= 4 and x.is_cuda and x.dtype == torch.bfloat16 and x.dim() == 1 and x.is_contiguous()
+        if ys is None:
+            ys = [torch.empty((w.m,), dtype=torch.bfloat16, device=self.device) for w in weights]
+        y32 = [torch.empty((w.m,), dtype=torch.float32, device=self.device) for w in weights] if want_f32 else None
+        wa = (C.c_void_p * n)(*[w.h for w in weights])
+        ya = (C.c_void_p * n)(*[y.data_ptr() for y in ys])
+        fa = (C.c_void_p * n)(*[t.data_ptr() for t in y32]) if want_f32 else None
+        ra = (C.c_void_p * n)(*[(r.data_ptr() if r is not None else None) for r in residuals]) if residuals else None
+        fold = _Fold(int(mode), float(eps), aux.data_ptr() if aux is not None else None, ra)
+        self.check(self.lib.hq_linear_group_fold(self.h, wa, n, x.data_ptr(), C.byref(fold), ya, fa, _stream_ptr(self.device)))
+        return (ys, y32) if want_f32 else ys
+
+    def layer(self, wq, wk, wv, wo, wgate, wup, wdown, g_attn: torch.Tensor, g_mlp: torch.Tensor, eps, kv, q_heads):
+        return Layer(self, (wq, wk, wv, wo, wgate, wup, wdown), g_attn, g_mlp, eps, kv, q_heads)
 
     def import_weight(self, header: "WeightHeader", blob, sub_off):
         """hq_weight_import from host numpy arrays (the pair Weight.export_host returns)."""
@@ -325,6 +365,32 @@ class Weight:
                                                      y.data_ptr() if y is not None else None,
                                                      y32.data_ptr() if y32 is not None else None, _stream_ptr(self.ctx.device)))
         return y
+
+
+class Layer:
+    """hq_layer / hq_layer_decode: one decode step of a decoder layer (seven launches, glue folded into the linears)."""
+
+    def __init__(self, ctx: Context, weights, g_attn, g_mlp, eps, kv, q_heads):
+        self.ctx, self.weights, self.g_attn, self.g_mlp, self.kv = ctx, weights, g_attn, g_mlp, kv
+        self.c = _Layer(*[w.h for w in weights], g_attn.data_ptr(), g_mlp.data_ptr(), float(eps), kv.h, int(q_heads))
+        self.view = _LayerScratch()
+        ctx.check(ctx.lib.hq_layer_scratch_view(C.byref(self.c), C.byref(self.view)))
+        self.scratch = torch.empty((self.view.total,), dtype=torch.uint8, device=ctx.device)
+
+    def decode(self, h_in: torch.Tensor, h_out: torch.Tensor = None):
+        assert h_in.is_cuda and h_in.dtype == torch.bfloat16 and h_in.is_contiguous()
+        if h_out is None:
+            h_out = torch.empty_like(h_in)
+        self.ctx.check(self.ctx.lib.hq_layer_decode(self.ctx.h, C.byref(self.c), h_in.data_ptr(), h_out.data_ptr(),
+                                                    self.scratch.data_ptr(), self.view.total, _stream_ptr(self.ctx.device)))
+        return h_out
+
+    def scratch_tensor(self, name):
+        """bf16 view of one intermediate (q, k, v, a, h2, gate, up) of the last decode() - for parity tests."""
+        w = self.weights
+        n = {"q": w[0].m, "k": w[1].m, "v": w[2].m, "a": w[0].m, "h2": w[3].m, "gate": w[4].m, "up": w[5].m}[name]
+        off = getattr(self.view, name)
+        return self.scratch[off:off + 2 * n].view(torch.bfloat16)
 
 
 class KVCache:

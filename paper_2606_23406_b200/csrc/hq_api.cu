@@ -502,6 +502,96 @@ hq_status hq_linear_group(hq_ctx* ctx, const hq_weight* const* ws, int32_t n_w, 
                                (uint8_t*)ctx->ws, (cudaStream_t)stream);
 }
 
+hq_status hq_linear_group_fold(hq_ctx* ctx, const hq_weight* const* ws, int32_t n_w, const void* x_dev,
+                               const hq_fold* fold, void* const* ys_bf16_dev, float* const* ys_f32_or_null, void* stream) {
+    if (!ctx) return HQ_ERR_INVALID_ARG;
+    if (!ws || !x_dev || !fold || !ys_bf16_dev || n_w < 1 || n_w > 4) return fail(ctx, HQ_ERR_INVALID_ARG, "bad group arguments");
+    if (fold->mode < HQ_FOLD_NONE || fold->mode > HQ_FOLD_SILU_MUL) return fail(ctx, HQ_ERR_INVALID_ARG, "bad fold mode");
+    if (fold->mode != HQ_FOLD_NONE && !fold->aux_dev) return fail(ctx, HQ_ERR_INVALID_ARG, "the fold needs aux_dev");
+    if (((uintptr_t)x_dev & 7) || ((uintptr_t)fold->aux_dev & 7)) return fail(ctx, HQ_ERR_INVALID_ARG, "x_dev / aux_dev must be 8-byte aligned");
+    int64_t ldys[4];
+    for (int i = 0; i < n_w; ++i) {
+        if (!ws[i] || !ys_bf16_dev[i]) return fail(ctx, HQ_ERR_INVALID_ARG, "null weight or output in group");
+        if (ws[i]->n_in != ws[0]->n_in) return fail(ctx, HQ_ERR_SHAPE, "the weights of a group must share n_in");
+        if (ws[i]->ctx != ctx) return fail(ctx, HQ_ERR_INVALID_ARG, "a weight belongs to another context");
+        ldys[i] = ws[i]->m;
+    }
+    HQ_ENTER(ctx);
+    if (!linear_group_compatible(ws, n_w)) return fail(ctx, HQ_ERR_UNSUPPORTED, "the folds need E8 / tile 128 / k <= 3 weights that share a launch");
+    size_t need = linear_group_workspace_bytes(ctx, ws, n_w, 1);
+    if (need > ctx->ws_bytes) {
+        if (ctx->ws) { HQ_CUDA_CHECK(ctx, cudaDeviceSynchronize()); ctx_free(ctx, ctx->ws); ctx->ws = nullptr; ctx->ws_bytes = 0; }
+        ctx->ws = ctx_alloc(ctx, need);
+        if (!ctx->ws) return HQ_ERR_ALLOC;
+        ctx->ws_bytes = need;
+    }
+    return launch_linear_group(ctx, ws, n_w, x_dev, HQ_BF16, 1, ws[0]->n_in, ys_bf16_dev, ldys, ys_f32_or_null, nullptr,
+                               (uint8_t*)ctx->ws, (cudaStream_t)stream, fold);
+}
+
+static size_t a256(size_t v) { return (v + 255) & ~(size_t)255; }
+hq_status hq_layer_scratch_view(const hq_layer* L, hq_layer_scratch* out) {
+    if (!L || !out || !L->wq || !L->wk || !L->wgate || !L->wo) return HQ_ERR_INVALID_ARG;
+    size_t o = 0;
+    out->q = o; o += a256((size_t)L->wq->m * 2);
+    out->k = o; o += a256((size_t)L->wk->m * 2);
+    out->v = o; o += a256((size_t)L->wk->m * 2);
+    out->a = o; o += a256((size_t)L->wq->m * 2);
+    out->h2 = o; o += a256((size_t)L->wo->m * 2);
+    out->gate = o; o += a256((size_t)L->wgate->m * 2);
+    out->up = o; o += a256((size_t)L->wgate->m * 2);
+    out->total = o;
+    return HQ_OK;
+}
+
+hq_status hq_layer_decode(hq_ctx* ctx, const hq_layer* L, const void* h_in_dev, void* h_out_dev, void* scratch_dev,
+                          size_t scratch_bytes, void* stream) {
+    if (!ctx) return HQ_ERR_INVALID_ARG;
+    if (!L || !h_in_dev || !h_out_dev || !scratch_dev) return fail(ctx, HQ_ERR_INVALID_ARG, "null argument");
+    if (!L->wq || !L->wk || !L->wv || !L->wo || !L->wgate || !L->wup || !L->wdown || !L->g_attn_dev || !L->g_mlp_dev || !L->kv)
+        return fail(ctx, HQ_ERR_INVALID_ARG, "incomplete layer");
+    const int64_t hidden = L->wq->n_in, d = L->kv->cfg.head_dim, Hkv = L->kv->cfg.kv_heads, ffn = L->wgate->m;
+    if (L->q_heads <= 0 || L->wq->m != (int64_t)L->q_heads * d || L->wk->m != Hkv * d || L->wv->m != Hkv * d ||
+        L->wk->n_in != hidden || L->wv->n_in != hidden || L->wo->n_in != L->wq->m || L->wo->m != hidden ||
+        L->wgate->n_in != hidden || L->wup->n_in != hidden || L->wup->m != ffn || L->wdown->n_in != ffn || L->wdown->m != hidden)
+        return fail(ctx, HQ_ERR_SHAPE, "the layer's weight shapes do not fit together");
+    hq_layer_scratch sv;
+    hq_layer_scratch_view(L, &sv);
+    if (scratch_bytes < sv.total || ((uintptr_t)scratch_dev & 255)) return fail(ctx, HQ_ERR_INVALID_ARG, "scratch too small or not 256-byte aligned");
+    uint8_t* sc = (uint8_t*)scratch_dev;
+    void *q = sc + sv.q, *k = sc + sv.k, *v = sc + sv.v, *a = sc + sv.a, *h2 = sc + sv.h2, *gate = sc + sv.gate, *up = sc + sv.up;
+    hq_status s;
+    {   // q, k, v = W RMSNorm(h)
+        const hq_weight* ws[3] = {L->wq, L->wk, L->wv};
+        void* ys[3] = {q, k, v};
+        hq_fold f = {HQ_FOLD_RMSNORM, L->eps, L->g_attn_dev, nullptr};
+        if ((s = hq_linear_group_fold(ctx, ws, 3, h_in_dev, &f, ys, nullptr, stream)) != HQ_OK) return s;
+    }
+    if ((s = hq_kv_append(ctx, L->kv, k, v, 1, stream)) != HQ_OK) return s;
+    if ((s = hq_attend(ctx, L->kv, q, L->q_heads, a, nullptr, stream)) != HQ_OK) return s;
+    {   // h2 = h + W_o a
+        const hq_weight* ws[1] = {L->wo};
+        void* ys[1] = {h2};
+        const void* res[1] = {h_in_dev};
+        hq_fold f = {HQ_FOLD_NONE, 0.0f, nullptr, res};
+        if ((s = hq_linear_group_fold(ctx, ws, 1, a, &f, ys, nullptr, stream)) != HQ_OK) return s;
+    }
+    {   // gate, up = W RMSNorm(h2)
+        const hq_weight* ws[2] = {L->wgate, L->wup};
+        void* ys[2] = {gate, up};
+        hq_fold f = {HQ_FOLD_RMSNORM, L->eps, L->g_mlp_dev, nullptr};
+        if ((s = hq_linear_group_fold(ctx, ws, 2, h2, &f, ys, nullptr, stream)) != HQ_OK) return s;
+    }
+    {   // h_out = h2 + W_down (silu(gate) * up)
+        const hq_weight* ws[1] = {L->wdown};
+        void* ys[1] = {h_out_dev};
+        const void* res[1] = {h2};
+        hq_fold f = {HQ_FOLD_SILU_MUL, 0.0f, up, res};
+        if ((s = hq_linear_group_fold(ctx, ws, 1, gate, &f, ys, nullptr, stream)) != HQ_OK) return s;
+    }
+    return HQ_OK;
+}
+
 // ---------------------------------------------------------------------------------------------
 hq_status hq_kv_create(hq_ctx* ctx, const hq_kv_config* cfg, hq_kv** out) {
     if (!ctx) return HQ_ERR_INVALID_ARG;

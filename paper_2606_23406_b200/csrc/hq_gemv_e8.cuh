@@ -36,7 +36,7 @@ __host__ __device__ constexpr uint32_t gv_xq_bytes(int n_kt) { return (uint32_t)
 template <int NWG>
 __host__ __device__ constexpr size_t gv_smem_bytes(int n_kt) {
     return 1024 + (size_t)E8_LUT_BYTES + gv_xq_bytes(n_kt) + (size_t)((n_kt * 4 + 127) & ~127) +
-           (size_t)NWG * 128 * (E8_SCR_STRIDE * 4 + 16 + GV_STAGE_WORDS * 4) + 8 * (NWG * 4 + 1) + 16;
+           (size_t)NWG * 128 * (E8_SCR_STRIDE * 4 + 16 + GV_STAGE_WORDS * 4) + 8 * (NWG * 4 + 1) + 16 + GV_MAX_KT * 4;
 }
 
 // The rare row the SWAR decoder declines (a unary quotient >= 16, or more than E8_NW U words): that lane alone walks its
@@ -194,6 +194,60 @@ __device__ __forceinline__ void gv_load_ragged(const uint8_t* sgp, bool dense, u
     else gv_load_ragged_all(uarea, stg_a, nw);
 }
 
+// The folds of a decoder layer into the activation prologue (FORMAT R8 / R9; "the butterfly folds into the
+// preceding LayerNorm"): the element the RHT sees is bf16((h r) g) or bf16(silu_c(a) b) instead of x itself.
+struct GvFold {
+    int mode;                      // 0 plain, 1 RMSNorm, 2 SiLU.mul
+    float eps;
+    const __nv_bfloat16* aux;      // gain (mode 1) or the second factor (mode 2)
+    uint32_t ssq_a;                // shared memory: n_kt tile sums of squares (mode 1)
+    int n_in;
+};
+__device__ __forceinline__ float gv_bf16r(float v) { return __bfloat162float(__float2bfloat16_rn(v)); }
+__device__ __forceinline__ float gv_exp_c(float t) {   // FORMAT R9, every step one IEEE fp32 operation
+    t = fminf(fmaxf(t, -87.0f), 88.0f);
+    const float m = rintf(__fmul_rn(t, 0x1.715476p+0f));
+    float f = __fmaf_rn(m, -0x1.62e000p-1f, t);
+    f = __fmaf_rn(m, -0x1.0bfbe8p-15f, f);
+    float p = 0x1.a01a02p-13f;
+    p = __fmaf_rn(p, f, 0x1.6c16c2p-10f);
+    p = __fmaf_rn(p, f, 0x1.111112p-7f);
+    p = __fmaf_rn(p, f, 0x1.555556p-5f);
+    p = __fmaf_rn(p, f, 0x1.555556p-3f);
+    p = __fmaf_rn(p, f, 0.5f);
+    p = __fmaf_rn(p, f, 1.0f);
+    p = __fmaf_rn(p, f, 1.0f);
+    return __fmul_rn(p, __int_as_float(((int)m + 127) << 23));
+}
+__device__ __forceinline__ float gv_silu_c(float a) { return __fdiv_rn(a, __fadd_rn(1.0f, gv_exp_c(-a))); }
+__device__ __forceinline__ void gv_unpack_bf16x4(uint2 v, float* x) {
+    x[0] = __uint_as_float(v.x << 16); x[1] = __uint_as_float(v.x & 0xffff0000u);
+    x[2] = __uint_as_float(v.y << 16); x[3] = __uint_as_float(v.y & 0xffff0000u);
+}
+// R8: r = 1 / sqrt(treesum(h^2) / n + eps).  R2's tree over the whole vector = the tree inside each tile of 128 (two
+// in-lane levels, five shuffle levels) followed by the tree over the tile sums (lane l holds tiles 4l .. 4l+3, absent
+// ones zero).  Every warp of the CTA takes part (block barrier inside); the tile sums are shared through ssq_a.
+template <int NW>
+__device__ __forceinline__ float gv_rms_scale(const void* xp, const GvFold& fo, int n_kt, int wid, int lane) {
+    for (int kt = wid; kt < n_kt; kt += NW) {
+        float a[4];
+        gv_unpack_bf16x4(__ldg((const uint2*)((const __nv_bfloat16*)xp + (int64_t)kt * 128 + 4 * lane)), a);
+        float s = __fadd_rn(__fadd_rn(__fmul_rn(a[0], a[0]), __fmul_rn(a[1], a[1])), __fadd_rn(__fmul_rn(a[2], a[2]), __fmul_rn(a[3], a[3])));
+#pragma unroll
+        for (int m = 1; m < 32; m <<= 1) s = __fadd_rn(s, __shfl_xor_sync(0xffffffffu, s, m));
+        if (lane == 0) asm volatile("st.shared.f32 [%0], %1;" ::"r"(fo.ssq_a + kt * 4), "f"(s) : "memory");
+    }
+    __syncthreads();
+    float v[4];
+#pragma unroll
+    for (int e = 0; e < 4; ++e) v[e] = 4 * lane + e < n_kt ? lds_f32(fo.ssq_a + (4 * lane + e) * 4) : 0.0f;
+    float s = __fadd_rn(__fadd_rn(v[0], v[1]), __fadd_rn(v[2], v[3]));
+#pragma unroll
+    for (int m = 1; m < 32; m <<= 1) s = __fadd_rn(s, __shfl_xor_sync(0xffffffffu, s, m));
+    const float ms = __fdiv_rn(s, (float)fo.n_in);
+    return __fdiv_rn(1.0f, __fsqrt_rn(__fadd_rn(ms, fo.eps)));
+}
+
 __device__ __forceinline__ void gv_load_x(const void* xp, int dtype, bool vec, const int8_t* dsign, int kt, int lane, float* x, uint32_t& sg) {
     const int64_t base = (int64_t)kt * 128 + 4 * lane;
     if (vec && dtype == HQ_BF16) {
@@ -222,8 +276,8 @@ __device__ __forceinline__ void gv_load_x(const void* xp, int dtype, bool vec, c
 template <int K, int NW>
 __device__ __noinline__ void gv_first_prologue(const void* xp, int dtype, const int8_t* dsign, int n_kt, uint32_t xq_a,
                                                uint32_t sx_a, int wid, int lane, int kt0, int nt, const uint8_t* blob,
-                                               const uint32_t* soff, int has, int dense_i, uint32_t stg_a, uint32_t ret_a
-) {
+                                               const uint32_t* soff, int has, int dense_i, uint32_t stg_a, uint32_t ret_a,
+                                               GvFold fo) {
     constexpr int KW = 4 * K;
     const bool dense = dense_i != 0;
     uint32_t off0 = 0, off1 = 0;
@@ -238,7 +292,9 @@ __device__ __noinline__ void gv_first_prologue(const void* xp, int dtype, const 
     uint32_t sg = 0, sgn = 0;
     auto tile_of = [&](int j) { const int kt = kt0 + j; return kt >= n_kt ? kt - n_kt : kt; };
     int j = wid;
-    if (j < nt) gv_load_x(xp, dtype, vec, dsign, tile_of(j), lane, xn, sgn);
+    uint2 auxn = make_uint2(0u, 0u);
+    auto load_aux = [&](int kt) { if (fo.mode) auxn = __ldg((const uint2*)(fo.aux + (int64_t)kt * 128 + 4 * lane)); };
+    if (j < nt) { gv_load_x(xp, dtype, vec, dsign, tile_of(j), lane, xn, sgn); load_aux(tile_of(j)); }
     uint32_t ul = 0, nrm = 0;
     const uint8_t* sgp = blob + 16 * (size_t)off0;
     if (has) {
@@ -246,12 +302,21 @@ __device__ __noinline__ void gv_first_prologue(const void* xp, int dtype, const 
         gv_load_r<KW>(sgp, lane, stg_a);
     }
     bool ragged_due = has != 0;
+    // R8: the scale of the whole vector, behind the first tile's loads (one more block barrier; mode is CTA-uniform)
+    const float rms_r = fo.mode == 1 ? gv_rms_scale<NW>(xp, fo, n_kt, wid, lane) : 1.0f;
 #pragma unroll 1
     for (; j < nt; j += NW) {
         const int kt = tile_of(j);
+        if (fo.mode) {   // the bf16 vector a separate RMSNorm / SiLU.mul kernel would have written, element by element
+            float ax[4];
+            gv_unpack_bf16x4(auxn, ax);
+#pragma unroll
+            for (int e = 0; e < 4; ++e)
+                xn[e] = gv_bf16r(fo.mode == 1 ? __fmul_rn(__fmul_rn(xn[e], rms_r), ax[e]) : __fmul_rn(gv_silu_c(xn[e]), ax[e]));
+        }
 #pragma unroll
         for (int e = 0; e < 4; ++e) x[e] = (sgn >> (8 * e)) & 0x80u ? -xn[e] : xn[e];
-        if (j + NW < nt) gv_load_x(xp, dtype, vec, dsign, tile_of(j + NW), lane, xn, sgn);
+        if (j + NW < nt) { gv_load_x(xp, dtype, vec, dsign, tile_of(j + NW), lane, xn, sgn); load_aux(tile_of(j + NW)); }
         int qv[4];
         const float sx = warp_act_tile128(x, lane, qv);
         if (ragged_due) {   // the header has arrived behind the FWHT
@@ -303,6 +368,7 @@ k_gemv_e8(E8Params p) {
     uint64_t* bar_w = bars + wid;            // this warp's MMAs done
     uint64_t* bar_lut = bars + NW;
     uint32_t* tmem_slot = (uint32_t*)(bars + NW + 1);
+    const GvFold fold{p.fold_mode, p.fold_eps, p.fold_aux, smem_u32(bars + NW + 3), p.n_kt * 128};
 
     if (wid == 0) tmem_alloc(tmem_slot, 512);
     if (tid == 0) {
@@ -340,7 +406,7 @@ k_gemv_e8(E8Params p) {
     const int nt_cta = (int)min((int64_t)n_kt, cta_e - cta_b), kt0_cta = (int)(cta_b % n_kt);
 
     if (f >= f_end) {   // nothing to do for this warp group: it still helps with the activations and joins the barriers
-        gv_first_prologue<K, NW>(p.x, p.dtype, p.dsign, n_kt, xq_a, sx_a, wid, lane, kt0_cta, nt_cta, nullptr, nullptr, 0, 0, stg_a, scr_a);
+        gv_first_prologue<K, NW>(p.x, p.dtype, p.dsign, n_kt, xq_a, sx_a, wid, lane, kt0_cta, nt_cta, nullptr, nullptr, 0, 0, stg_a, scr_a, fold);
         tc_fence_before();
         __syncthreads();
         if (wid == 0) tmem_dealloc(*tmem_slot, 512);
@@ -389,7 +455,7 @@ k_gemv_e8(E8Params p) {
         const uint8_t* sgp_c;
         if (first_seg) {   // the kernel's first tile: its loads are interleaved with the activation prologue (all warps meet there)
             gv_first_prologue<K, NW>(p.x, p.dtype, p.dsign, n_kt, xq_a, sx_a, wid, lane, kt0_cta, nt_cta, blob, soff,
-                                     (ka + 1 < kb) ? 2 : 1, dense ? 1 : 0, stg_a, scr_a);
+                                     (ka + 1 < kb) ? 2 : 1, dense ? 1 : 0, stg_a, scr_a, fold);
             first_seg = false;
             ul_c = lds32(scr_a); nrm_c = lds32(scr_a + 4); off_n1 = lds32(scr_a + 8);
             sgp_c = blob + 16 * (size_t)lds32(scr_a + 12);
@@ -501,6 +567,7 @@ k_gemv_e8(E8Params p) {
         }
         if (row_in) {
             if (ka == 0 && kb == n_kt) {
+                if (p.res[w]) yacc = __fadd_rn(yacc, __bfloat162float(p.res[w][r]));   // R10
                 if (p.y_bf16[w]) p.y_bf16[w][r] = __float2bfloat16_rn(yacc);
                 if (p.y_f32[w]) p.y_f32[w][r] = yacc;
             } else {
@@ -550,6 +617,7 @@ k_gemv_e8(E8Params p) {
 #pragma unroll
             for (int u = 0; u < 8; ++u) sum += v[u];
         }
+        if (p.res[w]) sum = __fadd_rn(sum, __bfloat162float(p.res[w][r]));   // R10
         if (p.y_bf16[w]) p.y_bf16[w][r] = __float2bfloat16_rn(sum);
         if (p.y_f32[w]) p.y_f32[w][r] = sum;
     }

@@ -154,7 +154,7 @@ bool linear_group_compatible(const hq_weight* const* ws, int n_w);
 size_t linear_group_workspace_bytes(const hq_ctx* ctx, const hq_weight* const* ws, int n_w, int64_t B);
 hq_status launch_linear_group(hq_ctx* ctx, const hq_weight* const* ws, int n_w, const void* x, int dtype, int64_t B,
                               int64_t ldx, void* const* ys_bf16, const int64_t* ldys, float* const* ys_f32,
-                              int32_t* acc_i32, uint8_t* wsbuf, cudaStream_t st);
+                              int32_t* acc_i32, uint8_t* wsbuf, cudaStream_t st, const hq_fold* fold = nullptr);
 bool linear_uses_e8_fast(const hq_weight* w);
 hq_status launch_decode_ceiling(hq_ctx* ctx, const hq_weight* w, int reps, cudaStream_t st, double* scalars_per_s);
 // hq_linear_static: the address of the static scratch array (once per device, that device current), and the launch

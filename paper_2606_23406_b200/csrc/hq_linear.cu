@@ -464,10 +464,14 @@ static hq_status launch_large(hq_ctx* ctx, const hq_weight* const* ws, int n_w, 
 // one activation cast, ONE fused decode + MMA launch over the stacked row blocks of all weights, one finalize each
 hq_status launch_linear_group(hq_ctx* ctx, const hq_weight* const* ws, int n_w, const void* x, int dtype, int64_t B,
                               int64_t ldx, void* const* ys_bf16, const int64_t* ldys, float* const* ys_f32,
-                              int32_t* acc_i32, uint8_t* wsbuf, cudaStream_t st) {
+                              int32_t* acc_i32, uint8_t* wsbuf, cudaStream_t st, const hq_fold* fold) {
     const hq_weight* w0 = ws[0];
     int64_t n_rb = 0;
     for (int i = 0; i < n_w; ++i) n_rb += ws[i]->n_rb;
+    if (fold && (B != 1 || w0->n_kt > GV_MAX_KT || dtype != HQ_BF16)) {   // the folds live in the batch-1 kernel's prologue / epilogue
+        ctx->err = "the RMSNorm / SiLU.mul / residual folds need batch 1, bf16 and n_in <= 16384";
+        return HQ_ERR_UNSUPPORTED;
+    }
     if (B >= LG_MIN_B) return launch_large(ctx, ws, n_w, x, dtype, B, ldx, ys_bf16, ldys, ys_f32, acc_i32, wsbuf, st);
     E8Plan pl = e8_plan(ctx, n_rb, w0->n_kt, w0->n_in, B);
     // the tile descriptor of the fused kernel packs its fields (hq_linear_e8.cuh E8Desc): reject shapes that would alias
@@ -514,6 +518,10 @@ hq_status launch_linear_group(hq_ctx* ctx, const hq_weight* const* ws, int n_w, 
     p.u_dense = ((min_ulen + 31) >> 5) >= (uint32_t)E8_DENSE ? E8_DENSE : 0;
     p.bblob = bblob; p.B = B; p.acc_i32 = (n_w == 1) ? acc_i32 : nullptr;
     p.x = x; p.dtype = dtype; p.dsign = w0->dsign;
+    if (fold) {
+        p.fold_mode = fold->mode; p.fold_eps = fold->eps; p.fold_aux = (const __nv_bfloat16*)fold->aux_dev;
+        for (int i = 0; i < n_w; ++i) p.res[i] = fold->residuals_dev ? (const __nv_bfloat16*)fold->residuals_dev[i] : nullptr;
+    }
     if (gemv) p.n_items = (int)(n_rb * w0->n_kt);   // the batch-1 kernel partitions tiles, not items
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     if (ctx->prof) {

@@ -67,6 +67,11 @@ struct E8Params {
     const void* x;              // [n_in] bf16 or f32
     int dtype;
     const int8_t* dsign;        // [n_in] RHT signs
+    // the folds of a decoder layer (FORMAT R8-R10), batch-1 kernel only
+    int fold_mode;              // 0 plain; 1 RMSNorm: x = residual stream h, fold_aux = gain; 2 SiLU.mul: x = gate, fold_aux = up
+    float fold_eps;
+    const __nv_bfloat16* fold_aux;          // [n_in] bf16
+    const __nv_bfloat16* res[E8_MAXW];      // [m_w] bf16 added to the output (R10), may be null
 };
 
 // Tile descriptor, three registers; the stream of tiles of one warp group is advanced without divisions.
