@@ -222,6 +222,59 @@ def measure_attend(ctx, hq, dev, peak_gbs):
     return res
 
 
+def measure_layer_step(ctx, hq, dev, layers, peak_gbs, context=32768, steps=12):
+    """SURVEY §8(f)3 / PAPER.md Table 10's decode shape (L496-511): one token through whole decoder layers
+    (hq_layer_decode: RMSNorm and SiLU.mul folded into the linears' prologues, residuals into their epilogues, KV append,
+    attend) on the bench's compressed Llama-3.1-8B-shaped layers, each with its own 2-bps KV cache at `context` tokens.
+    Launched eagerly (the cache position is host state), 7 launches per layer; the layers are cycled so weights and
+    caches come from HBM."""
+    import torch
+    H, d, QH, hidden = 8, 128, 32, 4096
+    snr_kv = float(np.float32(9.68))
+    K = torch.from_numpy(hq_synth.kv_tokens(context, H, d, seed=4)).to(dev).to(torch.bfloat16)
+    V = torch.from_numpy(hq_synth.kv_tokens(context, H, d, seed=5)).to(dev).to(torch.bfloat16)
+    g = torch.ones((hidden,), dtype=torch.bfloat16, device=dev)
+    objs, kv_bytes = [], 0.0
+    for l, ws in enumerate(layers):
+        kv = ctx.kv_create(H, d, context + 256, hq.Lattice.E8, snr_kv, (0, 0), 4 + l, rotation=1, dither=1, window=32)
+        kv.append(K, V)
+        ex = kv.export()
+        Tn = int(ex["n_tokens"])
+        kv_bytes += (float(ex["upos"].astype(np.int64).sum()) + 2.0 * H * Tn * float(ex["rbits"]) + 32.0 * 2 * H * Tn) / 8.0
+        objs.append((ctx.layer(ws["q"], ws["k"], ws["v"], ws["o"], ws["gate"], ws["up"], ws["down"], g, g, 1e-5, kv, QH), kv))
+    del K, V
+    kv_bytes /= len(layers)
+    w_bytes = float(np.mean([sum((w.info.payload_bits + w.info.norm_bits + w.info.length_bits) / 8.0 for w in ws.values())
+                             for ws in layers]))
+    h = torch.from_numpy(hq_synth.activations(1, hidden, seed=99)[0]).to(dev).to(torch.bfloat16)
+    h_out = torch.empty_like(h)
+
+    def token():   # one token through all layers (fresh h per layer keeps the magnitudes of the synthetic weights bounded)
+        for layer, _ in objs:
+            layer.decode(h, h_out)
+    for _ in range(3):
+        token()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        token()
+    e1.record()
+    torch.cuda.synchronize()
+    us = 1e3 * e0.elapsed_time(e1) / (steps * len(objs))
+    ok = bool(torch.isfinite(h_out.float()).all())
+    alg = w_bytes + kv_bytes
+    gbs = alg / (us * 1e-6) / 1e9
+    for layer, kv in objs:
+        kv.free()
+    return {"bound": "hbm", "unit": "GB/s", "achieved": gbs, "peak": peak_gbs, "frac": gbs / peak_gbs,
+            "us_per_layer_step": us, "tokens_per_s_at_32_layers": 1e6 / (32.0 * us), "context_tokens": context,
+            "launches_per_layer": 7, "alg_bytes_per_layer_step": alg, "weight_bytes": w_bytes, "kv_bytes": kv_bytes,
+            "finite": ok, "bf16_bytes_per_layer_step": 2.0 * 218103808 + 2.0 * 2 * H * d * context,
+            "call": "hq_layer_decode (eager): q+k+v [RMSNorm fold] -> hq_kv_append -> hq_attend (split + combine) -> o [+ residual] -> gate+up [RMSNorm fold] -> down [SiLU.mul fold, + residual]",
+            "workload": "Llama-3.1-8B-shaped decoder layer, E8 4 bps weights, E8 2 bps KV cache (signs rotation, dither, window 32), batch 1"}
+
+
 def measure_config3(ctx, hq, dev, copies=5):
     """BASELINE config 3 (reduced): a 14336 x 4096 Gaussian weight; lattice x rate at tile 128, E8 4 bps at tiles 64 / 256.
     `copies` distinct weights per point (5 x ~31 MB > the 126 MB L2) are cycled so the GEMV reads HBM, not L2."""
@@ -271,7 +324,7 @@ def main():
     ap.add_argument("--layers", type=int, default=4)
     ap.add_argument("--impl", default="ours")
     ap.add_argument("--skip-extras", action="store_true")
-    ap.add_argument("--only", choices=("decode_ceiling", "large_m", "attend", "config3"), default=None,
+    ap.add_argument("--only", choices=("decode_ceiling", "large_m", "attend", "config3", "layer_step"), default=None,
                     help="run one secondary measurement alone and print its JSON (the command the ncu captures under profiles/ name)")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -299,6 +352,12 @@ def main():
             out = measure_large_m(ctx, hq, dev, reps=3)
         elif args.only == "attend":
             out = measure_attend(ctx, hq, dev, peaks()[0])
+        elif args.only == "layer_step":
+            lw = []
+            for l in range(args.layers):
+                lw.append({name: ctx.encode_weights(torch.from_numpy(hq_synth.llama_weight(l, name)).to(dev).to(torch.bfloat16),
+                                                    hq.Lattice.E8, 128, SNR_E8_4BPS, seed=l) for name in NAMES})
+            out = measure_layer_step(ctx, hq, dev, lw, peaks()[0])
         else:
             out = measure_config3(ctx, hq, dev)
         print(json.dumps({"only": args.only, "result": out}))
@@ -506,7 +565,8 @@ def main():
             extras["cublas_bf16_gemv_ms_per_layer"] = f"failed: {ex}"
         if world == 1:
             for key, fn in (("large_m", lambda: measure_large_m(ctx, hq, dev)),
-                            ("attend", lambda: measure_attend(ctx, hq, dev, peak))):
+                            ("attend", lambda: measure_attend(ctx, hq, dev, peak)),
+                            ("layer_step", lambda: measure_layer_step(ctx, hq, dev, layers, peak))):
                 try:
                     roofline[key] = fn()
                 except Exception as ex:  # noqa: BLE001
