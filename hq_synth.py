@@ -62,6 +62,14 @@ def kv_tokens(n_tok, heads, d, seed, token0=0):
     return to_bf16_f32(x)
 
 
+def haar_matrix(d, seed):
+    """A Haar-uniform orthogonal matrix S [d, d] (the qjl rotation, §3.4: drawn once per layer): QR of a
+    Gaussian matrix with the sign convention that makes the distribution uniform; fp32."""
+    g = np.random.default_rng([seed, 7]).standard_normal((d, d))
+    q, r = np.linalg.qr(g)
+    return np.ascontiguousarray((q * np.sign(np.diag(r))[None, :]).astype(np.float32))
+
+
 def calib_tiles(nt, n, seed=42):
     """iid N(0,1) calibration tiles (B.1: ~1e5 tiles, seed 42)."""
     return np.random.default_rng(seed).standard_normal((nt, n), dtype=np.float32)

@@ -892,11 +892,31 @@ void hqo_dequant_weights(const int8_t* codes, const uint16_t* norms, int64_t m, 
 
 /* ------------------------------------------------------------------------------------------ */
 /* KV path (§5.2): encode vectors [n_tok, heads, d] of one role.                        */
-/* rotation: 0 none, 1 signs.  token0 = index of the first token of this call.                   */
+/* rotation: 0 none, 1 signs, 2 qjl (dense Q).  token0 = index of the first token of this call.   */
 /* ------------------------------------------------------------------------------------------ */
+/* rotation 2 = qjl (§3.4, eq.(2); Table 4): a dense orthogonal S = Q [d][d] row-major, drawn Haar-uniform
+ * once per layer by the caller and passed in; u'_i = sum_j Q_ij u_j accumulated in j order with one fused multiply-add
+ * per term (FORMAT R11 - canonical because it decides the codes).                                                   */
+static void qjl_apply_f32(const float* Q, int d, float* u) {
+    float r[1024];
+    for (int i = 0; i < d; ++i) {
+        float acc = 0.0f;
+        for (int j = 0; j < d; ++j) acc = fmaf(Q[i * d + j], u[j], acc);
+        r[i] = acc;
+    }
+    memcpy(u, r, (size_t)d * sizeof(float));
+}
+int64_t hqo_kv_quantize_q(const float* kv, int64_t n_tok, int heads, int d, int64_t token0, int role,
+                          int lattice, double snr_db, int rotation, int dither, uint64_t seed, const float* Q,
+                          int8_t* codes /*[n_tok,heads,d]*/, uint16_t* norms /*[n_tok,heads]*/);
 int64_t hqo_kv_quantize(const float* kv, int64_t n_tok, int heads, int d, int64_t token0, int role,
                         int lattice, double snr_db, int rotation, int dither, uint64_t seed,
                         int8_t* codes /*[n_tok,heads,d]*/, uint16_t* norms /*[n_tok,heads]*/) {
+    return hqo_kv_quantize_q(kv, n_tok, heads, d, token0, role, lattice, snr_db, rotation, dither, seed, NULL, codes, norms);
+}
+int64_t hqo_kv_quantize_q(const float* kv, int64_t n_tok, int heads, int d, int64_t token0, int role,
+                          int lattice, double snr_db, int rotation, int dither, uint64_t seed, const float* Q,
+                          int8_t* codes /*[n_tok,heads,d]*/, uint16_t* norms /*[n_tok,heads]*/) {
     float A = (float)(hqo_alpha(lattice, snr_db) * sqrt((double)d));
     int8_t *D = (int8_t*)malloc((size_t)d), *S = (int8_t*)malloc((size_t)d);
     int64_t clamps = 0;
@@ -909,6 +929,7 @@ int64_t hqo_kv_quantize(const float* kv, int64_t n_tok, int heads, int d, int64_
             hqo_rht_f32(kv + (t * heads + h) * d, D, d, u);
             if (rotation == 1)
                 for (int i = 0; i < d; ++i) u[i] = (S[i] < 0) ? -u[i] : u[i];
+            if (rotation == 2) qjl_apply_f32(Q, d, u);
             clamps += quantize_tile(lattice, d, A, u, dither, seed, (uint32_t)(token0 + t),
                                     (uint32_t)h, (uint32_t)role, codes + (t * heads + h) * d,
                                     norms + t * heads + h);
@@ -944,7 +965,7 @@ int64_t hqo_kv_unpack_token(int lattice, int d, const int* k, const uint32_t* re
 /* reconstruct one cached vector the long way (O4): decode -> c - U -> un-normalize -> Sᵀ -> RHT⁻¹ */
 static void kv_reconstruct(const int8_t* codes, uint16_t norm_bits, int d, int lattice, double inv_A,
                            int rotation, int dither, uint64_t seed, uint32_t token, uint32_t head,
-                           uint32_t role, const int8_t* D, const int8_t* S, double* out) {
+                           uint32_t role, const int8_t* D, const int8_t* S, const float* Q, double* out) {
     double u[1024];
     double sc = (double)f16_bits_to_f32(norm_bits) * inv_A;
     int dim = lattice;
@@ -960,11 +981,28 @@ static void kv_reconstruct(const int8_t* codes, uint16_t norm_bits, int d, int l
     if (norm_bits == 0) for (int i = 0; i < d; ++i) u[i] = 0.0;
     if (rotation == 1)
         for (int i = 0; i < d; ++i) u[i] = (S[i] < 0) ? -u[i] : u[i];
+    if (rotation == 2) { /* S^T (eq.(2)): u_j <- sum_i Q_ij u_i */
+        double r[1024];
+        for (int j = 0; j < d; ++j) {
+            double acc = 0.0;
+            for (int i = 0; i < d; ++i) acc += (double)Q[i * d + j] * u[i];
+            r[j] = acc;
+        }
+        memcpy(u, r, (size_t)d * sizeof(double));
+    }
     rht_inverse_f64(u, D, d, out);
 }
+void hqo_kv_reconstruct_q(const int8_t* codes, const uint16_t* norms, int64_t n_tok, int heads, int d, int64_t token0,
+                          int role, int lattice, double snr_db, int rotation, int dither, uint64_t seed, const float* Q,
+                          double* out);
 void hqo_kv_reconstruct(const int8_t* codes /*[n_tok,heads,d]*/, const uint16_t* norms, int64_t n_tok,
                         int heads, int d, int64_t token0, int role, int lattice, double snr_db,
                         int rotation, int dither, uint64_t seed, double* out /*[n_tok,heads,d]*/) {
+    hqo_kv_reconstruct_q(codes, norms, n_tok, heads, d, token0, role, lattice, snr_db, rotation, dither, seed, NULL, out);
+}
+void hqo_kv_reconstruct_q(const int8_t* codes /*[n_tok,heads,d]*/, const uint16_t* norms, int64_t n_tok,
+                          int heads, int d, int64_t token0, int role, int lattice, double snr_db,
+                          int rotation, int dither, uint64_t seed, const float* Q, double* out /*[n_tok,heads,d]*/) {
     double inv_A = 1.0 / (hqo_alpha(lattice, snr_db) * sqrt((double)d));
     int8_t *D = (int8_t*)malloc((size_t)d), *S = (int8_t*)malloc((size_t)d);
     hqo_signs(seed, 1u, d, D);
@@ -974,7 +1012,7 @@ void hqo_kv_reconstruct(const int8_t* codes /*[n_tok,heads,d]*/, const uint16_t*
         for (int h = 0; h < heads; ++h)
             kv_reconstruct(codes + (t * heads + h) * d, norms[t * heads + h], d, lattice, inv_A,
                            rotation, dither, seed, (uint32_t)(token0 + t), (uint32_t)h,
-                           (uint32_t)role, D, S, out + (t * heads + h) * d);
+                           (uint32_t)role, D, S, Q, out + (t * heads + h) * d);
     free(D); free(S);
 }
 

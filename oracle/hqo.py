@@ -250,12 +250,16 @@ def dequant_weights(codes, norms, lattice, n_tile, snr_db, seed):
 
 
 # ---------------------------------------------------------------- KV (O1 with rotate + dither, O4)
-def kv_quantize(kv, token0, role, lattice, snr_db, rotation, dither, seed):
+def kv_quantize(kv, token0, role, lattice, snr_db, rotation, dither, seed, qjl=None):
+    """rotation 2 (qjl): `qjl` is the dense orthogonal matrix S [d, d] (row-major fp32), an input (§3.4)."""
     kv = _c(kv, np.float32); n_tok, heads, d = kv.shape
     codes = np.zeros((n_tok, heads, d), np.int8); norms = np.zeros((n_tok, heads), np.uint16)
-    clamps = lib().hqo_kv_quantize(_p(kv), C.c_int64(n_tok), C.c_int(heads), C.c_int(d), C.c_int64(token0),
-                                   C.c_int(role), lattice, C.c_double(snr_db), C.c_int(rotation),
-                                   C.c_int(dither), C.c_uint64(seed), _p(codes), _p(norms))
+    Q = _c(qjl, np.float32) if qjl is not None else None
+    assert (rotation == 2) == (Q is not None) and (Q is None or Q.shape == (d, d))
+    clamps = lib().hqo_kv_quantize_q(_p(kv), C.c_int64(n_tok), C.c_int(heads), C.c_int(d), C.c_int64(token0),
+                                     C.c_int(role), lattice, C.c_double(snr_db), C.c_int(rotation),
+                                     C.c_int(dither), C.c_uint64(seed), _p(Q) if Q is not None else None,
+                                     _p(codes), _p(norms))
     return codes, norms, clamps
 
 
@@ -280,12 +284,14 @@ def kv_unpack_token(lattice, d, k, rem, t, una, upos):
     return codes, used
 
 
-def kv_reconstruct(codes, norms, token0, role, lattice, snr_db, rotation, dither, seed):
+def kv_reconstruct(codes, norms, token0, role, lattice, snr_db, rotation, dither, seed, qjl=None):
     codes = _c(codes, np.int8); norms = _c(norms, np.uint16); n_tok, heads, d = codes.shape
     out = np.zeros((n_tok, heads, d), np.float64)
-    lib().hqo_kv_reconstruct(_p(codes), _p(norms), C.c_int64(n_tok), C.c_int(heads), C.c_int(d),
-                             C.c_int64(token0), C.c_int(role), lattice, C.c_double(snr_db), C.c_int(rotation),
-                             C.c_int(dither), C.c_uint64(seed), _p(out))
+    Q = _c(qjl, np.float32) if qjl is not None else None
+    assert (rotation == 2) == (Q is not None)
+    lib().hqo_kv_reconstruct_q(_p(codes), _p(norms), C.c_int64(n_tok), C.c_int(heads), C.c_int(d),
+                               C.c_int64(token0), C.c_int(role), lattice, C.c_double(snr_db), C.c_int(rotation),
+                               C.c_int(dither), C.c_uint64(seed), _p(Q) if Q is not None else None, _p(out))
     return out
 
 
