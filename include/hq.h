@@ -42,7 +42,7 @@ typedef enum {
 
 typedef enum { HQ_Z = 1, HQ_A2 = 2, HQ_D4 = 4, HQ_E8 = 8 } hq_lattice;     /* §3.2, §4.5; value = dimension */
 typedef enum { HQ_F32 = 0, HQ_BF16 = 1 } hq_dtype;
-typedef enum { HQ_ROT_NONE = 0, HQ_ROT_SIGNS = 1, HQ_ROT_QJL = 2 } hq_rotation; /* §4.2, §3.4; QJL (Haar) -> HQ_ERR_UNSUPPORTED */
+typedef enum { HQ_ROT_NONE = 0, HQ_ROT_SIGNS = 1, HQ_ROT_QJL = 2 } hq_rotation; /* §4.2, §3.4; QJL = a dense Haar matrix given in hq_kv_config.qjl_dev */
 
 /* Device-memory allocator supplied by the caller (the Python binding backs it with torch). */
 typedef struct {
@@ -295,6 +295,14 @@ typedef struct {
     int64_t una_capacity_bits;  /* capacity of each (role, head) U stream; 0 = auto: max_tokens * head_dim *
                                    max(4, 1.3 * (1 + (0.8 alpha + 0.5) / 2^k)) bits (E|zz| ~ 0.8 alpha on a normalized vector).
                                    A vector that does not fit is NOT written; the cache turns sticky HQ_ERR_FORMAT. */
+    const float* qjl_dev;       /* HQ_ROT_QJL (§3.4 L184-188 eq.(2); the paper's default KV rotation at >= 2 bps, Table 4):
+                                   the orthogonal matrix S [head_dim][head_dim], fp32 row-major, DEVICE memory, drawn
+                                   Haar-uniform once per layer by the caller (the library draws no matrices; orthogonality is
+                                   not checked).  Copied at hq_kv_create: the caller may free it afterwards.  Encode applies
+                                   u' = S u after the RHT (FORMAT R11: canonical fma accumulation in column order, so the
+                                   codes are reproducible bit for bit); hq_attend rotates the query by S and un-rotates the code-domain sum by S^T, one
+                                   head_dim x head_dim matvec per QUERY head instead of the paper's O(T D^2) per layer (L502).
+                                   Must be NULL for the other rotations. */
 } hq_kv_config;
 
 hq_status hq_kv_create(hq_ctx* ctx, const hq_kv_config* cfg, hq_kv** out);

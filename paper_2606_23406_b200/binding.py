@@ -32,7 +32,8 @@ class _CodecConfig(C.Structure):
 
 class _KVConfig(C.Structure):
     _fields_ = [("kv_heads", C.c_int32), ("head_dim", C.c_int32), ("max_tokens", C.c_int64), ("codec", _CodecConfig),
-                ("rotation", C.c_int32), ("dither", C.c_int32), ("window", C.c_int32), ("una_capacity_bits", C.c_int64)]
+                ("rotation", C.c_int32), ("dither", C.c_int32), ("window", C.c_int32), ("una_capacity_bits", C.c_int64),
+                ("qjl_dev", C.c_void_p)]
 
 
 class _WeightInfo(C.Structure):
@@ -266,9 +267,13 @@ class Context:
 
     # ---- KV ----
     def kv_create(self, kv_heads, head_dim, max_tokens, lattice, snr_db, rice_k, seed, rotation=1, dither=1,
-                  window=32, una_capacity_bits=0):
+                  window=32, una_capacity_bits=0, qjl: torch.Tensor = None):
+        """rotation 2 (qjl): `qjl` = the Haar matrix S [head_dim, head_dim] fp32 on the device (copied by the library)."""
         codec = _CodecConfig(lattice, head_dim, float(snr_db), (C.c_int32 * 2)(int(rice_k[0]), int(rice_k[1])), seed)
-        cfg = _KVConfig(kv_heads, head_dim, max_tokens, codec, rotation, dither, window, int(una_capacity_bits))
+        if qjl is not None:
+            assert qjl.is_cuda and qjl.dtype == torch.float32 and qjl.is_contiguous() and tuple(qjl.shape) == (head_dim, head_dim)
+        cfg = _KVConfig(kv_heads, head_dim, max_tokens, codec, rotation, dither, window, int(una_capacity_bits),
+                        qjl.data_ptr() if qjl is not None else None)
         h = C.c_void_p()
         self.check(self.lib.hq_kv_create(self.h, C.byref(cfg), C.byref(h)))
         return KVCache(self, h, kv_heads, head_dim, max_tokens)

@@ -600,8 +600,8 @@ hq_status hq_kv_create(hq_ctx* ctx, const hq_kv_config* cfg, hq_kv** out) {
     if (!valid_lattice(cfg->codec.lattice)) return fail(ctx, HQ_ERR_INVALID_ARG, "bad lattice");
     if (!valid_tile(cfg->head_dim) || cfg->codec.n_tile != cfg->head_dim || cfg->kv_heads <= 0 || cfg->max_tokens <= 0)
         return fail(ctx, HQ_ERR_SHAPE, "head_dim must be 64/128/256 and equal codec.n_tile");
-    if (cfg->rotation == HQ_ROT_QJL) return fail(ctx, HQ_ERR_UNSUPPORTED, "rotation qjl is not built (SURVEY §8(f)1)");
-    if (cfg->rotation != HQ_ROT_NONE && cfg->rotation != HQ_ROT_SIGNS) return fail(ctx, HQ_ERR_INVALID_ARG, "bad rotation");
+    if (cfg->rotation != HQ_ROT_NONE && cfg->rotation != HQ_ROT_SIGNS && cfg->rotation != HQ_ROT_QJL) return fail(ctx, HQ_ERR_INVALID_ARG, "bad rotation");
+    if ((cfg->rotation == HQ_ROT_QJL) != (cfg->qjl_dev != nullptr)) return fail(ctx, HQ_ERR_INVALID_ARG, "rotation qjl needs qjl_dev, the other rotations must not pass one");
     if (cfg->una_capacity_bits < 0) return fail(ctx, HQ_ERR_INVALID_ARG, "una_capacity_bits must be >= 0");
     HQ_ENTER(ctx);
     if (cfg->codec.rice_k[0] < 0 || cfg->codec.rice_k[0] > 7 || cfg->codec.rice_k[1] > 7)
@@ -645,6 +645,11 @@ hq_status hq_kv_create(hq_ctx* ctx, const hq_kv_config* cfg, hq_kv** out) {
     kv->dsign = (int8_t*)ctx_alloc(ctx, d);
     kv->ssign = (int8_t*)ctx_alloc(ctx, d);
     kv->counters = (unsigned long long*)ctx_alloc(ctx, 64);
+    if (cfg->rotation == HQ_ROT_QJL) {
+        kv->qjl = (float*)ctx_alloc(ctx, (size_t)2 * d * d * sizeof(float));
+        if (!kv->qjl) { hq_kv_free(ctx, kv); return HQ_ERR_ALLOC; }
+    }
+    kv->cfg.qjl_dev = nullptr;   // the cache keeps its own copy
     kv->att_ws_bytes = attend_workspace_bytes(ctx, kv);
     kv->att_ws = (float*)ctx_alloc(ctx, kv->att_ws_bytes);
     if (cudaHostAlloc((void**)&kv->flag_host, 64, cudaHostAllocMapped) != cudaSuccess ||
@@ -667,6 +672,10 @@ hq_status hq_kv_create(hq_ctx* ctx, const hq_kv_config* cfg, hq_kv** out) {
     cudaMemset(kv->counters, 0, 64);
     launch_signs(cfg->codec.seed, 1u, d, kv->dsign, 0);
     launch_signs(cfg->codec.seed, 2u, d, kv->ssign, 0);
+    if (kv->qjl) {
+        cudaMemcpyAsync(kv->qjl, cfg->qjl_dev, (size_t)d * d * sizeof(float), cudaMemcpyDeviceToDevice, 0);
+        launch_transpose_f32(kv->qjl, kv->qjl + (size_t)d * d, d, 0);
+    }
     cudaError_t e = cudaDeviceSynchronize();
     if (e != cudaSuccess) {
         ctx->err = cudaGetErrorString(e);
@@ -682,7 +691,7 @@ void hq_kv_free(hq_ctx* ctx, hq_kv* kv) {
     if (!ctx) ctx = kv->ctx;
     ctx_free(ctx, kv->rem); ctx_free(ctx, kv->una); ctx_free(ctx, kv->ulen); ctx_free(ctx, kv->norm);
     ctx_free(ctx, kv->blk_off); ctx_free(ctx, kv->upos); ctx_free(ctx, kv->ring); ctx_free(ctx, kv->dsign);
-    ctx_free(ctx, kv->ssign); ctx_free(ctx, kv->counters); ctx_free(ctx, kv->scratch_codes); ctx_free(ctx, kv->att_ws);
+    ctx_free(ctx, kv->ssign); ctx_free(ctx, kv->qjl); ctx_free(ctx, kv->counters); ctx_free(ctx, kv->scratch_codes); ctx_free(ctx, kv->att_ws);
     if (kv->flag_host) { cudaDeviceSynchronize(); cudaFreeHost(kv->flag_host); }
     delete kv;
 }
@@ -721,7 +730,7 @@ hq_status hq_kv_append(hq_ctx* ctx, hq_kv* kv, const void* k_dev, const void* v_
             uint16_t* norm_r = kv->norm + (int64_t)role * H * kv->cfg.max_tokens;
             launch_quantize_kv(src, nt, H, d, token0, role, kv->cfg.codec.lattice, kv->A, kv->cfg.rotation,
                                kv->cfg.dither, kv->cfg.codec.seed, kv->dsign, kv->ssign, codes, norm_r,
-                               kv->cfg.max_tokens, kv->counters, st);
+                               kv->cfg.max_tokens, kv->counters, st, kv->qjl ? kv->qjl + (size_t)d * d : nullptr);
             launch_kv_pack(codes, nt, H, d, token0, role, kv->cfg.codec.lattice, kv->k0, kv->k1, kv->rbits,
                            kv->cfg.max_tokens, kv->rem_words, kv->una_words, kv->n_blk, kv->rem, kv->una, kv->ulen,
                            kv->blk_off, kv->upos, err_flag, st);

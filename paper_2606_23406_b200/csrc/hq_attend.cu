@@ -95,12 +95,13 @@ struct AttendParams {
     uint64_t seed;
     const __nv_bfloat16* q;  // [q_heads, d]
     const int8_t *dsign, *ssign;
+    const float *qjl, *qjl_t;   // HQ_ROT_QJL: S row-major and S transposed (null otherwise)
     float* ws;               // [H][n_split][G][d + 2]
 };
 
 // q' = S * RHT(q) for one head, in smem (fp32), by one warp (FORMAT R1 order; any order would do here)
 __device__ inline void warp_query_transform(float* s, int d, const int8_t* dsign, const int8_t* ssign, int rotation,
-                                            int lane) {
+                                            const float* __restrict__ qjl_t, int lane) {
     for (int i = lane; i < d; i += 32)
         if (dsign[i] < 0) s[i] = -s[i];
     for (int h = 1; h < d; h <<= 1) {
@@ -119,6 +120,22 @@ __device__ inline void warp_query_transform(float* s, int d, const int8_t* dsign
         s[i] = (rotation == HQ_ROT_SIGNS && ssign[i] < 0) ? -v : v;
     }
     __syncwarp();
+    if (rotation == HQ_ROT_QJL) {   // q' = S RHT(q) (§3.4 eq.(2)): one d x d matvec per query head, not per cached token (L502)
+        float acc[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) acc[k] = 0.0f;
+        for (int j = 0; j < d; ++j) {
+            const float sj = s[j];
+#pragma unroll
+            for (int k = 0; k < 8; ++k)
+                if (k * 32 < d) acc[k] = fmaf(__ldg(qjl_t + (int64_t)j * d + k * 32 + lane), sj, acc[k]);
+        }
+        __syncwarp();
+#pragma unroll
+        for (int k = 0; k < 8; ++k)
+            if (k * 32 < d) s[k * 32 + lane] = acc[k];
+        __syncwarp();
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -228,7 +245,7 @@ k_attend_split(AttendParams p) {
     // q' = S RHT(q): transformed in the vt area (one row of d floats per head), then stored coordinate-major
     for (int i = tid; i < G * d; i += 128) vt[i] = __bfloat162float(p.q[(h * G) * d + i]);
     __syncthreads();
-    for (int g = warp; g < G; g += 4) warp_query_transform(vt + g * d, d, p.dsign, p.ssign, p.rotation, lane);
+    for (int g = warp; g < G; g += 4) warp_query_transform(vt + g * d, d, p.dsign, p.ssign, p.rotation, p.qjl_t, lane);
     __syncthreads();
     for (int i = tid; i < d * GP; i += 128) {
         const int j = i / GP, g = i % GP;
@@ -428,6 +445,13 @@ __global__ void k_attend_combine(AttendParams p, const __nv_bfloat16* ring, int 
     // un-rotate the code-domain sum: x = D H (S u) / sqrt(d)
     code[j] = (p.rotation == HQ_ROT_SIGNS && p.ssign[j] < 0) ? -a : a;
     __syncthreads();
+    if (p.rotation == HQ_ROT_QJL) {   // S^T: code_j <- sum_i S_ij code_i (thread j walks column j of S: coalesced)
+        float r = 0.0f;
+        for (int i = 0; i < d; ++i) r = fmaf(__ldg(p.qjl + (int64_t)i * d + j), code[i], r);
+        __syncthreads();
+        code[j] = r;
+        __syncthreads();
+    }
     for (int hh = 1; hh < d; hh <<= 1) {
         float x = 0.0f, y = 0.0f;
         int i = 0;
@@ -489,6 +513,7 @@ hq_status launch_attend(hq_ctx* ctx, const hq_kv* kv, const void* q, int q_heads
     p.inv_sqrt_d = (float)(1.0 / sqrt((double)d));
     p.seed = kv->cfg.codec.seed;
     p.q = (const __nv_bfloat16*)q; p.dsign = kv->dsign; p.ssign = kv->ssign; p.ws = kv->att_ws;
+    p.qjl = kv->qjl; p.qjl_t = kv->qjl ? kv->qjl + (size_t)kv->cfg.head_dim * kv->cfg.head_dim : nullptr;
     const int GP = p.G <= 4 ? 4 : 8;
     size_t smem = ((size_t)GP * d + 128 * (size_t)(d + 1) + (size_t)GP * 128 + (size_t)GP * 4) * sizeof(float);
 #define HQ_AT(L)                                                                                                   \

@@ -96,13 +96,39 @@ __device__ inline int quantize_blocks(const float* u, int n, float g, bool with_
 
 constexpr int QW_WARPS = 4;
 
+// FORMAT R11 (qjl rotation, eq.(2)): u'_i = sum_j Q_ij u_j, accumulated in increasing j with one fused
+// multiply-add per term (canonical: the result decides the codes).  u[n] in shared memory, one warp;
+// qt = S transposed ([j][i]: the lanes' loads are coalesced and hit L1 - the matrix is 64 KB at d = 128).
+__device__ __forceinline__ void warp_qjl_apply(float* u, int n, const float* __restrict__ qt, int lane) {
+    float acc[8];   // n <= 256: outputs lane, lane + 32, ...
+#pragma unroll
+    for (int k = 0; k < 8; ++k) acc[k] = 0.0f;
+    for (int j = 0; j < n; ++j) {
+        const float uj = u[j];
+#pragma unroll
+        for (int k = 0; k < 8; ++k)
+            if (k * 32 < n) acc[k] = __fmaf_rn(__ldg(qt + (int64_t)j * n + k * 32 + lane), uj, acc[k]);
+    }
+    __syncwarp();
+#pragma unroll
+    for (int k = 0; k < 8; ++k)
+        if (k * 32 < n) u[k * 32 + lane] = acc[k];
+    __syncwarp();
+}
+
+__global__ void k_transpose_f32(const float* __restrict__ a, float* __restrict__ at, int n) {
+    const int i = blockIdx.x, j = threadIdx.x;   // at[j][i] = a[i][j]
+    at[(int64_t)j * n + i] = a[(int64_t)i * n + j];
+}
+void launch_transpose_f32(const float* a, float* at, int n, cudaStream_t st) { k_transpose_f32<<<n, n, 0, st>>>(a, at, n); }
+
 // mode 0: weights (tile = (row, kt));  mode 1: KV (tile = (token, head), rotation, dither)
 template <int LAT, int MODE>
 __global__ void __launch_bounds__(QW_WARPS * 32)
 k_quantize(const void* X, int dtype, int64_t n_tiles, int64_t n_kt, int64_t ld, int n, float A,
            const int8_t* dsign, const int8_t* ssign, int rotation, int dither, uint64_t seed, int64_t token0,
            int role, int H, int64_t max_tokens, int8_t* codes, uint16_t* norms, unsigned long long* counters,
-           int want_totals) {
+           int want_totals, const float* qjl_t) {
     extern __shared__ float smem[];
     int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     float* u = smem + warp * 2 * n;
@@ -123,6 +149,10 @@ k_quantize(const void* X, int dtype, int64_t n_tiles, int64_t n_kt, int64_t ld, 
         if (MODE == 1 && rotation == HQ_ROT_SIGNS)
             for (int i = lane; i < n; i += 32)
                 if (ssign[i] < 0) u[i] = -u[i];
+        if (MODE == 1 && rotation == HQ_ROT_QJL) {
+            __syncwarp();
+            warp_qjl_apply(u, n, qjl_t, lane);
+        }
         for (int i = lane; i < n; i += 32) t[i] = __fmul_rn(u[i], u[i]);
         float ss = warp_treesum(t, n, lane);
         float rho32 = __fsqrt_rn(ss);
@@ -163,11 +193,11 @@ static void launch_quantize_any(int lattice, dim3 grid, size_t smem, cudaStream_
                                 int64_t n_tiles, int64_t n_kt, int64_t ld, int n, float A, const int8_t* dsign,
                                 const int8_t* ssign, int rotation, int dither, uint64_t seed, int64_t token0,
                                 int role, int H, int64_t max_tokens, int8_t* codes, uint16_t* norms,
-                                unsigned long long* counters, int want_totals) {
+                                unsigned long long* counters, int want_totals, const float* qjl_t = nullptr) {
 #define HQ_LAUNCH_Q(L)                                                                                        \
     k_quantize<L, MODE><<<grid, QW_WARPS * 32, smem, st>>>(X, dtype, n_tiles, n_kt, ld, n, A, dsign, ssign,   \
                                                            rotation, dither, seed, token0, role, H,           \
-                                                           max_tokens, codes, norms, counters, want_totals)
+                                                           max_tokens, codes, norms, counters, want_totals, qjl_t)
     switch (lattice) {
         case LAT_Z: HQ_LAUNCH_Q(LAT_Z); break;
         case LAT_A2: HQ_LAUNCH_Q(LAT_A2); break;
@@ -190,13 +220,13 @@ void launch_quantize_weights(const void* W, int dtype, int64_t m, int64_t n_in, 
 void launch_quantize_kv(const void* x, int64_t n_tok, int H, int d, int64_t token0, int role, int lattice,
                         float A, int rotation, int dither, uint64_t seed, const int8_t* dsign,
                         const int8_t* ssign, int8_t* codes, uint16_t* norm_out, int64_t max_tokens,
-                        unsigned long long* counters, cudaStream_t st) {
+                        unsigned long long* counters, cudaStream_t st, const float* qjl_t) {
     int64_t n_tiles = n_tok * H;
     int64_t blocks = (n_tiles + QW_WARPS - 1) / QW_WARPS;
     if (blocks > 148 * 16) blocks = 148 * 16;
     launch_quantize_any<1>(lattice, dim3((unsigned)blocks), QW_WARPS * 2 * d * sizeof(float), st, x, HQ_BF16,
                            n_tiles, H, 0, d, A, dsign, ssign, rotation, dither, seed, token0, role, H, max_tokens,
-                           codes, norm_out, counters, 0);
+                           codes, norm_out, counters, 0, qjl_t);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -967,6 +997,7 @@ struct KvAppend1 {
     float A;
     uint64_t seed;
     const int8_t *dsign, *ssign;
+    const float* qjl_t;            // HQ_ROT_QJL: S transposed
     uint32_t *rem, *una, *blk_off, *upos;
     uint16_t *ulen, *norm;
     __nv_bfloat16* ring;
@@ -993,6 +1024,10 @@ k_kv_append1(KvAppend1 p) {
     if (p.rotation == HQ_ROT_SIGNS)
         for (int i = lane; i < d; i += 32)
             if (p.ssign[i] < 0) u[i] = -u[i];
+    if (p.rotation == HQ_ROT_QJL) {
+        __syncwarp();
+        warp_qjl_apply(u, d, p.qjl_t, lane);
+    }
     for (int i = lane; i < d; i += 32) t[i] = __fmul_rn(u[i], u[i]);
     const float ss = warp_treesum(t, d, lane);
     const uint16_t hb = f32_to_f16_bits_sat(__fsqrt_rn(ss));
@@ -1053,6 +1088,7 @@ void launch_kv_append1(const hq_kv* kv, const void* k, const void* v, cudaStream
     p.k0 = kv->k0; p.k1 = kv->k1; p.rbits = kv->rbits; p.window = kv->cfg.window;
     p.token = kv->n_tokens; p.max_tokens = kv->cfg.max_tokens; p.rem_words = kv->rem_words; p.una_words = kv->una_words;
     p.n_blk = kv->n_blk; p.A = kv->A; p.seed = kv->cfg.codec.seed; p.dsign = kv->dsign; p.ssign = kv->ssign;
+    p.qjl_t = kv->qjl ? kv->qjl + (size_t)p.d * p.d : nullptr;
     p.rem = kv->rem; p.una = kv->una; p.blk_off = kv->blk_off; p.upos = kv->upos; p.ulen = kv->ulen; p.norm = kv->norm;
     p.ring = kv->ring; p.counters = kv->counters; p.flag = kv->flag_dev;
     const size_t smem = (size_t)p.d * (4 + 4 + 1 + 1);

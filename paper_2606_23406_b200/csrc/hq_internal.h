@@ -69,6 +69,7 @@ struct hq_kv {
     __nv_bfloat16* ring;  // [2][window][H][d]
     int8_t* dsign;      // [d]
     int8_t* ssign;      // [d]
+    float* qjl;         // HQ_ROT_QJL: [2][d][d] - S row-major, then S transposed (null otherwise)
     unsigned long long* counters;  // [0] clamp count
     int* flag_host;                // mapped pinned host word: 0 ok, 1 a U-section past 65534 bits, 2 U stream full (sticky)
     int* flag_dev;                 // its device alias (the append kernels raise it, the host polls it without a sync)
@@ -113,7 +114,8 @@ void launch_quantize_weights(const void* W, int dtype, int64_t m, int64_t n_in, 
 void launch_quantize_kv(const void* x, int64_t n_tok, int H, int d, int64_t token0, int role, int lattice,
                         float A, int rotation, int dither, uint64_t seed, const int8_t* dsign,
                         const int8_t* ssign, int8_t* codes, uint16_t* norm_out, int64_t max_tokens,
-                        unsigned long long* counters, cudaStream_t st);
+                        unsigned long long* counters, cudaStream_t st, const float* qjl_t = nullptr);
+void launch_transpose_f32(const float* a, float* at, int n, cudaStream_t st);
 // activations: x [B, n_in] -> q int8 [B, n_in], s_x [B, n_kt], optional u
 void launch_act_quant(const void* x, int dtype, int64_t B, int64_t n_in, int64_t ldx, int lattice, int n,
                       const int8_t* dsign, int8_t* q, float* s_x, float* u, cudaStream_t st);
