@@ -405,24 +405,44 @@ __global__ void k_attend_combine(AttendParams p, const __nv_bfloat16* ring, int 
     float* code = sm;        // [d] code-domain accumulator
     float* sc = code + d;    // [window] window scores
     float* qf = sc + (window > 0 ? window : 1);  // [d]
+    float* fs = qf + d;      // [n_split] exp(m_s - m), 0 for an empty split
+    float* ls = fs + p.n_split;   // [n_split] the split's softmax denominator
+    float* red = ls + p.n_split;  // [d / 32] block reduction
     __shared__ float s_m, s_l;
     const int qh = blockIdx.x, h = qh / G, g = qh % G, j = threadIdx.x;
-    // global max over splits
+    const float* wbase = p.ws + ((int64_t)h * p.n_split * G + g) * (d + 2);   // split s at + s * G * (d + 2)
+    const int64_t wstride = (int64_t)G * (d + 2);
+    // global max over splits: thread j takes splits j, j + d, ... (independent loads), then a block reduction
     float m = -INFINITY;
-    for (int s = 0; s < p.n_split; ++s) {
-        const float* w = p.ws + ((int64_t)(h * p.n_split + s) * G + g) * (d + 2);
-        if (w[d + 1] > 0.0f) m = fmaxf(m, w[d]);
+    for (int s = j; s < p.n_split; s += d) {
+        const float* w = wbase + s * wstride;
+        const float ms = __ldcg(w + d), l = __ldcg(w + d + 1);
+        fs[s] = ms;
+        ls[s] = l;
+        if (l > 0.0f) m = fmaxf(m, ms);
     }
+#pragma unroll
+    for (int o = 16; o; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((j & 31) == 0) red[j >> 5] = m;
     // window scores (original domain, exact bf16 K)
     qf[j] = __bfloat162float(p.q[qh * d + j]);
     __syncthreads();
+    for (int i = 0; i < d / 32; ++i) m = fmaxf(m, red[i]);
     const int64_t w0 = p.Tc;
     const int nw = (int)(T - w0);
     if (j < nw) {
         int64_t t = w0 + j;
-        const __nv_bfloat16* kr = ring + ((int64_t)(0 * window + (t % window)) * p.H + h) * d;
+        const uint4* kr = (const uint4*)(ring + ((int64_t)(0 * window + (t % window)) * p.H + h) * d);   // rows are 2 d bytes: 16-byte aligned
         float dot = 0.0f;
-        for (int i = 0; i < d; ++i) dot += qf[i] * __bfloat162float(kr[i]);
+        for (int i8 = 0; i8 < d / 8; ++i8) {
+            const uint4 v = __ldg(kr + i8);
+            const uint32_t wv[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                dot += qf[8 * i8 + 2 * e] * __uint_as_float(wv[e] << 16);
+                dot += qf[8 * i8 + 2 * e + 1] * __uint_as_float(wv[e] & 0xffff0000u);
+            }
+        }
         sc[j] = dot * p.inv_sqrt_d;
     }
     __syncthreads();
@@ -433,14 +453,21 @@ __global__ void k_attend_combine(AttendParams p, const __nv_bfloat16* ring, int 
     }
     __syncthreads();
     m = s_m;
+    for (int s = j; s < p.n_split; s += d) fs[s] = ls[s] > 0.0f ? __expf(fs[s] - m) : 0.0f;
+    __syncthreads();
+    // the splits in split order (deterministic), eight loads in flight at a time
     float a = 0.0f, l = 0.0f;
-    for (int s = 0; s < p.n_split; ++s) {
-        const float* w = p.ws + ((int64_t)(h * p.n_split + s) * G + g) * (d + 2);
-        if (w[d + 1] > 0.0f) {
-            float f = __expf(w[d] - m);
-            a += f * w[j];
-            l += f * w[d + 1];
-        }
+    for (int s0 = 0; s0 < p.n_split; s0 += 8) {
+        float v[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) v[u] = (s0 + u < p.n_split && ls[s0 + u] > 0.0f) ? __ldcg(wbase + (s0 + u) * wstride + j) : 0.0f;
+#pragma unroll
+        for (int u = 0; u < 8; ++u)
+            if (s0 + u < p.n_split && ls[s0 + u] > 0.0f) {
+                const float f = fs[s0 + u];
+                a += f * v[u];
+                l += f * ls[s0 + u];
+            }
     }
     // un-rotate the code-domain sum: x = D H (S u) / sqrt(d)
     code[j] = (p.rotation == HQ_ROT_SIGNS && p.ssign[j] < 0) ? -a : a;
@@ -549,7 +576,7 @@ hq_status launch_attend(hq_ctx* ctx, const hq_kv* kv, const void* q, int q_heads
         p.n_split = 0;
     }
 #undef HQ_AT
-    size_t smem2 = (size_t)(2 * d + (window > 0 ? window : 1)) * sizeof(float);
+    size_t smem2 = (size_t)(2 * d + (window > 0 ? window : 1) + 2 * p.n_split + d / 32) * sizeof(float);
     k_attend_combine<<<q_heads, d, smem2, st>>>(p, kv->ring, (int)window, kv->n_tokens, (__nv_bfloat16*)out_bf16, out_f32);
     HQ_CUDA_CHECK(ctx, cudaGetLastError());
     return HQ_OK;
