@@ -843,6 +843,73 @@ void hqo_linear(const int8_t* codes, const uint16_t* norms, int64_t m, int64_t n
         }
 }
 
+/* ------------------------------------------------------------------------------------------ */
+/* §4.8 L299 / §6.3: the FP8-E4M3 cast of both MMA operands ("a per-tile FP8 or INT8 cast for the MMA");        */
+/* FORMAT R12.  E4M3 (fn): 1 sign, 4 exponent (bias 7), 3 mantissa bits; normals 2^-6 .. 448, subnormal step 2^-9;   */
+/* round to nearest even, magnitudes that would round above 448 saturate to 448.                                      */
+/* ------------------------------------------------------------------------------------------ */
+float hqo_e4m3_round(float v) {
+    if (v != v) return v;
+    float a = fabsf(v), r;
+    if (a >= 448.0f) r = 448.0f;
+    else if (a < 0x1p-6f) r = rintf(a * 512.0f) / 512.0f;          /* subnormals: multiples of 2^-9 */
+    else {
+        int e;
+        (void)frexpf(a, &e);                                       /* a = f * 2^e, f in [0.5, 1): 2^(e-1) <= a */
+        float step = ldexpf(1.0f, e - 1 - 3);                      /* 3 mantissa bits */
+        r = rintf(a / step) * step;                                /* power-of-two division: exact; rintf = RNE */
+        if (r > 448.0f) r = 448.0f;
+    }
+    return v < 0.0f ? -r : r;
+}
+void hqo_e4m3_round_array(const float* v, int64_t n, float* out) {
+    for (int64_t i = 0; i < n; ++i) out[i] = hqo_e4m3_round(v[i]);
+}
+
+/* activations (R12): u by R1; amax; q8_i = e4m3(u_i * (448 / amax)); s_x = amax / 448.  E8 / D4 / Z (no sqrt 3 factor). */
+void hqo_act_quant_fp8(const float* x, int64_t B, int64_t n_in, int64_t ldx, int n, uint64_t seed,
+                       float* q8 /*[B,n_in] E4M3 values*/, float* s_x /*[B,n_kt]*/) {
+    int64_t n_kt = n_in / n;
+    int8_t* d = (int8_t*)malloc((size_t)n_in);
+    hqo_signs(seed, 1u, n_in, d);
+    for (int64_t b = 0; b < B; ++b)
+        for (int64_t kt = 0; kt < n_kt; ++kt) {
+            float u[1024], amax = 0.0f;
+            hqo_rht_f32(x + b * ldx + kt * n, d + kt * n, n, u);
+            for (int i = 0; i < n; ++i)
+                if (fabsf(u[i]) > amax) amax = fabsf(u[i]);
+            float* qq = q8 + b * n_in + kt * n;
+            if (amax == 0.0f) {
+                for (int i = 0; i < n; ++i) qq[i] = 0.0f;
+                s_x[b * n_kt + kt] = 0.0f;
+                continue;
+            }
+            float inv = 448.0f / amax;
+            for (int i = 0; i < n; ++i) qq[i] = hqo_e4m3_round(u[i] * inv);
+            s_x[b * n_kt + kt] = amax / 448.0f;
+        }
+    free(d);
+}
+
+/* y[b,r] = Σ_kt (ρ[r,kt]/(α√n))·s_x[b,kt]·Σ_{i in tile} e4m3(c[r,i])·q8[b,i]   (double; products of two E4M3 values are exact) */
+void hqo_linear_fp8(const int8_t* codes, const uint16_t* norms, int64_t m, int64_t n_in, int lattice, int n,
+                    double snr_db, const float* q8, const float* s_x, int64_t B, double* y /*[B,m]*/) {
+    int64_t n_kt = n_in / n;
+    double inv_A = 1.0 / (hqo_alpha(lattice, snr_db) * sqrt((double)n));
+#pragma omp parallel for schedule(static)
+    for (int64_t r = 0; r < m; ++r)
+        for (int64_t b = 0; b < B; ++b) {
+            double yy = 0.0;
+            for (int64_t kt = 0; kt < n_kt; ++kt) {
+                double a = 0.0;
+                for (int i = 0; i < n; ++i)
+                    a += (double)hqo_e4m3_round((float)codes[r * n_in + kt * n + i]) * (double)q8[b * n_in + kt * n + i];
+                yy += (double)f16_bits_to_f32(norms[r * n_kt + kt]) * inv_A * (double)s_x[b * n_kt + kt] * a;
+            }
+            y[b * m + r] = yy;
+        }
+}
+
 /* sampled version for sizes where the full contraction is too slow on a CPU: outputs (b_s, r_s) */
 void hqo_linear_sampled(const int8_t* codes, const uint16_t* norms, int64_t m, int64_t n_in,
                         int lattice, int n, double snr_db, const int8_t* q, const float* s_x,

@@ -350,3 +350,27 @@ def silu_mul_bf16(a, b):
     a = _c(a, np.float32); b = _c(b, np.float32); x = np.empty_like(a)
     lib().hqo_silu_mul_bf16(_p(a), _p(b), C.c_int64(a.size), _p(x))
     return x
+
+
+# ---- FP8-E4M3 MMA cast (§4.8, §6.3; FORMAT R12)
+def e4m3_round(x):
+    x = _c(x, np.float32); out = np.empty_like(x)
+    lib().hqo_e4m3_round_array(_p(x), C.c_int64(x.size), _p(out))
+    return out
+
+
+def act_quant_fp8(x, n_tile, seed):
+    x = _c(x, np.float32); B, n_in = x.shape
+    q8 = np.zeros((B, n_in), np.float32); s_x = np.zeros((B, n_in // n_tile), np.float32)
+    lib().hqo_act_quant_fp8(_p(x), C.c_int64(B), C.c_int64(n_in), C.c_int64(n_in), C.c_int(n_tile), C.c_uint64(seed),
+                            _p(q8), _p(s_x))
+    return q8, s_x
+
+
+def linear_fp8(codes, norms, lattice, n_tile, snr_db, q8, s_x):
+    codes = _c(codes, np.int8); norms = _c(norms, np.uint16); q8 = _c(q8, np.float32); s_x = _c(s_x, np.float32)
+    m, n_in = codes.shape; B = q8.shape[0]
+    y = np.zeros((B, m), np.float64)
+    lib().hqo_linear_fp8(_p(codes), _p(norms), C.c_int64(m), C.c_int64(n_in), lattice, C.c_int(n_tile),
+                         C.c_double(snr_db), _p(q8), _p(s_x), C.c_int64(B), _p(y))
+    return y
