@@ -163,7 +163,7 @@ def measure_large_m(ctx, hq, dev, reps=10):
     del a, b
     res["peak"], res["peak_source"] = peak, "torch._int_mm 8192^3 INT8, measured in this run"
     res["peak_nominal_dense_int8"] = 4500.0
-    tot_ops, tot_ms = 0.0, 0.0
+    tot_ops, tot_ms, fp8_ms = 0.0, 0.0, []
     for m, n_in, seed in ((16384, 4096, 5), (4096, 16384, 7)):
         W = torch.from_numpy(hq_synth.gaussian_weight(m, n_in, seed=seed)).to(dev).to(torch.bfloat16)
         w = ctx.encode_weights(W, hq.Lattice.E8, LARGE_M_TILE, SNR_E8_4BPS, seed=seed)
@@ -175,9 +175,16 @@ def measure_large_m(ctx, hq, dev, reps=10):
         res["gemms"].append({"shape": f"8192 tokens x {n_in} -> {m}", "ms": ms, "TOPS": ops / (ms * 1e-3) / 1e12,
                              "frac": ops / (ms * 1e-3) / 1e12 / peak})
         tot_ops += ops; tot_ms += ms
+        # the same GEMM with the FP8-E4M3 cast of PAPER.md §4.8 (hq_linear_cast: kind::f8f6f4, fp32 accumulator)
+        ms8 = _time_cuda(lambda: w.linear_cast(X, hq.CAST_FP8_E4M3, y=y), reps=reps, warm=2)
+        fp8_ms.append(ms8)
         w.free(); del X, y
     res["achieved"] = tot_ops / (tot_ms * 1e-3) / 1e12
     res["frac"] = res["achieved"] / peak
+    fp8_tops = tot_ops / (sum(fp8_ms) * 1e-3) / 1e12
+    res["fp8_e4m3"] = {"ms": fp8_ms, "achieved": fp8_tops, "peak": peak, "frac": fp8_tops / peak,
+                       "peak_source": "the in-run INT8 peak x 1.0 (B200's nominal dense FP8 : INT8 ratio)",
+                       "what": "hq_linear_cast(HQ_CAST_FP8_E4M3) on the same two GEMMs (SURVEY §8(f)2)"}
     res["n_tile"] = LARGE_M_TILE
     res["workload"] = "BASELINE configs[4]: 8192 tokens x (4096 -> 16384, 16384 -> 4096), E8 4 bps, bf16 activations through the per-tile RHT"
     return res

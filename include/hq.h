@@ -195,6 +195,19 @@ hq_status hq_linear(hq_ctx* ctx, const hq_weight* w, const void* x_dev, int32_t 
                     int32_t* acc_i32_dev_or_null, void* stream);
 
 /*
+ * hq_linear with the MMA cast of §4.8 chosen by the caller ("cast at the matmul boundary to FP8-E4M3/INT8";
+ * §6.3 L433-448 compares the two).  HQ_CAST_INT8 is hq_linear.  HQ_CAST_FP8_E4M3 (docs/FORMAT.md R12): the
+ * decoded integer coordinates and the RHT'd activations (per-tile amax -> 448) are rounded to E4M3 and contracted by
+ * tcgen05.mma kind::f8f6f4 into an fp32 accumulator; y = sum_kt (rho / (alpha sqrt n)) s_x acc as for INT8.  Built for the
+ * compute-bound regime on the large-M pipeline: E8, tile 128 or 256, k <= 3, batch >= 64 - anything else ->
+ * HQ_ERR_UNSUPPORTED.  The accumulation order inside the tensor core is the hardware's: y meets the 1e-3 bar against
+ * the reference, it is not bit-reproducible across GPU generations.  NVFP4 / MXFP4 (§6.4) are not built.
+ */
+typedef enum { HQ_CAST_INT8 = 0, HQ_CAST_FP8_E4M3 = 1 } hq_cast;
+hq_status hq_linear_cast(hq_ctx* ctx, const hq_weight* w, const void* x_dev, int32_t dtype, int64_t batch, int64_t ldx,
+                         void* y_bf16_dev, int64_t ldy, float* y_f32_dev_or_null, int32_t cast, void* stream);
+
+/*
  * Several weights applied to the SAME x in one fused launch (q/k/v or gate/up of a decoder layer: §5.1 L309 quantizes
  * every nn.Linear separately, the forward shares the input).  ws[i] -> ys_bf16[i] [batch, m_i] (leading dimension
  * ldys[i]).  From 2 activation rows the results are bit-identical to n_w separate hq_linear calls; at batch 1 the K range of

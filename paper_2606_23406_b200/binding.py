@@ -73,6 +73,7 @@ class _LayerScratch(C.Structure):
 
 
 FOLD_NONE, FOLD_RMSNORM, FOLD_SILU_MUL = 0, 1, 2
+CAST_INT8, CAST_FP8_E4M3 = 0, 1
 
 
 class _KVView(C.Structure):
@@ -91,7 +92,7 @@ _lib = None
 EXPORTS = ["hq_create", "hq_destroy", "hq_last_error", "hq_measure_decode_ceiling", "hq_alpha", "hq_snr_for_bps", "hq_profile_enable", "hq_profile_read",
            "hq_encode_weights", "hq_weight_free", "hq_weight_get_info", "hq_weight_stats", "hq_weight_export",
            "hq_weight_export_host", "hq_weight_import", "hq_decode_int8", "hq_act_quant", "hq_linear",
-           "hq_linear_group", "hq_linear_group_fold", "hq_layer_scratch_view", "hq_layer_decode", "hq_linear_static", "hq_linear_workspace_bytes", "hq_kv_create", "hq_kv_free", "hq_kv_append", "hq_attend", "hq_kv_export",
+           "hq_linear_cast", "hq_linear_group", "hq_linear_group_fold", "hq_layer_scratch_view", "hq_layer_decode", "hq_linear_static", "hq_linear_workspace_bytes", "hq_kv_create", "hq_kv_free", "hq_kv_append", "hq_attend", "hq_kv_export",
            "hq_kv_decode_int8"]
 
 
@@ -123,6 +124,7 @@ def load_library():
     lib.hq_decode_int8.argtypes = [vp, vp, vp, vp, vp]
     lib.hq_act_quant.argtypes = [vp, vp, vp, i32, i64, i64, vp, vp, vp, vp]
     lib.hq_linear.argtypes = [vp, vp, vp, i32, i64, i64, vp, i64, vp, vp, vp]
+    lib.hq_linear_cast.argtypes = [vp, vp, vp, i32, i64, i64, vp, i64, vp, i32, vp]
     lib.hq_linear_static.argtypes = [vp, vp, vp, i32, vp, vp, vp]
     lib.hq_linear_group.argtypes = [vp, C.POINTER(vp), i32, vp, i32, i64, i64, C.POINTER(vp), C.POINTER(i64), C.POINTER(vp), vp]
     lib.hq_linear_group_fold.argtypes = [vp, C.POINTER(vp), i32, vp, C.POINTER(_Fold), C.POINTER(vp), C.POINTER(vp), vp]
@@ -360,6 +362,19 @@ class Weight:
             return y, y32, acc
         return y
 
+
+    def linear_cast(self, x: torch.Tensor, cast: int, y: torch.Tensor = None, want_f32=False):
+        """hq_linear_cast: cast 0 = INT8 (hq_linear), 1 = FP8-E4M3 operands with an fp32 tensor-core accumulator."""
+        dev = self.ctx.device
+        assert x.is_cuda and x.dim() == 2 and x.stride(1) == 1
+        B = x.shape[0]
+        if y is None:
+            y = torch.empty((B, self.m), dtype=torch.bfloat16, device=dev)
+        y32 = torch.empty((B, self.m), dtype=torch.float32, device=dev) if want_f32 else None
+        self.ctx.check(self.ctx.lib.hq_linear_cast(self.ctx.h, self.h, x.data_ptr(), _dtype_code(x), B, x.stride(0),
+                                                   y.data_ptr(), y.stride(0), y32.data_ptr() if want_f32 else None,
+                                                   int(cast), _stream_ptr(dev)))
+        return (y, y32) if want_f32 else y
 
     def linear_static(self, x: torch.Tensor, y: torch.Tensor, y32: torch.Tensor = None):
         """hq_linear_static: one activation row, outputs given by the caller, no allocation anywhere in the call."""

@@ -57,6 +57,53 @@ __device__ __forceinline__ float warp_act_tile128(float* x, int lane, int* q) {
     return (amax == 0.0f) ? 0.0f : __fdiv_rn(amax, 127.0f);
 }
 
+// The FP8-E4M3 cast of the same tile (FORMAT R12; §4.8): identical RHT, then q8 = e4m3(u * 448 / amax) as
+// bytes (in q[], low 8 bits) and s_x = amax / 448.
+__device__ __forceinline__ float warp_act_tile128_fp8(float* x, int lane, int* q) {
+    {
+        float a = x[0], c = x[1];
+        x[0] = __fadd_rn(a, c); x[1] = __fsub_rn(a, c);
+        a = x[2]; c = x[3];
+        x[2] = __fadd_rn(a, c); x[3] = __fsub_rn(a, c);
+        a = x[0]; c = x[2];
+        x[0] = __fadd_rn(a, c); x[2] = __fsub_rn(a, c);
+        a = x[1]; c = x[3];
+        x[1] = __fadd_rn(a, c); x[3] = __fsub_rn(a, c);
+    }
+#pragma unroll
+    for (int m = 1; m < 32; m <<= 1) {
+        const float sg1 = (lane & m) ? -1.0f : 1.0f;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const float o = __shfl_xor_sync(0xffffffffu, x[j], m);
+            x[j] = __fmaf_rn(x[j], sg1, o);
+        }
+    }
+    const float cn = (float)(1.0 / sqrt(128.0));
+    float amax = 0.0f;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        x[j] = __fmul_rn(x[j], cn);
+        amax = fmaxf(amax, fabsf(x[j]));
+    }
+#pragma unroll
+    for (int sft = 16; sft; sft >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, sft));
+    if (amax == 0.0f) {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) q[j] = 0;
+        return 0.0f;
+    }
+    const float inv = __fdiv_rn(448.0f, amax);
+#pragma unroll
+    for (int j = 0; j < 4; j += 2) {
+        uint16_t r;
+        asm("cvt.rn.satfinite.e4m3x2.f32 %0, %1, %2;" : "=h"(r) : "f"(__fmul_rn(x[j + 1], inv)), "f"(__fmul_rn(x[j], inv)));
+        q[j] = (int)(r & 0xffu);
+        q[j + 1] = (int)(r >> 8);
+    }
+    return __fdiv_rn(amax, 448.0f);
+}
+
 // NT tiles at once, stage by stage (the tiles are independent: their shuffles and roundings interleave, so the latency
 // is that of one tile); per tile the same operations in the same order as warp_act_tile128: bit-identical.
 // x[i][4], q[i][4], sx[i] for tile i; tiles with on[i] == false (warp-uniform) are skipped.

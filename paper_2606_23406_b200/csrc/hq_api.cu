@@ -459,6 +459,30 @@ hq_status hq_linear(hq_ctx* ctx, const hq_weight* w, const void* x_dev, int32_t 
                          (uint8_t*)ctx->ws, st);
 }
 
+hq_status hq_linear_cast(hq_ctx* ctx, const hq_weight* w, const void* x_dev, int32_t dtype, int64_t batch, int64_t ldx,
+                         void* y_bf16_dev, int64_t ldy, float* y_f32_dev_or_null, int32_t cast, void* stream) {
+    if (!ctx) return HQ_ERR_INVALID_ARG;
+    if (cast == HQ_CAST_INT8) return hq_linear(ctx, w, x_dev, dtype, batch, ldx, y_bf16_dev, ldy, y_f32_dev_or_null, nullptr, stream);
+    if (cast != HQ_CAST_FP8_E4M3) return fail(ctx, HQ_ERR_INVALID_ARG, "bad cast");
+    if (!w || !x_dev || (!y_bf16_dev && !y_f32_dev_or_null)) return fail(ctx, HQ_ERR_INVALID_ARG, "null argument");
+    if (batch <= 0 || ldx < w->n_in || (y_bf16_dev && ldy < w->m)) return fail(ctx, HQ_ERR_SHAPE, "bad batch / ldx / ldy");
+    if (dtype != HQ_F32 && dtype != HQ_BF16) return fail(ctx, HQ_ERR_INVALID_ARG, "bad dtype");
+    if (w->ctx != ctx) return fail(ctx, HQ_ERR_INVALID_ARG, "the weight belongs to another context");
+    if (w->lattice != HQ_E8 || (w->n != 128 && w->n != 256) || w->k0 > 3 || batch < 64)
+        return fail(ctx, HQ_ERR_UNSUPPORTED, "the FP8 cast needs an E8 weight at tile 128 or 256, k <= 3 and batch >= 64");
+    HQ_ENTER(ctx);
+    const size_t need = (((size_t)((batch + 255) / 256) * (w->n_in / 128) * (256 * 128 + 256 * 4) + 255) & ~(size_t)255) +
+                        (((size_t)w->n_rb * (w->n_in / 128) * (16384 + 512) + 255) & ~(size_t)255) + 256;
+    if (need > ctx->ws_bytes) {
+        if (ctx->ws) { HQ_CUDA_CHECK(ctx, cudaDeviceSynchronize()); ctx_free(ctx, ctx->ws); ctx->ws = nullptr; ctx->ws_bytes = 0; }
+        ctx->ws = ctx_alloc(ctx, need);
+        if (!ctx->ws) return HQ_ERR_ALLOC;
+        ctx->ws_bytes = need;
+    }
+    return launch_linear_fp8(ctx, w, x_dev, dtype, batch, ldx, y_bf16_dev, ldy, y_f32_dev_or_null, (uint8_t*)ctx->ws,
+                             (cudaStream_t)stream);
+}
+
 hq_status hq_linear_static(hq_ctx* ctx, const hq_weight* w, const void* x_dev, int32_t dtype, void* y_bf16_dev,
                            float* y_f32_dev_or_null, void* stream) {
     if (!ctx) return HQ_ERR_INVALID_ARG;

@@ -277,7 +277,7 @@ k_act_quant(const void* X, int dtype, int64_t n_tiles, int64_t n_kt, int64_t ldx
 // weights (e8_kcol: 32c + 4i + b for block 4c+b, coordinate i), followed by NB fp32 scales s_x.  n = 128.
 __global__ void __launch_bounds__(QW_WARPS * 32)
 k_act_blob(const void* X, int dtype, int64_t B, int64_t n_kt, int64_t ldx, const int8_t* dsign, int NB,
-           uint8_t* bblob) {
+           uint8_t* bblob, int fp8) {
     // The tile lives in registers: lane l holds elements 4l .. 4l+3.  FORMAT R1's butterflies (ascending stride, a+b to
     // the lower index, a-b to the upper) are two in-register stages and five shuffle stages: the same additions on the
     // same pairs as warp_rht_inplace, so the result is bit-identical to k_act_quant.
@@ -325,10 +325,10 @@ k_act_blob(const void* X, int dtype, int64_t B, int64_t n_kt, int64_t ldx, const
 #pragma unroll
             for (int j = 0; j < 4; ++j)
                 if ((sg >> (8 * j)) & 0x80u) x[j] = -x[j];
-            sx = warp_act_tile128(x, lane, qv4);
+            sx = fp8 ? warp_act_tile128_fp8(x, lane, qv4) : warp_act_tile128(x, lane, qv4);   // FORMAT R7 or R12
         }
 #pragma unroll
-        for (int j = 0; j < 4; ++j) srow[colb + 4 * j] = (uint8_t)(int8_t)qv4[j];
+        for (int j = 0; j < 4; ++j) srow[colb + 4 * j] = (uint8_t)qv4[j];
         __syncwarp();
         // one coalesced 128-byte row: lane l owns operand columns 4l .. 4l+3 = 16-byte chunk l>>2 (swizzled), word l&3
         const uint32_t w4 = ((const uint32_t*)srow)[lane];
@@ -382,7 +382,7 @@ __device__ __forceinline__ void a256_fwht16(uint64_t* P) {
 
 struct A256Raw { uint4 a, b, sg; };   // a lane's 16 bf16 elements and their 16 sign bytes
 
-template <bool FAST>   // FAST: bf16 rows whose 16-element groups can be read as 16-byte words
+template <bool FAST, bool FP8>   // FAST: bf16 rows whose 16-element groups can be read as 16-byte words; FP8: E4M3 cast (FORMAT R12)
 __global__ void __launch_bounds__(A256_WARPS * 32, A256_CTAS)
 k_act_blob256(const void* X, int dtype, int64_t B, int64_t n_kt, int64_t ldx, const int8_t* dsign, int NB, uint8_t* bblob) {
     extern __shared__ float smem[];
@@ -472,13 +472,18 @@ k_act_blob256(const void* X, int dtype, int64_t B, int64_t n_kt, int64_t ldx, co
         uint32_t pk[2][2] = {{0u, 0u}, {0u, 0u}};                // pk[chunk][jj]: codes of elements m = 8 chunk + 4 jj .. + 3 (x 16 + l)
         float sx = 0.0f;
         if (amax != 0.0f) {
-            const float inv = __fdiv_rn(127.0f, amax);
+            const float inv = __fdiv_rn(FP8 ? 448.0f : 127.0f, amax);
             const uint64_t inv2 = a256_pack(__float_as_uint(inv), __float_as_uint(inv));
             uint32_t qlo[8], qhi[8];
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
                 float a, c;
                 a256_unpack(a256_mul2(P[j], inv2), a, c);
+                if (FP8) {   // byte 0 of qlo / qhi = e4m3(a) / e4m3(c): the packing below takes byte 0 only
+                    const uint32_t r = f32x2_to_e4m3x2(a, c);
+                    qlo[j] = r; qhi[j] = r >> 8;
+                    continue;
+                }
                 // rint + clamp to +-127 + cast in one instruction: |x| <= amax bounds |x * inv| by 127 (1 + 2^-23), which
                 // rounds to 127, so the saturating convert can never return -128 and equals FORMAT R7's clamp(rint(.))
                 asm("cvt.rni.sat.s8.f32 %0, %1;" : "=r"(qlo[j]) : "f"(a));
@@ -489,7 +494,7 @@ k_act_blob256(const void* X, int dtype, int64_t B, int64_t n_kt, int64_t ldx, co
                 pk[0][jj] = __byte_perm(__byte_perm(qlo[4 * jj], qlo[4 * jj + 1], 0x0040), __byte_perm(qlo[4 * jj + 2], qlo[4 * jj + 3], 0x0040), 0x5410);
                 pk[1][jj] = __byte_perm(__byte_perm(qhi[4 * jj], qhi[4 * jj + 1], 0x0040), __byte_perm(qhi[4 * jj + 2], qhi[4 * jj + 3], 0x0040), 0x5410);
             }
-            sx = __fdiv_rn(amax, 127.0f);
+            sx = __fdiv_rn(amax, FP8 ? 448.0f : 127.0f);
         }
         // lane l (bit 3 clear) and lane l + 8 hold bytes {0, 2} and {1, 3} of every word: the low lane assembles chunk 0, the
         // high lane chunk 1
@@ -516,28 +521,28 @@ k_act_blob256(const void* X, int dtype, int64_t B, int64_t n_kt, int64_t ldx, co
 }
 
 void launch_act_blob256(const void* x, int dtype, int64_t B, int64_t n_in, int64_t ldx, const int8_t* dsign, int NB,
-                        uint8_t* bblob, cudaStream_t st) {
+                        uint8_t* bblob, cudaStream_t st, int fp8) {
     const int64_t n_kt = n_in / 256, n_bt = (B + NB - 1) / NB, n_pairs = n_bt * NB * ((n_kt + 1) / 2);
     int64_t blocks = (n_pairs + A256_WARPS - 1) / A256_WARPS;
     if (blocks > 148 * A256_CTAS) blocks = 148 * A256_CTAS;
     // n_pairs < 2^32 always: 2^32 pairs of 512 bf16 activations would be 4.4 TB of x
     const bool fast = dtype == HQ_BF16 && ((((uintptr_t)x) | (uintptr_t)(ldx * 2)) & 15) == 0;
-    if (fast)
-        launch_pdl(k_act_blob256<true>, dim3((unsigned)blocks), dim3(A256_WARPS * 32), A256_WARPS * A256_WFLOATS * sizeof(float), st, x,
-                   dtype, B, n_kt, ldx, dsign, NB, bblob);
-    else
-        launch_pdl(k_act_blob256<false>, dim3((unsigned)blocks), dim3(A256_WARPS * 32), A256_WARPS * A256_WFLOATS * sizeof(float), st, x,
-                   dtype, B, n_kt, ldx, dsign, NB, bblob);
+#define HQ_A256(FAST_, FP8_)                                                                                                     \
+    launch_pdl(k_act_blob256<FAST_, FP8_>, dim3((unsigned)blocks), dim3(A256_WARPS * 32), A256_WARPS * A256_WFLOATS * sizeof(float), \
+               st, x, dtype, B, n_kt, ldx, dsign, NB, bblob)
+    if (fast) { if (fp8) HQ_A256(true, true); else HQ_A256(true, false); }
+    else { if (fp8) HQ_A256(false, true); else HQ_A256(false, false); }
+#undef HQ_A256
 }
 
 void launch_act_blob(const void* x, int dtype, int64_t B, int64_t n_in, int64_t ldx, const int8_t* dsign, int NB,
-                     uint8_t* bblob, cudaStream_t st) {
+                     uint8_t* bblob, cudaStream_t st, int fp8) {
     int64_t n_kt = n_in / 128, n_bt = (B + NB - 1) / NB, n_tiles = n_bt * NB * n_kt;
     int64_t blocks = (n_tiles + QW_WARPS - 1) / QW_WARPS;
     if (blocks > 148 * 16) blocks = 148 * 16;
     // n_tiles < 2^32 always: 2^32 tiles of 128 bf16 activations would be 1.1 TB of x
     launch_pdl(k_act_blob, dim3((unsigned)blocks), dim3(QW_WARPS * 32), QW_WARPS * 128 * sizeof(float), st, x, dtype, B, n_kt, ldx,
-               dsign, NB, bblob);
+               dsign, NB, bblob, fp8);
 }
 
 void launch_act_quant(const void* x, int dtype, int64_t B, int64_t n_in, int64_t ldx, int lattice, int n,

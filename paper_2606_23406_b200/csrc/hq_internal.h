@@ -121,10 +121,10 @@ void launch_act_quant(const void* x, int dtype, int64_t B, int64_t n_in, int64_t
                       const int8_t* dsign, int8_t* q, float* s_x, float* u, cudaStream_t st);
 // activations as the E8 fused kernel's B operand tiles (UMMA layout, permuted K, + scales); n_tile = 128
 void launch_act_blob(const void* x, int dtype, int64_t B, int64_t n_in, int64_t ldx, const int8_t* dsign, int NB,
-                     uint8_t* bblob, cudaStream_t st);
+                     uint8_t* bblob, cudaStream_t st, int fp8 = 0);
 // the same for RHT tiles of 256: two operand chunks of 128 K-bytes per tile (large-M path at n_tile = 256)
 void launch_act_blob256(const void* x, int dtype, int64_t B, int64_t n_in, int64_t ldx, const int8_t* dsign, int NB,
-                        uint8_t* bblob, cudaStream_t st);
+                        uint8_t* bblob, cudaStream_t st, int fp8 = 0);
 // ulen_tmp[sg*32 + i] for all sub-groups (0 for absent rows); err_flag[0] set if a tile exceeds 8160 bits,
 // err_flag[4] = max over present rows of 65535 - ulen, err_flag[5] = max over present rows of ulen
 void launch_tile_ulen(const int8_t* codes, int64_t m, int64_t n_in, int lattice, int n, int k0, int k1,
@@ -158,6 +158,8 @@ hq_status launch_linear_group(hq_ctx* ctx, const hq_weight* const* ws, int n_w, 
                               int64_t ldx, void* const* ys_bf16, const int64_t* ldys, float* const* ys_f32,
                               int32_t* acc_i32, uint8_t* wsbuf, cudaStream_t st, const hq_fold* fold = nullptr);
 bool linear_uses_e8_fast(const hq_weight* w);
+hq_status launch_linear_fp8(hq_ctx* ctx, const hq_weight* w, const void* x, int dtype, int64_t B, int64_t ldx, void* y_bf16,
+                            int64_t ldy, float* y_f32, uint8_t* wsbuf, cudaStream_t st);
 hq_status launch_decode_ceiling(hq_ctx* ctx, const hq_weight* w, int reps, cudaStream_t st, double* scalars_per_s);
 // hq_linear_static: the address of the static scratch array (once per device, that device current), and the launch
 hq_status linear_static_setup(hq_ctx* ctx);

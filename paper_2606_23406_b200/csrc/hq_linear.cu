@@ -391,7 +391,7 @@ size_t linear_workspace_bytes(const hq_ctx* ctx, const hq_weight* w, int64_t B) 
 // scratch copy and one warp-specialised GEMM.  The scratch copy is reused by the weights of a group (stream order).
 static hq_status launch_large(hq_ctx* ctx, const hq_weight* const* ws, int n_w, const void* x, int dtype, int64_t B,
                               int64_t ldx, void* const* ys_bf16, const int64_t* ldys, float* const* ys_f32, int32_t* acc_i32,
-                              uint8_t* wsbuf, cudaStream_t st) {
+                              uint8_t* wsbuf, cudaStream_t st, int fp8 = 0) {
     const hq_weight* w0 = ws[0];
     const int64_t n_bt = (B + LG_NB - 1) / LG_NB;
     const int nch = w0->n / 128;                       // operand chunks of 128 K-bytes per RHT tile (tile 128 or 256)
@@ -401,8 +401,8 @@ static hq_status launch_large(hq_ctx* ctx, const hq_weight* const* ws, int n_w, 
     // fork: the first weight's decode does not depend on x, it runs on the side stream beside the activation cast
     HQ_CUDA_CHECK(ctx, cudaEventRecord(ctx->ev_fork, st));
     HQ_CUDA_CHECK(ctx, cudaStreamWaitEvent(ctx->side, ctx->ev_fork, 0));
-    if (nch == 1) launch_act_blob(x, dtype, B, w0->n_in, ldx, w0->dsign, LG_NB, bblob, st);
-    else launch_act_blob256(x, dtype, B, w0->n_in, ldx, w0->dsign, LG_NB, bblob, st);
+    if (nch == 1) launch_act_blob(x, dtype, B, w0->n_in, ldx, w0->dsign, LG_NB, bblob, st, fp8);
+    else launch_act_blob256(x, dtype, B, w0->n_in, ldx, w0->dsign, LG_NB, bblob, st, fp8);
     HQ_CUDA_CHECK(ctx, cudaGetLastError());
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     if (ctx->prof) {
@@ -421,18 +421,19 @@ static hq_status launch_large(hq_ctx* ctx, const hq_weight* const* ws, int n_w, 
         const int64_t dpairs = ((int64_t)w->n_rb * d.n_kt + 1) / 2, dmax = (int64_t)ctx->sm_count * 3;   // 3 CTAs of 256 threads per SM
         dim3 dgrid((unsigned)(dpairs < dmax ? dpairs : dmax));
         cudaStream_t dst = i == 0 ? ctx->side : st;   // later weights reuse the scratch copy: stream order after the GEMM
+#define HQ_LD1(KK, TT, F8)                                                                                                 \
+    do {                                                                                                                   \
+        HQ_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_e8_decode_ablob<KK, TT, F8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dsmem)); \
+        k_e8_decode_ablob<KK, TT, F8><<<dgrid, 256, dsmem, dst>>>(d);                                                      \
+    } while (0)
 #define HQ_LD(KK)                                                                                                          \
     case KK:                                                                                                               \
-        if (nch == 1) {                                                                                                    \
-            HQ_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_e8_decode_ablob<KK, 128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dsmem)); \
-            k_e8_decode_ablob<KK, 128><<<dgrid, 256, dsmem, dst>>>(d);                                                     \
-        } else {                                                                                                           \
-            HQ_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_e8_decode_ablob<KK, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dsmem)); \
-            k_e8_decode_ablob<KK, 256><<<dgrid, 256, dsmem, dst>>>(d);                                                     \
-        }                                                                                                                  \
+        if (nch == 1) { if (fp8) HQ_LD1(KK, 128, true); else HQ_LD1(KK, 128, false); }                                     \
+        else { if (fp8) HQ_LD1(KK, 256, true); else HQ_LD1(KK, 256, false); }                                              \
         break
         switch (w->k0) { HQ_LD(0); HQ_LD(1); HQ_LD(2); HQ_LD(3); }
 #undef HQ_LD
+#undef HQ_LD1
         HQ_CUDA_CHECK(ctx, cudaGetLastError());
         if (i == 0) {   // join
             HQ_CUDA_CHECK(ctx, cudaEventRecord(ctx->ev_join, ctx->side));
@@ -444,13 +445,14 @@ static hq_status launch_large(hq_ctx* ctx, const hq_weight* const* ws, int n_w, 
         g.acc_i32 = (n_w == 1) ? acc_i32 : nullptr;
         const int64_t tiles = (int64_t)g.n_rb * g.n_bt;
         const unsigned grid = (unsigned)(tiles < ctx->sm_count ? tiles : ctx->sm_count);
-        if (nch == 1) {
-            HQ_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_e8_gemm_large<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LG_SMEM));
-            k_e8_gemm_large<1><<<grid, 384, LG_SMEM, st>>>(g);
-        } else {
-            HQ_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_e8_gemm_large<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LG_SMEM));
-            k_e8_gemm_large<2><<<grid, 384, LG_SMEM, st>>>(g);
-        }
+#define HQ_LGEMM(NCH_, F8)                                                                                                 \
+    do {                                                                                                                   \
+        HQ_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_e8_gemm_large<NCH_, F8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LG_SMEM)); \
+        k_e8_gemm_large<NCH_, F8><<<grid, 384, LG_SMEM, st>>>(g);                                                          \
+    } while (0)
+        if (nch == 1) { if (fp8) HQ_LGEMM(1, true); else HQ_LGEMM(1, false); }
+        else { if (fp8) HQ_LGEMM(2, true); else HQ_LGEMM(2, false); }
+#undef HQ_LGEMM
         HQ_CUDA_CHECK(ctx, cudaGetLastError());
     }
     if (ctx->prof) {
@@ -459,6 +461,12 @@ static hq_status launch_large(hq_ctx* ctx, const hq_weight* const* ws, int n_w, 
         ctx->prof_ev.push_back(e1);
     }
     return HQ_OK;
+}
+
+// hq_linear_cast with HQ_CAST_FP8_E4M3 (§4.8): the large-M pipeline with E4M3 operands and an fp32 accumulator
+hq_status launch_linear_fp8(hq_ctx* ctx, const hq_weight* w, const void* x, int dtype, int64_t B, int64_t ldx, void* y_bf16,
+                            int64_t ldy, float* y_f32, uint8_t* wsbuf, cudaStream_t st) {
+    return launch_large(ctx, &w, 1, x, dtype, B, ldx, &y_bf16, &ldy, &y_f32, nullptr, wsbuf, st, 1);
 }
 
 // one activation cast, ONE fused decode + MMA launch over the stacked row blocks of all weights, one finalize each

@@ -43,7 +43,8 @@ struct E8AblobParams {
 
 // TILE = RHT tile of the weight (128 or 256).  A tile of 256 is written as two operand chunks of 128 K-bytes (K index
 // inside the tile: 32c + 4i + b for block 4c + b, coordinate i; chunk = c / 4), each followed by the same 128 row scales.
-template <int K, int TILE>
+// FP8: the decoded integer coordinates are written as E4M3 bytes (FORMAT R12; §4.8) for the f8f6f4 GEMM.
+template <int K, int TILE, bool FP8 = false>
 __global__ void __launch_bounds__(256) k_e8_decode_ablob(E8AblobParams p) {   // two tiles per CTA pass: warps 0-3 and 4-7
     extern __shared__ __align__(16) uint8_t smem_raw[];
     constexpr int KW = K * TILE / 32;              // R words per row
@@ -114,6 +115,10 @@ __global__ void __launch_bounds__(256) k_e8_decode_ablob(E8AblobParams p) {   //
 #pragma unroll
                 for (int i = 0; i < 8; ++i) C[i] = 0u;
             }
+            if (FP8) {
+#pragma unroll
+                for (int i = 0; i < 8; ++i) C[i] = s8x4_to_e4m3x4(C[i]);
+            }
             uint8_t* rowp = tile + (c >> 2) * LG_ABLOB + (t >> 3) * 1024 + (t & 7) * 128;
             *(uint4*)(rowp + (((2 * (c & 3)) ^ (t & 7)) << 4)) = make_uint4(C[0], C[1], C[2], C[3]);
             *(uint4*)(rowp + (((2 * (c & 3) + 1) ^ (t & 7)) << 4)) = make_uint4(C[4], C[5], C[6], C[7]);
@@ -127,7 +132,8 @@ __global__ void __launch_bounds__(256) k_e8_decode_ablob(E8AblobParams p) {   //
                 for (int e = 0; e < 8; ++e) {
                     const int col = e8_kcol(8 * (bk & 15) + e);
                     uint8_t* rowp = tile + (bk >> 4) * LG_ABLOB + (t >> 3) * 1024 + (t & 7) * 128;
-                    rowp[(((col >> 4) ^ (t & 7)) << 4) | (col & 15)] = (uint8_t)(int8_t)c[e];
+                    rowp[(((col >> 4) ^ (t & 7)) << 4) | (col & 15)] =
+                        FP8 ? (uint8_t)(s8x4_to_e4m3x4((uint32_t)(uint8_t)(int8_t)c[e]) & 0xffu) : (uint8_t)(int8_t)c[e];
                 }
             });
         }
@@ -171,7 +177,8 @@ struct E8LargeParams {
 // NCH = operand chunks (TMA stages of 128 K-bytes) per RHT tile: 1 (tile 128) or 2 (tile 256).  The INT32 accumulator runs
 // over the NCH chunks of a tile and is drained once per TILE: at tile 256 the rescale costs half as many issue slots per
 // MAC (the tile is chosen on kernel grounds).  p.n_kt counts chunks.
-template <int NCH>
+// FP8: both operands hold E4M3 bytes, the MMA is kind::f8f6f4 with an fp32 accumulator (no int -> float in the drain).
+template <int NCH, bool FP8 = false>
 __global__ void __launch_bounds__(384, 1) k_e8_gemm_large(E8LargeParams p) {
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
@@ -225,7 +232,7 @@ __global__ void __launch_bounds__(384, 1) k_e8_gemm_large(E8LargeParams p) {
                 }
             }
         } else if (tid == 32) {   // ---- MMA issuer
-            const uint32_t idesc = make_idesc_i8(128, LG_NB);
+            const uint32_t idesc = FP8 ? make_idesc_e4m3(128, LG_NB) : make_idesc_i8(128, LG_NB);
             uint32_t it = 0;
             for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
                 for (int kt = 0; kt < p.n_kt; ++kt, ++it) {
@@ -236,8 +243,10 @@ __global__ void __launch_bounds__(384, 1) k_e8_gemm_large(E8LargeParams p) {
                     tc_fence_after();
                     const uint32_t sb = smem_a + s * LG_STAGE, sa = sb + LG_NB * 128u;
 #pragma unroll
-                    for (int ks = 0; ks < 4; ++ks)
-                        mma_i8(tmem + a * LG_NB, make_desc_sw128(sa + ks * 32), make_desc_sw128(sb + ks * 32), idesc, (ks > 0 || ch > 0));
+                    for (int ks = 0; ks < 4; ++ks) {
+                        if (FP8) mma_e4m3(tmem + a * LG_NB, make_desc_sw128(sa + ks * 32), make_desc_sw128(sb + ks * 32), idesc, (ks > 0 || ch > 0));
+                        else mma_i8(tmem + a * LG_NB, make_desc_sw128(sa + ks * 32), make_desc_sw128(sb + ks * 32), idesc, (ks > 0 || ch > 0));
+                    }
                     mma_commit(&empty[s]);
                     if (ch == NCH - 1) mma_commit(&acc_full[a]);
                 }
@@ -302,8 +311,8 @@ __global__ void __launch_bounds__(384, 1) k_e8_gemm_large(E8LargeParams p) {
 #pragma unroll
                     for (int e = 0; e < 8; ++e) {
                         const uint4 s4 = lds128(sx_a + (c0 + 4 * e) * 4);
-                        const uint64_t f01 = pack_f32x2((float)(int)vc[4 * e + 0], (float)(int)vc[4 * e + 1]);
-                        const uint64_t f23 = pack_f32x2((float)(int)vc[4 * e + 2], (float)(int)vc[4 * e + 3]);
+                        const uint64_t f01 = FP8 ? pack_u32x2(vc[4 * e + 0], vc[4 * e + 1]) : pack_f32x2((float)(int)vc[4 * e + 0], (float)(int)vc[4 * e + 1]);
+                        const uint64_t f23 = FP8 ? pack_u32x2(vc[4 * e + 2], vc[4 * e + 3]) : pack_f32x2((float)(int)vc[4 * e + 2], (float)(int)vc[4 * e + 3]);
                         yacc[(c0 >> 1) + 2 * e + 0] = fma_f32x2(mul_f32x2(f01, sw2), pack_u32x2(s4.x, s4.y), yacc[(c0 >> 1) + 2 * e + 0]);
                         yacc[(c0 >> 1) + 2 * e + 1] = fma_f32x2(mul_f32x2(f23, sw2), pack_u32x2(s4.z, s4.w), yacc[(c0 >> 1) + 2 * e + 1]);
                     }

@@ -163,6 +163,35 @@ __host__ __device__ constexpr uint32_t make_idesc_i8(int M, int N) {
     return (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
 }
 
+// kind::f8f6f4 with both operands E4M3 (format code 0), FP32 accumulator (c format 1), K-major, M x N (§4.8: the FP8 cast)
+__host__ __device__ constexpr uint32_t make_idesc_e4m3(int M, int N) {
+    return (1u << 4) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
+}
+__device__ __forceinline__ void mma_e4m3(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f8f6f4 [%0], %1, %2, %3, p;\n\t}"
+        ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+// four INT8 lattice coordinates (one word) -> four E4M3 bytes, round to nearest even (FORMAT R12): c + 128 as an unsigned
+// byte under the exponent of 1024 is the f16 number 1152 + c exactly; minus 1152; f16x2 -> e4m3x2.
+__device__ __forceinline__ uint32_t s8x4_to_e4m3x4(uint32_t c) {
+    const uint32_t v = c ^ 0x80808080u;
+    uint32_t lo = __byte_perm(v, 0x64646464u, 0x4140), hi = __byte_perm(v, 0x64646464u, 0x4342);
+    uint16_t r0, r1;
+    asm("{\n\t.reg .b32 t;\n\tsub.rn.f16x2 t, %1, %2;\n\tcvt.rn.satfinite.e4m3x2.f16x2 %0, t;\n\t}" : "=h"(r0) : "r"(lo), "r"(0x64806480u));
+    asm("{\n\t.reg .b32 t;\n\tsub.rn.f16x2 t, %1, %2;\n\tcvt.rn.satfinite.e4m3x2.f16x2 %0, t;\n\t}" : "=h"(r1) : "r"(hi), "r"(0x64806480u));
+    return (uint32_t)r0 | ((uint32_t)r1 << 16);
+}
+// two fp32 -> E4M3 bytes: the result's LOW byte is e4m3(lo), the next byte e4m3(hi)
+__device__ __forceinline__ uint32_t f32x2_to_e4m3x2(float lo, float hi) {
+    uint16_t r;
+    asm("cvt.rn.satfinite.e4m3x2.f32 %0, %1, %2;" : "=h"(r) : "f"(hi), "f"(lo));
+    return (uint32_t)r;
+}
+
 // byte offset of (row r, K-byte c) inside a K-major SWIZZLE_128B operand of `rows` rows:
 // 128-byte-wide atoms side by side along K, each rows*128 bytes.
 __device__ __forceinline__ uint32_t sw128_offset(int rows, int r, int c) {
