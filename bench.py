@@ -229,7 +229,7 @@ def measure_attend(ctx, hq, dev, peak_gbs):
     return res
 
 
-def measure_layer_step(ctx, hq, dev, layers, peak_gbs, context=32768, steps=12):
+def measure_layer_step(ctx, hq, dev, layers, peak_gbs, context=32768, steps=12, short=True):
     """SURVEY §8(f)3 / PAPER.md Table 10's decode shape (L496-511): one token through whole decoder layers
     (hq_layer_decode: RMSNorm and SiLU.mul folded into the linears' prologues, residuals into their epilogues, KV append,
     attend) on the bench's compressed Llama-3.1-8B-shaped layers, each with its own 2-bps KV cache at `context` tokens.
@@ -243,7 +243,8 @@ def measure_layer_step(ctx, hq, dev, layers, peak_gbs, context=32768, steps=12):
     g = torch.ones((hidden,), dtype=torch.bfloat16, device=dev)
     objs, kv_bytes = [], 0.0
     for l, ws in enumerate(layers):
-        kv = ctx.kv_create(H, d, context + 256, hq.Lattice.E8, snr_kv, (0, 0), 4 + l, rotation=1, dither=1, window=32)
+        kv = ctx.kv_create(H, d, context + 256, hq.Lattice.E8, snr_kv, (0, 0), 4 + l, rotation=1, dither=1, window=32,
+                           device_position=True)
         kv.append(K, V)
         ex = kv.export()
         Tn = int(ex["n_tokens"])
@@ -270,15 +271,44 @@ def measure_layer_step(ctx, hq, dev, layers, peak_gbs, context=32768, steps=12):
     torch.cuda.synchronize()
     us = 1e3 * e0.elapsed_time(e1) / (steps * len(objs))
     ok = bool(torch.isfinite(h_out.float()).all())
+    # the same token step as ONE CUDA graph per layer: the caches keep their position on the device, every replay is the
+    # next token (tests/test_gpu_graph.py: bit-identical to the eager calls)
+    st = torch.cuda.Stream()
+    graphs = []
+    with torch.cuda.stream(st):
+        for layer, _ in objs:
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=st):
+                layer.decode(h, h_out)
+            graphs.append(g)
+        for _ in range(2):
+            for g in graphs:
+                g.replay()
+        st.synchronize()
+        g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        g0.record(st)
+        for _ in range(steps):
+            for g in graphs:
+                g.replay()
+        g1.record(st)
+        st.synchronize()
+    us_graph = 1e3 * g0.elapsed_time(g1) / (steps * len(objs))
+    ok = ok and bool(torch.isfinite(h_out.float()).all()) and objs[0][1].sync_position() == context + 3 + steps + 2 + steps
     alg = w_bytes + kv_bytes
     gbs = alg / (us * 1e-6) / 1e9
     for layer, kv in objs:
         kv.free()
+    short_ctx = None
+    if short:   # the launch-bound end of the same call: 1024 tokens of context
+        r = measure_layer_step(ctx, hq, dev, layers, peak_gbs, context=1024, steps=steps, short=False)
+        short_ctx = {"context_tokens": 1024, "us_per_layer_step": r["us_per_layer_step"],
+                     "us_per_layer_step_graph": r["us_per_layer_step_graph"], "finite": r["finite"]}
     return {"bound": "hbm", "unit": "GB/s", "achieved": gbs, "peak": peak_gbs, "frac": gbs / peak_gbs,
-            "us_per_layer_step": us, "tokens_per_s_at_32_layers": 1e6 / (32.0 * us), "context_tokens": context,
+            "us_per_layer_step": us, "us_per_layer_step_graph": us_graph, "tokens_per_s_at_32_layers": 1e6 / (32.0 * min(us, us_graph)),
+            "context_tokens": context,
             "launches_per_layer": 7, "alg_bytes_per_layer_step": alg, "weight_bytes": w_bytes, "kv_bytes": kv_bytes,
-            "finite": ok, "bf16_bytes_per_layer_step": 2.0 * 218103808 + 2.0 * 2 * H * d * context,
-            "call": "hq_layer_decode (eager): q+k+v [RMSNorm fold] -> hq_kv_append -> hq_attend (split + combine) -> o [+ residual] -> gate+up [RMSNorm fold] -> down [SiLU.mul fold, + residual]",
+            "finite": ok, "short_context": short_ctx, "bf16_bytes_per_layer_step": 2.0 * 218103808 + 2.0 * 2 * H * d * context,
+            "call": "hq_layer_decode (eager, and as one CUDA graph per layer on device_position caches): q+k+v [RMSNorm fold] -> hq_kv_append -> hq_attend (split + combine) -> o [+ residual] -> gate+up [RMSNorm fold] -> down [SiLU.mul fold, + residual]",
             "workload": "Llama-3.1-8B-shaped decoder layer, E8 4 bps weights, E8 2 bps KV cache (signs rotation, dither, window 32), batch 1"}
 
 

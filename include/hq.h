@@ -276,8 +276,10 @@ hq_status hq_linear_group_fold(hq_ctx* ctx, const hq_weight* const* ws, int32_t 
  *   h_out = h2 + W_down (silu(gate) * up)      hq_linear_group_fold, SiLU.mul prologue + residual   (1 launch)
  * Rotary position embedding is not part of the paper's method and is not applied (the weights are synthetic).
  * h_in, h_out [hidden] bf16 dev (may alias).  scratch_dev: hq_layer_scratch_bytes() bytes, 256-byte aligned, holds q, k, v,
- * a, h2, gate, up (bf16); hq_layer_scratch_view returns their offsets for parity tests.  The token position is host state
- * of the cache (hq_kv_append): a captured CUDA graph of this call replays the SAME position.
+ * a, h2, gate, up (bf16); hq_layer_scratch_view returns their offsets for parity tests.  With a cache created with
+ * hq_kv_config.device_position = 1 the call can be captured into ONE CUDA graph after one eager warm-up call (which sizes
+ * the library's workspaces) and every replay is the next token; with a host-position cache a captured graph replays the
+ * SAME position.
  * Shapes: wq [q_heads d, hidden], wk / wv [kv_heads d, hidden], wo [hidden, q_heads d], wgate / wup [ffn, hidden],
  * wdown [hidden, ffn]; d = the cache's head_dim.  Mismatch -> HQ_ERR_SHAPE.
  */
@@ -316,6 +318,14 @@ typedef struct {
                                    codes are reproducible bit for bit); hq_attend rotates the query by S and un-rotates the code-domain sum by S^T, one
                                    head_dim x head_dim matvec per QUERY head instead of the paper's O(T D^2) per layer (L502).
                                    Must be NULL for the other rotations. */
+    int32_t device_position;    /* 1: the number of held tokens lives in DEVICE memory.  A single-token hq_kv_append reads
+                                   its token index there and advances it, hq_attend reads the context length there and is
+                                   launched over a split count fixed by max_tokens - so a CUDA graph that captured
+                                   hq_kv_append(1 token) / hq_attend / hq_layer_decode stays correct on every replay (each
+                                   replay is the next token).  A replayed append past max_tokens writes nothing and turns the
+                                   cache sticky HQ_ERR_FORMAT.  The host's own count is refreshed from the device (one
+                                   blocking 4-byte copy) by multi-token hq_kv_append, hq_kv_export, hq_kv_decode_int8 and
+                                   hq_kv_sync_position.  0: the count is host state (a captured graph replays one position). */
 } hq_kv_config;
 
 hq_status hq_kv_create(hq_ctx* ctx, const hq_kv_config* cfg, hq_kv** out);
@@ -325,6 +335,10 @@ void hq_kv_free(hq_ctx* ctx, hq_kv* kv);
  * rotate -> normalize -> dither -> nearest point -> strip -> Rice) into the FORMAT §6 container and
  * writes the bf16 ring.  Token indices continue from the tokens already held. */
 hq_status hq_kv_append(hq_ctx* ctx, hq_kv* kv, const void* k_dev, const void* v_dev, int64_t n_tok, void* stream);
+
+/* device_position caches only: wait for the stream work issued so far and read the held-token count back (returned in
+ * *n_tokens_out, may be NULL).  A no-op that returns the host count for other caches. */
+hq_status hq_kv_sync_position(hq_ctx* ctx, hq_kv* kv, int64_t* n_tokens_out);
 
 /* One decode step of attention (L178) for q [q_heads, head_dim] bf16 dev over all held tokens:
  * tokens [0, T-window) from the bitstream (decoded in the code domain), [T-window, T) from the ring.

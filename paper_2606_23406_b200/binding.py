@@ -33,7 +33,7 @@ class _CodecConfig(C.Structure):
 class _KVConfig(C.Structure):
     _fields_ = [("kv_heads", C.c_int32), ("head_dim", C.c_int32), ("max_tokens", C.c_int64), ("codec", _CodecConfig),
                 ("rotation", C.c_int32), ("dither", C.c_int32), ("window", C.c_int32), ("una_capacity_bits", C.c_int64),
-                ("qjl_dev", C.c_void_p)]
+                ("qjl_dev", C.c_void_p), ("device_position", C.c_int32)]
 
 
 class _WeightInfo(C.Structure):
@@ -92,7 +92,7 @@ _lib = None
 EXPORTS = ["hq_create", "hq_destroy", "hq_last_error", "hq_measure_decode_ceiling", "hq_alpha", "hq_snr_for_bps", "hq_profile_enable", "hq_profile_read",
            "hq_encode_weights", "hq_weight_free", "hq_weight_get_info", "hq_weight_stats", "hq_weight_export",
            "hq_weight_export_host", "hq_weight_import", "hq_decode_int8", "hq_act_quant", "hq_linear",
-           "hq_linear_cast", "hq_linear_group", "hq_linear_group_fold", "hq_layer_scratch_view", "hq_layer_decode", "hq_linear_static", "hq_linear_workspace_bytes", "hq_kv_create", "hq_kv_free", "hq_kv_append", "hq_attend", "hq_kv_export",
+           "hq_linear_cast", "hq_linear_group", "hq_linear_group_fold", "hq_layer_scratch_view", "hq_layer_decode", "hq_linear_static", "hq_linear_workspace_bytes", "hq_kv_create", "hq_kv_free", "hq_kv_append", "hq_kv_sync_position", "hq_attend", "hq_kv_export",
            "hq_kv_decode_int8"]
 
 
@@ -134,6 +134,7 @@ def load_library():
     lib.hq_kv_create.argtypes = [vp, C.POINTER(_KVConfig), C.POINTER(vp)]
     lib.hq_kv_free.argtypes = [vp, vp]; lib.hq_kv_free.restype = None
     lib.hq_kv_append.argtypes = [vp, vp, vp, vp, i64, vp]
+    lib.hq_kv_sync_position.argtypes = [vp, vp, C.POINTER(i64)]
     lib.hq_attend.argtypes = [vp, vp, vp, i32, vp, vp, vp]
     lib.hq_kv_export.argtypes = [vp, vp, C.POINTER(_KVView)]
     lib.hq_kv_decode_int8.argtypes = [vp, vp, i32, i64, i64, vp, vp]
@@ -269,13 +270,13 @@ class Context:
 
     # ---- KV ----
     def kv_create(self, kv_heads, head_dim, max_tokens, lattice, snr_db, rice_k, seed, rotation=1, dither=1,
-                  window=32, una_capacity_bits=0, qjl: torch.Tensor = None):
+                  window=32, una_capacity_bits=0, qjl: torch.Tensor = None, device_position=False):
         """rotation 2 (qjl): `qjl` = the Haar matrix S [head_dim, head_dim] fp32 on the device (copied by the library)."""
         codec = _CodecConfig(lattice, head_dim, float(snr_db), (C.c_int32 * 2)(int(rice_k[0]), int(rice_k[1])), seed)
         if qjl is not None:
             assert qjl.is_cuda and qjl.dtype == torch.float32 and qjl.is_contiguous() and tuple(qjl.shape) == (head_dim, head_dim)
         cfg = _KVConfig(kv_heads, head_dim, max_tokens, codec, rotation, dither, window, int(una_capacity_bits),
-                        qjl.data_ptr() if qjl is not None else None)
+                        qjl.data_ptr() if qjl is not None else None, 1 if device_position else 0)
         h = C.c_void_p()
         self.check(self.lib.hq_kv_create(self.h, C.byref(cfg), C.byref(h)))
         return KVCache(self, h, kv_heads, head_dim, max_tokens)
@@ -428,6 +429,12 @@ class KVCache:
         assert tuple(k.shape[1:]) == (self.kv_heads, self.head_dim)
         self.ctx.check(self.ctx.lib.hq_kv_append(self.ctx.h, self.h, k.data_ptr(), v.data_ptr(), k.shape[0],
                                                  _stream_ptr(self.ctx.device)))
+
+    def sync_position(self) -> int:
+        """hq_kv_sync_position: the held-token count (read back from the device for device_position caches)."""
+        n = C.c_int64(0)
+        self.ctx.check(self.ctx.lib.hq_kv_sync_position(self.ctx.h, self.h, C.byref(n)))
+        return int(n.value)
 
     def attend(self, q: torch.Tensor, out: torch.Tensor = None, want_f32=False):
         dev = self.ctx.device

@@ -40,6 +40,17 @@ hq_status kv_flag_status(hq_ctx* ctx, const hq_kv* kv) {
     const int f = *(volatile int*)kv->flag_host;
     if (f == 1) return fail(ctx, HQ_ERR_FORMAT, "a vector's U-section exceeds 65534 bits (FORMAT §4); the cache is unusable");
     if (f == 2) return fail(ctx, HQ_ERR_FORMAT, "U-stream capacity exceeded (hq_kv_config.una_capacity_bits); the cache is unusable");
+    if (f == 3) return fail(ctx, HQ_ERR_FORMAT, "a replayed append ran past max_tokens (device_position cache); the cache is unusable");
+    return HQ_OK;
+}
+
+// device_position caches: the host's token count follows the device's (blocking)
+static hq_status kv_refresh_position(hq_ctx* ctx, hq_kv* kv) {
+    if (!kv->pos_dev) return HQ_OK;
+    uint32_t t = 0;
+    HQ_CUDA_CHECK(ctx, cudaDeviceSynchronize());
+    HQ_CUDA_CHECK(ctx, cudaMemcpy(&t, kv->pos_dev, 4, cudaMemcpyDeviceToHost));
+    kv->n_tokens = (int64_t)t;
     return HQ_OK;
 }
 
@@ -674,6 +685,11 @@ hq_status hq_kv_create(hq_ctx* ctx, const hq_kv_config* cfg, hq_kv** out) {
         if (!kv->qjl) { hq_kv_free(ctx, kv); return HQ_ERR_ALLOC; }
     }
     kv->cfg.qjl_dev = nullptr;   // the cache keeps its own copy
+    if (cfg->device_position) {
+        kv->pos_dev = (uint32_t*)ctx_alloc(ctx, 256);
+        if (!kv->pos_dev) { hq_kv_free(ctx, kv); return HQ_ERR_ALLOC; }
+        cudaMemset(kv->pos_dev, 0, 256);
+    }
     kv->att_ws_bytes = attend_workspace_bytes(ctx, kv);
     kv->att_ws = (float*)ctx_alloc(ctx, kv->att_ws_bytes);
     if (cudaHostAlloc((void**)&kv->flag_host, 64, cudaHostAllocMapped) != cudaSuccess ||
@@ -715,7 +731,7 @@ void hq_kv_free(hq_ctx* ctx, hq_kv* kv) {
     if (!ctx) ctx = kv->ctx;
     ctx_free(ctx, kv->rem); ctx_free(ctx, kv->una); ctx_free(ctx, kv->ulen); ctx_free(ctx, kv->norm);
     ctx_free(ctx, kv->blk_off); ctx_free(ctx, kv->upos); ctx_free(ctx, kv->ring); ctx_free(ctx, kv->dsign);
-    ctx_free(ctx, kv->ssign); ctx_free(ctx, kv->qjl); ctx_free(ctx, kv->counters); ctx_free(ctx, kv->scratch_codes); ctx_free(ctx, kv->att_ws);
+    ctx_free(ctx, kv->ssign); ctx_free(ctx, kv->qjl); ctx_free(ctx, kv->pos_dev); ctx_free(ctx, kv->counters); ctx_free(ctx, kv->scratch_codes); ctx_free(ctx, kv->att_ws);
     if (kv->flag_host) { cudaDeviceSynchronize(); cudaFreeHost(kv->flag_host); }
     delete kv;
 }
@@ -724,6 +740,10 @@ hq_status hq_kv_append(hq_ctx* ctx, hq_kv* kv, const void* k_dev, const void* v_
     if (!ctx) return HQ_ERR_INVALID_ARG;
     if (!kv || !k_dev || !v_dev) return fail(ctx, HQ_ERR_INVALID_ARG, "null argument");
     if (kv->ctx != ctx) return fail(ctx, HQ_ERR_INVALID_ARG, "the cache belongs to another context");
+    if (kv->pos_dev && n_tok > 1) {   // replays may have advanced the device's count past the host's
+        HQ_ENTER(ctx);
+        if (hq_status rs = kv_refresh_position(ctx, kv)) return rs;
+    }
     if (n_tok <= 0 || kv->n_tokens + n_tok > kv->cfg.max_tokens) return fail(ctx, HQ_ERR_SHAPE, "n_tok out of range");
     if (hq_status fs = kv_flag_status(ctx, kv)) return fs;
     HQ_ENTER(ctx);
@@ -763,6 +783,10 @@ hq_status hq_kv_append(hq_ctx* ctx, hq_kv* kv, const void* k_dev, const void* v_
     launch_kv_ring(k_dev, v_dev, n_tok, H, d, kv->n_tokens, kv->cfg.window, kv->ring, st);
     HQ_CUDA_CHECK(ctx, cudaGetLastError());
     kv->n_tokens += n_tok;
+    if (kv->pos_dev) {
+        launch_set_u32(kv->pos_dev, (uint32_t)kv->n_tokens, st);
+        HQ_CUDA_CHECK(ctx, cudaGetLastError());
+    }
     return HQ_OK;
 }
 
@@ -772,17 +796,28 @@ hq_status hq_attend(hq_ctx* ctx, const hq_kv* kv, const void* q_dev, int32_t q_h
     if (!kv || !q_dev || (!out_bf16_dev && !out_f32_dev_or_null)) return fail(ctx, HQ_ERR_INVALID_ARG, "null argument");
     if (q_heads <= 0 || q_heads % kv->cfg.kv_heads != 0 || q_heads / kv->cfg.kv_heads > 8 || q_heads > 64)
         return fail(ctx, HQ_ERR_SHAPE, "q_heads must be a multiple of kv_heads, group size <= 8, q_heads <= 64");
-    if (kv->n_tokens <= 0) return fail(ctx, HQ_ERR_SHAPE, "empty cache");
+    if (kv->n_tokens <= 0 && !kv->pos_dev) return fail(ctx, HQ_ERR_SHAPE, "empty cache");
     if (kv->ctx != ctx) return fail(ctx, HQ_ERR_INVALID_ARG, "the cache belongs to another context");
     if (hq_status fs = kv_flag_status(ctx, kv)) return fs;
     HQ_ENTER(ctx);
     return launch_attend(ctx, kv, q_dev, q_heads, out_bf16_dev, out_f32_dev_or_null, (cudaStream_t)stream);
 }
 
+hq_status hq_kv_sync_position(hq_ctx* ctx, hq_kv* kv, int64_t* n_tokens_out) {
+    if (!ctx) return HQ_ERR_INVALID_ARG;
+    if (!kv) return fail(ctx, HQ_ERR_INVALID_ARG, "null argument");
+    if (kv->ctx != ctx) return fail(ctx, HQ_ERR_INVALID_ARG, "the cache belongs to another context");
+    HQ_ENTER(ctx);
+    if (hq_status rs = kv_refresh_position(ctx, kv)) return rs;
+    if (n_tokens_out) *n_tokens_out = kv->n_tokens;
+    return kv_flag_status(ctx, kv);
+}
+
 hq_status hq_kv_export(hq_ctx* ctx, const hq_kv* kv, hq_kv_view* out) {
     if (!ctx) return HQ_ERR_INVALID_ARG;
     if (!kv || !out) return fail(ctx, HQ_ERR_INVALID_ARG, "null argument");
     HQ_ENTER(ctx);
+    if (hq_status rs = kv_refresh_position(ctx, const_cast<hq_kv*>(kv))) return rs;
     HQ_CUDA_CHECK(ctx, cudaDeviceSynchronize());
     unsigned long long hc[8];
     HQ_CUDA_CHECK(ctx, cudaMemcpy(hc, kv->counters, sizeof(hc), cudaMemcpyDeviceToHost));
@@ -799,6 +834,10 @@ hq_status hq_kv_decode_int8(hq_ctx* ctx, const hq_kv* kv, int32_t role, int64_t 
                             void* stream) {
     if (!ctx) return HQ_ERR_INVALID_ARG;
     if (!kv || !codes_dev || role < 0 || role > 1) return fail(ctx, HQ_ERR_INVALID_ARG, "bad argument");
+    if (kv->pos_dev) {
+        HQ_ENTER(ctx);
+        if (hq_status rs = kv_refresh_position(ctx, const_cast<hq_kv*>(kv))) return rs;
+    }
     if (t0 < 0 || n <= 0 || t0 + n > kv->n_tokens) return fail(ctx, HQ_ERR_SHAPE, "token range out of bounds");
     if (hq_status fs = kv_flag_status(ctx, kv)) return fs;
     HQ_ENTER(ctx);

@@ -97,7 +97,15 @@ struct AttendParams {
     const int8_t *dsign, *ssign;
     const float *qjl, *qjl_t;   // HQ_ROT_QJL: S row-major and S transposed (null otherwise)
     float* ws;               // [H][n_split][G][d + 2]
+    const uint32_t* pos_dev; // device_position caches: the held-token count is read here, not taken from Tc (graph replay)
+    int window;
 };
+// tokens served from the bitstream
+__device__ __forceinline__ int64_t attend_tc(const AttendParams& p) {
+    if (!p.pos_dev) return p.Tc;
+    const int64_t T = (int64_t)__ldcg(p.pos_dev);
+    return T > p.window ? T - p.window : 0;
+}
 
 // q' = S * RHT(q) for one head, in smem (fp32), by one warp (FORMAT R1 order; any order would do here)
 __device__ inline void warp_query_transform(float* s, int d, const int8_t* dsign, const int8_t* ssign, int rotation,
@@ -253,7 +261,8 @@ k_attend_split(AttendParams p) {
     }
     __syncthreads();
 
-    const int64_t nblk_total = (p.Tc + 127) / 128;
+    const int64_t Tc = attend_tc(p);
+    const int64_t nblk_total = (Tc + 127) / 128;
     const int64_t blk0 = (nblk_total * split) / p.n_split, blk1 = (nblk_total * (split + 1)) / p.n_split;   // balanced
 
     const PhiloxKeys rk = philox_round_keys(p.seed);
@@ -263,7 +272,7 @@ k_attend_split(AttendParams p) {
 
     for (int64_t blk = blk0; blk < blk1; ++blk) {
         const int64_t t = blk * 128 + tid;
-        const bool valid = t < p.Tc;
+        const bool valid = t < Tc;
         float pg[GP];
         for (int role = 0; role < 2; ++role) {
             const uint32_t* rem = p.rem + ((int64_t)role * p.H + h) * p.rem_words;
@@ -410,6 +419,7 @@ __global__ void k_attend_combine(AttendParams p, const __nv_bfloat16* ring, int 
     float* red = ls + p.n_split;  // [d / 32] block reduction
     __shared__ float s_m, s_l;
     const int qh = blockIdx.x, h = qh / G, g = qh % G, j = threadIdx.x;
+    if (p.pos_dev) T = (int64_t)__ldcg(p.pos_dev);
     const float* wbase = p.ws + ((int64_t)h * p.n_split * G + g) * (d + 2);   // split s at + s * G * (d + 2)
     const int64_t wstride = (int64_t)G * (d + 2);
     // global max over splits: thread j takes splits j, j + d, ... (independent loads), then a block reduction
@@ -428,7 +438,7 @@ __global__ void k_attend_combine(AttendParams p, const __nv_bfloat16* ring, int 
     qf[j] = __bfloat162float(p.q[qh * d + j]);
     __syncthreads();
     for (int i = 0; i < d / 32; ++i) m = fmaxf(m, red[i]);
-    const int64_t w0 = p.Tc;
+    const int64_t w0 = attend_tc(p);
     const int nw = (int)(T - w0);
     if (j < nw) {
         int64_t t = w0 + j;
@@ -513,6 +523,7 @@ __global__ void k_attend_combine(AttendParams p, const __nv_bfloat16* ring, int 
 static int attend_n_split(const hq_ctx* ctx, const hq_kv* kv) {
     int64_t window = kv->cfg.window;
     int64_t Tc = kv->n_tokens > window ? kv->n_tokens - window : 0;
+    if (kv->pos_dev) Tc = kv->cfg.max_tokens;   // fixed for the life of the cache: a captured launch stays valid as tokens arrive
     int64_t nblk = (Tc + 127) / 128;
     int64_t want = (ctx->sm_count * 3) / kv->cfg.kv_heads;   // one wave of the 3 resident CTAs per SM
     if (want < 1) want = 1;
@@ -536,6 +547,7 @@ hq_status launch_attend(hq_ctx* ctx, const hq_kv* kv, const void* q, int q_heads
     int64_t window = kv->cfg.window;
     p.Tc = kv->n_tokens > window ? kv->n_tokens - window : 0;
     p.n_split = attend_n_split(ctx, kv);
+    p.pos_dev = kv->pos_dev; p.window = (int)window;
     p.inv_A = (float)(1.0 / (kv->alpha * sqrt((double)d)));
     p.inv_sqrt_d = (float)(1.0 / sqrt((double)d));
     p.seed = kv->cfg.codec.seed;
@@ -554,12 +566,13 @@ hq_status launch_attend(hq_ctx* ctx, const hq_kv* kv, const void* q, int q_heads
         }                                                                                                          \
     } while (0)
     cudaEvent_t e0 = nullptr, e1 = nullptr;
-    if (ctx->prof && p.Tc > 0) {
+    const bool run_split = p.Tc > 0 || kv->pos_dev;   // a device-position cache always launches: the count may have grown
+    if (ctx->prof && run_split) {
         HQ_CUDA_CHECK(ctx, cudaEventCreate(&e0));
         HQ_CUDA_CHECK(ctx, cudaEventCreate(&e1));
         HQ_CUDA_CHECK(ctx, cudaEventRecord(e0, st));
     }
-    if (p.Tc > 0) {
+    if (run_split) {
         switch (kv->cfg.codec.lattice) {
             case LAT_Z: HQ_AT(LAT_Z); break;
             case LAT_A2: HQ_AT(LAT_A2); break;

@@ -120,6 +120,8 @@ __global__ void k_transpose_f32(const float* __restrict__ a, float* __restrict__
     const int i = blockIdx.x, j = threadIdx.x;   // at[j][i] = a[i][j]
     at[(int64_t)j * n + i] = a[(int64_t)i * n + j];
 }
+__global__ void k_set_u32(uint32_t* dst, uint32_t v) { *dst = v; }
+void launch_set_u32(uint32_t* dst, uint32_t v, cudaStream_t st) { k_set_u32<<<1, 1, 0, st>>>(dst, v); }
 void launch_transpose_f32(const float* a, float* at, int n, cudaStream_t st) { k_transpose_f32<<<n, n, 0, st>>>(a, at, n); }
 
 // mode 0: weights (tile = (row, kt));  mode 1: KV (tile = (token, head), rotation, dither)
@@ -1008,6 +1010,8 @@ struct KvAppend1 {
     __nv_bfloat16* ring;
     unsigned long long* counters;   // [0] clamps
     int* flag;                      // mapped host memory: error flag of the cache
+    uint32_t* pos_dev;              // device_position caches: [0] token count (read as this token's index, advanced by the
+                                    // last of the 2 H warps to finish), [1] their arrival counter; null: p.token is used
 };
 
 template <int LAT>
@@ -1015,6 +1019,24 @@ __global__ void __launch_bounds__(32)
 k_kv_append1(KvAppend1 p) {
     extern __shared__ float smf[];   // u[d] | t[d] | codes[d] (int8) | z[d] (u8)
     const int lane = threadIdx.x, h = blockIdx.x, role = blockIdx.y, d = p.d, H = p.H;
+    // every warp reads the position before its own arrival below; the last arrival writes the new one: no warp sees it early
+    const int64_t token = p.pos_dev ? (int64_t)*(volatile const uint32_t*)p.pos_dev : p.token;
+    auto arrive = [&]() {   // the warp's writes are done (or it wrote nothing)
+        __syncwarp();
+        if (p.pos_dev && lane == 0) {
+            __threadfence();
+            const unsigned prev = atomicAdd(p.pos_dev + 1, 1u);
+            if (prev == 2u * (unsigned)H - 1u) {
+                p.pos_dev[1] = 0u;
+                if (token < p.max_tokens) *(volatile uint32_t*)p.pos_dev = (uint32_t)token + 1u;
+            }
+        }
+    };
+    if (token >= p.max_tokens) {   // a replayed graph ran past the capacity: nothing is written, the cache turns sticky
+        if (lane == 0) kv_raise(p.flag, 3);
+        arrive();
+        return;
+    }
     float* u = smf;
     float* t = u + d;
     int8_t* codes = (int8_t*)(t + d);
@@ -1023,7 +1045,7 @@ k_kv_append1(KvAppend1 p) {
     for (int i = lane; i < d; i += 32) {
         const float xv = __bfloat162float(x[i]);
         u[i] = (p.dsign[i] < 0) ? -xv : xv;
-        if (p.window > 0) p.ring[((int64_t)(role * p.window + (p.token % p.window)) * H + h) * d + i] = x[i];
+        if (p.window > 0) p.ring[((int64_t)(role * p.window + (token % p.window)) * H + h) * d + i] = x[i];
     }
     warp_rht_inplace(u, d, lane);
     if (p.rotation == HQ_ROT_SIGNS)
@@ -1038,13 +1060,13 @@ k_kv_append1(KvAppend1 p) {
     const uint16_t hb = f32_to_f16_bits_sat(__fsqrt_rn(ss));
     const float rho = f16_bits_to_f32(hb);
     const int64_t rh = (int64_t)role * H + h;
-    if (lane == 0) p.norm[rh * p.max_tokens + p.token] = hb;
+    if (lane == 0) p.norm[rh * p.max_tokens + token] = hb;
     unsigned long long clamps = 0;
     if (rho == 0.0f) {
         for (int i = lane; i < d; i += 32) codes[i] = 0;
     } else {
         const float g = __fdiv_rn(p.A, rho);
-        clamps = (unsigned long long)quantize_blocks<LAT>(u, d, g, p.dither != 0, p.seed, (uint32_t)p.token, (uint32_t)h,
+        clamps = (unsigned long long)quantize_blocks<LAT>(u, d, g, p.dither != 0, p.seed, (uint32_t)token, (uint32_t)h,
                                                           (uint32_t)role, codes, lane, nullptr);
     }
     for (int o = 16; o; o >>= 1) clamps += __shfl_xor_sync(0xffffffffu, clamps, o);
@@ -1069,21 +1091,22 @@ k_kv_append1(KvAppend1 p) {
     uint32_t ustart = 0;
     if (lane == 0) {
         ustart = p.upos[rh];
-        if ((p.token & 127) == 0) p.blk_off[rh * (p.n_blk + 1) + (p.token >> 7)] = ustart;
+        if ((token & 127) == 0) p.blk_off[rh * (p.n_blk + 1) + (token >> 7)] = ustart;
         if (L >= 65535u) { kv_raise(p.flag, 1); L = 65535u; ustart = KV_NO_ROOM; }
         else if ((int64_t)ustart + L > p.una_words * 32 - 64) { kv_raise(p.flag, 2); ustart = KV_NO_ROOM; }
         else p.upos[rh] = ustart + L;
-        p.ulen[rh * p.max_tokens + p.token] = (uint16_t)L;
+        p.ulen[rh * p.max_tokens + token] = (uint16_t)L;
     }
     // pack: lane 0 writes the R-section, lane 1 the U-section (serial bit writers; 2 x 128 symbols)
     ustart = __shfl_sync(0xffffffffu, ustart, 0);
     if (lane == 0) {
-        BitWriter<StoreAtomicOr> bwr(StoreAtomicOr{p.rem + rh * p.rem_words}, (uint32_t)(p.token * p.rbits));
+        BitWriter<StoreAtomicOr> bwr(StoreAtomicOr{p.rem + rh * p.rem_words}, (uint32_t)(token * p.rbits));
         write_R<LAT>(bwr, z, d, p.k0, p.k1);
     } else if (lane == 1 && ustart != KV_NO_ROOM) {   // a vector that does not fit is not written (flag raised)
         BitWriter<StoreAtomicOr> bwu(StoreAtomicOr{p.una + rh * p.una_words}, ustart);
         write_U<LAT>(bwu, z, d, p.k0, p.k1);
     }
+    arrive();
 }
 
 void launch_kv_append1(const hq_kv* kv, const void* k, const void* v, cudaStream_t st) {
@@ -1095,7 +1118,7 @@ void launch_kv_append1(const hq_kv* kv, const void* k, const void* v, cudaStream
     p.n_blk = kv->n_blk; p.A = kv->A; p.seed = kv->cfg.codec.seed; p.dsign = kv->dsign; p.ssign = kv->ssign;
     p.qjl_t = kv->qjl ? kv->qjl + (size_t)p.d * p.d : nullptr;
     p.rem = kv->rem; p.una = kv->una; p.blk_off = kv->blk_off; p.upos = kv->upos; p.ulen = kv->ulen; p.norm = kv->norm;
-    p.ring = kv->ring; p.counters = kv->counters; p.flag = kv->flag_dev;
+    p.ring = kv->ring; p.counters = kv->counters; p.flag = kv->flag_dev; p.pos_dev = kv->pos_dev;
     const size_t smem = (size_t)p.d * (4 + 4 + 1 + 1);
     dim3 grid((unsigned)p.H, 2);
     switch (kv->cfg.codec.lattice) {

@@ -69,6 +69,7 @@ struct hq_kv {
     __nv_bfloat16* ring;  // [2][window][H][d]
     int8_t* dsign;      // [d]
     int8_t* ssign;      // [d]
+    uint32_t* pos_dev;  // device_position caches: [0] tokens held, [1] arrival counter of the single-token append (null otherwise)
     float* qjl;         // HQ_ROT_QJL: [2][d][d] - S row-major, then S transposed (null otherwise)
     unsigned long long* counters;  // [0] clamp count
     int* flag_host;                // mapped pinned host word: 0 ok, 1 a U-section past 65534 bits, 2 U stream full (sticky)
@@ -115,6 +116,7 @@ void launch_quantize_kv(const void* x, int64_t n_tok, int H, int d, int64_t toke
                         float A, int rotation, int dither, uint64_t seed, const int8_t* dsign,
                         const int8_t* ssign, int8_t* codes, uint16_t* norm_out, int64_t max_tokens,
                         unsigned long long* counters, cudaStream_t st, const float* qjl_t = nullptr);
+void launch_set_u32(uint32_t* dst, uint32_t v, cudaStream_t st);
 void launch_transpose_f32(const float* a, float* at, int n, cudaStream_t st);
 // activations: x [B, n_in] -> q int8 [B, n_in], s_x [B, n_kt], optional u
 void launch_act_quant(const void* x, int dtype, int64_t B, int64_t n_in, int64_t ldx, int lattice, int n,
