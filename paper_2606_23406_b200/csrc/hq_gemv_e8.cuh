@@ -285,6 +285,17 @@ __device__ __noinline__ void gv_first_prologue(const void* xp, int dtype, const 
         off0 = __ldg(soff);
         if (has > 1) off1 = __ldg(soff + 4);
     }
+    // The weights do not belong to the stream order (they are never written at inference time): the whole dependent chain
+    // of the first tile - offset -> header -> ragged words - is issued BEFORE griddepcontrol.wait, i.e. while the CTAs of
+    // the previous launch that are still running finish (a CTA of this kernel starts as soon as ITS SM is free).
+    uint32_t ul = 0, nrm = 0;
+    const uint8_t* sgp = blob + 16 * (size_t)off0;
+    if (has) {
+        gv_load_hdr_dense<KW>(sgp, lane, dense, stg_a, ul, nrm);
+        gv_load_r<KW>(sgp, lane, stg_a);
+        gv_load_ragged<KW>(sgp, dense, stg_a, ul);
+    }
+    bool ragged_due = false;
     griddep_wait();
     const bool vec = dtype == HQ_BF16 ? (((uintptr_t)xp) & 7) == 0 : (((uintptr_t)xp) & 15) == 0;
     const int col0 = act_col0(lane);
@@ -295,13 +306,6 @@ __device__ __noinline__ void gv_first_prologue(const void* xp, int dtype, const 
     uint2 auxn = make_uint2(0u, 0u);
     auto load_aux = [&](int kt) { if (fo.mode) auxn = __ldg((const uint2*)(fo.aux + (int64_t)kt * 128 + 4 * lane)); };
     if (j < nt) { gv_load_x(xp, dtype, vec, dsign, tile_of(j), lane, xn, sgn); load_aux(tile_of(j)); }
-    uint32_t ul = 0, nrm = 0;
-    const uint8_t* sgp = blob + 16 * (size_t)off0;
-    if (has) {
-        gv_load_hdr_dense<KW>(sgp, lane, dense, stg_a, ul, nrm);
-        gv_load_r<KW>(sgp, lane, stg_a);
-    }
-    bool ragged_due = has != 0;
     // R8: the scale of the whole vector, behind the first tile's loads (one more block barrier; mode is CTA-uniform)
     const float rms_r = fo.mode == 1 ? gv_rms_scale<NW>(xp, fo, n_kt, wid, lane) : 1.0f;
 #pragma unroll 1
