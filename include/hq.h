@@ -202,10 +202,13 @@ hq_status hq_linear(hq_ctx* ctx, const hq_weight* w, const void* x_dev, int32_t 
  * compute-bound regime on the large-M pipeline: E8, tile 128 or 256, k <= 3, batch >= 64 - anything else ->
  * HQ_ERR_UNSUPPORTED.  The accumulation order inside the tensor core is the hardware's: y meets the 1e-3 bar against
  * the reference, it is not bit-reproducible across GPU generations.  NVFP4 / MXFP4 (§6.4) are not built.
+ * acc_dev_or_null: parity / debug copy of every RHT tile's accumulator, [n_in / n_tile, batch, m_out]: int32 for
+ * HQ_CAST_INT8, float (the fp32 tensor-core accumulator) for HQ_CAST_FP8_E4M3.
  */
 typedef enum { HQ_CAST_INT8 = 0, HQ_CAST_FP8_E4M3 = 1 } hq_cast;
 hq_status hq_linear_cast(hq_ctx* ctx, const hq_weight* w, const void* x_dev, int32_t dtype, int64_t batch, int64_t ldx,
-                         void* y_bf16_dev, int64_t ldy, float* y_f32_dev_or_null, int32_t cast, void* stream);
+                         void* y_bf16_dev, int64_t ldy, float* y_f32_dev_or_null, void* acc_dev_or_null, int32_t cast,
+                         void* stream);
 
 /*
  * Several weights applied to the SAME x in one fused launch (q/k/v or gate/up of a decoder layer: §5.1 L309 quantizes

@@ -893,7 +893,8 @@ void hqo_act_quant_fp8(const float* x, int64_t B, int64_t n_in, int64_t ldx, int
 
 /* y[b,r] = Σ_kt (ρ[r,kt]/(α√n))·s_x[b,kt]·Σ_{i in tile} e4m3(c[r,i])·q8[b,i]   (double; products of two E4M3 values are exact) */
 void hqo_linear_fp8(const int8_t* codes, const uint16_t* norms, int64_t m, int64_t n_in, int lattice, int n,
-                    double snr_db, const float* q8, const float* s_x, int64_t B, double* y /*[B,m]*/) {
+                    double snr_db, const float* q8, const float* s_x, int64_t B, double* y /*[B,m]*/,
+                    double* acc /*[n_kt,B,m] or NULL: the per-tile sums*/, double* acc_abs /*[n_kt,B,m] or NULL: sums of |products|*/) {
     int64_t n_kt = n_in / n;
     double inv_A = 1.0 / (hqo_alpha(lattice, snr_db) * sqrt((double)n));
 #pragma omp parallel for schedule(static)
@@ -901,9 +902,14 @@ void hqo_linear_fp8(const int8_t* codes, const uint16_t* norms, int64_t m, int64
         for (int64_t b = 0; b < B; ++b) {
             double yy = 0.0;
             for (int64_t kt = 0; kt < n_kt; ++kt) {
-                double a = 0.0;
-                for (int i = 0; i < n; ++i)
-                    a += (double)hqo_e4m3_round((float)codes[r * n_in + kt * n + i]) * (double)q8[b * n_in + kt * n + i];
+                double a = 0.0, aa = 0.0;
+                for (int i = 0; i < n; ++i) {
+                    double t = (double)hqo_e4m3_round((float)codes[r * n_in + kt * n + i]) * (double)q8[b * n_in + kt * n + i];
+                    a += t;
+                    aa += fabs(t);
+                }
+                if (acc) acc[(kt * B + b) * m + r] = a;
+                if (acc_abs) acc_abs[(kt * B + b) * m + r] = aa;
                 yy += (double)f16_bits_to_f32(norms[r * n_kt + kt]) * inv_A * (double)s_x[b * n_kt + kt] * a;
             }
             y[b * m + r] = yy;

@@ -367,10 +367,13 @@ def act_quant_fp8(x, n_tile, seed):
     return q8, s_x
 
 
-def linear_fp8(codes, norms, lattice, n_tile, snr_db, q8, s_x):
+def linear_fp8(codes, norms, lattice, n_tile, snr_db, q8, s_x, want_acc=False):
     codes = _c(codes, np.int8); norms = _c(norms, np.uint16); q8 = _c(q8, np.float32); s_x = _c(s_x, np.float32)
     m, n_in = codes.shape; B = q8.shape[0]
     y = np.zeros((B, m), np.float64)
+    acc = np.zeros((n_in // n_tile, B, m), np.float64) if want_acc else None
+    acc_abs = np.zeros((n_in // n_tile, B, m), np.float64) if want_acc else None
     lib().hqo_linear_fp8(_p(codes), _p(norms), C.c_int64(m), C.c_int64(n_in), lattice, C.c_int(n_tile),
-                         C.c_double(snr_db), _p(q8), _p(s_x), C.c_int64(B), _p(y))
-    return y
+                         C.c_double(snr_db), _p(q8), _p(s_x), C.c_int64(B), _p(y),
+                         _p(acc) if want_acc else None, _p(acc_abs) if want_acc else None)
+    return (y, acc, acc_abs) if want_acc else y

@@ -124,7 +124,7 @@ def load_library():
     lib.hq_decode_int8.argtypes = [vp, vp, vp, vp, vp]
     lib.hq_act_quant.argtypes = [vp, vp, vp, i32, i64, i64, vp, vp, vp, vp]
     lib.hq_linear.argtypes = [vp, vp, vp, i32, i64, i64, vp, i64, vp, vp, vp]
-    lib.hq_linear_cast.argtypes = [vp, vp, vp, i32, i64, i64, vp, i64, vp, i32, vp]
+    lib.hq_linear_cast.argtypes = [vp, vp, vp, i32, i64, i64, vp, i64, vp, vp, i32, vp]
     lib.hq_linear_static.argtypes = [vp, vp, vp, i32, vp, vp, vp]
     lib.hq_linear_group.argtypes = [vp, C.POINTER(vp), i32, vp, i32, i64, i64, C.POINTER(vp), C.POINTER(i64), C.POINTER(vp), vp]
     lib.hq_linear_group_fold.argtypes = [vp, C.POINTER(vp), i32, vp, C.POINTER(_Fold), C.POINTER(vp), C.POINTER(vp), vp]
@@ -364,7 +364,7 @@ class Weight:
         return y
 
 
-    def linear_cast(self, x: torch.Tensor, cast: int, y: torch.Tensor = None, want_f32=False):
+    def linear_cast(self, x: torch.Tensor, cast: int, y: torch.Tensor = None, want_f32=False, want_acc=False):
         """hq_linear_cast: cast 0 = INT8 (hq_linear), 1 = FP8-E4M3 operands with an fp32 tensor-core accumulator."""
         dev = self.ctx.device
         assert x.is_cuda and x.dim() == 2 and x.stride(1) == 1
@@ -372,9 +372,15 @@ class Weight:
         if y is None:
             y = torch.empty((B, self.m), dtype=torch.bfloat16, device=dev)
         y32 = torch.empty((B, self.m), dtype=torch.float32, device=dev) if want_f32 else None
+        acc = None
+        if want_acc:   # [n_kt, B, m]: int32 (INT8 cast) or the fp32 tensor-core accumulator (FP8 cast)
+            acc = torch.empty((self.n_in // self.n_tile, B, self.m), dtype=torch.float32 if cast == CAST_FP8_E4M3 else torch.int32,
+                              device=dev)
         self.ctx.check(self.ctx.lib.hq_linear_cast(self.ctx.h, self.h, x.data_ptr(), _dtype_code(x), B, x.stride(0),
                                                    y.data_ptr(), y.stride(0), y32.data_ptr() if want_f32 else None,
-                                                   int(cast), _stream_ptr(dev)))
+                                                   acc.data_ptr() if want_acc else None, int(cast), _stream_ptr(dev)))
+        if want_acc:
+            return (y, y32, acc) if want_f32 else (y, acc)
         return (y, y32) if want_f32 else y
 
     def linear_static(self, x: torch.Tensor, y: torch.Tensor, y32: torch.Tensor = None):

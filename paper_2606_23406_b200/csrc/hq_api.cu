@@ -471,9 +471,11 @@ hq_status hq_linear(hq_ctx* ctx, const hq_weight* w, const void* x_dev, int32_t 
 }
 
 hq_status hq_linear_cast(hq_ctx* ctx, const hq_weight* w, const void* x_dev, int32_t dtype, int64_t batch, int64_t ldx,
-                         void* y_bf16_dev, int64_t ldy, float* y_f32_dev_or_null, int32_t cast, void* stream) {
+                         void* y_bf16_dev, int64_t ldy, float* y_f32_dev_or_null, void* acc_dev_or_null, int32_t cast,
+                         void* stream) {
     if (!ctx) return HQ_ERR_INVALID_ARG;
-    if (cast == HQ_CAST_INT8) return hq_linear(ctx, w, x_dev, dtype, batch, ldx, y_bf16_dev, ldy, y_f32_dev_or_null, nullptr, stream);
+    if (cast == HQ_CAST_INT8)
+        return hq_linear(ctx, w, x_dev, dtype, batch, ldx, y_bf16_dev, ldy, y_f32_dev_or_null, (int32_t*)acc_dev_or_null, stream);
     if (cast != HQ_CAST_FP8_E4M3) return fail(ctx, HQ_ERR_INVALID_ARG, "bad cast");
     if (!w || !x_dev || (!y_bf16_dev && !y_f32_dev_or_null)) return fail(ctx, HQ_ERR_INVALID_ARG, "null argument");
     if (batch <= 0 || ldx < w->n_in || (y_bf16_dev && ldy < w->m)) return fail(ctx, HQ_ERR_SHAPE, "bad batch / ldx / ldy");
@@ -490,8 +492,8 @@ hq_status hq_linear_cast(hq_ctx* ctx, const hq_weight* w, const void* x_dev, int
         if (!ctx->ws) return HQ_ERR_ALLOC;
         ctx->ws_bytes = need;
     }
-    return launch_linear_fp8(ctx, w, x_dev, dtype, batch, ldx, y_bf16_dev, ldy, y_f32_dev_or_null, (uint8_t*)ctx->ws,
-                             (cudaStream_t)stream);
+    return launch_linear_fp8(ctx, w, x_dev, dtype, batch, ldx, y_bf16_dev, ldy, y_f32_dev_or_null, (float*)acc_dev_or_null,
+                             (uint8_t*)ctx->ws, (cudaStream_t)stream);
 }
 
 hq_status hq_linear_static(hq_ctx* ctx, const hq_weight* w, const void* x_dev, int32_t dtype, void* y_bf16_dev,

@@ -161,7 +161,7 @@ hq_status launch_linear_group(hq_ctx* ctx, const hq_weight* const* ws, int n_w, 
                               int32_t* acc_i32, uint8_t* wsbuf, cudaStream_t st, const hq_fold* fold = nullptr);
 bool linear_uses_e8_fast(const hq_weight* w);
 hq_status launch_linear_fp8(hq_ctx* ctx, const hq_weight* w, const void* x, int dtype, int64_t B, int64_t ldx, void* y_bf16,
-                            int64_t ldy, float* y_f32, uint8_t* wsbuf, cudaStream_t st);
+                            int64_t ldy, float* y_f32, float* acc_f32, uint8_t* wsbuf, cudaStream_t st);
 hq_status launch_decode_ceiling(hq_ctx* ctx, const hq_weight* w, int reps, cudaStream_t st, double* scalars_per_s);
 // hq_linear_static: the address of the static scratch array (once per device, that device current), and the launch
 hq_status linear_static_setup(hq_ctx* ctx);

@@ -465,8 +465,9 @@ static hq_status launch_large(hq_ctx* ctx, const hq_weight* const* ws, int n_w, 
 
 // hq_linear_cast with HQ_CAST_FP8_E4M3 (§4.8): the large-M pipeline with E4M3 operands and an fp32 accumulator
 hq_status launch_linear_fp8(hq_ctx* ctx, const hq_weight* w, const void* x, int dtype, int64_t B, int64_t ldx, void* y_bf16,
-                            int64_t ldy, float* y_f32, uint8_t* wsbuf, cudaStream_t st) {
-    return launch_large(ctx, &w, 1, x, dtype, B, ldx, &y_bf16, &ldy, &y_f32, nullptr, wsbuf, st, 1);
+                            int64_t ldy, float* y_f32, float* acc_f32, uint8_t* wsbuf, cudaStream_t st) {
+    // the debug copy of the accumulators travels through the INT8 path's pointer: the kernel stores the TMEM words as they are
+    return launch_large(ctx, &w, 1, x, dtype, B, ldx, &y_bf16, &ldy, &y_f32, (int32_t*)acc_f32, wsbuf, st, 1);
 }
 
 // one activation cast, ONE fused decode + MMA launch over the stacked row blocks of all weights, one finalize each

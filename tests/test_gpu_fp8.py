@@ -49,10 +49,16 @@ def test_linear_fp8_matches_oracle(ctx, B, m, n_in, n_tile, k):
     w = ctx.encode_weights(_dev(W), 8, n_tile, SNR, seed, k)
     enc = hqo.encode_weights(W, hqo.E8, n_tile, SNR, seed, k)
     assert (w.decode_int8()[0].cpu().numpy() == enc["codes"]).all()
-    y, y32 = w.linear_cast(_dev(x), hq.CAST_FP8_E4M3, want_f32=True)
+    y, y32, acc = w.linear_cast(_dev(x), hq.CAST_FP8_E4M3, want_f32=True, want_acc=True)
     q8, sx8 = hqo.act_quant_fp8(x, n_tile, seed)
-    ref = hqo.linear_fp8(enc["codes"], enc["norms"], hqo.E8, n_tile, SNR, q8, sx8)
+    ref, acc_ref, acc_abs = hqo.linear_fp8(enc["codes"], enc["norms"], hqo.E8, n_tile, SNR, q8, sx8, want_acc=True)
     assert _rel_err(y32.cpu().numpy(), ref) < 1e-3
+    # The fp32 tensor-core accumulators of every (tile, activation row, weight row) against the exact sums of the E4M3
+    # products: fp32 summation of n_tile terms in any order errs by < n_tile * 2^-24 * sum|t| (1.5e-5 at 256); ONE operand
+    # that differs by one E4M3 step moves a sum by ~ (1/16) * sum|t| / n_tile = 2.4e-4 sum|t|.  So this bar pins both
+    # operands' E4M3 codes, element by element, through the production kernels.
+    err = np.abs(acc.cpu().numpy().astype(np.float64) - acc_ref)
+    assert (err <= 2e-5 * acc_abs + 1e-30).all(), float((err / (acc_abs + 1e-30)).max())
     ref_bf16 = hq_synth.to_bf16_f32(ref.astype(np.float32))
     tol = np.abs(ref_bf16) * 2.0 ** -7 + 1e-3 * np.sqrt((ref ** 2).mean())
     assert (np.abs(y.float().cpu().numpy() - ref_bf16) <= tol).all()
