@@ -237,7 +237,8 @@ k_attend_split(AttendParams p) {
     float* qs = sm;                            // [d][GP]   q' of the G query heads, coordinate-major
     float* vt = qs + d * GP;                   // [128][d+1]
     float* ps = vt + 128 * (d + 1);            // [128][GP]  p of the block's tokens
-    float* red = ps + 128 * GP;                // [GP][4] block reductions
+    float* red = ps + 128 * GP;                // [GP][4] block reductions (score max)
+    float* red2 = red + GP * 4;                // [GP][4] block reductions (sum of p)
     __shared__ uint32_t scan[4];
     __shared__ uint32_t lut_s[512];    // phase-1 table of the E8 decoder, [parity][byte]
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -364,6 +365,9 @@ k_attend_split(AttendParams p) {
                     float corr = (m_run[g] == -INFINITY) ? 0.0f : __expf(m_run[g] - m_new);
                     float pe = (valid && g < G) ? __expf(pg[g] - m_new) : 0.0f;
                     ps[tid * GP + g] = pe;
+                    float psum = pe;   // the block's softmax denominator, once (not per coordinate in the P V loop)
+                    for (int o = 16; o; o >>= 1) psum += __shfl_xor_sync(0xffffffffu, psum, o);
+                    if (lane == 0) red2[g * 4 + warp] = psum;
                     // every thread keeps the same running stats; l gets the block sum below
                     acc[g] *= corr; acc2[g] *= corr; l_run[g] *= corr; m_run[g] = m_new;
                 }
@@ -372,9 +376,9 @@ k_attend_split(AttendParams p) {
                 __syncthreads();
                 // P V: thread j = coordinate; one pass over the block's tokens for all heads
                 for (int j = tid, jj = 0; j < d; j += 128, ++jj) {
-                    float a[GP], lsum[GP];
+                    float a[GP];
 #pragma unroll
-                    for (int g = 0; g < GP; ++g) { a[g] = 0.0f; lsum[g] = 0.0f; }
+                    for (int g = 0; g < GP; ++g) a[g] = 0.0f;
 #pragma unroll 4
                     for (int tt = 0; tt < 128; ++tt) {
                         const float vv = vt[tt * (d + 1) + j];
@@ -382,12 +386,11 @@ k_attend_split(AttendParams p) {
                         for (int g4 = 0; g4 < GP; g4 += 4) {
                             const float4 p4 = *(const float4*)(ps + tt * GP + g4);
                             a[g4 + 0] += p4.x * vv; a[g4 + 1] += p4.y * vv; a[g4 + 2] += p4.z * vv; a[g4 + 3] += p4.w * vv;
-                            lsum[g4 + 0] += p4.x; lsum[g4 + 1] += p4.y; lsum[g4 + 2] += p4.z; lsum[g4 + 3] += p4.w;
                         }
                     }
 #pragma unroll
                     for (int g = 0; g < GP; ++g) {
-                        if (jj == 0) { acc[g] += a[g]; l_run[g] += lsum[g]; } else acc2[g] += a[g];
+                        if (jj == 0) { acc[g] += a[g]; l_run[g] += (red2[g * 4] + red2[g * 4 + 1]) + (red2[g * 4 + 2] + red2[g * 4 + 3]); } else acc2[g] += a[g];
                     }
                 }
                 __syncthreads();
@@ -554,7 +557,7 @@ hq_status launch_attend(hq_ctx* ctx, const hq_kv* kv, const void* q, int q_heads
     p.q = (const __nv_bfloat16*)q; p.dsign = kv->dsign; p.ssign = kv->ssign; p.ws = kv->att_ws;
     p.qjl = kv->qjl; p.qjl_t = kv->qjl ? kv->qjl + (size_t)kv->cfg.head_dim * kv->cfg.head_dim : nullptr;
     const int GP = p.G <= 4 ? 4 : 8;
-    size_t smem = ((size_t)GP * d + 128 * (size_t)(d + 1) + (size_t)GP * 128 + (size_t)GP * 4) * sizeof(float);
+    size_t smem = ((size_t)GP * d + 128 * (size_t)(d + 1) + (size_t)GP * 128 + (size_t)GP * 8) * sizeof(float);
 #define HQ_AT(L)                                                                                                   \
     do {                                                                                                           \
         if (GP == 4) {                                                                                             \
