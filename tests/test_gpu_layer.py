@@ -49,6 +49,12 @@ def _oracle_linear(e, x):
     return y[0]
 
 
+def _oracle_linear_seed(e, x, seed):
+    q, sx = hqo.act_quant(x[None], hqo.E8, 128, seed)
+    _, y = hqo.linear(e["codes"], e["norms"], hqo.E8, 128, SNR, q, sx, want_acc=False)
+    return y[0]
+
+
 def _rel_err(y, ref, floor=1e-3):
     ref = np.asarray(ref, np.float64)
     rms = np.sqrt((ref ** 2).mean())
@@ -193,4 +199,57 @@ def test_layer_decode_stage_by_stage(ctx, hidden, q_heads, kv_heads, ffn, T0):
     assert kv.export()["n_tokens"] == T0 + 2
     kv.free()
     for w in ws:
+        w.free()
+
+
+def test_layer_decode_full_size_llama_shapes_sampled_rows(ctx):
+    """The configuration bench.py's roofline.layer_step times (Llama-3.1-8B-shaped layer: hidden 4096, 32 query / 8 KV
+    heads of 128, FFN 14336; E8 4 bps weights, E8 2 bps cache with signs rotation, dither and a 32-token window), one
+    decode step after a 2048-token prefill, stage by stage.  The linears are checked on 96 sampled rows each (a row's
+    code and output are independent of the other rows, so the oracle encodes and contracts only those), attention in
+    full."""
+    hidden, q_heads, kv_heads, ffn, d, T0, window, eps, seed = 4096, 32, 8, 14336, 128, 2048, 32, 1e-5, 3
+    rng = np.random.default_rng(77)
+    names = ["q", "k", "v", "o", "gate", "up", "down"]
+    Ws = {n: hq_synth.llama_weight(1, n) for n in names}
+    ws = {n: ctx.encode_weights(_dev(Ws[n]), 8, 128, SNR, seed, (2, 2)) for n in names}
+    g1 = hq_synth.to_bf16_f32(1.0 + 0.1 * rng.standard_normal(hidden, dtype=np.float32))
+    g2 = hq_synth.to_bf16_f32(1.0 + 0.1 * rng.standard_normal(hidden, dtype=np.float32))
+    h = hq_synth.to_bf16_f32(rng.standard_normal(hidden, dtype=np.float32))
+    K0 = hq_synth.kv_tokens(T0, kv_heads, d, seed=4); V0 = hq_synth.kv_tokens(T0, kv_heads, d, seed=5)
+    kv = ctx.kv_create(kv_heads, d, T0 + 64, 8, SNR_KV, (0, 0), seed, rotation=1, dither=1, window=window)
+    kv.append(_dev(K0), _dev(V0))
+    layer = ctx.layer(*[ws[n] for n in names], _dev(g1), _dev(g2), eps, kv, q_heads)
+    h_out = _host(layer.decode(_dev(h)))
+    torch.cuda.synchronize()
+    got = {n: _host(layer.scratch_tensor(n)) for n in ("q", "k", "v", "a", "h2", "gate", "up")}
+
+    def check_rows(name, x, out, res=None):
+        W = Ws[name]; m = W.shape[0]
+        rows = np.sort(np.concatenate([rng.choice(m, 90, replace=False), [0, 1, 127, 128, m - 2, m - 1]]))
+        e = hqo.encode_weights(W[rows], hqo.E8, 128, SNR, seed, (2, 2))
+        ref = _oracle_linear_seed(e, x, seed)
+        if res is not None:
+            ref = ref + res[rows].astype(np.float64)
+        ref_bf16 = hq_synth.to_bf16_f32(ref.astype(np.float32))
+        tol = np.abs(ref_bf16) * 2.0 ** -7 + 1e-3 * np.sqrt((ref ** 2).mean())
+        assert (np.abs(out[rows].astype(np.float64) - ref_bf16) <= tol).all(), name
+
+    x1 = hqo.rmsnorm_bf16(h, g1, eps)
+    for n in ("q", "k", "v"):
+        check_rows(n, x1, got[n])
+    K = np.concatenate([K0, got["k"].reshape(1, kv_heads, d)]); V = np.concatenate([V0, got["v"].reshape(1, kv_heads, d)])
+    ck, nk, _ = hqo.kv_quantize(K, 0, 0, hqo.E8, SNR_KV, 1, 1, seed)
+    cv, nv, _ = hqo.kv_quantize(V, 0, 1, hqo.E8, SNR_KV, 1, 1, seed)
+    assert (kv.decode_int8(0, T0, 1).cpu().numpy() == ck[T0:]).all() and (kv.decode_int8(1, T0, 1).cpu().numpy() == cv[T0:]).all()
+    a_ref = hqo.attend(hqo.kv_reconstruct(ck, nk, 0, 0, hqo.E8, SNR_KV, 1, 1, seed),
+                       hqo.kv_reconstruct(cv, nv, 0, 1, hqo.E8, SNR_KV, 1, 1, seed), K, V, window=window,
+                       q=got["q"].reshape(q_heads, d))
+    _assert_bf16_close(got["a"], a_ref.reshape(-1), floor=2e-2)
+    check_rows("o", got["a"], got["h2"], res=h)
+    x2 = hqo.rmsnorm_bf16(got["h2"], g2, eps)
+    check_rows("gate", x2, got["gate"]); check_rows("up", x2, got["up"])
+    check_rows("down", hqo.silu_mul_bf16(got["gate"], got["up"]), h_out, res=got["h2"])
+    kv.free()
+    for w in ws.values():
         w.free()
