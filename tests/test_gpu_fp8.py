@@ -84,3 +84,24 @@ def test_linear_fp8_rejects_what_it_cannot_run(ctx):
     with pytest.raises(hq.HQError):
         w.linear_cast(_dev(hq_synth.activations(64, 512, seed=1)), 7)                        # no such cast
     w.free(); wd4.free()
+
+
+def test_linear_fp8_config5_full_size_sampled_outputs(ctx):
+    """BASELINE config 5's first GEMM at full size (8192 tokens x 4096 -> 16384, E8 4 bps, RHT tile 256) with the FP8 cast,
+    the call bench.py times as roofline.large_m.fp8_e4m3: 64 sampled weight rows x 64 sampled tokens (a row's code, a
+    token's activation cast and each output are independent of the rest)."""
+    import paper_2606_23406_b200 as hq
+    m, n_in, B, seed = 16384, 4096, 8192, 5
+    rng = np.random.default_rng(9)
+    W = hq_synth.gaussian_weight(m, n_in, seed=5)
+    x = hq_synth.activations(B, n_in, seed=6)
+    w = ctx.encode_weights(_dev(W), 8, 256, SNR, seed, (2, 2))
+    y, y32 = w.linear_cast(_dev(x), hq.CAST_FP8_E4M3, want_f32=True)
+    rows = np.sort(np.concatenate([rng.choice(m, 58, replace=False), [0, 127, 128, 255, m - 129, m - 1]]))
+    toks = np.sort(np.concatenate([rng.choice(B, 58, replace=False), [0, 255, 256, 511, B - 257, B - 1]]))
+    enc = hqo.encode_weights(W[rows], hqo.E8, 256, SNR, seed, (2, 2))
+    q8, sx8 = hqo.act_quant_fp8(x[toks], 256, seed)
+    ref = hqo.linear_fp8(enc["codes"], enc["norms"], hqo.E8, 256, SNR, q8, sx8)
+    got = y32.cpu().numpy()[np.ix_(toks, rows)]
+    assert _rel_err(got, ref) < 1e-3
+    w.free()
