@@ -90,3 +90,25 @@ def test_qjl_argument_checks(ctx):
         ctx.kv_create(2, 128, 64, hqo.E8, f32(9.68), (0, 0), 1, rotation=2, dither=1, window=0)            # qjl without a matrix
     with pytest.raises(hq.HQError):
         ctx.kv_create(2, 128, 64, hqo.E8, f32(9.68), (0, 0), 1, rotation=1, dither=1, window=0, qjl=Q)     # a matrix without qjl
+
+
+def test_qjl_attend_config4_shape_8192_tokens(ctx):
+    """Config 4's shape (8 KV heads x 128, 32 query heads, E8 2 bps, dither, 32-token window) with the paper's default
+    rotation at this rate (qjl, Table 4) over 8192 cached tokens: all 32 x 128 outputs against the long way round."""
+    T, H, d, QH, seed, snr = 8192, 8, 128, 32, 4, f32(9.68)
+    Q = hq_synth.haar_matrix(d, seed=123)
+    K = hq_synth.kv_tokens(T, H, d, seed=4); V = hq_synth.kv_tokens(T, H, d, seed=5)
+    q = hq_synth.activations(QH, d, seed=6)
+    kv = ctx.kv_create(H, d, T + 64, hqo.E8, snr, (0, 0), seed, rotation=2, dither=1, window=32, qjl=_dev(Q, torch.float32))
+    kv.append(_dev(K), _dev(V))
+    out, o32 = kv.attend(_dev(q), want_f32=True)
+    ck, nk, _ = hqo.kv_quantize(K, 0, 0, hqo.E8, snr, 2, 1, seed, qjl=Q)
+    cv, nv, _ = hqo.kv_quantize(V, 0, 1, hqo.E8, snr, 2, 1, seed, qjl=Q)
+    rng = np.random.default_rng(1)
+    for role, c in ((0, ck), (1, cv)):                                   # sampled tokens of the cache: codes bit-exact
+        for t in rng.choice(T, 24, replace=False):
+            assert (kv.decode_int8(role, int(t), 1).cpu().numpy()[0] == c[t]).all()
+    ref = hqo.attend(hqo.kv_reconstruct(ck, nk, 0, 0, hqo.E8, snr, 2, 1, seed, qjl=Q),
+                     hqo.kv_reconstruct(cv, nv, 0, 1, hqo.E8, snr, 2, 1, seed, qjl=Q), K, V, window=32, q=q)
+    assert _rel_err(o32.cpu().numpy(), ref, floor=2e-2) < 1e-3
+    kv.free()
