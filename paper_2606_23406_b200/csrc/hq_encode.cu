@@ -1102,9 +1102,25 @@ k_kv_append1(KvAppend1 p) {
     if (lane == 0) {
         BitWriter<StoreAtomicOr> bwr(StoreAtomicOr{p.rem + rh * p.rem_words}, (uint32_t)(token * p.rbits));
         write_R<LAT>(bwr, z, d, p.k0, p.k1);
-    } else if (lane == 1 && ustart != KV_NO_ROOM) {   // a vector that does not fit is not written (flag raised)
-        BitWriter<StoreAtomicOr> bwu(StoreAtomicOr{p.una + rh * p.una_words}, ustart);
-        write_U<LAT>(bwu, z, d, p.k0, p.k1);
+    }
+    if (ustart != KV_NO_ROOM) {   // a vector that does not fit is not written (flag raised)
+        // the U-section by all 32 lanes: lane l writes the unary codes of symbols [l d/32, (l+1) d/32) at the bit offset its
+        // predecessors' lengths add up to (an exclusive warp scan); words shared between lanes are merged by atomicOr
+        const int spl = d >> 5;
+        uint32_t mine = 0;
+        for (int j = lane * spl; j < (lane + 1) * spl; ++j) mine += 1u + ((uint32_t)z[j] >> (sym_class(LAT, j) ? p.k1 : p.k0));
+        uint32_t incl = mine;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t v = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += v;
+        }
+        BitWriter<StoreAtomicOr> bwu(StoreAtomicOr{p.una + rh * p.una_words}, ustart + (incl - mine));
+        for (int j = lane * spl; j < (lane + 1) * spl; ++j) {
+            bwu.skip((uint32_t)z[j] >> (sym_class(LAT, j) ? p.k1 : p.k0));
+            bwu.put(1u, 1);
+        }
+        bwu.finish();
     }
     arrive();
 }
