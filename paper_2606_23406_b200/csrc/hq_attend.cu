@@ -425,6 +425,11 @@ __global__ void k_attend_combine(AttendParams p, const __nv_bfloat16* ring, int 
     if (p.pos_dev) T = (int64_t)__ldcg(p.pos_dev);
     const float* wbase = p.ws + ((int64_t)h * p.n_split * G + g) * (d + 2);   // split s at + s * G * (d + 2)
     const int64_t wstride = (int64_t)G * (d + 2);
+    // this thread's coordinate of the first 64 splits' partial rows: issued now, needed after the max (one round trip for all)
+    constexpr int PRE = 64;
+    float pv[PRE];
+#pragma unroll
+    for (int u = 0; u < PRE; ++u) pv[u] = u < p.n_split ? __ldcg(wbase + u * wstride + j) : 0.0f;
     // global max over splits: thread j takes splits j, j + d, ... (independent loads), then a block reduction
     float m = -INFINITY;
     for (int s = j; s < p.n_split; s += d) {
@@ -470,7 +475,14 @@ __global__ void k_attend_combine(AttendParams p, const __nv_bfloat16* ring, int 
     __syncthreads();
     // the splits in split order (deterministic), eight loads in flight at a time
     float a = 0.0f, l = 0.0f;
-    for (int s0 = 0; s0 < p.n_split; s0 += 8) {
+#pragma unroll
+    for (int u = 0; u < PRE; ++u)
+        if (u < p.n_split && ls[u] > 0.0f) {
+            const float f = fs[u];
+            a += f * pv[u];
+            l += f * ls[u];
+        }
+    for (int s0 = PRE; s0 < p.n_split; s0 += 8) {
         float v[8];
 #pragma unroll
         for (int u = 0; u < 8; ++u) v[u] = (s0 + u < p.n_split && ls[s0 + u] > 0.0f) ? __ldcg(wbase + (s0 + u) * wstride + j) : 0.0f;
