@@ -253,3 +253,38 @@ def test_layer_decode_full_size_llama_shapes_sampled_rows(ctx):
     kv.free()
     for w in ws.values():
         w.free()
+
+
+def test_fold_edge_cases(ctx):
+    """Degenerate inputs of the folds: an all-zero residual stream (RMSNorm must give zeros, not NaN: eps), gates far outside
+    the exponential's clamp (+-100: silu -> 0 or the identity), a zero second factor, and a vector with one huge element
+    (the tree sum of squares and the bf16 rounding of tiny normalised values)."""
+    import paper_2606_23406_b200 as hq
+    n_in, m = 1024, 256
+    w, e = _enc(ctx, hq_synth.gaussian_weight(m, n_in, seed=41, outliers=True))
+    g = hq_synth.to_bf16_f32(np.linspace(0.5, 1.5, n_in).astype(np.float32))
+    # zero vector
+    ys, y32 = ctx.linear_group_fold([w], _dev(np.zeros(n_in, np.float32)), hq.FOLD_RMSNORM, aux=_dev(g), eps=1e-5, want_f32=True)
+    assert (y32[0] == 0).all() and torch.isfinite(ys[0].float()).all()
+    # one huge element
+    h = hq_synth.to_bf16_f32(np.random.default_rng(5).standard_normal(n_in, dtype=np.float32) * 1e-2)
+    h[77] = 3.0e4
+    h = hq_synth.to_bf16_f32(h)                                   # both sides see the same bf16 values
+    ys, y32 = ctx.linear_group_fold([w], _dev(h), hq.FOLD_RMSNORM, aux=_dev(g), eps=1e-6, want_f32=True)
+    x = hqo.rmsnorm_bf16(h, g, 1e-6)
+    _, y32_u = ctx.linear_group_fold([w], _dev(x), hq.FOLD_NONE, want_f32=True)
+    assert torch.equal(y32[0], y32_u[0])
+    assert _rel_err(_host(y32[0]), _oracle_linear(e, x)) < 1e-3
+    # gates beyond the clamp, zero factors
+    a = hq_synth.to_bf16_f32(np.random.default_rng(6).standard_normal(n_in, dtype=np.float32) * 3.0)
+    b = hq_synth.to_bf16_f32(np.random.default_rng(7).standard_normal(n_in, dtype=np.float32))
+    a[:8] = [100.0, -100.0, 88.0, -88.0, 87.5, -87.5, 0.0, -0.0]
+    b[8:16] = 0.0
+    a, b = hq_synth.to_bf16_f32(a), hq_synth.to_bf16_f32(b)
+    ys, y32 = ctx.linear_group_fold([w], _dev(a), hq.FOLD_SILU_MUL, aux=_dev(b), want_f32=True)
+    x = hqo.silu_mul_bf16(a, b)
+    assert np.isfinite(x).all()
+    _, y32_u = ctx.linear_group_fold([w], _dev(x), hq.FOLD_NONE, want_f32=True)
+    assert torch.equal(y32[0], y32_u[0])
+    assert _rel_err(_host(y32[0]), _oracle_linear(e, x)) < 1e-3
+    w.free()
