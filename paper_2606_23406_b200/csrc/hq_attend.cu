@@ -230,7 +230,10 @@ __device__ __forceinline__ void dither_e8_fast(const PhiloxKeys& rk, uint32_t bl
 // once into a byte row in shared memory, and ONE loop over the lattice blocks regenerates the dither and feeds the score
 // (K) or the v' row (V); nothing is unrolled over blocks or duplicated per decoder path.
 template <int LAT, int GP>
-__global__ void __launch_bounds__(128, 3)
+// 256 threads: threads 0..127 take the K rows of the block's 128 tokens (decode, dither, scores), threads 128..255 the V rows
+// (decode, dither, v' rows) AT THE SAME TIME - half the serial latency per block of the one-role-after-the-other loop and
+// 16 instead of 12 resident warps per SM; the P V product is then split over the two halves by tokens.
+__global__ void __launch_bounds__(256, 2)
 k_attend_split(AttendParams p) {
     extern __shared__ float sm[];
     const int d = p.d, G = p.G;
@@ -239,24 +242,26 @@ k_attend_split(AttendParams p) {
     float* ps = vt + 128 * (d + 1);            // [128][GP]  p of the block's tokens
     float* red = ps + 128 * GP;                // [GP][4] block reductions (score max)
     float* red2 = red + GP * 4;                // [GP][4] block reductions (sum of p)
-    __shared__ uint32_t scan[4];
+    const int KC = d + 68;                     // bytes per token of the K threads' rows: d codes + 17 nibble words
+    uint8_t* kc = (uint8_t*)(red2 + GP * 4);   // [128][KC]
+    __shared__ uint32_t scan[8];               // [role][4]
     __shared__ uint32_t lut_s[512];    // phase-1 table of the E8 decoder, [parity][byte]
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int tid = threadIdx.x, role = tid >> 7, tok = tid & 127, lane = tid & 31, warp = tok >> 5;   // warp: inside the role
     const int h = blockIdx.x / p.n_split, split = blockIdx.x % p.n_split;
-    for (int i = tid; i < 512; i += 128) lut_s[i] = unary_lut_entry(i & 255, i >> 8);
+    for (int i = tid; i < 512; i += 256) lut_s[i] = unary_lut_entry(i & 255, i >> 8);
     const uint32_t lut_a = smem_u32(lut_s);
     // nibble scratch of the E8 decoder: the last 17 words of this thread's (otherwise idle at that time) vt row
-    const uint32_t scr_a = smem_u32(vt + tid * (d + 1) + (d - 17));
+    const uint32_t scr_a = role ? smem_u32(vt + tok * (d + 1) + (d - 17)) : smem_u32(kc + tok * KC + d);
     // the token's INT8 codes: the last d bytes of its vt row.  The V loop overwrites the row with floats from the front
     // and reads the codes of a step before writing it, so the floats never reach codes still needed (4 j0 + 32 <= 3 d + 4 + j0 + 8)
-    uint8_t* crow = (uint8_t*)(vt + tid * (d + 1)) + (3 * d + 4);
+    uint8_t* crow = role ? (uint8_t*)(vt + tok * (d + 1)) + (3 * d + 4) : kc + tok * KC;
 
     // q' = S RHT(q): transformed in the vt area (one row of d floats per head), then stored coordinate-major
-    for (int i = tid; i < G * d; i += 128) vt[i] = __bfloat162float(p.q[(h * G) * d + i]);
+    for (int i = tid; i < G * d; i += 256) vt[i] = __bfloat162float(p.q[(h * G) * d + i]);
     __syncthreads();
-    for (int g = warp; g < G; g += 4) warp_query_transform(vt + g * d, d, p.dsign, p.ssign, p.rotation, p.qjl_t, lane);
+    for (int g = tid >> 5; g < G; g += 8) warp_query_transform(vt + g * d, d, p.dsign, p.ssign, p.rotation, p.qjl_t, lane);
     __syncthreads();
-    for (int i = tid; i < d * GP; i += 128) {
+    for (int i = tid; i < d * GP; i += 256) {
         const int j = i / GP, g = i % GP;
         qs[i] = g < G ? vt[g * d + j] : 0.0f;
     }
@@ -267,23 +272,23 @@ k_attend_split(AttendParams p) {
     const int64_t blk0 = (nblk_total * split) / p.n_split, blk1 = (nblk_total * (split + 1)) / p.n_split;   // balanced
 
     const PhiloxKeys rk = philox_round_keys(p.seed);
-    float m_run[GP], l_run[GP], acc[GP], acc2[GP];  // thread j owns coordinate j (and j + 128 when d == 256)
+    float m_run[GP], l_run[GP], acc[GP], acc2[GP];  // thread (j, half) owns coordinate j (and j + 128 when d == 256) over its half of a block's tokens
 #pragma unroll
     for (int g = 0; g < GP; ++g) { m_run[g] = -INFINITY; l_run[g] = 0.0f; acc[g] = 0.0f; acc2[g] = 0.0f; }
 
     for (int64_t blk = blk0; blk < blk1; ++blk) {
-        const int64_t t = blk * 128 + tid;
+        const int64_t t = blk * 128 + tok;
         const bool valid = t < Tc;
         float pg[GP];
-        for (int role = 0; role < 2; ++role) {
+        {
             const uint32_t* rem = p.rem + ((int64_t)role * p.H + h) * p.rem_words;
             const uint32_t* una = p.una + ((int64_t)role * p.H + h) * p.una_words;
             const uint16_t* ulen = p.ulen + ((int64_t)role * p.H + h) * p.max_tokens;
             const uint16_t* norm = p.norm + ((int64_t)role * p.H + h) * p.max_tokens;
             const uint32_t* blkoff = p.blk_off + ((int64_t)role * p.H + h) * (p.n_blk + 1);
             // every token of the block has been appended (t < T), those >= Tc are simply masked
-            uint32_t ul = (blk * 128 + tid < p.max_tokens) ? ulen[blk * 128 + tid] : 0;
-            uint32_t us = blkoff[blk] + row_ustart_128(ul, scan, tid);
+            uint32_t ul = (blk * 128 + tok < p.max_tokens) ? ulen[blk * 128 + tok] : 0;
+            uint32_t us = blkoff[blk] + row_ustart_128(ul, scan + 4 * role, tok);
             const float scale = valid ? f16_bits_to_f32(norm[t]) * p.inv_A : 0.0f;
             // ---- decode the token's codes into its byte row
             if (valid) {
@@ -307,7 +312,7 @@ k_attend_split(AttendParams p) {
             float dot[GP];
 #pragma unroll
             for (int g = 0; g < GP; ++g) dot[g] = 0.0f;
-            float* row = vt + tid * (d + 1);
+            float* row = vt + tok * (d + 1);
             // ---- one loop over the lattice blocks: codes - regenerated dither -> score terms (K) or the v' row (V)
             if (valid) {
                 constexpr int BL = LAT == LAT_E8 ? 8 : 4;   // coordinates per iteration (a multiple of the lattice dimension)
@@ -348,7 +353,7 @@ k_attend_split(AttendParams p) {
                 for (int j = 0; j < d; ++j) row[j] = 0.0f;
             }
             if (role == 0) {
-                // scores, block max, p
+                // scores and the warps' maxima
 #pragma unroll
                 for (int g = 0; g < GP; ++g) {
                     float s = (valid && g < G) ? dot[g] * scale * p.inv_sqrt_d : -INFINITY;
@@ -357,54 +362,65 @@ k_attend_split(AttendParams p) {
                     if (lane == 0) red[g * 4 + warp] = mx;
                     pg[g] = s;
                 }
-                __syncthreads();
+            }
+            __syncthreads();   // the maxima and the v' rows are written
 #pragma unroll
-                for (int g = 0; g < GP; ++g) {
-                    float mb = fmaxf(fmaxf(red[g * 4], red[g * 4 + 1]), fmaxf(red[g * 4 + 2], red[g * 4 + 3]));
-                    float m_new = fmaxf(m_run[g], mb);
-                    float corr = (m_run[g] == -INFINITY) ? 0.0f : __expf(m_run[g] - m_new);
+            for (int g = 0; g < GP; ++g) {
+                float mb = fmaxf(fmaxf(red[g * 4], red[g * 4 + 1]), fmaxf(red[g * 4 + 2], red[g * 4 + 3]));
+                float m_new = fmaxf(m_run[g], mb);
+                float corr = (m_run[g] == -INFINITY) ? 0.0f : __expf(m_run[g] - m_new);
+                if (role == 0) {
                     float pe = (valid && g < G) ? __expf(pg[g] - m_new) : 0.0f;
-                    ps[tid * GP + g] = pe;
+                    ps[tok * GP + g] = pe;
                     float psum = pe;   // the block's softmax denominator, once (not per coordinate in the P V loop)
                     for (int o = 16; o; o >>= 1) psum += __shfl_xor_sync(0xffffffffu, psum, o);
                     if (lane == 0) red2[g * 4 + warp] = psum;
-                    // every thread keeps the same running stats; l gets the block sum below
-                    acc[g] *= corr; acc2[g] *= corr; l_run[g] *= corr; m_run[g] = m_new;
                 }
-                __syncthreads();
-            } else {
-                __syncthreads();
-                // P V: thread j = coordinate; one pass over the block's tokens for all heads
-                for (int j = tid, jj = 0; j < d; j += 128, ++jj) {
-                    float a[GP];
-#pragma unroll
-                    for (int g = 0; g < GP; ++g) a[g] = 0.0f;
-#pragma unroll 4
-                    for (int tt = 0; tt < 128; ++tt) {
-                        const float vv = vt[tt * (d + 1) + j];
-#pragma unroll
-                        for (int g4 = 0; g4 < GP; g4 += 4) {
-                            const float4 p4 = *(const float4*)(ps + tt * GP + g4);
-                            a[g4 + 0] += p4.x * vv; a[g4 + 1] += p4.y * vv; a[g4 + 2] += p4.z * vv; a[g4 + 3] += p4.w * vv;
-                        }
-                    }
-#pragma unroll
-                    for (int g = 0; g < GP; ++g) {
-                        if (jj == 0) { acc[g] += a[g]; l_run[g] += (red2[g * 4] + red2[g * 4 + 1]) + (red2[g * 4 + 2] + red2[g * 4 + 3]); } else acc2[g] += a[g];
-                    }
-                }
-                __syncthreads();
+                // every thread keeps the same running stats; l gets the block sum below
+                acc[g] *= corr; acc2[g] *= corr; l_run[g] *= corr; m_run[g] = m_new;
             }
+            __syncthreads();   // p and its sums are written
+            // P V: thread = (coordinate, half of the block's tokens); the halves meet after the last block
+            for (int j = tok, jj = 0; j < d; j += 128, ++jj) {
+                float a[GP];
+#pragma unroll
+                for (int g = 0; g < GP; ++g) a[g] = 0.0f;
+#pragma unroll 4
+                for (int tt = 64 * role; tt < 64 * role + 64; ++tt) {
+                    const float vv = vt[tt * (d + 1) + j];
+#pragma unroll
+                    for (int g4 = 0; g4 < GP; g4 += 4) {
+                        const float4 p4 = *(const float4*)(ps + tt * GP + g4);
+                        a[g4 + 0] += p4.x * vv; a[g4 + 1] += p4.y * vv; a[g4 + 2] += p4.z * vv; a[g4 + 3] += p4.w * vv;
+                    }
+                }
+#pragma unroll
+                for (int g = 0; g < GP; ++g) {
+                    if (jj == 0) acc[g] += a[g]; else acc2[g] += a[g];
+                }
+            }
+#pragma unroll
+            for (int g = 0; g < GP; ++g) l_run[g] += (red2[g * 4] + red2[g * 4 + 1]) + (red2[g * 4 + 2] + red2[g * 4 + 3]);
+            __syncthreads();   // the block's rows, p and reductions may be overwritten
         }
     }
+    // the two token halves of every coordinate meet (vt is free now)
+    if (role == 1) {
+#pragma unroll
+        for (int g = 0; g < GP; ++g) { vt[(2 * g) * 128 + tok] = acc[g]; vt[(2 * g + 1) * 128 + tok] = acc2[g]; }
+    }
+    __syncthreads();
+    if (role == 1) return;
+#pragma unroll
+    for (int g = 0; g < GP; ++g) { acc[g] += vt[(2 * g) * 128 + tok]; acc2[g] += vt[(2 * g + 1) * 128 + tok]; }
     // write partials: [h][split][g][d + 2] = acc..., m, l   (threads with tid < d hold valid m/l)
     float* out = p.ws + ((int64_t)(h * p.n_split + split) * G) * (d + 2);
 #pragma unroll
     for (int g = 0; g < GP; ++g) {
         if (g < G) {
-            if (tid < d) out[g * (d + 2) + tid] = acc[g];
-            if (d > 128) out[g * (d + 2) + tid + 128] = acc2[g];
-            if (tid == 0) { out[g * (d + 2) + d] = m_run[g]; out[g * (d + 2) + d + 1] = l_run[g]; }
+            if (tok < d) out[g * (d + 2) + tok] = acc[g];
+            if (d > 128) out[g * (d + 2) + tok + 128] = acc2[g];
+            if (tok == 0) { out[g * (d + 2) + d] = m_run[g]; out[g * (d + 2) + d + 1] = l_run[g]; }
         }
     }
 }
@@ -540,7 +556,7 @@ static int attend_n_split(const hq_ctx* ctx, const hq_kv* kv) {
     int64_t Tc = kv->n_tokens > window ? kv->n_tokens - window : 0;
     if (kv->pos_dev) Tc = kv->cfg.max_tokens;   // fixed for the life of the cache: a captured launch stays valid as tokens arrive
     int64_t nblk = (Tc + 127) / 128;
-    int64_t want = (ctx->sm_count * 3) / kv->cfg.kv_heads;   // one wave of the 3 resident CTAs per SM
+    int64_t want = (ctx->sm_count * 2) / kv->cfg.kv_heads;   // one wave of the 2 resident CTAs (256 threads) per SM
     if (want < 1) want = 1;
     int64_t ns = nblk < want ? nblk : want;
     return (int)(ns < 1 ? 1 : ns);
@@ -569,15 +585,15 @@ hq_status launch_attend(hq_ctx* ctx, const hq_kv* kv, const void* q, int q_heads
     p.q = (const __nv_bfloat16*)q; p.dsign = kv->dsign; p.ssign = kv->ssign; p.ws = kv->att_ws;
     p.qjl = kv->qjl; p.qjl_t = kv->qjl ? kv->qjl + (size_t)kv->cfg.head_dim * kv->cfg.head_dim : nullptr;
     const int GP = p.G <= 4 ? 4 : 8;
-    size_t smem = ((size_t)GP * d + 128 * (size_t)(d + 1) + (size_t)GP * 128 + (size_t)GP * 8) * sizeof(float);
+    size_t smem = ((size_t)GP * d + 128 * (size_t)(d + 1) + (size_t)GP * 128 + (size_t)GP * 8) * sizeof(float) + 128 * (size_t)(d + 68);
 #define HQ_AT(L)                                                                                                   \
     do {                                                                                                           \
         if (GP == 4) {                                                                                             \
             HQ_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_attend_split<L, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
-            k_attend_split<L, 4><<<H * p.n_split, 128, smem, st>>>(p);                                             \
+            k_attend_split<L, 4><<<H * p.n_split, 256, smem, st>>>(p);                                             \
         } else {                                                                                                   \
             HQ_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_attend_split<L, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
-            k_attend_split<L, 8><<<H * p.n_split, 128, smem, st>>>(p);                                             \
+            k_attend_split<L, 8><<<H * p.n_split, 256, smem, st>>>(p);                                             \
         }                                                                                                          \
     } while (0)
     cudaEvent_t e0 = nullptr, e1 = nullptr;
