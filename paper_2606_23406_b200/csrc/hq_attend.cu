@@ -225,6 +225,83 @@ __device__ __forceinline__ void dither_e8_fast(const PhiloxKeys& rk, uint32_t bl
     for (int i = 0; i < 8; ++i) U[i] = __fsub_rn(y[i], pa ? fa[i] : fb[i]);
 }
 
+// ---- the same dither with packed fp32 pairs (sm_100 add / mul / fma .f32x2): the kernel is issue bound and the E8 nearest
+// point is 19 FADD + 6 FMUL per scalar, so two coordinates per instruction saves a sixth of all issue slots.  Pair k holds
+// coordinates (k, k + 4): elementwise steps pair up trivially, and the canonical tree sum of the squared distances
+// ((d0+d1)+(d2+d3)) + ((d4+d5)+(d6+d7)) is two packed levels and one scalar add.  Every operation is the same IEEE
+// round-to-nearest fp32 operation on the same values as in dither_e8_fast: a - b is fma(b, -1, a) (the product is exact),
+// y = w 2^-22 - 2 and (y - 1) / 2 are single fmas whose products are exact too.  Same decisions, same U.
+__device__ __forceinline__ uint64_t pk2(float lo, float hi) {
+    uint64_t r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void up2(uint64_t v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ uint64_t add2(uint64_t a, uint64_t b) { uint64_t r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ uint64_t mul2(uint64_t a, uint64_t b) { uint64_t r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ uint64_t fma2(uint64_t a, uint64_t b, uint64_t c) { uint64_t r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
+
+// Q_{D8} on packed pairs: z2[k] = (z_k, z_{k+4}); returns f2 likewise
+__device__ __forceinline__ void nearest_d8_p2(const uint64_t* z2, uint64_t* f2) {
+    const uint64_t M2 = pk2(12582912.0f, 12582912.0f), NM2 = pk2(-12582912.0f, -12582912.0f), N1 = pk2(-1.0f, -1.0f);
+    uint64_t dl2[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        f2[k] = add2(add2(z2[k], M2), NM2);    // rint: (z + M) - M
+        dl2[k] = fma2(f2[k], N1, z2[k]);       // z - f
+    }
+    float slo, shi;
+    up2(add2(add2(f2[0], f2[1]), add2(f2[2], f2[3])), slo, shi);
+    const bool odd = ((int)(slo + shi)) & 1;   // exact: small integers
+    float dl[8];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) up2(dl2[k], dl[k], dl[k + 4]);
+    float best = fabsf(dl[0]), dj = dl[0];
+    int j = 0;
+#pragma unroll
+    for (int i = 1; i < 8; ++i) {
+        const float a = fabsf(dl[i]);
+        const bool gt = a > best;
+        best = gt ? a : best; dj = gt ? dl[i] : dj; j = gt ? i : j;
+    }
+    const float step = odd ? (dj < 0.0f ? -1.0f : 1.0f) : 0.0f;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) f2[k] = add2(f2[k], pk2(j == k ? step : 0.0f, j == k + 4 ? step : 0.0f));
+}
+// U2[k] = (U_k, U_{k+4})
+__device__ __forceinline__ void dither_e8_packed(const PhiloxKeys& rk, uint32_t blk, uint32_t token, uint32_t headrole, uint64_t* U2) {
+    uint32_t o[8];
+    philox4x32_10_keys(2 * blk, token, headrole, 3u, rk, o);
+    philox4x32_10_keys(2 * blk + 1, token, headrole, 3u, rk, o + 4);
+    const uint64_t C22 = pk2(0x1p-22f, 0x1p-22f), N2 = pk2(-2.0f, -2.0f), H2 = pk2(0.5f, 0.5f), NH2 = pk2(-0.5f, -0.5f),
+                   T2 = pk2(2.0f, 2.0f), O2 = pk2(1.0f, 1.0f), N1 = pk2(-1.0f, -1.0f);
+    uint64_t y2[4], za2[4], zb2[4], fa2[4], fb2[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const uint64_t w2 = pk2((float)(2u * (o[k] >> 9) + 1u), (float)(2u * (o[k + 4] >> 9) + 1u));   // exact: < 2^24
+        y2[k] = fma2(w2, C22, N2);            // w 2^-22 - 2
+        za2[k] = mul2(y2[k], H2);             // y / 2
+        zb2[k] = fma2(y2[k], H2, NH2);        // (y - 1) / 2
+    }
+    nearest_d8_p2(za2, fa2);
+    nearest_d8_p2(zb2, fb2);
+    uint64_t da2[4], db2[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        fa2[k] = mul2(fa2[k], T2);            // a = 2 Q(y/2)
+        fb2[k] = fma2(fb2[k], T2, O2);        // b = 2 Q((y-1)/2) + 1
+        const uint64_t ea = fma2(fa2[k], N1, y2[k]), eb = fma2(fb2[k], N1, y2[k]);
+        da2[k] = mul2(ea, ea);
+        db2[k] = mul2(eb, eb);
+    }
+    float alo, ahi, blo, bhi;
+    up2(add2(add2(da2[0], da2[1]), add2(da2[2], da2[3])), alo, ahi);   // ((d0+d1)+(d2+d3), (d4+d5)+(d6+d7))
+    up2(add2(add2(db2[0], db2[1]), add2(db2[2], db2[3])), blo, bhi);
+    const bool pa = __fadd_rn(alo, ahi) <= __fadd_rn(blo, bhi);
+#pragma unroll
+    for (int k = 0; k < 4; ++k) U2[k] = fma2(pa ? fa2[k] : fb2[k], N1, y2[k]);
+}
+
 // GP = query heads per KV head padded to 4 or 8 (vector loads of q' and p).
 // Code size matters here (the dither regeneration is ~300 instructions per lattice block): a token's codes are decoded
 // once into a byte row in shared memory, and ONE loop over the lattice blocks regenerates the dither and feeds the score
@@ -325,13 +402,19 @@ k_attend_split(AttendParams p) {
                     for (int e = 0; e < BL; ++e) v[e] = (float)(int)(int8_t)((e < 4 ? w0 : w1) >> (8 * (e & 3)));
                     if (LAT == LAT_A2) { v[0] *= HQ_S3; v[2] *= HQ_S3; }
                     if (p.dither) {
+                        if (LAT == LAT_E8) {   // packed pairs (coordinate k, k + 4)
+                            uint64_t U2[4];
+                            dither_e8_packed(rk, (uint32_t)(j0 / LAT), (uint32_t)t, (uint32_t)h | ((uint32_t)role << 16), U2);
 #pragma unroll
-                        for (int sb = 0; sb < BL / LAT; ++sb) {
-                            float U[LAT];
-                            if (LAT == LAT_E8) dither_e8_fast(rk, (uint32_t)(j0 / LAT + sb), (uint32_t)t, (uint32_t)h | ((uint32_t)role << 16), U);
-                            else dither_block<LAT>(p.seed, (uint32_t)(j0 / LAT + sb), (uint32_t)t, (uint32_t)h, (uint32_t)role, U);
+                            for (int k = 0; k < 4; ++k) up2(fma2(U2[k], pk2(-1.0f, -1.0f), pk2(v[k], v[k + 4])), v[k], v[k + 4]);
+                        } else {
 #pragma unroll
-                            for (int e = 0; e < LAT; ++e) v[sb * LAT + e] -= U[e];
+                            for (int sb = 0; sb < BL / LAT; ++sb) {
+                                float U[LAT];
+                                dither_block<LAT>(p.seed, (uint32_t)(j0 / LAT + sb), (uint32_t)t, (uint32_t)h, (uint32_t)role, U);
+#pragma unroll
+                                for (int e = 0; e < LAT; ++e) v[sb * LAT + e] -= U[e];
+                            }
                         }
                     }
                     if (role == 0) {
