@@ -164,8 +164,9 @@ __device__ __forceinline__ void philox4x32_10_keys(uint32_t c0, uint32_t c1, uin
                                                    uint32_t* o) {
 #pragma unroll
     for (int r = 0; r < 10; ++r) {
-        const uint32_t h0 = __umulhi(0xD2511F53u, c0), l0 = 0xD2511F53u * c0;
-        const uint32_t h1 = __umulhi(0xCD9E8D57u, c2), l1 = 0xCD9E8D57u * c2;
+        uint32_t h0, l0, h1, l1;   // one 32 x 32 -> 64 multiply each (IMAD.WIDE), not a high and a low half
+        asm("{\n\t.reg .u64 t;\n\tmul.wide.u32 t, %2, %3;\n\tmov.b64 {%0, %1}, t;\n\t}" : "=r"(l0), "=r"(h0) : "r"(c0), "r"(0xD2511F53u));
+        asm("{\n\t.reg .u64 t;\n\tmul.wide.u32 t, %2, %3;\n\tmov.b64 {%0, %1}, t;\n\t}" : "=r"(l1), "=r"(h1) : "r"(c2), "r"(0xCD9E8D57u));
         c0 = h1 ^ c1 ^ rk.k0[r]; c1 = l1; c2 = h0 ^ c3 ^ rk.k1[r]; c3 = l0;
     }
     o[0] = c0; o[1] = c1; o[2] = c2; o[3] = c3;
@@ -386,9 +387,9 @@ k_attend_split(AttendParams p) {
                                       }
                                   });
             }
-            float dot[GP];
+            uint64_t dot2[GP / 2];   // (head 2i, head 2i + 1)
 #pragma unroll
-            for (int g = 0; g < GP; ++g) dot[g] = 0.0f;
+            for (int g = 0; g < GP / 2; ++g) dot2[g] = 0ull;
             float* row = vt + tok * (d + 1);
             // ---- one loop over the lattice blocks: codes - regenerated dither -> score terms (K) or the v' row (V)
             if (valid) {
@@ -420,11 +421,12 @@ k_attend_split(AttendParams p) {
                     if (role == 0) {
 #pragma unroll
                         for (int e = 0; e < BL; ++e) {
+                            const uint64_t vv = pk2(v[e], v[e]);
 #pragma unroll
-                            for (int g4 = 0; g4 < GP; g4 += 4) {
-                                const float4 q4 = *(const float4*)(qs + (j0 + e) * GP + g4);
-                                dot[g4 + 0] += q4.x * v[e]; dot[g4 + 1] += q4.y * v[e];
-                                dot[g4 + 2] += q4.z * v[e]; dot[g4 + 3] += q4.w * v[e];
+                            for (int g4 = 0; g4 < GP; g4 += 4) {   // two query heads per packed fma
+                                const ulonglong2 q2 = *(const ulonglong2*)(qs + (j0 + e) * GP + g4);
+                                dot2[g4 / 2] = fma2(q2.x, vv, dot2[g4 / 2]);
+                                dot2[g4 / 2 + 1] = fma2(q2.y, vv, dot2[g4 / 2 + 1]);
                             }
                         }
                     } else {
@@ -437,6 +439,10 @@ k_attend_split(AttendParams p) {
             }
             if (role == 0) {
                 // scores and the warps' maxima
+#pragma unroll
+                float dot[GP];
+#pragma unroll
+                for (int g = 0; g < GP / 2; ++g) up2(dot2[g], dot[2 * g], dot[2 * g + 1]);
 #pragma unroll
                 for (int g = 0; g < GP; ++g) {
                     float s = (valid && g < G) ? dot[g] * scale * p.inv_sqrt_d : -INFINITY;
@@ -465,21 +471,25 @@ k_attend_split(AttendParams p) {
             __syncthreads();   // p and its sums are written
             // P V: thread = (coordinate, half of the block's tokens); the halves meet after the last block
             for (int j = tok, jj = 0; j < d; j += 128, ++jj) {
-                float a[GP];
+                uint64_t a2[GP / 2];
 #pragma unroll
-                for (int g = 0; g < GP; ++g) a[g] = 0.0f;
+                for (int g = 0; g < GP / 2; ++g) a2[g] = 0ull;
 #pragma unroll 4
                 for (int tt = 64 * role; tt < 64 * role + 64; ++tt) {
-                    const float vv = vt[tt * (d + 1) + j];
+                    const float vf = vt[tt * (d + 1) + j];
+                    const uint64_t vv = pk2(vf, vf);
 #pragma unroll
                     for (int g4 = 0; g4 < GP; g4 += 4) {
-                        const float4 p4 = *(const float4*)(ps + tt * GP + g4);
-                        a[g4 + 0] += p4.x * vv; a[g4 + 1] += p4.y * vv; a[g4 + 2] += p4.z * vv; a[g4 + 3] += p4.w * vv;
+                        const ulonglong2 p2 = *(const ulonglong2*)(ps + tt * GP + g4);
+                        a2[g4 / 2] = fma2(p2.x, vv, a2[g4 / 2]);
+                        a2[g4 / 2 + 1] = fma2(p2.y, vv, a2[g4 / 2 + 1]);
                     }
                 }
 #pragma unroll
-                for (int g = 0; g < GP; ++g) {
-                    if (jj == 0) acc[g] += a[g]; else acc2[g] += a[g];
+                for (int g = 0; g < GP / 2; ++g) {
+                    float lo, hi;
+                    up2(a2[g], lo, hi);
+                    if (jj == 0) { acc[2 * g] += lo; acc[2 * g + 1] += hi; } else { acc2[2 * g] += lo; acc2[2 * g + 1] += hi; }
                 }
             }
 #pragma unroll
