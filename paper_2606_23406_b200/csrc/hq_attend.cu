@@ -639,7 +639,7 @@ __global__ void k_attend_combine(AttendParams p, const __nv_bfloat16* ring, int 
     }
     if (j == 0) s_l = l;
     __syncthreads();
-    o /= s_l;
+    o = s_l > 0.0f ? o / s_l : 0.0f;   // an empty device-position cache attends to nothing: zeros, not NaN
     if (out_bf16) out_bf16[qh * d + j] = __float2bfloat16_rn(o);
     if (out_f32) out_f32[qh * d + j] = o;
 }

@@ -102,3 +102,13 @@ def test_replay_past_capacity_writes_nothing_and_turns_sticky(ctx):
     with pytest.raises(hq.HQError):
         kv.sync_position()                           # sticky HQ_ERR_FORMAT
     kv.free()
+
+
+def test_attend_on_an_empty_device_position_cache_gives_zeros(ctx):
+    """A host-position cache rejects attend on an empty cache; a device-position cache cannot know (the count is on the
+    device): it must return zeros, not NaN."""
+    kv = ctx.kv_create(2, 128, 64, 8, SNR_KV, (0, 0), SEED, rotation=1, dither=1, window=32, device_position=True)
+    out = kv.attend(_dev(hq_synth.activations(4, 128, seed=1)))
+    torch.cuda.synchronize()
+    assert (out.float() == 0).all()
+    kv.free()
