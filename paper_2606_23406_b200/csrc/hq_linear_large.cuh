@@ -164,6 +164,19 @@ __device__ __forceinline__ uint64_t fma_f32x2(uint64_t a, uint64_t b, uint64_t c
     return r;
 }
 
+// Tile order of the persistent GEMM: panels of LG_PANEL row blocks, inside a panel batch-tile major.  The 148 tiles in
+// flight then touch LG_PANEL weight row blocks and ~148 / LG_PANEL batch tiles (a few MB of operands each way) instead of
+// every row block of the weight (the whole 69 MB scratch copy per wave in plain batch-tile-major order): the operand
+// tiles are re-read from L2, not from DRAM.
+constexpr int LG_PANEL = 16;
+__device__ __forceinline__ void lg_tile_coords(int tile, int n_rb, int n_bt, int& bt, int& rb) {
+    const int per_panel = LG_PANEL * n_bt;
+    const int panel = tile / per_panel, rem = tile - panel * per_panel;
+    const int rows = min(LG_PANEL, n_rb - panel * LG_PANEL);
+    bt = rem / rows;
+    rb = panel * LG_PANEL + (rem - bt * rows);
+}
+
 struct E8LargeParams {
     const uint8_t* ablob;   // [n_rb][n_kt][LG_ABLOB]
     const uint8_t* bblob;   // [n_bt][n_kt][LG_BBLOB]
@@ -211,7 +224,8 @@ __global__ void __launch_bounds__(384, 1) k_e8_gemm_large(E8LargeParams p) {
         if (tid == 0) {   // ---- TMA producer
             uint32_t it = 0;
             for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-                const int bt = tile / p.n_rb, rb = tile - bt * p.n_rb;
+                int bt, rb;
+                lg_tile_coords(tile, p.n_rb, p.n_bt, bt, rb);
                 const uint8_t* ag = p.ablob + (size_t)rb * p.n_kt * LG_ABLOB;
                 const uint8_t* bg = p.bblob + (size_t)bt * p.n_kt * LG_BBLOB;
                 for (int kt = 0; kt < p.n_kt; ++kt, ++it) {
@@ -279,7 +293,8 @@ __global__ void __launch_bounds__(384, 1) k_e8_gemm_large(E8LargeParams p) {
         const uint32_t n_steps = (uint32_t)my_tiles * (uint32_t)n_tl;
         if (n_steps) begin_step(0);
         for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-            const int bt = tile / p.n_rb, rb = tile - bt * p.n_rb;
+            int bt, rb;
+            lg_tile_coords(tile, p.n_rb, p.n_bt, bt, rb);
             for (int kt = 0; kt < n_tl; ++kt, ++it) {
                 const uint32_t q = it % LG_NSC, a = it & 1u;
                 const uint32_t sb = sc_a + q * LG_SCSLOT;
